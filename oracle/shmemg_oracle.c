@@ -1,0 +1,298 @@
+/*
+ * oracle/shmemg_oracle.c -- CPU ORACLE.  TEST INFRASTRUCTURE, NOT PRODUCT.
+ *
+ * A plain, slow, single-threaded, sequential simulator of N logical PEs with
+ * symmetric heaps, written from the paper (PAPER.md = /root/reference/PAPER.md at
+ * build time; cited as "L<n>") and SURVEY.md section 8(c).  It shares no code,
+ * header, table or helper with the CUDA path and neither imports the other.
+ * Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl
+ * reference legs may load this file.
+ *
+ * Nature of the result: none of these operations is an
+ * approximation.  Each op has a plain definition (memcpy, integer add,
+ * compare-and-swap, sum, concatenate, transpose); the oracle is that definition
+ * written out, executed in BATCH INDEX ORDER, each op running to completion at its
+ * turn.  That is one particular legal schedule under the paper's ordering rules
+ * (L116, L126, L365-L369, L377-L390); outputs that may legitimately differ between
+ * legal schedules (fetched values of fetch-add / compare-swap) are compared through
+ * invariants in tests/, not through this schedule.
+ *
+ * Pins (tests/test_oracle_pins.py, tests/test_litmus_model.py): numpy slice
+ * assignment, np.add.at / np.bincount, np.sum, math.fsum, np.concatenate,
+ * reshape/transpose closed forms, hand-computed 2-PE programs, and a brute-force
+ * schedule enumerator that is independent of this file.
+ * Parity against values printed in the paper: UNPINNED -- the paper prints no
+ * numeric example (L510); only its ordering/visibility rules are pinned.
+ *
+ * State: heap[p] = heap + p*heap_bytes, p = 0..npes-1 ("symmetric heap ... exists
+ * at each PE with the same size and allocation order", L108-L114).  All operands
+ * are symmetric offsets (L202, L355); AMO values are immediates.
+ */
+#include <stdint.h>
+#include <string.h>
+
+/* opcodes of the oracle's own descriptor format */
+enum {
+    ORC_PUT = 1, ORC_GET = 2, ORC_PUT_SIGNAL = 3, ORC_ATOMIC_ADD = 4, ORC_ATOMIC_FETCH_ADD = 5,
+    ORC_ATOMIC_COMPARE_SWAP = 6, ORC_SIGNAL_WAIT_UNTIL = 7, ORC_FENCE = 8, ORC_QUIET = 9,
+    ORC_BARRIER_ALL = 10
+};
+enum { ORC_SIGNAL_SET = 0, ORC_SIGNAL_ADD = 1 };
+enum { ORC_CMP_EQ = 0, ORC_CMP_NE, ORC_CMP_GT, ORC_CMP_GE, ORC_CMP_LT, ORC_CMP_LE };
+enum { ORC_OK = 0, ORC_ERR_RANGE = 1, ORC_ERR_WAIT_UNSATISFIED = 2, ORC_ERR_OPCODE = 3, ORC_ERR_ALIGN = 4 };
+
+typedef struct {
+    int32_t opcode, initiator, target, sig_op, cmp, _pad;
+    uint64_t rem_off;   /* offset in the TARGET's heap   (put dest, get source, AMO word)        */
+    uint64_t loc_off;   /* offset in the INITIATOR's heap (put source, get dest, fetch, wait word) */
+    uint64_t nbytes;
+    uint64_t value;     /* AMO operand / signal value / wait comparand */
+    uint64_t cond;      /* compare-swap condition */
+    uint64_t sig_off;   /* signal word in the TARGET's heap (put_signal) */
+} orc_op_t;
+
+static uint64_t ld64(const uint8_t *p) { uint64_t v; memcpy(&v, p, 8); return v; }
+static void st64(uint8_t *p, uint64_t v) { memcpy(p, &v, 8); }
+
+static int in_range(uint64_t off, uint64_t n, uint64_t heap_bytes) {
+    return off <= heap_bytes && n <= heap_bytes - off;
+}
+
+/*
+ * Execute ops[0..nops) in index order.  Returns ORC_OK or an error code with the
+ * offending op index in *err_index.  SURVEY.md 8(c) table, row by row.
+ */
+int orc_exec_batch(uint8_t *heap, int npes, uint64_t heap_bytes, const orc_op_t *ops, uint64_t nops,
+                   uint64_t *err_index) {
+    for (uint64_t k = 0; k < nops; ++k) {
+        const orc_op_t *o = &ops[k];
+        *err_index = k;
+        if (o->opcode == ORC_FENCE || o->opcode == ORC_QUIET || o->opcode == ORC_BARRIER_ALL) {
+            /* L377: "A fence orders subsequent operations with respect to prior ones ... quiet ensures
+             * completion of outstanding operations initiated by the caller"; L369 barrier is a visibility
+             * point.  In this schedule every earlier op has already completed: nothing to do. */
+            continue;
+        }
+        if (o->initiator < 0 || o->initiator >= npes || o->target < 0 || o->target >= npes) return ORC_ERR_RANGE;
+        uint8_t *ini = heap + (uint64_t)o->initiator * heap_bytes;
+        uint8_t *tgt = heap + (uint64_t)o->target * heap_bytes;
+        switch (o->opcode) {
+        case ORC_PUT:            /* "A put updates remote memory" (L116) */
+        case ORC_PUT_SIGNAL:
+            if (!in_range(o->rem_off, o->nbytes, heap_bytes) || !in_range(o->loc_off, o->nbytes, heap_bytes))
+                return ORC_ERR_RANGE;
+            memmove(tgt + o->rem_off, ini + o->loc_off, o->nbytes);
+            if (o->opcode == ORC_PUT_SIGNAL) {
+                /* put-with-signal (L218, L461): the signal word in the target's heap is updated after
+                 * the payload; SET or ADD (SURVEY.md reading 8). */
+                if (!in_range(o->sig_off, 8, heap_bytes)) return ORC_ERR_RANGE;
+                if (o->sig_off & 7) return ORC_ERR_ALIGN;
+                if (o->sig_op == ORC_SIGNAL_SET) st64(tgt + o->sig_off, o->value);
+                else st64(tgt + o->sig_off, ld64(tgt + o->sig_off) + o->value);
+            }
+            break;
+        case ORC_GET:            /* "a get fetches remote data into local memory" (L116) */
+            if (!in_range(o->rem_off, o->nbytes, heap_bytes) || !in_range(o->loc_off, o->nbytes, heap_bytes))
+                return ORC_ERR_RANGE;
+            memmove(ini + o->loc_off, tgt + o->rem_off, o->nbytes);
+            break;
+        case ORC_ATOMIC_ADD: {   /* "combine remote update with a compute operation (e.g., atomic add)" (L116) */
+            if (!in_range(o->rem_off, 8, heap_bytes)) return ORC_ERR_RANGE;
+            if (o->rem_off & 7) return ORC_ERR_ALIGN;
+            st64(tgt + o->rem_off, ld64(tgt + o->rem_off) + o->value);     /* mod 2^64 */
+            break;
+        }
+        case ORC_ATOMIC_FETCH_ADD: {   /* "may return the value prior to the update" (L116) */
+            if (!in_range(o->rem_off, 8, heap_bytes) || !in_range(o->loc_off, 8, heap_bytes)) return ORC_ERR_RANGE;
+            if ((o->rem_off | o->loc_off) & 7) return ORC_ERR_ALIGN;
+            uint64_t old = ld64(tgt + o->rem_off);
+            st64(tgt + o->rem_off, old + o->value);
+            st64(ini + o->loc_off, old);
+            break;
+        }
+        case ORC_ATOMIC_COMPARE_SWAP: {   /* OpenSHMEM 1.6 compare-swap, inherited via L361/L363 */
+            if (!in_range(o->rem_off, 8, heap_bytes) || !in_range(o->loc_off, 8, heap_bytes)) return ORC_ERR_RANGE;
+            if ((o->rem_off | o->loc_off) & 7) return ORC_ERR_ALIGN;
+            uint64_t old = ld64(tgt + o->rem_off);
+            if (old == o->cond) st64(tgt + o->rem_off, o->value);
+            st64(ini + o->loc_off, old);
+            break;
+        }
+        case ORC_SIGNAL_WAIT_UNTIL: {   /* wait (L116, L392): unsigned 64-bit comparison, reading 9 */
+            if (!in_range(o->loc_off, 8, heap_bytes)) return ORC_ERR_RANGE;
+            if (o->loc_off & 7) return ORC_ERR_ALIGN;
+            uint64_t s = ld64(ini + o->loc_off), v = o->value;
+            int ok;
+            switch (o->cmp) {
+            case ORC_CMP_EQ: ok = (s == v); break;
+            case ORC_CMP_NE: ok = (s != v); break;
+            case ORC_CMP_GT: ok = (s > v); break;
+            case ORC_CMP_GE: ok = (s >= v); break;
+            case ORC_CMP_LT: ok = (s < v); break;
+            case ORC_CMP_LE: ok = (s <= v); break;
+            default: return ORC_ERR_OPCODE;
+            }
+            /* batch index order must be a valid sequential schedule */
+            if (!ok) return ORC_ERR_WAIT_UNSATISFIED;
+            break;
+        }
+        default:
+            return ORC_ERR_OPCODE;
+        }
+    }
+    *err_index = nops;
+    return ORC_OK;
+}
+
+/* ---- homogeneous AMO batches (structure-of-arrays), executed in index order ------------------
+ * Word k of the symmetric int64/uint64 array at sym_off on PE tgt_pe[i] is
+ * heap[tgt_pe[i]][sym_off + 8*idx[i]].  Values are immediates (L355). */
+
+int orc_atomic_add_batch(uint8_t *heap, int npes, uint64_t heap_bytes, uint64_t sym_off,
+                         const int32_t *tgt_pe, const uint64_t *idx, const uint64_t *val, uint64_t n) {
+    for (uint64_t i = 0; i < n; ++i) {
+        uint64_t off = sym_off + 8 * idx[i];
+        if (tgt_pe[i] < 0 || tgt_pe[i] >= npes || !in_range(off, 8, heap_bytes)) return ORC_ERR_RANGE;
+        uint8_t *w = heap + (uint64_t)tgt_pe[i] * heap_bytes + off;
+        st64(w, ld64(w) + val[i]);
+    }
+    return ORC_OK;
+}
+
+int orc_atomic_fetch_add_batch(uint8_t *heap, int npes, uint64_t heap_bytes, uint64_t sym_off,
+                               const int32_t *tgt_pe, const uint64_t *idx, const uint64_t *val,
+                               uint64_t *fetched, uint64_t n) {
+    for (uint64_t i = 0; i < n; ++i) {
+        uint64_t off = sym_off + 8 * idx[i];
+        if (tgt_pe[i] < 0 || tgt_pe[i] >= npes || !in_range(off, 8, heap_bytes)) return ORC_ERR_RANGE;
+        uint8_t *w = heap + (uint64_t)tgt_pe[i] * heap_bytes + off;
+        uint64_t old = ld64(w);
+        st64(w, old + val[i]);
+        fetched[i] = old;
+    }
+    return ORC_OK;
+}
+
+int orc_atomic_compare_swap_batch(uint8_t *heap, int npes, uint64_t heap_bytes, uint64_t sym_off,
+                                  const int32_t *tgt_pe, const uint64_t *idx, const uint64_t *cond,
+                                  const uint64_t *val, uint64_t *fetched, uint64_t n) {
+    for (uint64_t i = 0; i < n; ++i) {
+        uint64_t off = sym_off + 8 * idx[i];
+        if (tgt_pe[i] < 0 || tgt_pe[i] >= npes || !in_range(off, 8, heap_bytes)) return ORC_ERR_RANGE;
+        uint8_t *w = heap + (uint64_t)tgt_pe[i] * heap_bytes + off;
+        uint64_t old = ld64(w);
+        if (old == cond[i]) st64(w, val[i]);
+        fetched[i] = old;
+    }
+    return ORC_OK;
+}
+
+/* ---- collectives on the world team (each is one atomic unit in batch order) ---- */
+
+/* sum_reduce, fp32: r[k] = sum over p (ascending PE order) of heap[p][src+4k], accumulated in fp64,
+ * rounded to nearest fp32 once; every PE's dest receives r (all-reduce; readings 13, 14).  L226. */
+int orc_sum_reduce_f32(uint8_t *heap, int npes, uint64_t heap_bytes, uint64_t dst_off, uint64_t src_off,
+                       uint64_t nreduce, double *r64_out /* optional: the fp64 sums, may be NULL */) {
+    if (!in_range(src_off, 4 * nreduce, heap_bytes) || !in_range(dst_off, 4 * nreduce, heap_bytes)) return ORC_ERR_RANGE;
+    for (uint64_t k = 0; k < nreduce; ++k) {
+        double acc = 0.0;
+        for (int p = 0; p < npes; ++p) {
+            float x; memcpy(&x, heap + (uint64_t)p * heap_bytes + src_off + 4 * k, 4);
+            acc += (double)x;
+        }
+        if (r64_out) r64_out[k] = acc;
+        float r = (float)acc;
+        for (int p = 0; p < npes; ++p) memcpy(heap + (uint64_t)p * heap_bytes + dst_off + 4 * k, &r, 4);
+    }
+    return ORC_OK;
+}
+
+/* sum_reduce, int64: wraparound two's-complement sum (bit-exact). */
+int orc_sum_reduce_i64(uint8_t *heap, int npes, uint64_t heap_bytes, uint64_t dst_off, uint64_t src_off,
+                       uint64_t nreduce) {
+    if (!in_range(src_off, 8 * nreduce, heap_bytes) || !in_range(dst_off, 8 * nreduce, heap_bytes)) return ORC_ERR_RANGE;
+    for (uint64_t k = 0; k < nreduce; ++k) {
+        uint64_t acc = 0;
+        for (int p = 0; p < npes; ++p) acc += ld64(heap + (uint64_t)p * heap_bytes + src_off + 8 * k);
+        for (int p = 0; p < npes; ++p) st64(heap + (uint64_t)p * heap_bytes + dst_off + 8 * k, acc);
+    }
+    return ORC_OK;
+}
+
+/* fcollect: for all j, p: heap[j][dst + p*n : +n] = heap[p][src : +n]  (concatenation in PE order) */
+int orc_fcollect(uint8_t *heap, int npes, uint64_t heap_bytes, uint64_t dst_off, uint64_t src_off, uint64_t n) {
+    if (!in_range(src_off, n, heap_bytes) || !in_range(dst_off, n * (uint64_t)npes, heap_bytes)) return ORC_ERR_RANGE;
+    for (int j = 0; j < npes; ++j)
+        for (int p = 0; p < npes; ++p)
+            memcpy(heap + (uint64_t)j * heap_bytes + dst_off + (uint64_t)p * n,
+                   heap + (uint64_t)p * heap_bytes + src_off, n);
+    return ORC_OK;
+}
+
+/* alltoall: for all i, j: heap[j][dst + i*n : +n] = heap[i][src + j*n : +n]; src and dst ranges must
+ * not overlap (reading 12), so reading the live heap equals reading a snapshot.  L218, L68. */
+int orc_alltoall(uint8_t *heap, int npes, uint64_t heap_bytes, uint64_t dst_off, uint64_t src_off, uint64_t n) {
+    uint64_t tot = n * (uint64_t)npes;
+    if (!in_range(src_off, tot, heap_bytes) || !in_range(dst_off, tot, heap_bytes)) return ORC_ERR_RANGE;
+    if (!(src_off + tot <= dst_off || dst_off + tot <= src_off)) return ORC_ERR_RANGE;
+    for (int i = 0; i < npes; ++i)
+        for (int j = 0; j < npes; ++j)
+            memcpy(heap + (uint64_t)j * heap_bytes + dst_off + (uint64_t)i * n,
+                   heap + (uint64_t)i * heap_bytes + src_off + (uint64_t)j * n, n);
+    return ORC_OK;
+}
+
+/* ---- application-side compute of the halo workload (config C2; SURVEY.md readings 21-23) ------
+ * Not part of the specification's operations: the stencil application's own kernels, restated on
+ * the CPU so the oracle can run the whole workload.  Both sides implement the same counter-based
+ * generator for the perturbation (allowed: "each side implements the same counter-based generator"). */
+
+static uint64_t fin64(uint64_t x) {
+    x ^= x >> 30; x *= 0xBF58476D1CE4E5B9ull;
+    x ^= x >> 27; x *= 0x94D049BB133111EBull;
+    x ^= x >> 31;
+    return x;
+}
+static uint64_t mix64(uint64_t seed, uint64_t stream, uint64_t i) {
+    uint64_t x = fin64(seed * 0xD1342543DE82EF95ull + stream * 0x9E3779B97F4A7C15ull + 0x2545F4914F6CDD1Dull);
+    return fin64(x ^ (i * 0x9E3779B97F4A7C15ull + 0x632BE59BD9B4E019ull));
+}
+
+/* delta(seed, round, gidx) = (mix64 mod 2^16) * 2^-30  (reading 22) */
+double orc_halo_delta(uint64_t seed, uint64_t round, uint64_t gidx) {
+    return (double)(mix64(seed, round, gidx) & 0xFFFFull) * 0x1.0p-30;
+}
+
+/* Perturb PE (px,py,pz)'s B^3 block U (x-major: U[(x*B+y)*B+z]) for one round:
+ * U[c] += delta(seed, round, global index of c in the (2B)^3 grid). */
+void orc_halo_perturb(double *U, uint64_t B, int px, int py, int pz, uint64_t seed, uint64_t round) {
+    uint64_t G = 2 * B;
+    for (uint64_t x = 0; x < B; ++x)
+        for (uint64_t y = 0; y < B; ++y)
+            for (uint64_t z = 0; z < B; ++z) {
+                uint64_t g = ((px * B + x) * G + (py * B + y)) * G + (pz * B + z);
+                U[(x * B + y) * B + z] += orc_halo_delta(seed, round, g);
+            }
+}
+
+/* Pack face f = 2*axis + dir (dir 0: index 0, dir 1: index B-1 along axis) of U into send[B*B];
+ * the two remaining axes keep their relative order (lower axis major). */
+void orc_halo_pack(const double *U, uint64_t B, int f, double *send) {
+    int axis = f >> 1, dir = f & 1;
+    uint64_t fix = dir ? B - 1 : 0;
+    for (uint64_t a = 0; a < B; ++a)
+        for (uint64_t b = 0; b < B; ++b) {
+            uint64_t x, y, z;
+            if (axis == 0)      { x = fix; y = a; z = b; }
+            else if (axis == 1) { x = a; y = fix; z = b; }
+            else                { x = a; y = b; z = fix; }
+            send[a * B + b] = U[(x * B + y) * B + z];
+        }
+}
+
+/* order-independent checksum of n 64-bit words: sum bits(x_k)*(2k+1) mod 2^64 (reading 23) */
+uint64_t orc_checksum64(const uint8_t *p, uint64_t n) {
+    uint64_t s = 0;
+    for (uint64_t k = 0; k < n; ++k) s += ld64(p + 8 * k) * (2 * k + 1);
+    return s;
+}
