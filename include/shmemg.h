@@ -1,0 +1,260 @@
+/*
+ * shmemg.h -- C ABI of the B200-native GPU-aware OpenSHMEM hot path.
+ *
+ * What this library is: the data-parallel hot path of the "OpenSHMEM Auxiliary Specification for
+ * GPU-Aware Communication" (arxiv/paper_2607_08006; cited below as PAPER L<line> of PAPER.md):
+ * batched one-sided operations on a GPU-scoped symmetric heap, executed for N logical PEs whose heaps
+ * are co-resident in one B200's HBM.  Every step of the path runs in hand-written sm_100a kernels;
+ * there is no CPU fallback and no dependence on any other library than the CUDA runtime.
+ *
+ * Conventions
+ *   - All N PEs live in one process, so every routine OpenSHMEM scopes to "the calling PE" takes an
+ *     explicit initiator `pe`.  Argument order follows OpenSHMEM: (dest, source, nbytes, pe).
+ *   - GPU-resident operands are SYMMETRIC OFFSETS (uint64_t byte offsets into every PE's heap window),
+ *     never raw pointers: "GPU-resident operands MUST be allocated from a symmetric space" (PAPER L287,
+ *     L351: "should not require device code to perform dynamic pointer classification").  The address of
+ *     offset `off` on PE `pe` is  slab + pe*heap_stride + off  ("predictable,
+ *     computable address offsets").
+ *   - `stream` arguments are raw `cudaStream_t` values passed as `void *` (NULL = legacy default stream).
+ *   - Pointers are marked HOST or DEVICE.  The library never allocates or frees device memory: the
+ *     caller owns the slab and every DEVICE array it passes, and must keep them valid until the stream
+ *     has passed the call.  The library owns only host bookkeeping plus a control region it carves from
+ *     the tail of the slab.
+ *   - Every routine returns SHMEMG_OK (0) or a negative SHMEMG_ERR_* for host-checkable misuse; nothing
+ *     is enqueued on error.  Data races, overlapping unordered writes and unsatisfiable waits are
+ *     undefined behaviour; an unsatisfiable wait hangs the stream (prohibited pattern,
+ *     PAPER L404).
+ *   - Execution path: every `_on_stream` routine is a HOST-ISSUED,
+ *     STREAM-TRIGGERED operation "whose execution is ordered relative to a GPU stream"; the library
+ *     "may use internal GPU kernels to accelerate" it.  Effects are visible to later work on the same
+ *     stream; host visibility needs cudaStreamSynchronize, which shmemg_quiet does.
+ */
+#ifndef SHMEMG_H
+#define SHMEMG_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define SHMEMG_API __attribute__((visibility("default")))
+
+typedef struct shmemg_world shmemg_world_t;   /* opaque, HOST */
+typedef struct shmemg_batch shmemg_batch_t;   /* opaque, HOST: a planned op batch */
+
+/* ---- return codes -------------------------------------------------------------------------- */
+enum {
+    SHMEMG_OK = 0,
+    SHMEMG_ERR_ARG = -1,      /* NULL handle/pointer, bad enum, npes < 1                      */
+    SHMEMG_ERR_PE = -2,       /* pe outside [0, npes)                                         */
+    SHMEMG_ERR_RANGE = -3,    /* offset + size outside the heap window                        */
+    SHMEMG_ERR_ALIGN = -4,    /* AMO / signal word not 8-byte aligned, typed buffer misaligned */
+    SHMEMG_ERR_NOMEM = -5,    /* symmetric heap exhausted / slab or plan buffer too small     */
+    SHMEMG_ERR_CUDA = -6,     /* a CUDA runtime call failed (see shmemg_last_cuda_error)       */
+    SHMEMG_ERR_OVERLAP = -7,  /* collective source/dest ranges partially overlap              */
+    SHMEMG_ERR_NODEVICE = -8  /* no sm_100 device / wrong architecture                        */
+};
+
+/* ---- teams and contexts: constants only in this build ------------------ */
+enum {
+    SHMEM_TEAM_WORLD = 0,
+    SHMEM_DEVICE_TEAM_WORLD = 1,    /* same membership as SHMEM_TEAM_WORLD            */
+    SHMEM_DEVICE_TEAM_SHARED = 2    /* all PEs share one GPU, so shared == world here (L357)       */
+};
+#define SHMEM_DEVICE_CTX_DEFAULT 0   /* the one default device context = one ordering domain per PE */
+
+/* ---- capability bits (shape left open by the paper) ------ */
+#define SHMEMG_CAP_GPU_HEAP_PRESENT           (1ull << 0)   /* a GPU symmetric heap exists (L299)        */
+#define SHMEMG_CAP_DEFAULT_HEAP_IS_GPU        (1ull << 1)   /* GPU-first: default heap type (L451)        */
+#define SHMEMG_CAP_HOST_INITIATED_GPU_BUFFERS (1ull << 2)   /* Tier-0 baseline (L465)                    */
+#define SHMEMG_CAP_STREAM_TRIGGERED           (1ull << 3)   /* _on_stream variants (L396, L412)          */
+#define SHMEMG_CAP_DEVICE_INITIATED           (1ull << 4)   /* __device__ entry points (L412, L465)      */
+#define SHMEMG_CAP_DEVICE_COLLECTIVES         (1ull << 5)   /* 0 in this build                           */
+#define SHMEMG_CAP_EXPLICIT_DEVICE_CTX        (1ull << 6)   /* 0 in this build                           */
+#define SHMEMG_CAP_PTR_DEVICE_ACCESSIBLE      (1ull << 7)   /* shmemg_ptr is a device pointer (L353)     */
+#define SHMEMG_CAP_PTR_HOST_ACCESSIBLE        (1ull << 8)   /* 0: not dereferenceable on the host (L456) */
+#define SHMEMG_CAP_PROGRESS_GPU_ONLY          (1ull << 9)   /* no host proxy needed (L394, L431)         */
+#define SHMEMG_CAP_PATH_DIRECT                (1ull << 10)  /* direct load/store path (L431)             */
+#define SHMEMG_CAP_ATOMICS_64                 (1ull << 11)  /* add / fetch-add / compare-swap on 64 bit  */
+#define SHMEMG_CAP_STREAM_COLLECTIVES         (1ull << 12)  /* barrier/alltoall/fcollect/reduce on stream */
+
+/* ---- lifecycle ------------------------------------------------------------------------------------ */
+
+/* Bytes the caller must provide for the slab: npes heap windows (stride = heap_bytes_per_pe rounded up
+ * to 512 B) plus the library's control region.  heap_bytes_per_pe == 0 means "take it from the
+ * environment variable SHMEMG_SYMMETRIC_SIZE" (bytes, optional K/M/G suffix).
+ * Returns 0 on invalid arguments. */
+SHMEMG_API size_t shmemg_slab_bytes_required(int npes, size_t heap_bytes_per_pe);
+
+/* Create a world of `npes` logical PEs over `device_slab` (DEVICE, 512-byte aligned, owned by the
+ * caller, >= shmemg_slab_bytes_required bytes).  GPU-first: the GPU symmetric heap exists right after
+ * init.  Zeroes the control region on the legacy default stream and synchronises.
+ * *out receives the handle (HOST). */
+SHMEMG_API int shmemg_init(int npes, size_t heap_bytes_per_pe, void *device_slab, size_t slab_bytes,
+                           shmemg_world_t **out);
+SHMEMG_API int shmemg_finalize(shmemg_world_t *w);
+SHMEMG_API int shmemg_n_pes(const shmemg_world_t *w);
+SHMEMG_API size_t shmemg_heap_bytes(const shmemg_world_t *w);    /* usable bytes per PE           */
+SHMEMG_API size_t shmemg_heap_stride(const shmemg_world_t *w);   /* distance between PE windows   */
+SHMEMG_API const char *shmemg_last_cuda_error(const shmemg_world_t *w);
+
+/* Capability discovery ("shmem_query_capabilities", section 6.5).  `team` is one of the
+ * SHMEM_*TEAM* constants; *caps (HOST) receives the SHMEMG_CAP_* mask active for that team. */
+SHMEMG_API int shmem_query_capabilities(const shmemg_world_t *w, int team, uint64_t *caps);
+
+/* ---- symmetric allocation in the GPU space ("shmemg_malloc") ---------------------------
+ * One call allocates on ALL PEs (one process owns all PEs, so the call is collective by construction)
+ * and yields ONE offset valid on every PE; allocation order and size are symmetric (L303).  Alignment
+ * >= 256 B.  Contents are unspecified after malloc/align, zero after calloc (enqueued on `stream`). */
+SHMEMG_API int shmemg_malloc(shmemg_world_t *w, size_t bytes, uint64_t *sym_off);
+SHMEMG_API int shmemg_calloc(shmemg_world_t *w, size_t count, size_t size, uint64_t *sym_off, void *stream);
+SHMEMG_API int shmemg_align(shmemg_world_t *w, size_t alignment, size_t bytes, uint64_t *sym_off);
+SHMEMG_API int shmemg_free(shmemg_world_t *w, uint64_t sym_off);
+/* shmem_ptr analog: DEVICE pointer to offset `sym_off` on PE `pe`, or NULL if the
+ * arguments are invalid.  Valid in the device access domain only (SHMEMG_CAP_PTR_DEVICE_ACCESSIBLE). */
+SHMEMG_API void *shmemg_ptr(const shmemg_world_t *w, uint64_t sym_off, int pe);
+
+/* Documented extension ("registered private ... source operands"): move bytes between a HOST
+ * buffer and PE `pe`'s window with cudaMemcpyAsync on `stream`.  Used by the end-to-end benchmark. */
+SHMEMG_API int shmemg_heap_write_on_stream(shmemg_world_t *w, int pe, uint64_t dst_off, const void *src_host,
+                                           size_t nbytes, void *stream);
+SHMEMG_API int shmemg_heap_read_on_stream(shmemg_world_t *w, int pe, void *dst_host, uint64_t src_off,
+                                          size_t nbytes, void *stream);
+
+/* ---- op batches: host-initiated enqueue on a stream ------------------------ */
+
+enum {
+    SHMEMG_OP_PUT = 1,                  /* heap[target][rem_off..] = heap[initiator][loc_off..]   (L116) */
+    SHMEMG_OP_GET = 2,                  /* heap[initiator][loc_off..] = heap[target][rem_off..]   (L116) */
+    SHMEMG_OP_PUT_SIGNAL = 3,           /* PUT, then signal word sig_off on target SET/ADD `value` (L218, L461) */
+    SHMEMG_OP_ATOMIC_ADD = 4,           /* u64 heap[target][rem_off] += value                      (L116) */
+    SHMEMG_OP_ATOMIC_FETCH_ADD = 5,     /* as ADD; old value -> u64 heap[initiator][loc_off]       (L116) */
+    SHMEMG_OP_ATOMIC_COMPARE_SWAP = 6,  /* if (*p == cond) *p = value; old -> heap[initiator][loc_off] (L361) */
+    SHMEMG_OP_SIGNAL_WAIT_UNTIL = 7,    /* initiator blocks until cmp(u64 heap[initiator][loc_off], value) (L116, L392) */
+    SHMEMG_OP_FENCE = 8,                /* orders initiator's later ops after its earlier ones      (L377) */
+    SHMEMG_OP_QUIET = 9,                /* initiator's earlier ops complete and are visible         (L377-L390) */
+    SHMEMG_OP_BARRIER_ALL = 10          /* all PEs: every earlier op of every PE complete           (L116, L369) */
+};
+enum { SHMEMG_SIGNAL_SET = 0, SHMEMG_SIGNAL_ADD = 1 };
+enum { SHMEMG_CMP_EQ = 0, SHMEMG_CMP_NE = 1, SHMEMG_CMP_GT = 2, SHMEMG_CMP_GE = 3, SHMEMG_CMP_LT = 4, SHMEMG_CMP_LE = 5 };
+
+/* One op descriptor, 64 bytes, HOST memory.  "Remote" = the target PE's window, "local" = the
+ * initiator's window.  Unused fields are ignored. */
+typedef struct shmemg_op {
+    uint8_t opcode;        /* SHMEMG_OP_*                                                     */
+    uint8_t sig_op;        /* SHMEMG_SIGNAL_* (PUT_SIGNAL)                                    */
+    uint8_t cmp;           /* SHMEMG_CMP_*    (SIGNAL_WAIT_UNTIL), unsigned 64-bit comparison */
+    uint8_t reserved0;
+    int32_t initiator_pe;
+    int32_t target_pe;
+    uint32_t reserved1;
+    uint64_t rem_off;      /* put dest / get source / AMO word, in the TARGET's window       */
+    uint64_t loc_off;      /* put source / get dest / fetch slot / wait word, in the INITIATOR's window */
+    uint64_t nbytes;       /* put / get / put_signal payload size; any size and alignment >= 0 */
+    uint64_t value;        /* AMO operand, signal value, or wait comparand                    */
+    uint64_t cond;         /* compare-swap condition                                          */
+    uint64_t sig_off;      /* signal word in the TARGET's window (8-byte aligned)             */
+} shmemg_op_t;
+
+/*
+ * Batch semantics:
+ *   - ops[0..nops) is an ordered program; REQUIREMENT: index order is a valid sequential schedule (a
+ *     SIGNAL_WAIT_UNTIL is satisfied by ops that precede it in the array).
+ *   - ops have non-blocking semantics: the executor may run ops of one PE in any order and
+ *     concurrently unless a FENCE / QUIET / SIGNAL_WAIT_UNTIL of that PE or a BARRIER_ALL lies between
+ *     them.  FENCE and QUIET are both implemented as "all earlier ops of this PE, to all targets, gets
+ *     and atomics included, are complete and visible before any later op of this PE starts" -- the
+ *     strong reading of L377, always conformant.  A wait also orders the PE's later ops after it.
+ *   - PUT_SIGNAL: the signal update is atomic w.r.t. other signal updates and waits, and becomes visible
+ *     only after the whole payload (release/acquire at GPU scope).
+ *   - atomicity does not imply ordering.
+ *   - batch end = kernel end = quiet for every PE + barrier (stronger than required; L377).
+ */
+
+/* DEVICE bytes needed for the plan of this op list (0 on invalid arguments). */
+SHMEMG_API size_t shmemg_batch_plan_bytes(const shmemg_world_t *w, const shmemg_op_t *ops_host, size_t nops);
+
+/* Validate `ops_host` (HOST, nops entries), resolve PE->address translation, cut the ops into tiles and
+ * upload the plan into `plan_dev` (DEVICE, 256-byte aligned, >= shmemg_batch_plan_bytes, caller-owned,
+ * must outlive the batch) on `stream`, then synchronise that stream.  On a bad descriptor returns the
+ * error code and stores its index in *bad_index (HOST, may be NULL).  A batch may be enqueued any
+ * number of times, but never concurrently with itself. */
+SHMEMG_API int shmemg_batch_create(shmemg_world_t *w, const shmemg_op_t *ops_host, size_t nops, void *plan_dev,
+                                   size_t plan_bytes, void *stream, shmemg_batch_t **out, size_t *bad_index);
+SHMEMG_API int shmemg_batch_destroy(shmemg_batch_t *b);
+/* Number of kernel launches one enqueue of this batch performs (for launch accounting). */
+SHMEMG_API int shmemg_batch_launches(const shmemg_batch_t *b);
+
+/* Launch the batch executor on `stream` (one persistent-grid kernel; tiles are claimed in batch order). */
+SHMEMG_API int shmemg_batch_enqueue_on_stream(shmemg_world_t *w, shmemg_batch_t *b, void *stream);
+
+/* ---- single operations on a stream (put/get, signal put/wait, barrier on stream) ------ */
+SHMEMG_API int shmemg_put_on_stream(shmemg_world_t *w, uint64_t dest_off, uint64_t source_off, size_t nbytes,
+                                    int pe /*initiator*/, int target_pe, void *stream);
+SHMEMG_API int shmemg_get_on_stream(shmemg_world_t *w, uint64_t dest_off, uint64_t source_off, size_t nbytes,
+                                    int pe /*initiator*/, int target_pe, void *stream);
+SHMEMG_API int shmemg_put_signal_on_stream(shmemg_world_t *w, uint64_t dest_off, uint64_t source_off, size_t nbytes,
+                                           uint64_t sig_off, uint64_t signal, int sig_op, int pe, int target_pe,
+                                           void *stream);
+/* Blocks the STREAM (not the host) until cmp(u64 heap[pe][sig_off], value).  Only ops enqueued EARLIER on
+ * the same stream, or device-initiated ops, can satisfy it (prohibited pattern otherwise). */
+SHMEMG_API int shmemg_signal_wait_until_on_stream(shmemg_world_t *w, uint64_t sig_off, int cmp, uint64_t value,
+                                                  int pe, void *stream);
+/* Stream order already completes every earlier `_on_stream` op before a later one starts, so these
+ * validate their arguments and enqueue nothing (ordering within a stream). */
+SHMEMG_API int shmemg_fence_on_stream(shmemg_world_t *w, int pe, void *stream);
+SHMEMG_API int shmemg_quiet_on_stream(shmemg_world_t *w, int pe, void *stream);
+/* Host-blocking quiet: stream-ordered quiet + cudaStreamSynchronize. */
+SHMEMG_API int shmemg_quiet(shmemg_world_t *w, int pe, void *stream);
+
+/* ---- homogeneous AMO batches, structure-of-arrays (PAPER L116, L224 case study 2) ---------------------
+ * Op i targets 64-bit word  heap[tgt_pe[i]][sym_off + 8*elem_idx[i]].  tgt_pe, elem_idx, val, cond and
+ * fetched_out are DEVICE arrays of n entries; elem_idx has `idx_bytes` (4 or 8) bytes per entry; `val` /
+ * `cond` may be NULL, in which case `val_scalar` / `cond_scalar` is used for every op (immediates, L355).
+ * There is NO ordering between the ops of one call (reading 7); fetched values are valid when the stream
+ * has passed the call.  flags: SHMEMG_AMO_* below.  64-bit integer types only (wraparound add). */
+#define SHMEMG_AMO_WARP_AGGREGATE 1u   /* combine same-address ops of a warp into one L2 atomic */
+SHMEMG_API int shmemg_atomic_add_batch_on_stream(shmemg_world_t *w, uint64_t sym_off, const int32_t *tgt_pe,
+                                                 const void *elem_idx, int idx_bytes, const uint64_t *val,
+                                                 uint64_t val_scalar, size_t n, uint32_t flags, void *stream);
+SHMEMG_API int shmemg_atomic_fetch_add_batch_on_stream(shmemg_world_t *w, uint64_t sym_off, const int32_t *tgt_pe,
+                                                       const void *elem_idx, int idx_bytes, const uint64_t *val,
+                                                       uint64_t val_scalar, uint64_t *fetched_out, size_t n,
+                                                       uint32_t flags, void *stream);
+SHMEMG_API int shmemg_atomic_compare_swap_batch_on_stream(shmemg_world_t *w, uint64_t sym_off, const int32_t *tgt_pe,
+                                                          const void *elem_idx, int idx_bytes, const uint64_t *cond,
+                                                          uint64_t cond_scalar, const uint64_t *val,
+                                                          uint64_t val_scalar, uint64_t *fetched_out, size_t n,
+                                                          uint32_t flags, void *stream);
+
+/* ---- collectives on SHMEM_TEAM_WORLD, one kernel each --------------------------
+ * Each collective is one atomic unit in stream order (kernel boundaries order it against its neighbours). */
+enum { SHMEMG_F32 = 0, SHMEMG_I64 = 1 };
+/* every PE's dest[k] = sum over all PEs (ascending PE order) of source[k], k < nreduce.  F32 accumulates
+ * in fp64 and rounds once; I64 wraps.  dest == source (exact aliasing) is allowed; partial overlap is not. */
+SHMEMG_API int shmemg_sum_reduce_on_stream(shmemg_world_t *w, int dtype, uint64_t dest_off, uint64_t source_off,
+                                           size_t nreduce, void *stream);
+/* every PE's dest[p*nbytes .. +nbytes) = PE p's source[0 .. nbytes)  (concatenation in PE order). */
+SHMEMG_API int shmemg_fcollect_on_stream(shmemg_world_t *w, uint64_t dest_off, uint64_t source_off, size_t nbytes,
+                                         void *stream);
+/* PE j's dest[i*nbytes .. +nbytes) = PE i's source[j*nbytes .. +nbytes)  (block index = peer PE). */
+SHMEMG_API int shmemg_alltoall_on_stream(shmemg_world_t *w, uint64_t dest_off, uint64_t source_off, size_t nbytes,
+                                         void *stream);
+/* Stream-level barrier: everything enqueued earlier on `stream` by any PE is complete and visible to
+ * everything enqueued later; bumps the world's barrier epoch (one tiny kernel). */
+SHMEMG_API int shmemg_barrier_all_on_stream(shmemg_world_t *w, void *stream);
+/* `count` back-to-back barriers among npes co-resident PE agents (one CTA per PE, cooperative launch) in
+ * ONE kernel: the in-kernel barrier whose per-iteration latency config C5 reports.  If `stamp_off` is not
+ * UINT64_MAX, the agents also run the round-stamp check of SURVEY.md 8(c): in round r agent p writes r into
+ * u64 heap[(p+1)%npes][stamp_off + 8*(r&1)], barrier, reads its own slot and counts a violation in
+ * u64 heap[p][stamp_off + 16] if it is not r.  The object at stamp_off is 24 bytes, zero-initialised. */
+SHMEMG_API int shmemg_barrier_all_repeat_on_stream(shmemg_world_t *w, uint32_t count, uint64_t stamp_off,
+                                                   void *stream);
+SHMEMG_API uint64_t shmemg_barrier_epoch(shmemg_world_t *w, void *stream);   /* synchronises `stream` */
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* SHMEMG_H */

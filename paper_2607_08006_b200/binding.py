@@ -1,0 +1,367 @@
+"""ctypes binding of include/shmemg.h and include/shmemg_app.h (same names, marshalling only)."""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import numpy as np
+import torch
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libshmemg.so")
+
+
+class ShmemgError(RuntimeError):
+    def __init__(self, code: int, what: str, detail: str = ""):
+        self.code = code
+        super().__init__("%s: %s%s" % (what, ERR.name(code), (" (%s)" % detail) if detail else ""))
+
+
+class ERR:
+    OK, ARG, PE, RANGE, ALIGN, NOMEM, CUDA, OVERLAP, NODEVICE = 0, -1, -2, -3, -4, -5, -6, -7, -8
+
+    @staticmethod
+    def name(code):
+        for k, v in vars(ERR).items():
+            if k.isupper() and v == code:
+                return "SHMEMG_ERR_" + k if code else "SHMEMG_OK"
+        return str(code)
+
+
+class OP:
+    PUT, GET, PUT_SIGNAL, ATOMIC_ADD, ATOMIC_FETCH_ADD, ATOMIC_COMPARE_SWAP, SIGNAL_WAIT_UNTIL, FENCE, QUIET, \
+        BARRIER_ALL = range(1, 11)
+
+
+class SIGNAL:
+    SET, ADD = 0, 1
+
+
+class CMP:
+    EQ, NE, GT, GE, LT, LE = range(6)
+
+
+class TEAM:
+    WORLD, DEVICE_WORLD, DEVICE_SHARED = 0, 1, 2
+
+
+class CAP:
+    GPU_HEAP_PRESENT = 1 << 0
+    DEFAULT_HEAP_IS_GPU = 1 << 1
+    HOST_INITIATED_GPU_BUFFERS = 1 << 2
+    STREAM_TRIGGERED = 1 << 3
+    DEVICE_INITIATED = 1 << 4
+    DEVICE_COLLECTIVES = 1 << 5
+    EXPLICIT_DEVICE_CTX = 1 << 6
+    PTR_DEVICE_ACCESSIBLE = 1 << 7
+    PTR_HOST_ACCESSIBLE = 1 << 8
+    PROGRESS_GPU_ONLY = 1 << 9
+    PATH_DIRECT = 1 << 10
+    ATOMICS_64 = 1 << 11
+    STREAM_COLLECTIVES = 1 << 12
+
+
+F32, I64 = 0, 1
+AMO_WARP_AGGREGATE = 1
+NO_STAMP = (1 << 64) - 1
+
+# shmemg_op_t, 64 bytes
+OP_DTYPE = np.dtype([
+    ("opcode", "u1"), ("sig_op", "u1"), ("cmp", "u1"), ("reserved0", "u1"),
+    ("initiator_pe", "i4"), ("target_pe", "i4"), ("reserved1", "u4"),
+    ("rem_off", "u8"), ("loc_off", "u8"), ("nbytes", "u8"), ("value", "u8"), ("cond", "u8"), ("sig_off", "u8"),
+])
+assert OP_DTYPE.itemsize == 64
+
+# every symbol include/shmemg.h and include/shmemg_app.h declare: name -> (restype, argtypes)
+_vp, _u64, _sz, _i, _u32 = C.c_void_p, C.c_uint64, C.c_size_t, C.c_int, C.c_uint32
+SYMBOLS = {
+    "shmemg_slab_bytes_required": (_sz, [_i, _sz]),
+    "shmemg_init": (_i, [_i, _sz, _vp, _sz, C.POINTER(_vp)]),
+    "shmemg_finalize": (_i, [_vp]),
+    "shmemg_n_pes": (_i, [_vp]),
+    "shmemg_heap_bytes": (_sz, [_vp]),
+    "shmemg_heap_stride": (_sz, [_vp]),
+    "shmemg_last_cuda_error": (C.c_char_p, [_vp]),
+    "shmem_query_capabilities": (_i, [_vp, _i, C.POINTER(_u64)]),
+    "shmemg_malloc": (_i, [_vp, _sz, C.POINTER(_u64)]),
+    "shmemg_calloc": (_i, [_vp, _sz, _sz, C.POINTER(_u64), _vp]),
+    "shmemg_align": (_i, [_vp, _sz, _sz, C.POINTER(_u64)]),
+    "shmemg_free": (_i, [_vp, _u64]),
+    "shmemg_ptr": (_vp, [_vp, _u64, _i]),
+    "shmemg_heap_write_on_stream": (_i, [_vp, _i, _u64, _vp, _sz, _vp]),
+    "shmemg_heap_read_on_stream": (_i, [_vp, _i, _vp, _u64, _sz, _vp]),
+    "shmemg_batch_plan_bytes": (_sz, [_vp, _vp, _sz]),
+    "shmemg_batch_create": (_i, [_vp, _vp, _sz, _vp, _sz, _vp, C.POINTER(_vp), C.POINTER(_sz)]),
+    "shmemg_batch_destroy": (_i, [_vp]),
+    "shmemg_batch_launches": (_i, [_vp]),
+    "shmemg_batch_enqueue_on_stream": (_i, [_vp, _vp, _vp]),
+    "shmemg_put_on_stream": (_i, [_vp, _u64, _u64, _sz, _i, _i, _vp]),
+    "shmemg_get_on_stream": (_i, [_vp, _u64, _u64, _sz, _i, _i, _vp]),
+    "shmemg_put_signal_on_stream": (_i, [_vp, _u64, _u64, _sz, _u64, _u64, _i, _i, _i, _vp]),
+    "shmemg_signal_wait_until_on_stream": (_i, [_vp, _u64, _i, _u64, _i, _vp]),
+    "shmemg_fence_on_stream": (_i, [_vp, _i, _vp]),
+    "shmemg_quiet_on_stream": (_i, [_vp, _i, _vp]),
+    "shmemg_quiet": (_i, [_vp, _i, _vp]),
+    "shmemg_atomic_add_batch_on_stream": (_i, [_vp, _u64, _vp, _vp, _i, _vp, _u64, _sz, _u32, _vp]),
+    "shmemg_atomic_fetch_add_batch_on_stream": (_i, [_vp, _u64, _vp, _vp, _i, _vp, _u64, _vp, _sz, _u32, _vp]),
+    "shmemg_atomic_compare_swap_batch_on_stream": (_i, [_vp, _u64, _vp, _vp, _i, _vp, _u64, _vp, _u64, _vp, _sz, _u32, _vp]),
+    "shmemg_sum_reduce_on_stream": (_i, [_vp, _i, _u64, _u64, _sz, _vp]),
+    "shmemg_fcollect_on_stream": (_i, [_vp, _u64, _u64, _sz, _vp]),
+    "shmemg_alltoall_on_stream": (_i, [_vp, _u64, _u64, _sz, _vp]),
+    "shmemg_barrier_all_on_stream": (_i, [_vp, _vp]),
+    "shmemg_barrier_all_repeat_on_stream": (_i, [_vp, _u32, _u64, _vp]),
+    "shmemg_barrier_epoch": (_u64, [_vp, _vp]),
+    "shmemg_app_halo_perturb_on_stream": (_i, [_vp, _u64, _u32, _u64, _u64, _vp]),
+    "shmemg_app_halo_pack_on_stream": (_i, [_vp, _u64, _u64, _u32, _vp]),
+    "shmemg_app_checksum64_on_stream": (_i, [_vp, _vp, _u64, _u64, _u32, _vp]),
+}
+
+_lib = None
+
+
+def lib():
+    """Load libshmemg.so.  Fails loudly: there is no fallback path."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise ImportError("libshmemg.so is not built (run `python -c 'import __graft_entry__ as g; g.build()'`); "
+                              "the CUDA extension is required, there is no CPU fallback")
+        L = C.CDLL(LIB_PATH)
+        for name, (res, args) in SYMBOLS.items():
+            fn = getattr(L, name)          # AttributeError if the library does not export a declared symbol
+            fn.restype, fn.argtypes = res, args
+        _lib = L
+    return _lib
+
+
+def _stream(stream=None) -> int:
+    s = torch.cuda.current_stream() if stream is None else stream
+    return s.cuda_stream
+
+
+def _dptr(t) -> int:
+    if t is None:
+        return 0
+    assert t.is_cuda and t.is_contiguous()
+    return t.data_ptr()
+
+
+class Batch:
+    """A planned op batch (shmemg_batch_t) plus the device plan buffer it lives in."""
+
+    def __init__(self, world: "World", ops: np.ndarray, stream=None):
+        assert ops.dtype == OP_DTYPE
+        ops = np.ascontiguousarray(ops)
+        self.world, self.nops = world, len(ops)
+        L = lib()
+        nbytes = L.shmemg_batch_plan_bytes(world.h, ops.ctypes.data, len(ops))
+        if nbytes == 0:
+            raise ShmemgError(ERR.ARG, "shmemg_batch_plan_bytes")
+        self.plan = torch.empty(nbytes, dtype=torch.uint8, device=world.device)
+        h, bad = C.c_void_p(), C.c_size_t(0)
+        rc = L.shmemg_batch_create(world.h, ops.ctypes.data, len(ops), self.plan.data_ptr(), nbytes, _stream(stream),
+                                   C.byref(h), C.byref(bad))
+        if rc:
+            raise ShmemgError(rc, "shmemg_batch_create", "op %d" % bad.value)
+        self.h = h
+        self.launches = L.shmemg_batch_launches(h)
+
+    def enqueue(self, stream=None):
+        self.world._chk(lib().shmemg_batch_enqueue_on_stream(self.world.h, self.h, _stream(stream)),
+                        "shmemg_batch_enqueue_on_stream")
+
+    def __del__(self):
+        if getattr(self, "h", None) and _lib is not None:
+            _lib.shmemg_batch_destroy(self.h)
+            self.h = None
+
+
+class World:
+    """npes logical PEs over one device slab (a torch uint8 tensor owned by this object)."""
+
+    def __init__(self, npes: int, heap_bytes: int, device="cuda:0"):
+        L = lib()
+        if not torch.cuda.is_available():
+            raise RuntimeError("no CUDA device: the shmemg hot path has no CPU fallback")
+        self.device = torch.device(device)
+        need = L.shmemg_slab_bytes_required(npes, heap_bytes)
+        if need == 0:
+            raise ShmemgError(ERR.ARG, "shmemg_slab_bytes_required")
+        self.slab = torch.empty(need, dtype=torch.uint8, device=self.device)   # torch allocations are >= 512-B aligned
+        h = C.c_void_p()
+        rc = L.shmemg_init(npes, heap_bytes, self.slab.data_ptr(), need, C.byref(h))
+        if rc:
+            raise ShmemgError(rc, "shmemg_init")
+        self.h = h
+        self.npes = L.shmemg_n_pes(h)
+        self.heap_bytes = L.shmemg_heap_bytes(h)
+        self.stride = L.shmemg_heap_stride(h)
+        self.launches = 0                  # kernels launched through this object (launch accounting)
+
+    def _chk(self, rc: int, what: str):
+        if rc:
+            detail = lib().shmemg_last_cuda_error(self.h).decode() if rc == ERR.CUDA else ""
+            raise ShmemgError(rc, what, detail)
+
+    def finalize(self):
+        if self.h:
+            lib().shmemg_finalize(self.h)
+            self.h = None
+
+    # ---- capability / allocation / translation -----------------------------------------------------------
+    def query_capabilities(self, team: int = TEAM.WORLD) -> int:
+        caps = C.c_uint64(0)
+        self._chk(lib().shmem_query_capabilities(self.h, team, C.byref(caps)), "shmem_query_capabilities")
+        return caps.value
+
+    def malloc(self, nbytes: int) -> int:
+        off = C.c_uint64(0)
+        self._chk(lib().shmemg_malloc(self.h, nbytes, C.byref(off)), "shmemg_malloc")
+        return off.value
+
+    def calloc(self, count: int, size: int, stream=None) -> int:
+        off = C.c_uint64(0)
+        self._chk(lib().shmemg_calloc(self.h, count, size, C.byref(off), _stream(stream)), "shmemg_calloc")
+        return off.value
+
+    def align(self, alignment: int, nbytes: int) -> int:
+        off = C.c_uint64(0)
+        self._chk(lib().shmemg_align(self.h, alignment, nbytes, C.byref(off)), "shmemg_align")
+        return off.value
+
+    def free(self, off: int):
+        self._chk(lib().shmemg_free(self.h, off), "shmemg_free")
+
+    def ptr(self, off: int, pe: int) -> int:
+        return lib().shmemg_ptr(self.h, off, pe) or 0
+
+    def view(self, off: int, nbytes: int, dtype=torch.uint8) -> torch.Tensor:
+        """[npes, nbytes/itemsize] strided torch view of a symmetric object (plumbing: fill / read back)."""
+        t = self.slab[: self.npes * self.stride].view(self.npes, self.stride)[:, off:off + nbytes]
+        return t if dtype == torch.uint8 else t.view(dtype)
+
+    def heap_write(self, pe: int, dst_off: int, src_host: torch.Tensor, stream=None):
+        assert not src_host.is_cuda and src_host.is_contiguous()
+        self._chk(lib().shmemg_heap_write_on_stream(self.h, pe, dst_off, src_host.data_ptr(),
+                                                    src_host.numel() * src_host.element_size(), _stream(stream)),
+                  "shmemg_heap_write_on_stream")
+
+    def heap_read(self, pe: int, dst_host: torch.Tensor, src_off: int, stream=None):
+        assert not dst_host.is_cuda and dst_host.is_contiguous()
+        self._chk(lib().shmemg_heap_read_on_stream(self.h, pe, dst_host.data_ptr(), src_off,
+                                                   dst_host.numel() * dst_host.element_size(), _stream(stream)),
+                  "shmemg_heap_read_on_stream")
+
+    # ---- batches and single ops ---------------------------------------------------------------------------------
+    def batch(self, ops: np.ndarray, stream=None) -> Batch:
+        return Batch(self, ops, stream)
+
+    def enqueue_batch(self, batch: Batch, stream=None):
+        batch.enqueue(stream)
+        self.launches += batch.launches
+
+    def put(self, dest_off, source_off, nbytes, pe, target_pe, stream=None):
+        self._chk(lib().shmemg_put_on_stream(self.h, dest_off, source_off, nbytes, pe, target_pe, _stream(stream)),
+                  "shmemg_put_on_stream")
+        self.launches += 1 if nbytes else 0
+
+    def get(self, dest_off, source_off, nbytes, pe, target_pe, stream=None):
+        self._chk(lib().shmemg_get_on_stream(self.h, dest_off, source_off, nbytes, pe, target_pe, _stream(stream)),
+                  "shmemg_get_on_stream")
+        self.launches += 1 if nbytes else 0
+
+    def put_signal(self, dest_off, source_off, nbytes, sig_off, signal, sig_op, pe, target_pe, stream=None):
+        self._chk(lib().shmemg_put_signal_on_stream(self.h, dest_off, source_off, nbytes, sig_off, signal, sig_op, pe,
+                                                    target_pe, _stream(stream)), "shmemg_put_signal_on_stream")
+        self.launches += 1
+
+    def signal_wait_until(self, sig_off, cmp, value, pe, stream=None):
+        self._chk(lib().shmemg_signal_wait_until_on_stream(self.h, sig_off, cmp, value, pe, _stream(stream)),
+                  "shmemg_signal_wait_until_on_stream")
+        self.launches += 1
+
+    def fence(self, pe, stream=None):
+        self._chk(lib().shmemg_fence_on_stream(self.h, pe, _stream(stream)), "shmemg_fence_on_stream")
+
+    def quiet_on_stream(self, pe, stream=None):
+        self._chk(lib().shmemg_quiet_on_stream(self.h, pe, _stream(stream)), "shmemg_quiet_on_stream")
+
+    def quiet(self, pe, stream=None):
+        self._chk(lib().shmemg_quiet(self.h, pe, _stream(stream)), "shmemg_quiet")
+
+    # ---- SoA AMO batches -------------------------------------------------------------------------------------------
+    @staticmethod
+    def _idx_bytes(elem_idx):
+        assert elem_idx.dtype in (torch.int32, torch.int64, torch.uint32, torch.uint64)
+        return elem_idx.element_size()
+
+    def atomic_add_batch(self, sym_off, tgt_pe, elem_idx, val=None, val_scalar=0, flags=0, stream=None):
+        n = tgt_pe.numel()
+        self._chk(lib().shmemg_atomic_add_batch_on_stream(self.h, sym_off, _dptr(tgt_pe), _dptr(elem_idx),
+                                                          self._idx_bytes(elem_idx), _dptr(val), val_scalar & NO_STAMP,
+                                                          n, flags, _stream(stream)),
+                  "shmemg_atomic_add_batch_on_stream")
+        self.launches += 1 if n else 0
+
+    def atomic_fetch_add_batch(self, sym_off, tgt_pe, elem_idx, fetched_out, val=None, val_scalar=0, flags=0,
+                               stream=None):
+        n = tgt_pe.numel()
+        self._chk(lib().shmemg_atomic_fetch_add_batch_on_stream(self.h, sym_off, _dptr(tgt_pe), _dptr(elem_idx),
+                                                                self._idx_bytes(elem_idx), _dptr(val),
+                                                                val_scalar & NO_STAMP, _dptr(fetched_out), n, flags,
+                                                                _stream(stream)),
+                  "shmemg_atomic_fetch_add_batch_on_stream")
+        self.launches += 1 if n else 0
+
+    def atomic_compare_swap_batch(self, sym_off, tgt_pe, elem_idx, fetched_out, cond=None, cond_scalar=0, val=None,
+                                  val_scalar=0, flags=0, stream=None):
+        n = tgt_pe.numel()
+        self._chk(lib().shmemg_atomic_compare_swap_batch_on_stream(self.h, sym_off, _dptr(tgt_pe), _dptr(elem_idx),
+                                                                   self._idx_bytes(elem_idx), _dptr(cond),
+                                                                   cond_scalar & NO_STAMP, _dptr(val),
+                                                                   val_scalar & NO_STAMP, _dptr(fetched_out), n, flags,
+                                                                   _stream(stream)),
+                  "shmemg_atomic_compare_swap_batch_on_stream")
+        self.launches += 1 if n else 0
+
+    # ---- collectives -------------------------------------------------------------------------------------------------
+    def sum_reduce(self, dtype, dest_off, source_off, nreduce, stream=None):
+        self._chk(lib().shmemg_sum_reduce_on_stream(self.h, dtype, dest_off, source_off, nreduce, _stream(stream)),
+                  "shmemg_sum_reduce_on_stream")
+        self.launches += 1 if nreduce else 0
+
+    def fcollect(self, dest_off, source_off, nbytes, stream=None):
+        self._chk(lib().shmemg_fcollect_on_stream(self.h, dest_off, source_off, nbytes, _stream(stream)),
+                  "shmemg_fcollect_on_stream")
+        self.launches += 1 if nbytes else 0
+
+    def alltoall(self, dest_off, source_off, nbytes, stream=None):
+        self._chk(lib().shmemg_alltoall_on_stream(self.h, dest_off, source_off, nbytes, _stream(stream)),
+                  "shmemg_alltoall_on_stream")
+        self.launches += 1 if nbytes else 0
+
+    def barrier_all(self, stream=None):
+        self._chk(lib().shmemg_barrier_all_on_stream(self.h, _stream(stream)), "shmemg_barrier_all_on_stream")
+        self.launches += 1
+
+    def barrier_all_repeat(self, count, stamp_off=NO_STAMP, stream=None):
+        self._chk(lib().shmemg_barrier_all_repeat_on_stream(self.h, count, stamp_off, _stream(stream)),
+                  "shmemg_barrier_all_repeat_on_stream")
+        self.launches += 1 if count else 0
+
+    def barrier_epoch(self, stream=None) -> int:
+        return lib().shmemg_barrier_epoch(self.h, _stream(stream))
+
+    # ---- halo application kernels (include/shmemg_app.h; not library ops) ---------------------------------------------
+    def app_halo_perturb(self, U_off, B, seed, rnd, stream=None):
+        self._chk(lib().shmemg_app_halo_perturb_on_stream(self.h, U_off, B, seed, rnd, _stream(stream)),
+                  "shmemg_app_halo_perturb_on_stream")
+
+    def app_halo_pack(self, send_off, U_off, B, stream=None):
+        self._chk(lib().shmemg_app_halo_pack_on_stream(self.h, send_off, U_off, B, _stream(stream)),
+                  "shmemg_app_halo_pack_on_stream")
+
+    def app_checksum64(self, out, sym_off, seg_bytes, nseg, stream=None):
+        self._chk(lib().shmemg_app_checksum64_on_stream(self.h, _dptr(out), sym_off, seg_bytes, nseg, _stream(stream)),
+                  "shmemg_app_checksum64_on_stream")

@@ -1,0 +1,311 @@
+// collectives.cu -- world-team collectives, one kernel each.
+//   alltoall   : tiled transpose-copy, 128-bit streaming accesses; HBM-bound, 2*N*N*blk bytes
+//   fcollect   : each source chunk is read once into registers and stored to all N destinations (write-bound)
+//   sum_reduce : one pass down the N windows per column group, fp64 accumulation for fp32, N-way replicated store
+//   barrier    : stream-level (kernel boundary) and in-kernel (one CTA per PE, cooperative launch)
+#include "internal.cuh"
+
+// ---- alltoall: PE j's dest block i = PE i's source block j -------------------------------------------------------
+__global__ void __launch_bounds__(SHMEMG_THREADS, 4)
+k_alltoall(uint8_t *base, size_t stride, uint64_t dst_off, uint64_t src_off, size_t blk, int npes, unsigned chunk,
+           unsigned chunks_per_blk) {
+    const size_t nwork = (size_t)npes * npes * chunks_per_blk;
+    for (size_t wk = blockIdx.x; wk < nwork; wk += gridDim.x) {
+        const unsigned c = (unsigned)(wk % chunks_per_blk);
+        const size_t ij = wk / chunks_per_blk;
+        const int j = (int)(ij % npes), i = (int)(ij / npes);        // source-major: PE i's row is read contiguously
+        const size_t off = (size_t)c * chunk;
+        size_t n = blk - off;
+        if (n > chunk) n = chunk;
+        copy_coop<8>(base + (size_t)j * stride + dst_off + (size_t)i * blk + off,
+                     base + (size_t)i * stride + src_off + (size_t)j * blk + off, n, threadIdx.x, SHMEMG_THREADS);
+    }
+}
+
+// ---- fcollect: PE j's dest[p*n .. +n) = PE p's source[0 .. n) for every j -------------------------------------------
+// work item = (source PE p, 16-byte-vector chunk of its block, group of destination PEs)
+template <int VPT>   // vectors per thread held in registers
+__global__ void __launch_bounds__(SHMEMG_THREADS, 4)
+k_fcollect_vec(uint8_t *base, size_t stride, uint64_t dst_off, uint64_t src_off, size_t nbytes, int npes,
+               unsigned chunks_per_blk, int dst_groups) {
+    const size_t nvec = nbytes >> 4;
+    const unsigned chunk_vecs = SHMEMG_THREADS * VPT;
+    const size_t nwork = (size_t)npes * chunks_per_blk * dst_groups;
+    const int per_group = (npes + dst_groups - 1) / dst_groups;
+    for (size_t wk = blockIdx.x; wk < nwork; wk += gridDim.x) {
+        const int g = (int)(wk % dst_groups);
+        const size_t pc = wk / dst_groups;
+        const unsigned c = (unsigned)(pc % chunks_per_blk);
+        const int p = (int)(pc / chunks_per_blk);
+        const int4 *s = reinterpret_cast<const int4 *>(base + (size_t)p * stride + src_off) + (size_t)c * chunk_vecs;
+        const size_t left = nvec - (size_t)c * chunk_vecs;
+        int4 v[VPT];
+#pragma unroll
+        for (int u = 0; u < VPT; ++u) {
+            const size_t k = threadIdx.x + (size_t)u * SHMEMG_THREADS;
+            if (k < left) v[u] = ld_stream16(s + k);
+        }
+        const int j0 = g * per_group, j1 = min(npes, j0 + per_group);
+        for (int j = j0; j < j1; ++j) {
+            int4 *d = reinterpret_cast<int4 *>(base + (size_t)j * stride + dst_off + (size_t)p * nbytes) + (size_t)c * chunk_vecs;
+#pragma unroll
+            for (int u = 0; u < VPT; ++u) {
+                const size_t k = threadIdx.x + (size_t)u * SHMEMG_THREADS;
+                if (k < left) st_stream16(d + k, v[u]);
+            }
+        }
+    }
+}
+// generic byte path (unaligned sizes/offsets): plain per-(p, j) cooperative copies
+__global__ void __launch_bounds__(SHMEMG_THREADS, 4)
+k_fcollect_bytes(uint8_t *base, size_t stride, uint64_t dst_off, uint64_t src_off, size_t nbytes, int npes) {
+    const size_t nwork = (size_t)npes * npes;
+    for (size_t wk = blockIdx.x; wk < nwork; wk += gridDim.x) {
+        const int j = (int)(wk % npes), p = (int)(wk / npes);
+        copy_coop<4>(base + (size_t)j * stride + dst_off + (size_t)p * nbytes, base + (size_t)p * stride + src_off, nbytes,
+                     threadIdx.x, SHMEMG_THREADS);
+    }
+}
+
+// ---- sum_reduce ----------------------------------------------------------------------------------------------------
+// Each thread owns one 16-byte column group (4 fp32 or 2 int64), walks the N windows in ascending PE order with
+// PEU loads in flight, then stores the result vector to all N destinations.
+#define PEU 8
+__global__ void __launch_bounds__(SHMEMG_THREADS)
+k_sum_reduce_f32(uint8_t *base, size_t stride, uint64_t dst_off, uint64_t src_off, size_t nvec, int npes) {
+    for (size_t k = (size_t)blockIdx.x * blockDim.x + threadIdx.x; k < nvec; k += (size_t)gridDim.x * blockDim.x) {
+        const uint8_t *s = base + src_off + (k << 4);
+        double a0 = 0.0, a1 = 0.0, a2 = 0.0, a3 = 0.0;
+        int p = 0;
+        for (; p + PEU <= npes; p += PEU) {
+            int4 v[PEU];
+#pragma unroll
+            for (int u = 0; u < PEU; ++u) v[u] = ld_stream16(s + (size_t)(p + u) * stride);
+#pragma unroll
+            for (int u = 0; u < PEU; ++u) {       // ascending PE order, fp64 accumulate (reading 13)
+                a0 += (double)__int_as_float(v[u].x);
+                a1 += (double)__int_as_float(v[u].y);
+                a2 += (double)__int_as_float(v[u].z);
+                a3 += (double)__int_as_float(v[u].w);
+            }
+        }
+        for (; p < npes; ++p) {
+            const int4 v = ld_stream16(s + (size_t)p * stride);
+            a0 += (double)__int_as_float(v.x); a1 += (double)__int_as_float(v.y);
+            a2 += (double)__int_as_float(v.z); a3 += (double)__int_as_float(v.w);
+        }
+        int4 r;
+        r.x = __float_as_int(__double2float_rn(a0)); r.y = __float_as_int(__double2float_rn(a1));
+        r.z = __float_as_int(__double2float_rn(a2)); r.w = __float_as_int(__double2float_rn(a3));
+        uint8_t *d = base + dst_off + (k << 4);
+#pragma unroll 8
+        for (int j = 0; j < npes; ++j) st_stream16(d + (size_t)j * stride, r);
+    }
+}
+__global__ void __launch_bounds__(SHMEMG_THREADS)
+k_sum_reduce_i64(uint8_t *base, size_t stride, uint64_t dst_off, uint64_t src_off, size_t nvec, int npes) {
+    for (size_t k = (size_t)blockIdx.x * blockDim.x + threadIdx.x; k < nvec; k += (size_t)gridDim.x * blockDim.x) {
+        const uint8_t *s = base + src_off + (k << 4);
+        unsigned long long a0 = 0, a1 = 0;
+        int p = 0;
+        for (; p + PEU <= npes; p += PEU) {
+            int4 v[PEU];
+#pragma unroll
+            for (int u = 0; u < PEU; ++u) v[u] = ld_stream16(s + (size_t)(p + u) * stride);
+#pragma unroll
+            for (int u = 0; u < PEU; ++u) {
+                a0 += ((unsigned long long)(unsigned)v[u].y << 32) | (unsigned)v[u].x;
+                a1 += ((unsigned long long)(unsigned)v[u].w << 32) | (unsigned)v[u].z;
+            }
+        }
+        for (; p < npes; ++p) {
+            const int4 v = ld_stream16(s + (size_t)p * stride);
+            a0 += ((unsigned long long)(unsigned)v.y << 32) | (unsigned)v.x;
+            a1 += ((unsigned long long)(unsigned)v.w << 32) | (unsigned)v.z;
+        }
+        int4 r;
+        r.x = (int)(unsigned)a0; r.y = (int)(unsigned)(a0 >> 32); r.z = (int)(unsigned)a1; r.w = (int)(unsigned)(a1 >> 32);
+        uint8_t *d = base + dst_off + (k << 4);
+#pragma unroll 8
+        for (int j = 0; j < npes; ++j) st_stream16(d + (size_t)j * stride, r);
+    }
+}
+// scalar tails / unaligned buffers: one element per thread
+template <typename T, typename ACC>
+__global__ void k_sum_reduce_scalar(uint8_t *base, size_t stride, uint64_t dst_off, uint64_t src_off, size_t first,
+                                    size_t n, int npes) {
+    for (size_t k = first + (size_t)blockIdx.x * blockDim.x + threadIdx.x; k < n; k += (size_t)gridDim.x * blockDim.x) {
+        ACC acc = 0;
+        for (int p = 0; p < npes; ++p)
+            acc += (ACC) * reinterpret_cast<const volatile T *>(base + (size_t)p * stride + src_off + k * sizeof(T));
+        const T r = (T)acc;
+        for (int j = 0; j < npes; ++j) *reinterpret_cast<T *>(base + (size_t)j * stride + dst_off + k * sizeof(T)) = r;
+    }
+}
+
+// ---- barriers ---------------------------------------------------------------------------------------------------------
+__global__ void k_barrier_epoch(CtlRegion *ctl) { atomicAdd(&ctl->barrier_epoch, 1ull); }
+
+// One CTA per PE agent, all co-resident (cooperative launch).  Sense-reversing counter barrier at GPU scope.
+__device__ __forceinline__ void pe_barrier(CtlRegion *ctl, unsigned npes, unsigned &gen) {
+    // thread 0 of the CTA acts for the PE
+    unsigned old;
+    asm volatile("atom.acq_rel.gpu.global.add.u32 %0, [%1], 1;" : "=r"(old) : "l"(&ctl->bar_count) : "memory");
+    if (old == npes - 1) {
+        ctl->bar_count = 0;                                      // ordered before the release below
+        asm volatile("st.release.gpu.global.u32 [%0], %1;" ::"l"(&ctl->bar_gen), "r"(gen + 1) : "memory");
+    } else {
+        while (ld_acquire_u32(&ctl->bar_gen) == gen) { }
+    }
+    gen++;
+}
+
+__global__ void __launch_bounds__(32) k_barrier_repeat(CtlRegion *ctl, uint8_t *base, size_t stride, unsigned npes,
+                                                       unsigned count, unsigned long long stamp_off, int do_stamp) {
+    if (threadIdx.x != 0) return;
+    const unsigned p = blockIdx.x;
+    unsigned gen = ld_acquire_u32(&ctl->bar_gen);          // all agents read the same value: nobody has arrived yet
+    if (!do_stamp) {
+        for (unsigned r = 0; r < count; ++r) pe_barrier(ctl, npes, gen);
+        return;
+    }
+    volatile unsigned long long *mine = reinterpret_cast<volatile unsigned long long *>(base + (size_t)p * stride + stamp_off);
+    volatile unsigned long long *right =
+        reinterpret_cast<volatile unsigned long long *>(base + (size_t)((p + 1) % npes) * stride + stamp_off);
+    unsigned long long bad = 0;
+    for (unsigned r = 1; r <= count; ++r) {
+        right[r & 1] = r;                 // "put" r into slot r&1 of the right neighbour
+        pe_barrier(ctl, npes, gen);       // barrier_all: the put is complete and visible
+        if (mine[r & 1] != r) bad++;      // my left neighbour's stamp of THIS round must be there
+        // no second barrier needed: slot r&1 is next written in round r+2, i.e. after barrier r+1, which this
+        // agent only reaches after the read above
+    }
+    mine[2] += bad;
+}
+
+// ---------------------------------------------------------------------------------------------------------
+// host entry points
+// ---------------------------------------------------------------------------------------------------------
+static bool ranges_overlap(uint64_t a, uint64_t b, uint64_t n_a, uint64_t n_b) { return a < b + n_b && b < a + n_a; }
+
+extern "C" int shmemg_alltoall_on_stream(shmemg_world_t *w, uint64_t dest_off, uint64_t source_off, size_t nbytes,
+                                         void *stream) {
+    if (!w) return SHMEMG_ERR_ARG;
+    const uint64_t tot = (uint64_t)nbytes * w->npes;
+    if (!shmemg_in_range(w, dest_off, tot) || !shmemg_in_range(w, source_off, tot)) return SHMEMG_ERR_RANGE;
+    if (nbytes == 0) return SHMEMG_OK;
+    if (ranges_overlap(dest_off, source_off, tot, tot)) return SHMEMG_ERR_OVERLAP;
+    const uint64_t maxgrid = (uint64_t)w->sm_count * w->ctas_per_sm;
+    unsigned chunk = 65536;
+    if (w->tile_bytes_override) chunk = (unsigned)w->tile_bytes_override;
+    else
+        while (chunk > 4096 && (uint64_t)w->npes * w->npes * ((nbytes + chunk - 1) / chunk) < maxgrid * 8) chunk >>= 1;
+    const unsigned cpb = (unsigned)((nbytes + chunk - 1) / chunk);
+    const uint64_t nwork = (uint64_t)w->npes * w->npes * cpb;
+    const unsigned grid = (unsigned)(nwork < maxgrid ? nwork : maxgrid);
+    k_alltoall<<<grid, SHMEMG_THREADS, 0, (cudaStream_t)stream>>>(w->base, w->stride, dest_off, source_off, nbytes,
+                                                                  w->npes, chunk, cpb);
+    SHMEMG_CUDA(w, cudaGetLastError());
+    return SHMEMG_OK;
+}
+
+extern "C" int shmemg_fcollect_on_stream(shmemg_world_t *w, uint64_t dest_off, uint64_t source_off, size_t nbytes,
+                                         void *stream) {
+    if (!w) return SHMEMG_ERR_ARG;
+    const uint64_t tot = (uint64_t)nbytes * w->npes;
+    if (!shmemg_in_range(w, dest_off, tot) || !shmemg_in_range(w, source_off, nbytes)) return SHMEMG_ERR_RANGE;
+    if (nbytes == 0) return SHMEMG_OK;
+    if (ranges_overlap(dest_off, source_off, tot, nbytes)) return SHMEMG_ERR_OVERLAP;
+    const uint64_t maxgrid = (uint64_t)w->sm_count * w->ctas_per_sm;
+    cudaStream_t st = (cudaStream_t)stream;
+    if (((dest_off | source_off | nbytes | w->stride) & 15) == 0) {
+        constexpr int VPT = 4;                                  // 256 threads * 4 * 16 B = 16 KiB per work item
+        const unsigned cpb = (unsigned)(((nbytes >> 4) + SHMEMG_THREADS * VPT - 1) / (SHMEMG_THREADS * VPT));
+        int groups = 1;                                         // split destinations until the grid is full
+        while (groups < w->npes && (uint64_t)w->npes * cpb * groups < maxgrid * 4) groups <<= 1;
+        if (groups > w->npes) groups = w->npes;
+        const uint64_t nwork = (uint64_t)w->npes * cpb * groups;
+        const unsigned grid = (unsigned)(nwork < maxgrid ? nwork : maxgrid);
+        k_fcollect_vec<VPT><<<grid, SHMEMG_THREADS, 0, st>>>(w->base, w->stride, dest_off, source_off, nbytes, w->npes,
+                                                             cpb, groups);
+    } else {
+        const uint64_t nwork = (uint64_t)w->npes * w->npes;
+        const unsigned grid = (unsigned)(nwork < maxgrid ? nwork : maxgrid);
+        k_fcollect_bytes<<<grid, SHMEMG_THREADS, 0, st>>>(w->base, w->stride, dest_off, source_off, nbytes, w->npes);
+    }
+    SHMEMG_CUDA(w, cudaGetLastError());
+    return SHMEMG_OK;
+}
+
+extern "C" int shmemg_sum_reduce_on_stream(shmemg_world_t *w, int dtype, uint64_t dest_off, uint64_t source_off,
+                                           size_t nreduce, void *stream) {
+    if (!w || (dtype != SHMEMG_F32 && dtype != SHMEMG_I64)) return SHMEMG_ERR_ARG;
+    const size_t esz = dtype == SHMEMG_F32 ? 4 : 8;
+    const uint64_t tot = (uint64_t)nreduce * esz;
+    if (!shmemg_in_range(w, dest_off, tot) || !shmemg_in_range(w, source_off, tot)) return SHMEMG_ERR_RANGE;
+    if ((dest_off | source_off) & (esz - 1)) return SHMEMG_ERR_ALIGN;
+    if (dest_off != source_off && ranges_overlap(dest_off, source_off, tot, tot)) return SHMEMG_ERR_OVERLAP;
+    if (nreduce == 0) return SHMEMG_OK;
+    cudaStream_t st = (cudaStream_t)stream;
+    const bool vec_ok = ((dest_off | source_off | w->stride) & 15) == 0;
+    const size_t nvec = vec_ok ? tot >> 4 : 0;
+    const size_t per_vec = 16 / esz;
+    if (nvec) {
+        size_t blocks = (nvec + SHMEMG_THREADS - 1) / SHMEMG_THREADS;
+        const size_t cap = (size_t)w->sm_count * 8 * 8;
+        if (blocks > cap) blocks = cap;
+        if (dtype == SHMEMG_F32)
+            k_sum_reduce_f32<<<(unsigned)blocks, SHMEMG_THREADS, 0, st>>>(w->base, w->stride, dest_off, source_off, nvec, w->npes);
+        else
+            k_sum_reduce_i64<<<(unsigned)blocks, SHMEMG_THREADS, 0, st>>>(w->base, w->stride, dest_off, source_off, nvec, w->npes);
+        SHMEMG_CUDA(w, cudaGetLastError());
+    }
+    const size_t first = nvec * per_vec;
+    if (first < nreduce) {
+        size_t blocks = (nreduce - first + 255) / 256;
+        if (blocks > 4096) blocks = 4096;
+        if (dtype == SHMEMG_F32)
+            k_sum_reduce_scalar<float, double><<<(unsigned)blocks, 256, 0, st>>>(w->base, w->stride, dest_off, source_off, first, nreduce, w->npes);
+        else
+            k_sum_reduce_scalar<unsigned long long, unsigned long long><<<(unsigned)blocks, 256, 0, st>>>(w->base, w->stride, dest_off, source_off, first, nreduce, w->npes);
+        SHMEMG_CUDA(w, cudaGetLastError());
+    }
+    return SHMEMG_OK;
+}
+
+extern "C" int shmemg_barrier_all_on_stream(shmemg_world_t *w, void *stream) {
+    if (!w) return SHMEMG_ERR_ARG;
+    k_barrier_epoch<<<1, 1, 0, (cudaStream_t)stream>>>(w->ctl);
+    SHMEMG_CUDA(w, cudaGetLastError());
+    return SHMEMG_OK;
+}
+
+extern "C" int shmemg_barrier_all_repeat_on_stream(shmemg_world_t *w, uint32_t count, uint64_t stamp_off, void *stream) {
+    if (!w) return SHMEMG_ERR_ARG;
+    const int do_stamp = stamp_off != UINT64_MAX;
+    if (do_stamp) {
+        if (!shmemg_in_range(w, stamp_off, 24)) return SHMEMG_ERR_RANGE;
+        if (stamp_off & 7) return SHMEMG_ERR_ALIGN;
+    }
+    if (count == 0) return SHMEMG_OK;
+    int per_sm = 0;
+    SHMEMG_CUDA(w, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_barrier_repeat, 32, 0));
+    if ((long long)per_sm * w->sm_count < w->npes) return SHMEMG_ERR_NOMEM;   // agents could not all be co-resident
+    CtlRegion *ctl = w->ctl;
+    uint8_t *base = w->base;
+    size_t stride = w->stride;
+    unsigned npes = (unsigned)w->npes;
+    unsigned long long so = do_stamp ? stamp_off : 0;
+    int ds = do_stamp;
+    void *args[] = {&ctl, &base, &stride, &npes, &count, &so, &ds};
+    SHMEMG_CUDA(w, cudaLaunchCooperativeKernel((void *)k_barrier_repeat, dim3(npes), dim3(32), args, 0, (cudaStream_t)stream));
+    return SHMEMG_OK;
+}
+
+extern "C" uint64_t shmemg_barrier_epoch(shmemg_world_t *w, void *stream) {
+    if (!w) return 0;
+    unsigned long long v = 0;
+    if (cudaMemcpyAsync(&v, &w->ctl->barrier_epoch, 8, cudaMemcpyDeviceToHost, (cudaStream_t)stream) != cudaSuccess) return 0;
+    cudaStreamSynchronize((cudaStream_t)stream);
+    return v;
+}

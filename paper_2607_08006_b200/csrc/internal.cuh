@@ -1,0 +1,164 @@
+// internal.cuh -- shared declarations of the shmemg CUDA path (sm_100a only).
+// Not part of the public boundary (include/shmemg.h); shares nothing with oracle/.
+#pragma once
+
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include <map>
+#include <string>
+
+#include "../../include/shmemg.h"
+
+#define SHMEMG_CTL_BYTES (64u * 1024u)     // control region carved from the tail of the slab
+#define SHMEMG_STRIDE_ALIGN 512u
+#define SHMEMG_MIN_ALIGN 256u
+#define SHMEMG_THREADS 256                 // threads per CTA of every copy-class kernel
+#define SHMEMG_SIG_SLOTS 1024              // completion counters for single put_signal launches
+
+// ---- control region layout (device) -------------------------------------------------------------------
+struct CtlRegion {
+    unsigned long long barrier_epoch;      // bumped by barrier_all_on_stream
+    unsigned int bar_count;                // in-kernel barrier: arrivals of the current generation
+    unsigned int bar_gen;                  // in-kernel barrier: generation (sense)
+    unsigned int pad[12];
+    unsigned int sig_counter[SHMEMG_SIG_SLOTS];   // last-arriver counters of single put_signal launches
+};
+
+// ---- host-side world ------------------------------------------------------------------------------------
+struct shmemg_world {
+    int npes = 0;
+    int device = 0;
+    int sm_count = 0;
+    size_t heap_bytes = 0;                 // usable bytes per PE
+    size_t stride = 0;                     // distance between PE windows
+    uint8_t *base = nullptr;               // DEVICE: window of PE 0
+    size_t slab_bytes = 0;
+    CtlRegion *ctl = nullptr;              // DEVICE
+    std::map<uint64_t, size_t> free_list;  // offset -> size, coalesced
+    std::map<uint64_t, size_t> live;       // offset -> size of live allocations
+    unsigned sig_seq = 0;
+    int ctas_per_sm = 4;                   // copy-class persistent grids: ctas_per_sm * sm_count CTAs
+    size_t tile_bytes_override = 0;        // SHMEMG_TILE_BYTES (experiments)
+    std::string last_cuda_error;
+};
+
+static inline int shmemg_cuda_fail(shmemg_world *w, cudaError_t e, const char *what) {
+    if (w) w->last_cuda_error = std::string(what) + ": " + cudaGetErrorString(e);
+    return SHMEMG_ERR_CUDA;
+}
+#define SHMEMG_CUDA(w, call)                                              \
+    do {                                                                  \
+        cudaError_t e__ = (call);                                         \
+        if (e__ != cudaSuccess) return shmemg_cuda_fail((w), e__, #call); \
+    } while (0)
+
+static inline bool shmemg_in_range(const shmemg_world *w, uint64_t off, uint64_t n) {
+    return off <= w->heap_bytes && n <= w->heap_bytes - off;
+}
+static inline bool shmemg_pe_ok(const shmemg_world *w, int pe) { return pe >= 0 && pe < w->npes; }
+// PE -> address translation (a3): base + pe*stride + off
+static inline uint8_t *shmemg_addr(const shmemg_world *w, int pe, uint64_t off) {
+    return w->base + (size_t)pe * w->stride + off;
+}
+
+#ifdef __CUDACC__
+// ---- memory-model primitives (GPU scope) --------------------------------------------------------------
+__device__ __forceinline__ unsigned ld_acquire_u32(const unsigned *p) {
+    unsigned v;
+    asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+    return v;
+}
+__device__ __forceinline__ unsigned long long ld_acquire_u64(const unsigned long long *p) {
+    unsigned long long v;
+    asm volatile("ld.acquire.gpu.global.u64 %0, [%1];" : "=l"(v) : "l"(p) : "memory");
+    return v;
+}
+__device__ __forceinline__ void red_release_add_u32(unsigned *p, unsigned v) {
+    asm volatile("red.release.gpu.global.add.u32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
+}
+__device__ __forceinline__ void red_release_add_u64(unsigned long long *p, unsigned long long v) {
+    asm volatile("red.release.gpu.global.add.u64 [%0], %1;" ::"l"(p), "l"(v) : "memory");
+}
+__device__ __forceinline__ void exch_release_u64(unsigned long long *p, unsigned long long v) {
+    asm volatile("{ .reg .b64 t; atom.release.gpu.global.exch.b64 t, [%0], %1; }" ::"l"(p), "l"(v) : "memory");
+}
+__device__ __forceinline__ bool cmp_u64(int cmp, unsigned long long s, unsigned long long v) {
+    switch (cmp) {
+    case SHMEMG_CMP_EQ: return s == v;
+    case SHMEMG_CMP_NE: return s != v;
+    case SHMEMG_CMP_GT: return s > v;
+    case SHMEMG_CMP_GE: return s >= v;
+    case SHMEMG_CMP_LT: return s < v;
+    default: return s <= v;
+    }
+}
+// signal update with release semantics: visible only after everything the caller has observed
+__device__ __forceinline__ void signal_update(unsigned long long *sig, unsigned long long v, int sig_op) {
+    if (sig_op == SHMEMG_SIGNAL_ADD) red_release_add_u64(sig, v);
+    else exch_release_u64(sig, v);
+}
+
+// ---- streaming 128-bit accesses: L2-coherent loads (never a stale L1 line), evict-first hints --------------
+__device__ __forceinline__ int4 ld_stream16(const void *p) {
+    int4 r;
+    asm volatile("ld.global.cg.v4.s32 {%0,%1,%2,%3}, [%4];" : "=r"(r.x), "=r"(r.y), "=r"(r.z), "=r"(r.w) : "l"(p));
+    return r;
+}
+__device__ __forceinline__ void st_stream16(void *p, const int4 &v) {
+    asm volatile("st.global.cg.v4.s32 [%0], {%1,%2,%3,%4};" ::"l"(p), "r"(v.x), "r"(v.y), "r"(v.z), "r"(v.w) : "memory");
+}
+
+template <typename T>
+__device__ __forceinline__ void copy_elems(uint8_t *dst, const uint8_t *src, size_t n, int tid, int nthr) {
+    T *d = reinterpret_cast<T *>(dst);
+    const volatile T *s = reinterpret_cast<const volatile T *>(src);
+    for (size_t i = tid; i < n; i += nthr) d[i] = s[i];
+}
+
+// Cooperative copy of n bytes, any alignment, by threads tid in [0, nthr).  Fast path: dst and src are
+// congruent mod 16 -> byte head, unrolled 128-bit body, byte tail.  Otherwise the widest element the
+// relative misalignment allows.  All loads bypass L1 (coherent at L2).
+template <int UNROLL>
+__device__ __forceinline__ void copy_coop(uint8_t *dst, const uint8_t *src, size_t n, int tid, int nthr) {
+    if (n == 0) return;
+    const unsigned rel = (unsigned)((reinterpret_cast<uintptr_t>(dst) ^ reinterpret_cast<uintptr_t>(src)) & 15u);
+    if (rel == 0) {
+        size_t head = (16u - (unsigned)(reinterpret_cast<uintptr_t>(dst) & 15u)) & 15u;
+        if (head > n) head = n;
+        if (tid < (int)head) dst[tid] = *reinterpret_cast<const volatile uint8_t *>(src + tid);
+        const size_t nvec = (n - head) >> 4;
+        int4 *d = reinterpret_cast<int4 *>(dst + head);
+        const int4 *s = reinterpret_cast<const int4 *>(src + head);
+        size_t i = tid;
+        const size_t step = (size_t)UNROLL * nthr;
+        for (; i + (size_t)(UNROLL - 1) * nthr < nvec; i += step) {
+            int4 v[UNROLL];
+#pragma unroll
+            for (int u = 0; u < UNROLL; ++u) v[u] = ld_stream16(s + i + (size_t)u * nthr);
+#pragma unroll
+            for (int u = 0; u < UNROLL; ++u) st_stream16(d + i + (size_t)u * nthr, v[u]);
+        }
+        for (; i < nvec; i += nthr) st_stream16(d + i, ld_stream16(s + i));
+        const size_t done = head + (nvec << 4);
+        const size_t tail = n - done;
+        if (tid < (int)tail) dst[done + tid] = *reinterpret_cast<const volatile uint8_t *>(src + done + tid);
+        return;
+    }
+    // relative misalignment: align dst to W, copy W-byte elements, byte head/tail
+    const unsigned W = (rel & 7u) == 0 ? 8u : (rel & 3u) == 0 ? 4u : (rel & 1u) == 0 ? 2u : 1u;
+    size_t head = (W - (unsigned)(reinterpret_cast<uintptr_t>(dst) & (W - 1u))) & (W - 1u);
+    if (head > n) head = n;
+    if (tid < (int)head) dst[tid] = *reinterpret_cast<const volatile uint8_t *>(src + tid);
+    const size_t nel = (n - head) / W;
+    switch (W) {
+    case 8: copy_elems<unsigned long long>(dst + head, src + head, nel, tid, nthr); break;
+    case 4: copy_elems<unsigned int>(dst + head, src + head, nel, tid, nthr); break;
+    case 2: copy_elems<unsigned short>(dst + head, src + head, nel, tid, nthr); break;
+    default: copy_elems<unsigned char>(dst + head, src + head, nel, tid, nthr); break;
+    }
+    const size_t done = head + nel * W;
+    const size_t tail = n - done;
+    if (tid < (int)tail) dst[done + tid] = *reinterpret_cast<const volatile uint8_t *>(src + done + tid);
+}
+#endif  // __CUDACC__

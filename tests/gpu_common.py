@@ -1,0 +1,55 @@
+"""Helpers shared by the GPU parity tests: run a neutral Program through the CUDA path (C-ABI via the
+binding) and through the oracle, and compare object by object."""
+from __future__ import annotations
+
+import numpy as np
+import torch
+
+from oracle import oracle as orc
+from paper_2607_08006_b200 import World
+from paper_2607_08006_b200.loader import Loaded
+
+DEV = "cuda:0"
+
+
+def heap_bytes_for(prog, slack=4096):
+    return sum((b + 255) // 256 * 256 for b in prog.obj_bytes) + slack
+
+
+def run_gpu(prog, batches=None, heap_bytes=None):
+    """batches: list of Programs sharing prog's objects (default: [prog]); each is one enqueue."""
+    hb = heap_bytes or heap_bytes_for(prog)
+    w = World(prog.npes, hb, DEV)
+    ld = Loaded(w, prog)
+    for q in (batches or [prog]):
+        b = w.batch(ld.translate(q))
+        w.enqueue_batch(b)
+    w.quiet(0)
+    return w, ld
+
+
+def run_oracle(prog, batches=None, heap_bytes=None):
+    hb = heap_bytes or heap_bytes_for(prog)
+    ow = orc.OracleWorld(prog.npes, hb)
+    ow.load_program(prog)
+    for q in (batches or [prog]):
+        ow.run_program(q)
+    return ow
+
+
+def assert_objects_equal(prog, ld, ow, names=None):
+    for name in (names or prog.obj_names):
+        g = ld.obj_numpy(name)
+        o = ow.obj(name)
+        if not np.array_equal(g, o):
+            bad = np.argwhere(g != o)
+            raise AssertionError("object %r differs at %d bytes; first (pe, byte) = %s" % (name, len(bad), bad[0]))
+
+
+def to_dev(a: np.ndarray) -> torch.Tensor:
+    a = np.ascontiguousarray(a)
+    if a.dtype == np.uint64:
+        a = a.view(np.int64)
+    if a.dtype == np.uint32:
+        a = a.view(np.int32)
+    return torch.from_numpy(a).to(DEV)

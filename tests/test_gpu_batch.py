@@ -1,0 +1,195 @@
+"""GPU parity: the batch executor (put/get/put_signal/wait/fence/quiet/barrier/AMOs through descriptors)
+against the CPU oracle, element by element, plus the brute-force outcome sets for tiny programs."""
+import numpy as np
+import pytest
+import torch
+
+from gpu_common import DEV, assert_objects_equal, heap_bytes_for, run_gpu, run_oracle
+from invariants import check_compare_swap_claim, check_fetch_add
+from litmus_model import enumerate_outcomes, to_spec_program
+from paper_2607_08006_b200 import CMP, ERR, OP, OP_DTYPE, ShmemgError, World
+from paper_2607_08006_b200.loader import Loaded
+from workloads import configs, gen, litmus
+from workloads.spec import Program
+
+pytestmark = pytest.mark.gpu
+M64 = (1 << 64) - 1
+
+
+@pytest.mark.parametrize("make", [
+    lambda: litmus.mp_fence(),
+    lambda: litmus.mp_fence(npes=64, rounds=6, nbytes=300000, lag=1),
+    lambda: litmus.mp_quiet_third_party(),
+    lambda: litmus.put_signal_sizes(),
+    lambda: litmus.signal_add_fanin(),
+    lambda: litmus.barrier_stamp(),
+    lambda: litmus.barrier_stamp(npes=128, rounds=12),
+], ids=["mp_fence", "mp_fence_big", "mp_quiet3", "put_signal_sizes", "signal_add_fanin", "barrier_stamp",
+        "barrier_stamp128"])
+def test_litmus_programs_match_oracle(make):
+    prog = make()
+    w, ld = run_gpu(prog)
+    ow = run_oracle(prog)
+    assert_objects_equal(prog, ld, ow)
+
+
+def test_barrier_stamp_log_is_round_numbers():
+    prog = litmus.barrier_stamp(npes=16, rounds=30)
+    w, ld = run_gpu(prog)
+    log = ld.obj_numpy("log", np.uint64)
+    assert (log[:, 1:] == np.arange(1, 31, dtype=np.uint64)).all()
+
+
+def test_random_put_get_program_unaligned():
+    """Race-free random puts/gets with arbitrary sizes and alignments: each op owns a private dest slot."""
+    npes, nops, slot = 6, 400, 5000
+    rng = np.random.default_rng(3)
+    prog = Program(npes)
+    src = gen.u64(npes * 40000 // 8, 77).view(np.uint8).reshape(npes, 40000)
+    prog.obj("src", 40000, src)
+    prog.obj("dst", nops * slot)
+    for k in range(nops):
+        i, t = int(rng.integers(npes)), int(rng.integers(npes))
+        n = int(rng.integers(0, slot - 32))
+        s, d = int(rng.integers(0, 40000 - n)), k * slot + int(rng.integers(0, 32))
+        if k % 2:
+            prog.put(i, t, ("dst", d), ("src", s), n)
+        else:
+            prog.get(i, t, ("dst", d), ("src", s), n)
+    w, ld = run_gpu(prog)
+    assert_objects_equal(prog, ld, run_oracle(prog))
+
+
+def test_random_amos_through_descriptors():
+    prog = litmus.random_amos()
+    w, ld = run_gpu(prog)
+    ow = run_oracle(prog)
+    assert_objects_equal(prog, ld, ow, names=["words"])          # finals are schedule-independent for adds...
+    ops = prog.ops
+    nw = prog.obj_bytes[0] // 8
+    words = ld.obj_numpy("words", np.uint64)
+    fetch = ld.obj_numpy("fetch", np.uint64)
+    key = ops["target"].astype(np.int64) * nw + (ops["rem_off"] // 8).astype(np.int64)
+    fa = ops["kind"] == 5
+    ad = ops["kind"] == 4
+    cs = ops["kind"] == 6
+    idx = np.arange(len(ops))
+    fetched = fetch[ops["initiator"], idx]                        # op i's private slot in its initiator's heap
+    # fetch-add invariant needs every update of the word: treat plain adds as unobserved updates by checking
+    # only words that received no plain add
+    plain_words = np.unique(key[ad])
+    sel = fa & ~np.isin(key, plain_words)
+    init = np.zeros(prog.npes * nw, dtype=np.uint64)
+    init.reshape(prog.npes, nw)[:, nw // 2:] = M64
+    fin = words.reshape(-1)
+    if sel.any():
+        sub_final = init.copy()
+        ks = np.unique(key[sel])
+        sub_final[ks] = fin[ks]
+        check_fetch_add(key[sel], ops["value"][sel], fetched[sel], init, sub_final)
+    cas_final = np.full(prog.npes * nw, M64, dtype=np.uint64)
+    kc = np.unique(key[cs])
+    cas_final[kc] = fin[kc]
+    check_compare_swap_claim(key[cs], ops["value"][cs], fetched[cs], cas_final)
+
+
+TINY = {
+    "mp_fence": ([[("put", 1, 0, 2), ("fence",), ("put", 1, 1, 3)], [("wait", 1, "eq", 1), ("get", 1, 4, 0)]],
+                 [[0, 0, 42, 1, 0], [0] * 5], [0, 0, 0, 1, 1]),
+    "mp_no_fence": ([[("put", 1, 0, 2), ("put", 1, 1, 3)], [("wait", 1, "eq", 1), ("get", 1, 4, 0)]],
+                    [[0, 0, 42, 1, 0], [0] * 5], [0, 0, 1, 1]),
+    "quiet_third_party": ([[("put", 1, 0, 2), ("quiet",), ("put", 2, 1, 3)], [],
+                           [("wait", 1, "eq", 1), ("get", 1, 4, 0)]],
+                          [[0, 0, 42, 1, 0], [0] * 5, [0] * 5], [0, 0, 0, 2, 2]),
+    "put_signal": ([[("put_signal", 1, 0, 2, 1, 9, "set")], [("wait", 1, "eq", 9), ("get", 1, 4, 0)]],
+                   [[0, 0, 42, 1, 0], [0] * 5], [0, 1, 1]),
+    "fadd_fadd": ([[("fadd", 1, 0, 2, 1)], [("fadd", 1, 0, 3, 1)]], [[0, 0], [0, 0]], [0, 1]),
+    "cas_cas": ([[("cas", 1, 0, M64, 100, 1)], [("cas", 1, 0, M64, 200, 1)]], [[M64, 0], [M64, 0]], [0, 1]),
+    "barrier": ([[("put", 1, 0, 2), ("barrier",), ("get", 0, 4, 0)], [("put", 0, 0, 2), ("barrier",), ("get", 1, 4, 0)]],
+                [[0, 0, 42, 0, 0], [0, 0, 43, 0, 0]], [0, 1, 0, 1, 0, 1]),
+    "quiet_readback": ([[("put", 1, 0, 2), ("quiet",), ("get", 1, 4, 0)], []], [[0, 0, 42, 0, 0], [0] * 5], [0, 0, 0]),
+    "add_fence_add": ([[("add", 1, 0, 7), ("fence",), ("add", 1, 1, 1)], [("wait", 1, "ge", 1), ("get", 1, 4, 0)]],
+                      [[0] * 5, [0] * 5], [0, 0, 0, 1, 1]),
+}
+
+
+@pytest.mark.parametrize("name", sorted(TINY))
+def test_tiny_programs_land_in_enumerated_outcome_set(name):
+    """The GPU's final state must be one of the states the ordering rules allow (brute force)."""
+    prog, init, order = TINY[name]
+    allowed = enumerate_outcomes(prog, init)
+    sp = to_spec_program(prog, init, order)
+    for _ in range(5):
+        w, ld = run_gpu(sp)
+        got = tuple(tuple(int(x) for x in row) for row in ld.obj_numpy("w", np.uint64))
+        assert got in allowed, (name, got)
+
+
+def test_batch_can_be_enqueued_repeatedly_and_stream_order_holds():
+    """Stream ordering: batch B enqueued after batch A on one stream reads everything A wrote;
+    an idempotent batch can be replayed (the last CTA re-arms the plan)."""
+    npes, blk = 8, 20000
+    a = configs.c3a_put_program(npes, blk)                       # src -> dst (transpose)
+    b = a.fork()
+    b.obj_names = a.obj_names
+    for i in range(npes):
+        for j in range(npes):
+            b.put(i, j, ("src", i * blk), ("dst", j * blk), blk)   # dst -> src (transpose back)
+    hb = heap_bytes_for(a)
+    w = World(npes, hb, DEV)
+    ld = Loaded(w, a)
+    ba, bb = w.batch(ld.translate(a)), w.batch(ld.translate(b))
+    src0 = ld.obj_numpy("src").copy()
+    for _ in range(3):
+        w.enqueue_batch(ba)
+        w.enqueue_batch(bb)
+    w.quiet(0)
+    exp_dst = src0.reshape(npes, npes, blk).transpose(1, 0, 2).reshape(npes, npes * blk)
+    assert np.array_equal(ld.obj_numpy("dst"), exp_dst)
+    assert np.array_equal(ld.obj_numpy("src"), src0)              # transpose of transpose
+
+
+def test_edge_cases_empty_and_zero_byte():
+    w = World(4, 1 << 16, DEV)
+    b = w.batch(np.zeros(0, dtype=OP_DTYPE))
+    w.enqueue_batch(b)
+    a = w.calloc(64, 8)
+    ops = np.zeros(3, dtype=OP_DTYPE)
+    ops["opcode"] = [OP.PUT, OP.PUT_SIGNAL, OP.SIGNAL_WAIT_UNTIL]
+    ops["initiator_pe"] = [0, 0, 1]
+    ops["target_pe"] = [1, 1, 1]
+    ops["rem_off"] = a
+    ops["loc_off"] = [a, a, a + 8]
+    ops["nbytes"] = 0                                             # zero-byte put and zero-byte put_signal
+    ops["sig_off"] = a + 8
+    ops["value"] = [0, 5, 5]
+    ops["cmp"] = CMP.EQ
+    w.enqueue_batch(w.batch(ops))
+    w.quiet(0)
+    v = w.view(a, 64 * 8, torch.int64).cpu().numpy()
+    assert v[1, 1] == 5 and v.sum() == 5
+    only_markers = np.zeros(3, dtype=OP_DTYPE)
+    only_markers["opcode"] = [OP.FENCE, OP.QUIET, OP.BARRIER_ALL]
+    w.enqueue_batch(w.batch(only_markers))
+    w.quiet(0)
+
+
+def test_bad_descriptors_are_rejected_on_the_host():
+    w = World(2, 4096, DEV)
+    def one(**kw):
+        o = np.zeros(1, dtype=OP_DTYPE)
+        for k, v in kw.items():
+            o[k] = v
+        return o
+    for kw, code in [
+        (dict(opcode=OP.PUT, target_pe=2, nbytes=8), ERR.PE),
+        (dict(opcode=OP.PUT, target_pe=1, rem_off=4090, nbytes=8), ERR.RANGE),
+        (dict(opcode=OP.ATOMIC_ADD, target_pe=1, rem_off=12), ERR.ALIGN),
+        (dict(opcode=OP.PUT_SIGNAL, target_pe=1, nbytes=8, sig_off=4), ERR.ALIGN),
+        (dict(opcode=OP.SIGNAL_WAIT_UNTIL, cmp=9), ERR.ARG),
+        (dict(opcode=77), ERR.ARG),
+        (dict(opcode=OP.FENCE, initiator_pe=5), ERR.PE),
+    ]:
+        with pytest.raises(ShmemgError) as e:
+            w.batch(one(**kw))
+        assert e.value.code == code, (kw, e.value)
