@@ -64,10 +64,12 @@ def test_random_amos_through_descriptors():
     prog = litmus.random_amos()
     w, ld = run_gpu(prog)
     ow = run_oracle(prog)
-    assert_objects_equal(prog, ld, ow, names=["words"])          # finals are schedule-independent for adds...
     ops = prog.ops
     nw = prog.obj_bytes[0] // 8
     words = ld.obj_numpy("words", np.uint64)
+    # add / fetch-add finals are schedule independent: bit-exact vs the oracle; CAS winners are not (invariants below)
+    assert np.array_equal(words[:, :nw // 2], ow.obj("words", np.uint64)[:, :nw // 2])
+    assert np.array_equal(words[:, nw // 2:] == M64, ow.obj("words", np.uint64)[:, nw // 2:] == M64)
     fetch = ld.obj_numpy("fetch", np.uint64)
     key = ops["target"].astype(np.int64) * nw + (ops["rem_off"] // 8).astype(np.int64)
     fa = ops["kind"] == 5

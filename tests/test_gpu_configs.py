@@ -85,7 +85,7 @@ def test_single_put_get_put_signal_wait_on_stream():
     assert np.array_equal(w.view(d, nb).cpu().numpy(), ow.view(od, nb))
     assert w.view(sig, 64, torch.int64).cpu().numpy()[3, 1] == 42
     with pytest.raises(ShmemgError):
-        w.put(d, s, nb + 1, 0, 1)
+        w.put(d, s, 4 * nb, 0, 1)               # runs past the end of the heap window
     with pytest.raises(ShmemgError):
         w.put_signal(d, s, 8, sig + 4, 1, SIGNAL.SET, 0, 1)
 
@@ -296,6 +296,9 @@ def test_sum_reduce_fcollect_ragged(npes, n, off):
         w.quiet(0)
         assert np.array_equal(w.view(d, 8 * n, torch.int64).cpu().numpy(), ow.view(od, 8 * n, np.int64))
     nb = 4 * n + (1 if off == 4 else 0)                         # odd byte count exercises the byte path
+    fs = gen.u64(npes * (nb // 8 + 1), 9).view(np.uint8).reshape(npes, -1)[:, :nb]
+    w.view(s, nb).copy_(torch.from_numpy(np.ascontiguousarray(fs)))
+    ow.view(os_, nb)[:] = fs
     w.fcollect(d, s, nb)
     ow.fcollect(od, os_, nb)
     w.quiet(0)
