@@ -1,0 +1,776 @@
+#!/usr/bin/env python
+"""bench.py -- the hot-path benchmark of the B200-native GPU-aware OpenSHMEM library.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl reference]
+
+One STEP is one pass of the whole hot path (every row of SURVEY.md 8(a)) over the five seeded synthetic workloads of
+BASELINE.json (C1 atomic adds, C2 halo exchange x50 rounds, C3 alltoall uniform + Zipf-skewed, C4 RMAT fetch-add +
+compare-swap, C5 sum_reduce / fcollect / 10 000 barriers), enqueued through the C-ABI on one stream.  Every library
+call is bracketed by CUDA events on the launching stream ("segments"); application compute of the halo workload
+(perturb, pack) and the re-initialisation of AMO targets run between segments and are not library time.
+
+  metric `rma_alltoall_GBps` : algorithmic bytes of the copy-class segments (put / put_signal / alltoall / fcollect /
+                               sum_reduce; read + write) / their summed device time, summed over ranks
+  `amo_mops`                 : AMO ops of C1 + C4 / their summed device time
+  `barrier`                  : us per barrier, in-kernel (128 co-resident PE agents) and stream-level
+  `roofline`                 : the copy-class kernel with the largest share of the timed step, against MEASURED_PEAKS.json
+  `e2e`                      : the same metric with every input copied from pinned HOST memory and every result read
+                               back to the host inside the timed region (shmemg_heap_write/read_on_stream)
+  `cpu_baseline`             : the CPU oracle (oracle/, single thread) on a bounded sample of the same workload
+
+`--impl reference` times the oracle alone (this tier's reference arm).  N > 1 runs N independent replicas (the path
+does not shard: north_star "no sharding and no inter-GPU transport"), one process per GPU, max-over-ranks timing.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import numpy as np  # noqa: E402
+
+METRIC, UNIT = "rma_alltoall_GBps", "GB/s"
+WORKLOAD = ("C1-C5 of BASELINE.json in one step: C3a alltoall 64 PEs x 64 KiB blocks; C3b 4096 Zipf(1.1) puts; "
+            "C2 halo 8 PEs x 6 faces x 512 KiB put_signal+wait x 50 rounds; C5 sum_reduce f32/i64 + fcollect on 128 PEs "
+            "+ 10 000 barriers; C1 65 536 atomic adds; C4 RMAT scale 22, 2^26 fetch-add + 2^26 compare-swap")
+HALO_ROUNDS = 50
+BARRIERS = 10000
+M64 = (1 << 64) - 1
+
+# dram__bytes_read.sum + dram__bytes_write.sum per launch from the `ncu --set full` capture summarised in
+# profiles/ (file named in each entry); None until a capture of that kernel exists.
+NCU_TRAFFIC = {}
+
+
+def parse_args():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
+    ap.add_argument("--no-e2e", action="store_true", help="skip the end-to-end (host buffers) leg")
+    ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
+    ap.add_argument("--small", action="store_true", help="reduced sizes (development only; marked in the JSON)")
+    ap.add_argument("--only", default="", help="comma-separated segment groups to run: c1,c2,c3a,c3b,c4,c5,barrier")
+    return ap.parse_args()
+
+
+def measured_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        try:
+            return float(json.load(open(p))["hbm_gbs"]), "MEASURED_PEAKS.json (measured)"
+        except Exception:
+            pass
+    return 6650.0, "B200_PROFILING.md fallback"
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled every 100 ms while the timed region runs."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.index, self.proc = index, None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q,
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+        except OSError:
+            self.proc = None
+
+    def stop(self):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.proc.terminate()
+        try:
+            out, _ = self.proc.communicate(timeout=5)
+        except subprocess.TimeoutExpired:
+            self.proc.kill()
+            out, _ = self.proc.communicate()
+        sm, mx, pw, reasons = [], [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for line in out.strip().splitlines():
+            f = [x.strip() for x in line.split(",")]
+            if len(f) < 7:
+                continue
+            try:
+                sm.append(float(f[0])); mx.append(float(f[1])); pw.append(float(f[2]))
+            except ValueError:
+                continue
+            for n, v in zip(names, f[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(n)
+        if not sm:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["no samples"]}
+        return {"sm_mhz": statistics.median(sm), "sm_max_mhz": max(mx), "power_w_max": max(pw), "samples": len(sm),
+                "reasons": sorted(reasons)}
+
+
+# ======================================================================================================================
+# inputs: generated once on the host by the seeded generators of workloads/ (no method arithmetic there)
+# ======================================================================================================================
+class Inputs:
+    def __init__(self, small: bool, groups):
+        from workloads import configs
+        self.small = small
+        t0 = time.time()
+        self.groups = groups
+        if "c1" in groups:
+            self.c1 = configs.c1_atomic_add()
+        if "c2" in groups:
+            self.halo = configs.Halo(64 if small else 256)
+            self.halo_U = self.halo.initial_U()
+        if "c3a" in groups:
+            self.c3a_npes, self.c3a_blk = (16, 65536) if small else (64, 65536)
+            self.c3a = configs.c3a_payload(self.c3a_npes, self.c3a_blk)
+        if "c3b" in groups:
+            self.c3b = configs.c3b_skewed(npes=16 if small else 64)
+        if "c4" in groups:
+            self.c4 = configs.c4_graph(scale=18 if small else 22)
+        if "c5" in groups or "barrier" in groups:
+            self.c5_npes, self.c5_bytes = (32, 1 << 20) if small else (128, 4 << 20)
+            self.c5_fc_bytes = 32768
+        if "c5" in groups:
+            self.c5_f32 = configs.c5_f32(self.c5_npes, self.c5_bytes // 4)
+            self.c5_i64 = configs.c5_i64(self.c5_npes, self.c5_bytes // 8)
+            self.c5_fc = configs.c5_fcollect_src(self.c5_npes, self.c5_fc_bytes)
+        self.gen_seconds = time.time() - t0
+
+
+# algorithmic bytes / ops of each segment: copies count read + write
+def segment_table(inp: Inputs):
+    seg = {}
+    g = inp.groups
+    if "c3a" in g:
+        n, b = inp.c3a_npes, inp.c3a_blk
+        seg["alltoall"] = dict(cls="copy", kernel="k_alltoall", bytes=2 * n * n * b, launches=1)
+    if "c3b" in g:
+        seg["put_batch_skewed"] = dict(cls="copy", kernel="k_batch_exec", bytes=2 * int(inp.c3b.sizes.sum()), launches=1)
+    if "c2" in g:
+        seg["halo_put_signal_wait"] = dict(cls="copy", kernel="k_batch_exec",
+                                           bytes=HALO_ROUNDS * 2 * 48 * inp.halo.face_bytes, launches=HALO_ROUNDS)
+    if "c5" in g:
+        n, nb = inp.c5_npes, inp.c5_bytes
+        seg["sum_reduce_f32"] = dict(cls="copy", kernel="k_sum_reduce_f32", bytes=2 * n * nb, launches=1)
+        seg["sum_reduce_i64"] = dict(cls="copy", kernel="k_sum_reduce_i64", bytes=2 * n * nb, launches=1)
+        seg["fcollect"] = dict(cls="copy", kernel="k_fcollect_vec",
+                               bytes=n * inp.c5_fc_bytes + n * n * inp.c5_fc_bytes, launches=1)
+    if "c1" in g:
+        seg["atomic_add"] = dict(cls="amo", kernel="k_amo<add>", ops=len(inp.c1.val), launches=2)   # + barrier kernel
+    if "c4" in g:
+        E = len(inp.c4.u)
+        seg["atomic_fetch_add"] = dict(cls="amo", kernel="k_amo<fetch_add>", ops=E, launches=1)
+        seg["atomic_compare_swap"] = dict(cls="amo", kernel="k_amo<compare_swap>", ops=E, launches=1)
+    if "barrier" in g:
+        seg["barrier_in_kernel"] = dict(cls="sync", kernel="k_barrier_repeat", ops=BARRIERS, launches=1)
+        seg["barrier_on_stream"] = dict(cls="sync", kernel="k_barrier_epoch", ops=BARRIERS, launches=BARRIERS)
+    return seg
+
+
+# ======================================================================================================================
+# CUDA arm: everything goes through the C-ABI (binding = argument marshalling only)
+# ======================================================================================================================
+class Recorder:
+    """CUDA-event pairs around library calls, on the launching (current) stream."""
+
+    def __init__(self, torch):
+        self.torch, self.pairs, self.on = torch, [], False
+
+    class _Seg:
+        def __init__(self, rec, name):
+            self.rec, self.name = rec, name
+
+        def __enter__(self):
+            if self.rec.on:
+                self.a = self.rec.torch.cuda.Event(enable_timing=True)
+                self.b = self.rec.torch.cuda.Event(enable_timing=True)
+                self.a.record()
+
+        def __exit__(self, *exc):
+            if self.rec.on:
+                self.b.record()
+                self.rec.pairs.append((self.name, self.a, self.b))
+
+    def seg(self, name):
+        return Recorder._Seg(self, name)
+
+    def totals_ms(self):
+        out = {}
+        for name, a, b in self.pairs:
+            out[name] = out.get(name, 0.0) + a.elapsed_time(b)
+        return out
+
+
+class CudaBench:
+    def __init__(self, inp: Inputs, device):
+        import torch
+        from paper_2607_08006_b200 import World
+        from paper_2607_08006_b200.binding import AMO_WARP_AGGREGATE
+        from paper_2607_08006_b200.loader import Loaded
+        self.torch, self.inp, self.dev = torch, inp, device
+        self.rec = Recorder(torch)
+        self.app_launches = 0
+        self.worlds = []
+        self.flags = AMO_WARP_AGGREGATE
+        g = inp.groups
+        dv = lambda a: torch.from_numpy(np.ascontiguousarray(a)).to(device)      # noqa: E731
+        if "c3a" in g:
+            n, b = inp.c3a_npes, inp.c3a_blk
+            w = World(n, 2 * n * b + 4096, device)
+            self.w3a, self.a_src, self.a_dst = w, w.malloc(n * b), w.malloc(n * b)
+            w.view(self.a_src, n * b).copy_(torch.from_numpy(inp.c3a))
+            w.view(self.a_dst, n * b).zero_()
+            self.worlds.append(w)
+        if "c3b" in g:
+            prog = inp.c3b.prog
+            hb = sum((x + 255) // 256 * 256 for x in prog.obj_bytes) + 4096
+            w = World(prog.npes, hb, device)
+            self.w3b, self.ld3b = w, Loaded(w, prog)
+            self.b3b = w.batch(self.ld3b.translate(prog))
+            self.worlds.append(w)
+        if "c2" in g:
+            h = inp.halo
+            prog = h.program(with_consume=False, with_U=False)
+            hb = h.B ** 3 * 8 + sum((x + 255) // 256 * 256 for x in prog.obj_bytes) + 8192
+            w = World(8, hb, device)
+            self.w2 = w
+            self.U_off = w.malloc(h.B ** 3 * 8)
+            w.view(self.U_off, h.B ** 3 * 8).copy_(torch.from_numpy(inp.halo_U.view(np.uint8)))
+            self.ld2 = Loaded(w, prog)
+            self.halo_batches = [w.batch(self.ld2.translate(h.round_ops(prog, r, False))) for r in range(1, HALO_ROUNDS + 1)]
+            self.worlds.append(w)
+        if "c5" in g or "barrier" in g:
+            n, nb = inp.c5_npes, inp.c5_bytes
+            w = World(n, 3 * nb + inp.c5_fc_bytes + 65536, device)
+            self.w5 = w
+            self.worlds.append(w)
+            self.stamp = w.calloc(3, 8)
+        if "c5" in g:
+            w = self.w5
+            self.s_f32, self.s_i64, self.d5, self.s_fc = w.malloc(nb), w.malloc(nb), w.malloc(nb), w.malloc(inp.c5_fc_bytes)
+            w.view(self.s_f32, nb, torch.float32).copy_(torch.from_numpy(inp.c5_f32))
+            w.view(self.s_i64, nb, torch.int64).copy_(torch.from_numpy(inp.c5_i64))
+            w.view(self.s_fc, inp.c5_fc_bytes).copy_(torch.from_numpy(inp.c5_fc))
+        if "c1" in g:
+            c = inp.c1
+            w = World(c.npes, c.nelem * 8 + 4096, device)
+            self.w1, self.A = w, w.calloc(c.nelem, 8)
+            self.c1_t, self.c1_i, self.c1_v = dv(c.tgt_pe), dv(c.idx.astype(np.int64)), dv(c.val)
+            self.worlds.append(w)
+        if "c4" in g:
+            q = inp.c4
+            vpp, E = q.verts_per_pe, len(q.u)
+            w = World(q.npes, 2 * vpp * 8 + 4096, device)
+            self.w4, self.deg, self.par = w, w.calloc(vpp, 8), w.malloc(vpp * 8)
+            self.c4_ou, self.c4_lu = dv(q.owner(q.u)), dv(q.local(q.u).astype(np.uint32).view(np.int32))
+            self.c4_ov, self.c4_lv = dv(q.owner(q.v)), dv(q.local(q.v).astype(np.uint32).view(np.int32))
+            self.c4_val = dv(q.u.astype(np.int64))
+            self.f_deg = torch.empty(E, dtype=torch.int64, device=device)
+            self.f_par = torch.empty(E, dtype=torch.int64, device=device)
+            self.worlds.append(w)
+        torch.cuda.synchronize(device)
+
+    def launches(self):
+        return sum(w.launches for w in self.worlds) + self.app_launches
+
+    # ---- one pass of the whole hot path; device-resident inputs ------------------------------------------------------
+    def step(self):
+        torch, inp, rec, g = self.torch, self.inp, self.rec, self.inp.groups
+        if "c3a" in g:
+            with rec.seg("alltoall"):
+                self.w3a.alltoall(self.a_dst, self.a_src, inp.c3a_blk)
+        if "c5" in g:
+            n = inp.c5_bytes
+            with rec.seg("sum_reduce_f32"):
+                self.w5.sum_reduce(0, self.d5, self.s_f32, n // 4)
+        if "c3b" in g:
+            with rec.seg("put_batch_skewed"):
+                self.w3b.enqueue_batch(self.b3b)
+        if "c5" in g:
+            with rec.seg("sum_reduce_i64"):
+                self.w5.sum_reduce(1, self.d5, self.s_i64, n // 8)
+            with rec.seg("fcollect"):
+                self.w5.fcollect(self.d5, self.s_fc, inp.c5_fc_bytes)
+        if "c2" in g:
+            h, w = inp.halo, self.w2
+            self.ld2.obj("sig").zero_()                                  # rounds restart at 1 every step
+            send_off = self.ld2.off["send"][0]
+            for r in range(1, HALO_ROUNDS + 1):
+                w.app_halo_perturb(self.U_off, h.B, h.seed, r)           # application compute, not library time
+                w.app_halo_pack(send_off, self.U_off, h.B)
+                self.app_launches += 2
+                with rec.seg("halo_put_signal_wait"):
+                    w.enqueue_batch(self.halo_batches[r - 1])
+        if "c1" in g:
+            self.w1.view(self.A, inp.c1.nelem * 8).zero_()
+            with rec.seg("atomic_add"):
+                self.w1.atomic_add_batch(self.A, self.c1_t, self.c1_i, val=self.c1_v, flags=self.flags)
+                self.w1.quiet_on_stream(0)
+                self.w1.barrier_all()
+        if "c4" in g:
+            vpp = inp.c4.verts_per_pe
+            self.w4.view(self.deg, vpp * 8).zero_()
+            self.w4.view(self.par, vpp * 8).fill_(255)
+            with rec.seg("atomic_fetch_add"):
+                self.w4.atomic_fetch_add_batch(self.deg, self.c4_ou, self.c4_lu, self.f_deg, val=None, val_scalar=1,
+                                               flags=self.flags)
+            with rec.seg("atomic_compare_swap"):
+                self.w4.atomic_compare_swap_batch(self.par, self.c4_ov, self.c4_lv, self.f_par, cond=None, cond_scalar=M64,
+                                                  val=self.c4_val, flags=self.flags)
+        if "barrier" in g:
+            with rec.seg("barrier_in_kernel"):
+                self.w5.barrier_all_repeat(BARRIERS)
+            with rec.seg("barrier_on_stream"):
+                for _ in range(BARRIERS):
+                    self.w5.barrier_all()
+
+    # ---- end-to-end: the same ops with HOST buffers, H2D / D2H inside the timed region --------------------------------
+    def setup_e2e(self):
+        torch, inp, g = self.torch, self.inp, self.inp.groups
+        pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory()      # noqa: E731
+        pz = lambda *shape, dt=torch.uint8: torch.empty(*shape, dtype=dt).pin_memory()  # noqa: E731
+        self.h2d = self.d2h = 0
+        if "c3a" in g:
+            self.h_a_src, self.h_a_dst = pin(inp.c3a), pz(*inp.c3a.shape)
+        if "c3b" in g:
+            self.h_b_src = pin(inp.c3b.prog.init["src"])
+            self.h_b_dst = pz(inp.c3b.prog.npes, inp.c3b.dst_bytes)
+        if "c2" in g:
+            fb = inp.halo.face_bytes
+            send = self.ld2.obj("send").cpu().contiguous()                      # faces of the last round: representative payload
+            self.h_send, self.h_ghost = send.pin_memory(), pz(8, 6 * fb)
+        if "c5" in g:
+            self.h_f32, self.h_i64, self.h_fc = pin(inp.c5_f32.view(np.uint8)), pin(inp.c5_i64.view(np.uint8)), pin(inp.c5_fc)
+            self.h_res = pz(3, inp.c5_bytes)
+        if "c1" in g:
+            c = inp.c1
+            self.h_c1 = [pin(c.tgt_pe), pin(c.idx.astype(np.int64)), pin(c.val)]
+            self.h_A = pz(c.npes, c.nelem * 8)
+        if "c4" in g:
+            self.h_c4 = [pin(t.cpu().numpy()) for t in (self.c4_ou, self.c4_lu, self.c4_ov, self.c4_lv, self.c4_val)]
+            E = len(inp.c4.u)
+            self.h_fdeg, self.h_fpar = pz(E, dt=torch.int64), pz(E, dt=torch.int64)
+            self.h_deg, self.h_par = pz(inp.c4.npes, inp.c4.verts_per_pe * 8), pz(inp.c4.npes, inp.c4.verts_per_pe * 8)
+
+    def _up(self, w, off, host2d):
+        for p in range(host2d.shape[0]):
+            w.heap_write(p, off, host2d[p])
+        self.h2d += host2d.numel() * host2d.element_size()
+
+    def _down(self, w, host2d, off):
+        for p in range(host2d.shape[0]):
+            w.heap_read(p, host2d[p], off)
+        self.d2h += host2d.numel() * host2d.element_size()
+
+    def e2e_step(self):
+        torch, inp, rec, g = self.torch, self.inp, self.rec, self.inp.groups
+        if "c3a" in g:
+            with rec.seg("alltoall"):
+                self._up(self.w3a, self.a_src, self.h_a_src)
+                self.w3a.alltoall(self.a_dst, self.a_src, inp.c3a_blk)
+                self._down(self.w3a, self.h_a_dst, self.a_dst)
+        if "c3b" in g:
+            with rec.seg("put_batch_skewed"):
+                self._up(self.w3b, self.ld3b.off["src"][0], self.h_b_src)
+                self.w3b.enqueue_batch(self.b3b)
+                self._down(self.w3b, self.h_b_dst, self.ld3b.off["dst"][0])
+        if "c5" in g:
+            n = inp.c5_bytes
+            with rec.seg("sum_reduce_f32"):
+                self._up(self.w5, self.s_f32, self.h_f32)
+                self.w5.sum_reduce(0, self.d5, self.s_f32, n // 4)
+                self._down(self.w5, self.h_res[0:1], self.d5)            # every PE holds the same result: read PE 0's
+            with rec.seg("sum_reduce_i64"):
+                self._up(self.w5, self.s_i64, self.h_i64)
+                self.w5.sum_reduce(1, self.d5, self.s_i64, n // 8)
+                self._down(self.w5, self.h_res[1:2], self.d5)
+            with rec.seg("fcollect"):
+                self._up(self.w5, self.s_fc, self.h_fc)
+                self.w5.fcollect(self.d5, self.s_fc, inp.c5_fc_bytes)
+                self._down(self.w5, self.h_res[2:3], self.d5)
+        if "c2" in g:
+            w, fb = self.w2, inp.halo.face_bytes
+            self.ld2.obj("sig").zero_()
+            send_off, ghost_off = self.ld2.off["send"][0], self.ld2.off["ghost"][0]
+            for r in range(1, HALO_ROUNDS + 1):
+                with rec.seg("halo_put_signal_wait"):
+                    self._up(w, send_off, self.h_send)
+                    w.enqueue_batch(self.halo_batches[r - 1])
+                    self._down(w, self.h_ghost, ghost_off + (r & 1) * 6 * fb)
+        if "c1" in g:
+            self.w1.view(self.A, inp.c1.nelem * 8).zero_()
+            with rec.seg("atomic_add"):
+                for d, h in zip((self.c1_t, self.c1_i, self.c1_v), self.h_c1):
+                    d.copy_(h, non_blocking=True)
+                    self.h2d += h.numel() * h.element_size()
+                self.w1.atomic_add_batch(self.A, self.c1_t, self.c1_i, val=self.c1_v, flags=self.flags)
+                self.w1.quiet_on_stream(0)
+                self.w1.barrier_all()
+                self._down(self.w1, self.h_A, self.A)
+        if "c4" in g:
+            vpp = inp.c4.verts_per_pe
+            self.w4.view(self.deg, vpp * 8).zero_()
+            self.w4.view(self.par, vpp * 8).fill_(255)
+            with rec.seg("atomic_fetch_add"):
+                for d, h in zip((self.c4_ou, self.c4_lu), self.h_c4[:2]):
+                    d.copy_(h, non_blocking=True)
+                    self.h2d += h.numel() * h.element_size()
+                self.w4.atomic_fetch_add_batch(self.deg, self.c4_ou, self.c4_lu, self.f_deg, val=None, val_scalar=1,
+                                               flags=self.flags)
+                self.h_fdeg.copy_(self.f_deg, non_blocking=True)
+                self.d2h += self.h_fdeg.numel() * 8
+                self._down(self.w4, self.h_deg, self.deg)
+            with rec.seg("atomic_compare_swap"):
+                for d, h in zip((self.c4_ov, self.c4_lv, self.c4_val), self.h_c4[2:]):
+                    d.copy_(h, non_blocking=True)
+                    self.h2d += h.numel() * h.element_size()
+                self.w4.atomic_compare_swap_batch(self.par, self.c4_ov, self.c4_lv, self.f_par, cond=None, cond_scalar=M64,
+                                                  val=self.c4_val, flags=self.flags)
+                self.h_fpar.copy_(self.f_par, non_blocking=True)
+                self.d2h += self.h_fpar.numel() * 8
+                self._down(self.w4, self.h_par, self.par)
+
+    # ---- ceilings measured in the same run ---------------------------------------------------------------------------
+    def ceilings(self, reps=5):
+        """L2-atomic ceilings (bare red / atom / cas at hashed addresses, include/shmemg_probe.h) on the C1 and C4
+        footprints, and the library's own plain-copy rate on the C5 world.  Returns Mops/s and GB/s (best of reps)."""
+        torch, inp, g = self.torch, self.inp, self.inp.groups
+        out = {}
+
+        def best(fn, units):
+            ts = []
+            for _ in range(reps + 1):
+                a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                a.record(); fn(); b.record(); b.synchronize()
+                ts.append(a.elapsed_time(b))
+            return units / (min(ts[1:]) * 1e-3)
+        if "c1" in g:
+            n = 1 << 24
+            out["red_add_512KiB_Mops"] = best(lambda: self.w1.probe_atomic(0, self.A, inp.c1.nelem, n), n) / 1e6
+        if "c4" in g:
+            n, vpp = len(inp.c4.u), inp.c4.verts_per_pe
+            out["red_add_32MiB_Mops"] = best(lambda: self.w4.probe_atomic(0, self.deg, vpp, n), n) / 1e6
+            out["atom_add_32MiB_Mops"] = best(lambda: self.w4.probe_atomic(1, self.deg, vpp, n), n) / 1e6
+            out["atom_cas_32MiB_Mops"] = best(lambda: self.w4.probe_atomic(2, self.par, vpp, n), n) / 1e6
+        if "c5" in g:
+            nb = inp.c5_bytes
+            out["copy_all_GBps"] = best(lambda: self.w5.probe_copy_all(self.d5, self.s_f32, nb), 2 * inp.c5_npes * nb) / 1e9
+        return out
+
+
+# ======================================================================================================================
+# oracle arm: the CPU oracle as it stands (single thread), on a bounded sample of the same step
+# ======================================================================================================================
+class OracleBench:
+    """Bounded sample of one step: C3a and C3b whole; C2 `halo_rounds` exchange rounds; C5 sum_reduce on the first
+    1/`reduce_div` of the elements (all PEs), fcollect whole; C1 whole; C4 the first 2^`c4_log2` edges."""
+
+    def __init__(self, inp: Inputs, halo_rounds=5, reduce_div=4, c4_log2=24):
+        from oracle import oracle as orc
+        self.orc, self.inp = orc, inp
+        g = inp.groups
+        self.halo_rounds, self.reduce_div = halo_rounds, reduce_div
+        self.sample = []
+        if "c3a" in g:
+            n, b = inp.c3a_npes, inp.c3a_blk
+            self.o3a = orc.OracleWorld(n, 2 * n * b + 512)
+            self.a_src, self.a_dst = self.o3a.malloc(n * b), self.o3a.malloc(n * b)
+            self.o3a.view(self.a_src, n * b)[:] = inp.c3a
+            self.sample.append("C3a whole")
+        if "c3b" in g:
+            prog = inp.c3b.prog
+            self.o3b = orc.OracleWorld(prog.npes, sum((x + 255) // 256 * 256 for x in prog.obj_bytes) + 512)
+            self.o3b.load_program(prog)
+            self.ops3b = self.o3b.translate(prog)
+            self.sample.append("C3b whole")
+        if "c2" in g:
+            h = inp.halo
+            prog = h.program(with_consume=False, with_U=False)
+            self.o2 = orc.OracleWorld(8, sum((x + 255) // 256 * 256 for x in prog.obj_bytes) + 512)
+            self.o2.load_program(prog)
+            self.o2.obj("send", np.uint64)[:] = np.arange(8 * 6 * h.face_bytes // 8, dtype=np.uint64).reshape(8, -1)
+            self.ops2 = [self.o2.translate(h.round_ops(prog, r, False)) for r in range(1, halo_rounds + 1)]
+            self.sample.append("C2 %d of %d exchange rounds (library ops only)" % (halo_rounds, HALO_ROUNDS))
+        if "c5" in g:
+            n, nb = inp.c5_npes, inp.c5_bytes
+            self.o5 = orc.OracleWorld(n, 3 * nb + inp.c5_fc_bytes + 1024)
+            self.s_f32, self.s_i64, self.d5 = self.o5.malloc(nb), self.o5.malloc(nb), self.o5.malloc(nb)
+            self.s_fc = self.o5.malloc(inp.c5_fc_bytes)
+            self.o5.view(self.s_f32, nb, np.float32)[:] = inp.c5_f32
+            self.o5.view(self.s_i64, nb, np.int64)[:] = inp.c5_i64
+            self.o5.view(self.s_fc, inp.c5_fc_bytes)[:] = inp.c5_fc
+            self.sample.append("C5 sum_reduce on the first 1/%d of the elements, fcollect whole" % reduce_div)
+        if "c1" in g:
+            c = inp.c1
+            self.o1 = orc.OracleWorld(c.npes, c.nelem * 8 + 512)
+            self.A = self.o1.malloc(c.nelem * 8)
+            self.sample.append("C1 whole")
+        if "c4" in g:
+            q = inp.c4
+            self.nedge = min(len(q.u), 1 << c4_log2)
+            self.o4 = orc.OracleWorld(q.npes, 2 * q.verts_per_pe * 8 + 512)
+            self.deg, self.par = self.o4.malloc(q.verts_per_pe * 8), self.o4.malloc(q.verts_per_pe * 8)
+            m = self.nedge
+            self.c4 = (q.owner(q.u[:m]), q.local(q.u[:m]), q.owner(q.v[:m]), q.local(q.v[:m]),
+                       np.ones(m, dtype=np.uint64), np.full(m, M64, dtype=np.uint64), q.u[:m].astype(np.uint64))
+            self.sample.append("C4 first %d of %d edges" % (m, len(q.u)))
+
+    def step(self):
+        """Returns {segment: (seconds, bytes or ops in the sample)}."""
+        inp, g, out = self.inp, self.inp.groups, {}
+        tm = time.perf_counter
+        if "c3a" in g:
+            t = tm(); self.o3a.alltoall(self.a_dst, self.a_src, inp.c3a_blk)
+            out["alltoall"] = (tm() - t, 2 * inp.c3a_npes ** 2 * inp.c3a_blk)
+        if "c3b" in g:
+            t = tm(); self.o3b.exec_ops(self.ops3b)
+            out["put_batch_skewed"] = (tm() - t, 2 * int(inp.c3b.sizes.sum()))
+        if "c2" in g:
+            self.o2.obj("sig")[:] = 0
+            t = tm()
+            for ops in self.ops2:
+                self.o2.exec_ops(ops)
+            out["halo_put_signal_wait"] = (tm() - t, self.halo_rounds * 2 * 48 * inp.halo.face_bytes)
+        if "c5" in g:
+            n, nb, dv = inp.c5_npes, inp.c5_bytes, self.reduce_div
+            t = tm(); self.o5.sum_reduce_f32(self.d5, self.s_f32, nb // 4 // dv)
+            out["sum_reduce_f32"] = (tm() - t, 2 * n * nb // dv)
+            t = tm(); self.o5.sum_reduce_i64(self.d5, self.s_i64, nb // 8 // dv)
+            out["sum_reduce_i64"] = (tm() - t, 2 * n * nb // dv)
+            t = tm(); self.o5.fcollect(self.d5, self.s_fc, inp.c5_fc_bytes)
+            out["fcollect"] = (tm() - t, n * inp.c5_fc_bytes * (n + 1))
+        if "c1" in g:
+            c = inp.c1
+            self.o1.view(self.A, c.nelem * 8)[:] = 0
+            t = tm(); self.o1.atomic_add_batch(self.A, c.tgt_pe, c.idx, c.val)
+            out["atomic_add"] = (tm() - t, len(c.val))
+        if "c4" in g:
+            vpp = inp.c4.verts_per_pe
+            self.o4.view(self.deg, vpp * 8)[:] = 0
+            self.o4.view(self.par, vpp * 8)[:] = 255
+            ou, lu, ov, lv, ones, cond, val = self.c4
+            t = tm(); self.o4.atomic_fetch_add_batch(self.deg, ou, lu, ones)
+            out["atomic_fetch_add"] = (tm() - t, self.nedge)
+            t = tm(); self.o4.atomic_compare_swap_batch(self.par, ov, lv, cond, val)
+            out["atomic_compare_swap"] = (tm() - t, self.nedge)
+        return out
+
+
+def class_rates(table, seg_seconds, seg_units):
+    """(copy GB/s, amo Mops/s) from per-segment seconds and units (bytes for copy-class, ops for amo-class)."""
+    cb = sum(seg_units[k] for k in seg_units if table[k]["cls"] == "copy")
+    cs = sum(seg_seconds[k] for k in seg_units if table[k]["cls"] == "copy")
+    ao = sum(seg_units[k] for k in seg_units if table[k]["cls"] == "amo")
+    as_ = sum(seg_seconds[k] for k in seg_units if table[k]["cls"] == "amo")
+    return (cb / cs / 1e9 if cs > 0 else 0.0), (ao / as_ / 1e6 if as_ > 0 else 0.0), cs, as_
+
+
+ALL_GROUPS = ["c1", "c2", "c3a", "c3b", "c4", "c5", "barrier"]
+
+
+def base_line(args, n_gpus):
+    return {"metric": METRIC, "unit": UNIT, "n_gpus": n_gpus, "steps": args.steps, "warmup": args.warmup,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "data": "synthetic",
+            "config": {"workload": WORKLOAD + (" [--small development sizes]" if args.small else ""),
+                       "parallelism": "replicas only (no sharding, no inter-GPU transport: north_star)",
+                       "l2": "inputs larger than L2: one step streams about 4.6 GiB through the 126 MB L2 between two "
+                             "uses of any buffer; by-nature L2-resident cases (C1's 512 KiB target, halo faces just packed) "
+                             "are kept as the application leaves them",
+                       "value_definition": "copy-class algorithmic bytes / summed CUDA-event time of the copy-class "
+                                           "segments (library calls only), summed over ranks"}}
+
+
+def run_reference(args):
+    """This tier's reference arm: the oracle, as it stands, on the host cores (rank 0 only)."""
+    if int(os.environ.get("RANK", "0")) != 0:
+        return
+    groups = [x for x in (args.only.split(",") if args.only else ALL_GROUPS) if x != "barrier"]
+    inp = Inputs(args.small, groups)
+    table = segment_table(inp)
+    ob = OracleBench(inp)
+    for _ in range(min(args.warmup, 1)):
+        ob.step()
+    secs, units = {}, {}
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        for k, (s, u) in ob.step().items():
+            secs[k] = secs.get(k, 0.0) + s
+            units[k] = units.get(k, 0) + u
+    wall = time.perf_counter() - t0
+    gbps, mops, _, _ = class_rates(table, secs, units)
+    line = base_line(args, args.gpus)
+    sample = "; ".join(ob.sample)
+    line.update({"impl": "reference", "value": gbps, "amo_mops": mops, "ms_per_step": wall / args.steps * 1e3, "dtype": "u8",
+                 "segments": {k: {"ms": secs[k] / args.steps * 1e3,
+                                  ("GBps" if table[k]["cls"] == "copy" else "Mops"):
+                                      units[k] / secs[k] / (1e9 if table[k]["cls"] == "copy" else 1e6)} for k in secs},
+                 "cpu_baseline": {"value": gbps, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
+                 "e2e": {"value": gbps, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+                 "gpu_launches": 0})
+    print(json.dumps(line))
+
+
+def run_cuda(args):
+    import torch
+    rank, world = int(os.environ.get("RANK", "0")), int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the shmemg hot path has no CPU fallback")
+    torch.cuda.set_device(local)
+    device = torch.device("cuda", local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=device)
+    groups = args.only.split(",") if args.only else ALL_GROUPS
+    inp = Inputs(args.small, groups)
+    table = segment_table(inp)
+    cb = CudaBench(inp, device)
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize(device)
+
+    # ---- device-resident leg ------------------------------------------------------------------------------------------
+    for _ in range(args.warmup):
+        cb.step()
+    barrier()
+    sampler = ClockSampler(local)
+    sampler.start()
+    l0 = cb.launches()
+    cb.rec.on = True
+    t_a, t_b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    t_a.record()
+    for _ in range(args.steps):
+        cb.step()
+    t_b.record()
+    barrier()
+    clocks = sampler.stop()
+    cb.rec.on = False
+    launches = cb.launches() - l0
+    whole_ms = t_a.elapsed_time(t_b)
+    seg_ms = cb.rec.totals_ms()                                   # summed over the K steps
+    cb.rec.pairs = []
+
+    # ---- end-to-end leg ---------------------------------------------------------------------------------------------------
+    e2e_ms, h2d, d2h = None, 0, 0
+    if not args.no_e2e:
+        cb.setup_e2e()
+        cb.e2e_step()
+        barrier()
+        cb.h2d = cb.d2h = 0
+        cb.rec.on = True
+        for _ in range(args.steps):
+            cb.e2e_step()
+        barrier()
+        cb.rec.on = False
+        e2e_ms = cb.rec.totals_ms()
+        h2d, d2h = cb.h2d // args.steps, cb.d2h // args.steps
+        cb.rec.pairs = []
+    ceil = cb.ceilings() if rank == 0 else {}
+
+    # ---- max over ranks of every segment time ---------------------------------------------------------------------------
+    names = sorted(seg_ms)
+    vec = torch.tensor([seg_ms[k] for k in names] + [whole_ms] + ([e2e_ms.get(k, 0.0) for k in names] if e2e_ms else []),
+                       dtype=torch.float64, device=device)
+    if dist is not None:
+        dist.all_reduce(vec, op=dist.ReduceOp.MAX)
+    vec = vec.cpu().tolist()
+    seg_ms = dict(zip(names, vec[:len(names)]))
+    whole_ms = vec[len(names)]
+    if e2e_ms:
+        e2e_ms = dict(zip(names, vec[len(names) + 1:]))
+    if rank != 0:
+        if dist is not None:
+            dist.destroy_process_group()
+        return
+
+    K = args.steps
+    units = {k: table[k].get("bytes", table[k].get("ops")) * K * world for k in names}
+    secs = {k: seg_ms[k] * 1e-3 for k in names}
+    gbps, mops, copy_s, amo_s = class_rates(table, secs, units)
+    peak, peak_src = measured_peaks()
+    segments = {}
+    for k in names:
+        t, per_launch_ms = table[k], seg_ms[k] / (K * table[k]["launches"])
+        d = {"kernel": t["kernel"], "ms_per_step": seg_ms[k] / K, "launches_per_step": t["launches"]}
+        if t["cls"] == "copy":
+            d["GBps"] = units[k] / world / secs[k] / 1e9
+            d["frac_of_measured_hbm"] = d["GBps"] / peak
+            d["frac_of_nominal_8TBps"] = d["GBps"] / 8000.0
+        elif t["cls"] == "amo":
+            d["Mops"] = units[k] / world / secs[k] / 1e6
+        else:
+            d["us_per_barrier"] = seg_ms[k] / K / t["ops"] * 1e3
+        d["us_per_launch"] = per_launch_ms * 1e3
+        segments[k] = d
+    if "atomic_add" in segments and "red_add_512KiB_Mops" in ceil:
+        segments["atomic_add"]["frac_of_l2_atomic_ceiling"] = segments["atomic_add"]["Mops"] / ceil["red_add_512KiB_Mops"]
+    if "atomic_fetch_add" in segments and "atom_add_32MiB_Mops" in ceil:
+        segments["atomic_fetch_add"]["frac_of_l2_atomic_ceiling"] = segments["atomic_fetch_add"]["Mops"] / ceil["atom_add_32MiB_Mops"]
+    if "atomic_compare_swap" in segments and "atom_cas_32MiB_Mops" in ceil:
+        segments["atomic_compare_swap"]["frac_of_l2_atomic_ceiling"] = segments["atomic_compare_swap"]["Mops"] / ceil["atom_cas_32MiB_Mops"]
+
+    # dominant copy-class kernel = largest share of the timed copy-class step time
+    roofline = None
+    copy_names = [k for k in names if table[k]["cls"] == "copy"]
+    if copy_names:
+        by_kernel = {}
+        for k in copy_names:
+            e = by_kernel.setdefault(table[k]["kernel"], [0.0, 0, 0])
+            e[0] += secs[k]; e[1] += units[k] // world; e[2] += table[k]["launches"] * K
+        kern = max(by_kernel, key=lambda x: by_kernel[x][0])
+        s, b, nl = by_kernel[kern]
+        roofline = {"bound": "hbm", "kernel": kern, "achieved": b / s / 1e9, "peak": peak, "unit": "GB/s",
+                    "frac": b / s / 1e9 / peak, "peak_source": peak_src, "share_of_copy_time": s / copy_s,
+                    "algorithmic_bytes_per_launch": b // nl, "avg_launch_us": s / nl * 1e6,
+                    "traffic": NCU_TRAFFIC.get(kern)}
+
+    line = base_line(args, world)
+    line.update({"value": gbps, "amo_mops": mops, "ms_per_step": whole_ms / K,
+                 "timed_ms_per_step": sum(seg_ms.values()) / K, "dtype": "u8 (copies), u64 (AMOs), f64-accumulated f32 / i64 (sum_reduce)",
+                 "segments": segments, "ceilings": ceil, "roofline": roofline, "clocks": clocks, "gpu_launches": launches,
+                 "input_generation_s": inp.gen_seconds})
+    if e2e_ms:
+        eu = {k: units[k] for k in names if k in e2e_ms and table[k]["cls"] != "sync"}
+        es = {k: e2e_ms[k] * 1e-3 for k in eu}
+        eg, em, _, _ = class_rates(table, es, eu)
+        line["e2e"] = {"value": eg, "unit": UNIT, "amo_mops": em, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
+                       "ms_per_step": sum(es.values()) / K * 1e3,
+                       "note": "inputs from pinned host memory and results back to the host inside every segment"}
+    if world == 1 and not args.no_cpu:
+        ob = OracleBench(inp)
+        res = ob.step()
+        osecs = {k: v[0] for k, v in res.items()}
+        ounits = {k: v[1] for k, v in res.items()}
+        og, om, ocs, oas = class_rates(table, osecs, ounits)
+        line["cpu_baseline"] = {"value": og, "unit": UNIT, "amo_mops": om, "cores": 1, "kind": "oracle",
+                                "sample": "; ".join(ob.sample), "seconds": sum(osecs.values()),
+                                "host_cores_available": os.cpu_count()}
+    print(json.dumps(line))
+    if dist is not None:
+        dist.destroy_process_group()
+
+
+def main():
+    args = parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_cuda(args)
+
+
+if __name__ == "__main__":
+    main()

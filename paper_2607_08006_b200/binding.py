@@ -1,4 +1,4 @@
-"""ctypes binding of include/shmemg.h and include/shmemg_app.h (same names, marshalling only)."""
+"""ctypes binding of include/shmemg.h, include/shmemg_app.h and include/shmemg_probe.h (same names, marshalling only)."""
 from __future__ import annotations
 
 import ctypes as C
@@ -115,6 +115,8 @@ SYMBOLS = {
     "shmemg_app_halo_perturb_on_stream": (_i, [_vp, _u64, _u32, _u64, _u64, _vp]),
     "shmemg_app_halo_pack_on_stream": (_i, [_vp, _u64, _u64, _u32, _vp]),
     "shmemg_app_checksum64_on_stream": (_i, [_vp, _vp, _u64, _u64, _u32, _vp]),
+    "shmemg_probe_atomic_on_stream": (_i, [_vp, _i, _u64, _u64, _sz, _vp]),
+    "shmemg_probe_copy_all_on_stream": (_i, [_vp, _u64, _u64, _sz, _vp]),
 }
 
 _lib = None
@@ -352,6 +354,15 @@ class World:
 
     def barrier_epoch(self, stream=None) -> int:
         return lib().shmemg_barrier_epoch(self.h, _stream(stream))
+
+    # ---- ceiling probes (include/shmemg_probe.h; measurement utilities, not library ops) ------------------------------
+    def probe_atomic(self, mode, sym_off, words_per_pe, n, stream=None):
+        self._chk(lib().shmemg_probe_atomic_on_stream(self.h, mode, sym_off, words_per_pe, n, _stream(stream)),
+                  "shmemg_probe_atomic_on_stream")
+
+    def probe_copy_all(self, dst_off, src_off, nbytes, stream=None):
+        self._chk(lib().shmemg_probe_copy_all_on_stream(self.h, dst_off, src_off, nbytes, _stream(stream)),
+                  "shmemg_probe_copy_all_on_stream")
 
     # ---- halo application kernels (include/shmemg_app.h; not library ops) ---------------------------------------------
     def app_halo_perturb(self, U_off, B, seed, rnd, stream=None):

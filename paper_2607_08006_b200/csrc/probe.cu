@@ -1,0 +1,85 @@
+// probe.cu -- ceiling probes (include/shmemg_probe.h): bare L2 atomics at hashed addresses and a plain
+// per-PE local copy.  Measurement utilities for bench.py; not operations of the specification.
+#include "internal.cuh"
+#include "../../include/shmemg_probe.h"
+
+__device__ __forceinline__ unsigned long long probe_hash(unsigned long long i) {
+    unsigned long long x = i * 0x9E3779B97F4A7C15ull + 0x632BE59BD9B4E019ull;
+    x ^= x >> 29; x *= 0xBF58476D1CE4E5B9ull;
+    x ^= x >> 32;
+    return x;
+}
+
+template <int MODE>
+__global__ void __launch_bounds__(256) k_probe_atomic(uint8_t *base, size_t stride, uint64_t sym_off, unsigned npes,
+                                                      unsigned long long words, size_t n, unsigned long long *sink) {
+    unsigned long long acc = 0;
+    const size_t T = (size_t)gridDim.x * blockDim.x;
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += T) {
+        const unsigned long long h = probe_hash(i);
+        const unsigned pe = (unsigned)(h % npes);
+        const unsigned long long wd = (h / npes) % words;
+        unsigned long long *p = reinterpret_cast<unsigned long long *>(base + (size_t)pe * stride + sym_off) + wd;
+        if (MODE == SHMEMG_PROBE_RED_ADD) {
+            asm volatile("red.relaxed.gpu.global.add.u64 [%0], %1;" ::"l"(p), "l"(0ull) : "memory");
+        } else if (MODE == SHMEMG_PROBE_ATOM_ADD) {
+            acc ^= atomicAdd(p, 0ull);
+        } else {
+            acc ^= atomicCAS(p, 0x5DEECE66D1234567ull ^ h, 0ull);   // compare value the word never holds
+        }
+    }
+    if (MODE != SHMEMG_PROBE_RED_ADD && acc == 0x0123456789ABCDEFull && n == (size_t)-1) *sink = acc;
+}
+
+__global__ void __launch_bounds__(SHMEMG_THREADS, 4)
+k_probe_copy_all(uint8_t *base, size_t stride, uint64_t dst_off, uint64_t src_off, size_t nbytes, unsigned npes,
+                 unsigned chunk, unsigned chunks_per_pe) {
+    const size_t nwork = (size_t)npes * chunks_per_pe;
+    for (size_t wk = blockIdx.x; wk < nwork; wk += gridDim.x) {
+        const unsigned p = (unsigned)(wk / chunks_per_pe), c = (unsigned)(wk % chunks_per_pe);
+        const size_t off = (size_t)c * chunk;
+        size_t m = nbytes - off;
+        if (m > chunk) m = chunk;
+        copy_coop<8>(base + (size_t)p * stride + dst_off + off, base + (size_t)p * stride + src_off + off, m, threadIdx.x,
+                     SHMEMG_THREADS);
+    }
+}
+
+extern "C" int shmemg_probe_atomic_on_stream(shmemg_world_t *w, int mode, uint64_t sym_off, uint64_t words_per_pe,
+                                             size_t n, void *stream) {
+    if (!w || mode < SHMEMG_PROBE_RED_ADD || mode > SHMEMG_PROBE_ATOM_CAS || words_per_pe == 0) return SHMEMG_ERR_ARG;
+    if (sym_off & 7) return SHMEMG_ERR_ALIGN;
+    if (words_per_pe > (w->heap_bytes >> 3) || !shmemg_in_range(w, sym_off, words_per_pe * 8)) return SHMEMG_ERR_RANGE;
+    if (n == 0) return SHMEMG_OK;
+    size_t blocks = (n + 255) / 256;
+    const size_t cap = (size_t)w->sm_count * 8 * 4;
+    if (blocks > cap) blocks = cap;
+    unsigned long long *sink = reinterpret_cast<unsigned long long *>(&w->ctl->pad[0]);
+    cudaStream_t st = (cudaStream_t)stream;
+    if (mode == SHMEMG_PROBE_RED_ADD)
+        k_probe_atomic<SHMEMG_PROBE_RED_ADD><<<(unsigned)blocks, 256, 0, st>>>(w->base, w->stride, sym_off, (unsigned)w->npes, words_per_pe, n, sink);
+    else if (mode == SHMEMG_PROBE_ATOM_ADD)
+        k_probe_atomic<SHMEMG_PROBE_ATOM_ADD><<<(unsigned)blocks, 256, 0, st>>>(w->base, w->stride, sym_off, (unsigned)w->npes, words_per_pe, n, sink);
+    else
+        k_probe_atomic<SHMEMG_PROBE_ATOM_CAS><<<(unsigned)blocks, 256, 0, st>>>(w->base, w->stride, sym_off, (unsigned)w->npes, words_per_pe, n, sink);
+    SHMEMG_CUDA(w, cudaGetLastError());
+    return SHMEMG_OK;
+}
+
+extern "C" int shmemg_probe_copy_all_on_stream(shmemg_world_t *w, uint64_t dst_off, uint64_t src_off, size_t nbytes,
+                                               void *stream) {
+    if (!w) return SHMEMG_ERR_ARG;
+    if (!shmemg_in_range(w, dst_off, nbytes) || !shmemg_in_range(w, src_off, nbytes)) return SHMEMG_ERR_RANGE;
+    if (nbytes == 0) return SHMEMG_OK;
+    if (dst_off < src_off + nbytes && src_off < dst_off + nbytes) return SHMEMG_ERR_OVERLAP;
+    const uint64_t maxgrid = (uint64_t)w->sm_count * w->ctas_per_sm;
+    unsigned chunk = 65536;
+    if (w->tile_bytes_override) chunk = (unsigned)w->tile_bytes_override;
+    const unsigned cpp = (unsigned)((nbytes + chunk - 1) / chunk);
+    const uint64_t nwork = (uint64_t)w->npes * cpp;
+    const unsigned grid = (unsigned)(nwork < maxgrid ? nwork : maxgrid);
+    k_probe_copy_all<<<grid, SHMEMG_THREADS, 0, (cudaStream_t)stream>>>(w->base, w->stride, dst_off, src_off, nbytes,
+                                                                        (unsigned)w->npes, chunk, cpp);
+    SHMEMG_CUDA(w, cudaGetLastError());
+    return SHMEMG_OK;
+}
