@@ -473,10 +473,11 @@ class CudaBench:
 # oracle arm: the CPU oracle as it stands (single thread), on a bounded sample of the same step
 # ======================================================================================================================
 class OracleBench:
-    """Bounded sample of one step: C3a and C3b whole; C2 `halo_rounds` exchange rounds; C5 sum_reduce on the first
+    """Bounded sample of one step (defaults: the whole step except the barrier-latency loops and the halo application
+    compute, about 5-10 s on one core): C3a and C3b whole; C2 `halo_rounds` exchange rounds; C5 sum_reduce on the first
     1/`reduce_div` of the elements (all PEs), fcollect whole; C1 whole; C4 the first 2^`c4_log2` edges."""
 
-    def __init__(self, inp: Inputs, halo_rounds=5, reduce_div=4, c4_log2=24):
+    def __init__(self, inp: Inputs, halo_rounds=HALO_ROUNDS, reduce_div=1, c4_log2=26):
         from oracle import oracle as orc
         self.orc, self.inp = orc, inp
         g = inp.groups
