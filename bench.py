@@ -154,7 +154,7 @@ def segment_table(inp: Inputs):
     g = inp.groups
     if "c3a" in g:
         n, b = inp.c3a_npes, inp.c3a_blk
-        seg["alltoall"] = dict(cls="copy", kernel="k_alltoall", bytes=2 * n * n * b, launches=1)
+        seg["alltoall"] = dict(cls="copy", kernel="k_alltoall_tma", bytes=2 * n * n * b, launches=1)
     if "c3b" in g:
         seg["put_batch_skewed"] = dict(cls="copy", kernel="k_batch_exec", bytes=2 * int(inp.c3b.sizes.sum()), launches=1)
     if "c2" in g:
@@ -164,7 +164,7 @@ def segment_table(inp: Inputs):
         n, nb = inp.c5_npes, inp.c5_bytes
         seg["sum_reduce_f32"] = dict(cls="copy", kernel="k_sum_reduce_f32", bytes=2 * n * nb, launches=1)
         seg["sum_reduce_i64"] = dict(cls="copy", kernel="k_sum_reduce_i64", bytes=2 * n * nb, launches=1)
-        seg["fcollect"] = dict(cls="copy", kernel="k_fcollect_vec",
+        seg["fcollect"] = dict(cls="copy", kernel="k_fcollect_tma",
                                bytes=n * inp.c5_fc_bytes + n * n * inp.c5_fc_bytes, launches=1)
     if "c1" in g:
         seg["atomic_add"] = dict(cls="amo", kernel="k_amo<add>", ops=len(inp.c1.val), launches=2)   # + barrier kernel
@@ -286,7 +286,25 @@ class CudaBench:
 
     # ---- one pass of the whole hot path; device-resident inputs ------------------------------------------------------
     def step(self):
+        """Order: the millisecond-long AMO kernels first, so the host runs ahead of the device and every later segment
+        measures device time with its launch already queued (the events bracket the kernel, not host launch latency)."""
         torch, inp, rec, g = self.torch, self.inp, self.rec, self.inp.groups
+        if "c4" in g:
+            vpp = inp.c4.verts_per_pe
+            self.w4.view(self.deg, vpp * 8).zero_()
+            self.w4.view(self.par, vpp * 8).fill_(255)
+            with rec.seg("atomic_fetch_add"):
+                self.w4.atomic_fetch_add_batch(self.deg, self.c4_ou, self.c4_lu, self.f_deg, val=None, val_scalar=1,
+                                               flags=self.flags)
+            with rec.seg("atomic_compare_swap"):
+                self.w4.atomic_compare_swap_batch(self.par, self.c4_ov, self.c4_lv, self.f_par, cond=None, cond_scalar=M64,
+                                                  val=self.c4_val, flags=self.flags)
+        if "c1" in g:
+            self.w1.view(self.A, inp.c1.nelem * 8).zero_()
+            with rec.seg("atomic_add"):
+                self.w1.atomic_add_batch(self.A, self.c1_t, self.c1_i, val=self.c1_v, flags=self.flags)
+                self.w1.quiet_on_stream(0)
+                self.w1.barrier_all()
         if "c3a" in g:
             with rec.seg("alltoall"):
                 self.w3a.alltoall(self.a_dst, self.a_src, inp.c3a_blk)
@@ -312,22 +330,6 @@ class CudaBench:
                 self.app_launches += 2
                 with rec.seg("halo_put_signal_wait"):
                     w.enqueue_batch(self.halo_batches[r - 1])
-        if "c1" in g:
-            self.w1.view(self.A, inp.c1.nelem * 8).zero_()
-            with rec.seg("atomic_add"):
-                self.w1.atomic_add_batch(self.A, self.c1_t, self.c1_i, val=self.c1_v, flags=self.flags)
-                self.w1.quiet_on_stream(0)
-                self.w1.barrier_all()
-        if "c4" in g:
-            vpp = inp.c4.verts_per_pe
-            self.w4.view(self.deg, vpp * 8).zero_()
-            self.w4.view(self.par, vpp * 8).fill_(255)
-            with rec.seg("atomic_fetch_add"):
-                self.w4.atomic_fetch_add_batch(self.deg, self.c4_ou, self.c4_lu, self.f_deg, val=None, val_scalar=1,
-                                               flags=self.flags)
-            with rec.seg("atomic_compare_swap"):
-                self.w4.atomic_compare_swap_batch(self.par, self.c4_ov, self.c4_lv, self.f_par, cond=None, cond_scalar=M64,
-                                                  val=self.c4_val, flags=self.flags)
         if "barrier" in g:
             with rec.seg("barrier_in_kernel"):
                 self.w5.barrier_all_repeat(BARRIERS)

@@ -1,171 +1,361 @@
-// batch.cu -- op-batch planner (host) and the persistent-grid batch executor kernel (sm_100a),
-// plus the single put/get/put_signal/wait `_on_stream` calls.  SURVEY.md 8(a) rows a5-a8, a12-a14.
+// batch.cu -- op-batch planner (host) and the persistent batch executor kernel (sm_100a), plus the single
+// put/get/put_signal/wait `_on_stream` calls.  SURVEY.md 8(a) rows a5-a8, a12-a14.
 //
 // Executor design:
-//   * the host planner resolves PE->address translation, cuts copy ops into tiles and groups consecutive
-//     AMO descriptors into runs; tiles are listed in batch order;
-//   * a persistent grid claims tiles with one global ticket IN BATCH ORDER, so a claimed tile only ever
-//     waits for tiles with smaller tickets, which are finished or held by running CTAs: no deadlock and no
-//     co-residency requirement;
-//   * ordering state: done[p] = completed ops of PE p, done[npes] = completed ops of all PEs (monotonic,
-//     release-incremented).  An op that follows a FENCE/QUIET/WAIT of its PE starts only when done[p] has
-//     reached the number of that PE's ops before the marker; an op after a BARRIER_ALL starts only when
-//     done[npes] has reached the number of ops before the barrier (acquire spin by one thread + bar.sync);
-//   * a multi-tile op completes at its last-arriving tile (fence + relaxed counter), which then performs
-//     the put_signal update with release semantics and the done[] increments.
+//   * the host planner resolves PE->address translation and cuts every op into self-contained 64-byte TILE RECORDS
+//     listed in batch order: bulk-copy tiles (<= 32 KiB, 16-byte aligned), register-path copy tiles (unaligned heads,
+//     tails and relatively misaligned transfers), runs of <= 128 AMO descriptors, waits, and no-data tiles;
+//   * one CTA per SM, warp-specialised:
+//       loader  (1 thread)  claims tiles with a global ticket IN BATCH ORDER, waits for the tile's dependencies,
+//                           issues the bulk load (cp.async.bulk global->shared) or hands the tile to the generic
+//                           warps; waits (SIGNAL_WAIT_UNTIL) are polled here;
+//       storer  (1 thread)  issues the bulk store (shared->global) when a stage has landed, and when the store has
+//                           completed does the tile's completion accounting (arrival, signal, done counters);
+//       generic (4 warps)   register-path copies and AMO runs.
+//     A claimed tile only ever waits for tiles with smaller tickets, which are finished or held by running CTAs whose
+//     three roles make progress independently: no deadlock and no co-residency requirement;
+//   * ordering state: done[p] = completed ops of PE p, done[npes] = completed ops of all PEs (monotonic, release-
+//     incremented).  An op that follows a FENCE/QUIET/WAIT of its PE starts only when done[p] has reached the number
+//     of that PE's ops before the marker; an op after a BARRIER_ALL only when done[npes] has reached the number of
+//     ops before the barrier (acquire spin).  Only ops that some later op depends on are counted;
+//   * the unit of claiming and of completion accounting is the SEGMENT: up to SEG_TILES_MAX consecutive bulk tiles of
+//     one op, streamed through one CTA's stage ring; release fences cost microseconds under load, so there is one per
+//     segment, not per tile.  An op cut into several pieces completes at its last-ARRIVING piece (acq_rel counter on
+//     arrive[op]), which performs the put_signal update with release semantics and the done[] increments.  Ops nobody
+//     depends on and that carry no signal do no accounting at all.
 #include <stdlib.h>
 #include <string.h>
 
 #include <vector>
 
-#include "internal.cuh"
+#include "tma_stream.cuh"
 
-#define AMO_RUN_MAX SHMEMG_THREADS
-#define OPF_COUNT_PE 0x10000u    // a later marker of this PE depends on this op: bump done[initiator]
-#define OPF_COUNT_ALL 0x20000u   // a later BARRIER_ALL depends on this op: bump done[npes]
+#define EXEC_THREADS 192          // warp 0: loader, warp 1: storer, warps 2-5: generic
+#define GEN_THREADS 128
+#define GEN_FIRST 64
+#define GEN_SLOTS 2
+#define GEN_TILE 16384u           // bytes per register-path copy tile
+#define AMO_RUN_MAX GEN_THREADS
+#define TMA_MIN_SPLIT 2048u       // below this, a transfer with unaligned ends is one register-path tile
+#define SEG_TILES_MAX 8u          // bulk tiles per segment (256 KiB)
+#define TRACE_SLOTS 8
+#define TRACE_CTAS 256
+#define TRACE_BYTES (TRACE_CTAS * TRACE_SLOTS * 8)   // per-CTA timestamps (SHMEMG_TRACE=1)
+#define WAIT_RUN_MAX 64u          // consecutive waits of one PE polled by one thread
 
-struct DevOp {            // 64 B, resolved on the host
-    uint64_t dst;         // copy destination / AMO target word
-    uint64_t src;         // copy source / AMO fetch slot (0 = none)
-    uint64_t nbytes;
-    uint64_t sig;         // put_signal: signal word on the target; wait: the local word
-    uint64_t value;
-    uint64_t cond;
-    uint32_t kind;        // bits 0-7 opcode, 8-15 sig_op or cmp, 16+ OPF_*
+// tile kinds (bits 0-7 of TileRec.kind); bits 8-15 hold sig_op (put_signal)
+enum { T_TMA = 1, T_COPY = 2, T_AMO = 3, T_WAIT = 4, T_NODATA = 5, T_END = 6 };
+#define TF_SEGEND 0x00010000u     // (ring only) last bulk tile of its segment: account when its store has completed
+#define TF_SIGNAL 0x00020000u     // op is a PUT_SIGNAL
+#define TF_CNT_PE 0x00040000u     // a later marker of this PE depends on this op: bump done[initiator]
+#define TF_CNT_ALL 0x00080000u    // a later BARRIER_ALL depends on this op: bump done[npes]
+#define TF_DEPS 0x00100000u       // dep_pe / dep_all are non-zero
+#define TF_ACCT (TF_SIGNAL | TF_CNT_PE | TF_CNT_ALL)
+
+struct TileRec {          // 64 B, self-contained
+    uint64_t dst;         // copy destination
+    uint64_t src;         // copy source; AMO run / wait run: address of the first AuxRec
+    uint64_t sig;         // put_signal: signal word on the target
+    uint64_t value;       // signal value
+    uint32_t nbytes;      // bytes of this piece (a segment spans several bulk tiles); AMO / wait run: number of records
+    uint32_t kind;
+    uint32_t op;          // unit index (arrive[op])
+    uint32_t nt;          // pieces of this op (arrive[op] advances by nt per launch)
     uint32_t initiator;
-    uint32_t dep_pe;      // start when done[initiator] >= dep_pe
-    uint32_t dep_all;     // and done[npes] >= dep_all
+    uint32_t dep_pe;      // start when done[initiator] has advanced by dep_pe in this launch
+    uint32_t dep_all;     // and done[npes] by dep_all
+    uint32_t pe_total;    // how far done[initiator] advances per launch (base of this launch = epoch * pe_total)
 };
-static_assert(sizeof(DevOp) == 64, "DevOp must be 64 bytes");
+static_assert(sizeof(TileRec) == 64, "TileRec must be 64 bytes");
 
-struct Tile { uint32_t op; uint32_t sub; };   // copy/wait: sub = tile index within op; AMO run: sub = count
+struct AuxRec {           // 64 B: one AMO descriptor or one wait condition, resolved on the host
+    uint64_t word;        // AMO target word / signal word to poll
+    uint64_t fetch;       // AMO fetch slot (0 = none)
+    uint64_t value;       // AMO operand / wait comparand
+    uint64_t cond;
+    uint32_t kind;        // bits 0-7 opcode, bits 8-15 cmp (wait), TF_CNT_*
+    uint32_t initiator;
+    uint32_t dep_pe;
+    uint32_t dep_all;
+    uint32_t pe_total;
+    uint32_t pad[3];
+};
+static_assert(sizeof(AuxRec) == 64, "AuxRec must be 64 bytes");
 
+// All run-time counters are MONOTONIC across launches, so a plan needs no re-arming and no exit protocol: one launch
+// performs exactly `ntiles` ticket claims, advances done[p] by pe_total[p], done[npes] by all_total and arrive[op] by
+// nt; the launch index (epoch) is ticket / ntiles at kernel entry and every threshold is taken relative to it
+// (wrap-safe 32-bit differences).
 struct PlanHeader {       // 256 B at the start of the plan buffer
-    uint32_t ntiles, nops, npes, tile_bytes;
-    uint32_t ticket, exited, pad0, pad1;
-    uint64_t ops_off, tiles_off, done_off, arrive_off;
-    uint64_t pad2[24];
+    uint32_t ntiles, nunits, npes, trace_on;
+    unsigned long long ticket;
+    uint32_t all_total, pad1;
+    uint64_t tiles_off, aux_off, done_off, arrive_off, trace_off;
+    uint64_t pad3[23];
 };
 static_assert(sizeof(PlanHeader) == 256, "PlanHeader must be 256 bytes");
 
+struct ExecArgs;
 struct shmemg_batch {
     shmemg_world *w;
     uint8_t *plan_dev;
     uint32_t ntiles;
     uint32_t grid;
+    uint32_t npes, all_total;
+    size_t tiles_off, done_off, arrive_off, trace_off;
+    bool trace_on;
 };
 
 // ---------------------------------------------------------------------------------------------------------
 // device
 // ---------------------------------------------------------------------------------------------------------
-__device__ __forceinline__ void wait_deps(const unsigned *done, unsigned npes, unsigned initiator, unsigned dep_pe,
-                                          unsigned dep_all) {
-    if (dep_pe) while (ld_acquire_u32(done + initiator) < dep_pe) __nanosleep(32);
-    if (dep_all) while (ld_acquire_u32(done + npes) < dep_all) __nanosleep(32);
+struct Epoch { unsigned e, all_total, npes; };    // e = launch index mod 2^32
+
+__device__ __forceinline__ void wait_deps(const unsigned *done, const Epoch &ep, unsigned initiator, unsigned dep_pe,
+                                          unsigned dep_all, unsigned pe_total) {
+    if (dep_pe) while (ld_relaxed_u32(done + initiator) - ep.e * pe_total < dep_pe) __nanosleep(20);
+    if (dep_all) while (ld_relaxed_u32(done + ep.npes) - ep.e * ep.all_total < dep_all) __nanosleep(20);
+    if (dep_pe | dep_all) fence_acquire();
 }
 
 __device__ __forceinline__ void count_done(unsigned *done, unsigned npes, unsigned kind, unsigned initiator) {
-    if (kind & OPF_COUNT_PE) red_release_add_u32(done + initiator, 1u);
-    if (kind & OPF_COUNT_ALL) red_release_add_u32(done + npes, 1u);
+    if (kind & TF_CNT_PE) red_release_add_u32(done + initiator, 1u);
+    if (kind & TF_CNT_ALL) red_release_add_u32(done + npes, 1u);
 }
 
-__device__ __forceinline__ void amo_one(const DevOp &o) {
-    unsigned long long *word = reinterpret_cast<unsigned long long *>(o.dst);
+// Completion accounting of one piece whose own writes are complete and visible to the calling thread.
+__device__ __forceinline__ void account(const TileRec &r, unsigned *done, unsigned *arrive, const Epoch &ep) {
+    if (!(r.kind & TF_ACCT)) return;
+    if (r.nt > 1) {
+        unsigned old;   // release: this piece's writes; acquire: the pieces that arrived earlier
+        asm volatile("atom.acq_rel.gpu.global.add.u32 %0, [%1], 1;" : "=r"(old) : "l"(arrive + r.op) : "memory");
+        if (old - ep.e * r.nt != r.nt - 1) return;                  // not the last piece of this launch to arrive
+    }
+    if (r.kind & TF_SIGNAL) signal_update(reinterpret_cast<unsigned long long *>(r.sig), r.value, (r.kind >> 8) & 0xff);
+    count_done(done, ep.npes, r.kind, r.initiator);
+}
+
+__device__ __forceinline__ void amo_one(const AuxRec &o) {
+    unsigned long long *word = reinterpret_cast<unsigned long long *>(o.word);
     const unsigned opc = o.kind & 0xffu;
     if (opc == SHMEMG_OP_ATOMIC_ADD) {
         asm volatile("red.relaxed.gpu.global.add.u64 [%0], %1;" ::"l"(word), "l"(o.value) : "memory");
     } else if (opc == SHMEMG_OP_ATOMIC_FETCH_ADD) {
         unsigned long long old = atomicAdd(word, (unsigned long long)o.value);
-        *reinterpret_cast<volatile unsigned long long *>(o.src) = old;
+        *reinterpret_cast<volatile unsigned long long *>(o.fetch) = old;
     } else {
         unsigned long long old = atomicCAS(word, (unsigned long long)o.cond, (unsigned long long)o.value);
-        *reinterpret_cast<volatile unsigned long long *>(o.src) = old;
+        *reinterpret_cast<volatile unsigned long long *>(o.fetch) = old;
     }
 }
 
-__global__ void __launch_bounds__(SHMEMG_THREADS, 4) k_batch_exec(uint8_t *plan) {
-    PlanHeader *hdr = reinterpret_cast<PlanHeader *>(plan);
-    const DevOp *__restrict__ ops = reinterpret_cast<const DevOp *>(plan + hdr->ops_off);
-    const Tile *__restrict__ tiles = reinterpret_cast<const Tile *>(plan + hdr->tiles_off);
-    unsigned *done = reinterpret_cast<unsigned *>(plan + hdr->done_off);
-    unsigned *arrive = reinterpret_cast<unsigned *>(plan + hdr->arrive_off);
-    const unsigned ntiles = hdr->ntiles, npes = hdr->npes, tile_bytes = hdr->tile_bytes;
+template <typename T> __device__ __forceinline__ T ld_rec(const T *p) {     // 64-byte immutable plan record
+    static_assert(sizeof(T) == 64, "64-byte records");
+    T r;
+    const int4 *s = reinterpret_cast<const int4 *>(p);
+    int4 *d = reinterpret_cast<int4 *>(&r);
+    d[0] = __ldg(s); d[1] = __ldg(s + 1); d[2] = __ldg(s + 2); d[3] = __ldg(s + 3);
+    return r;
+}
+
+// SHMEMG_TRACE=1 at batch creation: every CTA stamps %globaltimer at its role milestones into the plan's trace region
+__device__ __forceinline__ unsigned long long gtime() {
+    unsigned long long t;
+    asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t));
+    return t;
+}
+#define TRACE(slot) do { if (trace) trace[blockIdx.x * TRACE_SLOTS + (slot)] = gtime(); } while (0)
+
+// Everything a CTA needs to start is a kernel ARGUMENT (constant bank); the only global reads on the start-up path are
+// the first tile record and the ticket counter, issued together.
+struct ExecArgs {
+    const TileRec *tiles;
+    unsigned long long *ticket;
+    unsigned *done, *arrive;
+    unsigned long long *trace;     // nullptr unless SHMEMG_TRACE
+    unsigned ntiles, npes, all_total;
+};
+
+__global__ void __launch_bounds__(EXEC_THREADS, 1) k_batch_exec(const ExecArgs a) {
+    extern __shared__ __align__(1024) uint8_t stage[];
+    __shared__ __align__(16) TileRec ringA[SHMEMG_TMA_STAGES];
+    __shared__ __align__(16) TileRec ringG[GEN_SLOTS];
+    __shared__ uint64_t fullA[SHMEMG_TMA_STAGES], emptyA[SHMEMG_TMA_STAGES], fullG[GEN_SLOTS], emptyG[GEN_SLOTS];
+    __shared__ unsigned s_epoch;
+
+    const TileRec *tiles = a.tiles;
+    unsigned *done = a.done, *arrive = a.arrive;
+    const unsigned ntiles = a.ntiles;
     const int tid = threadIdx.x;
-    __shared__ unsigned s_ticket;
-    __shared__ unsigned s_last;
+    unsigned long long *trace = blockIdx.x < TRACE_CTAS ? a.trace : nullptr;
+    Epoch ep;
+    ep.e = 0; ep.all_total = a.all_total; ep.npes = a.npes;
 
-    if (tid == 0) s_ticket = atomicAdd(&hdr->ticket, 1u);
-    __syncthreads();
-    unsigned t = s_ticket;
-    while (t < ntiles) {
-        unsigned next = 0;
-        if (tid == 0) next = atomicAdd(&hdr->ticket, 1u);     // claim ahead: hides the L2 round trip
-        const Tile tl = tiles[t];
-        const unsigned kind0 = ops[tl.op].kind;
-        const unsigned opc = kind0 & 0xffu;
-        if (opc <= SHMEMG_OP_PUT_SIGNAL) {
-            // ---- copy tile -------------------------------------------------------------------------------
-            const DevOp o = ops[tl.op];
-            if (o.dep_pe | o.dep_all) {
-                if (tid == 0) wait_deps(done, npes, o.initiator, o.dep_pe, o.dep_all);
-                __syncthreads();
-            }
-            const uint64_t off = (uint64_t)tl.sub * tile_bytes;
-            uint64_t n = o.nbytes - off;
-            if (n > tile_bytes) n = tile_bytes;
-            copy_coop<8>(reinterpret_cast<uint8_t *>(o.dst + off), reinterpret_cast<const uint8_t *>(o.src + off), n,
-                         tid, SHMEMG_THREADS);
-            __syncthreads();                                   // every thread's stores precede thread 0's release
-            if (tid == 0) {
-                const unsigned nt = o.nbytes <= tile_bytes ? 1u : (unsigned)((o.nbytes + tile_bytes - 1) / tile_bytes);
-                bool last = true;
-                if (nt > 1) {
-                    __threadfence();
-                    last = (atomicAdd(arrive + tl.op, 1u) == nt - 1);
-                    if (last) __threadfence();
-                }
-                if (last) {
-                    if (opc == SHMEMG_OP_PUT_SIGNAL)
-                        signal_update(reinterpret_cast<unsigned long long *>(o.sig), o.value, (o.kind >> 8) & 0xff);
-                    count_done(done, npes, o.kind, o.initiator);
-                }
-                s_ticket = next;
-            }
-        } else if (opc == SHMEMG_OP_SIGNAL_WAIT_UNTIL) {
-            if (tid == 0) {
-                const DevOp o = ops[tl.op];
-                wait_deps(done, npes, o.initiator, o.dep_pe, o.dep_all);
-                const unsigned long long *sig = reinterpret_cast<const unsigned long long *>(o.sig);
-                const int cmp = (o.kind >> 8) & 0xff;
-                while (!cmp_u64(cmp, ld_acquire_u64(sig), o.value)) __nanosleep(64);
-                count_done(done, npes, o.kind, o.initiator);
-                s_ticket = next;
-            }
-        } else {
-            // ---- run of AMO descriptors: one thread per op ---------------------------------------------
-            if (tid < (int)tl.sub) {
-                const DevOp o = ops[tl.op + tid];
-                wait_deps(done, npes, o.initiator, o.dep_pe, o.dep_all);
-                amo_one(o);
-                count_done(done, npes, o.kind, o.initiator);
-            }
-            if (tid == 0) s_ticket = next;
-        }
-        __syncthreads();
-        t = s_ticket;
-        __syncthreads();                                       // nobody overwrites s_ticket before all have read it
+    if (tid == 0) {
+        TRACE(0);
+        for (int s = 0; s < SHMEMG_TMA_STAGES; ++s) { mbar_init(&fullA[s], 1); mbar_init(&emptyA[s], 1); }
+        for (int g = 0; g < GEN_SLOTS; ++g) { mbar_init(&fullG[g], 1); mbar_init(&emptyG[g], 1); }
+        mbar_init_fence();
     }
-    // last CTA out re-arms the plan so the batch can be enqueued again
-    if (tid == 0) s_last = (atomicAdd(&hdr->exited, 1u) == gridDim.x - 1);
     __syncthreads();
-    if (s_last) {
-        for (unsigned i = tid; i <= npes; i += SHMEMG_THREADS) done[i] = 0;
-        for (unsigned i = tid; i < hdr->nops; i += SHMEMG_THREADS) arrive[i] = 0;
-        if (tid == 0) { hdr->ticket = 0; hdr->exited = 0; }
+
+    if (tid == 0) {
+        // ---- loader -------------------------------------------------------------------------------------------
+        // The first ticket of CTA b is b (no atomic on the critical path, and the first wave is spread over all CTAs);
+        // later tickets are claimed one ahead, while the current piece is processed.
+        // Launch index: this launch's claims keep the counter inside [epoch*ntiles, (epoch+1)*ntiles) until the last
+        // CTA's failing claim, and a CTA reads it before making its own.  The consumers pick s_epoch up after their
+        // first ring hand-off (mbarrier release/acquire).
+        TRACE(1);
+        TileRec r0 = {};
+        if (blockIdx.x < ntiles) r0 = ld_rec(tiles + blockIdx.x);
+        ep.e = (unsigned)(ld_relaxed_u64(a.ticket) / ntiles);
+        s_epoch = ep.e;
+        const unsigned long long tbase = (unsigned long long)ep.e * ntiles;   // exact: epoch < 2^32 launches
+        unsigned ia = 0, ig = 0;
+        unsigned long long t0 = blockIdx.x;
+        while (t0 < ntiles) {
+            const unsigned long long t1 = atomicAdd(a.ticket, 1ull) - tbase + gridDim.x;
+            const unsigned k = r0.kind & 0xffu;
+            if (r0.kind & TF_DEPS) {
+                wait_deps(done, ep, r0.initiator, r0.dep_pe, r0.dep_all, r0.pe_total);
+                proxy_fence();                                       // acquire (generic proxy) before bulk reads
+            }
+            if (k == T_TMA) {                                        // one segment: stream its bulk tiles
+                for (unsigned off = 0; off < r0.nbytes; off += SHMEMG_TMA_TILE, ++ia) {
+                    const unsigned s = ia % SHMEMG_TMA_STAGES;
+                    const unsigned n = r0.nbytes - off < SHMEMG_TMA_TILE ? r0.nbytes - off : SHMEMG_TMA_TILE;
+                    mbar_wait(&emptyA[s], ((ia / SHMEMG_TMA_STAGES) & 1u) ^ 1u);
+                    TileRec q = r0;
+                    q.dst = r0.dst + off; q.nbytes = n;
+                    if (off + n == r0.nbytes) q.kind |= TF_SEGEND;
+                    ringA[s] = q;
+                    mbar_arrive_expect_tx(&fullA[s], n);
+                    bulk_g2s(stage + (size_t)s * SHMEMG_TMA_TILE, reinterpret_cast<const void *>(r0.src + off), n, &fullA[s]);
+                }
+            } else if (k == T_COPY || k == T_AMO) {
+                const unsigned g = ig % GEN_SLOTS;
+                mbar_wait(&emptyG[g], ((ig / GEN_SLOTS) & 1u) ^ 1u);
+                ringG[g] = r0;
+                mbar_arrive(&fullG[g]);
+                ig++;
+            } else if (k == T_WAIT) {
+                // a run of consecutive waits of one PE, polled in program order by this one thread
+                const AuxRec *wr = reinterpret_cast<const AuxRec *>(r0.src);
+                for (unsigned i = 0; i < r0.nbytes; ++i) {
+                    const unsigned long long *sig = reinterpret_cast<const unsigned long long *>(__ldg(&wr[i].word));
+                    const unsigned long long v = __ldg(&wr[i].value);
+                    const int cmp = (int)((__ldg(&wr[i].kind) >> 8) & 0xff);
+                    while (!cmp_u64(cmp, ld_relaxed_u64(sig), v)) __nanosleep(40);
+                }
+                fence_acquire();
+                count_done(done, ep.npes, r0.kind, r0.initiator);
+            } else {                                                 // T_NODATA: zero-byte put/get/put_signal
+                account(r0, done, arrive, ep);
+            }
+            t0 = t1;
+            if (t0 < ntiles) r0 = ld_rec(tiles + t0);
+        }
+        TRACE(2);
+        {   // end markers for both consumers
+            const unsigned s = ia % SHMEMG_TMA_STAGES;
+            mbar_wait(&emptyA[s], ((ia / SHMEMG_TMA_STAGES) & 1u) ^ 1u);
+            ringA[s].kind = T_END;
+            mbar_arrive(&fullA[s]);
+            const unsigned g = ig % GEN_SLOTS;
+            mbar_wait(&emptyG[g], ((ig / GEN_SLOTS) & 1u) ^ 1u);
+            ringG[g].kind = T_END;
+            mbar_arrive(&fullG[g]);
+        }
+    } else if (tid == 32) {
+        // ---- storer -------------------------------------------------------------------------------------------
+        bool have_prev = false, pend_acct = false;     // previous tile's stage not yet freed / segment not yet accounted
+        TileRec acct = {};
+        unsigned prev_s = 0;
+        for (unsigned i = 0;; ++i) {
+            const unsigned s = i % SHMEMG_TMA_STAGES, ph = (i / SHMEMG_TMA_STAGES) & 1u;
+            if (!mbar_test_wait(&fullA[s], ph)) {
+                if (have_prev) {              // starved: nothing may stay unaccounted while this role blocks
+                    if (pend_acct) { bulk_wait<0>(); proxy_fence(); account(acct, done, arrive, ep); pend_acct = false; }
+                    else bulk_wait_read<0>();
+                    mbar_arrive(&emptyA[prev_s]);
+                    have_prev = false;
+                }
+                mbar_wait(&fullA[s], ph);
+            }
+            const TileRec r = ringA[s];
+            if ((r.kind & 0xffu) == T_END) break;
+            ep.e = s_epoch;
+            bulk_s2g(reinterpret_cast<void *>(r.dst), stage + (size_t)s * SHMEMG_TMA_TILE, r.nbytes);
+            bulk_commit();
+            if (have_prev) {
+                // every group but the one just committed: has completed (a segment ended) / has read its stage
+                if (pend_acct) { bulk_wait<1>(); proxy_fence(); account(acct, done, arrive, ep); pend_acct = false; }
+                else bulk_wait_read<1>();
+                mbar_arrive(&emptyA[prev_s]);
+            }
+            if ((r.kind & TF_SEGEND) && (r.kind & TF_ACCT)) { acct = r; pend_acct = true; }
+            prev_s = s; have_prev = true;
+        }
+        TRACE(3);
+        bulk_wait<0>();
+        if (pend_acct) { proxy_fence(); account(acct, done, arrive, ep); }
+        TRACE(4);
+    } else if (tid >= GEN_FIRST) {
+        // ---- generic warps: register-path copies and AMO runs ----------------------------------------------
+        const int gt = tid - GEN_FIRST;
+        for (unsigned j = 0;; ++j) {
+            const unsigned g = j % GEN_SLOTS;
+            mbar_wait(&fullG[g], (j / GEN_SLOTS) & 1u);
+            const TileRec r = ringG[g];
+            const unsigned k = r.kind & 0xffu;
+            if (k == T_END) break;
+            ep.e = s_epoch;
+            if (k == T_COPY) {
+                copy_coop<4>(reinterpret_cast<uint8_t *>(r.dst), reinterpret_cast<const uint8_t *>(r.src), r.nbytes, gt,
+                             GEN_THREADS);
+                if (r.kind & TF_ACCT) __threadfence();
+            } else if (gt < (int)r.nbytes) {
+                const AuxRec o = ld_rec(reinterpret_cast<const AuxRec *>(r.src) + gt);
+                wait_deps(done, ep, o.initiator, o.dep_pe, o.dep_all, o.pe_total);
+                amo_one(o);
+                count_done(done, ep.npes, o.kind, o.initiator);
+            }
+            named_bar_sync(1, GEN_THREADS);
+            if (gt == 0) {
+                if (k == T_COPY) account(r, done, arrive, ep);
+                mbar_arrive(&emptyG[g]);
+            }
+        }
     }
 }
 
-// single copy on a stream: grid-stride over tiles, optional last-arriver signal
+// ---- single copy on a stream ------------------------------------------------------------------------------------
+// bulk-copy path (16-byte aligned): one issuing thread per CTA; optional last-arriver signal
+__global__ void __launch_bounds__(32) k_copy_single_tma(uint8_t *dst, const uint8_t *src, size_t nbytes,
+                                                        unsigned long long *sig, unsigned long long sig_value, int sig_op,
+                                                        unsigned *counter) {
+    extern __shared__ __align__(1024) uint8_t stage[];
+    __shared__ uint64_t full[SHMEMG_TMA_STAGES];
+    if (threadIdx.x != 0) return;
+    tma_stream_init(full);
+    const size_t nitems = (nbytes + SHMEMG_TMA_TILE - 1) / SHMEMG_TMA_TILE;
+    tma_stream_copy(stage, full, blockIdx.x, gridDim.x, nitems, [&](size_t k, const uint8_t *&s, uint8_t *&d, unsigned &n) {
+        const size_t off = k * SHMEMG_TMA_TILE;
+        s = src + off; d = dst + off;
+        n = (unsigned)(nbytes - off < SHMEMG_TMA_TILE ? nbytes - off : SHMEMG_TMA_TILE);
+    });
+    if (sig) {
+        proxy_fence();
+        __threadfence();
+        if (atomicAdd(counter, 1u) == gridDim.x - 1) {
+            __threadfence();
+            *counter = 0;
+            signal_update(sig, sig_value, sig_op);
+        }
+    }
+}
+// register path (any alignment): grid-stride over tiles, optional last-arriver signal
 __global__ void __launch_bounds__(SHMEMG_THREADS, 4)
 k_copy_single(uint8_t *dst, const uint8_t *src, size_t nbytes, unsigned tile_bytes, unsigned long long *sig,
               unsigned long long sig_value, int sig_op, unsigned *counter) {
@@ -190,7 +380,8 @@ k_copy_single(uint8_t *dst, const uint8_t *src, size_t nbytes, unsigned tile_byt
 }
 
 __global__ void k_wait_until(const unsigned long long *sig, int cmp, unsigned long long value) {
-    while (!cmp_u64(cmp, ld_acquire_u64(sig), value)) __nanosleep(100);
+    while (!cmp_u64(cmp, ld_relaxed_u64(sig), value)) __nanosleep(100);
+    fence_acquire();
 }
 
 // ---------------------------------------------------------------------------------------------------------
@@ -236,49 +427,109 @@ static bool is_marker(uint8_t opc) {
 }
 static bool is_amo(uint8_t opc) { return opc >= SHMEMG_OP_ATOMIC_ADD && opc <= SHMEMG_OP_ATOMIC_COMPARE_SWAP; }
 
-static uint32_t pick_tile_bytes(const shmemg_world *w, const shmemg_op_t *ops, size_t nops) {
-    if (w->tile_bytes_override) return (uint32_t)w->tile_bytes_override;
-    uint64_t total = 0;
-    for (size_t i = 0; i < nops; ++i)
-        if (ops[i].opcode >= SHMEMG_OP_PUT && ops[i].opcode <= SHMEMG_OP_PUT_SIGNAL) total += ops[i].nbytes;
-    const uint64_t grid = (uint64_t)w->sm_count * w->ctas_per_sm;
-    uint64_t want = total / (grid * 8) + 1;            // aim at >= 8 tiles per resident CTA
-    uint32_t tb = 8192;
-    while (tb < want && tb < 65536) tb <<= 1;
-    return tb;
+
+// Cut one copy op into (kind, offset, bytes) pieces.  Source and destination congruent mod 16: unaligned head and
+// tail go to the register path, the aligned body to bulk-copy tiles; otherwise register-path tiles throughout.
+struct Piece { uint32_t kind; uint64_t off; uint32_t n; };
+static void cut_copy(uint64_t dst, uint64_t src, uint64_t n, uint32_t seg_tiles, std::vector<Piece> &out) {
+    out.clear();
+    if (n == 0) { out.push_back({T_NODATA, 0, 0}); return; }
+    const bool congruent = ((dst ^ src) & 15) == 0;
+    const bool aligned = congruent && (dst & 15) == 0 && (n & 15) == 0;
+    if (aligned || (congruent && n >= TMA_MIN_SPLIT)) {
+        uint64_t head = (16 - (dst & 15)) & 15;
+        if (head > n) head = n;
+        const uint64_t body = (n - head) & ~15ull, tail = n - head - body;
+        if (head) out.push_back({T_COPY, 0, (uint32_t)head});
+        // balanced segments of at most seg_tiles bulk tiles
+        const uint64_t tiles = (body + SHMEMG_TMA_TILE - 1) / SHMEMG_TMA_TILE;
+        const uint64_t nseg = (tiles + seg_tiles - 1) / seg_tiles;
+        for (uint64_t g = 0, t0 = 0; g < nseg; ++g) {
+            const uint64_t t1 = (g + 1) * tiles / nseg;
+            const uint64_t b0 = t0 * SHMEMG_TMA_TILE, b1 = t1 * SHMEMG_TMA_TILE < body ? t1 * SHMEMG_TMA_TILE : body;
+            out.push_back({T_TMA, head + b0, (uint32_t)(b1 - b0)});
+            t0 = t1;
+        }
+        if (tail) out.push_back({T_COPY, head + body, (uint32_t)tail});
+        return;
+    }
+    for (uint64_t o = 0; o < n; o += GEN_TILE) out.push_back({T_COPY, o, (uint32_t)(n - o < GEN_TILE ? n - o : GEN_TILE)});
 }
 
-struct PlanSizes { size_t real_ops, ntiles, total; size_t ops_off, tiles_off, done_off, arrive_off; uint32_t tile_bytes; };
+// Segment length: a small batch is cut so that every SM gets about one segment (one completion fence per CTA);
+// a large batch uses the maximum (dynamic tickets balance it).
+static uint32_t pick_seg_tiles(const shmemg_world *w, const shmemg_op_t *ops, size_t nops) {
+    uint64_t tiles = 0;
+    for (size_t i = 0; i < nops; ++i)
+        if (ops[i].opcode >= SHMEMG_OP_PUT && ops[i].opcode <= SHMEMG_OP_PUT_SIGNAL)
+            tiles += (ops[i].nbytes + SHMEMG_TMA_TILE - 1) / SHMEMG_TMA_TILE;
+    const uint64_t per_sm = (tiles + w->sm_count - 1) / w->sm_count;
+    if (per_sm >= SEG_TILES_MAX) return SEG_TILES_MAX;
+    return per_sm < 1 ? 1u : (uint32_t)per_sm;
+}
 
-static PlanSizes plan_sizes(const shmemg_world *w, const shmemg_op_t *ops, size_t nops) {
-    PlanSizes s{};
-    s.tile_bytes = pick_tile_bytes(w, ops, nops);
-    size_t run = 0;
+// ---- planning units: a marker, one copy op, one AMO op, or a run of consecutive waits of one PE ----------------------
+struct Unit { uint8_t opc; int pe; size_t first, count; };    // [first, first+count) in the caller's op array
+
+static void build_units(const shmemg_op_t *ops, size_t nops, std::vector<Unit> &units) {
+    units.clear();
     for (size_t i = 0; i < nops; ++i) {
-        const uint8_t opc = ops[i].opcode;
-        if (is_marker(opc)) { run = 0; continue; }
-        s.real_ops++;
-        if (is_amo(opc)) {
+        const shmemg_op_t &o = ops[i];
+        if (o.opcode == SHMEMG_OP_SIGNAL_WAIT_UNTIL && !units.empty()) {
+            Unit &u = units.back();
+            if (u.opc == SHMEMG_OP_SIGNAL_WAIT_UNTIL && u.pe == o.initiator_pe && u.count < WAIT_RUN_MAX) { u.count++; continue; }
+        }
+        units.push_back({o.opcode, o.opcode == SHMEMG_OP_BARRIER_ALL ? 0 : o.initiator_pe, i, 1});
+    }
+}
+
+struct PlanSizes { size_t nunits, naux, ntiles, total; size_t tiles_off, aux_off, done_off, arrive_off, trace_off; };
+
+static void copy_endpoints(const shmemg_world *w, const shmemg_op_t &o, uint64_t &dst, uint64_t &src) {
+    const bool put = o.opcode != SHMEMG_OP_GET;
+    dst = (uint64_t)shmemg_addr(w, put ? o.target_pe : o.initiator_pe, put ? o.rem_off : o.loc_off);
+    src = (uint64_t)shmemg_addr(w, put ? o.initiator_pe : o.target_pe, put ? o.loc_off : o.rem_off);
+}
+
+static PlanSizes plan_sizes(const shmemg_world *w, const shmemg_op_t *ops, size_t nops, const std::vector<Unit> &units) {
+    PlanSizes s{};
+    size_t run = 0;
+    std::vector<Piece> pieces;
+    const uint32_t seg_tiles = pick_seg_tiles(w, ops, nops);
+    for (const Unit &u : units) {
+        if (is_marker(u.opc)) { run = 0; continue; }
+        s.nunits++;
+        if (is_amo(u.opc)) {
+            s.naux++;
             if (run == 0 || run == AMO_RUN_MAX) { s.ntiles++; run = 0; }
             run++;
             continue;
         }
         run = 0;
-        if (opc == SHMEMG_OP_SIGNAL_WAIT_UNTIL) s.ntiles++;
-        else s.ntiles += ops[i].nbytes <= s.tile_bytes ? 1 : (ops[i].nbytes + s.tile_bytes - 1) / s.tile_bytes;
+        if (u.opc == SHMEMG_OP_SIGNAL_WAIT_UNTIL) { s.ntiles++; s.naux += u.count; continue; }
+        uint64_t dst, src;
+        copy_endpoints(w, ops[u.first], dst, src);
+        cut_copy(dst, src, ops[u.first].nbytes, seg_tiles, pieces);
+        s.ntiles += pieces.size();
     }
     auto up = [](size_t x) { return (x + 255) / 256 * 256; };
-    s.ops_off = sizeof(PlanHeader);
-    s.tiles_off = s.ops_off + up(s.real_ops * sizeof(DevOp));
-    s.done_off = s.tiles_off + up(s.ntiles * sizeof(Tile));
+    s.tiles_off = sizeof(PlanHeader);
+    s.aux_off = s.tiles_off + up(s.ntiles * sizeof(TileRec));
+    s.done_off = s.aux_off + up(s.naux * sizeof(AuxRec));
     s.arrive_off = s.done_off + up(((size_t)w->npes + 1) * 4);
-    s.total = s.arrive_off + up(s.real_ops * 4) + 256;
+    s.trace_off = s.arrive_off + up(s.nunits * 4);
+    s.total = s.trace_off + TRACE_BYTES;
     return s;
 }
 
 extern "C" size_t shmemg_batch_plan_bytes(const shmemg_world_t *w, const shmemg_op_t *ops_host, size_t nops) {
     if (!w || (!ops_host && nops)) return 0;
-    return plan_sizes(w, ops_host, nops).total;
+    // an invalid descriptor is reported (with its index) by shmemg_batch_create, which never touches the plan then
+    for (size_t i = 0; i < nops; ++i)
+        if (validate_op(w, ops_host[i])) return sizeof(PlanHeader);
+    std::vector<Unit> units;
+    build_units(ops_host, nops, units);
+    return plan_sizes(w, ops_host, nops, units).total;
 }
 
 extern "C" int shmemg_batch_create(shmemg_world_t *w, const shmemg_op_t *ops, size_t nops, void *plan_dev,
@@ -293,91 +544,119 @@ extern "C" int shmemg_batch_create(shmemg_world_t *w, const shmemg_op_t *ops, si
             return rc;
         }
     }
-    const PlanSizes ps = plan_sizes(w, ops, nops);
+    std::vector<Unit> units;
+    build_units(ops, nops, units);
+    const PlanSizes ps = plan_sizes(w, ops, nops, units);
     if (plan_bytes < ps.total) return SHMEMG_ERR_NOMEM;
-    if (ps.ntiles >= 0xffffffffull || ps.real_ops >= 0xffffffffull) return SHMEMG_ERR_NOMEM;
+    if (ps.ntiles >= 0xffffffffull || ps.nunits >= 0xffffffffull) return SHMEMG_ERR_NOMEM;
+    const size_t nu = units.size();
+
+    // backward pass: which units does a LATER REAL unit depend on through a marker (or a wait)?
+    std::vector<uint8_t> cnt(nu, 0);            // bit 0: count on done[initiator]; bit 1: count on done[npes]
+    std::vector<uint32_t> pe_total(w->npes, 0); // how far done[p] advances per launch
+    uint32_t all_total = 0;
+    {
+        std::vector<uint8_t> later_real(w->npes, 0), need(w->npes, 0);
+        bool later_any = false, need_all = false;
+        for (size_t i = nu; i-- > 0;) {
+            const Unit &u = units[i];
+            if (u.opc == SHMEMG_OP_FENCE || u.opc == SHMEMG_OP_QUIET) {
+                if (later_real[u.pe]) need[u.pe] = 1;
+                continue;
+            }
+            if (u.opc == SHMEMG_OP_BARRIER_ALL) { if (later_any) need_all = true; continue; }
+            // a wait orders the PE's later ops after it: the wait and every earlier op of that PE are counted
+            if (u.opc == SHMEMG_OP_SIGNAL_WAIT_UNTIL && later_real[u.pe]) need[u.pe] = 1;
+            cnt[i] = (need[u.pe] ? 1 : 0) | (need_all ? 2 : 0);
+            if (cnt[i] & 1) pe_total[u.pe]++;
+            if (cnt[i] & 2) all_total++;
+            later_real[u.pe] = 1;
+            later_any = true;
+        }
+    }
 
     std::vector<uint8_t> host(ps.total, 0);
     PlanHeader *hdr = reinterpret_cast<PlanHeader *>(host.data());
-    DevOp *dops = reinterpret_cast<DevOp *>(host.data() + ps.ops_off);
-    Tile *tiles = reinterpret_cast<Tile *>(host.data() + ps.tiles_off);
+    TileRec *tiles = reinterpret_cast<TileRec *>(host.data() + ps.tiles_off);
+    AuxRec *aux = reinterpret_cast<AuxRec *>(host.data() + ps.aux_off);
     hdr->ntiles = (uint32_t)ps.ntiles;
-    hdr->nops = (uint32_t)ps.real_ops;
+    hdr->nunits = (uint32_t)ps.nunits;
     hdr->npes = (uint32_t)w->npes;
-    hdr->tile_bytes = ps.tile_bytes;
-    hdr->ops_off = ps.ops_off; hdr->tiles_off = ps.tiles_off; hdr->done_off = ps.done_off; hdr->arrive_off = ps.arrive_off;
+    hdr->all_total = all_total;
+    hdr->tiles_off = ps.tiles_off; hdr->aux_off = ps.aux_off; hdr->done_off = ps.done_off; hdr->arrive_off = ps.arrive_off;
+    hdr->trace_off = ps.trace_off;
+    if (const char *e = getenv("SHMEMG_TRACE")) hdr->trace_on = (uint32_t)atoi(e);
 
-    // forward pass: dependencies.  issued[p] = real ops of PE p so far; thresh[p] = what p's next op must see.
+    // forward pass: dependencies.  issued[p] = counted units of PE p so far; thresh[p] = what p's next unit must see.
+    // (Only counted units advance done[], and every unit before a marker that a later unit depends on is counted.)
     std::vector<uint32_t> issued(w->npes, 0), thresh(w->npes, 0);
-    std::vector<uint32_t> src_index;            // real op -> index in the caller's array
-    src_index.reserve(ps.real_ops);
     uint32_t all_issued = 0, all_thresh = 0;
-    size_t k = 0, nt = 0, run = 0;
-    for (size_t i = 0; i < nops; ++i) {
-        const shmemg_op_t &o = ops[i];
-        if (o.opcode == SHMEMG_OP_FENCE || o.opcode == SHMEMG_OP_QUIET) {
-            thresh[o.initiator_pe] = issued[o.initiator_pe]; run = 0; continue;
-        }
-        if (o.opcode == SHMEMG_OP_BARRIER_ALL) { all_thresh = all_issued; run = 0; continue; }
-        DevOp &d = dops[k];
-        const int ini = o.initiator_pe;
-        d.kind = o.opcode;
-        d.initiator = (uint32_t)ini;
-        d.dep_pe = thresh[ini];
-        d.dep_all = all_thresh;
-        d.value = o.value;
-        d.cond = o.cond;
-        d.nbytes = o.nbytes;
-        if (o.opcode == SHMEMG_OP_PUT || o.opcode == SHMEMG_OP_PUT_SIGNAL) {
-            d.dst = (uint64_t)shmemg_addr(w, o.target_pe, o.rem_off);
-            d.src = (uint64_t)shmemg_addr(w, ini, o.loc_off);
-            if (o.opcode == SHMEMG_OP_PUT_SIGNAL) {
-                d.sig = (uint64_t)shmemg_addr(w, o.target_pe, o.sig_off);
-                d.kind |= (uint32_t)o.sig_op << 8;
+    size_t k = 0, nt = 0, na = 0, run = 0;
+    std::vector<Piece> pieces;
+    const uint32_t seg_tiles = pick_seg_tiles(w, ops, nops);
+    auto aux_dev = [&](size_t idx) { return (uint64_t)((uint8_t *)plan_dev + ps.aux_off + idx * sizeof(AuxRec)); };
+    for (size_t ui = 0; ui < nu; ++ui) {
+        const Unit &u = units[ui];
+        const shmemg_op_t &o = ops[u.first];
+        if (u.opc == SHMEMG_OP_FENCE || u.opc == SHMEMG_OP_QUIET) { thresh[u.pe] = issued[u.pe]; run = 0; continue; }
+        if (u.opc == SHMEMG_OP_BARRIER_ALL) { all_thresh = all_issued; run = 0; continue; }
+        const int ini = u.pe;
+        const uint32_t flags = ((cnt[ui] & 1) ? TF_CNT_PE : 0) | ((cnt[ui] & 2) ? TF_CNT_ALL : 0);
+        const uint32_t dep_pe = thresh[ini], dep_all = all_thresh;
+        if (is_amo(u.opc)) {
+            AuxRec &d = aux[na];
+            d.word = (uint64_t)shmemg_addr(w, o.target_pe, o.rem_off);
+            d.fetch = u.opc == SHMEMG_OP_ATOMIC_ADD ? 0 : (uint64_t)shmemg_addr(w, ini, o.loc_off);
+            d.value = o.value; d.cond = o.cond;
+            d.kind = u.opc | flags;
+            d.initiator = (uint32_t)ini; d.dep_pe = dep_pe; d.dep_all = dep_all; d.pe_total = pe_total[ini];
+            if (run == 0 || run == AMO_RUN_MAX) {
+                TileRec &t = tiles[nt++];
+                t.kind = T_AMO; t.nbytes = 0; t.nt = 1; t.op = (uint32_t)k;
+                t.src = aux_dev(na);
+                run = 0;
             }
-        } else if (o.opcode == SHMEMG_OP_GET) {
-            d.dst = (uint64_t)shmemg_addr(w, ini, o.loc_off);
-            d.src = (uint64_t)shmemg_addr(w, o.target_pe, o.rem_off);
-        } else if (o.opcode == SHMEMG_OP_SIGNAL_WAIT_UNTIL) {
-            d.sig = (uint64_t)shmemg_addr(w, ini, o.loc_off);
-            d.kind |= (uint32_t)o.cmp << 8;
-        } else {   // AMO
-            d.dst = (uint64_t)shmemg_addr(w, o.target_pe, o.rem_off);
-            d.src = o.opcode == SHMEMG_OP_ATOMIC_ADD ? 0 : (uint64_t)shmemg_addr(w, ini, o.loc_off);
-            d.nbytes = 8;
-        }
-        // tiles
-        if (is_amo(o.opcode)) {
-            if (run == 0 || run == AMO_RUN_MAX) { tiles[nt].op = (uint32_t)k; tiles[nt].sub = 0; nt++; run = 0; }
-            tiles[nt - 1].sub++;
-            run++;
+            tiles[nt - 1].nbytes++;
+            run++; na++;
+        } else if (u.opc == SHMEMG_OP_SIGNAL_WAIT_UNTIL) {
+            run = 0;
+            TileRec &t = tiles[nt++];
+            t.kind = T_WAIT | flags | ((dep_pe | dep_all) ? TF_DEPS : 0);
+            t.src = aux_dev(na);
+            t.nbytes = (uint32_t)u.count;
+            t.nt = 1; t.op = (uint32_t)k; t.initiator = (uint32_t)ini; t.dep_pe = dep_pe; t.dep_all = dep_all;
+            t.pe_total = pe_total[ini];
+            for (size_t j = 0; j < u.count; ++j, ++na) {
+                const shmemg_op_t &wo = ops[u.first + j];
+                aux[na].word = (uint64_t)shmemg_addr(w, ini, wo.loc_off);
+                aux[na].value = wo.value;
+                aux[na].kind = SHMEMG_OP_SIGNAL_WAIT_UNTIL | ((uint32_t)wo.cmp << 8);
+                aux[na].initiator = (uint32_t)ini;
+            }
         } else {
             run = 0;
-            const size_t n = (o.opcode == SHMEMG_OP_SIGNAL_WAIT_UNTIL || o.nbytes <= ps.tile_bytes)
-                                 ? 1 : (o.nbytes + ps.tile_bytes - 1) / ps.tile_bytes;
-            for (size_t s = 0; s < n; ++s) { tiles[nt].op = (uint32_t)k; tiles[nt].sub = (uint32_t)s; nt++; }
+            uint64_t dst, src;
+            copy_endpoints(w, o, dst, src);
+            cut_copy(dst, src, o.nbytes, seg_tiles, pieces);
+            uint32_t f = flags | ((dep_pe | dep_all) ? TF_DEPS : 0);
+            uint64_t sig = 0;
+            if (u.opc == SHMEMG_OP_PUT_SIGNAL) {
+                f |= TF_SIGNAL | ((uint32_t)o.sig_op << 8);
+                sig = (uint64_t)shmemg_addr(w, o.target_pe, o.sig_off);
+            }
+            for (size_t p = 0; p < pieces.size(); ++p) {
+                TileRec &t = tiles[nt++];
+                t.dst = dst + pieces[p].off; t.src = src + pieces[p].off; t.nbytes = pieces[p].n;
+                t.kind = pieces[p].kind | f;
+                t.sig = sig; t.value = o.value;
+                t.op = (uint32_t)k; t.nt = (uint32_t)pieces.size(); t.initiator = (uint32_t)ini;
+                t.dep_pe = dep_pe; t.dep_all = dep_all; t.pe_total = pe_total[ini];
+            }
         }
-        issued[ini]++; all_issued++;
-        if (o.opcode == SHMEMG_OP_SIGNAL_WAIT_UNTIL) thresh[ini] = issued[ini];   // later ops of this PE follow the wait
-        src_index.push_back((uint32_t)i);
+        if (cnt[ui] & 1) issued[ini]++;
+        if (cnt[ui] & 2) all_issued++;
+        if (u.opc == SHMEMG_OP_SIGNAL_WAIT_UNTIL) thresh[ini] = issued[ini];   // later ops of this PE follow the wait
         k++;
-    }
-    // backward pass: which ops does a later marker depend on?
-    {
-        std::vector<uint8_t> later_pe(w->npes, 0);
-        bool later_all = false;
-        size_t kk = ps.real_ops;
-        for (size_t i = nops; i-- > 0;) {
-            const shmemg_op_t &o = ops[i];
-            if (o.opcode == SHMEMG_OP_FENCE || o.opcode == SHMEMG_OP_QUIET) { later_pe[o.initiator_pe] = 1; continue; }
-            if (o.opcode == SHMEMG_OP_BARRIER_ALL) { later_all = true; continue; }
-            kk--;
-            // A wait makes the PE's LATER ops depend on done[p] reaching the wait's own count, so the wait and
-            // every earlier op of that PE must be counted.
-            if (o.opcode == SHMEMG_OP_SIGNAL_WAIT_UNTIL) later_pe[o.initiator_pe] = 1;
-            if (later_pe[o.initiator_pe]) dops[kk].kind |= OPF_COUNT_PE;
-            if (later_all) dops[kk].kind |= OPF_COUNT_ALL;
-        }
     }
 
     cudaStream_t st = (cudaStream_t)stream;
@@ -388,8 +667,11 @@ extern "C" int shmemg_batch_create(shmemg_world_t *w, const shmemg_op_t *ops, si
     b->w = w;
     b->plan_dev = (uint8_t *)plan_dev;
     b->ntiles = (uint32_t)ps.ntiles;
-    const uint64_t maxgrid = (uint64_t)w->sm_count * w->ctas_per_sm;
+    const uint64_t maxgrid = (uint64_t)w->sm_count;
     b->grid = (uint32_t)(ps.ntiles < maxgrid ? (ps.ntiles ? ps.ntiles : 1) : maxgrid);
+    b->npes = (uint32_t)w->npes; b->all_total = all_total;
+    b->tiles_off = ps.tiles_off; b->done_off = ps.done_off; b->arrive_off = ps.arrive_off; b->trace_off = ps.trace_off;
+    b->trace_on = hdr->trace_on != 0;
     *out = b;
     return SHMEMG_OK;
 }
@@ -401,10 +683,27 @@ extern "C" int shmemg_batch_destroy(shmemg_batch_t *b) {
 }
 extern "C" int shmemg_batch_launches(const shmemg_batch_t *b) { return b ? (b->ntiles ? 1 : 0) : SHMEMG_ERR_ARG; }
 
+static int ensure_smem_attr(shmemg_world *w) {
+    if (w->smem_attr_set) return SHMEMG_OK;
+    SHMEMG_CUDA(w, cudaFuncSetAttribute(k_batch_exec, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SHMEMG_TMA_SMEM));
+    SHMEMG_CUDA(w, cudaFuncSetAttribute(k_copy_single_tma, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SHMEMG_TMA_SMEM));
+    w->smem_attr_set = true;
+    return SHMEMG_OK;
+}
+
 extern "C" int shmemg_batch_enqueue_on_stream(shmemg_world_t *w, shmemg_batch_t *b, void *stream) {
     if (!w || !b || b->w != w) return SHMEMG_ERR_ARG;
     if (b->ntiles == 0) return SHMEMG_OK;
-    k_batch_exec<<<b->grid, SHMEMG_THREADS, 0, (cudaStream_t)stream>>>(b->plan_dev);
+    int rc = ensure_smem_attr(w);
+    if (rc) return rc;
+    ExecArgs a;
+    a.tiles = reinterpret_cast<const TileRec *>(b->plan_dev + b->tiles_off);
+    a.ticket = &reinterpret_cast<PlanHeader *>(b->plan_dev)->ticket;
+    a.done = reinterpret_cast<unsigned *>(b->plan_dev + b->done_off);
+    a.arrive = reinterpret_cast<unsigned *>(b->plan_dev + b->arrive_off);
+    a.trace = b->trace_on ? reinterpret_cast<unsigned long long *>(b->plan_dev + b->trace_off) : nullptr;
+    a.ntiles = b->ntiles; a.npes = b->npes; a.all_total = b->all_total;
+    k_batch_exec<<<b->grid, EXEC_THREADS, SHMEMG_TMA_SMEM, (cudaStream_t)stream>>>(a);
     SHMEMG_CUDA(w, cudaGetLastError());
     return SHMEMG_OK;
 }
@@ -415,13 +714,22 @@ extern "C" int shmemg_batch_enqueue_on_stream(shmemg_world_t *w, shmemg_batch_t 
 static int launch_copy(shmemg_world *w, uint8_t *dst, const uint8_t *src, size_t nbytes, unsigned long long *sig,
                        uint64_t sig_value, int sig_op, cudaStream_t st) {
     if (nbytes == 0 && !sig) return SHMEMG_OK;
+    unsigned *counter = sig ? &w->ctl->sig_counter[(w->sig_seq++) % SHMEMG_SIG_SLOTS] : nullptr;
+    if (nbytes && (((uintptr_t)dst | (uintptr_t)src | nbytes) & 15) == 0 && !w->tile_bytes_override) {
+        int rc = ensure_smem_attr(w);
+        if (rc) return rc;
+        const uint64_t ntiles = (nbytes + SHMEMG_TMA_TILE - 1) / SHMEMG_TMA_TILE;
+        const uint32_t grid = (uint32_t)(ntiles < (uint64_t)w->sm_count ? ntiles : (uint64_t)w->sm_count);
+        k_copy_single_tma<<<grid, 32, SHMEMG_TMA_SMEM, st>>>(dst, src, nbytes, sig, sig_value, sig_op, counter);
+        SHMEMG_CUDA(w, cudaGetLastError());
+        return SHMEMG_OK;
+    }
     const uint64_t maxgrid = (uint64_t)w->sm_count * w->ctas_per_sm;
     uint32_t tb = 8192;
     while (tb < 65536 && nbytes / tb > maxgrid * 8) tb <<= 1;
     if (w->tile_bytes_override) tb = (uint32_t)w->tile_bytes_override;
     uint64_t ntiles = (nbytes + tb - 1) / tb;
     uint32_t grid = (uint32_t)(ntiles < maxgrid ? (ntiles ? ntiles : 1) : maxgrid);
-    unsigned *counter = sig ? &w->ctl->sig_counter[(w->sig_seq++) % SHMEMG_SIG_SLOTS] : nullptr;
     k_copy_single<<<grid, SHMEMG_THREADS, 0, st>>>(dst, src, nbytes, tb, sig, sig_value, sig_op, counter);
     SHMEMG_CUDA(w, cudaGetLastError());
     return SHMEMG_OK;

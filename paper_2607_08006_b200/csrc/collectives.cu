@@ -3,7 +3,7 @@
 //   fcollect   : each source chunk is read once into registers and stored to all N destinations (write-bound)
 //   sum_reduce : one pass down the N windows per column group, fp64 accumulation for fp32, N-way replicated store
 //   barrier    : stream-level (kernel boundary) and in-kernel (one CTA per PE, cooperative launch)
-#include "internal.cuh"
+#include "tma_stream.cuh"
 
 // ---- alltoall: PE j's dest block i = PE i's source block j -------------------------------------------------------
 __global__ void __launch_bounds__(SHMEMG_THREADS, 4)
@@ -20,6 +20,27 @@ k_alltoall(uint8_t *base, size_t stride, uint64_t dst_off, uint64_t src_off, siz
         copy_coop<8>(base + (size_t)j * stride + dst_off + (size_t)i * blk + off,
                      base + (size_t)i * stride + src_off + (size_t)j * blk + off, n, threadIdx.x, SHMEMG_THREADS);
     }
+}
+
+
+// bulk-copy path (block size, offsets and stride 16-byte aligned): one issuing thread per CTA, work item =
+// (source PE i, destination PE j, <= 32 KiB chunk), source-major so each CTA streams one PE's row
+__global__ void __launch_bounds__(32)
+k_alltoall_tma(uint8_t *base, size_t stride, uint64_t dst_off, uint64_t src_off, size_t blk, int npes, unsigned chunks_per_blk) {
+    extern __shared__ __align__(1024) uint8_t stage[];
+    __shared__ uint64_t full[SHMEMG_TMA_STAGES];
+    if (threadIdx.x != 0) return;
+    tma_stream_init(full);
+    const size_t nwork = (size_t)npes * npes * chunks_per_blk;
+    tma_stream_copy(stage, full, blockIdx.x, gridDim.x, nwork, [&](size_t wk, const uint8_t *&s, uint8_t *&d, unsigned &n) {
+        const unsigned c = (unsigned)(wk % chunks_per_blk);
+        const size_t ij = wk / chunks_per_blk;
+        const int j = (int)(ij % npes), i = (int)(ij / npes);
+        const size_t off = (size_t)c * SHMEMG_TMA_TILE;
+        n = (unsigned)(blk - off < SHMEMG_TMA_TILE ? blk - off : SHMEMG_TMA_TILE);
+        s = base + (size_t)i * stride + src_off + (size_t)j * blk + off;
+        d = base + (size_t)j * stride + dst_off + (size_t)i * blk + off;
+    });
 }
 
 // ---- fcollect: PE j's dest[p*n .. +n) = PE p's source[0 .. n) for every j -------------------------------------------
@@ -55,6 +76,54 @@ k_fcollect_vec(uint8_t *base, size_t stride, uint64_t dst_off, uint64_t src_off,
             }
         }
     }
+}
+
+// bulk-copy path: each work item (source PE p, <= 32 KiB chunk, group of destination PEs) is loaded into shared memory
+// ONCE and stored from there to every destination of the group; the source (N x nbytes) is read from HBM once and
+// from L2 by the other groups.  One issuing thread per CTA; STAGES-1 loads in flight ahead of the store front.
+__global__ void __launch_bounds__(32)
+k_fcollect_tma(uint8_t *base, size_t stride, uint64_t dst_off, uint64_t src_off, size_t nbytes, int npes,
+               unsigned chunks_per_blk, int dst_groups) {
+    extern __shared__ __align__(1024) uint8_t stage[];
+    __shared__ uint64_t full[SHMEMG_TMA_STAGES];
+    if (threadIdx.x != 0) return;
+    tma_stream_init(full);
+    const size_t nwork = (size_t)npes * chunks_per_blk * dst_groups;
+    const int per_group = (npes + dst_groups - 1) / dst_groups;
+    const size_t first = blockIdx.x, step = gridDim.x;
+    const size_t mine = first < nwork ? (nwork - first + step - 1) / step : 0;
+    auto decode = [&](size_t it, int &p, int &g, size_t &off, unsigned &n) {
+        const size_t wk = first + it * step;
+        g = (int)(wk % dst_groups);
+        const size_t pc = wk / dst_groups;
+        const unsigned c = (unsigned)(pc % chunks_per_blk);
+        p = (int)(pc / chunks_per_blk);
+        off = (size_t)c * SHMEMG_TMA_TILE;
+        n = (unsigned)(nbytes - off < SHMEMG_TMA_TILE ? nbytes - off : SHMEMG_TMA_TILE);
+    };
+    auto issue_load = [&](size_t it) {
+        int p, g; size_t off; unsigned n;
+        decode(it, p, g, off, n);
+        const int st = (int)(it % SHMEMG_TMA_STAGES);
+        mbar_arrive_expect_tx(&full[st], n);
+        bulk_g2s(stage + (size_t)st * SHMEMG_TMA_TILE, base + (size_t)p * stride + src_off + off, n, &full[st]);
+    };
+    for (size_t it = 0; it < mine && it < SHMEMG_TMA_STAGES - 1; ++it) issue_load(it);
+    for (size_t it = 0; it < mine; ++it) {
+        const int st = (int)(it % SHMEMG_TMA_STAGES);
+        mbar_wait(&full[st], (unsigned)((it / SHMEMG_TMA_STAGES) & 1));
+        int p, g; size_t off; unsigned n;
+        decode(it, p, g, off, n);
+        const int j0 = g * per_group, j1 = min(npes, j0 + per_group);
+        for (int j = j0; j < j1; ++j)
+            bulk_s2g(base + (size_t)j * stride + dst_off + (size_t)p * nbytes + off, stage + (size_t)st * SHMEMG_TMA_TILE, n);
+        bulk_commit();
+        if (it + SHMEMG_TMA_STAGES - 1 < mine) {
+            bulk_wait_read<1>();
+            issue_load(it + SHMEMG_TMA_STAGES - 1);
+        }
+    }
+    bulk_wait<0>();
 }
 // generic byte path (unaligned sizes/offsets): plain per-(p, j) cooperative copies
 __global__ void __launch_bounds__(SHMEMG_THREADS, 4)
@@ -186,6 +255,14 @@ __global__ void __launch_bounds__(32) k_barrier_repeat(CtlRegion *ctl, uint8_t *
 // ---------------------------------------------------------------------------------------------------------
 // host entry points
 // ---------------------------------------------------------------------------------------------------------
+static int collectives_smem_attr(shmemg_world *w) {
+    if (w->smem_attr_coll) return SHMEMG_OK;
+    SHMEMG_CUDA(w, cudaFuncSetAttribute(k_alltoall_tma, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SHMEMG_TMA_SMEM));
+    SHMEMG_CUDA(w, cudaFuncSetAttribute(k_fcollect_tma, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SHMEMG_TMA_SMEM));
+    w->smem_attr_coll = true;
+    return SHMEMG_OK;
+}
+
 static bool ranges_overlap(uint64_t a, uint64_t b, uint64_t n_a, uint64_t n_b) { return a < b + n_b && b < a + n_a; }
 
 extern "C" int shmemg_alltoall_on_stream(shmemg_world_t *w, uint64_t dest_off, uint64_t source_off, size_t nbytes,
@@ -195,6 +272,17 @@ extern "C" int shmemg_alltoall_on_stream(shmemg_world_t *w, uint64_t dest_off, u
     if (!shmemg_in_range(w, dest_off, tot) || !shmemg_in_range(w, source_off, tot)) return SHMEMG_ERR_RANGE;
     if (nbytes == 0) return SHMEMG_OK;
     if (ranges_overlap(dest_off, source_off, tot, tot)) return SHMEMG_ERR_OVERLAP;
+    cudaStream_t st = (cudaStream_t)stream;
+    if (((dest_off | source_off | nbytes | w->stride) & 15) == 0 && !w->tile_bytes_override) {
+        int rc = collectives_smem_attr(w);
+        if (rc) return rc;
+        const unsigned cpb = (unsigned)((nbytes + SHMEMG_TMA_TILE - 1) / SHMEMG_TMA_TILE);
+        const uint64_t nwork = (uint64_t)w->npes * w->npes * cpb;
+        const unsigned grid = (unsigned)(nwork < (uint64_t)w->sm_count ? nwork : (uint64_t)w->sm_count);
+        k_alltoall_tma<<<grid, 32, SHMEMG_TMA_SMEM, st>>>(w->base, w->stride, dest_off, source_off, nbytes, w->npes, cpb);
+        SHMEMG_CUDA(w, cudaGetLastError());
+        return SHMEMG_OK;
+    }
     const uint64_t maxgrid = (uint64_t)w->sm_count * w->ctas_per_sm;
     unsigned chunk = 65536;
     if (w->tile_bytes_override) chunk = (unsigned)w->tile_bytes_override;
@@ -203,8 +291,7 @@ extern "C" int shmemg_alltoall_on_stream(shmemg_world_t *w, uint64_t dest_off, u
     const unsigned cpb = (unsigned)((nbytes + chunk - 1) / chunk);
     const uint64_t nwork = (uint64_t)w->npes * w->npes * cpb;
     const unsigned grid = (unsigned)(nwork < maxgrid ? nwork : maxgrid);
-    k_alltoall<<<grid, SHMEMG_THREADS, 0, (cudaStream_t)stream>>>(w->base, w->stride, dest_off, source_off, nbytes,
-                                                                  w->npes, chunk, cpb);
+    k_alltoall<<<grid, SHMEMG_THREADS, 0, st>>>(w->base, w->stride, dest_off, source_off, nbytes, w->npes, chunk, cpb);
     SHMEMG_CUDA(w, cudaGetLastError());
     return SHMEMG_OK;
 }
@@ -218,7 +305,17 @@ extern "C" int shmemg_fcollect_on_stream(shmemg_world_t *w, uint64_t dest_off, u
     if (ranges_overlap(dest_off, source_off, tot, nbytes)) return SHMEMG_ERR_OVERLAP;
     const uint64_t maxgrid = (uint64_t)w->sm_count * w->ctas_per_sm;
     cudaStream_t st = (cudaStream_t)stream;
-    if (((dest_off | source_off | nbytes | w->stride) & 15) == 0) {
+    if (((dest_off | source_off | nbytes | w->stride) & 15) == 0 && !w->tile_bytes_override) {
+        int rc = collectives_smem_attr(w);
+        if (rc) return rc;
+        const unsigned cpb = (unsigned)((nbytes + SHMEMG_TMA_TILE - 1) / SHMEMG_TMA_TILE);
+        int groups = 1;                                         // split destinations until every SM has >= 8 items
+        while (groups < w->npes && (uint64_t)w->npes * cpb * groups < (uint64_t)w->sm_count * 8) groups <<= 1;
+        if (groups > w->npes) groups = w->npes;
+        const uint64_t nwork = (uint64_t)w->npes * cpb * groups;
+        const unsigned grid = (unsigned)(nwork < (uint64_t)w->sm_count ? nwork : (uint64_t)w->sm_count);
+        k_fcollect_tma<<<grid, 32, SHMEMG_TMA_SMEM, st>>>(w->base, w->stride, dest_off, source_off, nbytes, w->npes, cpb, groups);
+    } else if (((dest_off | source_off | nbytes | w->stride) & 15) == 0) {
         constexpr int VPT = 4;                                  // 256 threads * 4 * 16 B = 16 KiB per work item
         const unsigned cpb = (unsigned)(((nbytes >> 4) + SHMEMG_THREADS * VPT - 1) / (SHMEMG_THREADS * VPT));
         int groups = 1;                                         // split destinations until the grid is full

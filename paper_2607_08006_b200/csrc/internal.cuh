@@ -13,7 +13,9 @@
 #define SHMEMG_CTL_BYTES (64u * 1024u)     // control region carved from the tail of the slab
 #define SHMEMG_STRIDE_ALIGN 512u
 #define SHMEMG_MIN_ALIGN 256u
-#define SHMEMG_THREADS 256                 // threads per CTA of every copy-class kernel
+#define SHMEMG_THREADS 256                 // threads per CTA of the register-path copy kernels
+#define SHMEMG_TMA_TILE 32768u             // bytes per bulk-copy stage
+#define SHMEMG_TMA_STAGES 4                // stages per CTA (128 KiB of shared memory, one CTA per SM)
 #define SHMEMG_SIG_SLOTS 1024              // completion counters for single put_signal launches
 
 // ---- control region layout (device) -------------------------------------------------------------------
@@ -39,7 +41,9 @@ struct shmemg_world {
     std::map<uint64_t, size_t> live;       // offset -> size of live allocations
     unsigned sig_seq = 0;
     int ctas_per_sm = 4;                   // copy-class persistent grids: ctas_per_sm * sm_count CTAs
-    size_t tile_bytes_override = 0;        // SHMEMG_TILE_BYTES (experiments)
+    size_t tile_bytes_override = 0;        // SHMEMG_TILE_BYTES (experiments; forces the register copy path)
+    bool smem_attr_coll = false, smem_attr_probe = false;
+    bool smem_attr_set = false;            // dynamic shared memory opt-in done for the bulk-copy kernels
     std::string last_cuda_error;
 };
 
@@ -74,6 +78,18 @@ __device__ __forceinline__ unsigned long long ld_acquire_u64(const unsigned long
     asm volatile("ld.acquire.gpu.global.u64 %0, [%1];" : "=l"(v) : "l"(p) : "memory");
     return v;
 }
+// polling loads: relaxed (no L1 invalidate per probe); the caller issues ONE fence_acquire() after the poll succeeds
+__device__ __forceinline__ unsigned ld_relaxed_u32(const unsigned *p) {
+    unsigned v;
+    asm volatile("ld.relaxed.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+    return v;
+}
+__device__ __forceinline__ unsigned long long ld_relaxed_u64(const unsigned long long *p) {
+    unsigned long long v;
+    asm volatile("ld.relaxed.gpu.global.u64 %0, [%1];" : "=l"(v) : "l"(p) : "memory");
+    return v;
+}
+__device__ __forceinline__ void fence_acquire() { asm volatile("fence.acq_rel.gpu;" ::: "memory"); }
 __device__ __forceinline__ void red_release_add_u32(unsigned *p, unsigned v) {
     asm volatile("red.release.gpu.global.add.u32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
 }
@@ -97,6 +113,57 @@ __device__ __forceinline__ bool cmp_u64(int cmp, unsigned long long s, unsigned 
 __device__ __forceinline__ void signal_update(unsigned long long *sig, unsigned long long v, int sig_op) {
     if (sig_op == SHMEMG_SIGNAL_ADD) red_release_add_u64(sig, v);
     else exch_release_u64(sig, v);
+}
+
+
+// ---- mbarrier + bulk (TMA) copy primitives: cp.async.bulk moves contiguous 16-byte-aligned blocks between global and
+// shared memory without touching registers; one thread drives a whole pipeline (SASS: UBLKCP) -----------------------
+__device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(uint64_t *b, unsigned count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(b)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_init_fence() {       // make the initialised barriers visible to the async proxy
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint64_t *b) {
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(b)) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive_expect_tx(uint64_t *b, unsigned bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(b)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ bool mbar_try_wait(uint64_t *b, unsigned parity) {
+    unsigned ok;
+    asm volatile("{\n .reg .pred p;\n mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n selp.u32 %0, 1, 0, p;\n}"
+                 : "=r"(ok) : "r"(smem_u32(b)), "r"(parity) : "memory");
+    return ok != 0;
+}
+// non-blocking probe (try_wait may suspend the thread for an implementation-defined time before returning false)
+__device__ __forceinline__ bool mbar_test_wait(uint64_t *b, unsigned parity) {
+    unsigned ok;
+    asm volatile("{\n .reg .pred p;\n mbarrier.test_wait.parity.shared::cta.b64 p, [%1], %2;\n selp.u32 %0, 1, 0, p;\n}"
+                 : "=r"(ok) : "r"(smem_u32(b)), "r"(parity) : "memory");
+    return ok != 0;
+}
+__device__ __forceinline__ void mbar_wait(uint64_t *b, unsigned parity) {
+    while (!mbar_test_wait(b, parity)) { }
+}
+__device__ __forceinline__ void bulk_g2s(void *smem_dst, const void *gsrc, unsigned bytes, uint64_t *full) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                 ::"r"(smem_u32(smem_dst)), "l"(gsrc), "r"(bytes), "r"(smem_u32(full)) : "memory");
+}
+__device__ __forceinline__ void bulk_s2g(void *gdst, const void *smem_src, unsigned bytes) {
+    asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;"
+                 ::"l"(gdst), "r"(smem_u32(smem_src)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void bulk_commit() { asm volatile("cp.async.bulk.commit_group;" ::: "memory"); }
+// all but the N most recent bulk groups of this thread have finished READING shared memory / have COMPLETED
+template <int N> __device__ __forceinline__ void bulk_wait_read() { asm volatile("cp.async.bulk.wait_group.read %0;" ::"n"(N) : "memory"); }
+template <int N> __device__ __forceinline__ void bulk_wait() { asm volatile("cp.async.bulk.wait_group %0;" ::"n"(N) : "memory"); }
+// order this thread's generic-proxy accesses (acquire loads, release stores) against its async-proxy (bulk) accesses
+__device__ __forceinline__ void proxy_fence() { asm volatile("fence.proxy.async;" ::: "memory"); }
+__device__ __forceinline__ void named_bar_sync(int id, int nthreads) {
+    asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(nthreads) : "memory");
 }
 
 // ---- streaming 128-bit accesses: L2-coherent loads (never a stale L1 line), evict-first hints --------------

@@ -1,6 +1,6 @@
 // probe.cu -- ceiling probes (include/shmemg_probe.h): bare L2 atomics at hashed addresses and a plain
 // per-PE local copy.  Measurement utilities for bench.py; not operations of the specification.
-#include "internal.cuh"
+#include "tma_stream.cuh"
 #include "../../include/shmemg_probe.h"
 
 __device__ __forceinline__ unsigned long long probe_hash(unsigned long long i) {
@@ -45,6 +45,23 @@ k_probe_copy_all(uint8_t *base, size_t stride, uint64_t dst_off, uint64_t src_of
     }
 }
 
+
+__global__ void __launch_bounds__(32)
+k_probe_copy_all_tma(uint8_t *base, size_t stride, uint64_t dst_off, uint64_t src_off, size_t nbytes, unsigned npes,
+                     unsigned chunks_per_pe) {
+    extern __shared__ __align__(1024) uint8_t stage[];
+    __shared__ uint64_t full[SHMEMG_TMA_STAGES];
+    if (threadIdx.x != 0) return;
+    tma_stream_init(full);
+    tma_stream_copy(stage, full, blockIdx.x, gridDim.x, (size_t)npes * chunks_per_pe,
+                    [&](size_t wk, const uint8_t *&s, uint8_t *&d, unsigned &n) {
+        const size_t p = wk / chunks_per_pe, off = (wk % chunks_per_pe) * (size_t)SHMEMG_TMA_TILE;
+        n = (unsigned)(nbytes - off < SHMEMG_TMA_TILE ? nbytes - off : SHMEMG_TMA_TILE);
+        s = base + p * stride + src_off + off;
+        d = base + p * stride + dst_off + off;
+    });
+}
+
 extern "C" int shmemg_probe_atomic_on_stream(shmemg_world_t *w, int mode, uint64_t sym_off, uint64_t words_per_pe,
                                              size_t n, void *stream) {
     if (!w || mode < SHMEMG_PROBE_RED_ADD || mode > SHMEMG_PROBE_ATOM_CAS || words_per_pe == 0) return SHMEMG_ERR_ARG;
@@ -72,6 +89,19 @@ extern "C" int shmemg_probe_copy_all_on_stream(shmemg_world_t *w, uint64_t dst_o
     if (!shmemg_in_range(w, dst_off, nbytes) || !shmemg_in_range(w, src_off, nbytes)) return SHMEMG_ERR_RANGE;
     if (nbytes == 0) return SHMEMG_OK;
     if (dst_off < src_off + nbytes && src_off < dst_off + nbytes) return SHMEMG_ERR_OVERLAP;
+    if (((dst_off | src_off | nbytes | w->stride) & 15) == 0 && !w->tile_bytes_override) {
+        if (!w->smem_attr_probe) {
+            SHMEMG_CUDA(w, cudaFuncSetAttribute(k_probe_copy_all_tma, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SHMEMG_TMA_SMEM));
+            w->smem_attr_probe = true;
+        }
+        const unsigned cpp = (unsigned)((nbytes + SHMEMG_TMA_TILE - 1) / SHMEMG_TMA_TILE);
+        const uint64_t nwork = (uint64_t)w->npes * cpp;
+        const unsigned grid = (unsigned)(nwork < (uint64_t)w->sm_count ? nwork : (uint64_t)w->sm_count);
+        k_probe_copy_all_tma<<<grid, 32, SHMEMG_TMA_SMEM, (cudaStream_t)stream>>>(w->base, w->stride, dst_off, src_off, nbytes,
+                                                                                 (unsigned)w->npes, cpp);
+        SHMEMG_CUDA(w, cudaGetLastError());
+        return SHMEMG_OK;
+    }
     const uint64_t maxgrid = (uint64_t)w->sm_count * w->ctas_per_sm;
     unsigned chunk = 65536;
     if (w->tile_bytes_override) chunk = (unsigned)w->tile_bytes_override;
