@@ -175,6 +175,7 @@ def segment_table(inp: Inputs):
     if "barrier" in g:
         seg["barrier_in_kernel"] = dict(cls="sync", kernel="k_barrier_repeat", ops=BARRIERS, launches=1)
         seg["barrier_on_stream"] = dict(cls="sync", kernel="k_barrier_epoch", ops=BARRIERS, launches=BARRIERS)
+        seg["barrier_on_stream_graph"] = dict(cls="sync", kernel="k_barrier_epoch", ops=BARRIERS, launches=BARRIERS)
     return seg
 
 
@@ -216,13 +217,15 @@ class CudaBench:
     def __init__(self, inp: Inputs, device):
         import torch
         from paper_2607_08006_b200 import World
-        from paper_2607_08006_b200.binding import AMO_WARP_AGGREGATE
+        from paper_2607_08006_b200.binding import AMO_TEST_BEFORE_SWAP, AMO_WARP_AGGREGATE
         from paper_2607_08006_b200.loader import Loaded
         self.torch, self.inp, self.dev = torch, inp, device
         self.rec = Recorder(torch)
         self.app_launches = 0
+        self.barrier_graph = None
         self.worlds = []
-        self.flags = AMO_WARP_AGGREGATE
+        self.flags = 0                                 # warp aggregation buys nothing on these streams (profiles/)
+        self.cas_flags = AMO_TEST_BEFORE_SWAP          # scalar cond: failed swaps are resolved by a coherent load
         g = inp.groups
         dv = lambda a: torch.from_numpy(np.ascontiguousarray(a)).to(device)      # noqa: E731
         if "c3a" in g:
@@ -298,7 +301,7 @@ class CudaBench:
                                                flags=self.flags)
             with rec.seg("atomic_compare_swap"):
                 self.w4.atomic_compare_swap_batch(self.par, self.c4_ov, self.c4_lv, self.f_par, cond=None, cond_scalar=M64,
-                                                  val=self.c4_val, flags=self.flags)
+                                                  val=self.c4_val, flags=self.cas_flags)
         if "c1" in g:
             self.w1.view(self.A, inp.c1.nelem * 8).zero_()
             with rec.seg("atomic_add"):
@@ -336,6 +339,14 @@ class CudaBench:
             with rec.seg("barrier_on_stream"):
                 for _ in range(BARRIERS):
                     self.w5.barrier_all()
+            if self.barrier_graph is None:                               # the same 10 000 launches captured once (reading 24)
+                self.barrier_graph = torch.cuda.CUDAGraph()
+                with torch.cuda.graph(self.barrier_graph):
+                    for _ in range(BARRIERS):
+                        self.w5.barrier_all()
+            with rec.seg("barrier_on_stream_graph"):
+                self.barrier_graph.replay()
+                self.w5.launches += BARRIERS
 
     # ---- end-to-end: the same ops with HOST buffers, H2D / D2H inside the timed region --------------------------------
     def setup_e2e(self):
@@ -438,7 +449,7 @@ class CudaBench:
                     d.copy_(h, non_blocking=True)
                     self.h2d += h.numel() * h.element_size()
                 self.w4.atomic_compare_swap_batch(self.par, self.c4_ov, self.c4_lv, self.f_par, cond=None, cond_scalar=M64,
-                                                  val=self.c4_val, flags=self.flags)
+                                                  val=self.c4_val, flags=self.cas_flags)
                 self.h_fpar.copy_(self.f_par, non_blocking=True)
                 self.d2h += self.h_fpar.numel() * 8
                 self._down(self.w4, self.h_par, self.par)

@@ -216,6 +216,11 @@ SHMEMG_API int shmemg_quiet(shmemg_world_t *w, int pe, void *stream);
  * There is NO ordering between the ops of one call (reading 7); fetched values are valid when the stream
  * has passed the call.  flags: SHMEMG_AMO_* below.  64-bit integer types only (wraparound add). */
 #define SHMEMG_AMO_WARP_AGGREGATE 1u   /* combine same-address ops of a warp into one L2 atomic */
+/* compare-swap with a scalar cond only: read the word first (coherent L2 load) and issue the L2 atomic only while the
+ * word may still equal cond.  Legal because the ops of one call are unordered and each swaps only cond -> val: once a
+ * word differs from cond no op of the call can change it, so the loaded value is the failed swap's fetched value.
+ * Requires that nothing outside this call updates the target words while it runs (already undefined). */
+#define SHMEMG_AMO_TEST_BEFORE_SWAP 2u
 SHMEMG_API int shmemg_atomic_add_batch_on_stream(shmemg_world_t *w, uint64_t sym_off, const int32_t *tgt_pe,
                                                  const void *elem_idx, int idx_bytes, const uint64_t *val,
                                                  uint64_t val_scalar, size_t n, uint32_t flags, void *stream);

@@ -16,8 +16,8 @@ extern "C" {
 
 enum { SHMEMG_PROBE_RED_ADD = 0, SHMEMG_PROBE_ATOM_ADD = 1, SHMEMG_PROBE_ATOM_CAS = 2 };
 
-/* Issue `n` atomics on `stream`: op i targets u64 heap[h(i) % npes][sym_off + 8*((h(i) / npes) % words_per_pe)]
- * (uniformly random over npes*words_per_pe words), adding 0 (RED_ADD / ATOM_ADD) or comparing against a value the
+/* Issue `n` atomics on `stream`: op i targets u64 heap[pe(i)][sym_off + 8*wd(i)] with pe(i), wd(i) derived from a
+ * 64-bit hash of i by multiply-high (uniformly random over npes*words_per_pe words, no integer division), adding 0 (RED_ADD / ATOM_ADD) or comparing against a value the
  * word never holds (ATOM_CAS), so the heap is left unchanged.  words_per_pe >= 1; the object at sym_off must hold
  * 8*words_per_pe bytes.  Fetched values are xor-reduced per thread and stored only if the reduction is a value it
  * cannot take (keeps the atom.* results live without output traffic). */

@@ -63,6 +63,7 @@ class CAP:
 
 F32, I64 = 0, 1
 AMO_WARP_AGGREGATE = 1
+AMO_TEST_BEFORE_SWAP = 2
 NO_STAMP = (1 << 64) - 1
 
 # shmemg_op_t, 64 bytes

@@ -39,7 +39,7 @@ __device__ __forceinline__ unsigned long long shfl64(unsigned long long v, int l
     return __shfl_sync(FULL, v, lane);
 }
 
-template <int IDXB, int OP, bool AGG>
+template <int IDXB, int OP, bool AGG, bool TEST>
 __global__ void __launch_bounds__(256) k_amo(const AmoArgs a) {
     typedef typename IdxT<IDXB>::type idx_t;
     const idx_t *__restrict__ idx = reinterpret_cast<const idx_t *>(a.idx);
@@ -64,6 +64,21 @@ __global__ void __launch_bounds__(256) k_amo(const AmoArgs a) {
                 if (OP == AMO_CAS && cond) c[k] = cond[i];
             }
         }
+        if (OP == AMO_CAS && TEST) {
+            // test before compare-swap (scalar cond only): within one call a word that differs from cond can no longer
+            // change (every op swaps only cond -> val, val != cond), so a coherent load that sees such a value IS the
+            // failed compare-swap, linearised at the load; the L2 atomic is issued only while the word may still be cond.
+            unsigned long long cur[AMO_ITEMS];
+#pragma unroll
+            for (int k = 0; k < AMO_ITEMS; ++k)
+                cur[k] = (ok[k] && v[k] != c[k]) ? ld_relaxed_u64(reinterpret_cast<const unsigned long long *>(addr[k])) : c[k];
+#pragma unroll
+            for (int k = 0; k < AMO_ITEMS; ++k)
+                if (cur[k] != c[k]) {
+                    a.fetched[i0 + lane + (size_t)k * T] = cur[k];
+                    ok[k] = false;
+                }
+        }
 #pragma unroll
         for (int k = 0; k < AMO_ITEMS; ++k) {
             const size_t i = i0 + lane + (size_t)k * T;
@@ -79,6 +94,7 @@ __global__ void __launch_bounds__(256) k_amo(const AmoArgs a) {
                 }
                 continue;
             }
+            if (TEST && !__any_sync(FULL, ok[k])) continue;       // every lane was resolved by the test load
             // ---- warp aggregation: lanes that may not combine get a key no other lane can have ----
             const bool solo = !ok[k] || (OP == AMO_CAS && (cond != nullptr || v[k] == c[k]));
             const unsigned long long key = solo ? (unsigned long long)lane : addr[k];   // real addresses are >= 2^32
@@ -129,12 +145,17 @@ static int launch_amo(shmemg_world *w, const AmoArgs &a, int idx_bytes, uint32_t
     const size_t cap = (size_t)w->sm_count * 8 * 4;        // 8 resident CTAs per SM, ~4 waves worth of grid stride
     if (blocks > cap) blocks = cap;
     const bool agg = flags & SHMEMG_AMO_WARP_AGGREGATE;
+    const bool test = OP == AMO_CAS && (flags & SHMEMG_AMO_TEST_BEFORE_SWAP) && a.cond == nullptr;
     if (idx_bytes == 4) {
-        if (agg) k_amo<4, OP, true><<<(unsigned)blocks, threads, 0, st>>>(a);
-        else k_amo<4, OP, false><<<(unsigned)blocks, threads, 0, st>>>(a);
+        if (test) { if (agg) k_amo<4, OP, true, true><<<(unsigned)blocks, threads, 0, st>>>(a);
+                    else k_amo<4, OP, false, true><<<(unsigned)blocks, threads, 0, st>>>(a); }
+        else if (agg) k_amo<4, OP, true, false><<<(unsigned)blocks, threads, 0, st>>>(a);
+        else k_amo<4, OP, false, false><<<(unsigned)blocks, threads, 0, st>>>(a);
     } else {
-        if (agg) k_amo<8, OP, true><<<(unsigned)blocks, threads, 0, st>>>(a);
-        else k_amo<8, OP, false><<<(unsigned)blocks, threads, 0, st>>>(a);
+        if (test) { if (agg) k_amo<8, OP, true, true><<<(unsigned)blocks, threads, 0, st>>>(a);
+                    else k_amo<8, OP, false, true><<<(unsigned)blocks, threads, 0, st>>>(a); }
+        else if (agg) k_amo<8, OP, true, false><<<(unsigned)blocks, threads, 0, st>>>(a);
+        else k_amo<8, OP, false, false><<<(unsigned)blocks, threads, 0, st>>>(a);
     }
     SHMEMG_CUDA(w, cudaGetLastError());
     return SHMEMG_OK;

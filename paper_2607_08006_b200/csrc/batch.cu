@@ -8,10 +8,10 @@
 //   * one CTA per SM, warp-specialised:
 //       loader  (1 thread)  claims tiles with a global ticket IN BATCH ORDER, waits for the tile's dependencies,
 //                           issues the bulk load (cp.async.bulk global->shared) or hands the tile to the generic
-//                           warps; waits (SIGNAL_WAIT_UNTIL) are polled here;
+//                           warps;
 //       storer  (1 thread)  issues the bulk store (shared->global) when a stage has landed, and when the store has
 //                           completed does the tile's completion accounting (arrival, signal, done counters);
-//       generic (4 warps)   register-path copies and AMO runs.
+//       generic (4 warps)   register-path copies, AMO runs and runs of waits (SIGNAL_WAIT_UNTIL, one per thread).
 //     A claimed tile only ever waits for tiles with smaller tickets, which are finished or held by running CTAs whose
 //     three roles make progress independently: no deadlock and no co-residency requirement;
 //   * ordering state: done[p] = completed ops of PE p, done[npes] = completed ops of all PEs (monotonic, release-
@@ -41,7 +41,7 @@
 #define TRACE_SLOTS 8
 #define TRACE_CTAS 256
 #define TRACE_BYTES (TRACE_CTAS * TRACE_SLOTS * 8)   // per-CTA timestamps (SHMEMG_TRACE=1)
-#define WAIT_RUN_MAX 64u          // consecutive waits of one PE polled by one thread
+#define WAIT_RUN_MAX 128u         // consecutive waits of one PE polled by one tile (one per generic thread)
 
 // tile kinds (bits 0-7 of TileRec.kind); bits 8-15 hold sig_op (put_signal)
 enum { T_TMA = 1, T_COPY = 2, T_AMO = 3, T_WAIT = 4, T_NODATA = 5, T_END = 6 };
@@ -233,23 +233,12 @@ __global__ void __launch_bounds__(EXEC_THREADS, 1) k_batch_exec(const ExecArgs a
                     mbar_arrive_expect_tx(&fullA[s], n);
                     bulk_g2s(stage + (size_t)s * SHMEMG_TMA_TILE, reinterpret_cast<const void *>(r0.src + off), n, &fullA[s]);
                 }
-            } else if (k == T_COPY || k == T_AMO) {
+            } else if (k == T_COPY || k == T_AMO || k == T_WAIT) {   // generic warps (a wait run is polled one wait per thread)
                 const unsigned g = ig % GEN_SLOTS;
                 mbar_wait(&emptyG[g], ((ig / GEN_SLOTS) & 1u) ^ 1u);
                 ringG[g] = r0;
                 mbar_arrive(&fullG[g]);
                 ig++;
-            } else if (k == T_WAIT) {
-                // a run of consecutive waits of one PE, polled in program order by this one thread
-                const AuxRec *wr = reinterpret_cast<const AuxRec *>(r0.src);
-                for (unsigned i = 0; i < r0.nbytes; ++i) {
-                    const unsigned long long *sig = reinterpret_cast<const unsigned long long *>(__ldg(&wr[i].word));
-                    const unsigned long long v = __ldg(&wr[i].value);
-                    const int cmp = (int)((__ldg(&wr[i].kind) >> 8) & 0xff);
-                    while (!cmp_u64(cmp, ld_relaxed_u64(sig), v)) __nanosleep(40);
-                }
-                fence_acquire();
-                count_done(done, ep.npes, r0.kind, r0.initiator);
             } else {                                                 // T_NODATA: zero-byte put/get/put_signal
                 account(r0, done, arrive, ep);
             }
@@ -315,6 +304,15 @@ __global__ void __launch_bounds__(EXEC_THREADS, 1) k_batch_exec(const ExecArgs a
                 copy_coop<4>(reinterpret_cast<uint8_t *>(r.dst), reinterpret_cast<const uint8_t *>(r.src), r.nbytes, gt,
                              GEN_THREADS);
                 if (r.kind & TF_ACCT) __threadfence();
+            } else if (k == T_WAIT) {
+                // a run of consecutive waits of one PE: thread i polls wait i (all must hold; order is immaterial)
+                if (gt < (int)r.nbytes) {
+                    const AuxRec o = ld_rec(reinterpret_cast<const AuxRec *>(r.src) + gt);
+                    const unsigned long long *sig = reinterpret_cast<const unsigned long long *>(o.word);
+                    const int cmp = (int)((o.kind >> 8) & 0xff);
+                    while (!cmp_u64(cmp, ld_relaxed_u64(sig), o.value)) __nanosleep(32);
+                    fence_acquire();
+                }
             } else if (gt < (int)r.nbytes) {
                 const AuxRec o = ld_rec(reinterpret_cast<const AuxRec *>(r.src) + gt);
                 wait_deps(done, ep, o.initiator, o.dep_pe, o.dep_all, o.pe_total);
@@ -324,9 +322,11 @@ __global__ void __launch_bounds__(EXEC_THREADS, 1) k_batch_exec(const ExecArgs a
             named_bar_sync(1, GEN_THREADS);
             if (gt == 0) {
                 if (k == T_COPY) account(r, done, arrive, ep);
+                else if (k == T_WAIT) count_done(done, ep.npes, r.kind, r.initiator);   // release: cumulative over the bar
                 mbar_arrive(&emptyG[g]);
             }
         }
+        if (gt == 0) TRACE(5);
     }
 }
 

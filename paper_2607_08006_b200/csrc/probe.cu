@@ -16,9 +16,11 @@ __global__ void __launch_bounds__(256) k_probe_atomic(uint8_t *base, size_t stri
     unsigned long long acc = 0;
     const size_t T = (size_t)gridDim.x * blockDim.x;
     for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += T) {
+        // uniform over npes x words without integer division (a 64-bit modulo would make the probe ALU-bound):
+        // multiply-high of two independent halves of the hash
         const unsigned long long h = probe_hash(i);
-        const unsigned pe = (unsigned)(h % npes);
-        const unsigned long long wd = (h / npes) % words;
+        const unsigned pe = __umulhi((unsigned)h, npes);
+        const unsigned long long wd = __umul64hi(h ^ (h << 32), words);
         unsigned long long *p = reinterpret_cast<unsigned long long *>(base + (size_t)pe * stride + sym_off) + wd;
         if (MODE == SHMEMG_PROBE_RED_ADD) {
             asm volatile("red.relaxed.gpu.global.add.u64 [%0], %1;" ::"l"(p), "l"(0ull) : "memory");

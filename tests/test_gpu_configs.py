@@ -9,7 +9,7 @@ from gpu_common import DEV, assert_objects_equal, heap_bytes_for, run_gpu, run_o
 from invariants import check_compare_swap_claim, check_fetch_add
 from oracle import oracle as orc
 from paper_2607_08006_b200 import CAP, CMP, ERR, SIGNAL, TEAM, ShmemgError, World
-from paper_2607_08006_b200.binding import AMO_WARP_AGGREGATE, F32, I64
+from paper_2607_08006_b200.binding import AMO_TEST_BEFORE_SWAP, AMO_WARP_AGGREGATE, F32, I64
 from paper_2607_08006_b200.loader import Loaded
 from workloads import configs, gen
 
@@ -139,7 +139,7 @@ def _run_c4(g, flags):
     return degs, pars, f_deg.cpu().numpy().view(np.uint64), f_par.cpu().numpy().view(np.uint64)
 
 
-@pytest.mark.parametrize("flags", [0, AMO_WARP_AGGREGATE])
+@pytest.mark.parametrize("flags", [0, AMO_WARP_AGGREGATE, AMO_TEST_BEFORE_SWAP, AMO_WARP_AGGREGATE | AMO_TEST_BEFORE_SWAP])
 def test_c4_graph_small_full_oracle(flags):
     g = configs.c4_graph(scale=16, edge_factor=16, npes=32)
     degs, pars, f_deg, f_par = _run_c4(g, flags)
@@ -159,10 +159,32 @@ def test_c4_graph_small_full_oracle(flags):
     assert np.isin((pars[claimed] << np.uint64(32)) | claimed.astype(np.uint64), edges).all()   # valid in-neighbours
 
 
+def test_compare_swap_test_before_swap_with_noop_swaps():
+    """SHMEMG_AMO_TEST_BEFORE_SWAP when some ops have val == cond (a swap that leaves the word at cond): those ops go
+    straight to the L2 atomic; per slot the result must still be a legal linearisation of CAS(cond -> val)."""
+    n, slots = 1 << 18, 1 << 10
+    w = World(2, slots * 8 + 4096, DEV)
+    a = w.malloc(slots * 8)
+    w.view(a, slots * 8, torch.int64).fill_(-1)
+    key = (np.arange(n, dtype=np.int64) * 2654435761 % (2 * slots))
+    val = np.arange(1, n + 1, dtype=np.uint64)
+    val[::5] = M64                                                   # no-op swaps
+    f = torch.empty(n, dtype=torch.int64, device=DEV)
+    w.atomic_compare_swap_batch(a, to_dev((key // slots).astype(np.int32)), to_dev((key % slots).astype(np.uint32)), f,
+                                cond=None, cond_scalar=M64, val=to_dev(val), flags=AMO_TEST_BEFORE_SWAP)
+    w.quiet(0)
+    fin = w.view(a, slots * 8, torch.int64).cpu().numpy().view(np.uint64).reshape(-1)
+    fet = f.cpu().numpy().view(np.uint64)
+    real = val != M64
+    # ops that really swap obey the claim invariant among themselves; a no-op swap fetched cond or the final value
+    check_compare_swap_claim(key[real], val[real], fet[real], fin)
+    assert ((fet[~real] == M64) | (fet[~real] == fin[key[~real]])).all()
+
+
 def test_c4_graph_full_scale():
     """Config 4 at its full size (RMAT scale 22, 2^26 edges, 32 PEs) in the launch configuration bench.py times."""
     g = configs.c4_graph()
-    degs, pars, f_deg, f_par = _run_c4(g, AMO_WARP_AGGREGATE)
+    degs, pars, f_deg, f_par = _run_c4(g, AMO_TEST_BEFORE_SWAP)
     E = len(g.u)
     assert np.array_equal(degs, np.bincount(g.u, minlength=1 << 22).astype(np.uint64))   # = the oracle's pinned closed form
     ow = orc.OracleWorld(g.npes, g.verts_per_pe * 8 + 512)                           # oracle degrees, sequentially
