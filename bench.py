@@ -162,8 +162,8 @@ def segment_table(inp: Inputs):
                                            bytes=HALO_ROUNDS * 2 * 48 * inp.halo.face_bytes, launches=HALO_ROUNDS)
     if "c5" in g:
         n, nb = inp.c5_npes, inp.c5_bytes
-        seg["sum_reduce_f32"] = dict(cls="copy", kernel="k_sum_reduce_f32", bytes=2 * n * nb, launches=1)
-        seg["sum_reduce_i64"] = dict(cls="copy", kernel="k_sum_reduce_i64", bytes=2 * n * nb, launches=1)
+        seg["sum_reduce_f32"] = dict(cls="copy", kernel="k_sum_reduce_tma<f32>", bytes=2 * n * nb, launches=1)
+        seg["sum_reduce_i64"] = dict(cls="copy", kernel="k_sum_reduce_tma<i64>", bytes=2 * n * nb, launches=1)
         seg["fcollect"] = dict(cls="copy", kernel="k_fcollect_tma",
                                bytes=n * inp.c5_fc_bytes + n * n * inp.c5_fc_bytes, launches=1)
     if "c1" in g:

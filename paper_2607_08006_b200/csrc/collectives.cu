@@ -1,7 +1,8 @@
 // collectives.cu -- world-team collectives, one kernel each.
 //   alltoall   : tiled transpose-copy, 128-bit streaming accesses; HBM-bound, 2*N*N*blk bytes
 //   fcollect   : each source chunk is read once into registers and stored to all N destinations (write-bound)
-//   sum_reduce : one pass down the N windows per column group, fp64 accumulation for fp32, N-way replicated store
+//   sum_reduce : bulk-copy pipeline per column tile: N windows streamed through shared memory, fp64 accumulation for
+//                fp32 in ascending PE order, N-way replicated bulk store
 //   barrier    : stream-level (kernel boundary) and in-kernel (one CTA per PE, cooperative launch)
 #include "tma_stream.cuh"
 
@@ -136,67 +137,136 @@ k_fcollect_bytes(uint8_t *base, size_t stride, uint64_t dst_off, uint64_t src_of
     }
 }
 
-// ---- sum_reduce ----------------------------------------------------------------------------------------------------
-// Each thread owns one 16-byte column group (4 fp32 or 2 int64), walks the N windows in ascending PE order with
-// PEU loads in flight, then stores the result vector to all N destinations.
-#define PEU 8
-__global__ void __launch_bounds__(SHMEMG_THREADS)
-k_sum_reduce_f32(uint8_t *base, size_t stride, uint64_t dst_off, uint64_t src_off, size_t nvec, int npes) {
-    for (size_t k = (size_t)blockIdx.x * blockDim.x + threadIdx.x; k < nvec; k += (size_t)gridDim.x * blockDim.x) {
-        const uint8_t *s = base + src_off + (k << 4);
-        double a0 = 0.0, a1 = 0.0, a2 = 0.0, a3 = 0.0;
-        int p = 0;
-        for (; p + PEU <= npes; p += PEU) {
-            int4 v[PEU];
-#pragma unroll
-            for (int u = 0; u < PEU; ++u) v[u] = ld_stream16(s + (size_t)(p + u) * stride);
-#pragma unroll
-            for (int u = 0; u < PEU; ++u) {       // ascending PE order, fp64 accumulate (reading 13)
-                a0 += (double)__int_as_float(v[u].x);
-                a1 += (double)__int_as_float(v[u].y);
-                a2 += (double)__int_as_float(v[u].z);
-                a3 += (double)__int_as_float(v[u].w);
-            }
-        }
-        for (; p < npes; ++p) {
-            const int4 v = ld_stream16(s + (size_t)p * stride);
-            a0 += (double)__int_as_float(v.x); a1 += (double)__int_as_float(v.y);
-            a2 += (double)__int_as_float(v.z); a3 += (double)__int_as_float(v.w);
-        }
-        int4 r;
-        r.x = __float_as_int(__double2float_rn(a0)); r.y = __float_as_int(__double2float_rn(a1));
-        r.z = __float_as_int(__double2float_rn(a2)); r.w = __float_as_int(__double2float_rn(a3));
-        uint8_t *d = base + dst_off + (k << 4);
-#pragma unroll 8
-        for (int j = 0; j < npes; ++j) st_stream16(d + (size_t)j * stride, r);
+// ---- sum_reduce, bulk-copy pipeline (offsets, stride 16-byte aligned) ---------------------------------------------------
+// Work item = one column tile of RT bytes across all N windows.  Warp-specialised, one CTA per SM:
+//   loader  (warp 0, lane 0) streams the tile of PE 0, 1, ... N-1 into a ring of RS stages (RG PEs per stage, one
+//                            mbarrier transaction per stage), RS*RG*RT = 128 KiB in flight per SM, no registers;
+//   reducers (8 warps)       thread t owns the 16 bytes at offset 16t of the tile: it adds the stages in ascending PE
+//                            order (fp64 accumulators for fp32, reading 13), then writes the rounded result into one of
+//                            two shared output tiles;
+//   storer  (warp 1)         lane l bulk-stores the output tile to the windows l, l+32, ...; the tile is reused when its
+//                            stores have finished reading it, so the next item's reduction overlaps the N-way store.
+#ifndef RV
+#define RV 1                                  // 16-byte vectors per reducer thread and tile
+#endif
+#ifndef RG
+#define RG 4
+#endif
+#ifndef RS
+#define RS 8
+#endif
+#define RED_THREADS 256
+#define RT (RED_THREADS * 16u * RV)            // tile bytes per PE
+#define RED_CTA (64 + RED_THREADS)
+#define RED_SMEM ((size_t)RS * RG * RT + 2 * RT)
+
+template <int DT>
+__global__ void __launch_bounds__(RED_CTA, 1)
+k_sum_reduce_tma(uint8_t *base, size_t stride, uint64_t dst_off, uint64_t src_off, size_t nbytes, int npes) {
+    extern __shared__ __align__(1024) uint8_t smem[];
+    __shared__ uint64_t full[RS], empty[RS], out_full[2], out_empty[2];
+    uint8_t *out = smem + (size_t)RS * RG * RT;
+    const int tid = threadIdx.x;
+    const size_t ntiles = (nbytes + RT - 1) / RT;
+    const int ngroups = (npes + RG - 1) / RG;
+    if (tid == 0) {
+        for (int s = 0; s < RS; ++s) { mbar_init(&full[s], 1); mbar_init(&empty[s], RED_THREADS / 32); }
+        for (int b = 0; b < 2; ++b) { mbar_init(&out_full[b], RED_THREADS / 32); mbar_init(&out_empty[b], 1); }
+        mbar_init_fence();
     }
-}
-__global__ void __launch_bounds__(SHMEMG_THREADS)
-k_sum_reduce_i64(uint8_t *base, size_t stride, uint64_t dst_off, uint64_t src_off, size_t nvec, int npes) {
-    for (size_t k = (size_t)blockIdx.x * blockDim.x + threadIdx.x; k < nvec; k += (size_t)gridDim.x * blockDim.x) {
-        const uint8_t *s = base + src_off + (k << 4);
-        unsigned long long a0 = 0, a1 = 0;
-        int p = 0;
-        for (; p + PEU <= npes; p += PEU) {
-            int4 v[PEU];
-#pragma unroll
-            for (int u = 0; u < PEU; ++u) v[u] = ld_stream16(s + (size_t)(p + u) * stride);
-#pragma unroll
-            for (int u = 0; u < PEU; ++u) {
-                a0 += ((unsigned long long)(unsigned)v[u].y << 32) | (unsigned)v[u].x;
-                a1 += ((unsigned long long)(unsigned)v[u].w << 32) | (unsigned)v[u].z;
+    __syncthreads();
+    if (tid == 0) {
+        // ---- loader ----
+        unsigned it = 0;
+        for (size_t c = blockIdx.x; c < ntiles; c += gridDim.x) {
+            const size_t off = c * RT;
+            const unsigned tb = (unsigned)(nbytes - off < RT ? nbytes - off : RT);
+            const uint8_t *s0 = base + src_off + off;
+            for (int g = 0; g < ngroups; ++g, ++it) {
+                const unsigned s = it % RS;
+                mbar_wait(&empty[s], ((it / RS) & 1u) ^ 1u);
+                const int p0 = g * RG, cnt = min(RG, npes - p0);
+                mbar_arrive_expect_tx(&full[s], tb * cnt);
+                for (int j = 0; j < cnt; ++j)
+                    bulk_g2s(smem + ((size_t)s * RG + j) * RT, s0 + (size_t)(p0 + j) * stride, tb, &full[s]);
             }
         }
-        for (; p < npes; ++p) {
-            const int4 v = ld_stream16(s + (size_t)p * stride);
-            a0 += ((unsigned long long)(unsigned)v.y << 32) | (unsigned)v.x;
-            a1 += ((unsigned long long)(unsigned)v.w << 32) | (unsigned)v.z;
+    } else if (tid >= 32 && tid < 64) {
+        // ---- storer ----
+        const int lane = tid - 32;
+        unsigned k = 0;
+        for (size_t c = blockIdx.x; c < ntiles; c += gridDim.x, ++k) {
+            const unsigned b = k & 1u;
+            const size_t off = c * RT;
+            const unsigned tb = (unsigned)(nbytes - off < RT ? nbytes - off : RT);
+            mbar_wait(&out_full[b], (k >> 1) & 1u);
+            for (int p = lane; p < npes; p += 32) bulk_s2g(base + (size_t)p * stride + dst_off + off, out + (size_t)b * RT, tb);
+            bulk_commit();
+            if (k >= 1) {                       // the previous item's stores (other tile) have read their tile
+                bulk_wait_read<1>();
+                __syncwarp();
+                if (lane == 0) mbar_arrive(&out_empty[b ^ 1u]);
+            }
         }
-        int4 r;
-        r.x = (int)(unsigned)a0; r.y = (int)(unsigned)(a0 >> 32); r.z = (int)(unsigned)a1; r.w = (int)(unsigned)(a1 >> 32);
-        uint8_t *d = base + dst_off + (k << 4);
-#pragma unroll 8
-        for (int j = 0; j < npes; ++j) st_stream16(d + (size_t)j * stride, r);
+        bulk_wait<0>();
+    } else if (tid >= 64) {
+        // ---- reducers ----
+        const int t = tid - 64, lane = t & 31;
+        unsigned it = 0, k = 0;
+        for (size_t c = blockIdx.x; c < ntiles; c += gridDim.x, ++k) {
+            const size_t off = c * RT;
+            const unsigned tb = (unsigned)(nbytes - off < RT ? nbytes - off : RT);
+            double acc[RV][4];
+            unsigned long long ui[RV][2];
+#pragma unroll
+            for (int v = 0; v < RV; ++v) { acc[v][0] = acc[v][1] = acc[v][2] = acc[v][3] = 0.0; ui[v][0] = ui[v][1] = 0; }
+            for (int g = 0; g < ngroups; ++g, ++it) {
+                const unsigned s = it % RS;
+                mbar_wait(&full[s], (it / RS) & 1u);
+                const int cnt = min(RG, npes - g * RG);
+#pragma unroll
+                for (int j = 0; j < RG; ++j) {
+                    if (j < cnt) {
+#pragma unroll
+                        for (int v = 0; v < RV; ++v) {
+                            const unsigned o = ((unsigned)v * RED_THREADS + (unsigned)t) * 16u;
+                            if (o < tb) {
+                                const int4 x = *reinterpret_cast<const int4 *>(smem + ((size_t)s * RG + j) * RT + o);
+                                if (DT == SHMEMG_F32) {       // ascending PE order, fp64 accumulate (reading 13)
+                                    acc[v][0] += (double)__int_as_float(x.x); acc[v][1] += (double)__int_as_float(x.y);
+                                    acc[v][2] += (double)__int_as_float(x.z); acc[v][3] += (double)__int_as_float(x.w);
+                                } else {
+                                    ui[v][0] += ((unsigned long long)(unsigned)x.y << 32) | (unsigned)x.x;
+                                    ui[v][1] += ((unsigned long long)(unsigned)x.w << 32) | (unsigned)x.z;
+                                }
+                            }
+                        }
+                    }
+                }
+                __syncwarp();
+                if (lane == 0) mbar_arrive(&empty[s]);
+            }
+            const unsigned b = k & 1u;
+            if (k >= 2) mbar_wait(&out_empty[b], ((k >> 1) - 1u) & 1u);
+#pragma unroll
+            for (int v = 0; v < RV; ++v) {
+                const unsigned o = ((unsigned)v * RED_THREADS + (unsigned)t) * 16u;
+                if (o < tb) {
+                    int4 r;
+                    if (DT == SHMEMG_F32) {
+                        r.x = __float_as_int(__double2float_rn(acc[v][0])); r.y = __float_as_int(__double2float_rn(acc[v][1]));
+                        r.z = __float_as_int(__double2float_rn(acc[v][2])); r.w = __float_as_int(__double2float_rn(acc[v][3]));
+                    } else {
+                        r.x = (int)(unsigned)ui[v][0]; r.y = (int)(unsigned)(ui[v][0] >> 32);
+                        r.z = (int)(unsigned)ui[v][1]; r.w = (int)(unsigned)(ui[v][1] >> 32);
+                    }
+                    *reinterpret_cast<int4 *>(out + (size_t)b * RT + o) = r;
+                }
+            }
+            asm volatile("fence.proxy.async.shared::cta;" ::: "memory");    // generic writes -> visible to the bulk store
+            __syncwarp();
+            if (lane == 0) mbar_arrive(&out_full[b]);
+        }
     }
 }
 // scalar tails / unaligned buffers: one element per thread
@@ -259,6 +329,8 @@ static int collectives_smem_attr(shmemg_world *w) {
     if (w->smem_attr_coll) return SHMEMG_OK;
     SHMEMG_CUDA(w, cudaFuncSetAttribute(k_alltoall_tma, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SHMEMG_TMA_SMEM));
     SHMEMG_CUDA(w, cudaFuncSetAttribute(k_fcollect_tma, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SHMEMG_TMA_SMEM));
+    SHMEMG_CUDA(w, cudaFuncSetAttribute(k_sum_reduce_tma<SHMEMG_F32>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)RED_SMEM));
+    SHMEMG_CUDA(w, cudaFuncSetAttribute(k_sum_reduce_tma<SHMEMG_I64>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)RED_SMEM));
     w->smem_attr_coll = true;
     return SHMEMG_OK;
 }
@@ -348,13 +420,14 @@ extern "C" int shmemg_sum_reduce_on_stream(shmemg_world_t *w, int dtype, uint64_
     const size_t nvec = vec_ok ? tot >> 4 : 0;
     const size_t per_vec = 16 / esz;
     if (nvec) {
-        size_t blocks = (nvec + SHMEMG_THREADS - 1) / SHMEMG_THREADS;
-        const size_t cap = (size_t)w->sm_count * 8 * 8;
-        if (blocks > cap) blocks = cap;
+        int rc = collectives_smem_attr(w);
+        if (rc) return rc;
+        const size_t nb = nvec << 4, ntiles = (nb + RT - 1) / RT;
+        const unsigned grid = (unsigned)(ntiles < (size_t)w->sm_count ? ntiles : (size_t)w->sm_count);
         if (dtype == SHMEMG_F32)
-            k_sum_reduce_f32<<<(unsigned)blocks, SHMEMG_THREADS, 0, st>>>(w->base, w->stride, dest_off, source_off, nvec, w->npes);
+            k_sum_reduce_tma<SHMEMG_F32><<<grid, RED_CTA, RED_SMEM, st>>>(w->base, w->stride, dest_off, source_off, nb, w->npes);
         else
-            k_sum_reduce_i64<<<(unsigned)blocks, SHMEMG_THREADS, 0, st>>>(w->base, w->stride, dest_off, source_off, nvec, w->npes);
+            k_sum_reduce_tma<SHMEMG_I64><<<grid, RED_CTA, RED_SMEM, st>>>(w->base, w->stride, dest_off, source_off, nb, w->npes);
         SHMEMG_CUDA(w, cudaGetLastError());
     }
     const size_t first = nvec * per_vec;

@@ -295,7 +295,8 @@ def test_c5_sum_reduce_fcollect_barrier_full_size():
     assert (sv[:, 0] == 10000).all() and (sv[:, 1] == 9999).all()
 
 
-@pytest.mark.parametrize("npes,n,off", [(3, 1, 0), (5, 1001, 4), (9, 4097, 8), (4, 4099, 0), (2, 70000, 0)])
+@pytest.mark.parametrize("npes,n,off", [(3, 1, 0), (5, 1001, 4), (9, 4097, 8), (4, 4099, 0), (2, 70000, 0), (7, 700001, 0),
+                                        (33, 150001, 16)])
 def test_sum_reduce_fcollect_ragged(npes, n, off):
     hb = 8 * n * (npes + 2) + 16384
     w = World(npes, hb, DEV)
