@@ -45,9 +45,17 @@ HALO_ROUNDS = 50
 BARRIERS = 10000
 M64 = (1 << 64) - 1
 
-# dram__bytes_read.sum + dram__bytes_write.sum per launch from the `ncu --set full` capture summarised in
-# profiles/ (file named in each entry); None until a capture of that kernel exists.
-NCU_TRAFFIC = {}
+# dram__bytes_read.sum + dram__bytes_write.sum per launch of each copy-class segment's kernel, from the `ncu --set full`
+# captures summarised in profiles/r01b_ncu_full.md (cold L2 at launch, up to 126 MB of the kernel's own writes still in
+# L2 at its end, so write traffic < algorithmic writes; the halo faces are L2-resident by nature).
+NCU_TRAFFIC = {
+    "alltoall": 268449024 + 221673728,
+    "put_batch_skewed": 198664960 + 151857152,
+    "halo_put_signal_wait": 25207296 + 120064,
+    "sum_reduce_f32": 536885760 + 478708224,
+    "sum_reduce_i64": 536973312 + 479942656,
+    "fcollect": 4599552 + 477103872,
+}
 
 
 def parse_args():
@@ -743,14 +751,17 @@ def run_cuda(args):
     if copy_names:
         by_kernel = {}
         for k in copy_names:
-            e = by_kernel.setdefault(table[k]["kernel"], [0.0, 0, 0])
+            e = by_kernel.setdefault(table[k]["kernel"], [0.0, 0, 0, 0, True])
             e[0] += secs[k]; e[1] += units[k] // world; e[2] += table[k]["launches"] * K
+            e[3] += NCU_TRAFFIC.get(k, 0) * table[k]["launches"] * K
+            e[4] = e[4] and k in NCU_TRAFFIC
         kern = max(by_kernel, key=lambda x: by_kernel[x][0])
-        s, b, nl = by_kernel[kern]
+        s, b, nl, tr, tr_ok = by_kernel[kern]
         roofline = {"bound": "hbm", "kernel": kern, "achieved": b / s / 1e9, "peak": peak, "unit": "GB/s",
                     "frac": b / s / 1e9 / peak, "peak_source": peak_src, "share_of_copy_time": s / copy_s,
                     "algorithmic_bytes_per_launch": b // nl, "avg_launch_us": s / nl * 1e6,
-                    "traffic": NCU_TRAFFIC.get(kern)}
+                    "traffic": (tr // nl) if tr_ok and not inp.small else None,
+                    "traffic_source": "profiles/r01b_ncu_full.md (launch-weighted mean over the kernel's segments)"}
 
     line = base_line(args, world)
     line.update({"value": gbps, "amo_mops": mops, "ms_per_step": whole_ms / K,
