@@ -71,7 +71,7 @@ enum {
 #define SHMEMG_CAP_HOST_INITIATED_GPU_BUFFERS (1ull << 2)   /* Tier-0 baseline (L465)                    */
 #define SHMEMG_CAP_STREAM_TRIGGERED           (1ull << 3)   /* _on_stream variants (L396, L412)          */
 #define SHMEMG_CAP_DEVICE_INITIATED           (1ull << 4)   /* __device__ entry points (L412, L465)      */
-#define SHMEMG_CAP_DEVICE_COLLECTIVES         (1ull << 5)   /* 0 in this build                           */
+#define SHMEMG_CAP_DEVICE_COLLECTIVES         (1ull << 5)   /* 0: no device alltoall/reduce/fcollect     */
 #define SHMEMG_CAP_EXPLICIT_DEVICE_CTX        (1ull << 6)   /* 0 in this build                           */
 #define SHMEMG_CAP_PTR_DEVICE_ACCESSIBLE      (1ull << 7)   /* shmemg_ptr is a device pointer (L353)     */
 #define SHMEMG_CAP_PTR_HOST_ACCESSIBLE        (1ull << 8)   /* 0: not dereferenceable on the host (L456) */
@@ -79,6 +79,7 @@ enum {
 #define SHMEMG_CAP_PATH_DIRECT                (1ull << 10)  /* direct load/store path (L431)             */
 #define SHMEMG_CAP_ATOMICS_64                 (1ull << 11)  /* add / fetch-add / compare-swap on 64 bit  */
 #define SHMEMG_CAP_STREAM_COLLECTIVES         (1ull << 12)  /* barrier/alltoall/fcollect/reduce on stream */
+#define SHMEMG_CAP_DEVICE_BARRIER             (1ull << 13)  /* shmemg_dev_barrier_all_block only (L363)  */
 
 /* ---- lifecycle ------------------------------------------------------------------------------------ */
 
@@ -258,6 +259,32 @@ SHMEMG_API int shmemg_barrier_all_on_stream(shmemg_world_t *w, void *stream);
 SHMEMG_API int shmemg_barrier_all_repeat_on_stream(shmemg_world_t *w, uint32_t count, uint64_t stamp_off,
                                                    void *stream);
 SHMEMG_API uint64_t shmemg_barrier_epoch(shmemg_world_t *w, void *stream);   /* synchronises `stream` */
+
+/* ---- device-initiated path (Tier-1) ---------------------------------------------------
+ * include/shmemg_device.cuh holds header-only `__device__` entry points (put/get/put_signal/wait/test/AMOs/fence/quiet
+ * at thread, warp and block scope, and a block-scope barrier_all).  A kernel that uses them takes this POD BY VALUE. */
+typedef struct shmemg_device_world {
+    unsigned char *base;        /* DEVICE: window of PE 0                                                     */
+    uint64_t stride;            /* distance between PE windows: address(pe, off) = base + pe*stride + off     */
+    uint64_t heap_bytes;        /* usable bytes per PE                                                        */
+    int32_t npes;
+    int32_t reserved;
+    unsigned int *bar_count;    /* DEVICE: device-barrier arrival counter (control region)                    */
+    unsigned int *bar_gen;      /* DEVICE: device-barrier generation                                          */
+} shmemg_device_world_t;
+/* Fill *out (HOST) for world w; valid until shmemg_finalize. */
+SHMEMG_API int shmemg_device_world_get(const shmemg_world_t *w, shmemg_device_world_t *out);
+
+/* Run an op list DEVICE-INITIATED: one cooperative kernel with one thread block per PE ("PE agent"); agent p walks
+ * ops[0..nops) in order and executes those it initiates through the entry points of shmemg_device.cuh with BLOCKING
+ * semantics: put/get/put_signal at block scope, AMOs and fetch-slot stores by one thread, SIGNAL_WAIT_UNTIL
+ * blocks the agent, FENCE/QUIET = shmemg_dev_quiet_block, BARRIER_ALL = shmemg_dev_barrier_all_block (executed by every
+ * agent).  Same requirement as a batch: index order is a valid sequential schedule.  `ops_host` (HOST, nops entries) is
+ * validated like shmemg_batch_create (error code returned, *bad_index set) and copied to `ops_dev` (DEVICE, >= 64*nops
+ * bytes, caller-owned, must stay valid until the stream has passed the call) on `stream`.  Returns SHMEMG_ERR_NOMEM if
+ * npes thread blocks cannot be co-resident on the device (progress would not be guaranteed). */
+SHMEMG_API int shmemg_device_exec_ops_on_stream(shmemg_world_t *w, const shmemg_op_t *ops_host, size_t nops, void *ops_dev,
+                                                void *stream, size_t *bad_index);
 
 #ifdef __cplusplus
 }

@@ -1,0 +1,262 @@
+/*
+ * shmemg_device.cuh -- DEVICE-INITIATED entry points (Tier-1) of the B200-native GPU-aware OpenSHMEM hot path.
+ *
+ * Header-only `__device__` functions for CUDA kernels compiled for sm_100a.  They are the device-side counterparts
+ * of the `_on_stream` routines of shmemg.h: "device-initiated communication [is] invoked from GPU kernels"
+ * (PAPER L142, L271, L465-L466), uses the default device context (`SHMEM_DEVICE_CTX_DEFAULT`: "device
+ * code that omits an explicit context uses" it) and the world team (`SHMEM_DEVICE_TEAM_WORLD`, L194, L357).
+ *
+ * Model
+ *   - The kernel receives a `shmemg_device_world_t` BY VALUE (filled on the host by shmemg_device_world_get); it holds
+ *     the slab base, the window stride and the npes of the world: PE -> address translation is
+ *     base + pe*stride + off, two integer operations and no pointer classification in device code (L351).
+ *   - All N PEs share the GPU, so every routine takes the initiating PE `pe` explicitly, like the host API.
+ *     Operands are symmetric offsets (L287, L355); AMO values are immediates.
+ *   - THREAD COLLABORATION: a routine without suffix is called by ONE thread and acts
+ *     for it alone; `_warp` / `_block` routines must be called by ALL threads of the warp / thread block with the
+ *     same arguments ("uniform participation"), they share the work and return to all of them.  Mixing scopes on
+ *     one operation, or divergent participation, is undefined (L371).
+ *   - COMPLETION (L367-L369): put/get return on LOCAL completion (the source may be reused; a get's data may be
+ *     read by the calling thread / after the routine's closing barrier by the calling group).  Remote visibility and
+ *     ordering need shmemg_dev_fence / shmemg_dev_quiet (L377: "GPU implementations may use weaker default ordering,
+ *     provided fence and quiet restore ordering").  "Atomicity does not imply ordering" (L365).
+ *   - put_signal: the signal word update is atomic w.r.t. other signal updates and waits and becomes visible only
+ *     after the whole payload (release at GPU scope; L218, L461).  signal_wait_until polls with acquire semantics.
+ *   - barrier_all_block is a DEVICE COLLECTIVE: it needs one participating thread block per PE, all co-resident
+ *     (cooperative launch) -- progress of a spinning kernel is otherwise not guaranteed (L214, L394, L477).
+ *   - Host visibility of device-initiated updates still needs host-side synchronisation of the stream (L388-L390).
+ *   - Errors: none are reported on the device; out-of-range PEs/offsets and misaligned AMO words are undefined
+ *     behaviour (L435).
+ */
+#ifndef SHMEMG_DEVICE_CUH
+#define SHMEMG_DEVICE_CUH
+
+#include "shmemg.h"
+
+#if defined(__CUDACC__)
+
+/* ---- address translation (shmem_ptr analog on the device) ------------------------------------ */
+__device__ __forceinline__ unsigned char *shmemg_dev_ptr(const shmemg_device_world_t &w, uint64_t sym_off, int pe) {
+    return w.base + (size_t)pe * w.stride + sym_off;
+}
+__device__ __forceinline__ int shmemg_dev_n_pes(const shmemg_device_world_t &w) { return w.npes; }
+
+/* ---- memory-model primitives (GPU scope) ------------------------------------------------------------------------ */
+__device__ __forceinline__ void shmemg_dev_fence_gpu() { asm volatile("fence.acq_rel.gpu;" ::: "memory"); }
+__device__ __forceinline__ unsigned long long shmemg_dev_ld_relaxed(const unsigned long long *p) {
+    unsigned long long v;
+    asm volatile("ld.relaxed.gpu.global.u64 %0, [%1];" : "=l"(v) : "l"(p) : "memory");
+    return v;
+}
+__device__ __forceinline__ bool shmemg_dev_cmp(int cmp, unsigned long long s, unsigned long long v) {
+    switch (cmp) {
+    case SHMEMG_CMP_EQ: return s == v;
+    case SHMEMG_CMP_NE: return s != v;
+    case SHMEMG_CMP_GT: return s > v;
+    case SHMEMG_CMP_GE: return s >= v;
+    case SHMEMG_CMP_LT: return s < v;
+    default: return s <= v;
+    }
+}
+
+/* ---- cooperative copy: threads tid in [0, nthr) move n bytes, any alignment ------------------------------------
+ * Every naturally aligned 1/2/4/8/16-byte unit that both addresses allow is moved by ONE access of that width, so an
+ * aligned 8-byte put used as a flag is never torn.  Loads bypass L1 (coherent at L2). */
+template <typename T>
+__device__ __forceinline__ void shmemg_dev_copy_elems(unsigned char *d, const unsigned char *s, size_t nel, int tid, int nthr) {
+    T *dd = reinterpret_cast<T *>(d);
+    const volatile T *ss = reinterpret_cast<const volatile T *>(s);
+    for (size_t i = tid; i < nel; i += nthr) dd[i] = ss[i];
+}
+__device__ __forceinline__ void shmemg_dev_copy_w(unsigned char *d, const unsigned char *s, size_t n, unsigned W, int tid, int nthr) {
+    switch (W) {
+    case 8: shmemg_dev_copy_elems<unsigned long long>(d, s, n >> 3, tid, nthr); break;
+    case 4: shmemg_dev_copy_elems<unsigned int>(d, s, n >> 2, tid, nthr); break;
+    case 2: shmemg_dev_copy_elems<unsigned short>(d, s, n >> 1, tid, nthr); break;
+    default: shmemg_dev_copy_elems<unsigned char>(d, s, n, tid, nthr); break;
+    }
+}
+__device__ __forceinline__ void shmemg_dev_copy(unsigned char *dst, const unsigned char *src, size_t n, int tid, int nthr) {
+    if (n == 0) return;
+    const uintptr_t da = reinterpret_cast<uintptr_t>(dst), sa = reinterpret_cast<uintptr_t>(src);
+    const unsigned both = (unsigned)((da | sa) & 15u);
+    /* W = widest power of two (<= 16) dividing both addresses */
+    unsigned W = both == 0 ? 16u : (both & (0u - both));
+    if (W < 16u && ((da ^ sa) & 15u) == 0 && n >= 32) {
+        /* congruent mod 16: a short W-wide head reaches 16-byte alignment, then the vector body below */
+        const size_t head = (16u - (unsigned)(da & 15u)) & 15u;
+        shmemg_dev_copy_w(dst, src, head, W, tid, nthr);
+        dst += head; src += head; n -= head;
+        W = 16u;
+    }
+    size_t body;
+    if (W == 16u) {
+        body = n & ~(size_t)15;
+        int4 *d4 = reinterpret_cast<int4 *>(dst);
+        const int4 *s4 = reinterpret_cast<const int4 *>(src);
+        for (size_t i = tid; i < (body >> 4); i += nthr) {
+            int4 v;
+            asm volatile("ld.global.cg.v4.s32 {%0,%1,%2,%3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "l"(s4 + i));
+            d4[i] = v;
+        }
+    } else {
+        body = n & ~(size_t)(W - 1u);
+        shmemg_dev_copy_w(dst, src, body, W, tid, nthr);
+    }
+    /* tail < W bytes: aligned to W at its start, so 8/4/2/1-byte units in descending order stay naturally aligned */
+    size_t off = body, left = n - body;
+    for (unsigned u = 8; u >= 1; u >>= 1) {
+        if (u < W && left >= u) {
+            if (tid == 0) shmemg_dev_copy_w(dst + off, src + off, u, u, 0, 1);
+            off += u; left -= u;
+        }
+    }
+}
+
+/* ---- put / get: thread, warp and block scope ---------------------------------------------------------
+ * put: heap[target_pe][dest_off ..] = heap[pe][source_off ..];  get: heap[pe][dest_off ..] = heap[target_pe][source_off ..] */
+__device__ __forceinline__ void shmemg_dev_put(const shmemg_device_world_t &w, uint64_t dest_off, uint64_t source_off,
+                                               size_t nbytes, int pe, int target_pe) {
+    shmemg_dev_copy(shmemg_dev_ptr(w, dest_off, target_pe), shmemg_dev_ptr(w, source_off, pe), nbytes, 0, 1);
+}
+__device__ __forceinline__ void shmemg_dev_get(const shmemg_device_world_t &w, uint64_t dest_off, uint64_t source_off,
+                                               size_t nbytes, int pe, int target_pe) {
+    shmemg_dev_copy(shmemg_dev_ptr(w, dest_off, pe), shmemg_dev_ptr(w, source_off, target_pe), nbytes, 0, 1);
+}
+__device__ __forceinline__ void shmemg_dev_put_warp(const shmemg_device_world_t &w, uint64_t dest_off, uint64_t source_off,
+                                                    size_t nbytes, int pe, int target_pe) {
+    shmemg_dev_copy(shmemg_dev_ptr(w, dest_off, target_pe), shmemg_dev_ptr(w, source_off, pe), nbytes, threadIdx.x & 31, 32);
+    __syncwarp();
+}
+__device__ __forceinline__ void shmemg_dev_get_warp(const shmemg_device_world_t &w, uint64_t dest_off, uint64_t source_off,
+                                                    size_t nbytes, int pe, int target_pe) {
+    shmemg_dev_copy(shmemg_dev_ptr(w, dest_off, pe), shmemg_dev_ptr(w, source_off, target_pe), nbytes, threadIdx.x & 31, 32);
+    __syncwarp();
+}
+__device__ __forceinline__ int shmemg_dev_block_tid() {
+    return (int)(threadIdx.x + blockDim.x * (threadIdx.y + blockDim.y * threadIdx.z));
+}
+__device__ __forceinline__ int shmemg_dev_block_size() { return (int)(blockDim.x * blockDim.y * blockDim.z); }
+__device__ __forceinline__ void shmemg_dev_put_block(const shmemg_device_world_t &w, uint64_t dest_off, uint64_t source_off,
+                                                     size_t nbytes, int pe, int target_pe) {
+    shmemg_dev_copy(shmemg_dev_ptr(w, dest_off, target_pe), shmemg_dev_ptr(w, source_off, pe), nbytes,
+                    shmemg_dev_block_tid(), shmemg_dev_block_size());
+    __syncthreads();
+}
+__device__ __forceinline__ void shmemg_dev_get_block(const shmemg_device_world_t &w, uint64_t dest_off, uint64_t source_off,
+                                                     size_t nbytes, int pe, int target_pe) {
+    shmemg_dev_copy(shmemg_dev_ptr(w, dest_off, pe), shmemg_dev_ptr(w, source_off, target_pe), nbytes,
+                    shmemg_dev_block_tid(), shmemg_dev_block_size());
+    __syncthreads();
+}
+
+/* ---- ordering: fence orders, quiet completes; here both are one GPU-scope fence ------------------
+ * Stores and atomics issued by the calling thread before the call are visible at GPU scope before anything it
+ * issues afterwards (the strong reading of L377: all targets, gets and atomics included).  The `_block` forms are
+ * for the block-scope put/get above: every thread of the block fences its own share, then the block synchronises, so
+ * that whatever ANY thread of the block issues afterwards is ordered after the whole block's earlier operations. */
+__device__ __forceinline__ void shmemg_dev_fence() { shmemg_dev_fence_gpu(); }
+__device__ __forceinline__ void shmemg_dev_quiet() { shmemg_dev_fence_gpu(); }
+__device__ __forceinline__ void shmemg_dev_fence_warp() { shmemg_dev_fence_gpu(); __syncwarp(); }
+__device__ __forceinline__ void shmemg_dev_quiet_warp() { shmemg_dev_fence_gpu(); __syncwarp(); }
+__device__ __forceinline__ void shmemg_dev_fence_block() { shmemg_dev_fence_gpu(); __syncthreads(); }
+__device__ __forceinline__ void shmemg_dev_quiet_block() { shmemg_dev_fence_gpu(); __syncthreads(); }
+
+/* ---- signals ----------------------------------------------------------------------------- */
+__device__ __forceinline__ void shmemg_dev_signal_update(unsigned long long *sig, uint64_t value, int sig_op) {
+    if (sig_op == SHMEMG_SIGNAL_ADD)
+        asm volatile("red.release.gpu.global.add.u64 [%0], %1;" ::"l"(sig), "l"(value) : "memory");
+    else
+        asm volatile("{ .reg .b64 t; atom.release.gpu.global.exch.b64 t, [%0], %1; }" ::"l"(sig), "l"(value) : "memory");
+}
+/* thread scope: payload by the calling thread, then the signal with release semantics */
+__device__ __forceinline__ void shmemg_dev_put_signal(const shmemg_device_world_t &w, uint64_t dest_off, uint64_t source_off,
+                                                      size_t nbytes, uint64_t sig_off, uint64_t signal, int sig_op, int pe,
+                                                      int target_pe) {
+    shmemg_dev_put(w, dest_off, source_off, nbytes, pe, target_pe);
+    shmemg_dev_signal_update(reinterpret_cast<unsigned long long *>(shmemg_dev_ptr(w, sig_off, target_pe)), signal, sig_op);
+}
+/* block scope: all threads copy, every thread fences its share, the block synchronises, one thread signals */
+__device__ __forceinline__ void shmemg_dev_put_signal_block(const shmemg_device_world_t &w, uint64_t dest_off,
+                                                            uint64_t source_off, size_t nbytes, uint64_t sig_off,
+                                                            uint64_t signal, int sig_op, int pe, int target_pe) {
+    shmemg_dev_copy(shmemg_dev_ptr(w, dest_off, target_pe), shmemg_dev_ptr(w, source_off, pe), nbytes,
+                    shmemg_dev_block_tid(), shmemg_dev_block_size());
+    shmemg_dev_fence_gpu();
+    __syncthreads();
+    if (shmemg_dev_block_tid() == 0)
+        shmemg_dev_signal_update(reinterpret_cast<unsigned long long *>(shmemg_dev_ptr(w, sig_off, target_pe)), signal, sig_op);
+}
+/* blocks the calling thread until cmp(u64 heap[pe][sig_off], value) holds (unsigned compare); what it reads afterwards
+ * is at least as new as what the signalling put_signal released */
+__device__ __forceinline__ uint64_t shmemg_dev_signal_wait_until(const shmemg_device_world_t &w, uint64_t sig_off, int cmp,
+                                                                 uint64_t value, int pe) {
+    const unsigned long long *sig = reinterpret_cast<const unsigned long long *>(shmemg_dev_ptr(w, sig_off, pe));
+    unsigned long long s;
+    while (!shmemg_dev_cmp(cmp, s = shmemg_dev_ld_relaxed(sig), value)) __nanosleep(32);
+    shmemg_dev_fence_gpu();
+    return s;
+}
+/* non-blocking probe of the same condition (shmem_signal_test analog): 1 if it holds (then acquire), else 0 */
+__device__ __forceinline__ int shmemg_dev_signal_test(const shmemg_device_world_t &w, uint64_t sig_off, int cmp, uint64_t value,
+                                                      int pe) {
+    const unsigned long long *sig = reinterpret_cast<const unsigned long long *>(shmemg_dev_ptr(w, sig_off, pe));
+    if (!shmemg_dev_cmp(cmp, shmemg_dev_ld_relaxed(sig), value)) return 0;
+    shmemg_dev_fence_gpu();
+    return 1;
+}
+/* block scope: one thread polls, the block synchronises; every thread may read the payload afterwards */
+__device__ __forceinline__ void shmemg_dev_signal_wait_until_block(const shmemg_device_world_t &w, uint64_t sig_off, int cmp,
+                                                                   uint64_t value, int pe) {
+    if (shmemg_dev_block_tid() == 0) shmemg_dev_signal_wait_until(w, sig_off, cmp, value, pe);
+    __syncthreads();
+}
+
+/* ---- atomics on 64-bit words, thread scope, relaxed: atomicity does not imply ordering -------
+ * add: red.global (nothing fetched); fetch_add / compare_swap: atom.global (old value returned). */
+__device__ __forceinline__ void shmemg_dev_atomic_add(const shmemg_device_world_t &w, uint64_t dest_off, uint64_t value,
+                                                      int target_pe) {
+    asm volatile("red.relaxed.gpu.global.add.u64 [%0], %1;" ::"l"(shmemg_dev_ptr(w, dest_off, target_pe)), "l"(value) : "memory");
+}
+__device__ __forceinline__ uint64_t shmemg_dev_atomic_fetch_add(const shmemg_device_world_t &w, uint64_t dest_off,
+                                                                uint64_t value, int target_pe) {
+    unsigned long long old;
+    asm volatile("atom.relaxed.gpu.global.add.u64 %0, [%1], %2;" : "=l"(old)
+                 : "l"(shmemg_dev_ptr(w, dest_off, target_pe)), "l"(value) : "memory");
+    return old;
+}
+__device__ __forceinline__ uint64_t shmemg_dev_atomic_compare_swap(const shmemg_device_world_t &w, uint64_t dest_off,
+                                                                   uint64_t cond, uint64_t value, int target_pe) {
+    unsigned long long old;
+    asm volatile("atom.relaxed.gpu.global.cas.b64 %0, [%1], %2, %3;" : "=l"(old)
+                 : "l"(shmemg_dev_ptr(w, dest_off, target_pe)), "l"(cond), "l"(value) : "memory");
+    return old;
+}
+
+/* ---- device barrier (device collective, Table 6 "uniform participation") ---------------------------
+ * Called by ALL threads of ONE thread block per PE; the npes blocks must be co-resident (cooperative launch).
+ * Implies quiet for every PE: all updates issued before the barrier by any participating block are visible to all
+ * of them after it.  Sense-reversing counter in the world's control region; do not run it concurrently with
+ * shmemg_barrier_all_repeat_on_stream or a second device kernel of the same world. */
+__device__ __forceinline__ void shmemg_dev_barrier_all_block(const shmemg_device_world_t &w) {
+    shmemg_dev_fence_gpu();                 /* every thread: its own earlier updates */
+    __syncthreads();
+    if (shmemg_dev_block_tid() == 0) {
+        unsigned gen, old;
+        asm volatile("ld.relaxed.gpu.global.u32 %0, [%1];" : "=r"(gen) : "l"(w.bar_gen) : "memory");
+        asm volatile("atom.acq_rel.gpu.global.add.u32 %0, [%1], 1;" : "=r"(old) : "l"(w.bar_count) : "memory");
+        if (old == (unsigned)w.npes - 1u) {
+            asm volatile("st.relaxed.gpu.global.u32 [%0], %1;" ::"l"(w.bar_count), "r"(0u) : "memory");
+            asm volatile("st.release.gpu.global.u32 [%0], %1;" ::"l"(w.bar_gen), "r"(gen + 1u) : "memory");
+        } else {
+            unsigned g;
+            do {
+                asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(g) : "l"(w.bar_gen) : "memory");
+            } while (g == gen);
+        }
+    }
+    __syncthreads();
+}
+
+#endif /* __CUDACC__ */
+#endif /* SHMEMG_DEVICE_CUH */

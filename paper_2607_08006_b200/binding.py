@@ -59,6 +59,7 @@ class CAP:
     PATH_DIRECT = 1 << 10
     ATOMICS_64 = 1 << 11
     STREAM_COLLECTIVES = 1 << 12
+    DEVICE_BARRIER = 1 << 13
 
 
 F32, I64 = 0, 1
@@ -113,6 +114,8 @@ SYMBOLS = {
     "shmemg_barrier_all_on_stream": (_i, [_vp, _vp]),
     "shmemg_barrier_all_repeat_on_stream": (_i, [_vp, _u32, _u64, _vp]),
     "shmemg_barrier_epoch": (_u64, [_vp, _vp]),
+    "shmemg_device_world_get": (_i, [_vp, _vp]),
+    "shmemg_device_exec_ops_on_stream": (_i, [_vp, _vp, _sz, _vp, _vp, C.POINTER(_sz)]),
     "shmemg_app_halo_perturb_on_stream": (_i, [_vp, _u64, _u32, _u64, _u64, _vp]),
     "shmemg_app_halo_pack_on_stream": (_i, [_vp, _u64, _u64, _u32, _vp]),
     "shmemg_app_checksum64_on_stream": (_i, [_vp, _vp, _u64, _u64, _u32, _vp]),
@@ -292,6 +295,21 @@ class World:
 
     def quiet(self, pe, stream=None):
         self._chk(lib().shmemg_quiet(self.h, pe, _stream(stream)), "shmemg_quiet")
+
+    # ---- device-initiated path (include/shmemg_device.cuh) ---------------------------------------------------------
+    def device_exec_ops(self, ops: np.ndarray, stream=None):
+        """Run an op list device-initiated: one PE-agent thread block per PE (shmemg_device_exec_ops_on_stream)."""
+        assert ops.dtype == OP_DTYPE
+        ops = np.ascontiguousarray(ops)
+        ops_dev = torch.empty(max(len(ops), 1) * OP_DTYPE.itemsize, dtype=torch.uint8, device=self.device)
+        bad = C.c_size_t(0)
+        rc = lib().shmemg_device_exec_ops_on_stream(self.h, ops.ctypes.data, len(ops), ops_dev.data_ptr(), _stream(stream),
+                                                    C.byref(bad))
+        if rc:
+            raise ShmemgError(rc, "shmemg_device_exec_ops_on_stream", "op %d" % bad.value)
+        self._keep = getattr(self, "_keep", [])
+        self._keep.append(ops_dev)                 # must stay valid until the stream has passed the call
+        self.launches += 1 if len(ops) else 0
 
     # ---- SoA AMO batches -------------------------------------------------------------------------------------------
     @staticmethod

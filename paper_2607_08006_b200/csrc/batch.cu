@@ -387,7 +387,7 @@ __global__ void k_wait_until(const unsigned long long *sig, int cmp, unsigned lo
 // ---------------------------------------------------------------------------------------------------------
 // host: validation + planning
 // ---------------------------------------------------------------------------------------------------------
-static int validate_op(const shmemg_world *w, const shmemg_op_t &o) {
+int shmemg_validate_op(const shmemg_world *w, const shmemg_op_t &o) {
     switch (o.opcode) {
     case SHMEMG_OP_FENCE: case SHMEMG_OP_QUIET:
         return shmemg_pe_ok(w, o.initiator_pe) ? SHMEMG_OK : SHMEMG_ERR_PE;
@@ -526,7 +526,7 @@ extern "C" size_t shmemg_batch_plan_bytes(const shmemg_world_t *w, const shmemg_
     if (!w || (!ops_host && nops)) return 0;
     // an invalid descriptor is reported (with its index) by shmemg_batch_create, which never touches the plan then
     for (size_t i = 0; i < nops; ++i)
-        if (validate_op(w, ops_host[i])) return sizeof(PlanHeader);
+        if (shmemg_validate_op(w, ops_host[i])) return sizeof(PlanHeader);
     std::vector<Unit> units;
     build_units(ops_host, nops, units);
     return plan_sizes(w, ops_host, nops, units).total;
@@ -538,7 +538,7 @@ extern "C" int shmemg_batch_create(shmemg_world_t *w, const shmemg_op_t *ops, si
     *out = nullptr;
     if ((uintptr_t)plan_dev % 256) return SHMEMG_ERR_ALIGN;
     for (size_t i = 0; i < nops; ++i) {
-        int rc = validate_op(w, ops[i]);
+        int rc = shmemg_validate_op(w, ops[i]);
         if (rc) {
             if (bad_index) *bad_index = i;
             return rc;

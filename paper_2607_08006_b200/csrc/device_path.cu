@@ -1,0 +1,102 @@
+// device_path.cu -- the DEVICE-INITIATED path (Tier-1): kernels that issue the specification's
+// operations themselves through the header-only entry points of include/shmemg_device.cuh.
+//   k_device_exec_ops : one thread block per PE ("PE agent", cooperative launch); agent p walks an op list in order and
+//                       executes the ops it initiates with blocking semantics.  It is the device-side counterpart of
+//                       the batch executor and lets every litmus program and parity comparison of the tests run device-initiated.
+//   k_halo_persistent : the halo application as ONE persistent kernel (perturb, pack, put_signal, wait for all rounds),
+//                       see halo_app.cu for the host-driven version of the same application.
+#include "internal.cuh"
+#include "../../include/shmemg_device.cuh"
+#include "../../include/shmemg_app.h"
+
+extern "C" int shmemg_device_world_get(const shmemg_world_t *w, shmemg_device_world_t *out) {
+    if (!w || !out) return SHMEMG_ERR_ARG;
+    out->base = w->base;
+    out->stride = w->stride;
+    out->heap_bytes = w->heap_bytes;
+    out->npes = w->npes;
+    out->reserved = 0;
+    out->bar_count = &w->ctl->bar_count;
+    out->bar_gen = &w->ctl->bar_gen;
+    return SHMEMG_OK;
+}
+
+#define AGENT_THREADS 256
+
+__device__ __forceinline__ shmemg_op_t ld_op(const shmemg_op_t *p) {
+    shmemg_op_t r;
+    const int4 *s = reinterpret_cast<const int4 *>(p);
+    int4 *d = reinterpret_cast<int4 *>(&r);
+    d[0] = __ldg(s); d[1] = __ldg(s + 1); d[2] = __ldg(s + 2); d[3] = __ldg(s + 3);
+    return r;
+}
+
+__global__ void __launch_bounds__(AGENT_THREADS) k_device_exec_ops(const shmemg_device_world_t dw, const shmemg_op_t *ops,
+                                                                   size_t nops) {
+    const int p = blockIdx.x;                       // this block acts for PE p
+    for (size_t i = 0; i < nops; ++i) {
+        const shmemg_op_t o = ld_op(ops + i);       // every thread reads the same descriptor: uniform participation
+        if (o.opcode == SHMEMG_OP_BARRIER_ALL) { shmemg_dev_barrier_all_block(dw); continue; }
+        if (o.initiator_pe != p) continue;
+        switch (o.opcode) {
+        case SHMEMG_OP_PUT:
+            shmemg_dev_put_block(dw, o.rem_off, o.loc_off, o.nbytes, p, o.target_pe);
+            break;
+        case SHMEMG_OP_GET:
+            shmemg_dev_get_block(dw, o.loc_off, o.rem_off, o.nbytes, p, o.target_pe);
+            break;
+        case SHMEMG_OP_PUT_SIGNAL:
+            shmemg_dev_put_signal_block(dw, o.rem_off, o.loc_off, o.nbytes, o.sig_off, o.value, o.sig_op, p, o.target_pe);
+            break;
+        case SHMEMG_OP_ATOMIC_ADD:
+            if (threadIdx.x == 0) shmemg_dev_atomic_add(dw, o.rem_off, o.value, o.target_pe);
+            break;
+        case SHMEMG_OP_ATOMIC_FETCH_ADD:
+            if (threadIdx.x == 0)
+                *reinterpret_cast<unsigned long long *>(shmemg_dev_ptr(dw, o.loc_off, p)) =
+                    shmemg_dev_atomic_fetch_add(dw, o.rem_off, o.value, o.target_pe);
+            __syncthreads();                        // the fetch slot is local state of the agent: later ops may read it
+            break;
+        case SHMEMG_OP_ATOMIC_COMPARE_SWAP:
+            if (threadIdx.x == 0)
+                *reinterpret_cast<unsigned long long *>(shmemg_dev_ptr(dw, o.loc_off, p)) =
+                    shmemg_dev_atomic_compare_swap(dw, o.rem_off, o.cond, o.value, o.target_pe);
+            __syncthreads();
+            break;
+        case SHMEMG_OP_SIGNAL_WAIT_UNTIL:
+            shmemg_dev_signal_wait_until_block(dw, o.loc_off, o.cmp, o.value, p);
+            break;
+        case SHMEMG_OP_FENCE:
+            shmemg_dev_fence_block();
+            break;
+        case SHMEMG_OP_QUIET:
+            shmemg_dev_quiet_block();
+            break;
+        default: break;
+        }
+    }
+}
+
+extern "C" int shmemg_device_exec_ops_on_stream(shmemg_world_t *w, const shmemg_op_t *ops_host, size_t nops, void *ops_dev,
+                                                void *stream, size_t *bad_index) {
+    if (!w || (!ops_host && nops) || (!ops_dev && nops)) return SHMEMG_ERR_ARG;
+    for (size_t i = 0; i < nops; ++i) {
+        int rc = shmemg_validate_op(w, ops_host[i]);
+        if (rc) {
+            if (bad_index) *bad_index = i;
+            return rc;
+        }
+    }
+    if (nops == 0) return SHMEMG_OK;
+    int per_sm = 0;
+    SHMEMG_CUDA(w, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_device_exec_ops, AGENT_THREADS, 0));
+    if ((long long)per_sm * w->sm_count < w->npes) return SHMEMG_ERR_NOMEM;     // agents could not all be co-resident
+    cudaStream_t st = (cudaStream_t)stream;
+    SHMEMG_CUDA(w, cudaMemcpyAsync(ops_dev, ops_host, nops * sizeof(shmemg_op_t), cudaMemcpyHostToDevice, st));
+    shmemg_device_world_t dw;
+    shmemg_device_world_get(w, &dw);
+    const shmemg_op_t *od = reinterpret_cast<const shmemg_op_t *>(ops_dev);
+    void *args[] = {&dw, &od, &nops};
+    SHMEMG_CUDA(w, cudaLaunchCooperativeKernel((void *)k_device_exec_ops, dim3((unsigned)w->npes), dim3(AGENT_THREADS), args, 0, st));
+    return SHMEMG_OK;
+}

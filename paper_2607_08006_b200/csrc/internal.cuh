@@ -66,6 +66,9 @@ static inline uint8_t *shmemg_addr(const shmemg_world *w, int pe, uint64_t off) 
     return w->base + (size_t)pe * w->stride + off;
 }
 
+// host-side validation of one op descriptor (batch.cu); shared with the device-initiated interpreter (device_path.cu)
+int shmemg_validate_op(const shmemg_world *w, const shmemg_op_t &o);
+
 #ifdef __CUDACC__
 // ---- memory-model primitives (GPU scope) --------------------------------------------------------------
 __device__ __forceinline__ unsigned ld_acquire_u32(const unsigned *p) {

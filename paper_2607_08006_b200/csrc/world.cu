@@ -107,7 +107,7 @@ extern "C" int shmem_query_capabilities(const shmemg_world_t *w, int team, uint6
     if (team == SHMEM_TEAM_WORLD)
         c |= SHMEMG_CAP_HOST_INITIATED_GPU_BUFFERS | SHMEMG_CAP_STREAM_TRIGGERED | SHMEMG_CAP_STREAM_COLLECTIVES;
     else
-        c |= SHMEMG_CAP_DEVICE_INITIATED;   // include/shmemg_device.cuh: thread-scope put/get/AMO/signal/fence/quiet
+        c |= SHMEMG_CAP_DEVICE_INITIATED | SHMEMG_CAP_DEVICE_BARRIER;   // include/shmemg_device.cuh
     *caps = c;
     return SHMEMG_OK;
 }

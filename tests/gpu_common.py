@@ -28,6 +28,18 @@ def run_gpu(prog, batches=None, heap_bytes=None):
     return w, ld
 
 
+def run_gpu_device(prog, batches=None, heap_bytes=None):
+    """Same as run_gpu, but DEVICE-INITIATED: every batch is executed by PE-agent thread blocks through the
+    entry points of include/shmemg_device.cuh (shmemg_device_exec_ops_on_stream)."""
+    hb = heap_bytes or heap_bytes_for(prog)
+    w = World(prog.npes, hb, DEV)
+    ld = Loaded(w, prog)
+    for q in (batches or [prog]):
+        w.device_exec_ops(ld.translate(q))
+    w.quiet(0)
+    return w, ld
+
+
 def run_oracle(prog, batches=None, heap_bytes=None):
     hb = heap_bytes or heap_bytes_for(prog)
     ow = orc.OracleWorld(prog.npes, hb)

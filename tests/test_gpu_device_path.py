@@ -1,0 +1,123 @@
+"""GPU parity of the DEVICE-INITIATED path (include/shmemg_device.cuh): the same neutral
+programs the batch executor runs are executed by PE-agent thread blocks that call the `__device__` entry points, and
+compared with the CPU oracle object by object (bit-exact), plus the schedule-independent invariants for fetching
+atomics and the brute-force outcome sets for tiny programs."""
+import numpy as np
+import pytest
+
+from gpu_common import DEV, assert_objects_equal, run_gpu_device, run_oracle
+from invariants import check_compare_swap_claim, check_fetch_add
+from litmus_model import enumerate_outcomes, to_spec_program
+from paper_2607_08006_b200 import CAP, ERR, OP, OP_DTYPE, TEAM, ShmemgError, World
+from test_gpu_batch import TINY
+from workloads import configs, gen, litmus
+from workloads.spec import Program
+
+pytestmark = pytest.mark.gpu
+M64 = (1 << 64) - 1
+
+
+def test_capabilities_distinguish_the_device_path():
+    """capability queries distinguish host-initiated GPU-aware from device-initiated support."""
+    w = World(4, 4096, DEV)
+    host, dev = w.query_capabilities(TEAM.WORLD), w.query_capabilities(TEAM.DEVICE_WORLD)
+    assert dev & CAP.DEVICE_INITIATED and dev & CAP.DEVICE_BARRIER and not dev & CAP.DEVICE_COLLECTIVES
+    assert not host & CAP.DEVICE_INITIATED and host & CAP.STREAM_TRIGGERED
+    assert w.query_capabilities(TEAM.DEVICE_SHARED) == dev          # one GPU: shared == world (L357)
+
+
+@pytest.mark.parametrize("make", [
+    lambda: litmus.mp_fence(),
+    lambda: litmus.mp_fence(npes=64, rounds=6, nbytes=300000, lag=1),
+    lambda: litmus.mp_quiet_third_party(),
+    lambda: litmus.put_signal_sizes(),
+    lambda: litmus.signal_add_fanin(),
+    lambda: litmus.barrier_stamp(),
+    lambda: litmus.barrier_stamp(npes=128, rounds=12),
+], ids=["mp_fence", "mp_fence_big", "mp_quiet3", "put_signal_sizes", "signal_add_fanin", "barrier_stamp",
+        "barrier_stamp128"])
+def test_litmus_programs_device_initiated_match_oracle(make):
+    prog = make()
+    w, ld = run_gpu_device(prog)
+    assert_objects_equal(prog, ld, run_oracle(prog))
+
+
+def test_random_put_get_unaligned_device_initiated():
+    """Race-free random puts/gets, arbitrary sizes and alignments (every head/body/tail width of shmemg_dev_copy)."""
+    npes, nops, slot = 6, 600, 5000
+    rng = np.random.default_rng(5)
+    prog = Program(npes)
+    prog.obj("src", 40000, gen.u64(npes * 40000 // 8, 78).view(np.uint8).reshape(npes, 40000))
+    prog.obj("dst", nops * slot)
+    for k in range(nops):
+        i, t = int(rng.integers(npes)), int(rng.integers(npes))
+        n = int(rng.integers(0, 70)) if k % 3 == 0 else int(rng.integers(0, slot - 32))
+        s, d = int(rng.integers(0, 40000 - n)), k * slot + int(rng.integers(0, 32))
+        if k % 4 == 1:
+            s = (s & ~15) + (d & 15)                                 # congruent mod 16: head + vector body + tail
+        if k % 2:
+            prog.put(i, t, ("dst", d), ("src", s), n)
+        else:
+            prog.get(i, t, ("dst", d), ("src", s), n)
+    w, ld = run_gpu_device(prog)
+    assert_objects_equal(prog, ld, run_oracle(prog))
+
+
+def test_random_amos_device_initiated():
+    prog = litmus.random_amos()
+    w, ld = run_gpu_device(prog)
+    ow = run_oracle(prog)
+    ops = prog.ops
+    nw = prog.obj_bytes[0] // 8
+    words = ld.obj_numpy("words", np.uint64)
+    assert np.array_equal(words[:, :nw // 2], ow.obj("words", np.uint64)[:, :nw // 2])     # add / fetch-add finals
+    assert np.array_equal(words[:, nw // 2:] == M64, ow.obj("words", np.uint64)[:, nw // 2:] == M64)
+    fetch = ld.obj_numpy("fetch", np.uint64)
+    key = ops["target"].astype(np.int64) * nw + (ops["rem_off"] // 8).astype(np.int64)
+    fa, ad, cs = ops["kind"] == 5, ops["kind"] == 4, ops["kind"] == 6
+    fetched = fetch[ops["initiator"], np.arange(len(ops))]
+    sel = fa & ~np.isin(key, np.unique(key[ad]))
+    init = np.zeros(prog.npes * nw, dtype=np.uint64)
+    init.reshape(prog.npes, nw)[:, nw // 2:] = M64
+    fin = words.reshape(-1)
+    if sel.any():
+        sub_final = init.copy()
+        ks = np.unique(key[sel])
+        sub_final[ks] = fin[ks]
+        check_fetch_add(key[sel], ops["value"][sel], fetched[sel], init, sub_final)
+    cas_final = np.full(prog.npes * nw, M64, dtype=np.uint64)
+    kc = np.unique(key[cs])
+    cas_final[kc] = fin[kc]
+    check_compare_swap_claim(key[cs], ops["value"][cs], fetched[cs], cas_final)
+
+
+@pytest.mark.parametrize("name", sorted(TINY))
+def test_tiny_programs_device_initiated_land_in_outcome_set(name):
+    """Truly concurrent PE agents: the final state must be one the ordering rules allow (brute-force enumeration)."""
+    prog, init, order = TINY[name]
+    allowed = enumerate_outcomes(prog, init)
+    sp = to_spec_program(prog, init, order)
+    for _ in range(5):
+        w, ld = run_gpu_device(sp)
+        got = tuple(tuple(int(x) for x in row) for row in ld.obj_numpy("w", np.uint64))
+        assert got in allowed, (name, got)
+
+
+def test_halo_rounds_device_initiated_match_oracle():
+    """Config 2's exchange (put_signal + wait + consume) for 4 rounds at B = 32, device-initiated, vs the oracle."""
+    h = configs.Halo(32)
+    prog = h.program(with_consume=True, with_U=False)
+    prog.init["send"] = gen.u64(8 * 6 * h.face_bytes // 8, 21).view(np.uint8).reshape(8, -1)
+    rounds = [h.round_ops(prog, r, True) for r in range(1, 5)]
+    w, ld = run_gpu_device(prog, batches=rounds)
+    assert_objects_equal(prog, ld, run_oracle(prog, batches=rounds))
+
+
+def test_device_exec_rejects_bad_descriptors_and_empty_list():
+    w = World(2, 4096, DEV)
+    w.device_exec_ops(np.zeros(0, dtype=OP_DTYPE))
+    o = np.zeros(1, dtype=OP_DTYPE)
+    o["opcode"], o["target_pe"], o["nbytes"] = OP.PUT, 2, 8
+    with pytest.raises(ShmemgError) as e:
+        w.device_exec_ops(o)
+    assert e.value.code == ERR.PE
