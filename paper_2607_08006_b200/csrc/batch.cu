@@ -23,9 +23,11 @@
 //     segment, not per tile.  An op cut into several pieces completes at its last-ARRIVING piece (acq_rel counter on
 //     arrive[op]), which performs the put_signal update with release semantics and the done[] increments.  Ops nobody
 //     depends on and that carry no signal do no accounting at all.
+#include <stdio.h>
 #include <stdlib.h>
 #include <string.h>
 
+#include <algorithm>
 #include <vector>
 
 #include "tma_stream.cuh"
@@ -37,11 +39,18 @@
 #define GEN_TILE 16384u           // bytes per register-path copy tile
 #define AMO_RUN_MAX GEN_THREADS
 #define TMA_MIN_SPLIT 2048u       // below this, a transfer with unaligned ends is one register-path tile
-#define SEG_TILES_MAX 8u          // bulk tiles per segment (256 KiB)
+#define SEG_TILES_MAX 8u          // planner tiles (SHMEMG_TMA_TILE) per segment (256 KiB)
+// Executor ring geometry, chosen per batch by the planner (measured on B200, profiles/r01c):
+//   latency-bound batches (about one segment per SM): 12 stages of 16 KiB -- small stages start the store front early
+//     and a <= 192 KiB segment is loaded without re-using a stage (halo round 16.5 -> 15.1 us);
+//   streaming batches: 7 stages of 32 KiB -- 224 KiB in flight per SM towards HBM (C3b 72.6 -> 69.5 us).
+#define EXEC_STAGES_MAX 12
+#define EXEC_SMEM_MAX (7u * 32768u)
+#define EXEC_SMALL_PER_SM (256u * 1024u)   // bulk bytes per SM at or below which a batch counts as latency-bound
 #define TRACE_SLOTS 8
 #define TRACE_CTAS 256
 #define TRACE_BYTES (TRACE_CTAS * TRACE_SLOTS * 8)   // per-CTA timestamps (SHMEMG_TRACE=1)
-#define WAIT_RUN_MAX 128u         // consecutive waits of one PE polled by one tile (one per generic thread)
+#define WAIT_RUN_MAX GEN_THREADS  // consecutive waits (of any PEs) polled by one tile, one per generic thread
 
 // tile kinds (bits 0-7 of TileRec.kind); bits 8-15 hold sig_op (put_signal)
 enum { T_TMA = 1, T_COPY = 2, T_AMO = 3, T_WAIT = 4, T_NODATA = 5, T_END = 6 };
@@ -103,6 +112,7 @@ struct shmemg_batch {
     uint32_t grid;
     uint32_t npes, all_total;
     size_t tiles_off, done_off, arrive_off, trace_off;
+    uint32_t stage_bytes, nstages;
     bool trace_on;
 };
 
@@ -174,18 +184,20 @@ struct ExecArgs {
     unsigned *done, *arrive;
     unsigned long long *trace;     // nullptr unless SHMEMG_TRACE
     unsigned ntiles, npes, all_total;
+    unsigned stage_bytes, nstages;     // ring geometry
 };
 
 __global__ void __launch_bounds__(EXEC_THREADS, 1) k_batch_exec(const ExecArgs a) {
     extern __shared__ __align__(1024) uint8_t stage[];
-    __shared__ __align__(16) TileRec ringA[SHMEMG_TMA_STAGES];
+    __shared__ __align__(16) TileRec ringA[EXEC_STAGES_MAX];
     __shared__ __align__(16) TileRec ringG[GEN_SLOTS];
-    __shared__ uint64_t fullA[SHMEMG_TMA_STAGES], emptyA[SHMEMG_TMA_STAGES], fullG[GEN_SLOTS], emptyG[GEN_SLOTS];
+    __shared__ uint64_t fullA[EXEC_STAGES_MAX], emptyA[EXEC_STAGES_MAX], fullG[GEN_SLOTS], emptyG[GEN_SLOTS], epochB;
     __shared__ unsigned s_epoch;
 
     const TileRec *tiles = a.tiles;
     unsigned *done = a.done, *arrive = a.arrive;
     const unsigned ntiles = a.ntiles;
+    const unsigned STG = a.stage_bytes, NST = a.nstages;
     const int tid = threadIdx.x;
     unsigned long long *trace = blockIdx.x < TRACE_CTAS ? a.trace : nullptr;
     Epoch ep;
@@ -193,8 +205,9 @@ __global__ void __launch_bounds__(EXEC_THREADS, 1) k_batch_exec(const ExecArgs a
 
     if (tid == 0) {
         TRACE(0);
-        for (int s = 0; s < SHMEMG_TMA_STAGES; ++s) { mbar_init(&fullA[s], 1); mbar_init(&emptyA[s], 1); }
+        for (int s = 0; s < EXEC_STAGES_MAX; ++s) { mbar_init(&fullA[s], 1); mbar_init(&emptyA[s], 1); }
         for (int g = 0; g < GEN_SLOTS; ++g) { mbar_init(&fullG[g], 1); mbar_init(&emptyG[g], 1); }
+        mbar_init(&epochB, 1);
         mbar_init_fence();
     }
     __syncthreads();
@@ -204,15 +217,37 @@ __global__ void __launch_bounds__(EXEC_THREADS, 1) k_batch_exec(const ExecArgs a
         // The first ticket of CTA b is b (no atomic on the critical path, and the first wave is spread over all CTAs);
         // later tickets are claimed one ahead, while the current piece is processed.
         // Launch index: this launch's claims keep the counter inside [epoch*ntiles, (epoch+1)*ntiles) until the last
-        // CTA's failing claim, and a CTA reads it before making its own.  The consumers pick s_epoch up after their
-        // first ring hand-off (mbarrier release/acquire).
+        // CTA's failing claim, and a CTA reads it before making its own.  The read is a cold miss (about 1 us): it is
+        // issued first and consumed only after the first segment's loads are in flight; the consumers pick s_epoch up
+        // through the epochB mbarrier before their first completion accounting.
         TRACE(1);
+        const unsigned long long tk0 = ld_relaxed_u64(a.ticket);
         TileRec r0 = {};
         if (blockIdx.x < ntiles) r0 = ld_rec(tiles + blockIdx.x);
-        ep.e = (unsigned)(ld_relaxed_u64(a.ticket) / ntiles);
+        unsigned ia = 0, ig = 0;                                     // ia = stage index, pa = its lap parity
+        unsigned pa = 0, nissued = 0;
+        auto issue = [&](const TileRec &r, unsigned off) {
+            const unsigned s = ia;
+            const unsigned n = r.nbytes - off < STG ? r.nbytes - off : STG;
+            mbar_wait(&emptyA[s], pa ^ 1u);                              // passes at once on the ring's first lap
+            TileRec q = r;
+            q.dst = r.dst + off; q.nbytes = n;
+            if (off + n == r.nbytes) q.kind |= TF_SEGEND;
+            ringA[s] = q;
+            mbar_arrive_expect_tx(&fullA[s], n);
+            bulk_g2s(stage + (size_t)s * STG, reinterpret_cast<const void *>(r.src + off), n, &fullA[s]);
+            if (++ia == NST) { ia = 0; pa ^= 1u; }
+            ++nissued;
+        };
+        unsigned pre = 0;                                            // bytes of r0 already issued
+        if ((r0.kind & (0xffu | TF_DEPS)) == T_TMA) {                // no dependencies: start streaming before the epoch is known
+            for (; pre < r0.nbytes && nissued < NST; pre += STG) issue(r0, pre);
+            TRACE(6);
+        }
+        ep.e = (unsigned)(tk0 / ntiles);
         s_epoch = ep.e;
+        mbar_arrive(&epochB);
         const unsigned long long tbase = (unsigned long long)ep.e * ntiles;   // exact: epoch < 2^32 launches
-        unsigned ia = 0, ig = 0;
         unsigned long long t0 = blockIdx.x;
         while (t0 < ntiles) {
             const unsigned long long t1 = atomicAdd(a.ticket, 1ull) - tbase + gridDim.x;
@@ -222,17 +257,8 @@ __global__ void __launch_bounds__(EXEC_THREADS, 1) k_batch_exec(const ExecArgs a
                 proxy_fence();                                       // acquire (generic proxy) before bulk reads
             }
             if (k == T_TMA) {                                        // one segment: stream its bulk tiles
-                for (unsigned off = 0; off < r0.nbytes; off += SHMEMG_TMA_TILE, ++ia) {
-                    const unsigned s = ia % SHMEMG_TMA_STAGES;
-                    const unsigned n = r0.nbytes - off < SHMEMG_TMA_TILE ? r0.nbytes - off : SHMEMG_TMA_TILE;
-                    mbar_wait(&emptyA[s], ((ia / SHMEMG_TMA_STAGES) & 1u) ^ 1u);
-                    TileRec q = r0;
-                    q.dst = r0.dst + off; q.nbytes = n;
-                    if (off + n == r0.nbytes) q.kind |= TF_SEGEND;
-                    ringA[s] = q;
-                    mbar_arrive_expect_tx(&fullA[s], n);
-                    bulk_g2s(stage + (size_t)s * SHMEMG_TMA_TILE, reinterpret_cast<const void *>(r0.src + off), n, &fullA[s]);
-                }
+                for (unsigned off = pre; off < r0.nbytes; off += STG) issue(r0, off);
+                pre = 0;
             } else if (k == T_COPY || k == T_AMO || k == T_WAIT) {   // generic warps (a wait run is polled one wait per thread)
                 const unsigned g = ig % GEN_SLOTS;
                 mbar_wait(&emptyG[g], ((ig / GEN_SLOTS) & 1u) ^ 1u);
@@ -247,8 +273,8 @@ __global__ void __launch_bounds__(EXEC_THREADS, 1) k_batch_exec(const ExecArgs a
         }
         TRACE(2);
         {   // end markers for both consumers
-            const unsigned s = ia % SHMEMG_TMA_STAGES;
-            mbar_wait(&emptyA[s], ((ia / SHMEMG_TMA_STAGES) & 1u) ^ 1u);
+            const unsigned s = ia;
+            mbar_wait(&emptyA[s], pa ^ 1u);
             ringA[s].kind = T_END;
             mbar_arrive(&fullA[s]);
             const unsigned g = ig % GEN_SLOTS;
@@ -259,13 +285,14 @@ __global__ void __launch_bounds__(EXEC_THREADS, 1) k_batch_exec(const ExecArgs a
     } else if (tid == 32) {
         // ---- storer -------------------------------------------------------------------------------------------
         bool have_prev = false, pend_acct = false;     // previous tile's stage not yet freed / segment not yet accounted
+        bool have_epoch = false;
         TileRec acct = {};
         unsigned prev_s = 0;
-        for (unsigned i = 0;; ++i) {
-            const unsigned s = i % SHMEMG_TMA_STAGES, ph = (i / SHMEMG_TMA_STAGES) & 1u;
+        auto epoch = [&]() { if (!have_epoch) { mbar_wait(&epochB, 0); ep.e = s_epoch; have_epoch = true; } };
+        for (unsigned i = 0, s = 0, ph = 0;; ++i) {
             if (!mbar_test_wait(&fullA[s], ph)) {
                 if (have_prev) {              // starved: nothing may stay unaccounted while this role blocks
-                    if (pend_acct) { bulk_wait<0>(); proxy_fence(); account(acct, done, arrive, ep); pend_acct = false; }
+                    if (pend_acct) { bulk_wait<0>(); proxy_fence(); epoch(); account(acct, done, arrive, ep); pend_acct = false; }
                     else bulk_wait_read<0>();
                     mbar_arrive(&emptyA[prev_s]);
                     have_prev = false;
@@ -274,21 +301,22 @@ __global__ void __launch_bounds__(EXEC_THREADS, 1) k_batch_exec(const ExecArgs a
             }
             const TileRec r = ringA[s];
             if ((r.kind & 0xffu) == T_END) break;
-            ep.e = s_epoch;
-            bulk_s2g(reinterpret_cast<void *>(r.dst), stage + (size_t)s * SHMEMG_TMA_TILE, r.nbytes);
+            if (i == 0) TRACE(7);
+            bulk_s2g(reinterpret_cast<void *>(r.dst), stage + (size_t)s * STG, r.nbytes);
             bulk_commit();
             if (have_prev) {
                 // every group but the one just committed: has completed (a segment ended) / has read its stage
-                if (pend_acct) { bulk_wait<1>(); proxy_fence(); account(acct, done, arrive, ep); pend_acct = false; }
+                if (pend_acct) { bulk_wait<1>(); proxy_fence(); epoch(); account(acct, done, arrive, ep); pend_acct = false; }
                 else bulk_wait_read<1>();
                 mbar_arrive(&emptyA[prev_s]);
             }
             if ((r.kind & TF_SEGEND) && (r.kind & TF_ACCT)) { acct = r; pend_acct = true; }
             prev_s = s; have_prev = true;
+            if (++s == NST) { s = 0; ph ^= 1u; }
         }
         TRACE(3);
         bulk_wait<0>();
-        if (pend_acct) { proxy_fence(); account(acct, done, arrive, ep); }
+        if (pend_acct) { proxy_fence(); epoch(); account(acct, done, arrive, ep); }
         TRACE(4);
     } else if (tid >= GEN_FIRST) {
         // ---- generic warps: register-path copies and AMO runs ----------------------------------------------
@@ -299,19 +327,22 @@ __global__ void __launch_bounds__(EXEC_THREADS, 1) k_batch_exec(const ExecArgs a
             const TileRec r = ringG[g];
             const unsigned k = r.kind & 0xffu;
             if (k == T_END) break;
-            ep.e = s_epoch;
+            if (j == 0) { mbar_wait(&epochB, 0); ep.e = s_epoch; }
             if (k == T_COPY) {
                 copy_coop<4>(reinterpret_cast<uint8_t *>(r.dst), reinterpret_cast<const uint8_t *>(r.src), r.nbytes, gt,
                              GEN_THREADS);
                 if (r.kind & TF_ACCT) __threadfence();
             } else if (k == T_WAIT) {
-                // a run of consecutive waits of one PE: thread i polls wait i (all must hold; order is immaterial)
+                // a run of consecutive waits (any PEs): thread i polls wait i and accounts for it on its own
                 if (gt < (int)r.nbytes) {
                     const AuxRec o = ld_rec(reinterpret_cast<const AuxRec *>(r.src) + gt);
                     const unsigned long long *sig = reinterpret_cast<const unsigned long long *>(o.word);
                     const int cmp = (int)((o.kind >> 8) & 0xff);
-                    while (!cmp_u64(cmp, ld_relaxed_u64(sig), o.value)) __nanosleep(32);
+                    wait_deps(done, ep, o.initiator, o.dep_pe, o.dep_all, o.pe_total);
+                    for (unsigned spin = 0; !cmp_u64(cmp, ld_relaxed_u64(sig), o.value); ++spin)
+                        if (spin > 64) __nanosleep(32);
                     fence_acquire();
+                    count_done(done, ep.npes, o.kind, o.initiator);
                 }
             } else if (gt < (int)r.nbytes) {
                 const AuxRec o = ld_rec(reinterpret_cast<const AuxRec *>(r.src) + gt);
@@ -322,7 +353,6 @@ __global__ void __launch_bounds__(EXEC_THREADS, 1) k_batch_exec(const ExecArgs a
             named_bar_sync(1, GEN_THREADS);
             if (gt == 0) {
                 if (k == T_COPY) account(r, done, arrive, ep);
-                else if (k == T_WAIT) count_done(done, ep.npes, r.kind, r.initiator);   // release: cumulative over the bar
                 mbar_arrive(&emptyG[g]);
             }
         }
@@ -468,17 +498,13 @@ static uint32_t pick_seg_tiles(const shmemg_world *w, const shmemg_op_t *ops, si
     return per_sm < 1 ? 1u : (uint32_t)per_sm;
 }
 
-// ---- planning units: a marker, one copy op, one AMO op, or a run of consecutive waits of one PE ----------------------
+// ---- planning units: one per op (a marker, a copy op, an AMO, a wait) -------------------------------------------------
 struct Unit { uint8_t opc; int pe; size_t first, count; };    // [first, first+count) in the caller's op array
 
 static void build_units(const shmemg_op_t *ops, size_t nops, std::vector<Unit> &units) {
     units.clear();
     for (size_t i = 0; i < nops; ++i) {
         const shmemg_op_t &o = ops[i];
-        if (o.opcode == SHMEMG_OP_SIGNAL_WAIT_UNTIL && !units.empty()) {
-            Unit &u = units.back();
-            if (u.opc == SHMEMG_OP_SIGNAL_WAIT_UNTIL && u.pe == o.initiator_pe && u.count < WAIT_RUN_MAX) { u.count++; continue; }
-        }
         units.push_back({o.opcode, o.opcode == SHMEMG_OP_BARRIER_ALL ? 0 : o.initiator_pe, i, 1});
     }
 }
@@ -494,19 +520,20 @@ static void copy_endpoints(const shmemg_world *w, const shmemg_op_t &o, uint64_t
 static PlanSizes plan_sizes(const shmemg_world *w, const shmemg_op_t *ops, size_t nops, const std::vector<Unit> &units) {
     PlanSizes s{};
     size_t run = 0;
+    uint32_t run_kind = 0;
     std::vector<Piece> pieces;
     const uint32_t seg_tiles = pick_seg_tiles(w, ops, nops);
     for (const Unit &u : units) {
         if (is_marker(u.opc)) { run = 0; continue; }
         s.nunits++;
-        if (is_amo(u.opc)) {
+        if (is_amo(u.opc) || u.opc == SHMEMG_OP_SIGNAL_WAIT_UNTIL) {     // runs of AMOs / runs of waits: one tile each
+            const uint32_t rk = is_amo(u.opc) ? T_AMO : T_WAIT;
             s.naux++;
-            if (run == 0 || run == AMO_RUN_MAX) { s.ntiles++; run = 0; }
+            if (run == 0 || run == AMO_RUN_MAX || rk != run_kind) { s.ntiles++; run = 0; run_kind = rk; }
             run++;
             continue;
         }
         run = 0;
-        if (u.opc == SHMEMG_OP_SIGNAL_WAIT_UNTIL) { s.ntiles++; s.naux += u.count; continue; }
         uint64_t dst, src;
         copy_endpoints(w, ops[u.first], dst, src);
         cut_copy(dst, src, ops[u.first].nbytes, seg_tiles, pieces);
@@ -589,8 +616,10 @@ extern "C" int shmemg_batch_create(shmemg_world_t *w, const shmemg_op_t *ops, si
 
     // forward pass: dependencies.  issued[p] = counted units of PE p so far; thresh[p] = what p's next unit must see.
     // (Only counted units advance done[], and every unit before a marker that a later unit depends on is counted.)
-    std::vector<uint32_t> issued(w->npes, 0), thresh(w->npes, 0);
-    uint32_t all_issued = 0, all_thresh = 0;
+    // A wait only polls a local word: it follows the PE's fences / quiets (thresh_mark) but not its earlier waits, so the
+    // waits of one PE are polled concurrently; the PE's later real ops follow every one of them (thresh).
+    std::vector<uint32_t> issued(w->npes, 0), thresh(w->npes, 0), thresh_mark(w->npes, 0);
+    uint32_t all_issued = 0, all_thresh = 0, run_kind = 0;
     size_t k = 0, nt = 0, na = 0, run = 0;
     std::vector<Piece> pieces;
     const uint32_t seg_tiles = pick_seg_tiles(w, ops, nops);
@@ -598,7 +627,7 @@ extern "C" int shmemg_batch_create(shmemg_world_t *w, const shmemg_op_t *ops, si
     for (size_t ui = 0; ui < nu; ++ui) {
         const Unit &u = units[ui];
         const shmemg_op_t &o = ops[u.first];
-        if (u.opc == SHMEMG_OP_FENCE || u.opc == SHMEMG_OP_QUIET) { thresh[u.pe] = issued[u.pe]; run = 0; continue; }
+        if (u.opc == SHMEMG_OP_FENCE || u.opc == SHMEMG_OP_QUIET) { thresh[u.pe] = thresh_mark[u.pe] = issued[u.pe]; run = 0; continue; }
         if (u.opc == SHMEMG_OP_BARRIER_ALL) { all_thresh = all_issued; run = 0; continue; }
         const int ini = u.pe;
         const uint32_t flags = ((cnt[ui] & 1) ? TF_CNT_PE : 0) | ((cnt[ui] & 2) ? TF_CNT_ALL : 0);
@@ -610,29 +639,28 @@ extern "C" int shmemg_batch_create(shmemg_world_t *w, const shmemg_op_t *ops, si
             d.value = o.value; d.cond = o.cond;
             d.kind = u.opc | flags;
             d.initiator = (uint32_t)ini; d.dep_pe = dep_pe; d.dep_all = dep_all; d.pe_total = pe_total[ini];
-            if (run == 0 || run == AMO_RUN_MAX) {
+            if (run == 0 || run == AMO_RUN_MAX || run_kind != T_AMO) {
                 TileRec &t = tiles[nt++];
                 t.kind = T_AMO; t.nbytes = 0; t.nt = 1; t.op = (uint32_t)k;
                 t.src = aux_dev(na);
-                run = 0;
+                run = 0; run_kind = T_AMO;
             }
             tiles[nt - 1].nbytes++;
             run++; na++;
         } else if (u.opc == SHMEMG_OP_SIGNAL_WAIT_UNTIL) {
-            run = 0;
-            TileRec &t = tiles[nt++];
-            t.kind = T_WAIT | flags | ((dep_pe | dep_all) ? TF_DEPS : 0);
-            t.src = aux_dev(na);
-            t.nbytes = (uint32_t)u.count;
-            t.nt = 1; t.op = (uint32_t)k; t.initiator = (uint32_t)ini; t.dep_pe = dep_pe; t.dep_all = dep_all;
-            t.pe_total = pe_total[ini];
-            for (size_t j = 0; j < u.count; ++j, ++na) {
-                const shmemg_op_t &wo = ops[u.first + j];
-                aux[na].word = (uint64_t)shmemg_addr(w, ini, wo.loc_off);
-                aux[na].value = wo.value;
-                aux[na].kind = SHMEMG_OP_SIGNAL_WAIT_UNTIL | ((uint32_t)wo.cmp << 8);
-                aux[na].initiator = (uint32_t)ini;
+            AuxRec &d = aux[na];
+            d.word = (uint64_t)shmemg_addr(w, ini, o.loc_off);
+            d.value = o.value;
+            d.kind = SHMEMG_OP_SIGNAL_WAIT_UNTIL | ((uint32_t)o.cmp << 8) | flags;
+            d.initiator = (uint32_t)ini; d.dep_pe = thresh_mark[ini]; d.dep_all = dep_all; d.pe_total = pe_total[ini];
+            if (run == 0 || run == WAIT_RUN_MAX || run_kind != T_WAIT) {
+                TileRec &t = tiles[nt++];
+                t.kind = T_WAIT; t.nbytes = 0; t.nt = 1; t.op = (uint32_t)k;
+                t.src = aux_dev(na);
+                run = 0; run_kind = T_WAIT;
             }
+            tiles[nt - 1].nbytes++;
+            run++; na++;
         } else {
             run = 0;
             uint64_t dst, src;
@@ -672,6 +700,19 @@ extern "C" int shmemg_batch_create(shmemg_world_t *w, const shmemg_op_t *ops, si
     b->npes = (uint32_t)w->npes; b->all_total = all_total;
     b->tiles_off = ps.tiles_off; b->done_off = ps.done_off; b->arrive_off = ps.arrive_off; b->trace_off = ps.trace_off;
     b->trace_on = hdr->trace_on != 0;
+    {
+        uint64_t bulk = 0;
+        for (size_t i = 0; i < nops; ++i)
+            if (ops[i].opcode >= SHMEMG_OP_PUT && ops[i].opcode <= SHMEMG_OP_PUT_SIGNAL) bulk += ops[i].nbytes;
+        const bool small = bulk <= (uint64_t)EXEC_SMALL_PER_SM * (uint64_t)w->sm_count;
+        b->stage_bytes = small ? 16384u : 32768u;
+        b->nstages = small ? 12u : 7u;
+        if (const char *e = getenv("SHMEMG_EXEC_RING")) {            // experiments: "<stage_bytes>x<nstages>"
+            unsigned sb = 0, ns = 0;
+            if (sscanf(e, "%ux%u", &sb, &ns) == 2 && sb >= 1024 && sb % 16 == 0 && ns >= 2 && ns <= EXEC_STAGES_MAX &&
+                (uint64_t)sb * ns <= EXEC_SMEM_MAX) { b->stage_bytes = sb; b->nstages = ns; }
+        }
+    }
     *out = b;
     return SHMEMG_OK;
 }
@@ -685,7 +726,7 @@ extern "C" int shmemg_batch_launches(const shmemg_batch_t *b) { return b ? (b->n
 
 static int ensure_smem_attr(shmemg_world *w) {
     if (w->smem_attr_set) return SHMEMG_OK;
-    SHMEMG_CUDA(w, cudaFuncSetAttribute(k_batch_exec, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SHMEMG_TMA_SMEM));
+    SHMEMG_CUDA(w, cudaFuncSetAttribute(k_batch_exec, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)EXEC_SMEM_MAX));
     SHMEMG_CUDA(w, cudaFuncSetAttribute(k_copy_single_tma, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SHMEMG_TMA_SMEM));
     w->smem_attr_set = true;
     return SHMEMG_OK;
@@ -703,7 +744,8 @@ extern "C" int shmemg_batch_enqueue_on_stream(shmemg_world_t *w, shmemg_batch_t 
     a.arrive = reinterpret_cast<unsigned *>(b->plan_dev + b->arrive_off);
     a.trace = b->trace_on ? reinterpret_cast<unsigned long long *>(b->plan_dev + b->trace_off) : nullptr;
     a.ntiles = b->ntiles; a.npes = b->npes; a.all_total = b->all_total;
-    k_batch_exec<<<b->grid, EXEC_THREADS, SHMEMG_TMA_SMEM, (cudaStream_t)stream>>>(a);
+    a.stage_bytes = b->stage_bytes; a.nstages = b->nstages;
+    k_batch_exec<<<b->grid, EXEC_THREADS, (size_t)b->stage_bytes * b->nstages, (cudaStream_t)stream>>>(a);
     SHMEMG_CUDA(w, cudaGetLastError());
     return SHMEMG_OK;
 }
