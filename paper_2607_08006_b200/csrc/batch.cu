@@ -341,8 +341,10 @@ __global__ void __launch_bounds__(EXEC_THREADS, 1) k_batch_exec(const ExecArgs a
                     wait_deps(done, ep, o.initiator, o.dep_pe, o.dep_all, o.pe_total);
                     for (unsigned spin = 0; !cmp_u64(cmp, ld_relaxed_u64(sig), o.value); ++spin)
                         if (spin > 64) __nanosleep(32);
-                    fence_acquire();
-                    count_done(done, ep.npes, o.kind, o.initiator);
+                    if (o.kind & (TF_CNT_PE | TF_CNT_ALL)) {     // some later op of this launch follows the wait
+                        fence_acquire();
+                        count_done(done, ep.npes, o.kind, o.initiator);
+                    }                                            // else: the end of the kernel orders everything after it
                 }
             } else if (gt < (int)r.nbytes) {
                 const AuxRec o = ld_rec(reinterpret_cast<const AuxRec *>(r.src) + gt);
@@ -616,9 +618,13 @@ extern "C" int shmemg_batch_create(shmemg_world_t *w, const shmemg_op_t *ops, si
 
     // forward pass: dependencies.  issued[p] = counted units of PE p so far; thresh[p] = what p's next unit must see.
     // (Only counted units advance done[], and every unit before a marker that a later unit depends on is counted.)
-    // A wait only polls a local word: it follows the PE's fences / quiets (thresh_mark) but not its earlier waits, so the
-    // waits of one PE are polled concurrently; the PE's later real ops follow every one of them (thresh).
-    std::vector<uint32_t> issued(w->npes, 0), thresh(w->npes, 0), thresh_mark(w->npes, 0);
+    // Consecutive waits of one PE (no other unit of that PE between them) share the threshold that was in force when the
+    // run began, so they are polled concurrently; the threshold moves past the whole run at the PE's next unit
+    // (wait_run[p]).  A wait must NOT get a weaker threshold than that: done[p] counts completions in any order, and
+    // "done[p] >= issued-before-marker" means "everything before the marker is complete" only if nothing after the
+    // marker can count before the marker's threshold is reached.
+    std::vector<uint32_t> issued(w->npes, 0), thresh(w->npes, 0);
+    std::vector<uint8_t> wait_run(w->npes, 0);
     uint32_t all_issued = 0, all_thresh = 0, run_kind = 0;
     size_t k = 0, nt = 0, na = 0, run = 0;
     std::vector<Piece> pieces;
@@ -627,10 +633,11 @@ extern "C" int shmemg_batch_create(shmemg_world_t *w, const shmemg_op_t *ops, si
     for (size_t ui = 0; ui < nu; ++ui) {
         const Unit &u = units[ui];
         const shmemg_op_t &o = ops[u.first];
-        if (u.opc == SHMEMG_OP_FENCE || u.opc == SHMEMG_OP_QUIET) { thresh[u.pe] = thresh_mark[u.pe] = issued[u.pe]; run = 0; continue; }
+        if (u.opc == SHMEMG_OP_FENCE || u.opc == SHMEMG_OP_QUIET) { thresh[u.pe] = issued[u.pe]; wait_run[u.pe] = 0; run = 0; continue; }
         if (u.opc == SHMEMG_OP_BARRIER_ALL) { all_thresh = all_issued; run = 0; continue; }
         const int ini = u.pe;
         const uint32_t flags = ((cnt[ui] & 1) ? TF_CNT_PE : 0) | ((cnt[ui] & 2) ? TF_CNT_ALL : 0);
+        if (wait_run[ini] && u.opc != SHMEMG_OP_SIGNAL_WAIT_UNTIL) { thresh[ini] = issued[ini]; wait_run[ini] = 0; }
         const uint32_t dep_pe = thresh[ini], dep_all = all_thresh;
         if (is_amo(u.opc)) {
             AuxRec &d = aux[na];
@@ -652,7 +659,7 @@ extern "C" int shmemg_batch_create(shmemg_world_t *w, const shmemg_op_t *ops, si
             d.word = (uint64_t)shmemg_addr(w, ini, o.loc_off);
             d.value = o.value;
             d.kind = SHMEMG_OP_SIGNAL_WAIT_UNTIL | ((uint32_t)o.cmp << 8) | flags;
-            d.initiator = (uint32_t)ini; d.dep_pe = thresh_mark[ini]; d.dep_all = dep_all; d.pe_total = pe_total[ini];
+            d.initiator = (uint32_t)ini; d.dep_pe = dep_pe; d.dep_all = dep_all; d.pe_total = pe_total[ini];
             if (run == 0 || run == WAIT_RUN_MAX || run_kind != T_WAIT) {
                 TileRec &t = tiles[nt++];
                 t.kind = T_WAIT; t.nbytes = 0; t.nt = 1; t.op = (uint32_t)k;
@@ -683,7 +690,7 @@ extern "C" int shmemg_batch_create(shmemg_world_t *w, const shmemg_op_t *ops, si
         }
         if (cnt[ui] & 1) issued[ini]++;
         if (cnt[ui] & 2) all_issued++;
-        if (u.opc == SHMEMG_OP_SIGNAL_WAIT_UNTIL) thresh[ini] = issued[ini];   // later ops of this PE follow the wait
+        if (u.opc == SHMEMG_OP_SIGNAL_WAIT_UNTIL) wait_run[ini] = 1;           // later ops of this PE follow the run of waits
         k++;
     }
 

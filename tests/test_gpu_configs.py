@@ -120,6 +120,35 @@ def test_atomic_add_heavy_contention_and_scalar_value():
     assert v[0, :3].tolist() == (-2 * cnt).tolist() and v[1].sum() == 0
 
 
+@pytest.mark.parametrize("n", [1, 1025, 3 * 8192 + 77, (1 << 20) + 5])
+@pytest.mark.parametrize("flags", [0, AMO_WARP_AGGREGATE])
+@pytest.mark.parametrize("idx_dtype", [np.int64, np.uint32])
+def test_fetch_add_skewed_scalar_value_ragged(n, flags, idx_dtype):
+    """Ragged sizes, a skewed key distribution (many duplicates inside one warp), a scalar value > 1, non-zero initial
+    contents, an array that does not start at offset 0; per word the fetched values must be a permutation of the prefix
+    sums and the final words bit-exact."""
+    npes, words = 3, 5000
+    w = World(npes, words * 8 + 8192, DEV)
+    pad = w.malloc(256)                                      # the array does not start at offset 0
+    a = w.malloc(words * 8)
+    init = (gen.u64(npes * words, 77) >> np.uint64(2)).reshape(npes, words)
+    w.view(a, words * 8, torch.int64).copy_(torch.from_numpy(init.view(np.int64)))
+    r = gen.u64(n, 78)
+    key = ((r % np.uint64(npes * words)) >> (r >> np.uint64(60))).astype(np.int64)      # skewed towards small keys
+    tgt, idx = (key // words).astype(np.int32), (key % words).astype(idx_dtype)
+    f = torch.empty(n, dtype=torch.int64, device=DEV)
+    w.atomic_fetch_add_batch(a, to_dev(tgt), to_dev(idx), f, val=None, val_scalar=7, flags=flags)
+    w.quiet(0)
+    fin = w.view(a, words * 8, torch.int64).cpu().numpy().view(np.uint64).reshape(-1)
+    ow = orc.OracleWorld(npes, words * 8 + 8192)
+    ow.malloc(256)
+    oa = ow.malloc(words * 8)
+    ow.view(oa, words * 8, np.uint64)[:] = init
+    ow.atomic_fetch_add_batch(oa, tgt, idx.astype(np.int64), np.full(n, 7, dtype=np.uint64))
+    assert np.array_equal(fin, ow.view(oa, words * 8, np.uint64).reshape(-1))           # final words bit-exact
+    check_fetch_add(key, np.full(n, 7, dtype=np.uint64), f.cpu().numpy().view(np.uint64), init.reshape(-1), fin)
+
+
 # ---- C4 ---------------------------------------------------------------------------------------------------------
 def _run_c4(g, flags):
     vpp, E = g.verts_per_pe, len(g.u)

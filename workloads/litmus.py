@@ -162,3 +162,32 @@ def random_amos(npes: int = 8, nwords: int = 64, n_ops: int = 20000, seed: int =
             prog.atomic_compare_swap(p, int(tgt[i]), ("words", (nwords // 2 + int(word[i])) * 8),
                                      0xFFFFFFFFFFFFFFFF, i + 1, ("fetch", i * 8))
     return prog
+
+
+def wait_after_wait(npes: int = 4, groups: int = 6, chain: int = 24, nbytes: int = 1 << 20, seed: int = 16) -> Program:
+    """A later wait of a PE that is satisfied EARLIER than the PE's previous wait must not let the ops between them start.
+    Per group g (three PEs c, e, l; consumer c):  e: PUT_SIGNAL -> c (sig_early), at once.   l: `chain` x (PUT to itself;
+    QUIET), then PUT_SIGNAL data -> c (sig_late).   c: WAIT sig_late; GET data -> out; WAIT sig_early; GET early -> out2.
+    An executor that lets the second wait complete (and be counted) before the first one is satisfied starts the first GET
+    on stale data."""
+    assert npes >= 3
+    prog = Program(npes)
+    prog.obj("src", groups * nbytes, _payload(npes, groups * nbytes, seed, 0))
+    prog.obj("scratch", nbytes)
+    prog.obj("data", groups * nbytes)
+    prog.obj("early", groups * 64)
+    prog.obj("out", groups * nbytes)
+    prog.obj("out2", groups * 64)
+    prog.obj("sig", groups * 16)
+    for g in range(groups):
+        c, e, l = g % npes, (g + 1) % npes, (g + 2) % npes
+        prog.put_signal(e, c, ("early", g * 64), ("src", g * 64), 64, ("sig", g * 16 + 8), g + 1, SIGNAL_SET)
+        for _ in range(chain):
+            prog.put(l, l, ("scratch", 0), ("src", g * nbytes), nbytes)
+            prog.quiet(l)
+        prog.put_signal(l, c, ("data", g * nbytes), ("src", g * nbytes), nbytes, ("sig", g * 16), g + 1, SIGNAL_SET)
+        prog.signal_wait_until(c, ("sig", g * 16), CMP_EQ, g + 1)
+        prog.get(c, c, ("out", g * nbytes), ("data", g * nbytes), nbytes)
+        prog.signal_wait_until(c, ("sig", g * 16 + 8), CMP_EQ, g + 1)
+        prog.get(c, c, ("out2", g * 64), ("early", g * 64), 64)
+    return prog
