@@ -46,15 +46,15 @@ BARRIERS = 10000
 M64 = (1 << 64) - 1
 
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of each copy-class segment's kernel, from the `ncu --set full`
-# captures summarised in profiles/r01b_ncu_full.md (cold L2 at launch, up to 126 MB of the kernel's own writes still in
+# captures summarised in profiles/r01c_ncu_full.md (cold L2 at launch, up to 126 MB of the kernel's own writes still in
 # L2 at its end, so write traffic < algorithmic writes; the halo faces are L2-resident by nature).
 NCU_TRAFFIC = {
-    "alltoall": 268449024 + 221673728,
-    "put_batch_skewed": 198664960 + 151857152,
-    "halo_put_signal_wait": 25207296 + 120064,
-    "sum_reduce_f32": 536885760 + 478708224,
-    "sum_reduce_i64": 536973312 + 479942656,
-    "fcollect": 4599552 + 477103872,
+    "alltoall": 268450304 + 221164032,
+    "put_batch_skewed": 198646272 + 151099392,
+    "halo_put_signal_wait": 25210368 + 143872,
+    "sum_reduce_f32": 536884224 + 478725888,
+    "sum_reduce_i64": 536912896 + 479576576,
+    "fcollect": 4208640 + 476806656,
 }
 
 
@@ -761,7 +761,7 @@ def run_cuda(args):
                     "frac": b / s / 1e9 / peak, "peak_source": peak_src, "share_of_copy_time": s / copy_s,
                     "algorithmic_bytes_per_launch": b // nl, "avg_launch_us": s / nl * 1e6,
                     "traffic": (tr // nl) if tr_ok and not inp.small else None,
-                    "traffic_source": "profiles/r01b_ncu_full.md (launch-weighted mean over the kernel's segments)"}
+                    "traffic_source": "profiles/r01c_ncu_full.md (launch-weighted mean over the kernel's segments)"}
 
     line = base_line(args, world)
     line.update({"value": gbps, "amo_mops": mops, "ms_per_step": whole_ms / K,

@@ -55,6 +55,11 @@ def lib():
         L.orc_sum_reduce_i64.argtypes = [vp, i, u64, u64, u64, u64]
         L.orc_fcollect.argtypes = [vp, i, u64, u64, u64, u64]
         L.orc_alltoall.argtypes = [vp, i, u64, u64, u64, u64]
+        L.orc_broadcast.argtypes = [vp, i, u64, u64, u64, u64, i]
+        L.orc_reduce.argtypes = [vp, i, u64, i, i, u64, u64, u64]
+        L.orc_amo_batch.argtypes = [vp, i, u64, i, i, u64, vp, vp, vp, vp, u64]
+        L.orc_ibput.argtypes = [vp, i, u64, u64, u64, u64, u64, u64, u64, i, i, i]
+        L.orc_signal_test.argtypes = [vp, i, u64, u64, i, u64, i]
         L.orc_halo_delta.argtypes = [u64, u64, u64]
         L.orc_halo_delta.restype = C.c_double
         L.orc_halo_perturb.argtypes = [vp, u64, i, i, i, u64, u64]
@@ -189,6 +194,44 @@ class OracleWorld:
     def alltoall(self, dst_off, src_off, nbytes):
         _chk(lib().orc_alltoall(self.heap.ctypes.data, self.npes, self.heap_bytes, dst_off, src_off, nbytes),
              "alltoall")
+
+
+    # ---- NEXT-2 surface: broadcast, general reductions, generic AMOs, block-strided put/get, test ----
+    RED = {"sum": 0, "prod": 1, "min": 2, "max": 3, "and": 4, "or": 5, "xor": 6}
+    DTYPE = {"f32": 0, "i64": 1, "i32": 2, "f64": 3}
+    AMO = {"add": 0, "and": 1, "or": 2, "xor": 3, "swap": 4, "fetch": 5}
+
+    def broadcast(self, dst_off, src_off, nbytes, root):
+        _chk(lib().orc_broadcast(self.heap.ctypes.data, self.npes, self.heap_bytes, dst_off, src_off, nbytes, root),
+             "broadcast")
+
+    def reduce(self, op: str, dtype: str, dst_off, src_off, nreduce):
+        _chk(lib().orc_reduce(self.heap.ctypes.data, self.npes, self.heap_bytes, self.RED[op], self.DTYPE[dtype],
+                              dst_off, src_off, nreduce), "reduce")
+
+    def amo_batch(self, op: str, width: int, sym_off, tgt_pe, idx, val=None, fetch: bool = False):
+        tgt_pe = np.ascontiguousarray(tgt_pe, dtype=np.int32)
+        idx = _u64arr(idx)
+        val = None if val is None else _u64arr(val)
+        fetched = np.empty(len(idx), dtype=np.uint64) if fetch else None
+        _chk(lib().orc_amo_batch(self.heap.ctypes.data, self.npes, self.heap_bytes, self.AMO[op], width, sym_off,
+                                 tgt_pe.ctypes.data, idx.ctypes.data, None if val is None else val.ctypes.data,
+                                 fetched.ctypes.data if fetch else None, len(idx)), "amo_batch")
+        return fetched
+
+    def ibput(self, dst_off, src_off, dst_stride, src_stride, block, nblocks, pe, target):
+        _chk(lib().orc_ibput(self.heap.ctypes.data, self.npes, self.heap_bytes, dst_off, src_off, dst_stride,
+                             src_stride, block, nblocks, pe, target, 0), "ibput")
+
+    def ibget(self, dst_off, src_off, dst_stride, src_stride, block, nblocks, pe, target):
+        _chk(lib().orc_ibput(self.heap.ctypes.data, self.npes, self.heap_bytes, dst_off, src_off, dst_stride,
+                             src_stride, block, nblocks, pe, target, 1), "ibget")
+
+    def signal_test(self, sig_off, cmp, value, pe) -> bool:
+        r = lib().orc_signal_test(self.heap.ctypes.data, self.npes, self.heap_bytes, sig_off, cmp, value, pe)
+        if r < 0:
+            raise OracleError("signal_test: bad argument")
+        return bool(r)
 
 
 # ---- halo application compute (config C2) ----------------------------------------------------------

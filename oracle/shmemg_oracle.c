@@ -242,6 +242,146 @@ int orc_alltoall(uint8_t *heap, int npes, uint64_t heap_bytes, uint64_t dst_off,
     return ORC_OK;
 }
 
+/* ---- the rest of the OpenSHMEM op surface on the same heaps --------------
+ * The paper names these only by reference: broadcast among the host-side _on_stream variants (L218),
+ * "quiet, wait, and test" (L392), the AMO set and strided transfers through "inherited unchanged from
+ * OpenSHMEM 1.6" (L361).  Each is its plain definition, executed sequentially. */
+
+/* broadcast (team-based form): for all j (root included): heap[j][dst : +n] = heap[root][src : +n].  L218. */
+int orc_broadcast(uint8_t *heap, int npes, uint64_t heap_bytes, uint64_t dst_off, uint64_t src_off, uint64_t n,
+                  int root) {
+    if (root < 0 || root >= npes) return ORC_ERR_RANGE;
+    if (!in_range(src_off, n, heap_bytes) || !in_range(dst_off, n, heap_bytes)) return ORC_ERR_RANGE;
+    if (!(src_off + n <= dst_off || dst_off + n <= src_off)) return ORC_ERR_RANGE;
+    for (int j = 0; j < npes; ++j)
+        memcpy(heap + (uint64_t)j * heap_bytes + dst_off, heap + (uint64_t)root * heap_bytes + src_off, n);
+    return ORC_OK;
+}
+
+/* reductions: every PE's dest[k] = op over p (ASCENDING PE order) of source[k] on PE p (all-reduce).
+ * dtypes: 0 = fp32 (sum / prod accumulated in fp64, rounded to fp32 once; min / max exact),
+ *         1 = int64, 2 = int32 (wraparound two's-complement sum / prod; signed min / max; bitwise),
+ *         3 = fp64 (sum / prod accumulated in fp64 in PE order; min / max exact).
+ * Inputs of the floating-point reductions are NaN-free (undefined otherwise). */
+enum { ORC_RED_SUM = 0, ORC_RED_PROD, ORC_RED_MIN, ORC_RED_MAX, ORC_RED_AND, ORC_RED_OR, ORC_RED_XOR };
+enum { ORC_T_F32 = 0, ORC_T_I64 = 1, ORC_T_I32 = 2, ORC_T_F64 = 3 };
+
+static double red_f(int op, double a, double b) {
+    switch (op) {
+    case ORC_RED_SUM: return a + b;
+    case ORC_RED_PROD: return a * b;
+    case ORC_RED_MIN: return b < a ? b : a;
+    default: return b > a ? b : a;
+    }
+}
+static uint64_t red_u(int op, uint64_t a, uint64_t b, int is32) {
+    switch (op) {
+    case ORC_RED_SUM: return a + b;
+    case ORC_RED_PROD: return a * b;
+    case ORC_RED_MIN: return is32 ? ((int32_t)b < (int32_t)a ? b : a) : ((int64_t)b < (int64_t)a ? b : a);
+    case ORC_RED_MAX: return is32 ? ((int32_t)b > (int32_t)a ? b : a) : ((int64_t)b > (int64_t)a ? b : a);
+    case ORC_RED_AND: return a & b;
+    case ORC_RED_OR: return a | b;
+    default: return a ^ b;
+    }
+}
+
+int orc_reduce(uint8_t *heap, int npes, uint64_t heap_bytes, int op, int dtype, uint64_t dst_off, uint64_t src_off,
+               uint64_t nreduce) {
+    const uint64_t es = (dtype == ORC_T_I64 || dtype == ORC_T_F64) ? 8 : 4;
+    if (op < ORC_RED_SUM || op > ORC_RED_XOR || dtype < ORC_T_F32 || dtype > ORC_T_F64) return ORC_ERR_OPCODE;
+    if ((dtype == ORC_T_F32 || dtype == ORC_T_F64) && op >= ORC_RED_AND) return ORC_ERR_OPCODE;
+    if (!in_range(src_off, es * nreduce, heap_bytes) || !in_range(dst_off, es * nreduce, heap_bytes)) return ORC_ERR_RANGE;
+    for (uint64_t k = 0; k < nreduce; ++k) {
+        uint8_t out[8];
+        if (dtype == ORC_T_F32 || dtype == ORC_T_F64) {
+            double acc = 0.0;
+            for (int p = 0; p < npes; ++p) {
+                const uint8_t *q = heap + (uint64_t)p * heap_bytes + src_off + es * k;
+                double x;
+                if (dtype == ORC_T_F32) { float f; memcpy(&f, q, 4); x = (double)f; } else memcpy(&x, q, 8);
+                acc = p == 0 ? x : red_f(op, acc, x);
+            }
+            if (dtype == ORC_T_F32) { float f = (float)acc; memcpy(out, &f, 4); } else memcpy(out, &acc, 8);
+        } else {
+            uint64_t acc = 0;
+            for (int p = 0; p < npes; ++p) {
+                const uint8_t *q = heap + (uint64_t)p * heap_bytes + src_off + es * k;
+                uint64_t x = 0;
+                memcpy(&x, q, es);
+                acc = p == 0 ? x : red_u(op, acc, x, es == 4);
+            }
+            memcpy(out, &acc, es);          /* little-endian: the low `es` bytes */
+        }
+        for (int p = 0; p < npes; ++p) memcpy(heap + (uint64_t)p * heap_bytes + dst_off + es * k, out, es);
+    }
+    return ORC_OK;
+}
+
+/* generic AMO batch, structure-of-arrays, executed in index order on `width`-byte words (4 or 8):
+ *   word = heap[tgt_pe[i]][sym_off + width*idx[i]];  old = word;  word = f(old, val[i]);  fetched[i] = old (if asked).
+ * ADD / AND / OR / XOR; SWAP (word = val; without `fetched` this is atomic_set); FETCH (word unchanged: atomic_fetch).
+ * inc / fetch_inc are ADD with val = 1.  (OpenSHMEM 1.6 AMO set, L361.) */
+enum { ORC_AMO_ADD = 0, ORC_AMO_AND, ORC_AMO_OR, ORC_AMO_XOR, ORC_AMO_SWAP, ORC_AMO_FETCH };
+
+int orc_amo_batch(uint8_t *heap, int npes, uint64_t heap_bytes, int op, int width, uint64_t sym_off,
+                  const int32_t *tgt_pe, const uint64_t *idx, const uint64_t *val, uint64_t *fetched, uint64_t n) {
+    if (op < ORC_AMO_ADD || op > ORC_AMO_FETCH || (width != 4 && width != 8)) return ORC_ERR_OPCODE;
+    if (sym_off % (uint64_t)width) return ORC_ERR_ALIGN;
+    const uint64_t mask = width == 8 ? ~0ull : 0xffffffffull;
+    for (uint64_t i = 0; i < n; ++i) {
+        if (tgt_pe[i] < 0 || tgt_pe[i] >= npes || !in_range(sym_off + (uint64_t)width * idx[i], (uint64_t)width, heap_bytes))
+            return ORC_ERR_RANGE;
+        uint8_t *w = heap + (uint64_t)tgt_pe[i] * heap_bytes + sym_off + (uint64_t)width * idx[i];
+        uint64_t old = 0, v = val ? (val[i] & mask) : 0, nw;
+        memcpy(&old, w, (size_t)width);
+        switch (op) {
+        case ORC_AMO_ADD: nw = old + v; break;
+        case ORC_AMO_AND: nw = old & v; break;
+        case ORC_AMO_OR: nw = old | v; break;
+        case ORC_AMO_XOR: nw = old ^ v; break;
+        case ORC_AMO_SWAP: nw = v; break;
+        default: nw = old; break;
+        }
+        nw &= mask;
+        memcpy(w, &nw, (size_t)width);
+        if (fetched) fetched[i] = old;
+    }
+    return ORC_OK;
+}
+
+/* block-strided put / get (OpenSHMEM 1.6 ibput / ibget; iput / iget are the case block = one element):
+ * for b in [0, nblocks): dest[b*dst_stride : +block] = source[b*src_stride : +block], strides in BYTES.
+ * put: source on `pe`, dest on `target`; get: source on `target`, dest on `pe`. */
+int orc_ibput(uint8_t *heap, int npes, uint64_t heap_bytes, uint64_t dst_off, uint64_t src_off, uint64_t dst_stride,
+              uint64_t src_stride, uint64_t block, uint64_t nblocks, int pe, int target, int is_get) {
+    if (pe < 0 || pe >= npes || target < 0 || target >= npes) return ORC_ERR_RANGE;
+    if (nblocks == 0 || block == 0) return ORC_OK;
+    if (!in_range(dst_off, (nblocks - 1) * dst_stride + block, heap_bytes) ||
+        !in_range(src_off, (nblocks - 1) * src_stride + block, heap_bytes)) return ORC_ERR_RANGE;
+    const int dpe = is_get ? pe : target, spe = is_get ? target : pe;
+    for (uint64_t b = 0; b < nblocks; ++b)
+        memmove(heap + (uint64_t)dpe * heap_bytes + dst_off + b * dst_stride,
+                heap + (uint64_t)spe * heap_bytes + src_off + b * src_stride, block);
+    return ORC_OK;
+}
+
+/* signal test (L392): 1 if cmp(heap[pe][sig_off] as u64, value) holds now, else 0; never blocks. */
+int orc_signal_test(const uint8_t *heap, int npes, uint64_t heap_bytes, uint64_t sig_off, int cmp, uint64_t value,
+                    int pe) {
+    if (pe < 0 || pe >= npes || !in_range(sig_off, 8, heap_bytes) || (sig_off & 7)) return -1;
+    const uint64_t s = ld64(heap + (uint64_t)pe * heap_bytes + sig_off);
+    switch (cmp) {
+    case ORC_CMP_EQ: return s == value;
+    case ORC_CMP_NE: return s != value;
+    case ORC_CMP_GT: return s > value;
+    case ORC_CMP_GE: return s >= value;
+    case ORC_CMP_LT: return s < value;
+    case ORC_CMP_LE: return s <= value;
+    default: return -1;
+    }
+}
+
 /* ---- application-side compute of the halo workload (config C2; SURVEY.md readings 21-23) ------
  * Not part of the specification's operations: the stencil application's own kernels, restated on
  * the CPU so the oracle can run the whole workload.  Both sides implement the same counter-based
