@@ -235,13 +235,56 @@ SHMEMG_API int shmemg_atomic_compare_swap_batch_on_stream(shmemg_world_t *w, uin
                                                           uint64_t val_scalar, uint64_t *fetched_out, size_t n,
                                                           uint32_t flags, void *stream);
 
+/* Generic AMO batch on `width`-byte words (4 or 8), structure-of-arrays like the calls above (the AMO set of OpenSHMEM 1.6,
+ * inherited unchanged): word = heap[tgt_pe[i]][sym_off + width*elem_idx[i]]; old = word; word = f(old, val[i]);
+ * fetched_out[i] = old when fetched_out != NULL (zero-extended to 64 bits).  ADD / AND / OR / XOR; SWAP (word = val;
+ * with fetched_out == NULL this is atomic_set); FETCH (atomic read, fetched_out required, val ignored).  inc / fetch_inc
+ * are ADD with val_scalar = 1.  `val` (DEVICE, 64-bit entries, low `width` bytes used) may be NULL -> val_scalar.
+ * Non-fetching ops use red.global / st, fetching ops atom.global / ld.  No ordering between the ops of one call. */
+enum { SHMEMG_AMO_ADD = 0, SHMEMG_AMO_AND = 1, SHMEMG_AMO_OR = 2, SHMEMG_AMO_XOR = 3, SHMEMG_AMO_SWAP = 4,
+       SHMEMG_AMO_FETCH = 5 };
+SHMEMG_API int shmemg_atomic_op_batch_on_stream(shmemg_world_t *w, int amo, int width, uint64_t sym_off,
+                                                const int32_t *tgt_pe, const void *elem_idx, int idx_bytes,
+                                                const uint64_t *val, uint64_t val_scalar, uint64_t *fetched_out,
+                                                size_t n, void *stream);
+
+/* ---- block-strided put / get (OpenSHMEM 1.6 ibput / ibget; iput / iget are the case block = one element) ---------------
+ * for b in [0, nblocks): dest[b*dst_stride .. +block_bytes) = source[b*src_stride .. +block_bytes); strides in BYTES, any
+ * size and alignment.  put: source in `pe`'s window, dest in `target_pe`'s; get: source in `target_pe`'s, dest in `pe`'s.
+ * Destination blocks must not overlap each other or the source (undefined otherwise).  Stream-ordered like put / get. */
+SHMEMG_API int shmemg_ibput_on_stream(shmemg_world_t *w, uint64_t dest_off, uint64_t source_off, uint64_t dst_stride,
+                                      uint64_t src_stride, size_t block_bytes, size_t nblocks, int pe, int target_pe,
+                                      void *stream);
+SHMEMG_API int shmemg_ibget_on_stream(shmemg_world_t *w, uint64_t dest_off, uint64_t source_off, uint64_t dst_stride,
+                                      uint64_t src_stride, size_t block_bytes, size_t nblocks, int pe, int target_pe,
+                                      void *stream);
+
+/* signal test ("quiet, wait, and test"): *result_dev (DEVICE int32) = 1 if cmp(u64 heap[pe][sig_off], value)
+ * holds when the stream reaches the call, else 0; never blocks.  A result of 1 is an acquire: work enqueued later on the
+ * stream sees the payload the signal announced. */
+SHMEMG_API int shmemg_signal_test_on_stream(shmemg_world_t *w, uint64_t sig_off, int cmp, uint64_t value, int pe,
+                                            int32_t *result_dev, void *stream);
+
 /* ---- collectives on SHMEM_TEAM_WORLD, one kernel each --------------------------
  * Each collective is one atomic unit in stream order (kernel boundaries order it against its neighbours). */
-enum { SHMEMG_F32 = 0, SHMEMG_I64 = 1 };
+enum { SHMEMG_F32 = 0, SHMEMG_I64 = 1, SHMEMG_I32 = 2, SHMEMG_F64 = 3 };
 /* every PE's dest[k] = sum over all PEs (ascending PE order) of source[k], k < nreduce.  F32 accumulates
  * in fp64 and rounds once; I64 wraps.  dest == source (exact aliasing) is allowed; partial overlap is not. */
 SHMEMG_API int shmemg_sum_reduce_on_stream(shmemg_world_t *w, int dtype, uint64_t dest_off, uint64_t source_off,
                                            size_t nreduce, void *stream);
+/* General reduction (the reduction set OpenSHMEM 1.6 defines, inherited unchanged):
+ * every PE's dest[k] = op over all PEs (ascending PE order) of source[k].  SUM / PROD: fp32 accumulates in fp64 and rounds
+ * once, fp64 accumulates in fp64, integers wrap.  MIN / MAX: signed for I32 / I64; floating-point inputs must be NaN-free.
+ * AND / OR / XOR: I32 / I64 only (SHMEMG_ERR_ARG on F32 / F64).  Aliasing rules as for sum_reduce. */
+enum { SHMEMG_RED_SUM = 0, SHMEMG_RED_PROD = 1, SHMEMG_RED_MIN = 2, SHMEMG_RED_MAX = 3, SHMEMG_RED_AND = 4,
+       SHMEMG_RED_OR = 5, SHMEMG_RED_XOR = 6 };
+SHMEMG_API int shmemg_reduce_on_stream(shmemg_world_t *w, int op, int dtype, uint64_t dest_off, uint64_t source_off,
+                                       size_t nreduce, void *stream);
+/* broadcast (named among the stream-ordered collectives; team-based form): every PE's dest[0 .. nbytes),
+ * the root's included, = the root's source[0 .. nbytes).  Any size and alignment; source and dest ranges must not
+ * overlap (SHMEMG_ERR_OVERLAP). */
+SHMEMG_API int shmemg_broadcast_on_stream(shmemg_world_t *w, uint64_t dest_off, uint64_t source_off, size_t nbytes,
+                                          int root_pe, void *stream);
 /* every PE's dest[p*nbytes .. +nbytes) = PE p's source[0 .. nbytes)  (concatenation in PE order). */
 SHMEMG_API int shmemg_fcollect_on_stream(shmemg_world_t *w, uint64_t dest_off, uint64_t source_off, size_t nbytes,
                                          void *stream);

@@ -300,7 +300,7 @@ int orc_reduce(uint8_t *heap, int npes, uint64_t heap_bytes, int op, int dtype, 
                 const uint8_t *q = heap + (uint64_t)p * heap_bytes + src_off + es * k;
                 double x;
                 if (dtype == ORC_T_F32) { float f; memcpy(&f, q, 4); x = (double)f; } else memcpy(&x, q, 8);
-                acc = p == 0 ? x : red_f(op, acc, x);
+                acc = p == 0 ? (op == ORC_RED_SUM ? 0.0 + x : x) : red_f(op, acc, x);   /* SUM starts from +0.0, as orc_sum_reduce_f32 */
             }
             if (dtype == ORC_T_F32) { float f = (float)acc; memcpy(out, &f, 4); } else memcpy(out, &acc, 8);
         } else {

@@ -62,7 +62,17 @@ class CAP:
     DEVICE_BARRIER = 1 << 13
 
 
-F32, I64 = 0, 1
+F32, I64, I32, F64 = 0, 1, 2, 3
+
+
+class RED:
+    SUM, PROD, MIN, MAX, AND, OR, XOR = range(7)
+
+
+class AMO:
+    ADD, AND, OR, XOR, SWAP, FETCH = range(6)
+
+
 AMO_WARP_AGGREGATE = 1
 AMO_TEST_BEFORE_SWAP = 2
 NO_STAMP = (1 << 64) - 1
@@ -109,6 +119,12 @@ SYMBOLS = {
     "shmemg_atomic_fetch_add_batch_on_stream": (_i, [_vp, _u64, _vp, _vp, _i, _vp, _u64, _vp, _sz, _u32, _vp]),
     "shmemg_atomic_compare_swap_batch_on_stream": (_i, [_vp, _u64, _vp, _vp, _i, _vp, _u64, _vp, _u64, _vp, _sz, _u32, _vp]),
     "shmemg_sum_reduce_on_stream": (_i, [_vp, _i, _u64, _u64, _sz, _vp]),
+    "shmemg_reduce_on_stream": (_i, [_vp, _i, _i, _u64, _u64, _sz, _vp]),
+    "shmemg_broadcast_on_stream": (_i, [_vp, _u64, _u64, _sz, _i, _vp]),
+    "shmemg_atomic_op_batch_on_stream": (_i, [_vp, _i, _i, _u64, _vp, _vp, _i, _vp, _u64, _vp, _sz, _vp]),
+    "shmemg_ibput_on_stream": (_i, [_vp, _u64, _u64, _u64, _u64, _sz, _sz, _i, _i, _vp]),
+    "shmemg_ibget_on_stream": (_i, [_vp, _u64, _u64, _u64, _u64, _sz, _sz, _i, _i, _vp]),
+    "shmemg_signal_test_on_stream": (_i, [_vp, _u64, _i, _u64, _i, _vp, _vp]),
     "shmemg_fcollect_on_stream": (_i, [_vp, _u64, _u64, _sz, _vp]),
     "shmemg_alltoall_on_stream": (_i, [_vp, _u64, _u64, _sz, _vp]),
     "shmemg_barrier_all_on_stream": (_i, [_vp, _vp]),
@@ -351,6 +367,42 @@ class World:
         self._chk(lib().shmemg_sum_reduce_on_stream(self.h, dtype, dest_off, source_off, nreduce, _stream(stream)),
                   "shmemg_sum_reduce_on_stream")
         self.launches += 1 if nreduce else 0
+
+    def reduce(self, op, dtype, dest_off, source_off, nreduce, stream=None):
+        self._chk(lib().shmemg_reduce_on_stream(self.h, op, dtype, dest_off, source_off, nreduce, _stream(stream)),
+                  "shmemg_reduce_on_stream")
+        self.launches += 1 if nreduce else 0
+
+    def broadcast(self, dest_off, source_off, nbytes, root_pe, stream=None):
+        self._chk(lib().shmemg_broadcast_on_stream(self.h, dest_off, source_off, nbytes, root_pe, _stream(stream)),
+                  "shmemg_broadcast_on_stream")
+        self.launches += 1 if nbytes else 0
+
+    def atomic_op_batch(self, amo, width, sym_off, tgt_pe, elem_idx, val=None, val_scalar=0, fetched_out=None, stream=None):
+        n = tgt_pe.numel()
+        assert elem_idx.numel() == n and (val is None or val.numel() == n) and (fetched_out is None or fetched_out.numel() == n)
+        self._chk(lib().shmemg_atomic_op_batch_on_stream(self.h, amo, width, sym_off, _dptr(tgt_pe), _dptr(elem_idx),
+                                                         self._idx_bytes(elem_idx), _dptr(val), val_scalar & ((1 << 64) - 1),
+                                                         _dptr(fetched_out), n, _stream(stream)),
+                  "shmemg_atomic_op_batch_on_stream")
+        self.launches += 1 if n else 0
+
+    def ibput(self, dest_off, source_off, dst_stride, src_stride, block_bytes, nblocks, pe, target_pe, stream=None):
+        self._chk(lib().shmemg_ibput_on_stream(self.h, dest_off, source_off, dst_stride, src_stride, block_bytes, nblocks,
+                                               pe, target_pe, _stream(stream)), "shmemg_ibput_on_stream")
+        self.launches += 1 if block_bytes and nblocks else 0
+
+    def ibget(self, dest_off, source_off, dst_stride, src_stride, block_bytes, nblocks, pe, target_pe, stream=None):
+        self._chk(lib().shmemg_ibget_on_stream(self.h, dest_off, source_off, dst_stride, src_stride, block_bytes, nblocks,
+                                               pe, target_pe, _stream(stream)), "shmemg_ibget_on_stream")
+        self.launches += 1 if block_bytes and nblocks else 0
+
+    def signal_test(self, sig_off, cmp, value, pe, result_dev, stream=None):
+        """result_dev: a 1-element int32 CUDA tensor; read it after synchronising the stream."""
+        assert result_dev.dtype == torch.int32
+        self._chk(lib().shmemg_signal_test_on_stream(self.h, sig_off, cmp, value & ((1 << 64) - 1), pe, _dptr(result_dev),
+                                                     _stream(stream)), "shmemg_signal_test_on_stream")
+        self.launches += 1
 
     def fcollect(self, dest_off, source_off, nbytes, stream=None):
         self._chk(lib().shmemg_fcollect_on_stream(self.h, dest_off, source_off, nbytes, _stream(stream)),

@@ -160,7 +160,78 @@ k_fcollect_bytes(uint8_t *base, size_t stride, uint64_t dst_off, uint64_t src_of
 #define RED_CTA (64 + RED_THREADS)
 #define RED_SMEM ((size_t)RS * RG * RT + 2 * RT)
 
-template <int DT>
+// ---- element math of the reductions (a15 + NEXT-2): one 16-byte vector = 4 x fp32 / 4 x int32 / 2 x fp64 / 2 x int64.
+// fp32 SUM / PROD accumulate in fp64 and round once (reading 13); everything else is computed in its own type.
+// Accumulators start at the operation's identity, which gives the same bits as folding the PEs in ascending order for
+// NaN-free inputs (SUM starts from +0.0, so an all -0.0 column sums to +0.0: DESIGN.md reading 13).
+template <int OP> __device__ __forceinline__ double red_f64(double a, double b) {
+    return OP == SHMEMG_RED_SUM ? a + b : OP == SHMEMG_RED_PROD ? a * b : OP == SHMEMG_RED_MIN ? (b < a ? b : a) : (b > a ? b : a);
+}
+template <int OP, typename U, typename S> __device__ __forceinline__ U red_int(U a, U b) {
+    switch (OP) {
+    case SHMEMG_RED_SUM: return a + b;
+    case SHMEMG_RED_PROD: return a * b;
+    case SHMEMG_RED_MIN: return (S)b < (S)a ? b : a;
+    case SHMEMG_RED_MAX: return (S)b > (S)a ? b : a;
+    case SHMEMG_RED_AND: return a & b;
+    case SHMEMG_RED_OR: return a | b;
+    default: return a ^ b;
+    }
+}
+template <int OP> __device__ __forceinline__ double ident_f64() {
+    return OP == SHMEMG_RED_SUM ? 0.0 : OP == SHMEMG_RED_PROD ? 1.0 : OP == SHMEMG_RED_MIN ? __longlong_as_double(0x7ff0000000000000ll)
+                                                                                         : __longlong_as_double(0xfff0000000000000ll);
+}
+template <int OP, typename U> __device__ __forceinline__ U ident_int() {
+    switch (OP) {
+    case SHMEMG_RED_PROD: return (U)1;
+    case SHMEMG_RED_MIN: return (U)(~(U)0 >> 1);                 // signed maximum
+    case SHMEMG_RED_MAX: return (U)((U)1 << (sizeof(U) * 8 - 1));  // signed minimum
+    case SHMEMG_RED_AND: return (U)~(U)0;
+    default: return (U)0;
+    }
+}
+// accumulator of one 16-byte vector
+template <int DT, int OP> struct RedAcc {
+    double d[4];                       // F32 (4 lanes, fp64 for SUM/PROD; exact for MIN/MAX too) / F64 (2 lanes)
+    unsigned long long u[2];           // I64
+    unsigned w[4];                     // I32
+    __device__ __forceinline__ void init() {
+        if (DT == SHMEMG_F32 || DT == SHMEMG_F64) { d[0] = d[1] = d[2] = d[3] = ident_f64<OP>(); }
+        else if (DT == SHMEMG_I64) { u[0] = u[1] = ident_int<OP, unsigned long long>(); }
+        else { w[0] = w[1] = w[2] = w[3] = ident_int<OP, unsigned>(); }
+    }
+    __device__ __forceinline__ void add(const int4 &x) {
+        if (DT == SHMEMG_F32) {            // fp32 -> fp64 is exact, so MIN / MAX in fp64 are exact as well
+            d[0] = red_f64<OP>(d[0], (double)__int_as_float(x.x)); d[1] = red_f64<OP>(d[1], (double)__int_as_float(x.y));
+            d[2] = red_f64<OP>(d[2], (double)__int_as_float(x.z)); d[3] = red_f64<OP>(d[3], (double)__int_as_float(x.w));
+        } else if (DT == SHMEMG_F64) {
+            d[0] = red_f64<OP>(d[0], __hiloint2double(x.y, x.x)); d[1] = red_f64<OP>(d[1], __hiloint2double(x.w, x.z));
+        } else if (DT == SHMEMG_I64) {
+            u[0] = red_int<OP, unsigned long long, long long>(u[0], ((unsigned long long)(unsigned)x.y << 32) | (unsigned)x.x);
+            u[1] = red_int<OP, unsigned long long, long long>(u[1], ((unsigned long long)(unsigned)x.w << 32) | (unsigned)x.z);
+        } else {
+            w[0] = red_int<OP, unsigned, int>(w[0], (unsigned)x.x); w[1] = red_int<OP, unsigned, int>(w[1], (unsigned)x.y);
+            w[2] = red_int<OP, unsigned, int>(w[2], (unsigned)x.z); w[3] = red_int<OP, unsigned, int>(w[3], (unsigned)x.w);
+        }
+    }
+    __device__ __forceinline__ int4 result() const {
+        int4 r;
+        if (DT == SHMEMG_F32) {
+            r.x = __float_as_int(__double2float_rn(d[0])); r.y = __float_as_int(__double2float_rn(d[1]));
+            r.z = __float_as_int(__double2float_rn(d[2])); r.w = __float_as_int(__double2float_rn(d[3]));
+        } else if (DT == SHMEMG_F64) {
+            r.x = __double2loint(d[0]); r.y = __double2hiint(d[0]); r.z = __double2loint(d[1]); r.w = __double2hiint(d[1]);
+        } else if (DT == SHMEMG_I64) {
+            r.x = (int)(unsigned)u[0]; r.y = (int)(unsigned)(u[0] >> 32); r.z = (int)(unsigned)u[1]; r.w = (int)(unsigned)(u[1] >> 32);
+        } else {
+            r.x = (int)w[0]; r.y = (int)w[1]; r.z = (int)w[2]; r.w = (int)w[3];
+        }
+        return r;
+    }
+};
+
+template <int DT, int OP>
 __global__ void __launch_bounds__(RED_CTA, 1)
 k_sum_reduce_tma(uint8_t *base, size_t stride, uint64_t dst_off, uint64_t src_off, size_t nbytes, int npes) {
     extern __shared__ __align__(1024) uint8_t smem[];
@@ -216,10 +287,9 @@ k_sum_reduce_tma(uint8_t *base, size_t stride, uint64_t dst_off, uint64_t src_of
         for (size_t c = blockIdx.x; c < ntiles; c += gridDim.x, ++k) {
             const size_t off = c * RT;
             const unsigned tb = (unsigned)(nbytes - off < RT ? nbytes - off : RT);
-            double acc[RV][4];
-            unsigned long long ui[RV][2];
+            RedAcc<DT, OP> acc[RV];
 #pragma unroll
-            for (int v = 0; v < RV; ++v) { acc[v][0] = acc[v][1] = acc[v][2] = acc[v][3] = 0.0; ui[v][0] = ui[v][1] = 0; }
+            for (int v = 0; v < RV; ++v) acc[v].init();
             for (int g = 0; g < ngroups; ++g, ++it) {
                 const unsigned s = it % RS;
                 mbar_wait(&full[s], (it / RS) & 1u);
@@ -231,14 +301,8 @@ k_sum_reduce_tma(uint8_t *base, size_t stride, uint64_t dst_off, uint64_t src_of
                         for (int v = 0; v < RV; ++v) {
                             const unsigned o = ((unsigned)v * RED_THREADS + (unsigned)t) * 16u;
                             if (o < tb) {
-                                const int4 x = *reinterpret_cast<const int4 *>(smem + ((size_t)s * RG + j) * RT + o);
-                                if (DT == SHMEMG_F32) {       // ascending PE order, fp64 accumulate (reading 13)
-                                    acc[v][0] += (double)__int_as_float(x.x); acc[v][1] += (double)__int_as_float(x.y);
-                                    acc[v][2] += (double)__int_as_float(x.z); acc[v][3] += (double)__int_as_float(x.w);
-                                } else {
-                                    ui[v][0] += ((unsigned long long)(unsigned)x.y << 32) | (unsigned)x.x;
-                                    ui[v][1] += ((unsigned long long)(unsigned)x.w << 32) | (unsigned)x.z;
-                                }
+                                // ascending PE order (reading 13)
+                                acc[v].add(*reinterpret_cast<const int4 *>(smem + ((size_t)s * RG + j) * RT + o));
                             }
                         }
                     }
@@ -252,15 +316,7 @@ k_sum_reduce_tma(uint8_t *base, size_t stride, uint64_t dst_off, uint64_t src_of
             for (int v = 0; v < RV; ++v) {
                 const unsigned o = ((unsigned)v * RED_THREADS + (unsigned)t) * 16u;
                 if (o < tb) {
-                    int4 r;
-                    if (DT == SHMEMG_F32) {
-                        r.x = __float_as_int(__double2float_rn(acc[v][0])); r.y = __float_as_int(__double2float_rn(acc[v][1]));
-                        r.z = __float_as_int(__double2float_rn(acc[v][2])); r.w = __float_as_int(__double2float_rn(acc[v][3]));
-                    } else {
-                        r.x = (int)(unsigned)ui[v][0]; r.y = (int)(unsigned)(ui[v][0] >> 32);
-                        r.z = (int)(unsigned)ui[v][1]; r.w = (int)(unsigned)(ui[v][1] >> 32);
-                    }
-                    *reinterpret_cast<int4 *>(out + (size_t)b * RT + o) = r;
+                    *reinterpret_cast<int4 *>(out + (size_t)b * RT + o) = acc[v].result();
                 }
             }
             asm volatile("fence.proxy.async.shared::cta;" ::: "memory");    // generic writes -> visible to the bulk store
@@ -269,16 +325,27 @@ k_sum_reduce_tma(uint8_t *base, size_t stride, uint64_t dst_off, uint64_t src_of
         }
     }
 }
-// scalar tails / unaligned buffers: one element per thread
-template <typename T, typename ACC>
-__global__ void k_sum_reduce_scalar(uint8_t *base, size_t stride, uint64_t dst_off, uint64_t src_off, size_t first,
-                                    size_t n, int npes) {
+// scalar tails / unaligned buffers: one element per thread, the same element math on one lane of a vector
+template <int DT, int OP>
+__global__ void k_reduce_scalar(uint8_t *base, size_t stride, uint64_t dst_off, uint64_t src_off, size_t first, size_t n,
+                                int npes) {
+    constexpr size_t ES = (DT == SHMEMG_F32 || DT == SHMEMG_I32) ? 4 : 8;
     for (size_t k = first + (size_t)blockIdx.x * blockDim.x + threadIdx.x; k < n; k += (size_t)gridDim.x * blockDim.x) {
-        ACC acc = 0;
-        for (int p = 0; p < npes; ++p)
-            acc += (ACC) * reinterpret_cast<const volatile T *>(base + (size_t)p * stride + src_off + k * sizeof(T));
-        const T r = (T)acc;
-        for (int j = 0; j < npes; ++j) *reinterpret_cast<T *>(base + (size_t)j * stride + dst_off + k * sizeof(T)) = r;
+        RedAcc<DT, OP> acc;
+        acc.init();
+        for (int p = 0; p < npes; ++p) {
+            const uint8_t *q = base + (size_t)p * stride + src_off + k * ES;
+            int4 x = make_int4(0, 0, 0, 0);
+            x.x = (int)*reinterpret_cast<const volatile unsigned *>(q);
+            if (ES == 8) x.y = (int)*reinterpret_cast<const volatile unsigned *>(q + 4);
+            acc.add(x);
+        }
+        const int4 r = acc.result();
+        for (int j = 0; j < npes; ++j) {
+            uint8_t *q = base + (size_t)j * stride + dst_off + k * ES;
+            *reinterpret_cast<unsigned *>(q) = (unsigned)r.x;
+            if (ES == 8) *reinterpret_cast<unsigned *>(q + 4) = (unsigned)r.y;
+        }
     }
 }
 
@@ -329,8 +396,6 @@ static int collectives_smem_attr(shmemg_world *w) {
     if (w->smem_attr_coll) return SHMEMG_OK;
     SHMEMG_CUDA(w, cudaFuncSetAttribute(k_alltoall_tma, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SHMEMG_TMA_SMEM));
     SHMEMG_CUDA(w, cudaFuncSetAttribute(k_fcollect_tma, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SHMEMG_TMA_SMEM));
-    SHMEMG_CUDA(w, cudaFuncSetAttribute(k_sum_reduce_tma<SHMEMG_F32>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)RED_SMEM));
-    SHMEMG_CUDA(w, cudaFuncSetAttribute(k_sum_reduce_tma<SHMEMG_I64>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)RED_SMEM));
     w->smem_attr_coll = true;
     return SHMEMG_OK;
 }
@@ -411,10 +476,46 @@ extern "C" int shmemg_fcollect_on_stream(shmemg_world_t *w, uint64_t dest_off, u
     return SHMEMG_OK;
 }
 
-extern "C" int shmemg_sum_reduce_on_stream(shmemg_world_t *w, int dtype, uint64_t dest_off, uint64_t source_off,
-                                           size_t nreduce, void *stream) {
-    if (!w || (dtype != SHMEMG_F32 && dtype != SHMEMG_I64)) return SHMEMG_ERR_ARG;
-    const size_t esz = dtype == SHMEMG_F32 ? 4 : 8;
+template <int DT, int OP>
+static void launch_reduce(shmemg_world *w, uint64_t dest_off, uint64_t source_off, size_t nvec, size_t first, size_t nreduce,
+                          cudaStream_t st) {
+    static bool attr_set = false;
+    if (nvec) {
+        if (!attr_set) {
+            cudaFuncSetAttribute(k_sum_reduce_tma<DT, OP>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)RED_SMEM);
+            attr_set = true;
+        }
+        const size_t nb = nvec << 4, ntiles = (nb + RT - 1) / RT;
+        const unsigned grid = (unsigned)(ntiles < (size_t)w->sm_count ? ntiles : (size_t)w->sm_count);
+        k_sum_reduce_tma<DT, OP><<<grid, RED_CTA, RED_SMEM, st>>>(w->base, w->stride, dest_off, source_off, nb, w->npes);
+    }
+    if (first < nreduce) {
+        size_t blocks = (nreduce - first + 255) / 256;
+        if (blocks > 4096) blocks = 4096;
+        k_reduce_scalar<DT, OP><<<(unsigned)blocks, 256, 0, st>>>(w->base, w->stride, dest_off, source_off, first, nreduce, w->npes);
+    }
+}
+template <int DT>
+static int launch_reduce_op(shmemg_world *w, int op, uint64_t d, uint64_t s, size_t nvec, size_t first, size_t n, cudaStream_t st) {
+    switch (op) {
+    case SHMEMG_RED_SUM: launch_reduce<DT, SHMEMG_RED_SUM>(w, d, s, nvec, first, n, st); break;
+    case SHMEMG_RED_PROD: launch_reduce<DT, SHMEMG_RED_PROD>(w, d, s, nvec, first, n, st); break;
+    case SHMEMG_RED_MIN: launch_reduce<DT, SHMEMG_RED_MIN>(w, d, s, nvec, first, n, st); break;
+    case SHMEMG_RED_MAX: launch_reduce<DT, SHMEMG_RED_MAX>(w, d, s, nvec, first, n, st); break;
+    default:
+        if (DT == SHMEMG_F32 || DT == SHMEMG_F64) return SHMEMG_ERR_ARG;       // no bitwise reductions on floating point
+        if (op == SHMEMG_RED_AND) launch_reduce<DT == SHMEMG_F32 || DT == SHMEMG_F64 ? SHMEMG_I64 : DT, SHMEMG_RED_AND>(w, d, s, nvec, first, n, st);
+        else if (op == SHMEMG_RED_OR) launch_reduce<DT == SHMEMG_F32 || DT == SHMEMG_F64 ? SHMEMG_I64 : DT, SHMEMG_RED_OR>(w, d, s, nvec, first, n, st);
+        else launch_reduce<DT == SHMEMG_F32 || DT == SHMEMG_F64 ? SHMEMG_I64 : DT, SHMEMG_RED_XOR>(w, d, s, nvec, first, n, st);
+    }
+    return SHMEMG_OK;
+}
+
+extern "C" int shmemg_reduce_on_stream(shmemg_world_t *w, int op, int dtype, uint64_t dest_off, uint64_t source_off,
+                                       size_t nreduce, void *stream) {
+    if (!w || dtype < SHMEMG_F32 || dtype > SHMEMG_F64 || op < SHMEMG_RED_SUM || op > SHMEMG_RED_XOR) return SHMEMG_ERR_ARG;
+    if ((dtype == SHMEMG_F32 || dtype == SHMEMG_F64) && op >= SHMEMG_RED_AND) return SHMEMG_ERR_ARG;
+    const size_t esz = (dtype == SHMEMG_F32 || dtype == SHMEMG_I32) ? 4 : 8;
     const uint64_t tot = (uint64_t)nreduce * esz;
     if (!shmemg_in_range(w, dest_off, tot) || !shmemg_in_range(w, source_off, tot)) return SHMEMG_ERR_RANGE;
     if ((dest_off | source_off) & (esz - 1)) return SHMEMG_ERR_ALIGN;
@@ -423,29 +524,23 @@ extern "C" int shmemg_sum_reduce_on_stream(shmemg_world_t *w, int dtype, uint64_
     cudaStream_t st = (cudaStream_t)stream;
     const bool vec_ok = ((dest_off | source_off | w->stride) & 15) == 0;
     const size_t nvec = vec_ok ? tot >> 4 : 0;
-    const size_t per_vec = 16 / esz;
-    if (nvec) {
-        int rc = collectives_smem_attr(w);
-        if (rc) return rc;
-        const size_t nb = nvec << 4, ntiles = (nb + RT - 1) / RT;
-        const unsigned grid = (unsigned)(ntiles < (size_t)w->sm_count ? ntiles : (size_t)w->sm_count);
-        if (dtype == SHMEMG_F32)
-            k_sum_reduce_tma<SHMEMG_F32><<<grid, RED_CTA, RED_SMEM, st>>>(w->base, w->stride, dest_off, source_off, nb, w->npes);
-        else
-            k_sum_reduce_tma<SHMEMG_I64><<<grid, RED_CTA, RED_SMEM, st>>>(w->base, w->stride, dest_off, source_off, nb, w->npes);
-        SHMEMG_CUDA(w, cudaGetLastError());
+    const size_t first = nvec * (16 / esz);
+    int rc;
+    switch (dtype) {
+    case SHMEMG_F32: rc = launch_reduce_op<SHMEMG_F32>(w, op, dest_off, source_off, nvec, first, nreduce, st); break;
+    case SHMEMG_I64: rc = launch_reduce_op<SHMEMG_I64>(w, op, dest_off, source_off, nvec, first, nreduce, st); break;
+    case SHMEMG_I32: rc = launch_reduce_op<SHMEMG_I32>(w, op, dest_off, source_off, nvec, first, nreduce, st); break;
+    default: rc = launch_reduce_op<SHMEMG_F64>(w, op, dest_off, source_off, nvec, first, nreduce, st); break;
     }
-    const size_t first = nvec * per_vec;
-    if (first < nreduce) {
-        size_t blocks = (nreduce - first + 255) / 256;
-        if (blocks > 4096) blocks = 4096;
-        if (dtype == SHMEMG_F32)
-            k_sum_reduce_scalar<float, double><<<(unsigned)blocks, 256, 0, st>>>(w->base, w->stride, dest_off, source_off, first, nreduce, w->npes);
-        else
-            k_sum_reduce_scalar<unsigned long long, unsigned long long><<<(unsigned)blocks, 256, 0, st>>>(w->base, w->stride, dest_off, source_off, first, nreduce, w->npes);
-        SHMEMG_CUDA(w, cudaGetLastError());
-    }
+    if (rc) return rc;
+    SHMEMG_CUDA(w, cudaGetLastError());
     return SHMEMG_OK;
+}
+
+extern "C" int shmemg_sum_reduce_on_stream(shmemg_world_t *w, int dtype, uint64_t dest_off, uint64_t source_off,
+                                           size_t nreduce, void *stream) {
+    if (dtype != SHMEMG_F32 && dtype != SHMEMG_I64) return SHMEMG_ERR_ARG;
+    return shmemg_reduce_on_stream(w, SHMEMG_RED_SUM, dtype, dest_off, source_off, nreduce, stream);
 }
 
 extern "C" int shmemg_barrier_all_on_stream(shmemg_world_t *w, void *stream) {
