@@ -335,3 +335,23 @@ def test_signal_test_truth_table_and_acquire():
         w.signal_test(sig + 4, CMP.EQ, 0, 1, res)
     with pytest.raises(ShmemgError):
         w.signal_test(sig, 9, 0, 1, res)
+
+
+def test_reduce_signed_zero_corner_matches_oracle():
+    npes = 3
+    w, ow = pair(npes, 4096)
+    s, d = w.malloc(256), w.malloc(256)
+    os_, od = ow.malloc(256), ow.malloc(256)
+    x = np.full((npes, 8), -0.0, dtype=np.float32)
+    x[1, 4:] = 0.0
+    w.view(s, 32, torch.float32).copy_(torch.from_numpy(x))
+    ow.view(os_, 32, np.float32)[:] = x
+    for op in (RED.SUM, RED.PROD, RED.MIN, RED.MAX):
+        w.reduce(op, F32, d, s, 8)
+        w.quiet(0)
+        ow.reduce(ORC_OP[op], "f32", od, os_, 8)
+        g, o = w.view(d, 32).cpu().numpy().view(np.uint32), ow.view(od, 32, np.uint32)
+        if op in (RED.MIN, RED.MAX):                     # min(-0, +0): either zero is a correct result
+            assert np.array_equal(g[:, :4], o[:, :4]) and (g[:, 4:] & 0x7fffffff == 0).all()
+        else:
+            assert np.array_equal(g, o), op

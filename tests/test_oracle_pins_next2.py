@@ -256,3 +256,17 @@ def test_signal_test_truth_table():
         assert tuple(int(w.signal_test(8, cmp, v, 1)) for v in (4, 5, 6)) == exp
     assert w.signal_test(8, CMP_GT, M64, 1) is False                 # unsigned comparison
     assert w.signal_test(8, CMP_EQ, 0, 0) is True                    # PE 0's word is still 0
+
+
+def test_sum_of_negative_zeros_is_positive_zero_in_both_sum_routines():
+    """SUM = 0 + x_0 + x_1 + ... (IEEE: +0.0 + -0.0 = +0.0); MIN / MAX / PROD keep the sign of zero."""
+    w = orc.OracleWorld(3, 256)
+    w.view(0, 8, np.float32)[:] = np.float32(-0.0)
+    w.reduce("sum", "f32", 64, 0, 2)
+    assert w.view(64, 8, np.uint32).tolist() == [[0, 0]] * 3
+    w.sum_reduce_f32(128, 0, 2)
+    assert w.view(128, 8, np.uint32).tolist() == [[0, 0]] * 3
+    w.reduce("max", "f32", 64, 0, 2)
+    assert w.view(64, 8, np.uint32).tolist() == [[0x80000000] * 2] * 3
+    w.reduce("prod", "f32", 64, 0, 2)                    # (-0)(-0)(-0) = -0
+    assert w.view(64, 8, np.uint32).tolist() == [[0x80000000] * 2] * 3
