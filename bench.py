@@ -67,7 +67,7 @@ def parse_args():
     ap.add_argument("--no-e2e", action="store_true", help="skip the end-to-end (host buffers) leg")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
     ap.add_argument("--small", action="store_true", help="reduced sizes (development only; marked in the JSON)")
-    ap.add_argument("--only", default="", help="comma-separated segment groups to run: c1,c2,c3a,c3b,c4,c5,barrier")
+    ap.add_argument("--only", default="", help="comma-separated segment groups to run: c1,c2,c3a,c3b,c4,c5,barrier,next2")
     return ap.parse_args()
 
 
@@ -180,6 +180,18 @@ def segment_table(inp: Inputs):
         E = len(inp.c4.u)
         seg["atomic_fetch_add"] = dict(cls="amo", kernel="k_amo<fetch_add>", ops=E, launches=1)
         seg["atomic_compare_swap"] = dict(cls="amo", kernel="k_amo<compare_swap>", ops=E, launches=1)
+    if "next2" in g:
+        # NEXT-2 surface; reported per segment, NOT part of `value` / `amo_mops` (cls x*)
+        if "c5" in g:
+            n, nb = inp.c5_npes, inp.c5_bytes
+            seg["next2_broadcast"] = dict(cls="xcopy", kernel="k_broadcast_tma", bytes=(n + 1) * nb, launches=1)
+            seg["next2_reduce_max_i64"] = dict(cls="xcopy", kernel="k_sum_reduce_tma<i64,max>", bytes=2 * n * nb, launches=1)
+            seg["next2_reduce_min_f32"] = dict(cls="xcopy", kernel="k_sum_reduce_tma<f32,min>", bytes=2 * n * nb, launches=1)
+        if "c4" in g:
+            seg["next2_amo_xor"] = dict(cls="xamo", kernel="k_amo2<xor>", ops=len(inp.c4.u), launches=1)
+            seg["next2_amo_fetch_xor"] = dict(cls="xamo", kernel="k_amo2<fetch_xor>", ops=len(inp.c4.u), launches=1)
+        if "c2" in g:
+            seg["next2_ibput_faces"] = dict(cls="xcopy", kernel="k_ib_tma/k_ib_elem", bytes=3 * 2 * inp.halo.face_bytes, launches=3)
     if "barrier" in g:
         seg["barrier_in_kernel"] = dict(cls="sync", kernel="k_barrier_repeat", ops=BARRIERS, launches=1)
         seg["barrier_on_stream"] = dict(cls="sync", kernel="k_barrier_epoch", ops=BARRIERS, launches=BARRIERS)
@@ -341,6 +353,28 @@ class CudaBench:
                 self.app_launches += 2
                 with rec.seg("halo_put_signal_wait"):
                     w.enqueue_batch(self.halo_batches[r - 1])
+        if "next2" in g:
+            from paper_2607_08006_b200.binding import AMO, F32, I64, RED
+            if "c5" in g:
+                n = inp.c5_bytes
+                with rec.seg("next2_broadcast"):
+                    self.w5.broadcast(self.d5, self.s_i64, n, 3)
+                with rec.seg("next2_reduce_max_i64"):
+                    self.w5.reduce(RED.MAX, I64, self.d5, self.s_i64, n // 8)
+                with rec.seg("next2_reduce_min_f32"):
+                    self.w5.reduce(RED.MIN, F32, self.d5, self.s_f32, n // 4)
+            if "c4" in g:
+                with rec.seg("next2_amo_xor"):
+                    self.w4.atomic_op_batch(AMO.XOR, 8, self.deg, self.c4_ou, self.c4_lu, val=self.c4_val)
+                with rec.seg("next2_amo_fetch_xor"):
+                    self.w4.atomic_op_batch(AMO.XOR, 8, self.deg, self.c4_ou, self.c4_lu, val=self.c4_val, fetched_out=self.f_deg)
+            if "c2" in g:
+                h, B = inp.halo, inp.halo.B
+                send_off, fb = self.ld2.off["send"][0], inp.halo.face_bytes
+                with rec.seg("next2_ibput_faces"):             # the three face orientations straight out of the cube
+                    self.w2.ibput(send_off, self.U_off, 0, 0, fb, 1, 0, 1)
+                    self.w2.ibput(send_off + 2 * fb, self.U_off, B * 8, B * B * 8, B * 8, B, 0, 1)
+                    self.w2.ibput(send_off + 4 * fb, self.U_off, 8, B * 8, 8, B * B, 0, 1)
         if "barrier" in g:
             with rec.seg("barrier_in_kernel"):
                 self.w5.barrier_all_repeat(BARRIERS)
@@ -598,7 +632,27 @@ def class_rates(table, seg_seconds, seg_units):
     return (cb / cs / 1e9 if cs > 0 else 0.0), (ao / as_ / 1e6 if as_ > 0 else 0.0), cs, as_
 
 
-ALL_GROUPS = ["c1", "c2", "c3a", "c3b", "c4", "c5", "barrier"]
+ALL_GROUPS = ["c1", "c2", "c3a", "c3b", "c4", "c5", "barrier", "next2"]
+
+
+def max_over_ranks(dist, device, seg_ms, whole_ms, e2e_ms):
+    """Replicas only: every rank runs the same step on its own GPU; a segment's time is the MAX over ranks
+    (one all_reduce of a small vector, the only collective of the bench and not on the data path).  Returns
+    (names, seg_ms, whole_ms, e2e_ms) with the reduced values; `dist` None = single process."""
+    import torch
+    names = sorted(seg_ms)
+    vec = torch.tensor([seg_ms[k] for k in names] + [whole_ms] + ([e2e_ms.get(k, 0.0) for k in names] if e2e_ms else []),
+                       dtype=torch.float64, device=device)
+    if dist is not None:
+        dist.all_reduce(vec, op=dist.ReduceOp.MAX)
+    vec = vec.cpu().tolist()
+    out_e2e = dict(zip(names, vec[len(names) + 1:])) if e2e_ms else e2e_ms
+    return names, dict(zip(names, vec[:len(names)])), vec[len(names)], out_e2e
+
+
+def whole_job_units(table, names, steps, world):
+    """Units (bytes or ops) all ranks processed in the timed region: weak scaling, every replica does the full step."""
+    return {k: table[k].get("bytes", table[k].get("ops")) * steps * world for k in names}
 
 
 def base_line(args, n_gpus):
@@ -704,23 +758,14 @@ def run_cuda(args):
     ceil = cb.ceilings() if rank == 0 else {}
 
     # ---- max over ranks of every segment time ---------------------------------------------------------------------------
-    names = sorted(seg_ms)
-    vec = torch.tensor([seg_ms[k] for k in names] + [whole_ms] + ([e2e_ms.get(k, 0.0) for k in names] if e2e_ms else []),
-                       dtype=torch.float64, device=device)
-    if dist is not None:
-        dist.all_reduce(vec, op=dist.ReduceOp.MAX)
-    vec = vec.cpu().tolist()
-    seg_ms = dict(zip(names, vec[:len(names)]))
-    whole_ms = vec[len(names)]
-    if e2e_ms:
-        e2e_ms = dict(zip(names, vec[len(names) + 1:]))
+    names, seg_ms, whole_ms, e2e_ms = max_over_ranks(dist, device, seg_ms, whole_ms, e2e_ms)
     if rank != 0:
         if dist is not None:
             dist.destroy_process_group()
         return
 
     K = args.steps
-    units = {k: table[k].get("bytes", table[k].get("ops")) * K * world for k in names}
+    units = whole_job_units(table, names, K, world)
     secs = {k: seg_ms[k] * 1e-3 for k in names}
     gbps, mops, copy_s, amo_s = class_rates(table, secs, units)
     peak, peak_src = measured_peaks()
@@ -734,6 +779,13 @@ def run_cuda(args):
             d["frac_of_nominal_8TBps"] = d["GBps"] / 8000.0
         elif t["cls"] == "amo":
             d["Mops"] = units[k] / world / secs[k] / 1e6
+        elif t["cls"] == "xcopy":
+            d["GBps"] = units[k] / world / secs[k] / 1e9
+            d["frac_of_measured_hbm"] = d["GBps"] / peak
+            d["in_headline"] = False
+        elif t["cls"] == "xamo":
+            d["Mops"] = units[k] / world / secs[k] / 1e6
+            d["in_headline"] = False
         else:
             d["us_per_barrier"] = seg_ms[k] / K / t["ops"] * 1e3
         d["us_per_launch"] = per_launch_ms * 1e3
