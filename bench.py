@@ -178,7 +178,7 @@ def segment_table(inp: Inputs):
         seg["atomic_add"] = dict(cls="amo", kernel="k_amo<add>", ops=len(inp.c1.val), launches=2)   # + barrier kernel
     if "c4" in g:
         E = len(inp.c4.u)
-        seg["atomic_fetch_add"] = dict(cls="amo", kernel="k_amo<fetch_add>", ops=E, launches=1)
+        seg["atomic_fetch_add"] = dict(cls="amo", kernel="k_hot_sample + k_amo_hot_main<fetch_add>", ops=E, launches=2)
         seg["atomic_compare_swap"] = dict(cls="amo", kernel="k_amo<compare_swap>", ops=E, launches=1)
     if "next2" in g:
         # NEXT-2 surface; reported per segment, NOT part of `value` / `amo_mops` (cls x*)
@@ -237,7 +237,7 @@ class CudaBench:
     def __init__(self, inp: Inputs, device):
         import torch
         from paper_2607_08006_b200 import World
-        from paper_2607_08006_b200.binding import AMO_TEST_BEFORE_SWAP, AMO_WARP_AGGREGATE
+        from paper_2607_08006_b200.binding import AMO_HOT_AGGREGATE, AMO_TEST_BEFORE_SWAP
         from paper_2607_08006_b200.loader import Loaded
         self.torch, self.inp, self.dev = torch, inp, device
         self.rec = Recorder(torch)
@@ -245,6 +245,7 @@ class CudaBench:
         self.barrier_graph = None
         self.worlds = []
         self.flags = 0                                 # warp aggregation buys nothing on these streams (profiles/)
+        self.fadd_flags = AMO_HOT_AGGREGATE            # RMAT stream: the hot words are combined per CTA chunk (profiles/r01d)
         self.cas_flags = AMO_TEST_BEFORE_SWAP          # scalar cond: failed swaps are resolved by a coherent load
         g = inp.groups
         dv = lambda a: torch.from_numpy(np.ascontiguousarray(a)).to(device)      # noqa: E731
@@ -318,7 +319,7 @@ class CudaBench:
             self.w4.view(self.par, vpp * 8).fill_(255)
             with rec.seg("atomic_fetch_add"):
                 self.w4.atomic_fetch_add_batch(self.deg, self.c4_ou, self.c4_lu, self.f_deg, val=None, val_scalar=1,
-                                               flags=self.flags)
+                                               flags=self.fadd_flags)
             with rec.seg("atomic_compare_swap"):
                 self.w4.atomic_compare_swap_batch(self.par, self.c4_ov, self.c4_lv, self.f_par, cond=None, cond_scalar=M64,
                                                   val=self.c4_val, flags=self.cas_flags)
@@ -482,7 +483,7 @@ class CudaBench:
                     d.copy_(h, non_blocking=True)
                     self.h2d += h.numel() * h.element_size()
                 self.w4.atomic_fetch_add_batch(self.deg, self.c4_ou, self.c4_lu, self.f_deg, val=None, val_scalar=1,
-                                               flags=self.flags)
+                                               flags=self.fadd_flags)
                 self.h_fdeg.copy_(self.f_deg, non_blocking=True)
                 self.d2h += self.h_fdeg.numel() * 8
                 self._down(self.w4, self.h_deg, self.deg)

@@ -222,6 +222,15 @@ SHMEMG_API int shmemg_quiet(shmemg_world_t *w, int pe, void *stream);
  * word differs from cond no op of the call can change it, so the loaded value is the failed swap's fetched value.
  * Requires that nothing outside this call updates the target words while it runs (already undefined). */
 #define SHMEMG_AMO_TEST_BEFORE_SWAP 2u
+/* add / fetch-add with a scalar value (val == NULL), meant for skewed streams (same-line serialisation at the L2 atomic
+ * unit is the limiter there): a sampling kernel finds the hot words of the stream (up to 512); in the main kernel every CTA
+ * combines its ops on a hot word in shared memory and issues ONE L2 atomic per hot word (op k of the CTA's group fetches
+ * old + k*val_scalar: the group executes back to back, legal for the same reason as warp aggregation).  The sample only
+ * affects speed, never the result.  Uses scratch in the world's control region and a library-owned device buffer (n bytes,
+ * allocated with cudaMalloc on first use -- that call synchronises -- and freed by shmemg_finalize): two calls with this
+ * flag must be stream-ordered.  Ignored (the plain kernel runs) when val != NULL, n < 2^20 or n >= 2^33, or the slab has
+ * 2^32 or more 64-bit words. */
+#define SHMEMG_AMO_HOT_AGGREGATE 4u
 SHMEMG_API int shmemg_atomic_add_batch_on_stream(shmemg_world_t *w, uint64_t sym_off, const int32_t *tgt_pe,
                                                  const void *elem_idx, int idx_bytes, const uint64_t *val,
                                                  uint64_t val_scalar, size_t n, uint32_t flags, void *stream);

@@ -75,6 +75,7 @@ class AMO:
 
 AMO_WARP_AGGREGATE = 1
 AMO_TEST_BEFORE_SWAP = 2
+AMO_HOT_AGGREGATE = 4
 NO_STAMP = (1 << 64) - 1
 
 # shmemg_op_t, 64 bytes
@@ -339,7 +340,7 @@ class World:
                                                           self._idx_bytes(elem_idx), _dptr(val), val_scalar & NO_STAMP,
                                                           n, flags, _stream(stream)),
                   "shmemg_atomic_add_batch_on_stream")
-        self.launches += 1 if n else 0
+        self.launches += (2 if (flags & AMO_HOT_AGGREGATE) and val is None and n >= (1 << 20) else 1) if n else 0
 
     def atomic_fetch_add_batch(self, sym_off, tgt_pe, elem_idx, fetched_out, val=None, val_scalar=0, flags=0,
                                stream=None):
@@ -349,7 +350,8 @@ class World:
                                                                 val_scalar & NO_STAMP, _dptr(fetched_out), n, flags,
                                                                 _stream(stream)),
                   "shmemg_atomic_fetch_add_batch_on_stream")
-        self.launches += 1 if n else 0
+        # launch accounting: SHMEMG_AMO_HOT_AGGREGATE runs a sampling kernel in front of the main one (n >= 2^20, scalar value)
+        self.launches += (2 if (flags & AMO_HOT_AGGREGATE) and val is None and n >= (1 << 20) else 1) if n else 0
 
     def atomic_compare_swap_batch(self, sym_off, tgt_pe, elem_idx, fetched_out, cond=None, cond_scalar=0, val=None,
                                   val_scalar=0, flags=0, stream=None):

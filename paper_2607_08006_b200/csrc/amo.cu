@@ -137,6 +137,249 @@ __global__ void __launch_bounds__(256) k_amo(const AmoArgs a) {
     }
 }
 
+
+// ---- hot-set aggregation (SHMEMG_AMO_HOT_AGGREGATE; add / fetch-add with ONE scalar value) -----------------------------
+// A skewed op stream (C4: RMAT) is bound by same-line serialisation at the L2 atomic unit: the hottest 128-byte line takes
+// 0.71 % of the 2^26 ops and its ops alone last as long as the whole kernel (2.7 ns each), while the atomic units idle
+// (profiles/r01d).  Removing the 256 hottest words from the stream brings the plain kernel from 1339 to 721 us.  So:
+//   k_hot_sample     HOT_SAMPLES ops of the stream are fetched by 16 CTAs; the last one to finish counts them in a shared-memory
+//                    hash table and publishes the words seen at least HOT_THRESHOLD times (at most SHMEMG_HOT_MAX) in the
+//                    control region (about 40 us);
+//   k_amo_hot_main   k_amo's loop with a two-load shared-memory lookup per op.  Cold ops go straight to L2.  The hot ops of a
+//                    CTA are combined: ONE L2 atomic per hot word and CTA (count * val); a hot fetch-add receives
+//                    old + rank * val, its rank taken from the word's shared-memory counter.
+// Measured on C4 (2^26 fetch-adds, RMAT): 1340 -> 890 us.  What did NOT work on the way (profiles/r01d): a hash table over ALL
+// ops of a chunk (2000 us: barriers behind probe loops); contiguous chunks with per-thread hot bitmasks (1090-1530 us: 38-55
+// registers cut the number of L2 atomics in flight, which is what this kernel lives on); a separate fix-up kernel re-reading
+// the operands of the hot ops (430 us of 32-byte-sector traffic).
+// Linearisation: the hot ops of one CTA execute back to back, in rank order, at the instant of the CTA's L2 atomic on
+// that word -- legal because the ops of one call are unordered (PAPER L369 / reading 7), the same argument as for warp
+// aggregation.  Which words count as hot only changes the speed, never the result.
+#define HOT_SAMPLES 16384
+#define HOT_SLOTS_SAMPLE 24576u          // 8-byte {key, count} slots of the sampling table (192 KiB of shared memory)
+#define HOT_THRESHOLD 3u
+#define HOT_INDEX 4096u                  // per-CTA direct-mapped index of the hot words (8 KiB)
+#define HOT_NONE 0xffffu
+#define HOT_EMPTY 0xffffffffu
+
+__device__ __forceinline__ unsigned hot_hash(unsigned key, unsigned slots) {
+    return (unsigned)(((unsigned long long)(key * 0x9E3779B1u) * slots) >> 32);
+}
+
+// HOT_SAMPLES / 1024 CTAs of 1024 threads: every thread fetches ONE sample (one SM alone cannot keep 2 x 16384 scattered
+// sector loads in flight: 96 us) and stages its key; the CTA that finishes last builds the table from the staged keys.
+template <int IDXB>
+__global__ void __launch_bounds__(1024) k_hot_sample(const AmoArgs a, CtlRegion *ctl, unsigned *staged) {
+    typedef typename IdxT<IDXB>::type idx_t;
+    extern __shared__ __align__(16) unsigned long long stab[];       // {key (low), count (high)}
+    unsigned *tab = reinterpret_cast<unsigned *>(stab);
+    __shared__ unsigned n_hot, last;
+    const idx_t *__restrict__ idx = reinterpret_cast<const idx_t *>(a.idx);
+    const unsigned long long words_per_pe = a.stride >> 3, word0 = a.sym_off >> 3;
+    {
+        const size_t q = (size_t)blockIdx.x * 1024 + threadIdx.x, i = q * (a.n / HOT_SAMPLES);   // n >= 2^20: step >= 64
+        staged[q] = (unsigned)((unsigned long long)a.tgt_pe[i] * words_per_pe + word0 + (unsigned long long)idx[i]);
+    }
+    __threadfence();
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        last = atomicAdd(&ctl->hot_done, 1u) == gridDim.x - 1;
+        if (last) { ctl->hot_done = 0; n_hot = 0; }
+    }
+    __syncthreads();
+    if (!last) return;
+    __threadfence();
+    for (unsigned s = threadIdx.x; s < HOT_SLOTS_SAMPLE; s += 1024) stab[s] = (unsigned long long)HOT_EMPTY;
+    __syncthreads();
+    for (unsigned q = threadIdx.x; q < HOT_SAMPLES; q += 1024) {
+        const unsigned key = *reinterpret_cast<volatile unsigned *>(staged + q);
+        unsigned h = hot_hash(key, HOT_SLOTS_SAMPLE);
+        for (;;) {
+            const unsigned old = atomicCAS(&tab[2 * h], HOT_EMPTY, key);
+            if (old == HOT_EMPTY || old == key) break;
+            if (++h == HOT_SLOTS_SAMPLE) h = 0;
+        }
+        atomicAdd(&tab[2 * h + 1], 1u);
+    }
+    __syncthreads();
+    for (unsigned s = threadIdx.x; s < HOT_SLOTS_SAMPLE; s += 1024) {
+        if (tab[2 * s] != HOT_EMPTY && tab[2 * s + 1] >= HOT_THRESHOLD) {
+            const unsigned k = atomicAdd(&n_hot, 1u);
+            if (k < SHMEMG_HOT_MAX) ctl->hot_keys[k] = tab[2 * s];
+        }
+    }
+    __syncthreads();
+    if (threadIdx.x == 0) ctl->hot_n = n_hot < SHMEMG_HOT_MAX ? n_hot : SHMEMG_HOT_MAX;
+}
+
+// shared-memory lookup of the hot words: direct-mapped index hidx[hash(key)] -> j with hkeys[j] == key.  A hot word whose
+// index slot is taken by another one is simply not treated as hot (a few per cent): two loads, no loop.
+struct HotTable {
+    unsigned short hidx[HOT_INDEX];
+    unsigned hkeys[SHMEMG_HOT_MAX];
+    __device__ __forceinline__ void build(const CtlRegion *ctl, unsigned tid, unsigned nthr) {
+        for (unsigned s = tid; s < HOT_INDEX; s += nthr) hidx[s] = HOT_NONE;
+        for (unsigned s = tid; s < SHMEMG_HOT_MAX; s += nthr) hkeys[s] = HOT_EMPTY;
+        __syncthreads();
+        const unsigned nh = ctl->hot_n;
+        for (unsigned k = tid; k < nh; k += nthr) {
+            const unsigned key = ctl->hot_keys[k];
+            hkeys[k] = key;
+            hidx[hot_hash(key, HOT_INDEX)] = (unsigned short)k;       // racing writers: one wins, the losers stay cold
+        }
+        __syncthreads();
+    }
+    __device__ __forceinline__ int lookup(unsigned key) const {       // index of a hot word, or -1
+        const unsigned j = hidx[hot_hash(key, HOT_INDEX)] & (SHMEMG_HOT_MAX - 1);
+        return hkeys[j] == key ? (int)j : -1;
+    }
+};
+
+// k_amo's grid-stride loop (whole waves of resident CTAs).  Cold ops go to L2.  Hot ops:
+//   add        counted in shared memory; one red per hot word and CTA at the end;
+//   fetch-add  appended to the CTA's own list in `lists` (op index + hot-word index, coalesced 8-byte records; when the list
+//              is full the op simply goes to L2 like a cold one).  After the loop the CTA walks its list three times:
+//              rank = shared-memory counter of the word; base = ONE L2 atom.add(word, count * val) per hot word;
+//              fetched = base + rank * val.
+#define HOT_I_BITS 34                    // record = op index (34 bits) | hot-word index (9 bits) << 34 | rank (21 bits) << 43
+template <int IDXB, int OP>
+__global__ void __launch_bounds__(256, 6) k_amo_hot_main(const AmoArgs a, const CtlRegion *ctl, unsigned long long *lists, unsigned cap) {
+    typedef typename IdxT<IDXB>::type idx_t;
+    __shared__ HotTable ht;
+    __shared__ unsigned long long slot[SHMEMG_HOT_MAX];               // count; after the base atomics: the word's old value
+    __shared__ unsigned list_n;
+    const idx_t *__restrict__ idx = reinterpret_cast<const idx_t *>(a.idx);
+    const int *__restrict__ tgt = a.tgt_pe;
+    const unsigned long long words_per_pe = a.stride >> 3, word0 = a.sym_off >> 3;
+    unsigned long long *const slab = reinterpret_cast<unsigned long long *>(a.base);
+    unsigned long long *const list = lists + (size_t)blockIdx.x * cap;
+    for (unsigned s = threadIdx.x; s < SHMEMG_HOT_MAX; s += blockDim.x) slot[s] = 0;
+    if (threadIdx.x == 0) list_n = 0;
+    ht.build(ctl, threadIdx.x, blockDim.x);
+    const size_t T = (size_t)gridDim.x * blockDim.x;
+    const int lane = threadIdx.x & 31;
+    const size_t warp_first = ((size_t)blockIdx.x * blockDim.x + threadIdx.x) - lane;
+    for (size_t i0 = warp_first; i0 < a.n; i0 += T * AMO_ITEMS) {
+        unsigned key[AMO_ITEMS];
+        int hot[AMO_ITEMS];
+#pragma unroll
+        for (int k = 0; k < AMO_ITEMS; ++k) {
+            const size_t i = i0 + lane + (size_t)k * T;
+            key[k] = HOT_EMPTY;
+            if (i < a.n) key[k] = (unsigned)((unsigned long long)tgt[i] * words_per_pe + word0 + (unsigned long long)idx[i]);
+        }
+#pragma unroll
+        for (int k = 0; k < AMO_ITEMS; ++k) hot[k] = key[k] == HOT_EMPTY ? -2 : ht.lookup(key[k]);     // -2: no op, -1: cold
+        unsigned long long old[AMO_ITEMS];
+#pragma unroll
+        for (int k = 0; k < AMO_ITEMS; ++k) {                         // the L2 atomics first: everything below overlaps them
+            if (hot[k] == -1) {
+                if (OP == AMO_ADD) asm volatile("red.relaxed.gpu.global.add.u64 [%0], %1;" ::"l"(slab + key[k]), "l"(a.val_s) : "memory");
+                else old[k] = atomicAdd(slab + key[k], a.val_s);
+            } else if (OP == AMO_ADD && hot[k] >= 0) {
+                atomicAdd(reinterpret_cast<unsigned *>(&slot[hot[k]]), 1u);       // < 2^32 ops per CTA
+            }
+        }
+        if (OP == AMO_FADD) {
+#pragma unroll
+            for (int k = 0; k < AMO_ITEMS; ++k) {                     // warp-aggregated append to the CTA's list
+                const unsigned b = __ballot_sync(FULL, hot[k] >= 0);
+                if (b == 0) continue;
+                unsigned pos = 0;
+                if (lane == __ffs((int)b) - 1) pos = atomicAdd(&list_n, (unsigned)__popc(b));
+                pos = __shfl_sync(FULL, pos, __ffs((int)b) - 1) + (unsigned)__popc(b & ((1u << lane) - 1u));
+                if (hot[k] >= 0) {
+                    if (pos < cap) {
+                        list[pos] = (unsigned long long)(i0 + lane + (size_t)k * T) | ((unsigned long long)hot[k] << HOT_I_BITS);
+                    } else {                                          // list full: an ordinary L2 atomic after all
+                        old[k] = atomicAdd(slab + key[k], a.val_s);
+                        hot[k] = -1;
+                    }
+                }
+            }
+        }
+        if (OP == AMO_FADD) {
+#pragma unroll
+            for (int k = 0; k < AMO_ITEMS; ++k)
+                if (hot[k] == -1) a.fetched[i0 + lane + (size_t)k * T] = old[k];
+        }
+    }
+    __syncthreads();
+    if (OP == AMO_ADD) {
+        for (unsigned j = threadIdx.x; j < SHMEMG_HOT_MAX; j += blockDim.x) {
+            const unsigned long long c = slot[j];
+            if (c) asm volatile("red.relaxed.gpu.global.add.u64 [%0], %1;" ::"l"(slab + ht.hkeys[j]), "l"(c * a.val_s) : "memory");
+        }
+        return;
+    }
+    const unsigned nl = list_n < cap ? list_n : cap;
+    const unsigned long long imask = (1ull << HOT_I_BITS) - 1;
+    for (unsigned e = threadIdx.x; e < nl; e += blockDim.x) {         // own records: written by this CTA before the barrier
+        const unsigned long long r = list[e];
+        const unsigned j = (unsigned)(r >> HOT_I_BITS);
+        list[e] = r | ((unsigned long long)atomicAdd(reinterpret_cast<unsigned *>(&slot[j]), 1u) << 43);
+    }
+    __syncthreads();
+    for (unsigned j = threadIdx.x; j < SHMEMG_HOT_MAX; j += blockDim.x) {
+        const unsigned long long c = slot[j];
+        if (c) slot[j] = atomicAdd(slab + ht.hkeys[j], c * a.val_s);
+    }
+    __syncthreads();
+    for (unsigned e = threadIdx.x; e < nl; e += blockDim.x) {         // same thread wrote list[e] in the rank pass
+        const unsigned long long r = list[e];
+        a.fetched[r & imask] = slot[(r >> HOT_I_BITS) & (SHMEMG_HOT_MAX - 1)] + (r >> 43) * a.val_s;
+    }
+}
+
+// usable when the value is one scalar and every word of the slab has a 32-bit index; small calls keep the plain kernel
+static bool hot_agg_ok(const shmemg_world *w, const AmoArgs &a, uint32_t flags) {
+    return (flags & SHMEMG_AMO_HOT_AGGREGATE) && a.val == nullptr && (a.stride & 7) == 0 &&
+           ((uint64_t)w->npes * a.stride >> 3) < 0xffffffffull && a.n >= ((size_t)1 << 20) && a.n < ((size_t)1 << 33);
+}
+
+template <int OP>
+static int launch_amo_hot(shmemg_world *w, const AmoArgs &a, int idx_bytes, cudaStream_t st) {
+    static bool attr_set = false;
+    if (!attr_set) {
+        SHMEMG_CUDA(w, cudaFuncSetAttribute(k_hot_sample<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(HOT_SLOTS_SAMPLE * 8)));
+        SHMEMG_CUDA(w, cudaFuncSetAttribute(k_hot_sample<8>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(HOT_SLOTS_SAMPLE * 8)));
+        attr_set = true;
+    }
+    // whole waves of resident CTAs; every CTA may list up to 1/8 of its ops as hot (what does not fit goes to L2 directly)
+    int per_sm = 0;
+    if (idx_bytes == 4) cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_amo_hot_main<4, OP>, 256, 0);
+    else cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_amo_hot_main<8, OP>, 256, 0);
+    if (per_sm < 1) per_sm = 1;
+    size_t waves = 8;                                         // measured on C4: 1 wave 970 us, 8 waves 890 us, 32 waves 980 us
+    if (const char *e = getenv("SHMEMG_HOT_WAVES")) waves = (size_t)atoi(e) > 0 ? (size_t)atoi(e) : waves;   // experiments
+    const size_t blocks = (size_t)w->sm_count * per_sm * waves;
+    const size_t per_cta = (a.n + blocks - 1) / blocks;
+    if (per_cta >= ((size_t)1 << 21) * 8 || a.n >= ((size_t)1 << HOT_I_BITS)) return SHMEMG_ERR_NOMEM;   // caller falls back
+    const unsigned cap = (unsigned)(per_cta / 8 + 32);
+    unsigned long long *lists = nullptr;
+    {                                                         // library-owned scratch, grown on demand (first call synchronises)
+        const size_t need = (size_t)HOT_SAMPLES * 4 + (OP == AMO_FADD ? blocks * (size_t)cap * 8 : 0);
+        if (w->hot_scratch_bytes < need) {
+            if (w->hot_scratch) SHMEMG_CUDA(w, cudaFree(w->hot_scratch));
+            w->hot_scratch = nullptr; w->hot_scratch_bytes = 0;
+            SHMEMG_CUDA(w, cudaMalloc(&w->hot_scratch, need));
+            w->hot_scratch_bytes = need;
+        }
+        if (OP == AMO_FADD) lists = (unsigned long long *)((uint8_t *)w->hot_scratch + (size_t)HOT_SAMPLES * 4);
+    }
+    unsigned *staged = (unsigned *)w->hot_scratch;
+    if (idx_bytes == 4) {
+        k_hot_sample<4><<<HOT_SAMPLES / 1024, 1024, HOT_SLOTS_SAMPLE * 8, st>>>(a, w->ctl, staged);
+        k_amo_hot_main<4, OP><<<(unsigned)blocks, 256, 0, st>>>(a, w->ctl, lists, cap);
+    } else {
+        k_hot_sample<8><<<HOT_SAMPLES / 1024, 1024, HOT_SLOTS_SAMPLE * 8, st>>>(a, w->ctl, staged);
+        k_amo_hot_main<8, OP><<<(unsigned)blocks, 256, 0, st>>>(a, w->ctl, lists, cap);
+    }
+    const cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return shmemg_cuda_fail(w, e, "k_amo_hot");
+    return SHMEMG_OK;
+}
+
 template <int OP>
 static int launch_amo(shmemg_world *w, const AmoArgs &a, int idx_bytes, uint32_t flags, cudaStream_t st) {
     if (a.n == 0) return SHMEMG_OK;
@@ -178,6 +421,7 @@ extern "C" int shmemg_atomic_add_batch_on_stream(shmemg_world_t *w, uint64_t sym
     int rc = check_common(w, sym_off, tgt_pe, elem_idx, idx_bytes, n);
     if (rc) return rc;
     AmoArgs a{w->base, w->stride, sym_off, tgt_pe, elem_idx, (const unsigned long long *)val, val_scalar, nullptr, 0, nullptr, n};
+    if (hot_agg_ok(w, a, flags)) return launch_amo_hot<AMO_ADD>(w, a, idx_bytes, (cudaStream_t)stream);
     return launch_amo<AMO_ADD>(w, a, idx_bytes, flags, (cudaStream_t)stream);
 }
 
@@ -190,6 +434,7 @@ extern "C" int shmemg_atomic_fetch_add_batch_on_stream(shmemg_world_t *w, uint64
     if (n && !fetched_out) return SHMEMG_ERR_ARG;
     AmoArgs a{w->base, w->stride, sym_off, tgt_pe, elem_idx, (const unsigned long long *)val, val_scalar, nullptr, 0,
               (unsigned long long *)fetched_out, n};
+    if (hot_agg_ok(w, a, flags)) return launch_amo_hot<AMO_FADD>(w, a, idx_bytes, (cudaStream_t)stream);
     return launch_amo<AMO_FADD>(w, a, idx_bytes, flags, (cudaStream_t)stream);
 }
 

@@ -17,6 +17,7 @@
 #define SHMEMG_TMA_TILE 32768u             // bytes per bulk-copy stage
 #define SHMEMG_TMA_STAGES 4                // stages per CTA (128 KiB of shared memory, one CTA per SM)
 #define SHMEMG_SIG_SLOTS 1024              // completion counters for single put_signal launches
+#define SHMEMG_HOT_MAX 512                 // hot words tracked by SHMEMG_AMO_HOT_AGGREGATE
 
 // ---- control region layout (device) -------------------------------------------------------------------
 struct CtlRegion {
@@ -25,6 +26,9 @@ struct CtlRegion {
     unsigned int bar_gen;                  // in-kernel barrier: generation (sense)
     unsigned int pad[12];
     unsigned int sig_counter[SHMEMG_SIG_SLOTS];   // last-arriver counters of single put_signal launches
+    unsigned int hot_n;                    // SHMEMG_AMO_HOT_AGGREGATE: number of hot words found by the sampling kernel
+    unsigned int hot_done;                 // CTAs of the sampling kernel that have staged their keys
+    unsigned int hot_keys[SHMEMG_HOT_MAX]; // their slab word indices
 };
 
 // ---- host-side world ------------------------------------------------------------------------------------
@@ -44,6 +48,8 @@ struct shmemg_world {
     size_t tile_bytes_override = 0;        // SHMEMG_TILE_BYTES (experiments; forces the register copy path)
     bool smem_attr_coll = false, smem_attr_probe = false;
     bool smem_attr_set = false;            // dynamic shared memory opt-in done for the bulk-copy kernels
+    void *hot_scratch = nullptr;           // DEVICE: library-owned scratch of SHMEMG_AMO_HOT_AGGREGATE (grown on demand)
+    size_t hot_scratch_bytes = 0;
     std::string last_cuda_error;
 };
 

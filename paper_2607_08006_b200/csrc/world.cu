@@ -87,6 +87,7 @@ extern "C" int shmemg_init(int npes, size_t heap_bytes_per_pe, void *device_slab
 
 extern "C" int shmemg_finalize(shmemg_world_t *w) {
     if (!w) return SHMEMG_ERR_ARG;
+    if (w->hot_scratch) cudaFree(w->hot_scratch);
     delete w;
     return SHMEMG_OK;
 }

@@ -9,7 +9,7 @@ from gpu_common import DEV, assert_objects_equal, heap_bytes_for, run_gpu, run_o
 from invariants import check_compare_swap_claim, check_fetch_add
 from oracle import oracle as orc
 from paper_2607_08006_b200 import CAP, CMP, ERR, SIGNAL, TEAM, ShmemgError, World
-from paper_2607_08006_b200.binding import AMO_TEST_BEFORE_SWAP, AMO_WARP_AGGREGATE, F32, I64
+from paper_2607_08006_b200.binding import AMO_HOT_AGGREGATE, AMO_TEST_BEFORE_SWAP, AMO_WARP_AGGREGATE, F32, I64
 from paper_2607_08006_b200.loader import Loaded
 from workloads import configs, gen
 
@@ -112,16 +112,16 @@ def test_atomic_add_heavy_contention_and_scalar_value():
     a = w.calloc(8, 8)
     tgt = torch.zeros(n, dtype=torch.int32, device=DEV)
     idx = (torch.arange(n, device=DEV) % 3).to(torch.int32)
-    for flags in (0, AMO_WARP_AGGREGATE):
+    for flags in (0, AMO_WARP_AGGREGATE, AMO_HOT_AGGREGATE):
         w.atomic_add_batch(a, tgt, idx, val=None, val_scalar=M64, flags=flags)       # adds -1 (wraparound)
     w.quiet(0)
     v = w.view(a, 64, torch.int64).cpu().numpy()
     cnt = np.bincount(np.arange(n) % 3, minlength=3)
-    assert v[0, :3].tolist() == (-2 * cnt).tolist() and v[1].sum() == 0
+    assert v[0, :3].tolist() == (-3 * cnt).tolist() and v[1].sum() == 0
 
 
-@pytest.mark.parametrize("n", [1, 1025, 3 * 8192 + 77, (1 << 20) + 5])
-@pytest.mark.parametrize("flags", [0, AMO_WARP_AGGREGATE])
+@pytest.mark.parametrize("n", [1, 1025, 3 * 8192 + 77, (1 << 20) + 5, (1 << 21) + 1029])
+@pytest.mark.parametrize("flags", [0, AMO_WARP_AGGREGATE, AMO_HOT_AGGREGATE])
 @pytest.mark.parametrize("idx_dtype", [np.int64, np.uint32])
 def test_fetch_add_skewed_scalar_value_ragged(n, flags, idx_dtype):
     """Ragged sizes, a skewed key distribution (many duplicates inside one warp), a scalar value > 1, non-zero initial
@@ -168,7 +168,8 @@ def _run_c4(g, flags):
     return degs, pars, f_deg.cpu().numpy().view(np.uint64), f_par.cpu().numpy().view(np.uint64)
 
 
-@pytest.mark.parametrize("flags", [0, AMO_WARP_AGGREGATE, AMO_TEST_BEFORE_SWAP, AMO_WARP_AGGREGATE | AMO_TEST_BEFORE_SWAP])
+@pytest.mark.parametrize("flags", [0, AMO_WARP_AGGREGATE, AMO_TEST_BEFORE_SWAP, AMO_WARP_AGGREGATE | AMO_TEST_BEFORE_SWAP,
+                                   AMO_HOT_AGGREGATE | AMO_TEST_BEFORE_SWAP])
 def test_c4_graph_small_full_oracle(flags):
     g = configs.c4_graph(scale=16, edge_factor=16, npes=32)
     degs, pars, f_deg, f_par = _run_c4(g, flags)
@@ -213,7 +214,7 @@ def test_compare_swap_test_before_swap_with_noop_swaps():
 def test_c4_graph_full_scale():
     """Config 4 at its full size (RMAT scale 22, 2^26 edges, 32 PEs) in the launch configuration bench.py times."""
     g = configs.c4_graph()
-    degs, pars, f_deg, f_par = _run_c4(g, AMO_TEST_BEFORE_SWAP)
+    degs, pars, f_deg, f_par = _run_c4(g, AMO_HOT_AGGREGATE | AMO_TEST_BEFORE_SWAP)
     E = len(g.u)
     assert np.array_equal(degs, np.bincount(g.u, minlength=1 << 22).astype(np.uint64))   # = the oracle's pinned closed form
     ow = orc.OracleWorld(g.npes, g.verts_per_pe * 8 + 512)                           # oracle degrees, sequentially
