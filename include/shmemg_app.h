@@ -25,6 +25,17 @@ SHMEMG_API int shmemg_app_halo_pack_on_stream(shmemg_world_t *w, uint64_t send_o
  * `out` is a DEVICE array of npes*nseg uint64, overwritten. */
 SHMEMG_API int shmemg_app_checksum64_on_stream(shmemg_world_t *w, uint64_t *out, uint64_t sym_off, uint64_t seg_bytes,
                                                uint32_t nseg, void *stream);
+/* The halo application DEVICE-INITIATED and persistent ("kernel-boundary
+ * synchronisation limits strong scaling"): ONE cooperative kernel runs rounds first_round .. first_round+rounds-1.  Every PE is
+ * a group of thread blocks.  Per round: perturb the boundary cells; the group synchronises; six blocks put one face each
+ * straight out of the cube (shmemg_dev_ibput_block) into the neighbour's ghost[round & 1][face'] and signal sig[face'] = round
+ * (shmemg_dev_signal_block) while all other blocks already perturb the interior; at the end of the round the PE waits for
+ * its six signals (shmemg_dev_signal_wait_until).  No send buffer, no pack kernel, no kernel boundary between rounds.
+ * Results (U, ghost, sig) are bit-identical to rounds of perturb + pack + put_signal/wait batches.
+ * Returns SHMEMG_ERR_NOMEM if the blocks cannot all be co-resident. */
+SHMEMG_API int shmemg_app_halo_persistent_on_stream(shmemg_world_t *w, uint64_t U_off, uint64_t ghost_off, uint64_t sig_off,
+                                                    uint32_t B, uint64_t seed, uint64_t first_round, uint32_t rounds,
+                                                    void *stream);
 #ifdef __cplusplus
 }
 #endif

@@ -187,6 +187,35 @@ __device__ __forceinline__ void shmemg_dev_put_signal_block(const shmemg_device_
     if (shmemg_dev_block_tid() == 0)
         shmemg_dev_signal_update(reinterpret_cast<unsigned long long *>(shmemg_dev_ptr(w, sig_off, target_pe)), signal, sig_op);
 }
+/* block scope, block-strided (ibput analog): for b < nblocks: dest[b*dst_stride .. +block_bytes) on `target_pe` =
+ * source[b*src_stride .. +block_bytes) on `pe`; strides in bytes.  8-byte aligned blocks move one 64-bit word per thread
+ * (the contiguous side coalesces), anything else goes block by block through the any-alignment copy. */
+__device__ __forceinline__ void shmemg_dev_ibput_block(const shmemg_device_world_t &w, uint64_t dest_off, uint64_t source_off,
+                                                       uint64_t dst_stride, uint64_t src_stride, size_t block_bytes,
+                                                       size_t nblocks, int pe, int target_pe) {
+    unsigned char *d = shmemg_dev_ptr(w, dest_off, target_pe);
+    const unsigned char *s = shmemg_dev_ptr(w, source_off, pe);
+    const int tid = shmemg_dev_block_tid(), nthr = shmemg_dev_block_size();
+    if (((reinterpret_cast<uintptr_t>(d) | reinterpret_cast<uintptr_t>(s) | dst_stride | src_stride | block_bytes) & 7) == 0) {
+        const size_t wpb = block_bytes >> 3;
+        for (size_t e = tid; e < nblocks * wpb; e += nthr) {
+            const size_t b = e / wpb, k = e % wpb;
+            *reinterpret_cast<unsigned long long *>(d + b * dst_stride + 8 * k) =
+                *reinterpret_cast<const volatile unsigned long long *>(s + b * src_stride + 8 * k);
+        }
+    } else {
+        for (size_t b = 0; b < nblocks; ++b) shmemg_dev_copy(d + b * dst_stride, s + b * src_stride, block_bytes, tid, nthr);
+    }
+    __syncthreads();
+}
+/* block scope: signal only -- everything the BLOCK has put before becomes visible on target_pe before the signal */
+__device__ __forceinline__ void shmemg_dev_signal_block(const shmemg_device_world_t &w, uint64_t sig_off, uint64_t signal,
+                                                        int sig_op, int target_pe) {
+    shmemg_dev_fence_gpu();
+    __syncthreads();
+    if (shmemg_dev_block_tid() == 0)
+        shmemg_dev_signal_update(reinterpret_cast<unsigned long long *>(shmemg_dev_ptr(w, sig_off, target_pe)), signal, sig_op);
+}
 /* blocks the calling thread until cmp(u64 heap[pe][sig_off], value) holds (unsigned compare); what it reads afterwards
  * is at least as new as what the signalling put_signal released */
 __device__ __forceinline__ uint64_t shmemg_dev_signal_wait_until(const shmemg_device_world_t &w, uint64_t sig_off, int cmp,

@@ -136,6 +136,7 @@ SYMBOLS = {
     "shmemg_app_halo_perturb_on_stream": (_i, [_vp, _u64, _u32, _u64, _u64, _vp]),
     "shmemg_app_halo_pack_on_stream": (_i, [_vp, _u64, _u64, _u32, _vp]),
     "shmemg_app_checksum64_on_stream": (_i, [_vp, _vp, _u64, _u64, _u32, _vp]),
+    "shmemg_app_halo_persistent_on_stream": (_i, [_vp, _u64, _u64, _u64, _u32, _u64, _u64, _u32, _vp]),
     "shmemg_probe_atomic_on_stream": (_i, [_vp, _i, _u64, _u64, _sz, _vp]),
     "shmemg_probe_copy_all_on_stream": (_i, [_vp, _u64, _u64, _sz, _vp]),
 }
@@ -445,6 +446,10 @@ class World:
     def app_halo_pack(self, send_off, U_off, B, stream=None):
         self._chk(lib().shmemg_app_halo_pack_on_stream(self.h, send_off, U_off, B, _stream(stream)),
                   "shmemg_app_halo_pack_on_stream")
+
+    def app_halo_persistent(self, U_off, ghost_off, sig_off, B, seed, first_round, rounds, stream=None):
+        self._chk(lib().shmemg_app_halo_persistent_on_stream(self.h, U_off, ghost_off, sig_off, B, seed, first_round, rounds,
+                                                             _stream(stream)), "shmemg_app_halo_persistent_on_stream")
 
     def app_checksum64(self, out, sym_off, seg_bytes, nseg, stream=None):
         self._chk(lib().shmemg_app_checksum64_on_stream(self.h, _dptr(out), sym_off, seg_bytes, nseg, _stream(stream)),

@@ -97,3 +97,93 @@ extern "C" int shmemg_app_checksum64_on_stream(shmemg_world_t *w, uint64_t *out,
     SHMEMG_CUDA(w, cudaGetLastError());
     return SHMEMG_OK;
 }
+
+// ---- the same application, device-initiated and persistent (include/shmemg_app.h) -----------------------------------------
+#include "../../include/shmemg_device.cuh"
+
+__device__ __forceinline__ void halo_perturb_cell(double *U, size_t c, unsigned B, unsigned px, unsigned py, unsigned pz,
+                                                  unsigned long long seed, unsigned long long round) {
+    const size_t z = c % B, y = (c / B) % B, x = c / ((size_t)B * B), G = 2ull * B;
+    const size_t g = ((px * (size_t)B + x) * G + (py * (size_t)B + y)) * G + (pz * (size_t)B + z);
+    U[c] = U[c] + (double)(mix64(seed, round, g) & 0xFFFFull) * 0x1.0p-30;
+}
+// all blocks of one PE's group: arrive (release) and wait until the whole group has (acquire); counters are monotonic
+__device__ __forceinline__ void halo_group_sync(unsigned *bar, unsigned group) {
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        unsigned old;
+        asm volatile("atom.acq_rel.gpu.global.add.u32 %0, [%1], 1;" : "=r"(old) : "l"(bar) : "memory");
+        const unsigned target = (old / group + 1u) * group;
+        unsigned v;
+        do { asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(bar) : "memory"); } while ((int)(v - target) < 0);
+    }
+    __syncthreads();
+}
+
+__global__ void __launch_bounds__(512) k_halo_persistent(const shmemg_device_world_t dw, unsigned *group_bar, uint64_t U_off,
+                                                         uint64_t ghost_off, uint64_t sig_off, unsigned B, unsigned long long seed,
+                                                         unsigned long long first_round, unsigned rounds, unsigned group) {
+    const unsigned p = blockIdx.x / group, g = blockIdx.x % group;           // PE and block within the PE's group
+    const unsigned px = (p >> 2) & 1, py = (p >> 1) & 1, pz = p & 1;
+    double *U = reinterpret_cast<double *>(shmemg_dev_ptr(dw, U_off, (int)p));
+    const size_t n = (size_t)B * B * B, fb = (size_t)B * B * 8;
+    const size_t gt = (size_t)g * blockDim.x + threadIdx.x, GT = (size_t)group * blockDim.x;
+    for (unsigned long long r = first_round; r < first_round + rounds; ++r) {
+        // (a) boundary cells, each exactly once: x-planes; y-planes without the x-planes; z-planes without both
+        const size_t nx = 2ull * B * B, ny = B > 2 ? 2ull * (B - 2) * B : 0, nz = B > 2 ? 2ull * (B - 2) * (B - 2) : 0;
+        for (size_t k = gt; k < nx + ny + nz; k += GT) {
+            size_t x, y, z;
+            if (k < nx) { x = (k / ((size_t)B * B)) ? B - 1 : 0; y = (k / B) % B; z = k % B; }
+            else if (k < nx + ny) { const size_t q = k - nx; z = q % B; y = ((q / B) & 1) ? B - 1 : 0; x = 1 + q / (2ull * B); }
+            else { const size_t q = k - nx - ny; z = (q & 1) ? B - 1 : 0; y = 1 + (q >> 1) % (B - 2); x = 1 + (q >> 1) / (B - 2); }
+            if (B == 1 && k >= 1) continue;                                   // B = 1: one cell
+            halo_perturb_cell(U, (x * B + y) * B + z, B, px, py, pz, seed, r);
+        }
+        __threadfence();
+        halo_group_sync(group_bar + p, group);                               // the PE's boundary is final for this round
+        // (b) six blocks put one face each and signal; f = 2*axis + dir lands in slot 2*axis + (1-dir) of the neighbour
+        if (g < 6) {
+            const unsigned f = g, axis = f >> 1, dir = f & 1, t = p ^ (4u >> axis), fr = 2 * axis + (1 - dir);
+            const uint64_t dst = ghost_off + (((r & 1) * 6 + fr) * fb);
+            const size_t fix = dir ? B - 1 : 0;
+            if (axis == 0) shmemg_dev_ibput_block(dw, dst, U_off + fix * fb, 0, 0, fb, 1, (int)p, (int)t);
+            else if (axis == 1) shmemg_dev_ibput_block(dw, dst, U_off + fix * B * 8, (uint64_t)B * 8, fb, (size_t)B * 8, B, (int)p, (int)t);
+            else shmemg_dev_ibput_block(dw, dst, U_off + fix * 8, 8, (uint64_t)B * 8, 8, (size_t)B * B, (int)p, (int)t);
+            shmemg_dev_signal_block(dw, sig_off + fr * 8, r, SHMEMG_SIGNAL_SET, (int)t);
+        }
+        // (c) the interior, overlapping the exchange
+        for (size_t c = gt; c < n; c += GT) {
+            const size_t z = c % B, y = (c / B) % B, x = c / ((size_t)B * B);
+            if (x == 0 || x == B - 1 || y == 0 || y == B - 1 || z == 0 || z == B - 1) continue;
+            halo_perturb_cell(U, c, B, px, py, pz, seed, r);
+        }
+        // (d) this round's six faces have arrived (and may be consumed); also keeps neighbours within one round of each other
+        if (threadIdx.x < 6) shmemg_dev_signal_wait_until(dw, sig_off + threadIdx.x * 8, SHMEMG_CMP_GE, r, (int)p);
+        // (e) the face blocks have finished reading the boundary before anybody perturbs it again
+        halo_group_sync(group_bar + p, group);
+    }
+}
+
+extern "C" int shmemg_app_halo_persistent_on_stream(shmemg_world_t *w, uint64_t U_off, uint64_t ghost_off, uint64_t sig_off,
+                                                    uint32_t B, uint64_t seed, uint64_t first_round, uint32_t rounds,
+                                                    void *stream) {
+    if (!w || w->npes != 8 || B == 0) return SHMEMG_ERR_ARG;
+    const uint64_t fb = (uint64_t)B * B * 8;
+    if (!shmemg_in_range(w, U_off, fb * B) || !shmemg_in_range(w, ghost_off, 12 * fb) || !shmemg_in_range(w, sig_off, 48))
+        return SHMEMG_ERR_RANGE;
+    if ((U_off | ghost_off | sig_off) & 7) return SHMEMG_ERR_ALIGN;
+    if (rounds == 0) return SHMEMG_OK;
+    int per_sm = 0;
+    SHMEMG_CUDA(w, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_halo_persistent, 512, 0));
+    unsigned group = (unsigned)((size_t)w->sm_count * per_sm / 8);
+    if (group < 6) return SHMEMG_ERR_NOMEM;                                   // six face blocks per PE must be co-resident
+    if (group > 64) group = 64;
+    shmemg_device_world_t dw;
+    int rc = shmemg_device_world_get(w, &dw);
+    if (rc) return rc;
+    unsigned *bar = w->ctl->group_bar;
+    unsigned long long seed_ = seed, first_ = first_round;
+    void *args[] = {&dw, &bar, &U_off, &ghost_off, &sig_off, &B, &seed_, &first_, &rounds, &group};
+    SHMEMG_CUDA(w, cudaLaunchCooperativeKernel((void *)k_halo_persistent, dim3(8 * group), dim3(512), args, 0, (cudaStream_t)stream));
+    return SHMEMG_OK;
+}

@@ -26,6 +26,7 @@ struct CtlRegion {
     unsigned int bar_gen;                  // in-kernel barrier: generation (sense)
     unsigned int pad[12];
     unsigned int sig_counter[SHMEMG_SIG_SLOTS];   // last-arriver counters of single put_signal launches
+    unsigned int group_bar[128];           // per-PE arrival counters of multi-block PE agents (monotonic; halo_app.cu)
     unsigned int hot_n;                    // SHMEMG_AMO_HOT_AGGREGATE: number of hot words found by the sampling kernel
     unsigned int hot_done;                 // CTAs of the sampling kernel that have staged their keys
     unsigned int hot_keys[SHMEMG_HOT_MAX]; // their slab word indices

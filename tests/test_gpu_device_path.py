@@ -122,3 +122,33 @@ def test_device_exec_rejects_bad_descriptors_and_empty_list():
     with pytest.raises(ShmemgError) as e:
         w.device_exec_ops(o)
     assert e.value.code == ERR.PE
+
+
+@pytest.mark.parametrize("B,rounds,split", [(16, 20, 7), (5, 9, 9), (2, 4, 1), (1, 3, 3), (256, 2, 2)])
+def test_halo_persistent_device_initiated_matches_oracle(B, rounds, split):
+    """Config 2 run by ONE persistent device-initiated kernel (no pack kernel, no send buffer, no kernel boundary between
+    rounds): U, both ghost buffers and the signal words must be bit-identical to the oracle's perturb + pack + put_signal /
+    wait rounds.  `split`: the rounds are run as two launches (first `split`, then the rest) to cover a restart."""
+    from oracle import oracle as orc
+    from paper_2607_08006_b200.loader import Loaded
+    h = configs.Halo(B)
+    prog = h.program(with_consume=False)
+    hb = sum((b + 255) // 256 * 256 for b in prog.obj_bytes) + 4096
+    w = World(8, hb, DEV)
+    ld = Loaded(w, prog)
+    ow = orc.OracleWorld(8, hb)
+    ow.load_program(prog)
+    U_off, ghost_off, sig_off = ld.off["U"][0], ld.off["ghost"][0], ld.off["sig"][0]
+    w.app_halo_persistent(U_off, ghost_off, sig_off, B, h.seed, 1, split)
+    if rounds > split:
+        w.app_halo_persistent(U_off, ghost_off, sig_off, B, h.seed, split + 1, rounds - split)
+    w.quiet(0)
+    for r in range(1, rounds + 1):
+        Uo, so = ow.obj("U", np.float64), ow.obj("send", np.float64).reshape(8, 6, B * B)
+        for p in range(8):
+            orc.halo_perturb(Uo[p], B, h.coord(p), h.seed, r)
+            for f in range(6):
+                orc.halo_pack(Uo[p], B, f, so[p, f])
+        ow.run_program(h.round_ops(prog, r, False))
+    assert_objects_equal(prog, ld, ow, names=["ghost", "sig"])
+    assert np.array_equal(ld.obj_numpy("U", np.float64), ow.obj("U", np.float64))
