@@ -191,6 +191,10 @@ def segment_table(inp: Inputs):
             seg["next2_amo_xor"] = dict(cls="xamo", kernel="k_amo2<xor>", ops=len(inp.c4.u), launches=1)
             seg["next2_amo_fetch_xor"] = dict(cls="xamo", kernel="k_amo2<fetch_xor>", ops=len(inp.c4.u), launches=1)
         if "c2" in g:
+            # NEXT-1: the whole halo APPLICATION (compute + exchange) per round, three ways; us per round is what counts
+            seg["next1_halo_app_host_batches"] = dict(cls="xtime", kernel="k_halo_perturb + k_halo_pack + k_batch_exec", ops=HALO_ROUNDS, launches=3 * HALO_ROUNDS)
+            seg["next1_halo_app_persistent"] = dict(cls="xtime", kernel="k_halo_persistent (device-initiated)", ops=HALO_ROUNDS, launches=1)
+            seg["next1_halo_app_compute_only"] = dict(cls="xtime", kernel="k_halo_perturb", ops=HALO_ROUNDS, launches=HALO_ROUNDS)
             seg["next2_ibput_faces"] = dict(cls="xcopy", kernel="k_ib_tma/k_ib_elem", bytes=3 * 2 * inp.halo.face_bytes, launches=3)
     if "barrier" in g:
         seg["barrier_in_kernel"] = dict(cls="sync", kernel="k_barrier_repeat", ops=BARRIERS, launches=1)
@@ -202,6 +206,14 @@ def segment_table(inp: Inputs):
 # ======================================================================================================================
 # CUDA arm: everything goes through the C-ABI (binding = argument marshalling only)
 # ======================================================================================================================
+class _Null:
+    def __enter__(self):
+        return self
+
+    def __exit__(self, *exc):
+        return False
+
+
 class Recorder:
     """CUDA-event pairs around library calls, on the launching (current) stream."""
 
@@ -348,12 +360,13 @@ class CudaBench:
             h, w = inp.halo, self.w2
             self.ld2.obj("sig").zero_()                                  # rounds restart at 1 every step
             send_off = self.ld2.off["send"][0]
-            for r in range(1, HALO_ROUNDS + 1):
-                w.app_halo_perturb(self.U_off, h.B, h.seed, r)           # application compute, not library time
-                w.app_halo_pack(send_off, self.U_off, h.B)
-                self.app_launches += 2
-                with rec.seg("halo_put_signal_wait"):
-                    w.enqueue_batch(self.halo_batches[r - 1])
+            with rec.seg("next1_halo_app_host_batches") if "next2" in g else _Null():
+                for r in range(1, HALO_ROUNDS + 1):
+                    w.app_halo_perturb(self.U_off, h.B, h.seed, r)       # application compute, not library time
+                    w.app_halo_pack(send_off, self.U_off, h.B)
+                    self.app_launches += 2
+                    with rec.seg("halo_put_signal_wait"):
+                        w.enqueue_batch(self.halo_batches[r - 1])
         if "next2" in g:
             from paper_2607_08006_b200.binding import AMO, F32, I64, RED
             if "c5" in g:
@@ -371,6 +384,14 @@ class CudaBench:
                     self.w4.atomic_op_batch(AMO.XOR, 8, self.deg, self.c4_ou, self.c4_lu, val=self.c4_val, fetched_out=self.f_deg)
             if "c2" in g:
                 h, B = inp.halo, inp.halo.B
+                self.ld2.obj("sig").zero_()
+                with rec.seg("next1_halo_app_persistent"):     # the same 50 rounds in ONE device-initiated kernel
+                    self.w2.app_halo_persistent(self.U_off, self.ld2.off["ghost"][0], self.ld2.off["sig"][0], B, h.seed, 1, HALO_ROUNDS)
+                    self.app_launches += 1
+                with rec.seg("next1_halo_app_compute_only"):
+                    for r in range(1, HALO_ROUNDS + 1):
+                        self.w2.app_halo_perturb(self.U_off, B, h.seed, r)
+                    self.app_launches += HALO_ROUNDS
                 send_off, fb = self.ld2.off["send"][0], inp.halo.face_bytes
                 with rec.seg("next2_ibput_faces"):             # the three face orientations straight out of the cube
                     self.w2.ibput(send_off, self.U_off, 0, 0, fb, 1, 0, 1)
@@ -784,6 +805,9 @@ def run_cuda(args):
             d["GBps"] = units[k] / world / secs[k] / 1e9
             d["frac_of_measured_hbm"] = d["GBps"] / peak
             d["in_headline"] = False
+        elif t["cls"] == "xtime":
+            d["us_per_round"] = seg_ms[k] / K / t["ops"] * 1e3
+            d["in_headline"] = False
         elif t["cls"] == "xamo":
             d["Mops"] = units[k] / world / secs[k] / 1e6
             d["in_headline"] = False
@@ -818,7 +842,7 @@ def run_cuda(args):
 
     line = base_line(args, world)
     line.update({"value": gbps, "amo_mops": mops, "ms_per_step": whole_ms / K,
-                 "timed_ms_per_step": sum(seg_ms.values()) / K, "dtype": "u8 (copies), u64 (AMOs), f64-accumulated f32 / i64 (sum_reduce)",
+                 "timed_ms_per_step": sum(v for k, v in seg_ms.items() if table[k]["cls"] != "xtime") / K, "dtype": "u8 (copies), u64 (AMOs), f64-accumulated f32 / i64 (sum_reduce)",
                  "segments": segments, "ceilings": ceil, "roofline": roofline, "clocks": clocks, "gpu_launches": launches,
                  "input_generation_s": inp.gen_seconds})
     if e2e_ms:

@@ -27,12 +27,13 @@ SHMEMG_API int shmemg_app_checksum64_on_stream(shmemg_world_t *w, uint64_t *out,
                                                uint32_t nseg, void *stream);
 /* The halo application DEVICE-INITIATED and persistent ("kernel-boundary
  * synchronisation limits strong scaling"): ONE cooperative kernel runs rounds first_round .. first_round+rounds-1.  Every PE is
- * a group of thread blocks.  Per round: perturb the boundary cells; the group synchronises; six blocks put one face each
- * straight out of the cube (shmemg_dev_ibput_block) into the neighbour's ghost[round & 1][face'] and signal sig[face'] = round
- * (shmemg_dev_signal_block) while all other blocks already perturb the interior; at the end of the round the PE waits for
- * its six signals (shmemg_dev_signal_wait_until).  No send buffer, no pack kernel, no kernel boundary between rounds.
- * Results (U, ghost, sig) are bit-identical to rounds of perturb + pack + put_signal/wait batches.
- * Returns SHMEMG_ERR_NOMEM if the blocks cannot all be co-resident. */
+ * a group of thread blocks.  Six "face blocks" per PE: perturb the boundary cells, synchronise among themselves, put one face
+ * each straight out of the cube (shmemg_dev_ibput_block) into the neighbour's ghost[round & 1][face'], signal sig[face'] =
+ * round (shmemg_dev_signal_block) and wait for their own incoming face (shmemg_dev_signal_wait_until_block).  All other
+ * blocks perturb the interior and never wait inside a round; before the next round they check that the round's six faces
+ * have arrived.  No send buffer, no pack kernel, no kernel boundary between rounds; the exchange is hidden behind the interior
+ * update.  Results (U, ghost, sig) are bit-identical to rounds of perturb + pack + put_signal/wait batches.
+ * Returns SHMEMG_ERR_NOMEM if the blocks cannot all be co-resident.  B <= 1024. */
 SHMEMG_API int shmemg_app_halo_persistent_on_stream(shmemg_world_t *w, uint64_t U_off, uint64_t ghost_off, uint64_t sig_off,
                                                     uint32_t B, uint64_t seed, uint64_t first_round, uint32_t rounds,
                                                     void *stream);

@@ -197,11 +197,20 @@ __device__ __forceinline__ void shmemg_dev_ibput_block(const shmemg_device_world
     const unsigned char *s = shmemg_dev_ptr(w, source_off, pe);
     const int tid = shmemg_dev_block_tid(), nthr = shmemg_dev_block_size();
     if (((reinterpret_cast<uintptr_t>(d) | reinterpret_cast<uintptr_t>(s) | dst_stride | src_stride | block_bytes) & 7) == 0) {
-        const size_t wpb = block_bytes >> 3;
-        for (size_t e = tid; e < nblocks * wpb; e += nthr) {
-            const size_t b = e / wpb, k = e % wpb;
-            *reinterpret_cast<unsigned long long *>(d + b * dst_stride + 8 * k) =
-                *reinterpret_cast<const volatile unsigned long long *>(s + b * src_stride + 8 * k);
+        const size_t wpb = block_bytes >> 3, nw = nblocks * wpb;
+#pragma unroll 1
+        for (size_t e0 = tid; e0 < nw; e0 += (size_t)4 * nthr) {          /* four independent words in flight per thread */
+            unsigned long long v[4];
+#pragma unroll
+            for (int u = 0; u < 4; ++u) {
+                const size_t e = e0 + (size_t)u * nthr, b = e / wpb, k = e - b * wpb;
+                if (e < nw) v[u] = *reinterpret_cast<const volatile unsigned long long *>(s + b * src_stride + 8 * k);
+            }
+#pragma unroll
+            for (int u = 0; u < 4; ++u) {
+                const size_t e = e0 + (size_t)u * nthr, b = e / wpb, k = e - b * wpb;
+                if (e < nw) *reinterpret_cast<unsigned long long *>(d + b * dst_stride + 8 * k) = v[u];
+            }
         }
     } else {
         for (size_t b = 0; b < nblocks; ++b) shmemg_dev_copy(d + b * dst_stride, s + b * src_stride, block_bytes, tid, nthr);
