@@ -60,6 +60,10 @@ def lib():
         L.orc_amo_batch.argtypes = [vp, i, u64, i, i, u64, vp, vp, vp, vp, u64]
         L.orc_ibput.argtypes = [vp, i, u64, u64, u64, u64, u64, u64, u64, i, i, i]
         L.orc_signal_test.argtypes = [vp, i, u64, u64, i, u64, i]
+        L.orc_team_fcollect.argtypes = [vp, i, u64, i, i, i, u64, u64, u64]
+        L.orc_team_alltoall.argtypes = [vp, i, u64, i, i, i, u64, u64, u64]
+        L.orc_team_broadcast.argtypes = [vp, i, u64, i, i, i, u64, u64, u64, i]
+        L.orc_team_reduce.argtypes = [vp, i, u64, i, i, i, i, i, u64, u64, u64]
         L.orc_halo_delta.argtypes = [u64, u64, u64]
         L.orc_halo_delta.restype = C.c_double
         L.orc_halo_perturb.argtypes = [vp, u64, i, i, i, u64, u64]
@@ -226,6 +230,23 @@ class OracleWorld:
     def ibget(self, dst_off, src_off, dst_stride, src_stride, block, nblocks, pe, target):
         _chk(lib().orc_ibput(self.heap.ctypes.data, self.npes, self.heap_bytes, dst_off, src_off, dst_stride,
                              src_stride, block, nblocks, pe, target, 1), "ibget")
+
+    # ---- NEXT-3: collectives over a strided team (start, stride, size); ranks are team-relative ----
+    def team_fcollect(self, team, dst_off, src_off, nbytes):
+        _chk(lib().orc_team_fcollect(self.heap.ctypes.data, self.npes, self.heap_bytes, *team, dst_off, src_off, nbytes),
+             "team_fcollect")
+
+    def team_alltoall(self, team, dst_off, src_off, nbytes):
+        _chk(lib().orc_team_alltoall(self.heap.ctypes.data, self.npes, self.heap_bytes, *team, dst_off, src_off, nbytes),
+             "team_alltoall")
+
+    def team_broadcast(self, team, dst_off, src_off, nbytes, root_rank):
+        _chk(lib().orc_team_broadcast(self.heap.ctypes.data, self.npes, self.heap_bytes, *team, dst_off, src_off, nbytes,
+                                      root_rank), "team_broadcast")
+
+    def team_reduce(self, team, op: str, dtype: str, dst_off, src_off, nreduce):
+        _chk(lib().orc_team_reduce(self.heap.ctypes.data, self.npes, self.heap_bytes, *team, self.RED[op],
+                                   self.DTYPE[dtype], dst_off, src_off, nreduce), "team_reduce")
 
     def signal_test(self, sig_off, cmp, value, pe) -> bool:
         r = lib().orc_signal_test(self.heap.ctypes.data, self.npes, self.heap_bytes, sig_off, cmp, value, pe)

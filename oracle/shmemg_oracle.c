@@ -382,6 +382,67 @@ int orc_signal_test(const uint8_t *heap, int npes, uint64_t heap_bytes, uint64_t
     }
 }
 
+/* ---- team collectives ("PE collectives remain collective over a team of
+ * PEs").  A team is the strided PE set { start + k*stride : 0 <= k < size } (shmem_team_split_strided); team rank k is that
+ * PE.  Each collective is the world definition with "all PEs" replaced by "all team members, in team-rank order"; heaps of
+ * PEs outside the team are untouched.  The root of a broadcast is a TEAM RANK. */
+static int team_ok(int npes, int start, int stride, int size) {
+    return size >= 1 && start >= 0 && stride >= 1 && (long long)start + (long long)(size - 1) * stride < npes;
+}
+#define TPE(k) ((uint64_t)(start + (k) * stride))
+
+int orc_team_fcollect(uint8_t *heap, int npes, uint64_t heap_bytes, int start, int stride, int size, uint64_t dst_off,
+                      uint64_t src_off, uint64_t n) {
+    if (!team_ok(npes, start, stride, size)) return ORC_ERR_RANGE;
+    if (!in_range(src_off, n, heap_bytes) || !in_range(dst_off, n * (uint64_t)size, heap_bytes)) return ORC_ERR_RANGE;
+    for (int j = 0; j < size; ++j)
+        for (int k = 0; k < size; ++k)
+            memcpy(heap + TPE(j) * heap_bytes + dst_off + (uint64_t)k * n, heap + TPE(k) * heap_bytes + src_off, n);
+    return ORC_OK;
+}
+
+int orc_team_alltoall(uint8_t *heap, int npes, uint64_t heap_bytes, int start, int stride, int size, uint64_t dst_off,
+                      uint64_t src_off, uint64_t n) {
+    const uint64_t tot = n * (uint64_t)size;
+    if (!team_ok(npes, start, stride, size)) return ORC_ERR_RANGE;
+    if (!in_range(src_off, tot, heap_bytes) || !in_range(dst_off, tot, heap_bytes)) return ORC_ERR_RANGE;
+    if (!(src_off + tot <= dst_off || dst_off + tot <= src_off)) return ORC_ERR_RANGE;
+    for (int i = 0; i < size; ++i)
+        for (int j = 0; j < size; ++j)
+            memcpy(heap + TPE(j) * heap_bytes + dst_off + (uint64_t)i * n, heap + TPE(i) * heap_bytes + src_off + (uint64_t)j * n, n);
+    return ORC_OK;
+}
+
+int orc_team_broadcast(uint8_t *heap, int npes, uint64_t heap_bytes, int start, int stride, int size, uint64_t dst_off,
+                       uint64_t src_off, uint64_t n, int root_rank) {
+    if (!team_ok(npes, start, stride, size) || root_rank < 0 || root_rank >= size) return ORC_ERR_RANGE;
+    if (!in_range(src_off, n, heap_bytes) || !in_range(dst_off, n, heap_bytes)) return ORC_ERR_RANGE;
+    if (!(src_off + n <= dst_off || dst_off + n <= src_off)) return ORC_ERR_RANGE;
+    for (int j = 0; j < size; ++j)
+        memcpy(heap + TPE(j) * heap_bytes + dst_off, heap + TPE(root_rank) * heap_bytes + src_off, n);
+    return ORC_OK;
+}
+
+/* reduction over the team: gather the members' source rows into a scratch world of `size` PEs, reduce there with
+ * orc_reduce (ascending team rank = ascending scratch PE), scatter the result rows back to the members' dest. */
+#include <stdlib.h>
+int orc_team_reduce(uint8_t *heap, int npes, uint64_t heap_bytes, int start, int stride, int size, int op, int dtype,
+                    uint64_t dst_off, uint64_t src_off, uint64_t nreduce) {
+    const uint64_t es = (dtype == ORC_T_I64 || dtype == ORC_T_F64) ? 8 : 4, nb = es * nreduce;
+    if (!team_ok(npes, start, stride, size)) return ORC_ERR_RANGE;
+    if (!in_range(src_off, nb, heap_bytes) || !in_range(dst_off, nb, heap_bytes)) return ORC_ERR_RANGE;
+    if (nreduce == 0) return ORC_OK;
+    uint8_t *tmp = (uint8_t *)malloc((size_t)size * 2 * nb);
+    if (!tmp) return ORC_ERR_RANGE;
+    for (int k = 0; k < size; ++k) memcpy(tmp + (uint64_t)k * 2 * nb, heap + TPE(k) * heap_bytes + src_off, nb);
+    const int rc = orc_reduce(tmp, size, 2 * nb, op, dtype, nb, 0, nreduce);
+    if (rc == ORC_OK)
+        for (int k = 0; k < size; ++k) memcpy(heap + TPE(k) * heap_bytes + dst_off, tmp + (uint64_t)k * 2 * nb + nb, nb);
+    free(tmp);
+    return rc;
+}
+#undef TPE
+
 /* ---- application-side compute of the halo workload (config C2; SURVEY.md readings 21-23) ------
  * Not part of the specification's operations: the stencil application's own kernels, restated on
  * the CPU so the oracle can run the whole workload.  Both sides implement the same counter-based
