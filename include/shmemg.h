@@ -268,6 +268,26 @@ SHMEMG_API int shmemg_ibget_on_stream(shmemg_world_t *w, uint64_t dest_off, uint
                                       uint64_t src_stride, size_t block_bytes, size_t nblocks, int pe, int target_pe,
                                       void *stream);
 
+/* ---- teams ("PE collectives remain collective over a team of PEs", L357, L412) --------
+ * shmemg_team_split_strided: the PEs { start + k*stride : k < size } of `parent_team` (ranks of the parent; the three
+ * predefined teams are the world) form a new team; *new_team receives its handle (>= SHMEMG_TEAM_USER0).  Team rank k is the
+ * k-th member.  Teams live until shmemg_finalize.  The team collectives below are the world collectives with "all PEs"
+ * replaced by "all members in team-rank order"; windows of non-members are untouched; `root_rank` is a TEAM rank.  They run
+ * the same kernels on a strided view of the slab (member k's window = base + (start + k*stride) * heap_stride).
+ * shmem_query_capabilities accepts user team handles and answers as for SHMEM_TEAM_WORLD. */
+#define SHMEMG_TEAM_USER0 16
+SHMEMG_API int shmemg_team_split_strided(shmemg_world_t *w, int parent_team, int start, int stride, int size, int *new_team);
+SHMEMG_API int shmemg_team_n_pes(const shmemg_world_t *w, int team);
+SHMEMG_API int shmemg_team_translate_pe(const shmemg_world_t *w, int team, int rank);     /* world PE of a team rank, or < 0 */
+SHMEMG_API int shmemg_team_reduce_on_stream(shmemg_world_t *w, int team, int op, int dtype, uint64_t dest_off,
+                                            uint64_t source_off, size_t nreduce, void *stream);
+SHMEMG_API int shmemg_team_fcollect_on_stream(shmemg_world_t *w, int team, uint64_t dest_off, uint64_t source_off,
+                                              size_t nbytes, void *stream);
+SHMEMG_API int shmemg_team_alltoall_on_stream(shmemg_world_t *w, int team, uint64_t dest_off, uint64_t source_off,
+                                              size_t nbytes, void *stream);
+SHMEMG_API int shmemg_team_broadcast_on_stream(shmemg_world_t *w, int team, uint64_t dest_off, uint64_t source_off,
+                                               size_t nbytes, int root_rank, void *stream);
+
 /* signal test ("quiet, wait, and test"): *result_dev (DEVICE int32) = 1 if cmp(u64 heap[pe][sig_off], value)
  * holds when the stream reaches the call, else 0; never blocks.  A result of 1 is an acquire: work enqueued later on the
  * stream sees the payload the signal announced. */

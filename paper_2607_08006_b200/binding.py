@@ -127,6 +127,13 @@ SYMBOLS = {
     "shmemg_ibget_on_stream": (_i, [_vp, _u64, _u64, _u64, _u64, _sz, _sz, _i, _i, _vp]),
     "shmemg_signal_test_on_stream": (_i, [_vp, _u64, _i, _u64, _i, _vp, _vp]),
     "shmemg_fcollect_on_stream": (_i, [_vp, _u64, _u64, _sz, _vp]),
+    "shmemg_team_split_strided": (_i, [_vp, _i, _i, _i, _i, C.POINTER(_i)]),
+    "shmemg_team_n_pes": (_i, [_vp, _i]),
+    "shmemg_team_translate_pe": (_i, [_vp, _i, _i]),
+    "shmemg_team_reduce_on_stream": (_i, [_vp, _i, _i, _i, _u64, _u64, _sz, _vp]),
+    "shmemg_team_fcollect_on_stream": (_i, [_vp, _i, _u64, _u64, _sz, _vp]),
+    "shmemg_team_alltoall_on_stream": (_i, [_vp, _i, _u64, _u64, _sz, _vp]),
+    "shmemg_team_broadcast_on_stream": (_i, [_vp, _i, _u64, _u64, _sz, _i, _vp]),
     "shmemg_alltoall_on_stream": (_i, [_vp, _u64, _u64, _sz, _vp]),
     "shmemg_barrier_all_on_stream": (_i, [_vp, _vp]),
     "shmemg_barrier_all_repeat_on_stream": (_i, [_vp, _u32, _u64, _vp]),
@@ -406,6 +413,38 @@ class World:
         self._chk(lib().shmemg_signal_test_on_stream(self.h, sig_off, cmp, value & ((1 << 64) - 1), pe, _dptr(result_dev),
                                                      _stream(stream)), "shmemg_signal_test_on_stream")
         self.launches += 1
+
+    # ---- teams (NEXT-3) ---------------------------------------------------------------------------------------------------
+    def team_split_strided(self, parent_team, start, stride, size) -> int:
+        t = C.c_int(-1)
+        self._chk(lib().shmemg_team_split_strided(self.h, parent_team, start, stride, size, C.byref(t)), "shmemg_team_split_strided")
+        return t.value
+
+    def team_n_pes(self, team) -> int:
+        return lib().shmemg_team_n_pes(self.h, team)
+
+    def team_translate_pe(self, team, rank) -> int:
+        return lib().shmemg_team_translate_pe(self.h, team, rank)
+
+    def team_reduce(self, team, op, dtype, dest_off, source_off, nreduce, stream=None):
+        self._chk(lib().shmemg_team_reduce_on_stream(self.h, team, op, dtype, dest_off, source_off, nreduce, _stream(stream)),
+                  "shmemg_team_reduce_on_stream")
+        self.launches += 1 if nreduce else 0
+
+    def team_fcollect(self, team, dest_off, source_off, nbytes, stream=None):
+        self._chk(lib().shmemg_team_fcollect_on_stream(self.h, team, dest_off, source_off, nbytes, _stream(stream)),
+                  "shmemg_team_fcollect_on_stream")
+        self.launches += 1 if nbytes else 0
+
+    def team_alltoall(self, team, dest_off, source_off, nbytes, stream=None):
+        self._chk(lib().shmemg_team_alltoall_on_stream(self.h, team, dest_off, source_off, nbytes, _stream(stream)),
+                  "shmemg_team_alltoall_on_stream")
+        self.launches += 1 if nbytes else 0
+
+    def team_broadcast(self, team, dest_off, source_off, nbytes, root_rank, stream=None):
+        self._chk(lib().shmemg_team_broadcast_on_stream(self.h, team, dest_off, source_off, nbytes, root_rank, _stream(stream)),
+                  "shmemg_team_broadcast_on_stream")
+        self.launches += 1 if nbytes else 0
 
     def fcollect(self, dest_off, source_off, nbytes, stream=None):
         self._chk(lib().shmemg_fcollect_on_stream(self.h, dest_off, source_off, nbytes, _stream(stream)),

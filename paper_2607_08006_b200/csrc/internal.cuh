@@ -7,6 +7,7 @@
 
 #include <map>
 #include <string>
+#include <vector>
 
 #include "../../include/shmemg.h"
 
@@ -49,6 +50,9 @@ struct shmemg_world {
     size_t tile_bytes_override = 0;        // SHMEMG_TILE_BYTES (experiments; forces the register copy path)
     bool smem_attr_coll = false, smem_attr_probe = false;
     bool smem_attr_set = false;            // dynamic shared memory opt-in done for the bulk-copy kernels
+    struct Team { int start, stride, size; };
+    int teams_world_npes = 0;              // npes of the world while a team view is active (surface2.cu)
+    std::vector<Team> teams;               // user teams (shmemg_team_split_strided); handle = SHMEMG_TEAM_USER0 + index
     void *hot_scratch = nullptr;           // DEVICE: library-owned scratch of SHMEMG_AMO_HOT_AGGREGATE (grown on demand)
     size_t hot_scratch_bytes = 0;
     std::string last_cuda_error;

@@ -307,3 +307,68 @@ extern "C" int shmemg_signal_test_on_stream(shmemg_world_t *w, uint64_t sig_off,
     SHMEMG_CUDA(w, cudaGetLastError());
     return SHMEMG_OK;
 }
+
+// ---- teams (NEXT-3) -------------------------------------------------------------------------------------------------------
+// A team is a strided set of PEs; member k's window is base + (start + k*stride) * heap_stride, i.e. the team is itself a
+// "world" with base' = base + start*heap_stride, heap_stride' = stride*heap_stride, npes' = size.  The team collectives run the
+// world entry points on that view (the fields are swapped for the duration of the enqueue; kernels take them by value).
+static bool team_lookup(const shmemg_world *w, int team, shmemg_world::Team &t) {
+    if (team == SHMEM_TEAM_WORLD || team == SHMEM_DEVICE_TEAM_WORLD || team == SHMEM_DEVICE_TEAM_SHARED) {
+        t = {0, 1, w->teams_world_npes ? w->teams_world_npes : w->npes};
+        return true;
+    }
+    if (team < SHMEMG_TEAM_USER0 || (size_t)(team - SHMEMG_TEAM_USER0) >= w->teams.size()) return false;
+    t = w->teams[team - SHMEMG_TEAM_USER0];
+    return true;
+}
+struct TeamView {
+    shmemg_world *w;
+    uint8_t *base; size_t stride; int npes;
+    TeamView(shmemg_world *w_, const shmemg_world::Team &t) : w(w_), base(w_->base), stride(w_->stride), npes(w_->npes) {
+        w->teams_world_npes = npes;
+        w->base = base + (size_t)t.start * stride;
+        w->stride = stride * (size_t)t.stride;
+        w->npes = t.size;
+    }
+    ~TeamView() { w->base = base; w->stride = stride; w->npes = npes; w->teams_world_npes = 0; }
+};
+
+extern "C" int shmemg_team_split_strided(shmemg_world_t *w, int parent_team, int start, int stride, int size, int *new_team) {
+    if (!w || !new_team) return SHMEMG_ERR_ARG;
+    shmemg_world::Team p;
+    if (!team_lookup(w, parent_team, p)) return SHMEMG_ERR_ARG;
+    if (size < 1 || stride < 1 || start < 0 || (long long)start + (long long)(size - 1) * stride >= p.size) return SHMEMG_ERR_PE;
+    w->teams.push_back({p.start + start * p.stride, p.stride * stride, size});
+    *new_team = SHMEMG_TEAM_USER0 + (int)w->teams.size() - 1;
+    return SHMEMG_OK;
+}
+extern "C" int shmemg_team_n_pes(const shmemg_world_t *w, int team) {
+    shmemg_world::Team t;
+    return (w && team_lookup(w, team, t)) ? t.size : SHMEMG_ERR_ARG;
+}
+extern "C" int shmemg_team_translate_pe(const shmemg_world_t *w, int team, int rank) {
+    shmemg_world::Team t;
+    if (!w || !team_lookup(w, team, t)) return SHMEMG_ERR_ARG;
+    return (rank >= 0 && rank < t.size) ? t.start + rank * t.stride : SHMEMG_ERR_PE;
+}
+#define TEAM_CALL(call)                                        \
+    shmemg_world::Team t;                                      \
+    if (!w || !team_lookup(w, team, t)) return SHMEMG_ERR_ARG; \
+    TeamView view(w, t);                                       \
+    return call;
+extern "C" int shmemg_team_reduce_on_stream(shmemg_world_t *w, int team, int op, int dtype, uint64_t dest_off,
+                                            uint64_t source_off, size_t nreduce, void *stream) {
+    TEAM_CALL(shmemg_reduce_on_stream(w, op, dtype, dest_off, source_off, nreduce, stream))
+}
+extern "C" int shmemg_team_fcollect_on_stream(shmemg_world_t *w, int team, uint64_t dest_off, uint64_t source_off,
+                                              size_t nbytes, void *stream) {
+    TEAM_CALL(shmemg_fcollect_on_stream(w, dest_off, source_off, nbytes, stream))
+}
+extern "C" int shmemg_team_alltoall_on_stream(shmemg_world_t *w, int team, uint64_t dest_off, uint64_t source_off,
+                                              size_t nbytes, void *stream) {
+    TEAM_CALL(shmemg_alltoall_on_stream(w, dest_off, source_off, nbytes, stream))
+}
+extern "C" int shmemg_team_broadcast_on_stream(shmemg_world_t *w, int team, uint64_t dest_off, uint64_t source_off,
+                                               size_t nbytes, int root_rank, void *stream) {
+    TEAM_CALL(shmemg_broadcast_on_stream(w, dest_off, source_off, nbytes, root_rank, stream))
+}

@@ -99,6 +99,7 @@ extern "C" const char *shmemg_last_cuda_error(const shmemg_world_t *w) { return 
 
 extern "C" int shmem_query_capabilities(const shmemg_world_t *w, int team, uint64_t *caps) {
     if (!w || !caps) return SHMEMG_ERR_ARG;
+    if (team >= SHMEMG_TEAM_USER0 && (size_t)(team - SHMEMG_TEAM_USER0) < w->teams.size()) team = SHMEM_TEAM_WORLD;
     if (team != SHMEM_TEAM_WORLD && team != SHMEM_DEVICE_TEAM_WORLD && team != SHMEM_DEVICE_TEAM_SHARED)
         return SHMEMG_ERR_ARG;
     // Capabilities are per team.  All PEs share one GPU, so the three predefined teams have
