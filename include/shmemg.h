@@ -138,6 +138,7 @@ enum {
     SHMEMG_OP_QUIET = 9,                /* initiator's earlier ops complete and are visible         (L377-L390) */
     SHMEMG_OP_BARRIER_ALL = 10          /* all PEs: every earlier op of every PE complete           (L116, L369) */
 };
+#define SHMEMG_CTX_MAX 8
 enum { SHMEMG_SIGNAL_SET = 0, SHMEMG_SIGNAL_ADD = 1 };
 enum { SHMEMG_CMP_EQ = 0, SHMEMG_CMP_NE = 1, SHMEMG_CMP_GT = 2, SHMEMG_CMP_GE = 3, SHMEMG_CMP_LT = 4, SHMEMG_CMP_LE = 5 };
 
@@ -147,7 +148,8 @@ typedef struct shmemg_op {
     uint8_t opcode;        /* SHMEMG_OP_*                                                     */
     uint8_t sig_op;        /* SHMEMG_SIGNAL_* (PUT_SIGNAL)                                    */
     uint8_t cmp;           /* SHMEMG_CMP_*    (SIGNAL_WAIT_UNTIL), unsigned 64-bit comparison */
-    uint8_t reserved0;
+    uint8_t ctx;           /* context of the op, 0 .. SHMEMG_CTX_MAX-1 (0 = the default context): FENCE / QUIET /
+                            * SIGNAL_WAIT_UNTIL order only ops of the same (PE, context) pair */
     int32_t initiator_pe;
     int32_t target_pe;
     uint32_t reserved1;
@@ -168,6 +170,8 @@ typedef struct shmemg_op {
  *     them.  FENCE and QUIET are both implemented as "all earlier ops of this PE, to all targets, gets
  *     and atomics included, are complete and visible before any later op of this PE starts" -- the
  *     strong reading of L377, always conformant.  A wait also orders the PE's later ops after it.
+ *     "Of this PE" means: of the same (PE, ctx) pair -- contexts are independent ordering domains (L124-L130); a QUIET on
+ *     context 1 does not wait for the PE's traffic on context 0.  BARRIER_ALL covers every context of every PE.
  *   - PUT_SIGNAL: the signal update is atomic w.r.t. other signal updates and waits, and becomes visible
  *     only after the whole payload (release/acquire at GPU scope).
  *   - atomicity does not imply ordering.

@@ -80,7 +80,7 @@ NO_STAMP = (1 << 64) - 1
 
 # shmemg_op_t, 64 bytes
 OP_DTYPE = np.dtype([
-    ("opcode", "u1"), ("sig_op", "u1"), ("cmp", "u1"), ("reserved0", "u1"),
+    ("opcode", "u1"), ("sig_op", "u1"), ("cmp", "u1"), ("ctx", "u1"),
     ("initiator_pe", "i4"), ("target_pe", "i4"), ("reserved1", "u4"),
     ("rem_off", "u8"), ("loc_off", "u8"), ("nbytes", "u8"), ("value", "u8"), ("cond", "u8"), ("sig_off", "u8"),
 ])

@@ -422,12 +422,14 @@ __global__ void k_wait_until(const unsigned long long *sig, int cmp, unsigned lo
 int shmemg_validate_op(const shmemg_world *w, const shmemg_op_t &o) {
     switch (o.opcode) {
     case SHMEMG_OP_FENCE: case SHMEMG_OP_QUIET:
+        if (o.ctx >= SHMEMG_CTX_MAX) return SHMEMG_ERR_ARG;
         return shmemg_pe_ok(w, o.initiator_pe) ? SHMEMG_OK : SHMEMG_ERR_PE;
     case SHMEMG_OP_BARRIER_ALL:
         return SHMEMG_OK;
     default: break;
     }
     if (o.opcode < SHMEMG_OP_PUT || o.opcode > SHMEMG_OP_BARRIER_ALL) return SHMEMG_ERR_ARG;
+    if (o.ctx >= SHMEMG_CTX_MAX) return SHMEMG_ERR_ARG;
     if (!shmemg_pe_ok(w, o.initiator_pe)) return SHMEMG_ERR_PE;
     if (o.opcode == SHMEMG_OP_SIGNAL_WAIT_UNTIL) {
         if (o.cmp > SHMEMG_CMP_LE) return SHMEMG_ERR_ARG;
@@ -503,11 +505,19 @@ static uint32_t pick_seg_tiles(const shmemg_world *w, const shmemg_op_t *ops, si
 // ---- planning units: one per op (a marker, a copy op, an AMO, a wait) -------------------------------------------------
 struct Unit { uint8_t opc; int pe; size_t first, count; };    // [first, first+count) in the caller's op array
 
-static void build_units(const shmemg_op_t *ops, size_t nops, std::vector<Unit> &units) {
+// Ordering domains: FENCE / QUIET / SIGNAL_WAIT_UNTIL order the ops of ONE (PE, context) pair (a
+// context is an independent ordering domain); domain index = ctx * npes + pe.  Unit.pe holds that index.
+static int count_domains(const shmemg_world *w, const shmemg_op_t *ops, size_t nops) {
+    int nctx = 1;
+    for (size_t i = 0; i < nops; ++i)
+        if (ops[i].opcode != SHMEMG_OP_BARRIER_ALL && ops[i].ctx + 1 > nctx) nctx = ops[i].ctx + 1;
+    return nctx * w->npes;
+}
+static void build_units(const shmemg_world *w, const shmemg_op_t *ops, size_t nops, std::vector<Unit> &units) {
     units.clear();
     for (size_t i = 0; i < nops; ++i) {
         const shmemg_op_t &o = ops[i];
-        units.push_back({o.opcode, o.opcode == SHMEMG_OP_BARRIER_ALL ? 0 : o.initiator_pe, i, 1});
+        units.push_back({o.opcode, o.opcode == SHMEMG_OP_BARRIER_ALL ? 0 : o.initiator_pe + (int)o.ctx * w->npes, i, 1});
     }
 }
 
@@ -545,7 +555,7 @@ static PlanSizes plan_sizes(const shmemg_world *w, const shmemg_op_t *ops, size_
     s.tiles_off = sizeof(PlanHeader);
     s.aux_off = s.tiles_off + up(s.ntiles * sizeof(TileRec));
     s.done_off = s.aux_off + up(s.naux * sizeof(AuxRec));
-    s.arrive_off = s.done_off + up(((size_t)w->npes + 1) * 4);
+    s.arrive_off = s.done_off + up(((size_t)count_domains(w, ops, nops) + 1) * 4);
     s.trace_off = s.arrive_off + up(s.nunits * 4);
     s.total = s.trace_off + TRACE_BYTES;
     return s;
@@ -557,7 +567,7 @@ extern "C" size_t shmemg_batch_plan_bytes(const shmemg_world_t *w, const shmemg_
     for (size_t i = 0; i < nops; ++i)
         if (shmemg_validate_op(w, ops_host[i])) return sizeof(PlanHeader);
     std::vector<Unit> units;
-    build_units(ops_host, nops, units);
+    build_units(w, ops_host, nops, units);
     return plan_sizes(w, ops_host, nops, units).total;
 }
 
@@ -574,7 +584,7 @@ extern "C" int shmemg_batch_create(shmemg_world_t *w, const shmemg_op_t *ops, si
         }
     }
     std::vector<Unit> units;
-    build_units(ops, nops, units);
+    build_units(w, ops, nops, units);
     const PlanSizes ps = plan_sizes(w, ops, nops, units);
     if (plan_bytes < ps.total) return SHMEMG_ERR_NOMEM;
     if (ps.ntiles >= 0xffffffffull || ps.nunits >= 0xffffffffull) return SHMEMG_ERR_NOMEM;
@@ -582,10 +592,11 @@ extern "C" int shmemg_batch_create(shmemg_world_t *w, const shmemg_op_t *ops, si
 
     // backward pass: which units does a LATER REAL unit depend on through a marker (or a wait)?
     std::vector<uint8_t> cnt(nu, 0);            // bit 0: count on done[initiator]; bit 1: count on done[npes]
-    std::vector<uint32_t> pe_total(w->npes, 0); // how far done[p] advances per launch
+    const int ndom = count_domains(w, ops, nops);
+    std::vector<uint32_t> pe_total(ndom, 0);    // how far done[domain] advances per launch
     uint32_t all_total = 0;
     {
-        std::vector<uint8_t> later_real(w->npes, 0), need(w->npes, 0);
+        std::vector<uint8_t> later_real(ndom, 0), need(ndom, 0);
         bool later_any = false, need_all = false;
         for (size_t i = nu; i-- > 0;) {
             const Unit &u = units[i];
@@ -610,7 +621,7 @@ extern "C" int shmemg_batch_create(shmemg_world_t *w, const shmemg_op_t *ops, si
     AuxRec *aux = reinterpret_cast<AuxRec *>(host.data() + ps.aux_off);
     hdr->ntiles = (uint32_t)ps.ntiles;
     hdr->nunits = (uint32_t)ps.nunits;
-    hdr->npes = (uint32_t)w->npes;
+    hdr->npes = (uint32_t)ndom;
     hdr->all_total = all_total;
     hdr->tiles_off = ps.tiles_off; hdr->aux_off = ps.aux_off; hdr->done_off = ps.done_off; hdr->arrive_off = ps.arrive_off;
     hdr->trace_off = ps.trace_off;
@@ -623,8 +634,8 @@ extern "C" int shmemg_batch_create(shmemg_world_t *w, const shmemg_op_t *ops, si
     // (wait_run[p]).  A wait must NOT get a weaker threshold than that: done[p] counts completions in any order, and
     // "done[p] >= issued-before-marker" means "everything before the marker is complete" only if nothing after the
     // marker can count before the marker's threshold is reached.
-    std::vector<uint32_t> issued(w->npes, 0), thresh(w->npes, 0);
-    std::vector<uint8_t> wait_run(w->npes, 0);
+    std::vector<uint32_t> issued(ndom, 0), thresh(ndom, 0);
+    std::vector<uint8_t> wait_run(ndom, 0);
     uint32_t all_issued = 0, all_thresh = 0, run_kind = 0;
     size_t k = 0, nt = 0, na = 0, run = 0;
     std::vector<Piece> pieces;
@@ -704,7 +715,7 @@ extern "C" int shmemg_batch_create(shmemg_world_t *w, const shmemg_op_t *ops, si
     b->ntiles = (uint32_t)ps.ntiles;
     const uint64_t maxgrid = (uint64_t)w->sm_count;
     b->grid = (uint32_t)(ps.ntiles < maxgrid ? (ps.ntiles ? ps.ntiles : 1) : maxgrid);
-    b->npes = (uint32_t)w->npes; b->all_total = all_total;
+    b->npes = (uint32_t)ndom; b->all_total = all_total;          // index of the all-domains counter in done[]
     b->tiles_off = ps.tiles_off; b->done_off = ps.done_off; b->arrive_off = ps.arrive_off; b->trace_off = ps.trace_off;
     b->trace_on = hdr->trace_on != 0;
     {

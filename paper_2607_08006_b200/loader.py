@@ -32,6 +32,7 @@ class Loaded:
         out["opcode"] = ops["kind"]            # neutral kinds 1..10 coincide with SHMEMG_OP_* by construction
         out["sig_op"] = ops["sig_op"]
         out["cmp"] = ops["cmp"]
+        out["ctx"] = ops["ctx"]
         out["initiator_pe"] = ops["initiator"]
         out["target_pe"] = ops["target"]
         out["rem_off"] = base[ops["rem_obj"]] + ops["rem_off"]

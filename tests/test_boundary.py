@@ -35,7 +35,7 @@ def test_descriptor_layout_matches_header():
     d = binding.OP_DTYPE
     assert d.itemsize == 64
     offs = {n: d.fields[n][1] for n in d.names}
-    assert offs == {"opcode": 0, "sig_op": 1, "cmp": 2, "reserved0": 3, "initiator_pe": 4, "target_pe": 8,
+    assert offs == {"opcode": 0, "sig_op": 1, "cmp": 2, "ctx": 3, "initiator_pe": 4, "target_pe": 8,
                     "reserved1": 12, "rem_off": 16, "loc_off": 24, "nbytes": 32, "value": 40, "cond": 48, "sig_off": 56}
     hdr = open(os.path.join(ROOT, "include", "shmemg.h")).read()
     for k, v in vars(binding.OP).items():

@@ -195,3 +195,57 @@ def test_bad_descriptors_are_rejected_on_the_host():
         with pytest.raises(ShmemgError) as e:
             w.batch(one(**kw))
         assert e.value.code == code, (kw, e.value)
+
+
+def test_context_field_is_validated_and_quiet_is_per_context():
+    """ctx >= SHMEMG_CTX_MAX is rejected; a QUIET on an unused context orders nothing but is legal."""
+    from workloads.spec import Program
+    w = World(2, 1 << 16, DEV)
+    a = w.malloc(4096)
+    ops = np.zeros(3, dtype=OP_DTYPE)
+    ops["opcode"] = [OP.PUT, OP.QUIET, OP.PUT]
+    ops["initiator_pe"] = [0, 0, 0]
+    ops["target_pe"] = [1, 0, 1]
+    ops["rem_off"] = [a, 0, a + 64]
+    ops["loc_off"] = [a + 128, 0, a + 256]
+    ops["nbytes"] = [64, 0, 64]
+    ops["ctx"] = [0, 7, 3]
+    w.view(a, 4096).copy_(torch.arange(4096, device=DEV).to(torch.uint8).repeat(2, 1))
+    b = w.batch(ops)
+    w.enqueue_batch(b)
+    w.quiet(0)
+    v = w.view(a, 4096).cpu().numpy()
+    assert np.array_equal(v[1, :64], v[0, 128:192]) and np.array_equal(v[1, 64:128], v[0, 256:320])
+    ops["ctx"][1] = 8
+    with pytest.raises(ShmemgError):
+        w.batch(ops)
+
+
+def test_quiet_on_one_context_does_not_depend_on_the_other():
+    """White-box check of the plan (tile records, 64 B each after the 256-byte header; dependency threshold at byte 52,
+    ordering domain at byte 48): the flag put behind QUIET(ctx 1) waits for ONE op (the small put of ctx 1) in domain
+    npes + pe, not for the four bulk puts of ctx 0; with everything on ctx 0 it waits for all five."""
+    w = World(4, 8 << 20, DEV)
+    a = w.malloc(6 << 20)
+
+    def plan(ctx_small):
+        ops = np.zeros(7, dtype=OP_DTYPE)
+        ops["opcode"] = [OP.PUT] * 4 + [OP.PUT, OP.QUIET, OP.PUT]
+        ops["initiator_pe"] = 2
+        ops["target_pe"] = 3
+        ops["rem_off"] = [a + (k << 20) for k in range(4)] + [a + (4 << 20), 0, a + (5 << 20)]
+        ops["loc_off"] = ops["rem_off"]
+        ops["nbytes"] = [1 << 20] * 4 + [256, 0, 8]
+        ops["ctx"] = [0] * 4 + [ctx_small] * 3
+        b = w.batch(ops)
+        raw = b.plan.cpu().numpy()
+        ntiles = int(raw[:4].view(np.uint32)[0])
+        recs = raw[256:256 + 64 * ntiles].reshape(ntiles, 64)
+        last = recs[-1]
+        return int(last[48:52].view(np.uint32)[0]), int(last[52:56].view(np.uint32)[0]), b
+
+    dom, dep, b = plan(1)
+    assert (dom, dep) == (4 + 2, 1)
+    w.enqueue_batch(b); w.quiet(0)
+    dom, dep, b = plan(0)
+    assert (dom, dep) == (2, 5)

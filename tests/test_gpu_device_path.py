@@ -35,8 +35,9 @@ def test_capabilities_distinguish_the_device_path():
     lambda: litmus.barrier_stamp(),
     lambda: litmus.barrier_stamp(npes=128, rounds=12),
     lambda: litmus.wait_after_wait(),
+    lambda: litmus.two_contexts(),
 ], ids=["mp_fence", "mp_fence_big", "mp_quiet3", "put_signal_sizes", "signal_add_fanin", "barrier_stamp",
-        "barrier_stamp128", "wait_after_wait"])
+        "barrier_stamp128", "wait_after_wait", "two_contexts"])
 def test_litmus_programs_device_initiated_match_oracle(make):
     prog = make()
     w, ld = run_gpu_device(prog)

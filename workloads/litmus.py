@@ -191,3 +191,33 @@ def wait_after_wait(npes: int = 4, groups: int = 6, chain: int = 24, nbytes: int
         prog.signal_wait_until(c, ("sig", g * 16 + 8), CMP_EQ, g + 1)
         prog.get(c, c, ("out2", g * 64), ("early", g * 64), 64)
     return prog
+
+
+def two_contexts(npes: int = 8, rounds: int = 10, big: int = 1 << 20, small: int = 4096, seed: int = 17) -> Program:
+    """Every PE drives two contexts.  Context 0: a bulk stream (PUT big -> neighbour; QUIET(ctx 0); PUT_SIGNAL flag0).
+    Context 1: a latency chain (PUT small -> other neighbour; QUIET(ctx 1); PUT flag1) issued between the bulk ops.  Consumers
+    wait on the flags (on the context that produced them) and copy the payloads.  The result is the same for every legal
+    schedule; an executor that lets a QUIET of one context order NOTHING (or that mixes the domains up) breaks it."""
+    prog = Program(npes)
+    prog.obj("src", rounds * (big + small), _payload(npes, rounds * (big + small), seed, 0))
+    prog.obj("flagsrc", rounds * 8, np.tile(np.arange(1, rounds + 1, dtype=np.uint64), (npes, 1)))
+    prog.obj("bulk", rounds * big)
+    prog.obj("chain", rounds * small)
+    prog.obj("flag0", rounds * 8)
+    prog.obj("flag1", rounds * 8)
+    prog.obj("out", rounds * (big + small))
+    for r in range(rounds):
+        for p in range(npes):
+            t0, t1 = (p + 1) % npes, (p + 3) % npes
+            prog.put(p, t0, ("bulk", r * big), ("src", r * (big + small)), big, ctx=0)
+            prog.put(p, t1, ("chain", r * small), ("src", r * (big + small) + big), small, ctx=1)
+            prog.quiet(p, ctx=1)
+            prog.put(p, t1, ("flag1", r * 8), ("flagsrc", r * 8), 8, ctx=1)
+            prog.quiet(p, ctx=0)
+            prog.put_signal(p, t0, ("flag0", r * 8), ("flagsrc", r * 8), 0, ("flag0", r * 8), r + 1, SIGNAL_SET, ctx=0)
+        for t in range(npes):
+            prog.signal_wait_until(t, ("flag1", r * 8), CMP_EQ, r + 1, ctx=1)
+            prog.get(t, t, ("out", r * (big + small) + big), ("chain", r * small), small, ctx=1)
+            prog.signal_wait_until(t, ("flag0", r * 8), CMP_EQ, r + 1, ctx=0)
+            prog.get(t, t, ("out", r * (big + small)), ("bulk", r * big), big, ctx=0)
+    return prog

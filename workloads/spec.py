@@ -25,7 +25,7 @@ CMP_EQ, CMP_NE, CMP_GT, CMP_GE, CMP_LT, CMP_LE = range(6)
 NOBJ = -1
 
 OP_DTYPE = np.dtype([
-    ("kind", "u1"), ("sig_op", "u1"), ("cmp", "u1"), ("_pad", "u1"),
+    ("kind", "u1"), ("sig_op", "u1"), ("cmp", "u1"), ("ctx", "u1"),
     ("initiator", "i4"), ("target", "i4"),
     ("rem_obj", "i4"), ("loc_obj", "i4"), ("sig_obj", "i4"),
     ("rem_off", "u8"), ("loc_off", "u8"), ("nbytes", "u8"),
@@ -62,41 +62,41 @@ class Program:
 
     # ---- ops -----------------------------------------------------------------------------
     def _add(self, kind, initiator, target=0, rem=(NOBJ, 0), loc=(NOBJ, 0), nbytes=0, value=0, cond=0,
-             sig=(NOBJ, 0), sig_op=0, cmp=0):
+             sig=(NOBJ, 0), sig_op=0, cmp=0, ctx=0):
         def o(x):
             return (self.oid(x[0]) if isinstance(x[0], str) else int(x[0]), int(x[1]))
         rem, loc, sig = o(rem), o(loc), o(sig)
-        self._ops.append((kind, sig_op, cmp, 0, initiator, target, rem[0], loc[0], sig[0],
+        self._ops.append((kind, sig_op, cmp, ctx, initiator, target, rem[0], loc[0], sig[0],
                           rem[1], loc[1], nbytes, value & U64, cond & U64, sig[1]))
         self._arr = None
 
-    def put(self, pe, target, dst, src, nbytes):
-        self._add(PUT, pe, target, rem=dst, loc=src, nbytes=nbytes)
+    def put(self, pe, target, dst, src, nbytes, ctx=0):
+        self._add(PUT, pe, target, rem=dst, loc=src, nbytes=nbytes, ctx=ctx)
 
-    def get(self, pe, target, dst, src, nbytes):
-        self._add(GET, pe, target, rem=src, loc=dst, nbytes=nbytes)
+    def get(self, pe, target, dst, src, nbytes, ctx=0):
+        self._add(GET, pe, target, rem=src, loc=dst, nbytes=nbytes, ctx=ctx)
 
-    def put_signal(self, pe, target, dst, src, nbytes, sig, sig_value, sig_op=SIGNAL_SET):
+    def put_signal(self, pe, target, dst, src, nbytes, sig, sig_value, sig_op=SIGNAL_SET, ctx=0):
         self._add(PUT_SIGNAL, pe, target, rem=dst, loc=src, nbytes=nbytes, sig=sig, value=sig_value,
-                  sig_op=sig_op)
+                  sig_op=sig_op, ctx=ctx)
 
-    def atomic_add(self, pe, target, dst, value):
-        self._add(ATOMIC_ADD, pe, target, rem=dst, value=value, nbytes=8)
+    def atomic_add(self, pe, target, dst, value, ctx=0):
+        self._add(ATOMIC_ADD, pe, target, rem=dst, value=value, nbytes=8, ctx=ctx)
 
-    def atomic_fetch_add(self, pe, target, dst, value, fetch):
-        self._add(ATOMIC_FETCH_ADD, pe, target, rem=dst, loc=fetch, value=value, nbytes=8)
+    def atomic_fetch_add(self, pe, target, dst, value, fetch, ctx=0):
+        self._add(ATOMIC_FETCH_ADD, pe, target, rem=dst, loc=fetch, value=value, nbytes=8, ctx=ctx)
 
-    def atomic_compare_swap(self, pe, target, dst, cond, value, fetch):
-        self._add(ATOMIC_COMPARE_SWAP, pe, target, rem=dst, loc=fetch, value=value, cond=cond, nbytes=8)
+    def atomic_compare_swap(self, pe, target, dst, cond, value, fetch, ctx=0):
+        self._add(ATOMIC_COMPARE_SWAP, pe, target, rem=dst, loc=fetch, value=value, cond=cond, nbytes=8, ctx=ctx)
 
-    def signal_wait_until(self, pe, sig, cmp, value):
-        self._add(SIGNAL_WAIT_UNTIL, pe, pe, loc=sig, cmp=cmp, value=value)
+    def signal_wait_until(self, pe, sig, cmp, value, ctx=0):
+        self._add(SIGNAL_WAIT_UNTIL, pe, pe, loc=sig, cmp=cmp, value=value, ctx=ctx)
 
-    def fence(self, pe):
-        self._add(FENCE, pe, pe)
+    def fence(self, pe, ctx=0):
+        self._add(FENCE, pe, pe, ctx=ctx)
 
-    def quiet(self, pe):
-        self._add(QUIET, pe, pe)
+    def quiet(self, pe, ctx=0):
+        self._add(QUIET, pe, pe, ctx=ctx)
 
     def barrier_all(self):
         self._add(BARRIER_ALL, 0, 0)
