@@ -60,6 +60,8 @@ def lib():
         L.orc_amo_batch.argtypes = [vp, i, u64, i, i, u64, vp, vp, vp, vp, u64]
         L.orc_ibput.argtypes = [vp, i, u64, u64, u64, u64, u64, u64, u64, i, i, i]
         L.orc_signal_test.argtypes = [vp, i, u64, u64, i, u64, i]
+        L.orc_signal_test_vec.argtypes = [vp, i, u64, u64, u64, i, u64, i, vp]
+        L.orc_signal_test_vec.restype = C.c_int64
         L.orc_team_fcollect.argtypes = [vp, i, u64, i, i, i, u64, u64, u64]
         L.orc_team_alltoall.argtypes = [vp, i, u64, i, i, i, u64, u64, u64]
         L.orc_team_broadcast.argtypes = [vp, i, u64, i, i, i, u64, u64, u64, i]
@@ -230,6 +232,16 @@ class OracleWorld:
     def ibget(self, dst_off, src_off, dst_stride, src_stride, block, nblocks, pe, target):
         _chk(lib().orc_ibput(self.heap.ctypes.data, self.npes, self.heap_bytes, dst_off, src_off, dst_stride,
                              src_stride, block, nblocks, pe, target, 1), "ibget")
+
+    def signal_test_vec(self, sig_off, nelems, cmp, value, pe) -> np.ndarray:
+        """Ascending positions k < nelems with cmp(u64 heap[pe][sig_off + 8k], value): test_some; all = (len == nelems);
+        any = the first entry."""
+        idx = np.empty(max(nelems, 1), dtype=np.uint64)
+        n = lib().orc_signal_test_vec(self.heap.ctypes.data, self.npes, self.heap_bytes, sig_off, nelems, cmp, value, pe,
+                                      idx.ctypes.data)
+        if n < 0:
+            raise OracleError("signal_test_vec: bad argument")
+        return idx[:n].copy()
 
     # ---- NEXT-3: collectives over a strided team (start, stride, size); ranks are team-relative ----
     def team_fcollect(self, team, dst_off, src_off, nbytes):

@@ -382,6 +382,23 @@ int orc_signal_test(const uint8_t *heap, int npes, uint64_t heap_bytes, uint64_t
     }
 }
 
+/* vector forms of test (OpenSHMEM 1.6 test_all / test_any / test_some on nelems consecutive u64 words; L392): evaluated on
+ * the current state, never block.  `indices` (may be NULL) receives the satisfied positions in ascending order; the return
+ * value is their number, or -1 on a bad argument.  all: count == nelems; any: count > 0, the reported index is indices[0]
+ * (the LOWEST satisfied position); some: the whole list.  The wait_until_* forms are the same predicates required to hold
+ * (in a sequential schedule a wait must already be satisfied at its turn). */
+int64_t orc_signal_test_vec(const uint8_t *heap, int npes, uint64_t heap_bytes, uint64_t sig_off, uint64_t nelems, int cmp,
+                            uint64_t value, int pe, uint64_t *indices) {
+    if (pe < 0 || pe >= npes || (sig_off & 7) || !in_range(sig_off, 8 * nelems, heap_bytes)) return -1;
+    int64_t cnt = 0;
+    for (uint64_t k = 0; k < nelems; ++k) {
+        const int r = orc_signal_test(heap, npes, heap_bytes, sig_off + 8 * k, cmp, value, pe);
+        if (r < 0) return -1;
+        if (r) { if (indices) indices[cnt] = k; ++cnt; }
+    }
+    return cnt;
+}
+
 /* ---- team collectives ("PE collectives remain collective over a team of
  * PEs").  A team is the strided PE set { start + k*stride : 0 <= k < size } (shmem_team_split_strided); team rank k is that
  * PE.  Each collective is the world definition with "all PEs" replaced by "all team members, in team-rank order"; heaps of

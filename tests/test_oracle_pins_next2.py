@@ -270,3 +270,21 @@ def test_sum_of_negative_zeros_is_positive_zero_in_both_sum_routines():
     assert w.view(64, 8, np.uint32).tolist() == [[0x80000000] * 2] * 3
     w.reduce("prod", "f32", 64, 0, 2)                    # (-0)(-0)(-0) = -0
     assert w.view(64, 8, np.uint32).tolist() == [[0x80000000] * 2] * 3
+
+
+def test_signal_test_vec_equals_numpy_flatnonzero():
+    from workloads.spec import CMP_EQ, CMP_GE, CMP_GT, CMP_LE, CMP_LT, CMP_NE
+    w = orc.OracleWorld(3, 4096)
+    vals = (gen.u64(3 * 100, 241) % np.uint64(7)).reshape(3, 100)
+    w.view(256, 800, np.uint64)[:] = vals
+    ops = {CMP_EQ: np.equal, CMP_NE: np.not_equal, CMP_GT: np.greater, CMP_GE: np.greater_equal, CMP_LT: np.less, CMP_LE: np.less_equal}
+    for cmp, f in ops.items():
+        for v in (0, 3, 6, 7):
+            for pe in range(3):
+                got = w.signal_test_vec(256 + 8 * 5, 90, cmp, v, pe)
+                assert np.array_equal(got, np.flatnonzero(f(vals[pe, 5:95], np.uint64(v))))
+    assert len(w.signal_test_vec(256, 0, CMP_EQ, 0, 0)) == 0
+    with pytest.raises(orc.OracleError):
+        w.signal_test_vec(260, 4, CMP_EQ, 0, 0)
+    with pytest.raises(orc.OracleError):
+        w.signal_test_vec(256, 4, CMP_EQ, 0, 3)
