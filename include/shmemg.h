@@ -272,6 +272,21 @@ SHMEMG_API int shmemg_ibget_on_stream(shmemg_world_t *w, uint64_t dest_off, uint
                                       uint64_t src_stride, size_t block_bytes, size_t nblocks, int pe, int target_pe,
                                       void *stream);
 
+/* Vector forms on `nelems` consecutive u64 words of `pe`'s window starting at sig_off (OpenSHMEM 1.6 test_all / any / some and
+ * wait_until_all / any / some).  The satisfied positions (ascending) go to indices_dev[0 .. count) and their
+ * number to *count_dev (DEVICE uint64 arrays of nelems and 1 entries; either may be NULL), valid when the stream has passed the
+ * call.  test_vec never blocks: all = (count == nelems), any = (count > 0, indices_dev[0] the lowest), some = the list.
+ * wait_until_all blocks the stream until every word satisfies; wait_until_some (= wait_until_any: take indices_dev[0]) until
+ * at least one does and reports those that do at that moment.  A satisfied word is an acquire.  Same prohibited stream
+ * patterns as signal_wait_until_on_stream. */
+SHMEMG_API int shmemg_signal_test_vec_on_stream(shmemg_world_t *w, uint64_t sig_off, size_t nelems, int cmp, uint64_t value,
+                                                int pe, uint64_t *indices_dev, uint64_t *count_dev, void *stream);
+SHMEMG_API int shmemg_signal_wait_until_all_on_stream(shmemg_world_t *w, uint64_t sig_off, size_t nelems, int cmp,
+                                                      uint64_t value, int pe, void *stream);
+SHMEMG_API int shmemg_signal_wait_until_some_on_stream(shmemg_world_t *w, uint64_t sig_off, size_t nelems, int cmp,
+                                                       uint64_t value, int pe, uint64_t *indices_dev, uint64_t *count_dev,
+                                                       void *stream);
+
 /* ---- teams ("PE collectives remain collective over a team of PEs", L357, L412) --------
  * shmemg_team_split_strided: the PEs { start + k*stride : k < size } of `parent_team` (ranks of the parent; the three
  * predefined teams are the world) form a new team; *new_team receives its handle (>= SHMEMG_TEAM_USER0).  Team rank k is the

@@ -126,6 +126,9 @@ SYMBOLS = {
     "shmemg_ibput_on_stream": (_i, [_vp, _u64, _u64, _u64, _u64, _sz, _sz, _i, _i, _vp]),
     "shmemg_ibget_on_stream": (_i, [_vp, _u64, _u64, _u64, _u64, _sz, _sz, _i, _i, _vp]),
     "shmemg_signal_test_on_stream": (_i, [_vp, _u64, _i, _u64, _i, _vp, _vp]),
+    "shmemg_signal_test_vec_on_stream": (_i, [_vp, _u64, _sz, _i, _u64, _i, _vp, _vp, _vp]),
+    "shmemg_signal_wait_until_all_on_stream": (_i, [_vp, _u64, _sz, _i, _u64, _i, _vp]),
+    "shmemg_signal_wait_until_some_on_stream": (_i, [_vp, _u64, _sz, _i, _u64, _i, _vp, _vp, _vp]),
     "shmemg_fcollect_on_stream": (_i, [_vp, _u64, _u64, _sz, _vp]),
     "shmemg_team_split_strided": (_i, [_vp, _i, _i, _i, _i, C.POINTER(_i)]),
     "shmemg_team_n_pes": (_i, [_vp, _i]),
@@ -445,6 +448,23 @@ class World:
         self._chk(lib().shmemg_team_broadcast_on_stream(self.h, team, dest_off, source_off, nbytes, root_rank, _stream(stream)),
                   "shmemg_team_broadcast_on_stream")
         self.launches += 1 if nbytes else 0
+
+    def signal_test_vec(self, sig_off, nelems, cmp, value, pe, indices_dev=None, count_dev=None, stream=None):
+        self._chk(lib().shmemg_signal_test_vec_on_stream(self.h, sig_off, nelems, cmp, value & ((1 << 64) - 1), pe,
+                                                         _dptr(indices_dev), _dptr(count_dev), _stream(stream)),
+                  "shmemg_signal_test_vec_on_stream")
+        self.launches += 1
+
+    def signal_wait_until_all(self, sig_off, nelems, cmp, value, pe, stream=None):
+        self._chk(lib().shmemg_signal_wait_until_all_on_stream(self.h, sig_off, nelems, cmp, value & ((1 << 64) - 1), pe,
+                                                               _stream(stream)), "shmemg_signal_wait_until_all_on_stream")
+        self.launches += 1
+
+    def signal_wait_until_some(self, sig_off, nelems, cmp, value, pe, indices_dev=None, count_dev=None, stream=None):
+        self._chk(lib().shmemg_signal_wait_until_some_on_stream(self.h, sig_off, nelems, cmp, value & ((1 << 64) - 1), pe,
+                                                                _dptr(indices_dev), _dptr(count_dev), _stream(stream)),
+                  "shmemg_signal_wait_until_some_on_stream")
+        self.launches += 1
 
     def fcollect(self, dest_off, source_off, nbytes, stream=None):
         self._chk(lib().shmemg_fcollect_on_stream(self.h, dest_off, source_off, nbytes, _stream(stream)),

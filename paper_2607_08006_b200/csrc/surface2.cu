@@ -372,3 +372,55 @@ extern "C" int shmemg_team_broadcast_on_stream(shmemg_world_t *w, int team, uint
                                                size_t nbytes, int root_rank, void *stream) {
     TEAM_CALL(shmemg_broadcast_on_stream(w, dest_off, source_off, nbytes, root_rank, stream))
 }
+
+// ---- vector test / wait (OpenSHMEM 1.6 test_all / any / some and wait_until_all / any / some) -----------------
+// One block; thread t looks at words t, t + 256, ...  `wait`: the block polls until the mode's condition holds (all words /
+// at least one word).  Then thread 0 lists the satisfied positions in ascending order (at least the ones that made the
+// condition true; a word that becomes true in between is a legitimate member too) into indices_dev and their number into
+// count_dev (either may be NULL).  A satisfied result is an acquire.
+__global__ void __launch_bounds__(256) k_signal_vec(const unsigned long long *sig, size_t nelems, int cmp, unsigned long long value,
+                                                    int need_all, int wait, unsigned long long *indices, unsigned long long *count) {
+    for (;;) {
+        int ok_all = 1, ok_any = 0;
+        for (size_t k = threadIdx.x; k < nelems; k += blockDim.x) {
+            const bool ok = cmp_u64(cmp, ld_relaxed_u64(sig + k), value);
+            ok_all &= ok; ok_any |= ok;
+        }
+        const int all = __syncthreads_and(ok_all), any = __syncthreads_or(ok_any);
+        if (!wait || nelems == 0 || (need_all ? all : any)) break;
+        __nanosleep(64);
+    }
+    fence_acquire();
+    if (threadIdx.x == 0) {
+        unsigned long long n = 0;
+        for (size_t k = 0; k < nelems; ++k)
+            if (cmp_u64(cmp, ld_relaxed_u64(sig + k), value)) { if (indices) indices[n] = k; ++n; }
+        fence_acquire();
+        if (count) *count = n;
+    }
+}
+
+static int signal_vec(shmemg_world_t *w, uint64_t sig_off, size_t nelems, int cmp, uint64_t value, int pe, int need_all, int wait,
+                      uint64_t *indices_dev, uint64_t *count_dev, void *stream) {
+    if (!w || cmp < SHMEMG_CMP_EQ || cmp > SHMEMG_CMP_LE) return SHMEMG_ERR_ARG;
+    if (!shmemg_pe_ok(w, pe)) return SHMEMG_ERR_PE;
+    if (nelems > (SIZE_MAX >> 3) || !shmemg_in_range(w, sig_off, 8 * (uint64_t)nelems)) return SHMEMG_ERR_RANGE;
+    if (sig_off & 7) return SHMEMG_ERR_ALIGN;
+    k_signal_vec<<<1, 256, 0, (cudaStream_t)stream>>>(reinterpret_cast<const unsigned long long *>(shmemg_addr(w, pe, sig_off)), nelems,
+                                                     cmp, value, need_all, wait, (unsigned long long *)indices_dev,
+                                                     (unsigned long long *)count_dev);
+    SHMEMG_CUDA(w, cudaGetLastError());
+    return SHMEMG_OK;
+}
+extern "C" int shmemg_signal_test_vec_on_stream(shmemg_world_t *w, uint64_t sig_off, size_t nelems, int cmp, uint64_t value, int pe,
+                                                uint64_t *indices_dev, uint64_t *count_dev, void *stream) {
+    return signal_vec(w, sig_off, nelems, cmp, value, pe, 0, 0, indices_dev, count_dev, stream);
+}
+extern "C" int shmemg_signal_wait_until_all_on_stream(shmemg_world_t *w, uint64_t sig_off, size_t nelems, int cmp, uint64_t value,
+                                                      int pe, void *stream) {
+    return signal_vec(w, sig_off, nelems, cmp, value, pe, 1, 1, nullptr, nullptr, stream);
+}
+extern "C" int shmemg_signal_wait_until_some_on_stream(shmemg_world_t *w, uint64_t sig_off, size_t nelems, int cmp, uint64_t value,
+                                                       int pe, uint64_t *indices_dev, uint64_t *count_dev, void *stream) {
+    return signal_vec(w, sig_off, nelems, cmp, value, pe, 0, 1, indices_dev, count_dev, stream);
+}

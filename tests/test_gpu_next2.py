@@ -355,3 +355,37 @@ def test_reduce_signed_zero_corner_matches_oracle():
             assert np.array_equal(g[:, :4], o[:, :4]) and (g[:, 4:] & 0x7fffffff == 0).all()
         else:
             assert np.array_equal(g, o), op
+
+
+# ---- vector test / wait ------------------------------------------------------------------------------------------------
+def test_vector_test_and_wait_forms_match_oracle():
+    npes, n = 3, 700
+    w, ow = pair(npes, 1 << 16)
+    sig, osig = w.calloc(n, 8), ow.malloc(n * 8)
+    vals = (gen.u64(npes * n, 371) % np.uint64(5)).reshape(npes, n)
+    w.view(sig, n * 8, torch.int64).copy_(torch.from_numpy(vals.view(np.int64)))
+    ow.view(osig, n * 8, np.uint64)[:] = vals
+    idx = torch.full((n,), -1, dtype=torch.int64, device=DEV)
+    cnt = torch.full((1,), -1, dtype=torch.int64, device=DEV)
+    for cmp in (CMP.EQ, CMP.NE, CMP.GT, CMP.GE, CMP.LT, CMP.LE):
+        for v, pe, off, m in ((2, 0, 0, n), (0, 1, 8 * 3, n - 7), (4, 2, 8 * 100, 257), (9, 1, 0, 1), (1, 0, 8, 0)):
+            w.signal_test_vec(sig + off, m, cmp, v, pe, idx, cnt)
+            w.quiet(0)
+            exp = ow.signal_test_vec(osig + off, m, cmp, v, pe)
+            assert cnt.item() == len(exp) and np.array_equal(idx.cpu().numpy()[:len(exp)].view(np.uint64), exp), (cmp, v, pe)
+    # wait_until_all on words that a put_signal chain sets one by one (stream order makes them all true before the wait)
+    data = w.malloc(4096)
+    w.view(sig, n * 8).zero_()
+    for k in range(6):
+        w.put_signal(data, data, 64, sig + 8 * k, k + 1, SIGNAL.SET, 0, 2)
+    w.signal_wait_until_all(sig, 6, CMP.GE, 1, 2)
+    w.signal_wait_until_some(sig, 10, CMP.GE, 4, 2, idx, cnt)
+    w.quiet(0)
+    ow.view(osig, n * 8, np.uint64)[:] = 0
+    ow.view(osig, n * 8, np.uint64)[2, :6] = np.arange(1, 7)
+    exp = ow.signal_test_vec(osig, 10, CMP.GE, 4, 2)
+    assert cnt.item() == 3 and np.array_equal(idx.cpu().numpy()[:3].view(np.uint64), exp) and exp.tolist() == [3, 4, 5]
+    with pytest.raises(ShmemgError):
+        w.signal_test_vec(sig + 4, 2, CMP.EQ, 0, 0)
+    with pytest.raises(ShmemgError):
+        w.signal_wait_until_all(sig, 1 << 40, CMP.EQ, 0, 0)
