@@ -406,3 +406,18 @@ def test_c2_halo_full_size_rounds():
     assert np.array_equal(ld.obj_numpy("U", np.float64), ow.obj("U", np.float64))
     for a, b in zip(lg, lo):
         assert np.array_equal(a, b)
+
+
+def test_c1_final_array_matches_the_stored_oracle_checksum():
+    """tests/golden/oracle_checksums.txt is written from the oracle alone; the CUDA path must land on the same bytes."""
+    import hashlib
+    import os
+    stored = dict(ln.split() for ln in open(os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden",
+                                                         "oracle_checksums.txt")) if ln.strip() and ln[0] != "#")
+    wl = configs.c1_atomic_add()
+    w = World(wl.npes, wl.nelem * 8 + 4096, DEV)
+    a = w.calloc(wl.nelem, 8)
+    w.atomic_add_batch(a, to_dev(wl.tgt_pe), to_dev(wl.idx.astype(np.int64)), val=to_dev(wl.val))
+    w.quiet(0); w.barrier_all()
+    got = hashlib.sha256(w.view(a, wl.nelem * 8).cpu().numpy().tobytes()).hexdigest()[:32]
+    assert got == stored["c1_atomic_add_full"]
