@@ -502,6 +502,25 @@ static uint32_t pick_seg_tiles(const shmemg_world *w, const shmemg_op_t *ops, si
     return per_sm < 1 ? 1u : (uint32_t)per_sm;
 }
 
+// Per-op segment length.  Streaming batches: tickets are claimed in batch order, so whoever claims a 256 KiB segment last
+// works alone for microseconds while the other SMs idle; the copy ops that start within the last `sm_count * 8` planner
+// tiles (37 MB) of a streaming batch are therefore cut into 64 KiB segments (C3b 71.2 -> 68.6 us).
+#define SEG_TILES_TAIL 2u
+static void seg_tiles_per_op(const shmemg_world *w, const shmemg_op_t *ops, size_t nops, std::vector<uint32_t> &seg) {
+    const uint32_t base = pick_seg_tiles(w, ops, nops);
+    seg.assign(nops, base);
+    if (base < SEG_TILES_MAX) return;
+    uint64_t tiles = 0;
+    const uint64_t tail = (uint64_t)w->sm_count * 8;      // measured on C3b: (8, 2) 68.6 us; (8, 1) 69.6; (16, 2) 69.1; (32, 2) 70.7; none 71.2
+    const uint32_t tseg = SEG_TILES_TAIL;
+    for (size_t i = nops; i-- > 0;) {
+        if (ops[i].opcode < SHMEMG_OP_PUT || ops[i].opcode > SHMEMG_OP_PUT_SIGNAL) continue;
+        if (tiles >= tail) break;
+        seg[i] = tseg;
+        tiles += (ops[i].nbytes + SHMEMG_TMA_TILE - 1) / SHMEMG_TMA_TILE;
+    }
+}
+
 // ---- planning units: one per op (a marker, a copy op, an AMO, a wait) -------------------------------------------------
 struct Unit { uint8_t opc; int pe; size_t first, count; };    // [first, first+count) in the caller's op array
 
@@ -534,7 +553,8 @@ static PlanSizes plan_sizes(const shmemg_world *w, const shmemg_op_t *ops, size_
     size_t run = 0;
     uint32_t run_kind = 0;
     std::vector<Piece> pieces;
-    const uint32_t seg_tiles = pick_seg_tiles(w, ops, nops);
+    std::vector<uint32_t> seg_tiles;
+    seg_tiles_per_op(w, ops, nops, seg_tiles);
     for (const Unit &u : units) {
         if (is_marker(u.opc)) { run = 0; continue; }
         s.nunits++;
@@ -548,7 +568,7 @@ static PlanSizes plan_sizes(const shmemg_world *w, const shmemg_op_t *ops, size_
         run = 0;
         uint64_t dst, src;
         copy_endpoints(w, ops[u.first], dst, src);
-        cut_copy(dst, src, ops[u.first].nbytes, seg_tiles, pieces);
+        cut_copy(dst, src, ops[u.first].nbytes, seg_tiles[u.first], pieces);
         s.ntiles += pieces.size();
     }
     auto up = [](size_t x) { return (x + 255) / 256 * 256; };
@@ -639,7 +659,8 @@ extern "C" int shmemg_batch_create(shmemg_world_t *w, const shmemg_op_t *ops, si
     uint32_t all_issued = 0, all_thresh = 0, run_kind = 0;
     size_t k = 0, nt = 0, na = 0, run = 0;
     std::vector<Piece> pieces;
-    const uint32_t seg_tiles = pick_seg_tiles(w, ops, nops);
+    std::vector<uint32_t> seg_tiles;
+    seg_tiles_per_op(w, ops, nops, seg_tiles);
     auto aux_dev = [&](size_t idx) { return (uint64_t)((uint8_t *)plan_dev + ps.aux_off + idx * sizeof(AuxRec)); };
     for (size_t ui = 0; ui < nu; ++ui) {
         const Unit &u = units[ui];
@@ -683,7 +704,7 @@ extern "C" int shmemg_batch_create(shmemg_world_t *w, const shmemg_op_t *ops, si
             run = 0;
             uint64_t dst, src;
             copy_endpoints(w, o, dst, src);
-            cut_copy(dst, src, o.nbytes, seg_tiles, pieces);
+            cut_copy(dst, src, o.nbytes, seg_tiles[u.first], pieces);
             uint32_t f = flags | ((dep_pe | dep_all) ? TF_DEPS : 0);
             uint64_t sig = 0;
             if (u.opc == SHMEMG_OP_PUT_SIGNAL) {
