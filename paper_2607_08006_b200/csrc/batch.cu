@@ -478,11 +478,10 @@ static void cut_copy(uint64_t dst, uint64_t src, uint64_t n, uint32_t seg_tiles,
         // balanced segments of at most seg_tiles bulk tiles
         const uint64_t tiles = (body + SHMEMG_TMA_TILE - 1) / SHMEMG_TMA_TILE;
         const uint64_t nseg = (tiles + seg_tiles - 1) / seg_tiles;
-        for (uint64_t g = 0, t0 = 0; g < nseg; ++g) {
-            const uint64_t t1 = (g + 1) * tiles / nseg;
-            const uint64_t b0 = t0 * SHMEMG_TMA_TILE, b1 = t1 * SHMEMG_TMA_TILE < body ? t1 * SHMEMG_TMA_TILE : body;
-            out.push_back({T_TMA, head + b0, (uint32_t)(b1 - b0)});
-            t0 = t1;
+        for (uint64_t g = 0, b0 = 0; g < nseg; ++g) {            // equal byte shares, cut at 1 KiB (the executor re-tiles a segment)
+            const uint64_t b1 = g + 1 == nseg ? body : ((g + 1) * body / nseg) & ~1023ull;
+            if (b1 > b0) out.push_back({T_TMA, head + b0, (uint32_t)(b1 - b0)});
+            b0 = b1;
         }
         if (tail) out.push_back({T_COPY, head + body, (uint32_t)tail});
         return;
