@@ -45,17 +45,23 @@ HALO_ROUNDS = 50
 BARRIERS = 10000
 M64 = (1 << 64) - 1
 
-# dram__bytes_read.sum + dram__bytes_write.sum per launch of each copy-class segment's kernel, from the `ncu --set full`
-# captures summarised in profiles/r01c_ncu_full.md (cold L2 at launch, up to 126 MB of the kernel's own writes still in
-# L2 at its end, so write traffic < algorithmic writes; the halo faces are L2-resident by nature).
-NCU_TRAFFIC = {
-    "alltoall": 268450304 + 221164032,
-    "put_batch_skewed": 198646272 + 151099392,
-    "halo_put_signal_wait": 25210368 + 143872,
-    "sum_reduce_f32": 536884224 + 478725888,
-    "sum_reduce_i64": 536912896 + 479576576,
-    "fcollect": 4208640 + 476806656,
-}
+def ncu_traffic():
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch of each copy-class segment's kernel, from the committed
+    `ncu --set full` capture summarised in profiles/ (TRAFFIC_CSV; the .md beside it names the command).  Cold L2 at launch,
+    up to 126 MB of the kernel's own writes still in L2 at its end, so write traffic < algorithmic writes; the halo faces are
+    L2-resident by nature."""
+    out = {}
+    try:
+        for ln in open(os.path.join(ROOT, "profiles", TRAFFIC_CSV)):
+            f = [x.strip() for x in ln.split(",")]
+            if len(f) >= 4 and f[0] and f[0] != "segment" and not f[0].startswith("#"):
+                out[f[0]] = int(f[2]) + int(f[3])
+    except OSError:
+        pass
+    return out
+
+
+TRAFFIC_CSV = "r02_traffic.csv"
 
 
 def parse_args():
@@ -65,7 +71,8 @@ def parse_args():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
     ap.add_argument("--no-e2e", action="store_true", help="skip the end-to-end (host buffers) leg")
-    ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
+    ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg (and the verification against the oracle)")
+    ap.add_argument("--no-verify", action="store_true", help="skip the comparison of every segment's results with the oracle")
     ap.add_argument("--small", action="store_true", help="reduced sizes (development only; marked in the JSON)")
     ap.add_argument("--only", default="", help="comma-separated segment groups to run: c1,c2,c3a,c3b,c4,c5,barrier,next2")
     return ap.parse_args()
@@ -168,6 +175,13 @@ def segment_table(inp: Inputs):
     if "c2" in g:
         seg["halo_put_signal_wait"] = dict(cls="copy", kernel="k_batch_exec",
                                            bytes=HALO_ROUNDS * 2 * 48 * inp.halo.face_bytes, launches=HALO_ROUNDS)
+    # the ONE-CALL form of the two batch workloads (shmemg_enqueue_batch: device-resident descriptors planned on the device
+    # inside the timed segment, 2 launches); reported beside the pre-planned form, not part of `value`
+    if "c3b" in g:
+        seg["put_batch_skewed_onecall"] = dict(cls="xcopy", kernel="k_plan_batch + k_batch_exec", bytes=2 * int(inp.c3b.sizes.sum()), launches=1)
+    if "c2" in g:
+        seg["halo_put_signal_wait_onecall"] = dict(cls="xcopy", kernel="k_plan_batch + k_batch_exec",
+                                                   bytes=HALO_ROUNDS * 2 * 48 * inp.halo.face_bytes, launches=HALO_ROUNDS)
     if "c5" in g:
         n, nb = inp.c5_npes, inp.c5_bytes
         seg["sum_reduce_f32"] = dict(cls="copy", kernel="k_sum_reduce_tma<f32>", bytes=2 * n * nb, launches=1)
@@ -175,11 +189,13 @@ def segment_table(inp: Inputs):
         seg["fcollect"] = dict(cls="copy", kernel="k_fcollect_tma",
                                bytes=n * inp.c5_fc_bytes + n * n * inp.c5_fc_bytes, launches=1)
     if "c1" in g:
-        seg["atomic_add"] = dict(cls="amo", kernel="k_amo<add>", ops=len(inp.c1.val), launches=2)   # + barrier kernel
+        # operand / result streams per op (what HBM must move): C1 tgt_pe 4 + idx 8 + val 8
+        seg["atomic_add"] = dict(cls="amo", kernel="k_amo<add>", ops=len(inp.c1.val), launches=2, bytes_per_op=20)   # + barrier kernel
     if "c4" in g:
         E = len(inp.c4.u)
-        seg["atomic_fetch_add"] = dict(cls="amo", kernel="k_hot_sample + k_amo_hot_main<fetch_add>", ops=E, launches=2)
-        seg["atomic_compare_swap"] = dict(cls="amo", kernel="k_amo<compare_swap>", ops=E, launches=1)
+        # fetch-add: tgt_pe 4 + idx 4 read, 8 fetched written; compare-swap: tgt_pe 4 + idx 4 + val 8 read, 8 fetched written
+        seg["atomic_fetch_add"] = dict(cls="amo", kernel="k_hot_sample + k_amo_hot_main<fetch_add>", ops=E, launches=2, bytes_per_op=16)
+        seg["atomic_compare_swap"] = dict(cls="amo", kernel="k_amo<compare_swap>", ops=E, launches=1, bytes_per_op=24)
     if "next2" in g:
         # NEXT-2 surface; reported per segment, NOT part of `value` / `amo_mops` (cls x*)
         if "c5" in g:
@@ -254,6 +270,7 @@ class CudaBench:
         self.torch, self.inp, self.dev = torch, inp, device
         self.rec = Recorder(torch)
         self.app_launches = 0
+        self.plan_us = {}                              # host planning cost of the pre-planned batches (outside every timed region)
         self.barrier_graph = None
         self.worlds = []
         self.flags = 0                                 # warp aggregation buys nothing on these streams (profiles/)
@@ -273,7 +290,13 @@ class CudaBench:
             hb = sum((x + 255) // 256 * 256 for x in prog.obj_bytes) + 4096
             w = World(prog.npes, hb, device)
             self.w3b, self.ld3b = w, Loaded(w, prog)
-            self.b3b = w.batch(self.ld3b.translate(prog))
+            ops = self.ld3b.translate(prog)
+            t0 = time.perf_counter()
+            self.b3b = w.batch(ops)                                   # shmemg_batch_plan_bytes + shmemg_batch_create (ends in a stream sync)
+            self.plan_us["put_batch_skewed"] = {"nops": len(ops), "host_plan_us": (time.perf_counter() - t0) * 1e6}
+            self.ops3b_host = torch.from_numpy(ops.view(np.uint8).reshape(-1).copy()).pin_memory()
+            self.ops3b_dev = self.ops3b_host.to(device)
+            self.work3b = torch.empty(w.batch_work_bytes(len(ops), int(inp.c3b.sizes.sum())), dtype=torch.uint8, device=device)
             self.worlds.append(w)
         if "c2" in g:
             h = inp.halo
@@ -284,7 +307,16 @@ class CudaBench:
             self.U_off = w.malloc(h.B ** 3 * 8)
             w.view(self.U_off, h.B ** 3 * 8).copy_(torch.from_numpy(inp.halo_U.view(np.uint8)))
             self.ld2 = Loaded(w, prog)
-            self.halo_batches = [w.batch(self.ld2.translate(h.round_ops(prog, r, False))) for r in range(1, HALO_ROUNDS + 1)]
+            halo_ops = [self.ld2.translate(h.round_ops(prog, r, False)) for r in range(1, HALO_ROUNDS + 1)]
+            self.halo_batches, ts = [], []
+            for ops in halo_ops:
+                t0 = time.perf_counter()
+                self.halo_batches.append(w.batch(ops))
+                ts.append((time.perf_counter() - t0) * 1e6)
+            self.plan_us["halo_put_signal_wait"] = {"nops": len(halo_ops[0]), "host_plan_us": statistics.median(ts),
+                                                    "plans": HALO_ROUNDS}
+            self.halo_ops_host = [torch.from_numpy(o.view(np.uint8).reshape(-1).copy()).pin_memory() for o in halo_ops]
+            self.halo_ops_dev = [t.to(device) for t in self.halo_ops_host]
             self.worlds.append(w)
         if "c5" in g or "barrier" in g:
             n, nb = inp.c5_npes, inp.c5_bytes
@@ -367,6 +399,18 @@ class CudaBench:
                     self.app_launches += 2
                     with rec.seg("halo_put_signal_wait"):
                         w.enqueue_batch(self.halo_batches[r - 1])
+        if "c3b" in g:
+            with rec.seg("put_batch_skewed_onecall"):
+                self.w3b.enqueue_batch_dev(self.ops3b_dev, self.plan_us["put_batch_skewed"]["nops"], self.work3b)
+        if "c2" in g:
+            h, w = inp.halo, self.w2
+            self.ld2.obj("sig").zero_()
+            send_off = self.ld2.off["send"][0]
+            for r in range(1, HALO_ROUNDS + 1):
+                w.app_halo_pack(send_off, self.U_off, h.B)               # faces freshly written (L2), as in the rounds above
+                self.app_launches += 1
+                with rec.seg("halo_put_signal_wait_onecall"):
+                    w.enqueue_batch_dev(self.halo_ops_dev[r - 1], 96)    # plan arena of the world
         if "next2" in g:
             from paper_2607_08006_b200.binding import AMO, F32, I64, RED
             if "c5" in g:
@@ -458,9 +502,11 @@ class CudaBench:
                 self.w3a.alltoall(self.a_dst, self.a_src, inp.c3a_blk)
                 self._down(self.w3a, self.h_a_dst, self.a_dst)
         if "c3b" in g:
-            with rec.seg("put_batch_skewed"):
+            with rec.seg("put_batch_skewed"):                            # descriptors are host inputs too: one-call form
                 self._up(self.w3b, self.ld3b.off["src"][0], self.h_b_src)
-                self.w3b.enqueue_batch(self.b3b)
+                self.ops3b_dev.copy_(self.ops3b_host, non_blocking=True)
+                self.h2d += self.ops3b_host.numel()
+                self.w3b.enqueue_batch_dev(self.ops3b_dev, self.plan_us["put_batch_skewed"]["nops"], self.work3b)
                 self._down(self.w3b, self.h_b_dst, self.ld3b.off["dst"][0])
         if "c5" in g:
             n = inp.c5_bytes
@@ -483,7 +529,9 @@ class CudaBench:
             for r in range(1, HALO_ROUNDS + 1):
                 with rec.seg("halo_put_signal_wait"):
                     self._up(w, send_off, self.h_send)
-                    w.enqueue_batch(self.halo_batches[r - 1])
+                    self.halo_ops_dev[r - 1].copy_(self.halo_ops_host[r - 1], non_blocking=True)
+                    self.h2d += self.halo_ops_host[r - 1].numel()
+                    w.enqueue_batch_dev(self.halo_ops_dev[r - 1], 96)
                     self._down(w, self.h_ghost, ghost_off + (r & 1) * 6 * fb)
         if "c1" in g:
             self.w1.view(self.A, inp.c1.nelem * 8).zero_()
@@ -517,6 +565,116 @@ class CudaBench:
                 self.h_fpar.copy_(self.f_par, non_blocking=True)
                 self.d2h += self.h_fpar.numel() * 8
                 self._down(self.w4, self.h_par, self.par)
+
+    # ---- verification against the CPU oracle, after the timed loops and outside every timed region ------------------------
+    def verify(self, ob):
+        """Every segment's library call is made once more on the same inputs and its result buffers are compared with the
+        CPU oracle's (`ob`: an OracleBench holding the same inputs): bit-exact for copies, integer atomics and the fp32
+        reduction (the oracle accumulates in fp64 in PE order, as the kernel does); fetched values of fetch-add / compare-swap
+        through schedule-independent invariants.  Raises AssertionError on the first mismatch; returns {segment: True}."""
+        torch, inp, g, ok = self.torch, self.inp, self.inp.groups, {}
+        host = lambda t: t.cpu().numpy()                                           # noqa: E731
+        if "c3a" in g:
+            n, b = inp.c3a_npes, inp.c3a_blk
+            self.w3a.view(self.a_dst, n * b).zero_()
+            self.w3a.alltoall(self.a_dst, self.a_src, b)
+            ob.o3a.alltoall(ob.a_dst, ob.a_src, b)
+            assert np.array_equal(host(self.w3a.view(self.a_dst, n * b)), ob.o3a.view(ob.a_dst, n * b)), "alltoall"
+            ok["alltoall"] = True
+        if "c3b" in g:
+            ob.o3b.exec_ops(ob.ops3b)
+            want = ob.o3b.obj("dst")
+            for name, run in (("put_batch_skewed", lambda: self.w3b.enqueue_batch(self.b3b)),
+                              ("put_batch_skewed_onecall", lambda: self.w3b.enqueue_batch_dev(
+                                  self.ops3b_dev, self.plan_us["put_batch_skewed"]["nops"], self.work3b))):
+                self.ld3b.obj("dst").zero_()
+                run()
+                assert np.array_equal(host(self.ld3b.obj("dst")), want), name
+                ok[name] = True
+            assert self.w3b.batch_status(self.work3b) == (0, 0)
+        if "c5" in g:
+            n, nb = inp.c5_npes, inp.c5_bytes
+            for name, gpu, orc_ in (
+                    ("sum_reduce_f32", lambda: self.w5.sum_reduce(0, self.d5, self.s_f32, nb // 4),
+                     lambda: ob.o5.sum_reduce_f32(ob.d5, ob.s_f32, nb // 4)),
+                    ("sum_reduce_i64", lambda: self.w5.sum_reduce(1, self.d5, self.s_i64, nb // 8),
+                     lambda: ob.o5.sum_reduce_i64(ob.d5, ob.s_i64, nb // 8)),
+                    ("fcollect", lambda: self.w5.fcollect(self.d5, self.s_fc, inp.c5_fc_bytes),
+                     lambda: ob.o5.fcollect(ob.d5, ob.s_fc, inp.c5_fc_bytes))):
+                self.w5.view(self.d5, nb).zero_()
+                ob.o5.view(ob.d5, nb)[:] = 0
+                gpu(); orc_()
+                assert np.array_equal(host(self.w5.view(self.d5, nb)), ob.o5.view(ob.d5, nb)), name
+                ok[name] = True
+        if "c1" in g:
+            c = inp.c1
+            self.w1.view(self.A, c.nelem * 8).zero_()
+            self.w1.atomic_add_batch(self.A, self.c1_t, self.c1_i, val=self.c1_v, flags=self.flags)
+            self.w1.quiet_on_stream(0)
+            self.w1.barrier_all()
+            ob.o1.view(ob.A, c.nelem * 8)[:] = 0
+            ob.o1.atomic_add_batch(ob.A, c.tgt_pe, c.idx, c.val)
+            assert np.array_equal(host(self.w1.view(self.A, c.nelem * 8)), ob.o1.view(ob.A, c.nelem * 8)), "atomic_add"
+            ok["atomic_add"] = True
+        if "c4" in g:
+            q, vpp = inp.c4, inp.c4.verts_per_pe
+            self.w4.view(self.deg, vpp * 8).zero_()
+            self.w4.view(self.par, vpp * 8).fill_(255)
+            self.w4.atomic_fetch_add_batch(self.deg, self.c4_ou, self.c4_lu, self.f_deg, val=None, val_scalar=1, flags=self.fadd_flags)
+            self.w4.atomic_compare_swap_batch(self.par, self.c4_ov, self.c4_lv, self.f_par, cond=None, cond_scalar=M64,
+                                              val=self.c4_val, flags=self.cas_flags)
+            ob.o4.view(ob.deg, vpp * 8)[:] = 0
+            ou, lu, ov, lv, ones, cond, val = ob.c4
+            ob.o4.atomic_fetch_add_batch(ob.deg, ou, lu, ones)
+            deg = host(self.w4.view(self.deg, vpp * 8, torch.int64)).reshape(-1)
+            assert ob.nedge == len(q.u) and np.array_equal(deg, ob.o4.view(ob.deg, vpp * 8, np.int64).reshape(-1)), "degrees"
+            # fetch-add(1): the fetched values of a word are a permutation of 0 .. k-1 (range, sum and sum of squares; all
+            # partial sums are integers below 2^53, exact in the float64 accumulators of bincount)
+            f = host(self.f_deg).astype(np.float64)
+            k = deg.astype(np.int64)
+            assert (f >= 0).all() and (f < k[q.u]).all(), "fetched degree out of range"
+            assert np.array_equal(np.bincount(q.u, weights=f, minlength=len(k)).astype(np.int64), k * (k - 1) // 2), "fetch-add: sum of fetched values"
+            assert np.array_equal(np.bincount(q.u, weights=f * f, minlength=len(k)).astype(np.int64), (k - 1) * k * (2 * k - 1) // 6), "fetch-add: sum of squares"
+            # compare-swap(-1 -> u): one winner per touched slot, the slot holds the winner's u (an in-neighbour of v by
+            # construction: u is the source of the very edge whose op won), every loser fetched the final value
+            par = host(self.w4.view(self.par, vpp * 8, torch.int64)).reshape(-1)
+            fp = host(self.f_par)
+            won = fp == -1
+            assert np.array_equal(np.bincount(q.v[won], minlength=len(par)), (np.bincount(q.v, minlength=len(par)) > 0).astype(np.int64)), "slot not claimed exactly once"
+            assert np.array_equal(par[q.v[won]], q.u[won].astype(np.int64)), "parent is not the winner's source vertex"
+            assert np.array_equal(fp[~won], par[q.v[~won]]), "a losing compare-swap fetched something else than the final parent"
+            assert (par[np.bincount(q.v, minlength=len(par)) == 0] == -1).all(), "untouched parent slot modified"
+            ok["atomic_fetch_add"] = ok["atomic_compare_swap"] = True
+        if "c2" in g:
+            h, w, fb = inp.halo, self.w2, inp.halo.face_bytes
+            send_off = self.ld2.off["send"][0]
+            self.ld2.obj("sig").zero_()
+            self.ld2.obj("ghost").zero_()
+            snaps = {}
+            for r in range(1, HALO_ROUNDS + 1):                      # the 50 rounds of the timed step once more
+                w.app_halo_perturb(self.U_off, h.B, h.seed, r)
+                w.app_halo_pack(send_off, self.U_off, h.B)
+                if r > HALO_ROUNDS - 2:
+                    snaps[r] = host(self.ld2.obj("send")).copy()     # what the last two rounds send (one per ghost parity)
+                w.enqueue_batch(self.halo_batches[r - 1])
+            ghost, sig = host(self.ld2.obj("ghost")), host(self.ld2.obj("sig"))
+            o2 = ob.o2
+            o2.obj("ghost")[:] = 0
+            o2.obj("sig")[:] = 0
+            for r in sorted(snaps):
+                o2.obj("send")[:] = snaps[r]
+                o2.exec_ops(ob.ops2[r - 1])
+            assert np.array_equal(ghost, o2.obj("ghost")) and np.array_equal(sig, o2.obj("sig")), "halo ghosts / signal words"
+            ok["halo_put_signal_wait"] = True
+            self.ld2.obj("ghost").zero_()                            # the same two rounds through the one-call form
+            self.ld2.obj("sig").zero_()
+            for r in sorted(snaps):
+                self.ld2.obj("send").copy_(torch.from_numpy(snaps[r]))
+                w.enqueue_batch_dev(self.halo_ops_dev[r - 1], 96)
+            assert w.batch_status() == (0, 0)
+            assert np.array_equal(host(self.ld2.obj("ghost")), o2.obj("ghost")) and np.array_equal(host(self.ld2.obj("sig")), o2.obj("sig")), "halo, one-call form"
+            ok["halo_put_signal_wait_onecall"] = True
+        return ok
 
     # ---- ceilings measured in the same run ---------------------------------------------------------------------------
     def ceilings(self, reps=5):
@@ -814,6 +972,15 @@ def run_cuda(args):
         else:
             d["us_per_barrier"] = seg_ms[k] / K / t["ops"] * 1e3
         d["us_per_launch"] = per_launch_ms * 1e3
+        if k in cb.plan_us:
+            d["host_planning"] = dict(cb.plan_us[k], note="shmemg_batch_plan_bytes + shmemg_batch_create per batch (host pass, H2D, "
+                                      "stream sync); done once before the timed region, the plan is re-enqueued every step "
+                                      "(plan_reused: true); the one-call segment beside this one plans on the device inside "
+                                      "the timed region", plan_reused=True)
+        if t["cls"] == "amo" and "bytes_per_op" in t:
+            d["bytes_per_op"] = t["bytes_per_op"]
+            d["operand_stream_GBps"] = d["Mops"] * 1e6 * t["bytes_per_op"] / 1e9
+            d["frac_of_measured_hbm"] = d["operand_stream_GBps"] / peak
         segments[k] = d
     if "atomic_add" in segments and "red_add_512KiB_Mops" in ceil:
         segments["atomic_add"]["frac_of_l2_atomic_ceiling"] = segments["atomic_add"]["Mops"] / ceil["red_add_512KiB_Mops"]
@@ -825,20 +992,21 @@ def run_cuda(args):
     # dominant copy-class kernel = largest share of the timed copy-class step time
     roofline = None
     copy_names = [k for k in names if table[k]["cls"] == "copy"]
+    traffic = ncu_traffic()
     if copy_names:
         by_kernel = {}
         for k in copy_names:
             e = by_kernel.setdefault(table[k]["kernel"], [0.0, 0, 0, 0, True])
             e[0] += secs[k]; e[1] += units[k] // world; e[2] += table[k]["launches"] * K
-            e[3] += NCU_TRAFFIC.get(k, 0) * table[k]["launches"] * K
-            e[4] = e[4] and k in NCU_TRAFFIC
+            e[3] += traffic.get(k, 0) * table[k]["launches"] * K
+            e[4] = e[4] and k in traffic
         kern = max(by_kernel, key=lambda x: by_kernel[x][0])
         s, b, nl, tr, tr_ok = by_kernel[kern]
         roofline = {"bound": "hbm", "kernel": kern, "achieved": b / s / 1e9, "peak": peak, "unit": "GB/s",
                     "frac": b / s / 1e9 / peak, "peak_source": peak_src, "share_of_copy_time": s / copy_s,
                     "algorithmic_bytes_per_launch": b // nl, "avg_launch_us": s / nl * 1e6,
                     "traffic": (tr // nl) if tr_ok and not inp.small else None,
-                    "traffic_source": "profiles/r01c_ncu_full.md (launch-weighted mean over the kernel's segments)"}
+                    "traffic_source": "profiles/%s (ncu --set full capture; launch-weighted mean over the kernel's segments)" % TRAFFIC_CSV}
 
     line = base_line(args, world)
     line.update({"value": gbps, "amo_mops": mops, "ms_per_step": whole_ms / K,
@@ -851,10 +1019,17 @@ def run_cuda(args):
         eg, em, _, _ = class_rates(table, es, eu)
         line["e2e"] = {"value": eg, "unit": UNIT, "amo_mops": em, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
                        "ms_per_step": sum(es.values()) / K * 1e3,
-                       "note": "inputs from pinned host memory and results back to the host inside every segment"}
+                       "note": "inputs from pinned host memory and results back to the host inside every segment; the two "
+                               "batch workloads use the one-call form: their descriptors are copied from pinned host memory "
+                               "and planned on the device inside the timed segment (no plan is reused)"}
     if world == 1 and not args.no_cpu:
         ob = OracleBench(inp)
         res = ob.step()
+        if not args.no_verify:                                    # the oracle is test infrastructure: only here and in cpu_baseline
+            line["verified"] = cb.verify(ob)
+            for k, v in line["verified"].items():
+                if k in segments:
+                    segments[k]["verified"] = v
         osecs = {k: v[0] for k, v in res.items()}
         ounits = {k: v[1] for k, v in res.items()}
         og, om, ocs, oas = class_rates(table, osecs, ounits)

@@ -84,7 +84,7 @@ enum {
 /* ---- lifecycle ------------------------------------------------------------------------------------ */
 
 /* Bytes the caller must provide for the slab: npes heap windows (stride = heap_bytes_per_pe rounded up
- * to 512 B) plus the library's control region.  heap_bytes_per_pe == 0 means "take it from the
+ * to 512 B) plus the library's control region and plan arena (64 KiB + 4 MiB).  heap_bytes_per_pe == 0 means "take it from the
  * environment variable SHMEMG_SYMMETRIC_SIZE" (bytes, optional K/M/G suffix).
  * Returns 0 on invalid arguments. */
 SHMEMG_API size_t shmemg_slab_bytes_required(int npes, size_t heap_bytes_per_pe);
@@ -142,8 +142,8 @@ enum {
 enum { SHMEMG_SIGNAL_SET = 0, SHMEMG_SIGNAL_ADD = 1 };
 enum { SHMEMG_CMP_EQ = 0, SHMEMG_CMP_NE = 1, SHMEMG_CMP_GT = 2, SHMEMG_CMP_GE = 3, SHMEMG_CMP_LT = 4, SHMEMG_CMP_LE = 5 };
 
-/* One op descriptor, 64 bytes, HOST memory.  "Remote" = the target PE's window, "local" = the
- * initiator's window.  Unused fields are ignored. */
+/* One op descriptor, 64 bytes, in HOST memory (shmemg_batch_create, shmemg_device_exec_ops_on_stream) or DEVICE memory
+ * (shmemg_enqueue_batch).  "Remote" = the target PE's window, "local" = the initiator's window.  Unused fields are ignored. */
 typedef struct shmemg_op {
     uint8_t opcode;        /* SHMEMG_OP_*                                                     */
     uint8_t sig_op;        /* SHMEMG_SIGNAL_* (PUT_SIGNAL)                                    */
@@ -194,6 +194,31 @@ SHMEMG_API int shmemg_batch_launches(const shmemg_batch_t *b);
 
 /* Launch the batch executor on `stream` (one persistent-grid kernel; tiles are claimed in batch order). */
 SHMEMG_API int shmemg_batch_enqueue_on_stream(shmemg_world_t *w, shmemg_batch_t *b, void *stream);
+
+/*
+ * ONE-CALL FORM: host-initiated enqueue of a DEVICE-RESIDENT descriptor array ("on
+ * stream", L335 "An implementation may use internal GPU kernels to accelerate a host-issued or stream-triggered operation",
+ * L396).  `ops_dev` (DEVICE, 16-byte aligned, nops entries of shmemg_op_t, caller-owned, valid until the stream has passed
+ * the call) is planned ON THE DEVICE by one internal kernel (validation, PE -> address translation, tile cutting, dependency
+ * thresholds: the same plan shmemg_batch_create builds on the host) and executed by the batch executor launched behind it
+ * as a programmatic dependent.  No host pass over the descriptors, no synchronisation; the descriptors may have been written
+ * by earlier work on the stream (a kernel that generates the op list).  Batch semantics as above.
+ *   - shmemg_enqueue_batch uses the world's plan arena (4 MiB carved from the slab behind the control region; it holds a
+ *     batch of about 16 000 ops / 40 000 tile records).  Two calls that use the arena must be stream-ordered.
+ *   - shmemg_enqueue_batch_ws takes the workspace from the caller: `work_dev` (DEVICE, 256-byte aligned, work_bytes >=
+ *     shmemg_batch_work_bytes(w, nops, payload) where payload is an upper bound of the sum of the nbytes fields; valid until
+ *     the stream has passed the call; may be reused by a later call on the same stream).
+ *   Host-checkable misuse (NULL, alignment, a workspace too small for nops records) returns an error and enqueues nothing.
+ *   What only the device can see is reported in the plan header and nothing of the batch is executed: the first invalid
+ *   descriptor (same checks and codes as shmemg_batch_create), or SHMEMG_ERR_NOMEM when the tile records do not fit the
+ *   workspace.  shmemg_batch_status reads that status back (work_dev NULL = the arena; synchronises `stream`; *bad_index =
+ *   index of the bad descriptor, or the number of tile records needed).  More than 512 PEs: SHMEMG_ERR_ARG (plan on the host).
+ */
+SHMEMG_API size_t shmemg_batch_work_bytes(const shmemg_world_t *w, size_t nops, uint64_t payload_bytes);
+SHMEMG_API int shmemg_enqueue_batch(shmemg_world_t *w, const shmemg_op_t *ops_dev, size_t nops, void *stream);
+SHMEMG_API int shmemg_enqueue_batch_ws(shmemg_world_t *w, const shmemg_op_t *ops_dev, size_t nops, void *work_dev,
+                                       size_t work_bytes, void *stream);
+SHMEMG_API int shmemg_batch_status(shmemg_world_t *w, const void *work_dev, void *stream, int *status, size_t *bad_index);
 
 /* ---- single operations on a stream (put/get, signal put/wait, barrier on stream) ------ */
 SHMEMG_API int shmemg_put_on_stream(shmemg_world_t *w, uint64_t dest_off, uint64_t source_off, size_t nbytes,

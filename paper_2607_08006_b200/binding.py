@@ -109,6 +109,10 @@ SYMBOLS = {
     "shmemg_batch_destroy": (_i, [_vp]),
     "shmemg_batch_launches": (_i, [_vp]),
     "shmemg_batch_enqueue_on_stream": (_i, [_vp, _vp, _vp]),
+    "shmemg_batch_work_bytes": (_sz, [_vp, _sz, _u64]),
+    "shmemg_enqueue_batch": (_i, [_vp, _vp, _sz, _vp]),
+    "shmemg_enqueue_batch_ws": (_i, [_vp, _vp, _sz, _vp, _sz, _vp]),
+    "shmemg_batch_status": (_i, [_vp, _vp, _vp, C.POINTER(_i), C.POINTER(_sz)]),
     "shmemg_put_on_stream": (_i, [_vp, _u64, _u64, _sz, _i, _i, _vp]),
     "shmemg_get_on_stream": (_i, [_vp, _u64, _u64, _sz, _i, _i, _vp]),
     "shmemg_put_signal_on_stream": (_i, [_vp, _u64, _u64, _sz, _u64, _u64, _i, _i, _i, _vp]),
@@ -294,6 +298,28 @@ class World:
     def enqueue_batch(self, batch: Batch, stream=None):
         batch.enqueue(stream)
         self.launches += batch.launches
+
+    def batch_work_bytes(self, nops: int, payload_bytes: int) -> int:
+        return lib().shmemg_batch_work_bytes(self.h, nops, payload_bytes)
+
+    def enqueue_batch_dev(self, ops_dev: torch.Tensor, nops: int, work: torch.Tensor = None, stream=None):
+        """One-call form: `ops_dev` is a DEVICE uint8 tensor holding nops shmemg_op_t records; planned on the device.
+        work = None uses the world's plan arena (shmemg_enqueue_batch), else shmemg_enqueue_batch_ws."""
+        assert ops_dev.is_cuda and ops_dev.is_contiguous() and ops_dev.numel() * ops_dev.element_size() >= nops * 64
+        if work is None:
+            rc = lib().shmemg_enqueue_batch(self.h, ops_dev.data_ptr(), nops, _stream(stream))
+        else:
+            rc = lib().shmemg_enqueue_batch_ws(self.h, ops_dev.data_ptr(), nops, work.data_ptr(),
+                                               work.numel() * work.element_size(), _stream(stream))
+        self._chk(rc, "shmemg_enqueue_batch")
+        self.launches += 2 if nops else 0
+
+    def batch_status(self, work: torch.Tensor = None, stream=None):
+        """(status, bad_index) of the last one-call batch planned in `work` (None = the arena); synchronises the stream."""
+        st, bad = C.c_int(0), C.c_size_t(0)
+        self._chk(lib().shmemg_batch_status(self.h, 0 if work is None else work.data_ptr(), _stream(stream), C.byref(st),
+                                            C.byref(bad)), "shmemg_batch_status")
+        return st.value, bad.value
 
     def put(self, dest_off, source_off, nbytes, pe, target_pe, stream=None):
         self._chk(lib().shmemg_put_on_stream(self.h, dest_off, source_off, nbytes, pe, target_pe, _stream(stream)),

@@ -339,11 +339,10 @@ static bool hot_agg_ok(const shmemg_world *w, const AmoArgs &a, uint32_t flags) 
 
 template <int OP>
 static int launch_amo_hot(shmemg_world *w, const AmoArgs &a, int idx_bytes, cudaStream_t st) {
-    static bool attr_set = false;
-    if (!attr_set) {
+    if (!w->smem_attr_hot) {
         SHMEMG_CUDA(w, cudaFuncSetAttribute(k_hot_sample<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(HOT_SLOTS_SAMPLE * 8)));
         SHMEMG_CUDA(w, cudaFuncSetAttribute(k_hot_sample<8>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(HOT_SLOTS_SAMPLE * 8)));
-        attr_set = true;
+        w->smem_attr_hot = true;
     }
     // whole waves of resident CTAs; every CTA may list up to 1/8 of its ops as hot (what does not fit goes to L2 directly)
     int per_sm = 0;

@@ -31,80 +31,8 @@
 #include <vector>
 
 #include "tma_stream.cuh"
+#include "batch_plan.cuh"
 
-#define EXEC_THREADS 192          // warp 0: loader, warp 1: storer, warps 2-5: generic
-#define GEN_THREADS 128
-#define GEN_FIRST 64
-#define GEN_SLOTS 2
-#define GEN_TILE 16384u           // bytes per register-path copy tile
-#define AMO_RUN_MAX GEN_THREADS
-#define TMA_MIN_SPLIT 2048u       // below this, a transfer with unaligned ends is one register-path tile
-#define SEG_TILES_MAX 8u          // planner tiles (SHMEMG_TMA_TILE) per segment (256 KiB)
-// Executor ring geometry, chosen per batch by the planner (measured on B200, profiles/r01c):
-//   latency-bound batches (about one segment per SM): 12 stages of 16 KiB -- small stages start the store front early
-//     and a <= 192 KiB segment is loaded without re-using a stage (halo round 16.5 -> 15.1 us);
-//   streaming batches: 7 stages of 32 KiB -- 224 KiB in flight per SM towards HBM (C3b 72.6 -> 69.5 us).
-#define EXEC_STAGES_MAX 12
-#define EXEC_SMEM_MAX (7u * 32768u)
-#define EXEC_SMALL_PER_SM (256u * 1024u)   // bulk bytes per SM at or below which a batch counts as latency-bound
-#define TRACE_SLOTS 8
-#define TRACE_CTAS 256
-#define TRACE_BYTES (TRACE_CTAS * TRACE_SLOTS * 8)   // per-CTA timestamps (SHMEMG_TRACE=1)
-#define WAIT_RUN_MAX GEN_THREADS  // consecutive waits (of any PEs) polled by one tile, one per generic thread
-
-// tile kinds (bits 0-7 of TileRec.kind); bits 8-15 hold sig_op (put_signal)
-enum { T_TMA = 1, T_COPY = 2, T_AMO = 3, T_WAIT = 4, T_NODATA = 5, T_END = 6 };
-#define TF_SEGEND 0x00010000u     // (ring only) last bulk tile of its segment: account when its store has completed
-#define TF_SIGNAL 0x00020000u     // op is a PUT_SIGNAL
-#define TF_CNT_PE 0x00040000u     // a later marker of this PE depends on this op: bump done[initiator]
-#define TF_CNT_ALL 0x00080000u    // a later BARRIER_ALL depends on this op: bump done[npes]
-#define TF_DEPS 0x00100000u       // dep_pe / dep_all are non-zero
-#define TF_ACCT (TF_SIGNAL | TF_CNT_PE | TF_CNT_ALL)
-
-struct TileRec {          // 64 B, self-contained
-    uint64_t dst;         // copy destination
-    uint64_t src;         // copy source; AMO run / wait run: address of the first AuxRec
-    uint64_t sig;         // put_signal: signal word on the target
-    uint64_t value;       // signal value
-    uint32_t nbytes;      // bytes of this piece (a segment spans several bulk tiles); AMO / wait run: number of records
-    uint32_t kind;
-    uint32_t op;          // unit index (arrive[op])
-    uint32_t nt;          // pieces of this op (arrive[op] advances by nt per launch)
-    uint32_t initiator;
-    uint32_t dep_pe;      // start when done[initiator] has advanced by dep_pe in this launch
-    uint32_t dep_all;     // and done[npes] by dep_all
-    uint32_t pe_total;    // how far done[initiator] advances per launch (base of this launch = epoch * pe_total)
-};
-static_assert(sizeof(TileRec) == 64, "TileRec must be 64 bytes");
-
-struct AuxRec {           // 64 B: one AMO descriptor or one wait condition, resolved on the host
-    uint64_t word;        // AMO target word / signal word to poll
-    uint64_t fetch;       // AMO fetch slot (0 = none)
-    uint64_t value;       // AMO operand / wait comparand
-    uint64_t cond;
-    uint32_t kind;        // bits 0-7 opcode, bits 8-15 cmp (wait), TF_CNT_*
-    uint32_t initiator;
-    uint32_t dep_pe;
-    uint32_t dep_all;
-    uint32_t pe_total;
-    uint32_t pad[3];
-};
-static_assert(sizeof(AuxRec) == 64, "AuxRec must be 64 bytes");
-
-// All run-time counters are MONOTONIC across launches, so a plan needs no re-arming and no exit protocol: one launch
-// performs exactly `ntiles` ticket claims, advances done[p] by pe_total[p], done[npes] by all_total and arrive[op] by
-// nt; the launch index (epoch) is ticket / ntiles at kernel entry and every threshold is taken relative to it
-// (wrap-safe 32-bit differences).
-struct PlanHeader {       // 256 B at the start of the plan buffer
-    uint32_t ntiles, nunits, npes, trace_on;
-    unsigned long long ticket;
-    uint32_t all_total, pad1;
-    uint64_t tiles_off, aux_off, done_off, arrive_off, trace_off;
-    uint64_t pad3[23];
-};
-static_assert(sizeof(PlanHeader) == 256, "PlanHeader must be 256 bytes");
-
-struct ExecArgs;
 struct shmemg_batch {
     shmemg_world *w;
     uint8_t *plan_dev;
@@ -164,7 +92,9 @@ template <typename T> __device__ __forceinline__ T ld_rec(const T *p) {     // 6
     T r;
     const int4 *s = reinterpret_cast<const int4 *>(p);
     int4 *d = reinterpret_cast<int4 *>(&r);
-    d[0] = __ldg(s); d[1] = __ldg(s + 1); d[2] = __ldg(s + 2); d[3] = __ldg(s + 3);
+    // L2 loads (every record is read once, by one thread); not the read-only path: the plan of a one-call batch is written
+    // by the planning kernel while this kernel's CTAs are already resident (programmatic dependent launch)
+    d[0] = ld_stream16(s); d[1] = ld_stream16(s + 1); d[2] = ld_stream16(s + 2); d[3] = ld_stream16(s + 3);
     return r;
 }
 
@@ -176,17 +106,6 @@ __device__ __forceinline__ unsigned long long gtime() {
 }
 #define TRACE(slot) do { if (trace) trace[blockIdx.x * TRACE_SLOTS + (slot)] = gtime(); } while (0)
 
-// Everything a CTA needs to start is a kernel ARGUMENT (constant bank); the only global reads on the start-up path are
-// the first tile record and the ticket counter, issued together.
-struct ExecArgs {
-    const TileRec *tiles;
-    unsigned long long *ticket;
-    unsigned *done, *arrive;
-    unsigned long long *trace;     // nullptr unless SHMEMG_TRACE
-    unsigned ntiles, npes, all_total;
-    unsigned stage_bytes, nstages;     // ring geometry
-};
-
 __global__ void __launch_bounds__(EXEC_THREADS, 1) k_batch_exec(const ExecArgs a) {
     extern __shared__ __align__(1024) uint8_t stage[];
     __shared__ __align__(16) TileRec ringA[EXEC_STAGES_MAX];
@@ -196,8 +115,8 @@ __global__ void __launch_bounds__(EXEC_THREADS, 1) k_batch_exec(const ExecArgs a
 
     const TileRec *tiles = a.tiles;
     unsigned *done = a.done, *arrive = a.arrive;
-    const unsigned ntiles = a.ntiles;
-    const unsigned STG = a.stage_bytes, NST = a.nstages;
+    unsigned ntiles = a.ntiles;
+    unsigned STG = a.stage_bytes, NST = a.nstages;
     const int tid = threadIdx.x;
     unsigned long long *trace = blockIdx.x < TRACE_CTAS ? a.trace : nullptr;
     Epoch ep;
@@ -210,6 +129,24 @@ __global__ void __launch_bounds__(EXEC_THREADS, 1) k_batch_exec(const ExecArgs a
         mbar_init(&epochB, 1);
         mbar_init_fence();
     }
+    if (a.hdr) {
+        // One-call batch (shmemg_enqueue_batch): the planning kernel is the previous kernel of the stream and this one is
+        // launched as its programmatic dependent, so everything above overlaps the planner; from here on its writes
+        // (header, tile records, zeroed counters) are visible.  Coherent (L2) loads: nothing of the plan is in L1 yet.
+#ifdef SHMEMG_PLAN_TRACE
+        if (blockIdx.x == 0 && tid == 0) const_cast<PlanHeader *>(a.hdr)->pad3[8] = gtime();
+#endif
+        asm volatile("griddepcontrol.wait;" ::: "memory");
+#ifdef SHMEMG_PLAN_TRACE
+        if (blockIdx.x == 0 && tid == 0) const_cast<PlanHeader *>(a.hdr)->pad3[9] = gtime();
+#endif
+        const int4 h0 = ld_stream16(&a.hdr->ntiles);            // ntiles, nunits, npes, trace_on
+        const int4 h1 = ld_stream16(&a.hdr->stage_bytes);       // stage_bytes, nstages, status, pad
+        const unsigned at = *reinterpret_cast<const volatile unsigned *>(&a.hdr->all_total);
+        ntiles = h1.z == 0 ? (unsigned)h0.x : 0u;               // a rejected plan executes nothing
+        STG = (unsigned)h1.x; NST = (unsigned)h1.y;
+        ep.all_total = at;
+    }
     __syncthreads();
 
     if (tid == 0) {
@@ -221,7 +158,7 @@ __global__ void __launch_bounds__(EXEC_THREADS, 1) k_batch_exec(const ExecArgs a
         // issued first and consumed only after the first segment's loads are in flight; the consumers pick s_epoch up
         // through the epochB mbarrier before their first completion accounting.
         TRACE(1);
-        const unsigned long long tk0 = ld_relaxed_u64(a.ticket);
+        const unsigned long long tk0 = a.hdr ? 0ull : ld_relaxed_u64(a.ticket);   // one-call plans start at launch index 0
         TileRec r0 = {};
         if (blockIdx.x < ntiles) r0 = ld_rec(tiles + blockIdx.x);
         unsigned ia = 0, ig = 0;                                     // ia = stage index, pa = its lap parity
@@ -318,6 +255,9 @@ __global__ void __launch_bounds__(EXEC_THREADS, 1) k_batch_exec(const ExecArgs a
         bulk_wait<0>();
         if (pend_acct) { proxy_fence(); epoch(); account(acct, done, arrive, ep); }
         TRACE(4);
+#ifdef SHMEMG_PLAN_TRACE
+        if (a.hdr && blockIdx.x == 0) const_cast<PlanHeader *>(a.hdr)->pad3[10] = gtime();
+#endif
     } else if (tid >= GEN_FIRST) {
         // ---- generic warps: register-path copies and AMO runs ----------------------------------------------
         const int gt = tid - GEN_FIRST;
@@ -478,11 +418,11 @@ static void cut_copy(uint64_t dst, uint64_t src, uint64_t n, uint32_t seg_tiles,
         // balanced segments of at most seg_tiles bulk tiles
         const uint64_t tiles = (body + SHMEMG_TMA_TILE - 1) / SHMEMG_TMA_TILE;
         const uint64_t nseg = (tiles + seg_tiles - 1) / seg_tiles;
-        for (uint64_t g = 0, b0 = 0; g < nseg; ++g) {            // equal byte shares, cut at 1 KiB (the executor re-tiles a segment)
-            const uint64_t b1 = g + 1 == nseg ? body : ((g + 1) * body / nseg) & ~1023ull;
-            if (b1 > b0) out.push_back({T_TMA, head + b0, (uint32_t)(b1 - b0)});
-            b0 = b1;
-        }
+        // equal byte shares, cut at 1 KiB (the executor re-tiles a segment); one division per op: the device planner
+        // (plan_dev.cu) applies the same rule
+        const uint64_t share = ((body + nseg - 1) / nseg + 1023ull) & ~1023ull;
+        for (uint64_t b0 = 0; b0 < body; b0 += share)
+            out.push_back({T_TMA, head + b0, (uint32_t)(body - b0 < share ? body - b0 : share)});
         if (tail) out.push_back({T_COPY, head + body, (uint32_t)tail});
         return;
     }
@@ -560,7 +500,7 @@ static PlanSizes plan_sizes(const shmemg_world *w, const shmemg_op_t *ops, size_
         if (is_amo(u.opc) || u.opc == SHMEMG_OP_SIGNAL_WAIT_UNTIL) {     // runs of AMOs / runs of waits: one tile each
             const uint32_t rk = is_amo(u.opc) ? T_AMO : T_WAIT;
             s.naux++;
-            if (run == 0 || run == AMO_RUN_MAX || rk != run_kind) { s.ntiles++; run = 0; run_kind = rk; }
+            if (run == 0 || run == AMO_RUN_MAX || rk != run_kind || u.first % PLAN_CHUNK_OPS == 0) { s.ntiles++; run = 0; run_kind = rk; }
             run++;
             continue;
         }
@@ -615,7 +555,7 @@ extern "C" int shmemg_batch_create(shmemg_world_t *w, const shmemg_op_t *ops, si
     std::vector<uint32_t> pe_total(ndom, 0);    // how far done[domain] advances per launch
     uint32_t all_total = 0;
     {
-        std::vector<uint8_t> later_real(ndom, 0), need(ndom, 0);
+        std::vector<uint8_t> later_real(ndom, 0), later_nonwait(ndom, 0), need(ndom, 0);
         bool later_any = false, need_all = false;
         for (size_t i = nu; i-- > 0;) {
             const Unit &u = units[i];
@@ -624,12 +564,14 @@ extern "C" int shmemg_batch_create(shmemg_world_t *w, const shmemg_op_t *ops, si
                 continue;
             }
             if (u.opc == SHMEMG_OP_BARRIER_ALL) { if (later_any) need_all = true; continue; }
-            // a wait orders the PE's later ops after it: the wait and every earlier op of that PE are counted
-            if (u.opc == SHMEMG_OP_SIGNAL_WAIT_UNTIL && later_real[u.pe]) need[u.pe] = 1;
+            // a wait orders the domain's later ops after it: the wait and every earlier op of the domain are counted if
+            // an op other than a wait follows (waits that only other waits follow order nothing: the end of the kernel does)
+            if (u.opc == SHMEMG_OP_SIGNAL_WAIT_UNTIL && later_nonwait[u.pe]) need[u.pe] = 1;
             cnt[i] = (need[u.pe] ? 1 : 0) | (need_all ? 2 : 0);
             if (cnt[i] & 1) pe_total[u.pe]++;
             if (cnt[i] & 2) all_total++;
             later_real[u.pe] = 1;
+            if (u.opc != SHMEMG_OP_SIGNAL_WAIT_UNTIL) later_nonwait[u.pe] = 1;
             later_any = true;
         }
     }
@@ -673,11 +615,11 @@ extern "C" int shmemg_batch_create(shmemg_world_t *w, const shmemg_op_t *ops, si
         if (is_amo(u.opc)) {
             AuxRec &d = aux[na];
             d.word = (uint64_t)shmemg_addr(w, o.target_pe, o.rem_off);
-            d.fetch = u.opc == SHMEMG_OP_ATOMIC_ADD ? 0 : (uint64_t)shmemg_addr(w, ini, o.loc_off);
+            d.fetch = u.opc == SHMEMG_OP_ATOMIC_ADD ? 0 : (uint64_t)shmemg_addr(w, o.initiator_pe, o.loc_off);   // the PE, not the domain
             d.value = o.value; d.cond = o.cond;
             d.kind = u.opc | flags;
             d.initiator = (uint32_t)ini; d.dep_pe = dep_pe; d.dep_all = dep_all; d.pe_total = pe_total[ini];
-            if (run == 0 || run == AMO_RUN_MAX || run_kind != T_AMO) {
+            if (run == 0 || run == AMO_RUN_MAX || run_kind != T_AMO || u.first % PLAN_CHUNK_OPS == 0) {
                 TileRec &t = tiles[nt++];
                 t.kind = T_AMO; t.nbytes = 0; t.nt = 1; t.op = (uint32_t)k;
                 t.src = aux_dev(na);
@@ -687,11 +629,11 @@ extern "C" int shmemg_batch_create(shmemg_world_t *w, const shmemg_op_t *ops, si
             run++; na++;
         } else if (u.opc == SHMEMG_OP_SIGNAL_WAIT_UNTIL) {
             AuxRec &d = aux[na];
-            d.word = (uint64_t)shmemg_addr(w, ini, o.loc_off);
+            d.word = (uint64_t)shmemg_addr(w, o.initiator_pe, o.loc_off);
             d.value = o.value;
             d.kind = SHMEMG_OP_SIGNAL_WAIT_UNTIL | ((uint32_t)o.cmp << 8) | flags;
             d.initiator = (uint32_t)ini; d.dep_pe = dep_pe; d.dep_all = dep_all; d.pe_total = pe_total[ini];
-            if (run == 0 || run == WAIT_RUN_MAX || run_kind != T_WAIT) {
+            if (run == 0 || run == WAIT_RUN_MAX || run_kind != T_WAIT || u.first % PLAN_CHUNK_OPS == 0) {
                 TileRec &t = tiles[nt++];
                 t.kind = T_WAIT; t.nbytes = 0; t.nt = 1; t.op = (uint32_t)k;
                 t.src = aux_dev(na);
@@ -762,7 +704,7 @@ extern "C" int shmemg_batch_destroy(shmemg_batch_t *b) {
 }
 extern "C" int shmemg_batch_launches(const shmemg_batch_t *b) { return b ? (b->ntiles ? 1 : 0) : SHMEMG_ERR_ARG; }
 
-static int ensure_smem_attr(shmemg_world *w) {
+int shmemg_exec_smem_attr(shmemg_world *w) {
     if (w->smem_attr_set) return SHMEMG_OK;
     SHMEMG_CUDA(w, cudaFuncSetAttribute(k_batch_exec, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)EXEC_SMEM_MAX));
     SHMEMG_CUDA(w, cudaFuncSetAttribute(k_copy_single_tma, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SHMEMG_TMA_SMEM));
@@ -770,11 +712,25 @@ static int ensure_smem_attr(shmemg_world *w) {
     return SHMEMG_OK;
 }
 
+// Launch the executor.  after_planner: the previous kernel of the stream is the device planner, which releases its
+// dependents early (griddepcontrol.launch_dependents); with programmatic stream serialization the executor's CTAs are set up
+// while the planner still runs and block in griddepcontrol.wait until it has finished.
+int shmemg_exec_launch(shmemg_world *w, const ExecArgs &a, unsigned grid, size_t smem, cudaStream_t st, bool after_planner) {
+    int rc = shmemg_exec_smem_attr(w);
+    if (rc) return rc;
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3(grid); cfg.blockDim = dim3(EXEC_THREADS); cfg.dynamicSmemBytes = smem; cfg.stream = st;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    at[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = at; cfg.numAttrs = (after_planner && !getenv("SHMEMG_NO_PDL")) ? 1 : 0;     // SHMEMG_NO_PDL: experiments
+    SHMEMG_CUDA(w, cudaLaunchKernelEx(&cfg, k_batch_exec, a));
+    return SHMEMG_OK;
+}
+
 extern "C" int shmemg_batch_enqueue_on_stream(shmemg_world_t *w, shmemg_batch_t *b, void *stream) {
     if (!w || !b || b->w != w) return SHMEMG_ERR_ARG;
     if (b->ntiles == 0) return SHMEMG_OK;
-    int rc = ensure_smem_attr(w);
-    if (rc) return rc;
     ExecArgs a;
     a.tiles = reinterpret_cast<const TileRec *>(b->plan_dev + b->tiles_off);
     a.ticket = &reinterpret_cast<PlanHeader *>(b->plan_dev)->ticket;
@@ -783,9 +739,8 @@ extern "C" int shmemg_batch_enqueue_on_stream(shmemg_world_t *w, shmemg_batch_t 
     a.trace = b->trace_on ? reinterpret_cast<unsigned long long *>(b->plan_dev + b->trace_off) : nullptr;
     a.ntiles = b->ntiles; a.npes = b->npes; a.all_total = b->all_total;
     a.stage_bytes = b->stage_bytes; a.nstages = b->nstages;
-    k_batch_exec<<<b->grid, EXEC_THREADS, (size_t)b->stage_bytes * b->nstages, (cudaStream_t)stream>>>(a);
-    SHMEMG_CUDA(w, cudaGetLastError());
-    return SHMEMG_OK;
+    a.hdr = nullptr;
+    return shmemg_exec_launch(w, a, b->grid, (size_t)b->stage_bytes * b->nstages, (cudaStream_t)stream, false);
 }
 
 // ---------------------------------------------------------------------------------------------------------
@@ -796,7 +751,7 @@ static int launch_copy(shmemg_world *w, uint8_t *dst, const uint8_t *src, size_t
     if (nbytes == 0 && !sig) return SHMEMG_OK;
     unsigned *counter = sig ? &w->ctl->sig_counter[(w->sig_seq++) % SHMEMG_SIG_SLOTS] : nullptr;
     if (nbytes && (((uintptr_t)dst | (uintptr_t)src | nbytes) & 15) == 0 && !w->tile_bytes_override) {
-        int rc = ensure_smem_attr(w);
+        int rc = shmemg_exec_smem_attr(w);
         if (rc) return rc;
         const uint64_t ntiles = (nbytes + SHMEMG_TMA_TILE - 1) / SHMEMG_TMA_TILE;
         const uint32_t grid = (uint32_t)(ntiles < (uint64_t)w->sm_count ? ntiles : (uint64_t)w->sm_count);

@@ -479,11 +479,11 @@ extern "C" int shmemg_fcollect_on_stream(shmemg_world_t *w, uint64_t dest_off, u
 template <int DT, int OP>
 static void launch_reduce(shmemg_world *w, uint64_t dest_off, uint64_t source_off, size_t nvec, size_t first, size_t nreduce,
                           cudaStream_t st) {
-    static bool attr_set = false;
     if (nvec) {
-        if (!attr_set) {
-            cudaFuncSetAttribute(k_sum_reduce_tma<DT, OP>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)RED_SMEM);
-            attr_set = true;
+        if (!w->smem_attr_red[DT][OP]) {
+            if (cudaFuncSetAttribute(k_sum_reduce_tma<DT, OP>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)RED_SMEM) != cudaSuccess)
+                return;                                    // the caller's cudaGetLastError reports it
+            w->smem_attr_red[DT][OP] = true;
         }
         const size_t nb = nvec << 4, ntiles = (nb + RT - 1) / RT;
         const unsigned grid = (unsigned)(ntiles < (size_t)w->sm_count ? ntiles : (size_t)w->sm_count);

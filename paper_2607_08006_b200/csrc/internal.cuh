@@ -12,6 +12,7 @@
 #include "../../include/shmemg.h"
 
 #define SHMEMG_CTL_BYTES (64u * 1024u)     // control region carved from the tail of the slab
+#define SHMEMG_ARENA_BYTES (4u << 20)      // plan arena behind the control region: workspace of shmemg_enqueue_batch
 #define SHMEMG_STRIDE_ALIGN 512u
 #define SHMEMG_MIN_ALIGN 256u
 #define SHMEMG_THREADS 256                 // threads per CTA of the register-path copy kernels
@@ -48,8 +49,12 @@ struct shmemg_world {
     unsigned sig_seq = 0;
     int ctas_per_sm = 4;                   // copy-class persistent grids: ctas_per_sm * sm_count CTAs
     size_t tile_bytes_override = 0;        // SHMEMG_TILE_BYTES (experiments; forces the register copy path)
-    bool smem_attr_coll = false, smem_attr_probe = false;
-    bool smem_attr_set = false;            // dynamic shared memory opt-in done for the bulk-copy kernels
+    // dynamic shared memory opt-in (cudaFuncSetAttribute) done on THIS world's device, per kernel family
+    bool smem_attr_coll = false, smem_attr_probe = false, smem_attr_plan = false, smem_attr_hot = false;
+    bool smem_attr_bcast = false, smem_attr_ib = false;
+    bool smem_attr_red[4][7] = {};         // k_sum_reduce_tma<dtype, op>
+    bool smem_attr_set = false;            // the batch executor and the single-copy bulk kernel
+    uint8_t *arena = nullptr;              // DEVICE: plan arena (SHMEMG_ARENA_BYTES) behind the control region
     struct Team { int start, stride, size; };
     int teams_world_npes = 0;              // npes of the world while a team view is active (surface2.cu)
     std::vector<Team> teams;               // user teams (shmemg_team_split_strided); handle = SHMEMG_TEAM_USER0 + index

@@ -44,10 +44,9 @@ extern "C" int shmemg_broadcast_on_stream(shmemg_world_t *w, uint64_t dest_off, 
     if (ranges_overlap2(dest_off, source_off, nbytes, nbytes)) return SHMEMG_ERR_OVERLAP;
     cudaStream_t st = (cudaStream_t)stream;
     if (((dest_off | source_off | nbytes | w->stride) & 15) == 0 && !w->tile_bytes_override) {
-        static bool attr_set = false;
-        if (!attr_set) {
+        if (!w->smem_attr_bcast) {
             SHMEMG_CUDA(w, cudaFuncSetAttribute(k_broadcast_tma, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SHMEMG_TMA_SMEM));
-            attr_set = true;
+            w->smem_attr_bcast = true;
         }
         const uint64_t items = (uint64_t)((nbytes + SHMEMG_TMA_TILE - 1) / SHMEMG_TMA_TILE) * w->npes;
         const unsigned grid = (unsigned)(items < (uint64_t)w->sm_count ? items : (uint64_t)w->sm_count);
@@ -250,10 +249,9 @@ static int launch_ib(shmemg_world *w, uint64_t dest_off, uint64_t source_off, ui
     const uint64_t all = (uint64_t)(uintptr_t)dst | (uint64_t)(uintptr_t)src | dst_stride | src_stride | block;
     const uint64_t maxgrid = (uint64_t)w->sm_count * 8;
     if (block >= 1024 && (all & 15) == 0) {
-        static bool attr_set = false;
-        if (!attr_set) {
+        if (!w->smem_attr_ib) {
             SHMEMG_CUDA(w, cudaFuncSetAttribute(k_ib_tma, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SHMEMG_TMA_SMEM));
-            attr_set = true;
+            w->smem_attr_ib = true;
         }
         const uint64_t items = (uint64_t)nblocks * ((block + SHMEMG_TMA_TILE - 1) / SHMEMG_TMA_TILE);
         k_ib_tma<<<(unsigned)(items < (uint64_t)w->sm_count ? items : (uint64_t)w->sm_count), 32, SHMEMG_TMA_SMEM, st>>>(

@@ -30,7 +30,7 @@ extern "C" size_t shmemg_slab_bytes_required(int npes, size_t heap_bytes_per_pe)
     if (npes < 1) return 0;
     if (heap_bytes_per_pe == 0) heap_bytes_per_pe = env_heap_bytes();
     if (heap_bytes_per_pe == 0) return 0;
-    return (size_t)npes * round_up(heap_bytes_per_pe, SHMEMG_STRIDE_ALIGN) + SHMEMG_CTL_BYTES;
+    return (size_t)npes * round_up(heap_bytes_per_pe, SHMEMG_STRIDE_ALIGN) + SHMEMG_CTL_BYTES + SHMEMG_ARENA_BYTES;
 }
 
 extern "C" int shmemg_init(int npes, size_t heap_bytes_per_pe, void *device_slab, size_t slab_bytes,
@@ -65,6 +65,7 @@ extern "C" int shmemg_init(int npes, size_t heap_bytes_per_pe, void *device_slab
     w->base = (uint8_t *)device_slab;
     w->slab_bytes = slab_bytes;
     w->ctl = (CtlRegion *)(w->base + (size_t)npes * w->stride);
+    w->arena = (uint8_t *)w->ctl + SHMEMG_CTL_BYTES;
     w->free_list[0] = heap_bytes_per_pe;
     if (const char *s = getenv("SHMEMG_CTAS_PER_SM")) {
         int v = atoi(s);

@@ -28,6 +28,33 @@ def run_gpu(prog, batches=None, heap_bytes=None):
     return w, ld
 
 
+def ops_to_dev(ops: np.ndarray) -> torch.Tensor:
+    """shmemg_op_t records as a DEVICE uint8 tensor (input of the one-call form shmemg_enqueue_batch)."""
+    return torch.from_numpy(np.ascontiguousarray(ops).view(np.uint8).reshape(-1).copy()).to(DEV)
+
+
+def run_gpu_onecall(prog, batches=None, heap_bytes=None, arena=False):
+    """Same as run_gpu, through the ONE-CALL form: the descriptors are device-resident and planned on the device
+    (shmemg_enqueue_batch / shmemg_enqueue_batch_ws); the plan status is checked after every batch."""
+    hb = heap_bytes or heap_bytes_for(prog)
+    w = World(prog.npes, hb, DEV)
+    ld = Loaded(w, prog)
+    keep = []
+    for q in (batches or [prog]):
+        ops = ld.translate(q)
+        od = ops_to_dev(ops) if len(ops) else torch.zeros(64, dtype=torch.uint8, device=DEV)
+        work = None
+        if not arena:
+            payload = int(ops["nbytes"][(ops["opcode"] >= 1) & (ops["opcode"] <= 3)].sum())
+            work = torch.empty(w.batch_work_bytes(len(ops), payload), dtype=torch.uint8, device=DEV)
+        w.enqueue_batch_dev(od, len(ops), work)
+        if len(ops):
+            assert w.batch_status(work) == (0, 0)
+        keep.append((od, work))
+    w.quiet(0)
+    return w, ld
+
+
 def run_gpu_device(prog, batches=None, heap_bytes=None):
     """Same as run_gpu, but DEVICE-INITIATED: every batch is executed by PE-agent thread blocks through the
     entry points of include/shmemg_device.cuh (shmemg_device_exec_ops_on_stream)."""

@@ -25,6 +25,10 @@ Program format: prog[p] = list of ops, each a tuple:
   ("add", t, dst, v) / ("fadd", t, dst, v, fetch) / ("cas", t, dst, cond, v, fetch)
   ("wait", sig, cmp, v)  cmp in {"eq","ne","gt","ge","lt","le"}
   ("fence",) / ("quiet",) / ("barrier",)
+Contexts (reading 31): any op may carry a trailing "@c" (c = context number,
+default "@0").  A context is an independent stream of operations of its PE: PROGRAM ORDER, FENCE, QUIET and
+SIGNAL_WAIT_UNTIL act within one (PE, context) pair only; BARRIER_ALL covers every context of every PE.  The
+enumerator therefore runs one in-order program per (PE, context) domain; addresses still name PEs.
 """
 from __future__ import annotations
 
@@ -42,8 +46,29 @@ def _set(heaps, p, i, v):
     return tuple(h)
 
 
+def split_ctx(op):
+    """(op without its context tag, context number)"""
+    if isinstance(op[-1], str) and op[-1].startswith("@"):
+        return tuple(op[:-1]), int(op[-1][1:])
+    return tuple(op), 0
+
+
+def _domains(prog):
+    """Split per-PE programs into per-(PE, context) in-order programs; a barrier is replicated into every domain of
+    its PE.  Returns (owner PE of each domain, domain programs)."""
+    owner, dprog = [], []
+    for p, ops in enumerate(prog):
+        tagged = [split_ctx(op) for op in ops]
+        ctxs = sorted({c for op, c in tagged if op[0] != "barrier"}) or [0]
+        for c in ctxs:
+            owner.append(p)
+            dprog.append([op for op, cc in tagged if op[0] == "barrier" or cc == c])
+    return owner, dprog
+
+
 def enumerate_outcomes(prog, init_heaps, per_target_fence: bool = False, limit: int = 2_000_000):
     """Return the set of reachable final heaps (tuple of per-PE tuples of words)."""
+    owner, prog = _domains(prog)          # from here on "p" indexes a (PE, context) domain, owner[p] is its PE
     npes = len(prog)
     # fence_before[p][i] = number of fences among ops 0..i-1 of p (its "fence epoch")
     epoch = []
@@ -64,9 +89,10 @@ def enumerate_outcomes(prog, init_heaps, per_target_fence: bool = False, limit: 
                     return False
         return True
 
-    def deliver(heaps, p, item):
+    def deliver(heaps, d, item):
         i, stage = item
-        op = prog[p][i]
+        op = prog[d][i]
+        p = owner[d]                      # the initiating PE (local heap of gets / fetch slots / put sources)
         k = op[0]
         follow = None
         if k == "put":
@@ -136,7 +162,7 @@ def enumerate_outcomes(prog, init_heaps, per_target_fence: bool = False, limit: 
                     stack.append((pcs[:p] + (pcs[p] + 1,) + pcs[p + 1:], pends, heaps))
                     moved = True
             elif k == "wait":
-                if _CMP[op[2]](heaps[p][op[1]], op[3] & M64):
+                if _CMP[op[2]](heaps[owner[p]][op[1]], op[3] & M64):
                     stack.append((pcs[:p] + (pcs[p] + 1,) + pcs[p + 1:], pends, heaps))
                     moved = True
             elif k == "barrier":
@@ -169,28 +195,28 @@ def to_spec_program(prog, init_heaps, order):
     sp.obj("w", nw * 8, np.array(init_heaps, dtype=np.uint64))
     pcs = [0] * npes
     for p in order:
-        op = prog[p][pcs[p]]
+        op, c = split_ctx(prog[p][pcs[p]])
         pcs[p] += 1
         k = op[0]
         if k == "put":
-            sp.put(p, op[1], ("w", op[2] * 8), ("w", op[3] * 8), 8)
+            sp.put(p, op[1], ("w", op[2] * 8), ("w", op[3] * 8), 8, ctx=c)
         elif k == "get":
-            sp.get(p, op[1], ("w", op[2] * 8), ("w", op[3] * 8), 8)
+            sp.get(p, op[1], ("w", op[2] * 8), ("w", op[3] * 8), 8, ctx=c)
         elif k == "put_signal":
             sp.put_signal(p, op[1], ("w", op[2] * 8), ("w", op[3] * 8), 8, ("w", op[4] * 8), op[5],
-                          SIGNAL_SET if op[6] == "set" else SIGNAL_ADD)
+                          SIGNAL_SET if op[6] == "set" else SIGNAL_ADD, ctx=c)
         elif k == "add":
-            sp.atomic_add(p, op[1], ("w", op[2] * 8), op[3])
+            sp.atomic_add(p, op[1], ("w", op[2] * 8), op[3], ctx=c)
         elif k == "fadd":
-            sp.atomic_fetch_add(p, op[1], ("w", op[2] * 8), op[3], ("w", op[4] * 8))
+            sp.atomic_fetch_add(p, op[1], ("w", op[2] * 8), op[3], ("w", op[4] * 8), ctx=c)
         elif k == "cas":
-            sp.atomic_compare_swap(p, op[1], ("w", op[2] * 8), op[3], op[4], ("w", op[5] * 8))
+            sp.atomic_compare_swap(p, op[1], ("w", op[2] * 8), op[3], op[4], ("w", op[5] * 8), ctx=c)
         elif k == "wait":
-            sp.signal_wait_until(p, ("w", op[1] * 8), cmpmap[op[2]], op[3])
+            sp.signal_wait_until(p, ("w", op[1] * 8), cmpmap[op[2]], op[3], ctx=c)
         elif k == "fence":
-            sp.fence(p)
+            sp.fence(p, ctx=c)
         elif k == "quiet":
-            sp.quiet(p)
+            sp.quiet(p, ctx=c)
         elif k == "barrier":
             if p == 0:
                 sp.barrier_all()

@@ -51,10 +51,11 @@ def test_host_only_entry_points_without_gpu():
     from paper_2607_08006_b200 import binding
     L = binding.lib()
     assert L.shmemg_slab_bytes_required(0, 100) == 0
-    assert L.shmemg_slab_bytes_required(4, 1000) == 4 * 1024 + 65536
+    CTL = 65536 + (4 << 20)                    # control region + plan arena
+    assert L.shmemg_slab_bytes_required(4, 1000) == 4 * 1024 + CTL
     os.environ["SHMEMG_SYMMETRIC_SIZE"] = "2K"
     try:
-        assert L.shmemg_slab_bytes_required(3, 0) == 3 * 2048 + 65536
+        assert L.shmemg_slab_bytes_required(3, 0) == 3 * 2048 + CTL
     finally:
         del os.environ["SHMEMG_SYMMETRIC_SIZE"]
     assert L.shmemg_slab_bytes_required(3, 0) == 0
@@ -63,6 +64,8 @@ def test_host_only_entry_points_without_gpu():
     assert L.shmemg_n_pes(None) == binding.ERR.ARG
     assert L.shmemg_ptr(None, 0, 0) is None
     assert L.shmemg_batch_plan_bytes(None, None, 0) == 0
+    assert L.shmemg_batch_work_bytes(None, 10, 0) == 0
+    assert L.shmemg_enqueue_batch(None, None, 0, None) == binding.ERR.ARG
 
 
 def test_product_path_never_imports_oracle():

@@ -24,8 +24,11 @@ M64 = (1 << 64) - 1
     lambda: litmus.signal_add_fanin(),
     lambda: litmus.barrier_stamp(),
     lambda: litmus.barrier_stamp(npes=128, rounds=12),
+    lambda: litmus.wait_after_wait(),
+    lambda: litmus.two_contexts(),
+    lambda: litmus.contexts_amos_waits(),
 ], ids=["mp_fence", "mp_fence_big", "mp_quiet3", "put_signal_sizes", "signal_add_fanin", "barrier_stamp",
-        "barrier_stamp128"])
+        "barrier_stamp128", "wait_after_wait", "two_contexts", "contexts_amos_waits"])
 def test_litmus_programs_match_oracle(make):
     prog = make()
     w, ld = run_gpu(prog)
@@ -110,6 +113,13 @@ TINY = {
     "barrier": ([[("put", 1, 0, 2), ("barrier",), ("get", 0, 4, 0)], [("put", 0, 0, 2), ("barrier",), ("get", 1, 4, 0)]],
                 [[0, 0, 42, 0, 0], [0, 0, 43, 0, 0]], [0, 1, 0, 1, 0, 1]),
     "quiet_readback": ([[("put", 1, 0, 2), ("quiet",), ("get", 1, 4, 0)], []], [[0, 0, 42, 0, 0], [0] * 5], [0, 0, 0]),
+    # contexts (ctx > 0) with waits and fetching AMOs: fetch slots and wait words live in the PE's window, not the domain's
+    "ctx_quiet_independent": ([[("put", 1, 0, 2, "@0"), ("put", 1, 5, 5, "@1"), ("quiet", "@1"), ("put", 1, 1, 3, "@1")],
+                               [("wait", 1, "eq", 1, "@2"), ("get", 1, 4, 0, "@2")]],
+                              [[0, 0, 42, 1, 0, 7], [0] * 6], [0, 0, 0, 0, 1, 1]),
+    "ctx_fadd_cas_wait": ([[("fadd", 1, 0, 2, 1, "@3"), ("cas", 1, 2, M64, 9, 3, "@3"), ("quiet", "@3"), ("add", 1, 4, 1, "@3")],
+                           [("wait", 4, "ge", 1, "@1"), ("fadd", 1, 0, 5, 1, "@1"), ("cas", 1, 2, M64, 8, 3, "@1")]],
+                          [[0, 0, 0, 0, 0], [0, 0, M64, 0, 0]], [0, 0, 0, 0, 1, 1, 1]),
     "add_fence_add": ([[("add", 1, 0, 7), ("fence",), ("add", 1, 1, 1)], [("wait", 1, "ge", 1), ("get", 1, 4, 0)]],
                       [[0] * 5, [0] * 5], [0, 0, 0, 1, 1]),
 }

@@ -399,9 +399,20 @@ def test_c2_halo_50_rounds_small_grid():
         assert np.array_equal(a, b), "stale or wrong face in round %d" % (r + 1)
 
 
+def test_c2_halo_50_rounds_b128():
+    """All 50 rounds of config 2 on a 256^3 grid (128^3 blocks, 128 KiB faces): whole heap and the per-round checksum log."""
+    prog, ld, ow, lg, lo = _halo_run(B=128, rounds=50, consume=False)
+    assert_objects_equal(prog, ld, ow, names=["ghost", "sig", "send"])
+    assert np.array_equal(ld.obj_numpy("U", np.float64), ow.obj("U", np.float64))
+    assert len(lg) == 50
+    for r, (a, b) in enumerate(zip(lg, lo)):
+        assert np.array_equal(a, b), "stale or wrong face in round %d" % (r + 1)
+
+
 def test_c2_halo_full_size_rounds():
-    """Config 2 geometry at full size (512^3 grid, 256^3 blocks, 512 KiB faces), 3 rounds, whole-heap oracle compare."""
-    prog, ld, ow, lg, lo = _halo_run(B=256, rounds=3, consume=False)
+    """Config 2 geometry at full size (512^3 grid, 256^3 blocks, 512 KiB faces), 10 rounds, whole-heap oracle compare and
+    the checksum log of every round."""
+    prog, ld, ow, lg, lo = _halo_run(B=256, rounds=10, consume=False)
     assert_objects_equal(prog, ld, ow, names=["ghost", "sig", "send"])
     assert np.array_equal(ld.obj_numpy("U", np.float64), ow.obj("U", np.float64))
     for a, b in zip(lg, lo):

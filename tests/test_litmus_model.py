@@ -160,3 +160,41 @@ def test_oracle_inside_reachable_set_random_programs(seed):
     rng.shuffle(shuffled)            # per-PE op order is kept: `order` only says whose turn it is
     for order in ([0] * n0 + [1] * n1, [1] * n1 + [0] * n0, list(shuffled)):
         assert oracle_heaps(prog, init, order) in out
+
+
+def test_contexts_are_independent_ordering_domains():
+    """PAPER L124-L130 / L327, reading 31: fence / quiet / wait act within one (PE, context) pair.  A QUIET (or
+    FENCE) on context 1 does not complete (order) the PE's pending put on context 0; the same program on one context does."""
+    init = [[0, 0, 42, 1, 0, 7], [0] * 6]
+    #            PE0: data put on ctx A; small put + X + flag put on ctx B.   PE1: wait flag; read data.
+    def prog(a, b, x):
+        return [[("put", 1, 0, 2, a), ("put", 1, 5, 5, b), (x, b), ("put", 1, 1, 3, b)],
+                [("wait", 1, "eq", 1), ("get", 1, 4, 0)]]
+    for x in ("quiet", "fence"):
+        two = enumerate_outcomes(prog("@0", "@1", x), init)
+        assert {h[1][4] for h in two} == {0, 42}                # ctx 0's put may still be pending behind ctx 1's marker
+        assert {h[1][5] for h in two} == {7}                    # ... but ctx 1's own earlier put is ordered before the flag
+        one = enumerate_outcomes(prog("@0", "@0", x), init)
+        assert {h[1][4] for h in one} == {42} and len(one) == 1
+        same = enumerate_outcomes(prog("@1", "@1", x), init)    # the context number itself means nothing
+        assert same == one
+        assert oracle_heaps(prog("@0", "@1", x), init, [0, 0, 0, 0, 1, 1]) in two
+    # a wait blocks only its own context's stream: the ctx-0 put of PE1 may be delivered before PE1's ctx-1 wait returns
+    init2 = [[0, 0, 42, 1, 0, 0], [0, 0, 43, 0, 0, 0]]
+    w = [[("get", 1, 4, 0), ("quiet",), ("put", 1, 1, 3)],                     # PE0 reads PE1's word 0, then raises the flag
+         [("wait", 1, "eq", 1, "@1"), ("put", 1, 0, 2, "@1"), ("put", 1, 5, 2, "@0")]]
+    out = enumerate_outcomes(w, init2)
+    assert {h[0][4] for h in out} == {0}                        # the ctx-1 put follows the wait: PE0 always read the old word
+    assert {h[1][0] for h in out} == {43} and {h[1][5] for h in out} == {43}
+    assert oracle_heaps(w, init2, [0, 0, 0, 1, 1, 1]) in out
+
+
+def test_barrier_covers_every_context():
+    init = [[0, 0, 42, 0, 0], [0, 0, 43, 0, 0]]
+    prog = [[("put", 1, 0, 2, "@2"), ("barrier",), ("get", 0, 4, 0, "@1")],
+            [("put", 0, 0, 2, "@1"), ("barrier",), ("get", 1, 4, 0)]]
+    out = enumerate_outcomes(prog, init)
+    assert len(out) == 1
+    h = next(iter(out))
+    assert (h[0][4], h[1][4]) == (43, 42)
+    assert oracle_heaps(prog, init, [0, 1, 0, 1, 0, 1]) in out

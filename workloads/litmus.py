@@ -221,3 +221,31 @@ def two_contexts(npes: int = 8, rounds: int = 10, big: int = 1 << 20, small: int
             prog.signal_wait_until(t, ("flag0", r * 8), CMP_EQ, r + 1, ctx=0)
             prog.get(t, t, ("out", r * (big + small)), ("bulk", r * big), big, ctx=0)
     return prog
+
+
+def contexts_amos_waits(npes: int = 8, rounds: int = 12, seed: int = 18) -> Program:
+    """Fetching AMOs and waits on contexts > 0 (fetch slots and wait words are in the initiating PE's window whatever the
+    context).  Round r, PE p, context c = 1 + r % 3:  FETCH_ADD(+r+1) and COMPARE_SWAP(-1 -> id) on words that only p
+    touches on its neighbour t (so the fetched values are the same under every legal schedule), QUIET(c), then ATOMIC_ADD 1 on
+    t's flag word of the round.  t waits (on another context) for that flag and copies the two words."""
+    prog = Program(npes)
+    init = np.zeros((npes, rounds * 2), dtype=np.uint64)
+    init[:, 1::2] = np.uint64(0xFFFFFFFFFFFFFFFF)
+    init[:, 0::2] = gen.u64(npes * rounds, seed, 0).reshape(npes, rounds)
+    prog.obj("words", rounds * 16, init)
+    prog.obj("flag", rounds * 8)
+    prog.obj("fetch", rounds * 16)
+    prog.obj("out", rounds * 16)
+    for r in range(rounds):
+        c = 1 + r % 3
+        for p in range(npes):
+            t = (p + 1 + r % (npes - 1)) % npes
+            prog.atomic_fetch_add(p, t, ("words", r * 16), r + 1, ("fetch", r * 16), ctx=c)
+            prog.atomic_compare_swap(p, t, ("words", r * 16 + 8), 0xFFFFFFFFFFFFFFFF, 1000 * r + p, ("fetch", r * 16 + 8), ctx=c)
+            prog.quiet(p, ctx=c)
+            prog.atomic_add(p, t, ("flag", r * 8), 1, ctx=c)
+        for t in range(npes):
+            c2 = 1 + (r + 1) % 3
+            prog.signal_wait_until(t, ("flag", r * 8), CMP_GE, 1, ctx=c2)
+            prog.get(t, t, ("out", r * 16), ("words", r * 16), 16, ctx=c2)
+    return prog
