@@ -143,6 +143,7 @@ class Inputs:
         self.groups = groups
         if "c1" in groups:
             self.c1 = configs.c1_atomic_add()
+            self.c1_steady = configs.c1_atomic_add(n_ops=(1 << 18) if small else (1 << 24))   # same distribution
         if "c2" in groups:
             self.halo = configs.Halo(64 if small else 256)
             self.halo_U = self.halo.initial_U()
@@ -190,12 +191,17 @@ def segment_table(inp: Inputs):
                                bytes=n * inp.c5_fc_bytes + n * n * inp.c5_fc_bytes, launches=1)
     if "c1" in g:
         # operand / result streams per op (what HBM must move): C1 tgt_pe 4 + idx 8 + val 8
-        seg["atomic_add"] = dict(cls="amo", kernel="k_amo<add>", ops=len(inp.c1.val), launches=2, bytes_per_op=20)   # + barrier kernel
+        seg["atomic_add"] = dict(cls="amo", kernel="k_amo<add> (quiet + barrier folded into the launch)", ops=len(inp.c1.val),
+                                 launches=1, bytes_per_op=20)
+        # the same distribution, 2^24 ops: the kernel's steady-state rate (reported, not part of `amo_mops`)
+        seg["atomic_add_steady_2p24"] = dict(cls="xamo", kernel="k_amo<add>", ops=len(inp.c1_steady.val), launches=1, bytes_per_op=20)
     if "c4" in g:
         E = len(inp.c4.u)
         # fetch-add: tgt_pe 4 + idx 4 read, 8 fetched written; compare-swap: tgt_pe 4 + idx 4 + val 8 read, 8 fetched written
         seg["atomic_fetch_add"] = dict(cls="amo", kernel="k_hot_sample + k_amo_hot_main<fetch_add>", ops=E, launches=2, bytes_per_op=16)
-        seg["atomic_compare_swap"] = dict(cls="amo", kernel="k_amo<compare_swap>", ops=E, launches=1, bytes_per_op=24)
+        seg["atomic_compare_swap"] = dict(cls="amo", kernel="k_amo<compare_swap, test-before-swap>", ops=E, launches=1, bytes_per_op=24)
+        # every op an L2 atomic (no test load): the variant the atom.cas ceiling bounds; reported, not part of `amo_mops`
+        seg["atomic_compare_swap_plain"] = dict(cls="xamo", kernel="k_amo<compare_swap>", ops=E, launches=1, bytes_per_op=24)
     if "next2" in g:
         # NEXT-2 surface; reported per segment, NOT part of `value` / `amo_mops` (cls x*)
         if "c5" in g:
@@ -203,6 +209,8 @@ def segment_table(inp: Inputs):
             seg["next2_broadcast"] = dict(cls="xcopy", kernel="k_broadcast_tma", bytes=(n + 1) * nb, launches=1)
             seg["next2_reduce_max_i64"] = dict(cls="xcopy", kernel="k_sum_reduce_tma<i64,max>", bytes=2 * n * nb, launches=1)
             seg["next2_reduce_min_f32"] = dict(cls="xcopy", kernel="k_sum_reduce_tma<f32,min>", bytes=2 * n * nb, launches=1)
+            # NEXT-1: the same fp32 sum_reduce as a DEVICE collective (one thread block per PE calls shmemg_dev_sum_reduce_block)
+            seg["next1_dev_sum_reduce_f32"] = dict(cls="xcopy", kernel="k_device_collective (shmemg_dev_sum_reduce_block)", bytes=2 * n * nb, launches=1)
         if "c4" in g:
             seg["next2_amo_xor"] = dict(cls="xamo", kernel="k_amo2<xor>", ops=len(inp.c4.u), launches=1)
             seg["next2_amo_fetch_xor"] = dict(cls="xamo", kernel="k_amo2<fetch_xor>", ops=len(inp.c4.u), launches=1)
@@ -265,7 +273,8 @@ class CudaBench:
     def __init__(self, inp: Inputs, device):
         import torch
         from paper_2607_08006_b200 import World
-        from paper_2607_08006_b200.binding import AMO_HOT_AGGREGATE, AMO_TEST_BEFORE_SWAP
+        from paper_2607_08006_b200.binding import AMO_HOT_AGGREGATE, AMO_TEST_BEFORE_SWAP, AMO_THEN_BARRIER
+        self.c1_flags = AMO_THEN_BARRIER               # C1 ends with quiet + barrier: folded into the AMO launch
         from paper_2607_08006_b200.loader import Loaded
         self.torch, self.inp, self.dev = torch, inp, device
         self.rec = Recorder(torch)
@@ -335,6 +344,8 @@ class CudaBench:
             w = World(c.npes, c.nelem * 8 + 4096, device)
             self.w1, self.A = w, w.calloc(c.nelem, 8)
             self.c1_t, self.c1_i, self.c1_v = dv(c.tgt_pe), dv(c.idx.astype(np.int64)), dv(c.val)
+            cs = inp.c1_steady
+            self.c1s = (dv(cs.tgt_pe), dv(cs.idx.astype(np.int64)), dv(cs.val))
             self.worlds.append(w)
         if "c4" in g:
             q = inp.c4
@@ -346,6 +357,7 @@ class CudaBench:
             self.c4_val = dv(q.u.astype(np.int64))
             self.f_deg = torch.empty(E, dtype=torch.int64, device=device)
             self.f_par = torch.empty(E, dtype=torch.int64, device=device)
+            w.set_scratch_for(E)                       # caller-owned scratch of the hot-set kernels (the library allocates nothing)
             self.worlds.append(w)
         torch.cuda.synchronize(device)
 
@@ -367,12 +379,16 @@ class CudaBench:
             with rec.seg("atomic_compare_swap"):
                 self.w4.atomic_compare_swap_batch(self.par, self.c4_ov, self.c4_lv, self.f_par, cond=None, cond_scalar=M64,
                                                   val=self.c4_val, flags=self.cas_flags)
+            self.w4.view(self.par, vpp * 8).fill_(255)
+            with rec.seg("atomic_compare_swap_plain"):
+                self.w4.atomic_compare_swap_batch(self.par, self.c4_ov, self.c4_lv, self.f_par, cond=None, cond_scalar=M64,
+                                                  val=self.c4_val, flags=0)
         if "c1" in g:
             self.w1.view(self.A, inp.c1.nelem * 8).zero_()
             with rec.seg("atomic_add"):
-                self.w1.atomic_add_batch(self.A, self.c1_t, self.c1_i, val=self.c1_v, flags=self.flags)
-                self.w1.quiet_on_stream(0)
-                self.w1.barrier_all()
+                self.w1.atomic_add_batch(self.A, self.c1_t, self.c1_i, val=self.c1_v, flags=self.flags | self.c1_flags)
+            with rec.seg("atomic_add_steady_2p24"):
+                self.w1.atomic_add_batch(self.A, *self.c1s[:2], val=self.c1s[2], flags=self.flags)
         if "c3a" in g:
             with rec.seg("alltoall"):
                 self.w3a.alltoall(self.a_dst, self.a_src, inp.c3a_blk)
@@ -421,6 +437,8 @@ class CudaBench:
                     self.w5.reduce(RED.MAX, I64, self.d5, self.s_i64, n // 8)
                 with rec.seg("next2_reduce_min_f32"):
                     self.w5.reduce(RED.MIN, F32, self.d5, self.s_f32, n // 4)
+                with rec.seg("next1_dev_sum_reduce_f32"):
+                    self.w5.device_collective(0, self.d5, self.s_f32, n // 4, dtype=F32)
             if "c4" in g:
                 with rec.seg("next2_amo_xor"):
                     self.w4.atomic_op_batch(AMO.XOR, 8, self.deg, self.c4_ou, self.c4_lu, val=self.c4_val)
@@ -539,9 +557,7 @@ class CudaBench:
                 for d, h in zip((self.c1_t, self.c1_i, self.c1_v), self.h_c1):
                     d.copy_(h, non_blocking=True)
                     self.h2d += h.numel() * h.element_size()
-                self.w1.atomic_add_batch(self.A, self.c1_t, self.c1_i, val=self.c1_v, flags=self.flags)
-                self.w1.quiet_on_stream(0)
-                self.w1.barrier_all()
+                self.w1.atomic_add_batch(self.A, self.c1_t, self.c1_i, val=self.c1_v, flags=self.flags | self.c1_flags)
                 self._down(self.w1, self.h_A, self.A)
         if "c4" in g:
             vpp = inp.c4.verts_per_pe
@@ -609,9 +625,9 @@ class CudaBench:
         if "c1" in g:
             c = inp.c1
             self.w1.view(self.A, c.nelem * 8).zero_()
-            self.w1.atomic_add_batch(self.A, self.c1_t, self.c1_i, val=self.c1_v, flags=self.flags)
-            self.w1.quiet_on_stream(0)
-            self.w1.barrier_all()
+            e0 = self.w1.barrier_epoch()
+            self.w1.atomic_add_batch(self.A, self.c1_t, self.c1_i, val=self.c1_v, flags=self.flags | self.c1_flags)
+            assert self.w1.barrier_epoch() == e0 + 1, "the folded barrier did not happen"
             ob.o1.view(ob.A, c.nelem * 8)[:] = 0
             ob.o1.atomic_add_batch(ob.A, c.tgt_pe, c.idx, c.val)
             assert np.array_equal(host(self.w1.view(self.A, c.nelem * 8)), ob.o1.view(ob.A, c.nelem * 8)), "atomic_add"
@@ -693,11 +709,23 @@ class CudaBench:
         if "c1" in g:
             n = 1 << 24
             out["red_add_512KiB_Mops"] = best(lambda: self.w1.probe_atomic(0, self.A, inp.c1.nelem, n), n) / 1e6
+            # (iv) ONE address, without / with warp aggregation
+            out["red_add_single_address_Mops"] = best(lambda: self.w1.probe_atomic_stream(0, self.A, None, None, n), n) / 1e6
+            out["red_add_single_address_warp_aggregated_Mops"] = best(lambda: self.w1.probe_atomic_stream(0, self.A, None, None, n, True), n) / 1e6
+            out["atom_add_single_address_Mops"] = best(lambda: self.w1.probe_atomic_stream(1, self.A, None, None, n >> 2), n >> 2) / 1e6
+            out["atom_add_single_address_warp_aggregated_Mops"] = best(lambda: self.w1.probe_atomic_stream(1, self.A, None, None, n, True), n) / 1e6
+            # what an event pair around the smallest possible kernel costs in this run (launch floor of a 65 536-op batch)
+            out["empty_kernel_event_pair_us"] = 1e6 / best(lambda: self.w1.barrier_all(), 1)
         if "c4" in g:
             n, vpp = len(inp.c4.u), inp.c4.verts_per_pe
             out["red_add_32MiB_Mops"] = best(lambda: self.w4.probe_atomic(0, self.deg, vpp, n), n) / 1e6
             out["atom_add_32MiB_Mops"] = best(lambda: self.w4.probe_atomic(1, self.deg, vpp, n), n) / 1e6
             out["atom_cas_32MiB_Mops"] = best(lambda: self.w4.probe_atomic(2, self.par, vpp, n), n) / 1e6
+            # (iii) the bare atomic on the RMAT address stream itself (operands read, nothing written), without / with warp aggregation
+            for nm, mode, t_, i_, off in (("atom_add", 1, self.c4_ou, self.c4_lu, self.deg), ("red_add", 0, self.c4_ou, self.c4_lu, self.deg),
+                                          ("atom_cas", 2, self.c4_ov, self.c4_lv, self.par)):
+                out[nm + "_rmat_stream_Mops"] = best(lambda: self.w4.probe_atomic_stream(mode, off, t_, i_, n), n) / 1e6
+                out[nm + "_rmat_stream_warp_aggregated_Mops"] = best(lambda: self.w4.probe_atomic_stream(mode, off, t_, i_, n, True), n) / 1e6
         if "c5" in g:
             nb = inp.c5_bytes
             out["copy_all_GBps"] = best(lambda: self.w5.probe_copy_all(self.d5, self.s_f32, nb), 2 * inp.c5_npes * nb) / 1e9
@@ -969,6 +997,9 @@ def run_cuda(args):
         elif t["cls"] == "xamo":
             d["Mops"] = units[k] / world / secs[k] / 1e6
             d["in_headline"] = False
+            if "bytes_per_op" in t:
+                d["bytes_per_op"] = t["bytes_per_op"]
+                d["frac_of_measured_hbm"] = d["Mops"] * 1e6 * t["bytes_per_op"] / 1e9 / peak
         else:
             d["us_per_barrier"] = seg_ms[k] / K / t["ops"] * 1e3
         d["us_per_launch"] = per_launch_ms * 1e3
@@ -986,8 +1017,20 @@ def run_cuda(args):
         segments["atomic_add"]["frac_of_l2_atomic_ceiling"] = segments["atomic_add"]["Mops"] / ceil["red_add_512KiB_Mops"]
     if "atomic_fetch_add" in segments and "atom_add_32MiB_Mops" in ceil:
         segments["atomic_fetch_add"]["frac_of_l2_atomic_ceiling"] = segments["atomic_fetch_add"]["Mops"] / ceil["atom_add_32MiB_Mops"]
-    if "atomic_compare_swap" in segments and "atom_cas_32MiB_Mops" in ceil:
-        segments["atomic_compare_swap"]["frac_of_l2_atomic_ceiling"] = segments["atomic_compare_swap"]["Mops"] / ceil["atom_cas_32MiB_Mops"]
+    if "atomic_fetch_add" in segments and "atom_add_rmat_stream_Mops" in ceil:
+        segments["atomic_fetch_add"]["vs_bare_atom_add_on_the_same_stream"] = segments["atomic_fetch_add"]["Mops"] / ceil["atom_add_rmat_stream_Mops"]
+    if "atomic_compare_swap" in segments:
+        segments["atomic_compare_swap"]["note"] = ("test-before-swap: most of the 2^26 ops are resolved by a coherent load, so the atom.cas "
+                                                   "probe does not bound this variant; its own bound is the operand / result stream "
+                                                   "(bytes_per_op, frac_of_measured_hbm)")
+    if "atomic_compare_swap_plain" in segments and "atom_cas_32MiB_Mops" in ceil:
+        segments["atomic_compare_swap_plain"]["frac_of_l2_atomic_ceiling"] = segments["atomic_compare_swap_plain"]["Mops"] / ceil["atom_cas_32MiB_Mops"]
+        if "atom_cas_rmat_stream_Mops" in ceil:
+            segments["atomic_compare_swap_plain"]["vs_bare_atom_cas_on_the_same_stream"] = segments["atomic_compare_swap_plain"]["Mops"] / ceil["atom_cas_rmat_stream_Mops"]
+    if "atomic_add_steady_2p24" in segments and "red_add_512KiB_Mops" in ceil:
+        segments["atomic_add_steady_2p24"]["frac_of_l2_atomic_ceiling"] = segments["atomic_add_steady_2p24"]["Mops"] / ceil["red_add_512KiB_Mops"]
+    if "atomic_add" in segments and "empty_kernel_event_pair_us" in ceil:
+        segments["atomic_add"]["empty_kernel_event_pair_us"] = ceil["empty_kernel_event_pair_us"]
 
     # dominant copy-class kernel = largest share of the timed copy-class step time
     roofline = None

@@ -71,7 +71,7 @@ enum {
 #define SHMEMG_CAP_HOST_INITIATED_GPU_BUFFERS (1ull << 2)   /* Tier-0 baseline (L465)                    */
 #define SHMEMG_CAP_STREAM_TRIGGERED           (1ull << 3)   /* _on_stream variants (L396, L412)          */
 #define SHMEMG_CAP_DEVICE_INITIATED           (1ull << 4)   /* __device__ entry points (L412, L465)      */
-#define SHMEMG_CAP_DEVICE_COLLECTIVES         (1ull << 5)   /* 0: no device alltoall/reduce/fcollect     */
+#define SHMEMG_CAP_DEVICE_COLLECTIVES         (1ull << 5)   /* shmemg_dev_{sum_reduce,fcollect,alltoall,broadcast}_block (L226, L363) */
 #define SHMEMG_CAP_EXPLICIT_DEVICE_CTX        (1ull << 6)   /* 0 in this build                           */
 #define SHMEMG_CAP_PTR_DEVICE_ACCESSIBLE      (1ull << 7)   /* shmemg_ptr is a device pointer (L353)     */
 #define SHMEMG_CAP_PTR_HOST_ACCESSIBLE        (1ull << 8)   /* 0: not dereferenceable on the host (L456) */
@@ -255,11 +255,20 @@ SHMEMG_API int shmemg_quiet(shmemg_world_t *w, int pe, void *stream);
  * unit is the limiter there): a sampling kernel finds the hot words of the stream (up to 512); in the main kernel every CTA
  * combines its ops on a hot word in shared memory and issues ONE L2 atomic per hot word (op k of the CTA's group fetches
  * old + k*val_scalar: the group executes back to back, legal for the same reason as warp aggregation).  The sample only
- * affects speed, never the result.  Uses scratch in the world's control region and a library-owned device buffer (n bytes,
- * allocated with cudaMalloc on first use -- that call synchronises -- and freed by shmemg_finalize): two calls with this
- * flag must be stream-ordered.  Ignored (the plain kernel runs) when val != NULL, n < 2^20 or n >= 2^33, or the slab has
- * 2^32 or more 64-bit words. */
+ * affects speed, never the result.  Uses scratch in the world's control region and the caller-owned scratch buffer registered with
+ * shmemg_set_scratch (>= shmemg_amo_scratch_bytes(w, n)); two calls with this flag must be stream-ordered.  Ignored (the plain
+ * kernel runs) when no large enough scratch buffer is registered, val != NULL, n < 2^20 or n >= 2^33, or the slab has 2^32 or
+ * more 64-bit words. */
 #define SHMEMG_AMO_HOT_AGGREGATE 4u
+/* quiet for every PE + barrier_all folded into the same launch (config C1 ends with "quiet + barrier"): the end of the kernel
+ * completes every AMO of the call and orders it before later work on the stream; the CTA that finishes last bumps the world's
+ * barrier epoch, exactly what a following shmemg_barrier_all_on_stream would have done with a second launch. */
+#define SHMEMG_AMO_THEN_BARRIER 8u
+/* Caller-owned DEVICE scratch (256-byte aligned) for the calls that need some (SHMEMG_AMO_HOT_AGGREGATE); the library itself
+ * never allocates device memory.  Valid until replaced (scratch_dev NULL: none) or shmemg_finalize; calls that use it must be
+ * stream-ordered.  shmemg_amo_scratch_bytes: what a SHMEMG_AMO_HOT_AGGREGATE call of n ops needs. */
+SHMEMG_API size_t shmemg_amo_scratch_bytes(const shmemg_world_t *w, size_t n);
+SHMEMG_API int shmemg_set_scratch(shmemg_world_t *w, void *scratch_dev, size_t bytes);
 SHMEMG_API int shmemg_atomic_add_batch_on_stream(shmemg_world_t *w, uint64_t sym_off, const int32_t *tgt_pe,
                                                  const void *elem_idx, int idx_bytes, const uint64_t *val,
                                                  uint64_t val_scalar, size_t n, uint32_t flags, void *stream);
@@ -387,9 +396,20 @@ typedef struct shmemg_device_world {
     int32_t reserved;
     unsigned int *bar_count;    /* DEVICE: device-barrier arrival counter (control region)                    */
     unsigned int *bar_gen;      /* DEVICE: device-barrier generation                                          */
+    unsigned int *bar_flags;    /* DEVICE: one monotonic slot per PE of the flag barrier (shmemg_dev_barrier_all_block_pe) */
 } shmemg_device_world_t;
 /* Fill *out (HOST) for world w; valid until shmemg_finalize. */
 SHMEMG_API int shmemg_device_world_get(const shmemg_world_t *w, shmemg_device_world_t *out);
+
+/* Run ONE device collective of include/shmemg_device.cuh device-initiated ("thread-collaborative
+ * collective reductions ... device-callable collective operations", L363-L371 uniform participation): one cooperative kernel with
+ * one thread block per PE; block p calls shmemg_dev_<kind>_block(..., pe = p) with the arguments given here.  kind:
+ * SHMEMG_DEVCOLL_*; dtype (SUM_REDUCE only): SHMEMG_F32 / I64 / I32 / F64; n = nreduce (elements) or nbytes per block; root:
+ * BROADCAST only.  Same results as the stream collectives (fp32 sums accumulate in fp64 in ascending PE order: bit-equal).
+ * Returns SHMEMG_ERR_NOMEM if npes thread blocks cannot be co-resident. */
+enum { SHMEMG_DEVCOLL_SUM_REDUCE = 0, SHMEMG_DEVCOLL_FCOLLECT = 1, SHMEMG_DEVCOLL_ALLTOALL = 2, SHMEMG_DEVCOLL_BROADCAST = 3 };
+SHMEMG_API int shmemg_device_collective_on_stream(shmemg_world_t *w, int kind, int dtype, uint64_t dest_off, uint64_t source_off,
+                                                  size_t n, int root, void *stream);
 
 /* Run an op list DEVICE-INITIATED: one cooperative kernel with one thread block per PE ("PE agent"); agent p walks
  * ops[0..nops) in order and executes those it initiates through the entry points of shmemg_device.cuh with BLOCKING

@@ -287,13 +287,131 @@ __device__ __forceinline__ void shmemg_dev_barrier_all_block(const shmemg_device
             asm volatile("st.relaxed.gpu.global.u32 [%0], %1;" ::"l"(w.bar_count), "r"(0u) : "memory");
             asm volatile("st.release.gpu.global.u32 [%0], %1;" ::"l"(w.bar_gen), "r"(gen + 1u) : "memory");
         } else {
-            unsigned g;
+            unsigned g;                      /* relaxed polling (no L1 invalidate per probe), one acquire fence at the end */
             do {
-                asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(g) : "l"(w.bar_gen) : "memory");
+                asm volatile("ld.relaxed.gpu.global.u32 %0, [%1];" : "=r"(g) : "l"(w.bar_gen) : "memory");
             } while (g == gen);
+            shmemg_dev_fence_gpu();
         }
     }
     __syncthreads();
+}
+
+/* The same barrier for callers that know which PE they act for (one thread block per PE, all co-resident): FLAG barrier, no
+ * read-modify-write -- block p publishes the barrier's number in slot p (release), its first warp polls all slots (relaxed,
+ * 128 slots per 16-byte-per-lane probe) and fences once.  Do not mix with shmemg_dev_barrier_all_block in one kernel. */
+__device__ __forceinline__ void shmemg_dev_barrier_all_block_pe(const shmemg_device_world_t &w, int pe) {
+    shmemg_dev_fence_gpu();                 /* every thread: its own earlier updates */
+    __syncthreads();
+    if (shmemg_dev_block_tid() < 32) {
+        const unsigned lane = (unsigned)shmemg_dev_block_tid(), npes = (unsigned)w.npes;
+        unsigned gen;
+        asm volatile("ld.relaxed.gpu.global.u32 %0, [%1];" : "=r"(gen) : "l"(w.bar_flags + pe) : "memory");
+        ++gen;
+        __syncwarp();
+        if (lane == 0) asm volatile("st.relaxed.gpu.global.u32 [%0], %1;" ::"l"(w.bar_flags + pe), "r"(gen) : "memory");
+        for (unsigned q0 = 0; q0 < npes; q0 += 128) {
+            const unsigned q = q0 + 4 * lane;
+            for (;;) {
+                bool ok = true;
+                if (q < npes) {
+                    unsigned f0, f1, f2, f3;
+                    asm volatile("ld.relaxed.gpu.global.v4.u32 {%0,%1,%2,%3}, [%4];" : "=r"(f0), "=r"(f1), "=r"(f2), "=r"(f3) : "l"(w.bar_flags + q) : "memory");
+                    ok = (int)(f0 - gen) >= 0 && (q + 1 >= npes || (int)(f1 - gen) >= 0) && (q + 2 >= npes || (int)(f2 - gen) >= 0) &&
+                         (q + 3 >= npes || (int)(f3 - gen) >= 0);
+                }
+                if (__all_sync(0xffffffffu, ok)) break;
+            }
+        }
+        shmemg_dev_fence_gpu();
+    }
+    __syncthreads();
+}
+
+/* ---- device collectives (PAPER L226 case study 3 "thread-collaborative collective reductions", L363-L371, Table 6 "Device
+ * collectives: if provided, uniform participation") ------------------------------------------------------------------------
+ * Block scope, ONE thread block per PE: ALL npes blocks (co-resident: cooperative launch) call the routine with the same
+ * arguments except `pe`, every thread of each block takes part.  Each routine is a barrier on entry (every PE's source is
+ * complete) and on exit (every PE's dest is complete and visible to every PE).  Same definitions as the stream collectives of
+ * shmemg.h; source and dest ranges must not overlap (sum_reduce: dest == source allowed). */
+
+/* every PE's dest[k] = sum over PEs (ascending) of source[k].  Reduce-scatter + all-gather: block p sums the p-th share of the
+ * elements over all N windows (fp32: fp64 accumulation, one rounding -- bit-equal to the stream collective) and stores the result
+ * into all N windows, so every element is read N times and written N times in total, the same traffic as k_sum_reduce_tma. */
+template <typename T, typename ACC>
+__device__ __forceinline__ void shmemg_dev_sum_share(const shmemg_device_world_t &w, uint64_t dest_off, uint64_t source_off,
+                                                     size_t lo, size_t hi, int tid, int nthr) {
+    for (size_t k = lo + tid; k < hi; k += nthr) {
+        ACC acc = (ACC)0;
+        for (int q = 0; q < w.npes; ++q)
+            acc += (ACC) * reinterpret_cast<const volatile T *>(shmemg_dev_ptr(w, source_off, q) + k * sizeof(T));
+        const T r = (T)acc;
+        for (int j = 0; j < w.npes; ++j) *reinterpret_cast<T *>(shmemg_dev_ptr(w, dest_off, j) + k * sizeof(T)) = r;
+    }
+}
+__device__ __forceinline__ void shmemg_dev_sum_reduce_block(const shmemg_device_world_t &w, int dtype, uint64_t dest_off,
+                                                            uint64_t source_off, size_t nreduce, int pe) {
+    shmemg_dev_barrier_all_block_pe(w, pe);
+    const int tid = shmemg_dev_block_tid(), nthr = shmemg_dev_block_size();
+    const size_t per = (nreduce + (size_t)w.npes - 1) / (size_t)w.npes;
+    const size_t lo = per * (size_t)pe < nreduce ? per * (size_t)pe : nreduce, hi = lo + per < nreduce ? lo + per : nreduce;
+    if (dtype == SHMEMG_F32) {
+        /* four columns per thread and PE: 16-byte loads when the share is aligned, ascending PE order, fp64 accumulators */
+        const bool vec = ((dest_off | source_off | (uint64_t)w.stride | (uint64_t)(uintptr_t)w.base) & 15) == 0 && (lo & 3) == 0;
+        size_t done = lo;
+        if (vec) {
+            const size_t nv = (hi - lo) >> 2;
+            for (size_t v = tid; v < nv; v += nthr) {
+                double a0 = 0.0, a1 = 0.0, a2 = 0.0, a3 = 0.0;
+                const size_t byte = (lo + 4 * v) * 4;
+#pragma unroll 4
+                for (int q = 0; q < w.npes; ++q) {
+                    float4 x;
+                    asm volatile("ld.global.cg.v4.f32 {%0,%1,%2,%3}, [%4];" : "=f"(x.x), "=f"(x.y), "=f"(x.z), "=f"(x.w)
+                                 : "l"(shmemg_dev_ptr(w, source_off, q) + byte));
+                    a0 += (double)x.x; a1 += (double)x.y; a2 += (double)x.z; a3 += (double)x.w;
+                }
+                const float4 r = make_float4((float)a0, (float)a1, (float)a2, (float)a3);
+                for (int j = 0; j < w.npes; ++j) *reinterpret_cast<float4 *>(shmemg_dev_ptr(w, dest_off, j) + byte) = r;
+            }
+            done = lo + (nv << 2);
+        }
+        shmemg_dev_sum_share<float, double>(w, dest_off, source_off, done, hi, tid, nthr);
+    } else if (dtype == SHMEMG_I64) {
+        shmemg_dev_sum_share<unsigned long long, unsigned long long>(w, dest_off, source_off, lo, hi, tid, nthr);
+    } else if (dtype == SHMEMG_I32) {
+        shmemg_dev_sum_share<unsigned, unsigned>(w, dest_off, source_off, lo, hi, tid, nthr);
+    } else {
+        shmemg_dev_sum_share<double, double>(w, dest_off, source_off, lo, hi, tid, nthr);
+    }
+    shmemg_dev_barrier_all_block_pe(w, pe);
+}
+/* every PE's dest[p*nbytes .. +nbytes) = PE p's source: block p puts its block into all N windows */
+__device__ __forceinline__ void shmemg_dev_fcollect_block(const shmemg_device_world_t &w, uint64_t dest_off, uint64_t source_off,
+                                                          size_t nbytes, int pe) {
+    shmemg_dev_barrier_all_block_pe(w, pe);
+    const int tid = shmemg_dev_block_tid(), nthr = shmemg_dev_block_size();
+    for (int j = 0; j < w.npes; ++j)
+        shmemg_dev_copy(shmemg_dev_ptr(w, dest_off + (uint64_t)pe * nbytes, j), shmemg_dev_ptr(w, source_off, pe), nbytes, tid, nthr);
+    shmemg_dev_barrier_all_block_pe(w, pe);
+}
+/* PE j's dest[i*nbytes .. +nbytes) = PE i's source[j*nbytes .. +nbytes): block i puts its N blocks */
+__device__ __forceinline__ void shmemg_dev_alltoall_block(const shmemg_device_world_t &w, uint64_t dest_off, uint64_t source_off,
+                                                          size_t nbytes, int pe) {
+    shmemg_dev_barrier_all_block_pe(w, pe);
+    const int tid = shmemg_dev_block_tid(), nthr = shmemg_dev_block_size();
+    for (int j = 0; j < w.npes; ++j)
+        shmemg_dev_copy(shmemg_dev_ptr(w, dest_off + (uint64_t)pe * nbytes, j), shmemg_dev_ptr(w, source_off + (uint64_t)j * nbytes, pe),
+                        nbytes, tid, nthr);
+    shmemg_dev_barrier_all_block_pe(w, pe);
+}
+/* every PE's dest = the root's source: every block gets the root's block (the root's own dest included) */
+__device__ __forceinline__ void shmemg_dev_broadcast_block(const shmemg_device_world_t &w, uint64_t dest_off, uint64_t source_off,
+                                                           size_t nbytes, int root_pe, int pe) {
+    shmemg_dev_barrier_all_block_pe(w, pe);
+    shmemg_dev_copy(shmemg_dev_ptr(w, dest_off, pe), shmemg_dev_ptr(w, source_off, root_pe), nbytes, shmemg_dev_block_tid(),
+                    shmemg_dev_block_size());
+    shmemg_dev_barrier_all_block_pe(w, pe);
 }
 
 #endif /* __CUDACC__ */

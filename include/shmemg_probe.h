@@ -24,6 +24,14 @@ enum { SHMEMG_PROBE_RED_ADD = 0, SHMEMG_PROBE_ATOM_ADD = 1, SHMEMG_PROBE_ATOM_CA
 SHMEMG_API int shmemg_probe_atomic_on_stream(shmemg_world_t *w, int mode, uint64_t sym_off, uint64_t words_per_pe,
                                              size_t n, void *stream);
 
+/* The same bare atomics on a GIVEN address stream: op i targets u64 heap[tgt_pe[i]][sym_off + 8*elem_idx[i]] (DEVICE arrays of n
+ * entries: the workload's own operand arrays, e.g. the RMAT endpoints of config C4), or, with tgt_pe == elem_idx == NULL, on the
+ * ONE word heap[0][sym_off].  aggregate != 0: a warp issues one atomic per distinct address (what SHMEMG_AMO_WARP_AGGREGATE
+ * does).  Adds 0 / compares against a value the word never holds: the heap is left unchanged.  These are the like-for-like
+ * ceilings of SURVEY.md 8(d) (iii) "RMAT-skewed as C4" and (iv) "single address". */
+SHMEMG_API int shmemg_probe_atomic_stream_on_stream(shmemg_world_t *w, int mode, uint64_t sym_off, const int32_t *tgt_pe,
+                                                    const uint32_t *elem_idx, size_t n, int aggregate, void *stream);
+
 /* Plain device copy ceiling with the library's own streaming loop: heap[pe_dst][dst_off..] = heap[pe_src][src_off..]
  * is shmemg_put_on_stream; this probe instead reports nothing new and exists only so bench.py can time the kernel
  * on one contiguous `nbytes` range per PE pair for every PE at once (npes independent copies, one launch). */

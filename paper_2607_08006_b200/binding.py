@@ -73,9 +73,14 @@ class AMO:
     ADD, AND, OR, XOR, SWAP, FETCH = range(6)
 
 
+class DEVCOLL:
+    SUM_REDUCE, FCOLLECT, ALLTOALL, BROADCAST = range(4)
+
+
 AMO_WARP_AGGREGATE = 1
 AMO_TEST_BEFORE_SWAP = 2
 AMO_HOT_AGGREGATE = 4
+AMO_THEN_BARRIER = 8
 NO_STAMP = (1 << 64) - 1
 
 # shmemg_op_t, 64 bytes
@@ -120,6 +125,8 @@ SYMBOLS = {
     "shmemg_fence_on_stream": (_i, [_vp, _i, _vp]),
     "shmemg_quiet_on_stream": (_i, [_vp, _i, _vp]),
     "shmemg_quiet": (_i, [_vp, _i, _vp]),
+    "shmemg_amo_scratch_bytes": (_sz, [_vp, _sz]),
+    "shmemg_set_scratch": (_i, [_vp, _vp, _sz]),
     "shmemg_atomic_add_batch_on_stream": (_i, [_vp, _u64, _vp, _vp, _i, _vp, _u64, _sz, _u32, _vp]),
     "shmemg_atomic_fetch_add_batch_on_stream": (_i, [_vp, _u64, _vp, _vp, _i, _vp, _u64, _vp, _sz, _u32, _vp]),
     "shmemg_atomic_compare_swap_batch_on_stream": (_i, [_vp, _u64, _vp, _vp, _i, _vp, _u64, _vp, _u64, _vp, _sz, _u32, _vp]),
@@ -146,12 +153,14 @@ SYMBOLS = {
     "shmemg_barrier_all_repeat_on_stream": (_i, [_vp, _u32, _u64, _vp]),
     "shmemg_barrier_epoch": (_u64, [_vp, _vp]),
     "shmemg_device_world_get": (_i, [_vp, _vp]),
+    "shmemg_device_collective_on_stream": (_i, [_vp, _i, _i, _u64, _u64, _sz, _i, _vp]),
     "shmemg_device_exec_ops_on_stream": (_i, [_vp, _vp, _sz, _vp, _vp, C.POINTER(_sz)]),
     "shmemg_app_halo_perturb_on_stream": (_i, [_vp, _u64, _u32, _u64, _u64, _vp]),
     "shmemg_app_halo_pack_on_stream": (_i, [_vp, _u64, _u64, _u32, _vp]),
     "shmemg_app_checksum64_on_stream": (_i, [_vp, _vp, _u64, _u64, _u32, _vp]),
     "shmemg_app_halo_persistent_on_stream": (_i, [_vp, _u64, _u64, _u64, _u32, _u64, _u64, _u32, _vp]),
     "shmemg_probe_atomic_on_stream": (_i, [_vp, _i, _u64, _u64, _sz, _vp]),
+    "shmemg_probe_atomic_stream_on_stream": (_i, [_vp, _i, _u64, _vp, _vp, _sz, _i, _vp]),
     "shmemg_probe_copy_all_on_stream": (_i, [_vp, _u64, _u64, _sz, _vp]),
 }
 
@@ -365,7 +374,23 @@ class World:
         self._keep.append(ops_dev)                 # must stay valid until the stream has passed the call
         self.launches += 1 if len(ops) else 0
 
+    def device_collective(self, kind, dest_off, source_off, n, dtype=0, root=0, stream=None):
+        """One device collective run device-initiated: block p calls shmemg_dev_<kind>_block (include/shmemg_device.cuh)."""
+        self._chk(lib().shmemg_device_collective_on_stream(self.h, kind, dtype, dest_off, source_off, n, root, _stream(stream)),
+                  "shmemg_device_collective_on_stream")
+        self.launches += 1 if n else 0
+
     # ---- SoA AMO batches -------------------------------------------------------------------------------------------
+    def set_scratch_for(self, n: int):
+        """Register a caller-owned scratch buffer large enough for SHMEMG_AMO_HOT_AGGREGATE calls of up to n ops."""
+        need = lib().shmemg_amo_scratch_bytes(self.h, n)
+        self._scratch = torch.empty(need, dtype=torch.uint8, device=self.device)
+        self._chk(lib().shmemg_set_scratch(self.h, self._scratch.data_ptr(), need), "shmemg_set_scratch")
+
+    def _hot(self, flags, val, n):
+        return bool(flags & AMO_HOT_AGGREGATE) and val is None and n >= (1 << 20) and getattr(self, "_scratch", None) is not None \
+            and self._scratch.numel() >= lib().shmemg_amo_scratch_bytes(self.h, n)
+
     @staticmethod
     def _idx_bytes(elem_idx):
         assert elem_idx.dtype in (torch.int32, torch.int64, torch.uint32, torch.uint64)
@@ -377,7 +402,7 @@ class World:
                                                           self._idx_bytes(elem_idx), _dptr(val), val_scalar & NO_STAMP,
                                                           n, flags, _stream(stream)),
                   "shmemg_atomic_add_batch_on_stream")
-        self.launches += (2 if (flags & AMO_HOT_AGGREGATE) and val is None and n >= (1 << 20) else 1) if n else 0
+        self.launches += (2 if self._hot(flags, val, n) else 1) if n or (flags & AMO_THEN_BARRIER) else 0
 
     def atomic_fetch_add_batch(self, sym_off, tgt_pe, elem_idx, fetched_out, val=None, val_scalar=0, flags=0,
                                stream=None):
@@ -388,7 +413,7 @@ class World:
                                                                 _stream(stream)),
                   "shmemg_atomic_fetch_add_batch_on_stream")
         # launch accounting: SHMEMG_AMO_HOT_AGGREGATE runs a sampling kernel in front of the main one (n >= 2^20, scalar value)
-        self.launches += (2 if (flags & AMO_HOT_AGGREGATE) and val is None and n >= (1 << 20) else 1) if n else 0
+        self.launches += (2 if self._hot(flags, val, n) else 1) if n or (flags & AMO_THEN_BARRIER) else 0
 
     def atomic_compare_swap_batch(self, sym_off, tgt_pe, elem_idx, fetched_out, cond=None, cond_scalar=0, val=None,
                                   val_scalar=0, flags=0, stream=None):
@@ -518,6 +543,11 @@ class World:
     def probe_atomic(self, mode, sym_off, words_per_pe, n, stream=None):
         self._chk(lib().shmemg_probe_atomic_on_stream(self.h, mode, sym_off, words_per_pe, n, _stream(stream)),
                   "shmemg_probe_atomic_on_stream")
+
+    def probe_atomic_stream(self, mode, sym_off, tgt_pe, elem_idx, n, aggregate=False, stream=None):
+        self._chk(lib().shmemg_probe_atomic_stream_on_stream(self.h, mode, sym_off, _dptr(tgt_pe), _dptr(elem_idx), n,
+                                                             1 if aggregate else 0, _stream(stream)),
+                  "shmemg_probe_atomic_stream_on_stream")
 
     def probe_copy_all(self, dst_off, src_off, nbytes, stream=None):
         self._chk(lib().shmemg_probe_copy_all_on_stream(self.h, dst_off, src_off, nbytes, _stream(stream)),

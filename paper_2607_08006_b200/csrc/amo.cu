@@ -33,14 +33,34 @@ struct AmoArgs {
     unsigned long long cond_s;
     unsigned long long *fetched;
     size_t n;
+    CtlRegion *then_barrier;       // SHMEMG_AMO_THEN_BARRIER: the CTA that finishes last bumps the world's barrier epoch
 };
+
+// quiet + barrier_all folded into the end of an AMO kernel: the end of the kernel completes every AMO of the call (quiet for
+// every PE) and orders it before everything later on the stream; what a separate barrier launch would add is the epoch bump,
+// which the last CTA to finish performs after a GPU-scope fence.
+__device__ __forceinline__ void amo_then_barrier(CtlRegion *ctl) {
+    if (!ctl) return;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        __threadfence();
+        if (atomicAdd(&ctl->amo_done, 1u) == gridDim.x - 1) {
+            ctl->amo_done = 0;
+            __threadfence();
+            atomicAdd(&ctl->barrier_epoch, 1ull);
+        }
+    }
+}
 
 __device__ __forceinline__ unsigned long long shfl64(unsigned long long v, int lane) {
     return __shfl_sync(FULL, v, lane);
 }
 
+#ifndef AMO_MIN_CTAS
+#define AMO_MIN_CTAS 1
+#endif
 template <int IDXB, int OP, bool AGG, bool TEST>
-__global__ void __launch_bounds__(256) k_amo(const AmoArgs a) {
+__global__ void __launch_bounds__(256, AMO_MIN_CTAS) k_amo(const AmoArgs a) {
     typedef typename IdxT<IDXB>::type idx_t;
     const idx_t *__restrict__ idx = reinterpret_cast<const idx_t *>(a.idx);
     const int *__restrict__ tgt = a.tgt_pe;
@@ -135,6 +155,7 @@ __global__ void __launch_bounds__(256) k_amo(const AmoArgs a) {
             }
         }
     }
+    amo_then_barrier(a.then_barrier);
 }
 
 
@@ -310,6 +331,7 @@ __global__ void __launch_bounds__(256, 6) k_amo_hot_main(const AmoArgs a, const 
             const unsigned long long c = slot[j];
             if (c) asm volatile("red.relaxed.gpu.global.add.u64 [%0], %1;" ::"l"(slab + ht.hkeys[j]), "l"(c * a.val_s) : "memory");
         }
+        amo_then_barrier(a.then_barrier);
         return;
     }
     const unsigned nl = list_n < cap ? list_n : cap;
@@ -329,6 +351,7 @@ __global__ void __launch_bounds__(256, 6) k_amo_hot_main(const AmoArgs a, const 
         const unsigned long long r = list[e];
         a.fetched[r & imask] = slot[(r >> HOT_I_BITS) & (SHMEMG_HOT_MAX - 1)] + (r >> 43) * a.val_s;
     }
+    amo_then_barrier(a.then_barrier);
 }
 
 // usable when the value is one scalar and every word of the slab has a 32-bit index; small calls keep the plain kernel
@@ -354,19 +377,13 @@ static int launch_amo_hot(shmemg_world *w, const AmoArgs &a, int idx_bytes, cuda
     const size_t blocks = (size_t)w->sm_count * per_sm * waves;
     const size_t per_cta = (a.n + blocks - 1) / blocks;
     if (per_cta >= ((size_t)1 << 21) * 8 || a.n >= ((size_t)1 << HOT_I_BITS)) return SHMEMG_ERR_NOMEM;   // caller falls back
-    const unsigned cap = (unsigned)(per_cta / 8 + 32);
-    unsigned long long *lists = nullptr;
-    {                                                         // library-owned scratch, grown on demand (first call synchronises)
-        const size_t need = (size_t)HOT_SAMPLES * 4 + (OP == AMO_FADD ? blocks * (size_t)cap * 8 : 0);
-        if (w->hot_scratch_bytes < need) {
-            if (w->hot_scratch) SHMEMG_CUDA(w, cudaFree(w->hot_scratch));
-            w->hot_scratch = nullptr; w->hot_scratch_bytes = 0;
-            SHMEMG_CUDA(w, cudaMalloc(&w->hot_scratch, need));
-            w->hot_scratch_bytes = need;
-        }
-        if (OP == AMO_FADD) lists = (unsigned long long *)((uint8_t *)w->hot_scratch + (size_t)HOT_SAMPLES * 4);
-    }
-    unsigned *staged = (unsigned *)w->hot_scratch;
+    unsigned cap = (unsigned)(per_cta / 8 + 32);
+    if (cap > (1u << 21)) cap = 1u << 21;                     // the rank field of a hot-op record is 21 bits
+    // scratch comes from the caller (shmemg_set_scratch): the library allocates no device memory
+    const size_t need = (size_t)HOT_SAMPLES * 4 + (OP == AMO_FADD ? blocks * (size_t)cap * 8 : 0);
+    if (!w->scratch || w->scratch_bytes < need) return SHMEMG_ERR_NOMEM;     // caller falls back to the plain kernel
+    unsigned long long *lists = OP == AMO_FADD ? (unsigned long long *)((uint8_t *)w->scratch + (size_t)HOT_SAMPLES * 4) : nullptr;
+    unsigned *staged = (unsigned *)w->scratch;
     if (idx_bytes == 4) {
         k_hot_sample<4><<<HOT_SAMPLES / 1024, 1024, HOT_SLOTS_SAMPLE * 8, st>>>(a, w->ctl, staged);
         k_amo_hot_main<4, OP><<<(unsigned)blocks, 256, 0, st>>>(a, w->ctl, lists, cap);
@@ -381,9 +398,11 @@ static int launch_amo_hot(shmemg_world *w, const AmoArgs &a, int idx_bytes, cuda
 
 template <int OP>
 static int launch_amo(shmemg_world *w, const AmoArgs &a, int idx_bytes, uint32_t flags, cudaStream_t st) {
-    if (a.n == 0) return SHMEMG_OK;
+    if (a.n == 0) return a.then_barrier ? shmemg_barrier_all_on_stream(w, st) : SHMEMG_OK;
     const int threads = 256;
-    size_t blocks = (a.n + (size_t)threads * AMO_ITEMS - 1) / ((size_t)threads * AMO_ITEMS);
+    // one op per thread until the grid is full (a 65 536-op batch then runs on 256 CTAs instead of 64: its time is the latency
+    // of one trip, so it wants every SM), AMO_ITEMS ops per thread and trip beyond that
+    size_t blocks = (a.n + (size_t)threads - 1) / (size_t)threads;
     const size_t cap = (size_t)w->sm_count * 8 * 4;        // 8 resident CTAs per SM, ~4 waves worth of grid stride
     if (blocks > cap) blocks = cap;
     const bool agg = flags & SHMEMG_AMO_WARP_AGGREGATE;
@@ -419,8 +438,12 @@ extern "C" int shmemg_atomic_add_batch_on_stream(shmemg_world_t *w, uint64_t sym
                                                  uint64_t val_scalar, size_t n, uint32_t flags, void *stream) {
     int rc = check_common(w, sym_off, tgt_pe, elem_idx, idx_bytes, n);
     if (rc) return rc;
-    AmoArgs a{w->base, w->stride, sym_off, tgt_pe, elem_idx, (const unsigned long long *)val, val_scalar, nullptr, 0, nullptr, n};
-    if (hot_agg_ok(w, a, flags)) return launch_amo_hot<AMO_ADD>(w, a, idx_bytes, (cudaStream_t)stream);
+    AmoArgs a{w->base, w->stride, sym_off, tgt_pe, elem_idx, (const unsigned long long *)val, val_scalar, nullptr, 0, nullptr, n,
+              (flags & SHMEMG_AMO_THEN_BARRIER) ? w->ctl : nullptr};
+    if (hot_agg_ok(w, a, flags)) {
+        rc = launch_amo_hot<AMO_ADD>(w, a, idx_bytes, (cudaStream_t)stream);
+        if (rc != SHMEMG_ERR_NOMEM) return rc;                 // no (or too small a) scratch buffer: the plain kernel
+    }
     return launch_amo<AMO_ADD>(w, a, idx_bytes, flags, (cudaStream_t)stream);
 }
 
@@ -432,8 +455,11 @@ extern "C" int shmemg_atomic_fetch_add_batch_on_stream(shmemg_world_t *w, uint64
     if (rc) return rc;
     if (n && !fetched_out) return SHMEMG_ERR_ARG;
     AmoArgs a{w->base, w->stride, sym_off, tgt_pe, elem_idx, (const unsigned long long *)val, val_scalar, nullptr, 0,
-              (unsigned long long *)fetched_out, n};
-    if (hot_agg_ok(w, a, flags)) return launch_amo_hot<AMO_FADD>(w, a, idx_bytes, (cudaStream_t)stream);
+              (unsigned long long *)fetched_out, n, (flags & SHMEMG_AMO_THEN_BARRIER) ? w->ctl : nullptr};
+    if (hot_agg_ok(w, a, flags)) {
+        rc = launch_amo_hot<AMO_FADD>(w, a, idx_bytes, (cudaStream_t)stream);
+        if (rc != SHMEMG_ERR_NOMEM) return rc;
+    }
     return launch_amo<AMO_FADD>(w, a, idx_bytes, flags, (cudaStream_t)stream);
 }
 
@@ -446,6 +472,28 @@ extern "C" int shmemg_atomic_compare_swap_batch_on_stream(shmemg_world_t *w, uin
     if (rc) return rc;
     if (n && !fetched_out) return SHMEMG_ERR_ARG;
     AmoArgs a{w->base, w->stride, sym_off, tgt_pe, elem_idx, (const unsigned long long *)val, val_scalar,
-              (const unsigned long long *)cond, cond_scalar, (unsigned long long *)fetched_out, n};
+              (const unsigned long long *)cond, cond_scalar, (unsigned long long *)fetched_out, n,
+              (flags & SHMEMG_AMO_THEN_BARRIER) ? w->ctl : nullptr};
     return launch_amo<AMO_CAS>(w, a, idx_bytes, flags, (cudaStream_t)stream);
+}
+
+
+// ---- caller-provided scratch (the library allocates no device memory) -------------------------------------------------------
+extern "C" size_t shmemg_amo_scratch_bytes(const shmemg_world_t *w, size_t n) {
+    if (!w) return 0;
+    // what launch_amo_hot needs for a fetch-add batch of n ops: staged sample keys + the per-CTA hot-op lists
+    int per_sm = 0;
+    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_amo_hot_main<4, AMO_FADD>, 256, 0);
+    if (per_sm < 1) per_sm = 1;
+    const size_t blocks = (size_t)w->sm_count * per_sm * 8;
+    size_t cap = (n + blocks - 1) / blocks / 8 + 32;
+    if (cap > ((size_t)1 << 21)) cap = (size_t)1 << 21;
+    return (size_t)HOT_SAMPLES * 4 + blocks * cap * 8;
+}
+extern "C" int shmemg_set_scratch(shmemg_world_t *w, void *scratch_dev, size_t bytes) {
+    if (!w || (!scratch_dev && bytes)) return SHMEMG_ERR_ARG;
+    if ((uintptr_t)scratch_dev % 256) return SHMEMG_ERR_ALIGN;
+    w->scratch = scratch_dev;
+    w->scratch_bytes = scratch_dev ? bytes : 0;
+    return SHMEMG_OK;
 }

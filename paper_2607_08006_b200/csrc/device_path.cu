@@ -18,6 +18,7 @@ extern "C" int shmemg_device_world_get(const shmemg_world_t *w, shmemg_device_wo
     out->reserved = 0;
     out->bar_count = &w->ctl->bar_count;
     out->bar_gen = &w->ctl->bar_gen;
+    out->bar_flags = w->ctl->bar_flags;
     return SHMEMG_OK;
 }
 
@@ -98,5 +99,50 @@ extern "C" int shmemg_device_exec_ops_on_stream(shmemg_world_t *w, const shmemg_
     const shmemg_op_t *od = reinterpret_cast<const shmemg_op_t *>(ops_dev);
     void *args[] = {&dw, &od, &nops};
     SHMEMG_CUDA(w, cudaLaunchCooperativeKernel((void *)k_device_exec_ops, dim3((unsigned)w->npes), dim3(AGENT_THREADS), args, 0, st));
+    return SHMEMG_OK;
+}
+
+
+// ---- one device collective, device-initiated: one thread block per PE calls the block-scope routine of shmemg_device.cuh ----
+#define COLL_THREADS 1024
+__global__ void __launch_bounds__(COLL_THREADS) k_device_collective(const shmemg_device_world_t dw, int kind, int dtype, uint64_t dest_off,
+                                                                    uint64_t source_off, size_t n, int root) {
+    const int p = blockIdx.x;
+    switch (kind) {
+    case SHMEMG_DEVCOLL_SUM_REDUCE: shmemg_dev_sum_reduce_block(dw, dtype, dest_off, source_off, n, p); break;
+    case SHMEMG_DEVCOLL_FCOLLECT: shmemg_dev_fcollect_block(dw, dest_off, source_off, n, p); break;
+    case SHMEMG_DEVCOLL_ALLTOALL: shmemg_dev_alltoall_block(dw, dest_off, source_off, n, p); break;
+    default: shmemg_dev_broadcast_block(dw, dest_off, source_off, n, root, p); break;
+    }
+}
+
+extern "C" int shmemg_device_collective_on_stream(shmemg_world_t *w, int kind, int dtype, uint64_t dest_off, uint64_t source_off,
+                                                  size_t n, int root, void *stream) {
+    if (!w || kind < SHMEMG_DEVCOLL_SUM_REDUCE || kind > SHMEMG_DEVCOLL_BROADCAST) return SHMEMG_ERR_ARG;
+    uint64_t dbytes = n, sbytes = n;
+    if (kind == SHMEMG_DEVCOLL_SUM_REDUCE) {
+        if (dtype < SHMEMG_F32 || dtype > SHMEMG_F64) return SHMEMG_ERR_ARG;
+        const uint64_t esz = (dtype == SHMEMG_F32 || dtype == SHMEMG_I32) ? 4 : 8;
+        dbytes = sbytes = (uint64_t)n * esz;
+        if ((dest_off | source_off) & (esz - 1)) return SHMEMG_ERR_ALIGN;
+    } else if (kind == SHMEMG_DEVCOLL_FCOLLECT) {
+        dbytes = (uint64_t)n * w->npes;
+    } else if (kind == SHMEMG_DEVCOLL_ALLTOALL) {
+        dbytes = sbytes = (uint64_t)n * w->npes;
+    } else if (!shmemg_pe_ok(w, root)) {
+        return SHMEMG_ERR_PE;
+    }
+    if (!shmemg_in_range(w, dest_off, dbytes) || !shmemg_in_range(w, source_off, sbytes)) return SHMEMG_ERR_RANGE;
+    if (n == 0) return SHMEMG_OK;
+    const bool overlap = dest_off < source_off + sbytes && source_off < dest_off + dbytes;
+    if (overlap && !(kind == SHMEMG_DEVCOLL_SUM_REDUCE && dest_off == source_off)) return SHMEMG_ERR_OVERLAP;
+    int per_sm = 0;
+    SHMEMG_CUDA(w, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_device_collective, COLL_THREADS, 0));
+    if ((long long)per_sm * w->sm_count < w->npes || w->npes > SHMEMG_BAR_FLAGS) return SHMEMG_ERR_NOMEM;
+    shmemg_device_world_t dw;
+    shmemg_device_world_get(w, &dw);
+    void *args[] = {&dw, &kind, &dtype, &dest_off, &source_off, &n, &root};
+    SHMEMG_CUDA(w, cudaLaunchCooperativeKernel((void *)k_device_collective, dim3((unsigned)w->npes), dim3(COLL_THREADS), args, 0,
+                                               (cudaStream_t)stream));
     return SHMEMG_OK;
 }

@@ -19,6 +19,7 @@
 #define SHMEMG_TMA_TILE 32768u             // bytes per bulk-copy stage
 #define SHMEMG_TMA_STAGES 4                // stages per CTA (128 KiB of shared memory, one CTA per SM)
 #define SHMEMG_SIG_SLOTS 1024              // completion counters for single put_signal launches
+#define SHMEMG_BAR_FLAGS 2048               // PE agents the in-kernel flag barrier supports
 #define SHMEMG_HOT_MAX 512                 // hot words tracked by SHMEMG_AMO_HOT_AGGREGATE
 
 // ---- control region layout (device) -------------------------------------------------------------------
@@ -29,6 +30,8 @@ struct CtlRegion {
     unsigned int pad[12];
     unsigned int sig_counter[SHMEMG_SIG_SLOTS];   // last-arriver counters of single put_signal launches
     unsigned int group_bar[128];           // per-PE arrival counters of multi-block PE agents (monotonic; halo_app.cu)
+    unsigned int bar_flags[SHMEMG_BAR_FLAGS];   // in-kernel flag barrier: slot p = number of the last barrier agent p has entered
+    unsigned int amo_done;                 // SHMEMG_AMO_THEN_BARRIER: CTAs of the AMO kernel that have finished
     unsigned int hot_n;                    // SHMEMG_AMO_HOT_AGGREGATE: number of hot words found by the sampling kernel
     unsigned int hot_done;                 // CTAs of the sampling kernel that have staged their keys
     unsigned int hot_keys[SHMEMG_HOT_MAX]; // their slab word indices
@@ -58,8 +61,8 @@ struct shmemg_world {
     struct Team { int start, stride, size; };
     int teams_world_npes = 0;              // npes of the world while a team view is active (surface2.cu)
     std::vector<Team> teams;               // user teams (shmemg_team_split_strided); handle = SHMEMG_TEAM_USER0 + index
-    void *hot_scratch = nullptr;           // DEVICE: library-owned scratch of SHMEMG_AMO_HOT_AGGREGATE (grown on demand)
-    size_t hot_scratch_bytes = 0;
+    void *scratch = nullptr;               // DEVICE: caller-owned scratch (shmemg_set_scratch), used by SHMEMG_AMO_HOT_AGGREGATE
+    size_t scratch_bytes = 0;
     std::string last_cuda_error;
 };
 

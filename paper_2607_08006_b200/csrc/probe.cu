@@ -33,6 +33,34 @@ __global__ void __launch_bounds__(256) k_probe_atomic(uint8_t *base, size_t stri
     if (MODE != SHMEMG_PROBE_RED_ADD && acc == 0x0123456789ABCDEFull && n == (size_t)-1) *sink = acc;
 }
 
+// The same bare atomics on a GIVEN address stream (op i -> word elem_idx[i] of PE tgt_pe[i]: the workload's own operand
+// arrays, 8 bytes read per op, nothing written) or on ONE address, with or without warp aggregation (one L2 atomic per
+// distinct address and warp, as SHMEMG_AMO_WARP_AGGREGATE issues them): the like-for-like ceilings of SURVEY.md 8(d) (iii) / (iv).
+template <int MODE, bool AGG, bool STREAM>
+__global__ void __launch_bounds__(256) k_probe_atomic2(uint8_t *base, size_t stride, uint64_t sym_off, const int *tgt_pe,
+                                                       const unsigned *elem_idx, size_t n, unsigned long long *sink) {
+    unsigned long long acc = 0;
+    const size_t T = (size_t)gridDim.x * blockDim.x;
+    const int lane = threadIdx.x & 31;
+    const size_t first = ((size_t)blockIdx.x * blockDim.x + threadIdx.x) - lane;
+    for (size_t i0 = first; i0 < n; i0 += T) {                 // warp-uniform trip count (match.any below)
+        const size_t i = i0 + lane;
+        const bool ok = i < n;
+        unsigned long long *p = reinterpret_cast<unsigned long long *>(base + sym_off);
+        if (STREAM && ok) p = reinterpret_cast<unsigned long long *>(base + (size_t)tgt_pe[i] * stride + sym_off) + elem_idx[i];
+        bool issue = ok;
+        if (AGG) {
+            const unsigned grp = __match_any_sync(0xffffffffu, ok ? (unsigned long long)p : (unsigned long long)lane);
+            issue = ok && lane == __ffs(grp) - 1;
+        }
+        if (!issue) continue;
+        if (MODE == SHMEMG_PROBE_RED_ADD) asm volatile("red.relaxed.gpu.global.add.u64 [%0], %1;" ::"l"(p), "l"(0ull) : "memory");
+        else if (MODE == SHMEMG_PROBE_ATOM_ADD) acc ^= atomicAdd(p, 0ull);
+        else acc ^= atomicCAS(p, 0x5DEECE66D1234567ull ^ (unsigned long long)i, 0ull);
+    }
+    if (MODE != SHMEMG_PROBE_RED_ADD && acc == 0x0123456789ABCDEFull && n == (size_t)-1) *sink = acc;
+}
+
 __global__ void __launch_bounds__(SHMEMG_THREADS, 4)
 k_probe_copy_all(uint8_t *base, size_t stride, uint64_t dst_off, uint64_t src_off, size_t nbytes, unsigned npes,
                  unsigned chunk, unsigned chunks_per_pe) {
@@ -81,6 +109,33 @@ extern "C" int shmemg_probe_atomic_on_stream(shmemg_world_t *w, int mode, uint64
         k_probe_atomic<SHMEMG_PROBE_ATOM_ADD><<<(unsigned)blocks, 256, 0, st>>>(w->base, w->stride, sym_off, (unsigned)w->npes, words_per_pe, n, sink);
     else
         k_probe_atomic<SHMEMG_PROBE_ATOM_CAS><<<(unsigned)blocks, 256, 0, st>>>(w->base, w->stride, sym_off, (unsigned)w->npes, words_per_pe, n, sink);
+    SHMEMG_CUDA(w, cudaGetLastError());
+    return SHMEMG_OK;
+}
+
+template <int MODE> static void launch_probe2(bool agg, bool stream_src, unsigned blocks, cudaStream_t st, uint8_t *base, size_t stride,
+                                              uint64_t sym_off, const int *tgt, const unsigned *idx, size_t n, unsigned long long *sink) {
+    if (agg) { if (stream_src) k_probe_atomic2<MODE, true, true><<<blocks, 256, 0, st>>>(base, stride, sym_off, tgt, idx, n, sink);
+               else k_probe_atomic2<MODE, true, false><<<blocks, 256, 0, st>>>(base, stride, sym_off, tgt, idx, n, sink); }
+    else { if (stream_src) k_probe_atomic2<MODE, false, true><<<blocks, 256, 0, st>>>(base, stride, sym_off, tgt, idx, n, sink);
+           else k_probe_atomic2<MODE, false, false><<<blocks, 256, 0, st>>>(base, stride, sym_off, tgt, idx, n, sink); }
+}
+
+extern "C" int shmemg_probe_atomic_stream_on_stream(shmemg_world_t *w, int mode, uint64_t sym_off, const int32_t *tgt_pe,
+                                                    const uint32_t *elem_idx, size_t n, int aggregate, void *stream) {
+    if (!w || mode < SHMEMG_PROBE_RED_ADD || mode > SHMEMG_PROBE_ATOM_CAS || ((tgt_pe == nullptr) != (elem_idx == nullptr))) return SHMEMG_ERR_ARG;
+    if (sym_off & 7) return SHMEMG_ERR_ALIGN;
+    if (!shmemg_in_range(w, sym_off, 8)) return SHMEMG_ERR_RANGE;
+    if (n == 0) return SHMEMG_OK;
+    size_t blocks = (n + 255) / 256;
+    const size_t cap = (size_t)w->sm_count * 8 * 4;
+    if (blocks > cap) blocks = cap;
+    unsigned long long *sink = reinterpret_cast<unsigned long long *>(&w->ctl->pad[0]);
+    cudaStream_t st = (cudaStream_t)stream;
+    const bool src = tgt_pe != nullptr;
+    if (mode == SHMEMG_PROBE_RED_ADD) launch_probe2<SHMEMG_PROBE_RED_ADD>(aggregate != 0, src, (unsigned)blocks, st, w->base, w->stride, sym_off, tgt_pe, elem_idx, n, sink);
+    else if (mode == SHMEMG_PROBE_ATOM_ADD) launch_probe2<SHMEMG_PROBE_ATOM_ADD>(aggregate != 0, src, (unsigned)blocks, st, w->base, w->stride, sym_off, tgt_pe, elem_idx, n, sink);
+    else launch_probe2<SHMEMG_PROBE_ATOM_CAS>(aggregate != 0, src, (unsigned)blocks, st, w->base, w->stride, sym_off, tgt_pe, elem_idx, n, sink);
     SHMEMG_CUDA(w, cudaGetLastError());
     return SHMEMG_OK;
 }

@@ -88,7 +88,6 @@ extern "C" int shmemg_init(int npes, size_t heap_bytes_per_pe, void *device_slab
 
 extern "C" int shmemg_finalize(shmemg_world_t *w) {
     if (!w) return SHMEMG_ERR_ARG;
-    if (w->hot_scratch) cudaFree(w->hot_scratch);
     delete w;
     return SHMEMG_OK;
 }
@@ -110,7 +109,7 @@ extern "C" int shmem_query_capabilities(const shmemg_world_t *w, int team, uint6
     if (team == SHMEM_TEAM_WORLD)
         c |= SHMEMG_CAP_HOST_INITIATED_GPU_BUFFERS | SHMEMG_CAP_STREAM_TRIGGERED | SHMEMG_CAP_STREAM_COLLECTIVES;
     else
-        c |= SHMEMG_CAP_DEVICE_INITIATED | SHMEMG_CAP_DEVICE_BARRIER;   // include/shmemg_device.cuh
+        c |= SHMEMG_CAP_DEVICE_INITIATED | SHMEMG_CAP_DEVICE_BARRIER | SHMEMG_CAP_DEVICE_COLLECTIVES;   // include/shmemg_device.cuh
     *caps = c;
     return SHMEMG_OK;
 }

@@ -9,7 +9,8 @@ from gpu_common import DEV, assert_objects_equal, heap_bytes_for, run_gpu, run_o
 from invariants import check_compare_swap_claim, check_fetch_add
 from oracle import oracle as orc
 from paper_2607_08006_b200 import CAP, CMP, ERR, SIGNAL, TEAM, ShmemgError, World
-from paper_2607_08006_b200.binding import AMO_HOT_AGGREGATE, AMO_TEST_BEFORE_SWAP, AMO_WARP_AGGREGATE, F32, I64
+from paper_2607_08006_b200.binding import (AMO_HOT_AGGREGATE, AMO_TEST_BEFORE_SWAP, AMO_THEN_BARRIER, AMO_WARP_AGGREGATE,
+                                           F32, I64)
 from paper_2607_08006_b200.loader import Loaded
 from workloads import configs, gen
 
@@ -106,18 +107,48 @@ def test_c1_atomic_add_bit_exact(flags, idx_dtype):
     assert np.array_equal(w.view(a, wl.nelem * 8).cpu().numpy(), ow.view(oa, wl.nelem * 8))
 
 
+def test_c1_quiet_and_barrier_folded_into_the_amo_launch():
+    """SHMEMG_AMO_THEN_BARRIER: one launch does the adds, the quiet and the barrier (epoch bump by the last CTA); every AMO
+    entry point, the hot-set kernels and the empty call included."""
+    wl = configs.c1_atomic_add()
+    w = World(wl.npes, wl.nelem * 8 + 4096, DEV)
+    a = w.calloc(wl.nelem, 8)
+    t, i, v = to_dev(wl.tgt_pe), to_dev(wl.idx.astype(np.int64)), to_dev(wl.val)
+    e0, l0 = w.barrier_epoch(), w.launches
+    w.atomic_add_batch(a, t, i, val=v, flags=AMO_THEN_BARRIER)
+    assert w.launches == l0 + 1 and w.barrier_epoch() == e0 + 1
+    ow = orc.OracleWorld(wl.npes, wl.nelem * 8 + 4096)
+    oa = ow.malloc(wl.nelem * 8)
+    ow.atomic_add_batch(oa, wl.tgt_pe, wl.idx, wl.val)
+    assert np.array_equal(w.view(a, wl.nelem * 8).cpu().numpy(), ow.view(oa, wl.nelem * 8))
+    f = torch.empty(len(wl.val), dtype=torch.int64, device=DEV)
+    w.atomic_fetch_add_batch(a, t, i, f, val=v, flags=AMO_THEN_BARRIER)
+    w.atomic_compare_swap_batch(a, t, i, f, cond_scalar=0, val_scalar=1, flags=AMO_THEN_BARRIER)
+    e = torch.empty(0, dtype=torch.int32, device=DEV)
+    w.atomic_add_batch(a, e, e, val_scalar=1, flags=AMO_THEN_BARRIER)                # no ops: still a barrier
+    assert w.barrier_epoch() == e0 + 4
+    n = 1 << 20
+    w.set_scratch_for(n)
+    z = torch.zeros(n, dtype=torch.int32, device=DEV)
+    f = torch.empty(n, dtype=torch.int64, device=DEV)
+    w.atomic_fetch_add_batch(a, z, z, f, val_scalar=1, flags=AMO_THEN_BARRIER | AMO_HOT_AGGREGATE)
+    w.atomic_add_batch(a, z, z, val_scalar=1, flags=AMO_THEN_BARRIER | AMO_HOT_AGGREGATE)
+    assert w.barrier_epoch() == e0 + 6
+
+
 def test_atomic_add_heavy_contention_and_scalar_value():
     n = 1 << 20
     w = World(2, 4096, DEV)
     a = w.calloc(8, 8)
     tgt = torch.zeros(n, dtype=torch.int32, device=DEV)
     idx = (torch.arange(n, device=DEV) % 3).to(torch.int32)
-    for flags in (0, AMO_WARP_AGGREGATE, AMO_HOT_AGGREGATE):
+    for flags in (0, AMO_WARP_AGGREGATE, AMO_HOT_AGGREGATE, AMO_HOT_AGGREGATE):
         w.atomic_add_batch(a, tgt, idx, val=None, val_scalar=M64, flags=flags)       # adds -1 (wraparound)
+        w.set_scratch_for(n)                   # third pass: no scratch registered -> the plain kernel; fourth: the hot-set kernels
     w.quiet(0)
     v = w.view(a, 64, torch.int64).cpu().numpy()
     cnt = np.bincount(np.arange(n) % 3, minlength=3)
-    assert v[0, :3].tolist() == (-3 * cnt).tolist() and v[1].sum() == 0
+    assert v[0, :3].tolist() == (-4 * cnt).tolist() and v[1].sum() == 0
 
 
 @pytest.mark.parametrize("n", [1, 1025, 3 * 8192 + 77, (1 << 20) + 5, (1 << 21) + 1029])
@@ -137,6 +168,7 @@ def test_fetch_add_skewed_scalar_value_ragged(n, flags, idx_dtype):
     key = ((r % np.uint64(npes * words)) >> (r >> np.uint64(60))).astype(np.int64)      # skewed towards small keys
     tgt, idx = (key // words).astype(np.int32), (key % words).astype(idx_dtype)
     f = torch.empty(n, dtype=torch.int64, device=DEV)
+    w.set_scratch_for(n)                                     # caller-owned scratch of the hot-set kernels
     w.atomic_fetch_add_batch(a, to_dev(tgt), to_dev(idx), f, val=None, val_scalar=7, flags=flags)
     w.quiet(0)
     fin = w.view(a, words * 8, torch.int64).cpu().numpy().view(np.uint64).reshape(-1)
@@ -158,6 +190,7 @@ def _run_c4(g, flags):
     w.view(par, vpp * 8, torch.int64).fill_(-1)
     f_deg = torch.empty(E, dtype=torch.int64, device=DEV)
     f_par = torch.empty(E, dtype=torch.int64, device=DEV)
+    w.set_scratch_for(E)
     w.atomic_fetch_add_batch(deg, to_dev(g.owner(g.u)), to_dev(g.local(g.u).astype(np.uint32)), f_deg, val=None,
                              val_scalar=1, flags=flags)
     w.atomic_compare_swap_batch(par, to_dev(g.owner(g.v)), to_dev(g.local(g.v).astype(np.uint32)), f_par,

@@ -66,6 +66,7 @@ def test_whole_window_transfer_and_single_word_storm():
     w.view(0, 8, torch.int64).zero_()
     z = torch.zeros(n, dtype=torch.int32, device=DEV)
     f = torch.empty(n, dtype=torch.int64, device=DEV)
+    w.set_scratch_for(n)
     w.atomic_fetch_add_batch(0, z, z, f, val_scalar=3, flags=AMO_HOT_AGGREGATE)
     w.quiet(0)
     assert w.view(0, 8, torch.int64).cpu().numpy()[0, 0] == 3 * n

@@ -21,7 +21,8 @@ def test_capabilities_distinguish_the_device_path():
     """capability queries distinguish host-initiated GPU-aware from device-initiated support."""
     w = World(4, 4096, DEV)
     host, dev = w.query_capabilities(TEAM.WORLD), w.query_capabilities(TEAM.DEVICE_WORLD)
-    assert dev & CAP.DEVICE_INITIATED and dev & CAP.DEVICE_BARRIER and not dev & CAP.DEVICE_COLLECTIVES
+    assert dev & CAP.DEVICE_INITIATED and dev & CAP.DEVICE_BARRIER and dev & CAP.DEVICE_COLLECTIVES
+    assert not host & CAP.DEVICE_COLLECTIVES
     assert not host & CAP.DEVICE_INITIATED and host & CAP.STREAM_TRIGGERED
     assert w.query_capabilities(TEAM.DEVICE_SHARED) == dev          # one GPU: shared == world (L357)
 
@@ -153,3 +154,71 @@ def test_halo_persistent_device_initiated_matches_oracle(B, rounds, split):
         ow.run_program(h.round_ops(prog, r, False))
     assert_objects_equal(prog, ld, ow, names=["ghost", "sig"])
     assert np.array_equal(ld.obj_numpy("U", np.float64), ow.obj("U", np.float64))
+
+
+# ---- device collectives (shmemg_dev_{sum_reduce,fcollect,alltoall,broadcast}_block) ----------------------
+from oracle import oracle as orc                                       # noqa: E402
+from paper_2607_08006_b200.binding import DEVCOLL, F32, F64, I32, I64   # noqa: E402
+import torch                                                            # noqa: E402
+
+
+def _worlds(npes, hb):
+    return World(npes, hb, DEV), orc.OracleWorld(npes, hb)
+
+
+@pytest.mark.parametrize("npes,n,off", [(8, 4096, 0), (128, 1 << 14, 0), (5, 1001, 4), (3, 7, 0), (16, 1, 8), (128, 100, 0)])
+def test_device_sum_reduce_matches_oracle(npes, n, off):
+    """fp32 (fp64 accumulation in PE order: bit-equal to the oracle's (float) of the fp64 sum), int64, int32, fp64; ragged
+    counts, fewer elements than PEs, unaligned (to 16 B) offsets, in place."""
+    w, ow = _worlds(npes, 16 * n + 8192)
+    s, d = w.malloc(8 * n + 64) + off, w.malloc(8 * n + 64) + off
+    os_, od = ow.malloc(8 * n + 64) + off, ow.malloc(8 * n + 64) + off
+    xf = gen.normal_f32(npes * n, 31).reshape(npes, n)
+    w.view(s, 4 * n, torch.float32).copy_(torch.from_numpy(xf)); ow.view(os_, 4 * n, np.float32)[:] = xf
+    w.device_collective(DEVCOLL.SUM_REDUCE, d, s, n, dtype=F32); ow.sum_reduce_f32(od, os_, n); w.quiet(0)
+    assert np.array_equal(w.view(d, 4 * n, torch.float32).cpu().numpy(), ow.view(od, 4 * n, np.float32))
+    xi = gen.uniform_i64(npes * n, -(1 << 40), 1 << 40, 32).reshape(npes, n)
+    o8 = off & ~7
+    s8, d8, os8, od8 = s - off + o8, d - off + o8, os_ - off + o8, od - off + o8
+    w.view(s8, 8 * n, torch.int64).copy_(torch.from_numpy(xi)); ow.view(os8, 8 * n, np.int64)[:] = xi
+    w.device_collective(DEVCOLL.SUM_REDUCE, d8, s8, n, dtype=I64); ow.sum_reduce_i64(od8, os8, n); w.quiet(0)
+    assert np.array_equal(w.view(d8, 8 * n, torch.int64).cpu().numpy(), ow.view(od8, 8 * n, np.int64))
+    w.device_collective(DEVCOLL.SUM_REDUCE, s8, s8, n, dtype=I64); ow.sum_reduce_i64(os8, os8, n); w.quiet(0)     # in place
+    assert np.array_equal(w.view(s8, 8 * n, torch.int64).cpu().numpy(), ow.view(os8, 8 * n, np.int64))
+    for dt, name, tt, nt in ((I32, "i32", torch.int32, np.int32), (F64, "f64", torch.float64, np.float64)):
+        esz = np.dtype(nt).itemsize
+        x = (gen.uniform_i64(npes * n, -1000, 1000, 33).reshape(npes, n)).astype(nt)
+        w.view(s8, esz * n, tt).copy_(torch.from_numpy(x)); ow.view(os8, esz * n, nt)[:] = x
+        w.device_collective(DEVCOLL.SUM_REDUCE, d8, s8, n, dtype=dt); ow.reduce("sum", name, od8, os8, n); w.quiet(0)
+        assert np.array_equal(w.view(d8, esz * n, tt).cpu().numpy(), ow.view(od8, esz * n, nt))
+
+
+@pytest.mark.parametrize("npes,nb,off", [(8, 4096, 0), (64, 32768, 0), (7, 1001, 3), (128, 513, 0), (4, 1, 5)])
+def test_device_fcollect_alltoall_broadcast_match_oracle(npes, nb, off):
+    w, ow = _worlds(npes, 3 * npes * (nb + 16) + 8192)
+    s, d = w.malloc(npes * nb + 64) + off, w.malloc(npes * nb + 64) + (off * 7) % 16
+    os_, od = ow.malloc(npes * nb + 64) + off, ow.malloc(npes * nb + 64) + (off * 7) % 16
+    pay = np.ascontiguousarray(gen.u64(npes * (npes * nb // 8 + 1), 41).view(np.uint8).reshape(npes, -1)[:, :npes * nb])
+    w.view(s, npes * nb).copy_(torch.from_numpy(pay)); ow.view(os_, npes * nb)[:] = pay
+    w.device_collective(DEVCOLL.ALLTOALL, d, s, nb); ow.alltoall(od, os_, nb); w.quiet(0)
+    assert np.array_equal(w.view(d, npes * nb).cpu().numpy(), ow.view(od, npes * nb))
+    w.device_collective(DEVCOLL.FCOLLECT, d, s, nb); ow.fcollect(od, os_, nb); w.quiet(0)
+    assert np.array_equal(w.view(d, npes * nb).cpu().numpy(), ow.view(od, npes * nb))
+    for root in (0, npes - 1):
+        w.device_collective(DEVCOLL.BROADCAST, d, s, nb, root=root); ow.broadcast(od, os_, nb, root); w.quiet(0)
+        assert np.array_equal(w.view(d, npes * nb).cpu().numpy(), ow.view(od, npes * nb))
+
+
+def test_device_collective_argument_checks():
+    w = World(4, 1 << 16, DEV)
+    a, b = w.malloc(4096), w.malloc(4096)
+    for kw, code in [(dict(kind=9, dest_off=b, source_off=a, n=8), ERR.ARG),
+                     (dict(kind=DEVCOLL.SUM_REDUCE, dest_off=b, source_off=a, n=8, dtype=7), ERR.ARG),
+                     (dict(kind=DEVCOLL.SUM_REDUCE, dest_off=b + 4, source_off=a, n=8, dtype=I64), ERR.ALIGN),
+                     (dict(kind=DEVCOLL.ALLTOALL, dest_off=b, source_off=a, n=1 << 15), ERR.RANGE),
+                     (dict(kind=DEVCOLL.FCOLLECT, dest_off=a + 64, source_off=a, n=256), ERR.OVERLAP),
+                     (dict(kind=DEVCOLL.BROADCAST, dest_off=b, source_off=a, n=8, root=4), ERR.PE)]:
+        with pytest.raises(ShmemgError) as e:
+            w.device_collective(**kw)
+        assert e.value.code == code, (kw, e.value)
+    w.device_collective(DEVCOLL.FCOLLECT, b, a, 0)               # zero bytes: nothing enqueued
