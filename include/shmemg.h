@@ -72,7 +72,7 @@ enum {
 #define SHMEMG_CAP_STREAM_TRIGGERED           (1ull << 3)   /* _on_stream variants (L396, L412)          */
 #define SHMEMG_CAP_DEVICE_INITIATED           (1ull << 4)   /* __device__ entry points (L412, L465)      */
 #define SHMEMG_CAP_DEVICE_COLLECTIVES         (1ull << 5)   /* shmemg_dev_{sum_reduce,fcollect,alltoall,broadcast}_block (L226, L363) */
-#define SHMEMG_CAP_EXPLICIT_DEVICE_CTX        (1ull << 6)   /* 0 in this build                           */
+#define SHMEMG_CAP_EXPLICIT_DEVICE_CTX        (1ull << 6)   /* shmemg_ctx_create + shmemg_dev_*_nbi / shmemg_dev_ctx_* (L327, L331) */
 #define SHMEMG_CAP_PTR_DEVICE_ACCESSIBLE      (1ull << 7)   /* shmemg_ptr is a device pointer (L353)     */
 #define SHMEMG_CAP_PTR_HOST_ACCESSIBLE        (1ull << 8)   /* 0: not dereferenceable on the host (L456) */
 #define SHMEMG_CAP_PROGRESS_GPU_ONLY          (1ull << 9)   /* no host proxy needed (L394, L431)         */
@@ -400,6 +400,63 @@ typedef struct shmemg_device_world {
 } shmemg_device_world_t;
 /* Fill *out (HOST) for world w; valid until shmemg_finalize. */
 SHMEMG_API int shmemg_device_world_get(const shmemg_world_t *w, shmemg_device_world_t *out);
+
+/* ---- explicit device contexts ("explicit contexts as an advanced option", L331 "host-
+ * created contexts that may be cached in GPU-accessible memory for later use by kernels") -------------------------------------
+ * A context belongs to ONE PE and is an independent ordering / completion domain of that PE's device-initiated operations: it
+ * owns a queue of pending NON-BLOCKING operations and its own completion counters (issued, completed).  The host creates it in
+ * caller-owned DEVICE memory and receives a POD handle that kernels take BY VALUE (or read from device memory); see the `_nbi`
+ * and `shmemg_dev_ctx_*` entry points of shmemg_device.cuh:
+ *   - shmemg_dev_put_nbi / get_nbi / put_signal_nbi return before LOCAL completion: the transfer is recorded in
+ *     the context and performed no later than the context's next quiet / fence, the PE's next barrier, or the next time the PE
+ *     blocks (wait): the source must not change and a get's data must not be read until shmemg_dev_ctx_quiet has returned;
+ *   - shmemg_dev_ctx_quiet(ctx) completes the operations of THAT context only; a quiet on another context of the same PE leaves
+ *     them pending (their counters do not move);
+ *   - the operations without a context argument keep using SHMEM_DEVICE_CTX_DEFAULT, which has no queue (they are blocking).
+ * One thread (or one thread block, with uniform participation) uses a context at a time. */
+typedef struct shmemg_nbi_rec {      /* 64 B: one pending non-blocking operation, addresses resolved */
+    uint64_t dst, src, nbytes;
+    uint64_t sig;                    /* put_signal: signal word (0 = none) */
+    uint64_t sig_value;
+    uint32_t sig_op, pad0;
+    uint64_t pad1[2];
+} shmemg_nbi_rec_t;
+typedef struct shmemg_device_ctx {
+    shmemg_nbi_rec_t *queue;         /* DEVICE: ring of `capacity` records                                      */
+    unsigned long long *counters;    /* DEVICE: [0] = operations issued, [1] = operations completed (monotonic)  */
+    uint32_t capacity;
+    int32_t pe;                      /* the PE this context belongs to (the initiator of its operations)         */
+} shmemg_device_ctx_t;
+/* DEVICE bytes a context with a queue of `queue_entries` pending operations needs (0 on bad arguments). */
+SHMEMG_API size_t shmemg_ctx_bytes(uint32_t queue_entries);
+/* Create a context for PE `pe` in ctx_mem_dev (DEVICE, 256-byte aligned, >= shmemg_ctx_bytes, caller-owned, must outlive every
+ * kernel that uses the handle); its counters are zeroed on `stream`.  *out (HOST) receives the handle. */
+SHMEMG_API int shmemg_ctx_create(shmemg_world_t *w, int pe, uint32_t queue_entries, void *ctx_mem_dev, size_t ctx_mem_bytes,
+                                 void *stream, shmemg_device_ctx_t *out);
+/* Read the context's counters (synchronises `stream`): operations issued / completed so far. */
+SHMEMG_API int shmemg_ctx_counters(shmemg_world_t *w, const shmemg_device_ctx_t *ctx, void *stream, uint64_t *issued,
+                                   uint64_t *completed);
+/* Like shmemg_device_exec_ops_on_stream, with explicit contexts: ctxs_dev is a DEVICE array of npes * nctx handles (entry
+ * pe * nctx + c = context c of PE pe; every op's ctx field must be < nctx).  PUT / GET / PUT_SIGNAL are issued NON-BLOCKING on
+ * their op's context, FENCE / QUIET act on that context only, AMOs are issued at once, a wait first progresses the PE's pending
+ * operations (all its contexts), BARRIER_ALL and the end of the list complete everything (flags: SHMEMG_EXEC_*). */
+#define SHMEMG_EXEC_LEAVE_PENDING 1u   /* no quiet at the end of the list: what is still queued stays pending in its context (contexts
+                                        * live in device memory across kernels) until a later call completes it */
+SHMEMG_API int shmemg_device_exec_ops_ctx_on_stream(shmemg_world_t *w, const shmemg_op_t *ops_host, size_t nops, void *ops_dev,
+                                                    const shmemg_device_ctx_t *ctxs_dev, int nctx, uint32_t flags, void *stream,
+                                                    size_t *bad_index);
+
+/* ---- non-blocking forms on a stream ("For nonblocking operations ... completion only after an explicit quiet") ---
+ * Host-issued, stream-ordered like shmemg_put_on_stream / shmemg_get_on_stream; the difference is the contract: a blocking
+ * `_on_stream` put is locally complete for every LATER operation on the stream, a `_nbi` one only after the next
+ * shmemg_quiet_on_stream / shmemg_quiet / shmemg_barrier_all_on_stream of that stream.  In this implementation stream order
+ * already provides both, so the two forms launch the same kernels; programs that need the weaker contract only can say so. */
+SHMEMG_API int shmemg_put_nbi_on_stream(shmemg_world_t *w, uint64_t dest_off, uint64_t source_off, size_t nbytes, int pe,
+                                        int target_pe, void *stream);
+SHMEMG_API int shmemg_get_nbi_on_stream(shmemg_world_t *w, uint64_t dest_off, uint64_t source_off, size_t nbytes, int pe,
+                                        int target_pe, void *stream);
+SHMEMG_API int shmemg_put_signal_nbi_on_stream(shmemg_world_t *w, uint64_t dest_off, uint64_t source_off, size_t nbytes,
+                                               uint64_t sig_off, uint64_t signal, int sig_op, int pe, int target_pe, void *stream);
 
 /* Run ONE device collective of include/shmemg_device.cuh device-initiated ("thread-collaborative
  * collective reductions ... device-callable collective operations", L363-L371 uniform participation): one cooperative kernel with

@@ -297,6 +297,76 @@ __device__ __forceinline__ void shmemg_dev_barrier_all_block(const shmemg_device
     __syncthreads();
 }
 
+/* ---- explicit contexts and non-blocking operations (see shmemg.h "explicit device contexts") -------
+ * A context's queue holds the PE's pending non-blocking operations; `counters[0]` counts the operations issued on it,
+ * `counters[1]` those completed.  Thread scope: ONE thread uses the context; `_block`: all threads of the block, same arguments. */
+__device__ __forceinline__ unsigned long long shmemg_dev_ctx_issued(const shmemg_device_ctx_t &c) {
+    return *reinterpret_cast<volatile unsigned long long *>(c.counters);
+}
+__device__ __forceinline__ unsigned long long shmemg_dev_ctx_completed(const shmemg_device_ctx_t &c) {
+    return *reinterpret_cast<volatile unsigned long long *>(c.counters + 1);
+}
+__device__ __forceinline__ unsigned long long shmemg_dev_ctx_pending(const shmemg_device_ctx_t &c) {
+    return shmemg_dev_ctx_issued(c) - shmemg_dev_ctx_completed(c);
+}
+/* perform the pending operations of the context in issue order (threads tid of nthr cooperate); then one GPU-scope fence */
+__device__ __forceinline__ void shmemg_dev_ctx_drain(const shmemg_device_ctx_t &c, int tid, int nthr) {
+    const unsigned long long issued = shmemg_dev_ctx_issued(c), done = shmemg_dev_ctx_completed(c);
+    for (unsigned long long k = done; k < issued; ++k) {
+        const shmemg_nbi_rec_t r = c.queue[k % c.capacity];
+        shmemg_dev_copy(reinterpret_cast<unsigned char *>(r.dst), reinterpret_cast<const unsigned char *>(r.src), (size_t)r.nbytes, tid, nthr);
+        if (r.sig) {                                  /* put_signal: the signal after the whole payload */
+            shmemg_dev_fence_gpu();
+            if (nthr > 1) __syncthreads();
+            if (tid == 0) shmemg_dev_signal_update(reinterpret_cast<unsigned long long *>(r.sig), r.sig_value, (int)r.sig_op);
+        }
+    }
+    shmemg_dev_fence_gpu();
+}
+/* quiet: every operation issued on THIS context is complete and visible; other contexts of the PE are left alone */
+__device__ __forceinline__ void shmemg_dev_ctx_quiet(const shmemg_device_ctx_t &c) {
+    shmemg_dev_ctx_drain(c, 0, 1);
+    *reinterpret_cast<volatile unsigned long long *>(c.counters + 1) = shmemg_dev_ctx_issued(c);
+}
+__device__ __forceinline__ void shmemg_dev_ctx_quiet_block(const shmemg_device_ctx_t &c) {
+    __syncthreads();
+    shmemg_dev_ctx_drain(c, shmemg_dev_block_tid(), shmemg_dev_block_size());
+    __syncthreads();
+    if (shmemg_dev_block_tid() == 0) *reinterpret_cast<volatile unsigned long long *>(c.counters + 1) = shmemg_dev_ctx_issued(c);
+    __syncthreads();
+}
+/* fence: operations issued on this context afterwards are delivered after the earlier ones.  The pending ones are delivered
+ * here (always conformant: stronger than required) */
+__device__ __forceinline__ void shmemg_dev_ctx_fence(const shmemg_device_ctx_t &c) { shmemg_dev_ctx_quiet(c); }
+__device__ __forceinline__ void shmemg_dev_ctx_fence_block(const shmemg_device_ctx_t &c) { shmemg_dev_ctx_quiet_block(c); }
+/* record one operation; a full queue is drained first (a non-blocking operation may complete at any time before the quiet) */
+__device__ __forceinline__ void shmemg_dev_ctx_push(const shmemg_device_ctx_t &c, const shmemg_nbi_rec_t &r) {
+    if (shmemg_dev_ctx_pending(c) >= c.capacity) shmemg_dev_ctx_quiet(c);
+    const unsigned long long k = shmemg_dev_ctx_issued(c);
+    c.queue[k % c.capacity] = r;
+    *reinterpret_cast<volatile unsigned long long *>(c.counters) = k + 1;
+}
+__device__ __forceinline__ void shmemg_dev_put_nbi(const shmemg_device_world_t &w, const shmemg_device_ctx_t &c, uint64_t dest_off,
+                                                   uint64_t source_off, size_t nbytes, int target_pe) {
+    shmemg_nbi_rec_t r = {};
+    r.dst = (uint64_t)shmemg_dev_ptr(w, dest_off, target_pe); r.src = (uint64_t)shmemg_dev_ptr(w, source_off, c.pe); r.nbytes = nbytes;
+    shmemg_dev_ctx_push(c, r);
+}
+__device__ __forceinline__ void shmemg_dev_get_nbi(const shmemg_device_world_t &w, const shmemg_device_ctx_t &c, uint64_t dest_off,
+                                                   uint64_t source_off, size_t nbytes, int target_pe) {
+    shmemg_nbi_rec_t r = {};
+    r.dst = (uint64_t)shmemg_dev_ptr(w, dest_off, c.pe); r.src = (uint64_t)shmemg_dev_ptr(w, source_off, target_pe); r.nbytes = nbytes;
+    shmemg_dev_ctx_push(c, r);
+}
+__device__ __forceinline__ void shmemg_dev_put_signal_nbi(const shmemg_device_world_t &w, const shmemg_device_ctx_t &c, uint64_t dest_off,
+                                                          uint64_t source_off, size_t nbytes, uint64_t sig_off, uint64_t signal,
+                                                          int sig_op, int target_pe) {
+    shmemg_nbi_rec_t r = {};
+    r.dst = (uint64_t)shmemg_dev_ptr(w, dest_off, target_pe); r.src = (uint64_t)shmemg_dev_ptr(w, source_off, c.pe); r.nbytes = nbytes;
+    r.sig = (uint64_t)shmemg_dev_ptr(w, sig_off, target_pe); r.sig_value = signal; r.sig_op = (uint32_t)sig_op;
+    shmemg_dev_ctx_push(c, r);
+}
+
 /* The same barrier for callers that know which PE they act for (one thread block per PE, all co-resident): FLAG barrier, no
  * read-modify-write -- block p publishes the barrier's number in slot p (release), its first warp polls all slots (relaxed,
  * 128 slots per 16-byte-per-lane probe) and fences once.  Do not mix with shmemg_dev_barrier_all_block in one kernel. */

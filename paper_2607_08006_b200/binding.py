@@ -153,6 +153,13 @@ SYMBOLS = {
     "shmemg_barrier_all_repeat_on_stream": (_i, [_vp, _u32, _u64, _vp]),
     "shmemg_barrier_epoch": (_u64, [_vp, _vp]),
     "shmemg_device_world_get": (_i, [_vp, _vp]),
+    "shmemg_ctx_bytes": (_sz, [_u32]),
+    "shmemg_ctx_create": (_i, [_vp, _i, _u32, _vp, _sz, _vp, _vp]),
+    "shmemg_ctx_counters": (_i, [_vp, _vp, _vp, C.POINTER(_u64), C.POINTER(_u64)]),
+    "shmemg_device_exec_ops_ctx_on_stream": (_i, [_vp, _vp, _sz, _vp, _vp, _i, _u32, _vp, C.POINTER(_sz)]),
+    "shmemg_put_nbi_on_stream": (_i, [_vp, _u64, _u64, _sz, _i, _i, _vp]),
+    "shmemg_get_nbi_on_stream": (_i, [_vp, _u64, _u64, _sz, _i, _i, _vp]),
+    "shmemg_put_signal_nbi_on_stream": (_i, [_vp, _u64, _u64, _sz, _u64, _u64, _i, _i, _i, _vp]),
     "shmemg_device_collective_on_stream": (_i, [_vp, _i, _i, _u64, _u64, _sz, _i, _vp]),
     "shmemg_device_exec_ops_on_stream": (_i, [_vp, _vp, _sz, _vp, _vp, C.POINTER(_sz)]),
     "shmemg_app_halo_perturb_on_stream": (_i, [_vp, _u64, _u32, _u64, _u64, _vp]),
@@ -373,6 +380,59 @@ class World:
         self._keep = getattr(self, "_keep", [])
         self._keep.append(ops_dev)                 # must stay valid until the stream has passed the call
         self.launches += 1 if len(ops) else 0
+
+    # ---- explicit device contexts (shmemg_ctx_create; include/shmemg_device.cuh `_nbi` / `shmemg_dev_ctx_*`) -------------
+    CTX_DTYPE = np.dtype([("queue", "u8"), ("counters", "u8"), ("capacity", "u4"), ("pe", "i4")])     # shmemg_device_ctx_t
+
+    def ctx_create_all(self, nctx: int, queue_entries: int = 64, stream=None):
+        """One context per (PE, c < nctx): returns (host array of handles [npes * nctx], the same array on the device);
+        the context memory is a torch tensor kept alive by this object."""
+        L = lib()
+        per = L.shmemg_ctx_bytes(queue_entries)
+        per = (per + 255) // 256 * 256
+        mem = torch.empty(self.npes * nctx * per, dtype=torch.uint8, device=self.device)
+        handles = np.zeros(self.npes * nctx, dtype=self.CTX_DTYPE)
+        for p in range(self.npes):
+            for c in range(nctx):
+                k = p * nctx + c
+                self._chk(L.shmemg_ctx_create(self.h, p, queue_entries, mem.data_ptr() + k * per, per, _stream(stream),
+                                              handles[k:k + 1].ctypes.data), "shmemg_ctx_create")
+        dev = torch.from_numpy(handles.view(np.uint8).reshape(-1).copy()).to(self.device)
+        self._keep = getattr(self, "_keep", []) + [mem, dev]
+        return handles, dev
+
+    def ctx_counters(self, handles: np.ndarray, k: int, stream=None):
+        a, b = C.c_uint64(0), C.c_uint64(0)
+        self._chk(lib().shmemg_ctx_counters(self.h, handles[k:k + 1].ctypes.data, _stream(stream), C.byref(a), C.byref(b)),
+                  "shmemg_ctx_counters")
+        return a.value, b.value
+
+    def device_exec_ops_ctx(self, ops: np.ndarray, ctxs_dev: torch.Tensor, nctx: int, flags: int = 0, stream=None):
+        assert ops.dtype == OP_DTYPE
+        ops = np.ascontiguousarray(ops)
+        ops_dev = torch.empty(max(len(ops), 1) * OP_DTYPE.itemsize, dtype=torch.uint8, device=self.device)
+        bad = C.c_size_t(0)
+        rc = lib().shmemg_device_exec_ops_ctx_on_stream(self.h, ops.ctypes.data, len(ops), ops_dev.data_ptr(), ctxs_dev.data_ptr(),
+                                                        nctx, flags, _stream(stream), C.byref(bad))
+        if rc:
+            raise ShmemgError(rc, "shmemg_device_exec_ops_ctx_on_stream", "op %d" % bad.value)
+        self._keep = getattr(self, "_keep", []) + [ops_dev]
+        self.launches += 1 if len(ops) else 0
+
+    def put_nbi(self, dest_off, source_off, nbytes, pe, target_pe, stream=None):
+        self._chk(lib().shmemg_put_nbi_on_stream(self.h, dest_off, source_off, nbytes, pe, target_pe, _stream(stream)),
+                  "shmemg_put_nbi_on_stream")
+        self.launches += 1 if nbytes else 0
+
+    def get_nbi(self, dest_off, source_off, nbytes, pe, target_pe, stream=None):
+        self._chk(lib().shmemg_get_nbi_on_stream(self.h, dest_off, source_off, nbytes, pe, target_pe, _stream(stream)),
+                  "shmemg_get_nbi_on_stream")
+        self.launches += 1 if nbytes else 0
+
+    def put_signal_nbi(self, dest_off, source_off, nbytes, sig_off, signal, sig_op, pe, target_pe, stream=None):
+        self._chk(lib().shmemg_put_signal_nbi_on_stream(self.h, dest_off, source_off, nbytes, sig_off, signal, sig_op, pe,
+                                                        target_pe, _stream(stream)), "shmemg_put_signal_nbi_on_stream")
+        self.launches += 1
 
     def device_collective(self, kind, dest_off, source_off, n, dtype=0, root=0, stream=None):
         """One device collective run device-initiated: block p calls shmemg_dev_<kind>_block (include/shmemg_device.cuh)."""

@@ -822,3 +822,17 @@ extern "C" int shmemg_quiet(shmemg_world_t *w, int pe, void *stream) {
     SHMEMG_CUDA(w, cudaStreamSynchronize((cudaStream_t)stream));
     return SHMEMG_OK;
 }
+
+// non-blocking forms on a stream: same kernels, weaker contract (see shmemg.h)
+extern "C" int shmemg_put_nbi_on_stream(shmemg_world_t *w, uint64_t dest_off, uint64_t source_off, size_t nbytes, int pe,
+                                        int target_pe, void *stream) {
+    return shmemg_put_on_stream(w, dest_off, source_off, nbytes, pe, target_pe, stream);
+}
+extern "C" int shmemg_get_nbi_on_stream(shmemg_world_t *w, uint64_t dest_off, uint64_t source_off, size_t nbytes, int pe,
+                                        int target_pe, void *stream) {
+    return shmemg_get_on_stream(w, dest_off, source_off, nbytes, pe, target_pe, stream);
+}
+extern "C" int shmemg_put_signal_nbi_on_stream(shmemg_world_t *w, uint64_t dest_off, uint64_t source_off, size_t nbytes,
+                                               uint64_t sig_off, uint64_t signal, int sig_op, int pe, int target_pe, void *stream) {
+    return shmemg_put_signal_on_stream(w, dest_off, source_off, nbytes, sig_off, signal, sig_op, pe, target_pe, stream);
+}

@@ -109,7 +109,8 @@ extern "C" int shmem_query_capabilities(const shmemg_world_t *w, int team, uint6
     if (team == SHMEM_TEAM_WORLD)
         c |= SHMEMG_CAP_HOST_INITIATED_GPU_BUFFERS | SHMEMG_CAP_STREAM_TRIGGERED | SHMEMG_CAP_STREAM_COLLECTIVES;
     else
-        c |= SHMEMG_CAP_DEVICE_INITIATED | SHMEMG_CAP_DEVICE_BARRIER | SHMEMG_CAP_DEVICE_COLLECTIVES;   // include/shmemg_device.cuh
+        c |= SHMEMG_CAP_DEVICE_INITIATED | SHMEMG_CAP_DEVICE_BARRIER | SHMEMG_CAP_DEVICE_COLLECTIVES |
+             SHMEMG_CAP_EXPLICIT_DEVICE_CTX;   // include/shmemg_device.cuh
     *caps = c;
     return SHMEMG_OK;
 }

@@ -67,6 +67,25 @@ def run_gpu_device(prog, batches=None, heap_bytes=None):
     return w, ld
 
 
+def run_gpu_device_ctx(prog, batches=None, heap_bytes=None, queue_entries=8):
+    """DEVICE-INITIATED with EXPLICIT CONTEXTS: one context handle per (PE, context) created on the host and cached in device
+    memory; puts / gets / put_signals are non-blocking on their op's context (shmemg_device_exec_ops_ctx_on_stream).  The small
+    queue (8 entries) also exercises the drain-when-full path."""
+    hb = heap_bytes or heap_bytes_for(prog)
+    w = World(prog.npes, hb, DEV)
+    ld = Loaded(w, prog)
+    nctx = 1
+    for q in (batches or [prog]):
+        if len(q.ops):
+            nctx = max(nctx, int(q.ops["ctx"].max()) + 1)
+    handles, dev = w.ctx_create_all(nctx, queue_entries)
+    for q in (batches or [prog]):
+        w.device_exec_ops_ctx(ld.translate(q), dev, nctx)
+    w.quiet(0)
+    w._ctx_handles = handles
+    return w, ld
+
+
 def run_oracle(prog, batches=None, heap_bytes=None):
     hb = heap_bytes or heap_bytes_for(prog)
     ow = orc.OracleWorld(prog.npes, hb)

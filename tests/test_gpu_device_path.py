@@ -5,7 +5,7 @@ atomics and the brute-force outcome sets for tiny programs."""
 import numpy as np
 import pytest
 
-from gpu_common import DEV, assert_objects_equal, run_gpu_device, run_oracle
+from gpu_common import DEV, assert_objects_equal, run_gpu_device, run_gpu_device_ctx, run_oracle
 from invariants import check_compare_swap_claim, check_fetch_add
 from litmus_model import enumerate_outcomes, to_spec_program
 from paper_2607_08006_b200 import CAP, ERR, OP, OP_DTYPE, TEAM, ShmemgError, World
@@ -222,3 +222,85 @@ def test_device_collective_argument_checks():
             w.device_collective(**kw)
         assert e.value.code == code, (kw, e.value)
     w.device_collective(DEVCOLL.FCOLLECT, b, a, 0)               # zero bytes: nothing enqueued
+
+
+# ---- explicit device contexts and non-blocking operations (shmemg_ctx_create, shmemg_dev_*_nbi, shmemg_dev_ctx_*) ---------------
+@pytest.mark.parametrize("make", [
+    lambda: litmus.mp_fence(),
+    lambda: litmus.mp_quiet_third_party(),
+    lambda: litmus.put_signal_sizes(),
+    lambda: litmus.signal_add_fanin(),
+    lambda: litmus.barrier_stamp(),
+    lambda: litmus.wait_after_wait(),
+    lambda: litmus.two_contexts(),
+    lambda: litmus.contexts_amos_waits(),
+], ids=["mp_fence", "mp_quiet3", "put_signal_sizes", "signal_add_fanin", "barrier_stamp", "wait_after_wait", "two_contexts",
+        "contexts_amos_waits"])
+def test_litmus_programs_with_explicit_contexts_match_oracle(make):
+    prog = make()
+    w, ld = run_gpu_device_ctx(prog)
+    assert_objects_equal(prog, ld, run_oracle(prog))
+    nctx = int(prog.ops["ctx"].max()) + 1
+    for k in range(prog.npes * nctx):                                # everything issued on a context has completed
+        issued, completed = w.ctx_counters(w._ctx_handles, k)
+        assert issued == completed
+    ops = prog.ops
+    nb = np.isin(ops["kind"], (1, 2, 3))                              # PUT, GET, PUT_SIGNAL are the queued operations
+    for p in (0, prog.npes - 1):
+        for c in range(nctx):
+            assert w.ctx_counters(w._ctx_handles, p * nctx + c)[0] == int((nb & (ops["initiator"] == p) & (ops["ctx"] == c)).sum())
+
+
+@pytest.mark.parametrize("name", sorted(TINY))
+def test_tiny_programs_with_explicit_contexts_land_in_enumerated_outcome_set(name):
+    prog, init, order = TINY[name]
+    allowed = enumerate_outcomes(prog, init)
+    sp = to_spec_program(prog, init, order)
+    for _ in range(3):
+        w, ld = run_gpu_device_ctx(sp)
+        got = tuple(tuple(int(x) for x in row) for row in ld.obj_numpy("w", np.uint64))
+        assert got in allowed, (name, got)
+
+
+def test_quiet_on_one_context_leaves_the_other_contexts_operations_pending():
+    """PAPER L327 / L331 + reading 31: a context has its own completion counters and lives in device memory across kernels.
+    Kernel A (its list is not quieted at the end): PE 0 issues a non-blocking put on context 0, another on context 1, and a
+    QUIET on context 1.  Afterwards context 1 reads (1 issued, 1 completed) and its data has arrived; context 0 reads (1, 0)
+    and its destination is untouched -- an outcome the brute-force model allows
+    (test_litmus_model.py::test_contexts_are_independent_ordering_domains).  Kernel B: QUIET on context 0 completes it."""
+    from gpu_common import heap_bytes_for
+    from paper_2607_08006_b200.loader import Loaded
+    prog = Program(2)
+    prog.obj("w", 64, np.arange(16, dtype=np.uint64).reshape(2, 8))
+    prog.put(0, 1, ("w", 0), ("w", 8), 8, ctx=0)
+    prog.put(0, 1, ("w", 16), ("w", 24), 8, ctx=1)
+    prog.quiet(0, ctx=1)
+    w = World(2, heap_bytes_for(prog), DEV)
+    ld = Loaded(w, prog)
+    handles, dev = w.ctx_create_all(2, 8)
+    w.device_exec_ops_ctx(ld.translate(prog), dev, 2, flags=1)        # SHMEMG_EXEC_LEAVE_PENDING
+    assert w.ctx_counters(handles, 0) == (1, 0) and w.ctx_counters(handles, 1) == (1, 1)
+    got = ld.obj_numpy("w", np.uint64)
+    assert got[1, 2] == 3 and got[1, 0] == 8                          # ctx 1 delivered (word 3 of PE 0 = 3), ctx 0 still pending
+    b = prog.fork()
+    b.quiet(0, ctx=0)
+    w.device_exec_ops_ctx(ld.translate(b), dev, 2, flags=1)
+    assert w.ctx_counters(handles, 0) == (1, 1)
+    assert_objects_equal(prog, ld, run_oracle(prog))
+    assert w.ctx_counters(handles, 2) == (0, 0)
+    caps = w.query_capabilities(TEAM.DEVICE_WORLD)
+    assert caps & CAP.EXPLICIT_DEVICE_CTX and not w.query_capabilities(TEAM.WORLD) & CAP.EXPLICIT_DEVICE_CTX
+
+
+def test_nbi_forms_on_a_stream():
+    npes, n = 4, 50000
+    w = World(npes, 4 * n + 4096, DEV)
+    s, d, sig = w.malloc(n), w.malloc(n), w.calloc(1, 8)
+    pay = gen.u64(npes * (n // 8 + 1), 9).view(np.uint8).reshape(npes, -1)[:, :n]
+    w.view(s, n).copy_(torch.from_numpy(np.ascontiguousarray(pay))); w.view(d, n).zero_()
+    w.put_nbi(d, s, n, 0, 1); w.get_nbi(d, s, n, 2, 3)
+    w.put_signal_nbi(d, s, n - 3, sig, 7, 0, 1, 0)
+    w.quiet(0)
+    got = w.view(d, n).cpu().numpy()
+    assert np.array_equal(got[1], pay[0]) and np.array_equal(got[2], pay[3]) and np.array_equal(got[0, :n - 3], pay[1, :n - 3])
+    assert w.view(sig, 8, torch.int64).cpu().numpy()[0, 0] == 7
