@@ -55,6 +55,8 @@ def lib():
         L.orc_sum_reduce_i64.argtypes = [vp, i, u64, u64, u64, u64]
         L.orc_fcollect.argtypes = [vp, i, u64, u64, u64, u64]
         L.orc_alltoall.argtypes = [vp, i, u64, u64, u64, u64]
+        L.orc_alltoalls.argtypes = [vp, i, u64, u64, u64, u64, u64, u64, u64, u64, u64]
+        L.orc_copy_spaces.argtypes = [vp, u64, vp, u64, i, i, u64, i, u64, u64]
         L.orc_broadcast.argtypes = [vp, i, u64, u64, u64, u64, i]
         L.orc_reduce.argtypes = [vp, i, u64, i, i, u64, u64, u64]
         L.orc_amo_batch.argtypes = [vp, i, u64, i, i, u64, vp, vp, vp, vp, u64]
@@ -201,6 +203,40 @@ class OracleWorld:
         _chk(lib().orc_alltoall(self.heap.ctypes.data, self.npes, self.heap_bytes, dst_off, src_off, nbytes),
              "alltoall")
 
+
+    # ---- NEXT-4: block-strided alltoall (FFT-style transposes), the CPU space of the two-space model -------------------
+    def alltoalls(self, dst_off, src_off, dst_pe_stride, src_pe_stride, dst_block_stride, src_block_stride, block, nblocks):
+        _chk(lib().orc_alltoalls(self.heap.ctypes.data, self.npes, self.heap_bytes, dst_off, src_off, dst_pe_stride,
+                                 src_pe_stride, dst_block_stride, src_block_stride, block, nblocks), "alltoalls")
+
+    def attach_cpu_space(self, cpu_heap_bytes: int):
+        """The CPU half of the two-space model: a second array of npes windows with its own allocator."""
+        self.cpu_heap_bytes = int(cpu_heap_bytes)
+        self.cpu_heap = np.zeros((self.npes, self.cpu_heap_bytes), dtype=np.uint8)
+        self._cpu_brk = 0
+
+    def cpu_malloc(self, nbytes: int) -> int:
+        off = (self._cpu_brk + self.ALIGN - 1) // self.ALIGN * self.ALIGN
+        if off + nbytes > self.cpu_heap_bytes:
+            raise OracleError("CPU symmetric heap exhausted")
+        self._cpu_brk = off + nbytes
+        return off
+
+    def cpu_view(self, off: int, nbytes: int, dtype=np.uint8) -> np.ndarray:
+        return self.cpu_heap[:, off:off + nbytes].view(dtype)
+
+    def _space(self, space: int):
+        return (self.heap, self.heap_bytes) if space == 0 else (self.cpu_heap, self.cpu_heap_bytes)
+
+    def put_space(self, dst_space, dst_off, src_space, src_off, nbytes, pe, target):
+        """heap[dst_space][target][dst_off : +n] = heap[src_space][pe][src_off : +n]; space 0 = GPU, 1 = CPU."""
+        (dh, db), (sh, sb) = self._space(dst_space), self._space(src_space)
+        _chk(lib().orc_copy_spaces(dh.ctypes.data, db, sh.ctypes.data, sb, self.npes, target, dst_off, pe, src_off, nbytes), "put_space")
+
+    def get_space(self, dst_space, dst_off, src_space, src_off, nbytes, pe, target):
+        """heap[dst_space][pe][dst_off : +n] = heap[src_space][target][src_off : +n]."""
+        (dh, db), (sh, sb) = self._space(dst_space), self._space(src_space)
+        _chk(lib().orc_copy_spaces(dh.ctypes.data, db, sh.ctypes.data, sb, self.npes, pe, dst_off, target, src_off, nbytes), "get_space")
 
     # ---- NEXT-2 surface: broadcast, general reductions, generic AMOs, block-strided put/get, test ----
     RED = {"sum": 0, "prod": 1, "min": 2, "max": 3, "and": 4, "or": 5, "xor": 6}

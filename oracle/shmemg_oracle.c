@@ -242,6 +242,40 @@ int orc_alltoall(uint8_t *heap, int npes, uint64_t heap_bytes, uint64_t dst_off,
     return ORC_OK;
 }
 
+/* block-strided alltoall (the transpose of "FFT-driven spectral phases, many-to-many exchanges",
+ * L68; generalises OpenSHMEM 1.6 alltoalls, inherited via L361): for all source PEs i, destination PEs j and blocks b < nblocks
+ *     heap[j][dst + i*dst_pe_stride + b*dst_block_stride : +block] = heap[i][src + j*src_pe_stride + b*src_block_stride : +block]
+ * (strides in bytes).  alltoalls(dest, source, dst, sst, nelems) on elements of es bytes is the case block = es, nblocks = nelems,
+ * block strides = dst*es / sst*es, pe strides = nelems*dst*es / nelems*sst*es.  Source and destination footprints must not
+ * overlap, and no two (i, b) may write the same destination bytes (both undefined otherwise). */
+int orc_alltoalls(uint8_t *heap, int npes, uint64_t heap_bytes, uint64_t dst_off, uint64_t src_off, uint64_t dst_pe_stride,
+                  uint64_t src_pe_stride, uint64_t dst_block_stride, uint64_t src_block_stride, uint64_t block,
+                  uint64_t nblocks) {
+    if (block == 0 || nblocks == 0) return ORC_OK;
+    uint64_t dspan = (uint64_t)(npes - 1) * dst_pe_stride + (nblocks - 1) * dst_block_stride + block;
+    uint64_t sspan = (uint64_t)(npes - 1) * src_pe_stride + (nblocks - 1) * src_block_stride + block;
+    if (!in_range(dst_off, dspan, heap_bytes) || !in_range(src_off, sspan, heap_bytes)) return ORC_ERR_RANGE;
+    if (!(src_off + sspan <= dst_off || dst_off + dspan <= src_off)) return ORC_ERR_RANGE;
+    for (int i = 0; i < npes; ++i)
+        for (int j = 0; j < npes; ++j)
+            for (uint64_t b = 0; b < nblocks; ++b)
+                memcpy(heap + (uint64_t)j * heap_bytes + dst_off + (uint64_t)i * dst_pe_stride + b * dst_block_stride,
+                       heap + (uint64_t)i * heap_bytes + src_off + (uint64_t)j * src_pe_stride + b * src_block_stride, block);
+    return ORC_OK;
+}
+
+/* Two-space model (L313-L317, Fig. 4: "CPU space: default symmetric heap (host-attached)" beside the GPU space): a put / get
+ * whose operands may live in either space.  The two spaces are two independent arrays of npes windows; `dheap` / `sheap` are the
+ * destination's and the source's space.  put: heap_dst[target][dst : +n] = heap_src[pe][src : +n]; get: heap_dst[pe][dst : +n] =
+ * heap_src[target][src : +n] -- the caller passes (dst_pe, src_pe) accordingly. */
+int orc_copy_spaces(uint8_t *dheap, uint64_t dheap_bytes, uint8_t *sheap, uint64_t sheap_bytes, int npes, int dst_pe, uint64_t dst_off,
+                    int src_pe, uint64_t src_off, uint64_t n) {
+    if (dst_pe < 0 || dst_pe >= npes || src_pe < 0 || src_pe >= npes) return ORC_ERR_RANGE;
+    if (!in_range(dst_off, n, dheap_bytes) || !in_range(src_off, n, sheap_bytes)) return ORC_ERR_RANGE;
+    memmove(dheap + (uint64_t)dst_pe * dheap_bytes + dst_off, sheap + (uint64_t)src_pe * sheap_bytes + src_off, n);
+    return ORC_OK;
+}
+
 /* ---- the rest of the OpenSHMEM op surface on the same heaps --------------
  * The paper names these only by reference: broadcast among the host-side _on_stream variants (L218),
  * "quiet, wait, and test" (L392), the AMO set and strided transfers through "inherited unchanged from

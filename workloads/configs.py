@@ -193,3 +193,36 @@ def c5_i64(npes: int = 128, nelem: int = 1 << 19, seed: int = 4) -> np.ndarray:
 
 def c5_fcollect_src(npes: int = 128, nbytes: int = 32768, seed: int = 4) -> np.ndarray:
     return gen.u64(npes * nbytes // 8, seed, stream=2).view(np.uint8).reshape(npes, nbytes)
+
+
+# ------------------------------------------------------------------------------------------------
+# NEXT-4 (i): FFT-style transpose ("FFT-driven spectral phases, many-to-many exchanges")
+# ------------------------------------------------------------------------------------------------
+@dataclass
+class FftTranspose:
+    """Slab transpose of a global array A[X][Y][Z] of `es`-byte elements (complex64: es = 8) over npes PEs: PE p holds the x-slab
+    A[p*X/N : (p+1)*X/N, :, :]; afterwards PE q holds the y-slab B[x][yl][z] = A[x][q*Y/N + yl][z] (all x, x-major).  Seen as a
+    block-strided alltoall: PE i sends to PE j, for each of its X/N local x, the contiguous chunk of Y/N rows."""
+    npes: int
+    X: int
+    Y: int
+    Z: int
+    es: int
+    A: np.ndarray                 # uint8 [npes, X/N * Y * Z * es]: the x-slabs
+
+    @property
+    def slab_bytes(self):
+        return self.X // self.npes * self.Y * self.Z * self.es
+
+    def params(self):
+        """(block_bytes, nblocks, src_block_stride, src_pe_stride, dst_block_stride, dst_pe_stride) of the alltoalls call."""
+        yn, xn = self.Y // self.npes, self.X // self.npes
+        block = yn * self.Z * self.es
+        return block, xn, self.Y * self.Z * self.es, block, block, xn * block
+
+
+def fft_transpose(npes: int = 64, X: int = 1024, Y: int = 1024, Z: int = 256, es: int = 8, seed: int = 5) -> FftTranspose:
+    assert X % npes == 0 and Y % npes == 0
+    n = X * Y * Z * es
+    A = gen.normal_f32(n // 4, seed, stream=0).view(np.uint8).reshape(npes, n // npes)        # complex64 = two N(0,1) floats
+    return FftTranspose(npes, X, Y, Z, es, A)
