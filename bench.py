@@ -74,7 +74,7 @@ def parse_args():
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg (and the verification against the oracle)")
     ap.add_argument("--no-verify", action="store_true", help="skip the comparison of every segment's results with the oracle")
     ap.add_argument("--small", action="store_true", help="reduced sizes (development only; marked in the JSON)")
-    ap.add_argument("--only", default="", help="comma-separated segment groups to run: c1,c2,c3a,c3b,c4,c5,barrier,next2")
+    ap.add_argument("--only", default="", help="comma-separated segment groups to run: c1,c2,c3a,c3b,c4,c5,barrier,next2,next4")
     return ap.parse_args()
 
 
@@ -154,6 +154,9 @@ class Inputs:
             self.c3b = configs.c3b_skewed(npes=16 if small else 64)
         if "c4" in groups:
             self.c4 = configs.c4_graph(scale=18 if small else 22)
+        if "next4" in groups:
+            # NEXT-4 (i): slab transpose of a 1024 x 1024 x 256 complex64 array (2 GiB) over 64 PEs
+            self.fft = configs.fft_transpose(16, 128, 128, 64) if small else configs.fft_transpose()
         if "c5" in groups or "barrier" in groups:
             self.c5_npes, self.c5_bytes = (32, 1 << 20) if small else (128, 4 << 20)
             self.c5_fc_bytes = 32768
@@ -220,6 +223,8 @@ def segment_table(inp: Inputs):
             seg["next1_halo_app_persistent"] = dict(cls="xtime", kernel="k_halo_persistent (device-initiated)", ops=HALO_ROUNDS, launches=1)
             seg["next1_halo_app_compute_only"] = dict(cls="xtime", kernel="k_halo_perturb", ops=HALO_ROUNDS, launches=HALO_ROUNDS)
             seg["next2_ibput_faces"] = dict(cls="xcopy", kernel="k_ib_tma/k_ib_elem", bytes=3 * 2 * inp.halo.face_bytes, launches=3)
+    if "next4" in g:
+        seg["next4_fft_transpose_alltoalls"] = dict(cls="xcopy", kernel="k_alltoalls_tma", bytes=2 * inp.fft.A.size, launches=1)
     if "barrier" in g:
         seg["barrier_in_kernel"] = dict(cls="sync", kernel="k_barrier_repeat", ops=BARRIERS, launches=1)
         seg["barrier_on_stream"] = dict(cls="sync", kernel="k_barrier_epoch", ops=BARRIERS, launches=BARRIERS)
@@ -326,6 +331,13 @@ class CudaBench:
                                                     "plans": HALO_ROUNDS}
             self.halo_ops_host = [torch.from_numpy(o.view(np.uint8).reshape(-1).copy()).pin_memory() for o in halo_ops]
             self.halo_ops_dev = [t.to(device) for t in self.halo_ops_host]
+            self.worlds.append(w)
+        if "next4" in g:
+            t = inp.fft
+            w = World(t.npes, 2 * t.slab_bytes + 4096, device)
+            self.wf, self.f_src, self.f_dst = w, w.malloc(t.slab_bytes), w.malloc(t.slab_bytes)
+            w.view(self.f_src, t.slab_bytes).copy_(torch.from_numpy(t.A))
+            w.view(self.f_dst, t.slab_bytes).zero_()
             self.worlds.append(w)
         if "c5" in g or "barrier" in g:
             n, nb = inp.c5_npes, inp.c5_bytes
@@ -459,6 +471,10 @@ class CudaBench:
                     self.w2.ibput(send_off, self.U_off, 0, 0, fb, 1, 0, 1)
                     self.w2.ibput(send_off + 2 * fb, self.U_off, B * 8, B * B * 8, B * 8, B, 0, 1)
                     self.w2.ibput(send_off + 4 * fb, self.U_off, 8, B * 8, 8, B * B, 0, 1)
+        if "next4" in g:
+            block, nblocks, sbs, sps, dbs, dps = inp.fft.params()
+            with rec.seg("next4_fft_transpose_alltoalls"):
+                self.wf.alltoalls(self.f_dst, self.f_src, dps, sps, dbs, sbs, block, nblocks)
         if "barrier" in g:
             with rec.seg("barrier_in_kernel"):
                 self.w5.barrier_all_repeat(BARRIERS)
@@ -661,6 +677,17 @@ class CudaBench:
             assert np.array_equal(fp[~won], par[q.v[~won]]), "a losing compare-swap fetched something else than the final parent"
             assert (par[np.bincount(q.v, minlength=len(par)) == 0] == -1).all(), "untouched parent slot modified"
             ok["atomic_fetch_add"] = ok["atomic_compare_swap"] = True
+        if "next4" in g:
+            t = inp.fft
+            block, nblocks, sbs, sps, dbs, dps = t.params()
+            self.wf.view(self.f_dst, t.slab_bytes).zero_()
+            self.wf.alltoalls(self.f_dst, self.f_src, dps, sps, dbs, sbs, block, nblocks)
+            ow = ob.orc.OracleWorld(t.npes, 2 * t.slab_bytes + 512)
+            os_, od = ow.malloc(t.slab_bytes), ow.malloc(t.slab_bytes)
+            ow.view(os_, t.slab_bytes)[:] = t.A
+            ow.alltoalls(od, os_, dps, sps, dbs, sbs, block, nblocks)
+            assert np.array_equal(host(self.wf.view(self.f_dst, t.slab_bytes)), ow.view(od, t.slab_bytes)), "fft transpose"
+            ok["next4_fft_transpose_alltoalls"] = True
         if "c2" in g:
             h, w, fb = inp.halo, self.w2, inp.halo.face_bytes
             send_off = self.ld2.off["send"][0]
@@ -840,7 +867,7 @@ def class_rates(table, seg_seconds, seg_units):
     return (cb / cs / 1e9 if cs > 0 else 0.0), (ao / as_ / 1e6 if as_ > 0 else 0.0), cs, as_
 
 
-ALL_GROUPS = ["c1", "c2", "c3a", "c3b", "c4", "c5", "barrier", "next2"]
+ALL_GROUPS = ["c1", "c2", "c3a", "c3b", "c4", "c5", "barrier", "next2", "next4"]
 
 
 def max_over_ranks(dist, device, seg_ms, whole_ms, e2e_ms):
@@ -879,7 +906,7 @@ def run_reference(args):
     """This tier's reference arm: the oracle, as it stands, on the host cores (rank 0 only)."""
     if int(os.environ.get("RANK", "0")) != 0:
         return
-    groups = [x for x in (args.only.split(",") if args.only else ALL_GROUPS) if x != "barrier"]
+    groups = [x for x in (args.only.split(",") if args.only else ALL_GROUPS) if x not in ("barrier", "next4")]
     inp = Inputs(args.small, groups)
     table = segment_table(inp)
     ob = OracleBench(inp)

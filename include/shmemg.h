@@ -79,7 +79,8 @@ enum {
 #define SHMEMG_CAP_PATH_DIRECT                (1ull << 10)  /* direct load/store path (L431)             */
 #define SHMEMG_CAP_ATOMICS_64                 (1ull << 11)  /* add / fetch-add / compare-swap on 64 bit  */
 #define SHMEMG_CAP_STREAM_COLLECTIVES         (1ull << 12)  /* barrier/alltoall/fcollect/reduce on stream */
-#define SHMEMG_CAP_DEVICE_BARRIER             (1ull << 13)  /* shmemg_dev_barrier_all_block only (L363)  */
+#define SHMEMG_CAP_DEVICE_BARRIER             (1ull << 13)  /* shmemg_dev_barrier_all_block (L363)       */
+#define SHMEMG_CAP_CPU_HEAP_PRESENT           (1ull << 14)  /* the CPU space of the two-space model is attached (L313-L317) */
 
 /* ---- lifecycle ------------------------------------------------------------------------------------ */
 
@@ -116,6 +117,25 @@ SHMEMG_API int shmemg_free(shmemg_world_t *w, uint64_t sym_off);
 /* shmem_ptr analog: DEVICE pointer to offset `sym_off` on PE `pe`, or NULL if the
  * arguments are invalid.  Valid in the device access domain only (SHMEMG_CAP_PTR_DEVICE_ACCESSIBLE). */
 SHMEMG_API void *shmemg_ptr(const shmemg_world_t *w, uint64_t sym_off, int pe);
+
+/* ---- the two-space model (Fig. 4 "Two-space model (baseline)": a GPU space and a "CPU
+ * space: default symmetric heap (host-attached)"; L456 access domains) ---------------------------------------------------------
+ * The GPU space is the heap of shmemg_init.  shmemg_cpu_heap_attach adds the CPU space: npes windows of heap_bytes_per_pe bytes
+ * (stride rounded up to 512 B) in `host_slab`, PAGE-LOCKED host memory owned by the caller (cudaHostAlloc / torch pin_memory;
+ * SHMEMG_ERR_ARG otherwise), at most once per world.  shmemg_cpu_malloc / shmemg_cpu_free allocate symmetric offsets in it (its
+ * own allocator: an offset names ONE space), shmemg_cpu_ptr is dereferenceable on the HOST.  shmemg_put_space_on_stream /
+ * shmemg_get_space_on_stream are put / get whose dest and source each name their space: GPU <-> GPU runs the copy kernels,
+ * anything that touches the CPU space is a DMA transfer on `stream`.  shmem_query_capabilities reports
+ * SHMEMG_CAP_CPU_HEAP_PRESENT once it is attached; AMOs, signals and collectives stay in the GPU space. */
+enum { SHMEMG_SPACE_GPU = 0, SHMEMG_SPACE_CPU = 1 };
+SHMEMG_API int shmemg_cpu_heap_attach(shmemg_world_t *w, void *host_slab, size_t heap_bytes_per_pe, size_t slab_bytes);
+SHMEMG_API int shmemg_cpu_malloc(shmemg_world_t *w, size_t bytes, uint64_t *sym_off);
+SHMEMG_API int shmemg_cpu_free(shmemg_world_t *w, uint64_t sym_off);
+SHMEMG_API void *shmemg_cpu_ptr(const shmemg_world_t *w, uint64_t sym_off, int pe);      /* HOST pointer, or NULL */
+SHMEMG_API int shmemg_put_space_on_stream(shmemg_world_t *w, int dest_space, uint64_t dest_off, int source_space, uint64_t source_off,
+                                          size_t nbytes, int pe, int target_pe, void *stream);
+SHMEMG_API int shmemg_get_space_on_stream(shmemg_world_t *w, int dest_space, uint64_t dest_off, int source_space, uint64_t source_off,
+                                          size_t nbytes, int pe, int target_pe, void *stream);
 
 /* Documented extension ("registered private ... source operands"): move bytes between a HOST
  * buffer and PE `pe`'s window with cudaMemcpyAsync on `stream`.  Used by the end-to-end benchmark. */
@@ -298,7 +318,8 @@ SHMEMG_API int shmemg_atomic_op_batch_on_stream(shmemg_world_t *w, int amo, int 
 /* ---- block-strided put / get (OpenSHMEM 1.6 ibput / ibget; iput / iget are the case block = one element) ---------------
  * for b in [0, nblocks): dest[b*dst_stride .. +block_bytes) = source[b*src_stride .. +block_bytes); strides in BYTES, any
  * size and alignment.  put: source in `pe`'s window, dest in `target_pe`'s; get: source in `target_pe`'s, dest in `pe`'s.
- * Destination blocks must not overlap each other or the source (undefined otherwise).  Stream-ordered like put / get. */
+ * Destination blocks must not overlap each other (dst_stride < block_bytes with nblocks > 1: SHMEMG_ERR_OVERLAP) or the source
+ * (undefined otherwise).  Stream-ordered like put / get. */
 SHMEMG_API int shmemg_ibput_on_stream(shmemg_world_t *w, uint64_t dest_off, uint64_t source_off, uint64_t dst_stride,
                                       uint64_t src_stride, size_t block_bytes, size_t nblocks, int pe, int target_pe,
                                       void *stream);
@@ -373,6 +394,17 @@ SHMEMG_API int shmemg_fcollect_on_stream(shmemg_world_t *w, uint64_t dest_off, u
 /* PE j's dest[i*nbytes .. +nbytes) = PE i's source[j*nbytes .. +nbytes)  (block index = peer PE). */
 SHMEMG_API int shmemg_alltoall_on_stream(shmemg_world_t *w, uint64_t dest_off, uint64_t source_off, size_t nbytes,
                                          void *stream);
+/* Block-strided alltoall (the transposes of "FFT-driven spectral phases, many-to-many exchanges", PAPER L68;
+ * generalises OpenSHMEM 1.6 alltoalls, inherited unchanged, L361): for all source PEs i, destination PEs j and blocks b < nblocks
+ *     PE j's dest[i*dst_pe_stride + b*dst_block_stride .. +block_bytes) = PE i's source[j*src_pe_stride + b*src_block_stride .. +block_bytes)
+ * (strides in BYTES).  A slab transpose of A[X][Y][Z] over N PEs is block = (Y/N)*Z*es, nblocks = X/N, src_block_stride = Y*Z*es,
+ * src_pe_stride = block, dst_block_stride = block, dst_pe_stride = nblocks*block; alltoalls(dest, source, dst, sst, nelems) on
+ * es-byte elements is block = es, nblocks = nelems, block strides dst*es / sst*es, pe strides nelems times those.  Any size and
+ * alignment; the source and destination footprints must not overlap, nor two destination blocks (SHMEMG_ERR_OVERLAP where the
+ * strides make it certain, undefined otherwise). */
+SHMEMG_API int shmemg_alltoalls_on_stream(shmemg_world_t *w, uint64_t dest_off, uint64_t source_off, uint64_t dst_pe_stride,
+                                          uint64_t src_pe_stride, uint64_t dst_block_stride, uint64_t src_block_stride,
+                                          size_t block_bytes, size_t nblocks, void *stream);
 /* Stream-level barrier: everything enqueued earlier on `stream` by any PE is complete and visible to
  * everything enqueued later; bumps the world's barrier epoch (one tiny kernel). */
 SHMEMG_API int shmemg_barrier_all_on_stream(shmemg_world_t *w, void *stream);

@@ -60,6 +60,7 @@ class CAP:
     ATOMICS_64 = 1 << 11
     STREAM_COLLECTIVES = 1 << 12
     DEVICE_BARRIER = 1 << 13
+    CPU_HEAP_PRESENT = 1 << 14
 
 
 F32, I64, I32, F64 = 0, 1, 2, 3
@@ -148,6 +149,13 @@ SYMBOLS = {
     "shmemg_team_fcollect_on_stream": (_i, [_vp, _i, _u64, _u64, _sz, _vp]),
     "shmemg_team_alltoall_on_stream": (_i, [_vp, _i, _u64, _u64, _sz, _vp]),
     "shmemg_team_broadcast_on_stream": (_i, [_vp, _i, _u64, _u64, _sz, _i, _vp]),
+    "shmemg_alltoalls_on_stream": (_i, [_vp, _u64, _u64, _u64, _u64, _u64, _u64, _sz, _sz, _vp]),
+    "shmemg_cpu_heap_attach": (_i, [_vp, _vp, _sz, _sz]),
+    "shmemg_cpu_malloc": (_i, [_vp, _sz, C.POINTER(_u64)]),
+    "shmemg_cpu_free": (_i, [_vp, _u64]),
+    "shmemg_cpu_ptr": (_vp, [_vp, _u64, _i]),
+    "shmemg_put_space_on_stream": (_i, [_vp, _i, _u64, _i, _u64, _sz, _i, _i, _vp]),
+    "shmemg_get_space_on_stream": (_i, [_vp, _i, _u64, _i, _u64, _sz, _i, _i, _vp]),
     "shmemg_alltoall_on_stream": (_i, [_vp, _u64, _u64, _sz, _vp]),
     "shmemg_barrier_all_on_stream": (_i, [_vp, _vp]),
     "shmemg_barrier_all_repeat_on_stream": (_i, [_vp, _u32, _u64, _vp]),
@@ -581,6 +589,47 @@ class World:
         self._chk(lib().shmemg_fcollect_on_stream(self.h, dest_off, source_off, nbytes, _stream(stream)),
                   "shmemg_fcollect_on_stream")
         self.launches += 1 if nbytes else 0
+
+    def alltoalls(self, dest_off, source_off, dst_pe_stride, src_pe_stride, dst_block_stride, src_block_stride, block_bytes,
+                  nblocks, stream=None):
+        self._chk(lib().shmemg_alltoalls_on_stream(self.h, dest_off, source_off, dst_pe_stride, src_pe_stride, dst_block_stride,
+                                                   src_block_stride, block_bytes, nblocks, _stream(stream)),
+                  "shmemg_alltoalls_on_stream")
+        self.launches += 1 if block_bytes and nblocks else 0
+
+    # ---- the CPU space of the two-space model ------------------------------------------------------------------------------
+    def cpu_heap_attach(self, heap_bytes: int):
+        """Attach a CPU space of heap_bytes per PE in pinned host memory owned by this object."""
+        stride = (heap_bytes + 511) // 512 * 512
+        self.cpu_slab = torch.empty(self.npes * stride, dtype=torch.uint8).pin_memory()
+        self.cpu_stride = stride
+        self._chk(lib().shmemg_cpu_heap_attach(self.h, self.cpu_slab.data_ptr(), heap_bytes, self.cpu_slab.numel()),
+                  "shmemg_cpu_heap_attach")
+
+    def cpu_malloc(self, nbytes: int) -> int:
+        off = C.c_uint64(0)
+        self._chk(lib().shmemg_cpu_malloc(self.h, nbytes, C.byref(off)), "shmemg_cpu_malloc")
+        return off.value
+
+    def cpu_free(self, off: int):
+        self._chk(lib().shmemg_cpu_free(self.h, off), "shmemg_cpu_free")
+
+    def cpu_ptr(self, off: int, pe: int) -> int:
+        return lib().shmemg_cpu_ptr(self.h, off, pe) or 0
+
+    def cpu_view(self, off: int, nbytes: int) -> torch.Tensor:
+        """[npes, nbytes] HOST view of an object of the CPU space."""
+        return self.cpu_slab.view(self.npes, self.cpu_stride)[:, off:off + nbytes]
+
+    def put_space(self, dst_space, dest_off, src_space, source_off, nbytes, pe, target_pe, stream=None):
+        self._chk(lib().shmemg_put_space_on_stream(self.h, dst_space, dest_off, src_space, source_off, nbytes, pe, target_pe,
+                                                   _stream(stream)), "shmemg_put_space_on_stream")
+        self.launches += 1 if nbytes and dst_space == 0 and src_space == 0 else 0
+
+    def get_space(self, dst_space, dest_off, src_space, source_off, nbytes, pe, target_pe, stream=None):
+        self._chk(lib().shmemg_get_space_on_stream(self.h, dst_space, dest_off, src_space, source_off, nbytes, pe, target_pe,
+                                                   _stream(stream)), "shmemg_get_space_on_stream")
+        self.launches += 1 if nbytes and dst_space == 0 and src_space == 0 else 0
 
     def alltoall(self, dest_off, source_off, nbytes, stream=None):
         self._chk(lib().shmemg_alltoall_on_stream(self.h, dest_off, source_off, nbytes, _stream(stream)),

@@ -44,6 +44,61 @@ k_alltoall_tma(uint8_t *base, size_t stride, uint64_t dst_off, uint64_t src_off,
     });
 }
 
+// ---- block-strided alltoall (NEXT-4 (i): FFT-style transposes) --------------------------------------------------
+// PE j's dest[i*dps + b*dbs .. +blk) = PE i's source[j*sps + b*sbs .. +blk).  Work items are ordered (source PE i, block b,
+// destination PE j, chunk): for a slab transpose the chunks of consecutive j are contiguous in the source, so every CTA streams
+// its share of the source like a plain copy and scatters 32 KiB pieces over the destination windows.
+struct A2asArgs {
+    uint8_t *base;
+    size_t stride;
+    uint64_t dst_off, src_off, dps, sps, dbs, sbs, blk, nblocks;
+    int npes;
+};
+__global__ void __launch_bounds__(32) k_alltoalls_tma(const A2asArgs a, unsigned cpb) {
+    extern __shared__ __align__(1024) uint8_t stage[];
+    __shared__ uint64_t full[SHMEMG_TMA_STAGES];
+    if (threadIdx.x != 0) return;
+    tma_stream_init(full);
+    const size_t nwork = (size_t)a.npes * a.nblocks * a.npes * cpb;
+    tma_stream_copy(stage, full, blockIdx.x, gridDim.x, nwork, [&](size_t wk, const uint8_t *&s, uint8_t *&d, unsigned &n) {
+        const unsigned c = (unsigned)(wk % cpb);
+        size_t r = wk / cpb;
+        const size_t j = r % a.npes; r /= a.npes;
+        const size_t b = r % a.nblocks, i = r / a.nblocks;
+        const size_t off = (size_t)c * SHMEMG_TMA_TILE;
+        n = (unsigned)(a.blk - off < SHMEMG_TMA_TILE ? a.blk - off : SHMEMG_TMA_TILE);
+        s = a.base + i * a.stride + a.src_off + j * a.sps + b * a.sbs + off;
+        d = a.base + j * a.stride + a.dst_off + i * a.dps + b * a.dbs + off;
+    });
+}
+// any alignment: one CTA per (i, b, j, 16 KiB chunk)
+__global__ void __launch_bounds__(SHMEMG_THREADS, 4) k_alltoalls_generic(const A2asArgs a, unsigned cpb) {
+    const size_t nwork = (size_t)a.npes * a.nblocks * a.npes * cpb;
+    for (size_t wk = blockIdx.x; wk < nwork; wk += gridDim.x) {
+        const unsigned c = (unsigned)(wk % cpb);
+        size_t r = wk / cpb;
+        const size_t j = r % a.npes; r /= a.npes;
+        const size_t b = r % a.nblocks, i = r / a.nblocks;
+        const size_t off = (size_t)c * 16384;
+        const size_t n = a.blk - off < 16384 ? a.blk - off : 16384;
+        copy_coop<4>(a.base + j * a.stride + a.dst_off + i * a.dps + b * a.dbs + off,
+                     a.base + i * a.stride + a.src_off + j * a.sps + b * a.sbs + off, n, threadIdx.x, SHMEMG_THREADS);
+    }
+}
+// naturally aligned elements of 4 / 8 / 16 bytes (the OpenSHMEM alltoalls form): one element per thread; consecutive threads
+// take consecutive blocks b of one (i, j) pair
+template <typename T>
+__global__ void __launch_bounds__(256) k_alltoalls_elem(const A2asArgs a) {
+    const size_t n = (size_t)a.npes * a.npes * a.nblocks;
+    for (size_t e = (size_t)blockIdx.x * blockDim.x + threadIdx.x; e < n; e += (size_t)gridDim.x * blockDim.x) {
+        const size_t b = e % a.nblocks, ij = e / a.nblocks, j = ij % a.npes, i = ij / a.npes;
+        uint8_t *d = a.base + j * a.stride + a.dst_off + i * a.dps + b * a.dbs;
+        const uint8_t *s = a.base + i * a.stride + a.src_off + j * a.sps + b * a.sbs;
+        if constexpr (sizeof(T) == 16) st_stream16(d, ld_stream16(s));
+        else *reinterpret_cast<T *>(d) = *reinterpret_cast<const volatile T *>(s);
+    }
+}
+
 // ---- fcollect: PE j's dest[p*n .. +n) = PE p's source[0 .. n) for every j -------------------------------------------
 // work item = (source PE p, 16-byte-vector chunk of its block, group of destination PEs)
 template <int VPT>   // vectors per thread held in registers
@@ -414,6 +469,7 @@ static int collectives_smem_attr(shmemg_world *w) {
     if (w->smem_attr_coll) return SHMEMG_OK;
     SHMEMG_CUDA(w, cudaFuncSetAttribute(k_alltoall_tma, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SHMEMG_TMA_SMEM));
     SHMEMG_CUDA(w, cudaFuncSetAttribute(k_fcollect_tma, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SHMEMG_TMA_SMEM));
+    SHMEMG_CUDA(w, cudaFuncSetAttribute(k_alltoalls_tma, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SHMEMG_TMA_SMEM));
     w->smem_attr_coll = true;
     return SHMEMG_OK;
 }
@@ -447,6 +503,49 @@ extern "C" int shmemg_alltoall_on_stream(shmemg_world_t *w, uint64_t dest_off, u
     const uint64_t nwork = (uint64_t)w->npes * w->npes * cpb;
     const unsigned grid = (unsigned)(nwork < maxgrid ? nwork : maxgrid);
     k_alltoall<<<grid, SHMEMG_THREADS, 0, st>>>(w->base, w->stride, dest_off, source_off, nbytes, w->npes, chunk, cpb);
+    SHMEMG_CUDA(w, cudaGetLastError());
+    return SHMEMG_OK;
+}
+
+extern "C" int shmemg_alltoalls_on_stream(shmemg_world_t *w, uint64_t dest_off, uint64_t source_off, uint64_t dst_pe_stride,
+                                          uint64_t src_pe_stride, uint64_t dst_block_stride, uint64_t src_block_stride,
+                                          size_t block_bytes, size_t nblocks, void *stream) {
+    if (!w) return SHMEMG_ERR_ARG;
+    if (block_bytes == 0 || nblocks == 0) return SHMEMG_OK;
+    const uint64_t N = (uint64_t)w->npes, hb = w->heap_bytes;
+    // spans (overflow-safe: every term is checked against the heap size first)
+    if (block_bytes > hb || (N > 1 && (dst_pe_stride > hb || src_pe_stride > hb)) ||
+        (nblocks > 1 && (dst_block_stride > hb || src_block_stride > hb)) || nblocks > hb)
+        return SHMEMG_ERR_RANGE;
+    const uint64_t dspan = (N - 1) * dst_pe_stride + (nblocks - 1) * dst_block_stride + block_bytes;
+    const uint64_t sspan = (N - 1) * src_pe_stride + (nblocks - 1) * src_block_stride + block_bytes;
+    if (!shmemg_in_range(w, dest_off, dspan) || !shmemg_in_range(w, source_off, sspan)) return SHMEMG_ERR_RANGE;
+    if (ranges_overlap(dest_off, source_off, dspan, sspan)) return SHMEMG_ERR_OVERLAP;
+    // destination blocks of one PE pair / of two source PEs that cannot help overlapping
+    if ((nblocks > 1 && dst_block_stride < block_bytes) || (N > 1 && dst_pe_stride < block_bytes)) return SHMEMG_ERR_OVERLAP;
+    A2asArgs a{w->base, w->stride, dest_off, source_off, dst_pe_stride, src_pe_stride, dst_block_stride, src_block_stride,
+               block_bytes, nblocks, w->npes};
+    const uint64_t all = dest_off | source_off | dst_pe_stride | src_pe_stride | dst_block_stride | src_block_stride | block_bytes |
+                         (uint64_t)w->stride | (uint64_t)(uintptr_t)w->base;
+    cudaStream_t st = (cudaStream_t)stream;
+    const uint64_t maxgrid = (uint64_t)w->sm_count * w->ctas_per_sm;
+    if (block_bytes >= 1024 && (all & 15) == 0 && !w->tile_bytes_override) {
+        int rc = collectives_smem_attr(w);
+        if (rc) return rc;
+        const unsigned cpb = (unsigned)((block_bytes + SHMEMG_TMA_TILE - 1) / SHMEMG_TMA_TILE);
+        const uint64_t nwork = N * nblocks * N * cpb;
+        k_alltoalls_tma<<<(unsigned)(nwork < (uint64_t)w->sm_count ? nwork : (uint64_t)w->sm_count), 32, SHMEMG_TMA_SMEM, st>>>(a, cpb);
+    } else if ((block_bytes == 4 || block_bytes == 8 || block_bytes == 16) && (all & (block_bytes - 1)) == 0) {
+        const uint64_t n = N * N * nblocks;
+        const unsigned grid = (unsigned)((n + 255) / 256 < maxgrid * 2 ? (n + 255) / 256 : maxgrid * 2);
+        if (block_bytes == 4) k_alltoalls_elem<unsigned><<<grid, 256, 0, st>>>(a);
+        else if (block_bytes == 8) k_alltoalls_elem<unsigned long long><<<grid, 256, 0, st>>>(a);
+        else k_alltoalls_elem<int4><<<grid, 256, 0, st>>>(a);
+    } else {
+        const unsigned cpb = (unsigned)((block_bytes + 16383) / 16384);
+        const uint64_t nwork = N * nblocks * N * cpb;
+        k_alltoalls_generic<<<(unsigned)(nwork < maxgrid ? nwork : maxgrid), SHMEMG_THREADS, 0, st>>>(a, cpb);
+    }
     SHMEMG_CUDA(w, cudaGetLastError());
     return SHMEMG_OK;
 }

@@ -49,6 +49,10 @@ struct shmemg_world {
     CtlRegion *ctl = nullptr;              // DEVICE
     std::map<uint64_t, size_t> free_list;  // offset -> size, coalesced
     std::map<uint64_t, size_t> live;       // offset -> size of live allocations
+    // the CPU space of the two-space model: npes windows in caller-owned pinned HOST memory
+    uint8_t *cpu_base = nullptr;
+    size_t cpu_heap_bytes = 0, cpu_stride = 0;
+    std::map<uint64_t, size_t> cpu_free_list, cpu_live;
     unsigned sig_seq = 0;
     int ctas_per_sm = 4;                   // copy-class persistent grids: ctas_per_sm * sm_count CTAs
     size_t tile_bytes_override = 0;        // SHMEMG_TILE_BYTES (experiments; forces the register copy path)

@@ -244,6 +244,7 @@ static int launch_ib(shmemg_world *w, uint64_t dest_off, uint64_t source_off, ui
     if (dst_stride && (dspan - block) / dst_stride != nblocks - 1) return SHMEMG_ERR_RANGE;       // overflow
     if (src_stride && (sspan - block) / src_stride != nblocks - 1) return SHMEMG_ERR_RANGE;
     if (!shmemg_in_range(w, dest_off, dspan) || !shmemg_in_range(w, source_off, sspan)) return SHMEMG_ERR_RANGE;
+    if (nblocks > 1 && dst_stride < block) return SHMEMG_ERR_OVERLAP;      // destination blocks would overlap each other
     uint8_t *dst = shmemg_addr(w, dst_pe, dest_off);
     const uint8_t *src = shmemg_addr(w, src_pe, source_off);
     const uint64_t all = (uint64_t)(uintptr_t)dst | (uint64_t)(uintptr_t)src | dst_stride | src_stride | block;

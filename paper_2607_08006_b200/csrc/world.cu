@@ -106,6 +106,7 @@ extern "C" int shmem_query_capabilities(const shmemg_world_t *w, int team, uint6
     // the same membership; they differ in which initiation paths they scope (L357, L412).
     uint64_t c = SHMEMG_CAP_GPU_HEAP_PRESENT | SHMEMG_CAP_DEFAULT_HEAP_IS_GPU | SHMEMG_CAP_PTR_DEVICE_ACCESSIBLE |
                  SHMEMG_CAP_PROGRESS_GPU_ONLY | SHMEMG_CAP_PATH_DIRECT | SHMEMG_CAP_ATOMICS_64;
+    if (w->cpu_base) c |= SHMEMG_CAP_CPU_HEAP_PRESENT;      // the CPU half of the two-space model is attached (L313-L317)
     if (team == SHMEM_TEAM_WORLD)
         c |= SHMEMG_CAP_HOST_INITIATED_GPU_BUFFERS | SHMEMG_CAP_STREAM_TRIGGERED | SHMEMG_CAP_STREAM_COLLECTIVES;
     else
@@ -116,20 +117,26 @@ extern "C" int shmem_query_capabilities(const shmemg_world_t *w, int team, uint6
 }
 
 // ---- symmetric allocator: first fit over a coalescing free list; one offset for all PEs (a2) ---------------
+static int alloc_in(std::map<uint64_t, size_t> &free_list, std::map<uint64_t, size_t> &live, size_t alignment, size_t bytes,
+                    uint64_t *sym_off);
 static int alloc_impl(shmemg_world *w, size_t alignment, size_t bytes, uint64_t *sym_off) {
     if (!w || !sym_off) return SHMEMG_ERR_ARG;
+    return alloc_in(w->free_list, w->live, alignment, bytes, sym_off);
+}
+static int alloc_in(std::map<uint64_t, size_t> &free_list, std::map<uint64_t, size_t> &live, size_t alignment, size_t bytes,
+                    uint64_t *sym_off) {
     if (alignment < SHMEMG_MIN_ALIGN) alignment = SHMEMG_MIN_ALIGN;
     if (alignment & (alignment - 1)) return SHMEMG_ERR_ARG;
     if (bytes == 0) bytes = 1;
     bytes = round_up(bytes, SHMEMG_MIN_ALIGN);
-    for (auto it = w->free_list.begin(); it != w->free_list.end(); ++it) {
+    for (auto it = free_list.begin(); it != free_list.end(); ++it) {
         const uint64_t start = it->first, size = it->second;
         const uint64_t a = round_up(start, alignment);
         if (a + bytes > start + size || a + bytes < a) continue;
-        w->free_list.erase(it);
-        if (a > start) w->free_list[start] = a - start;
-        if (a + bytes < start + size) w->free_list[a + bytes] = start + size - (a + bytes);
-        w->live[a] = bytes;
+        free_list.erase(it);
+        if (a > start) free_list[start] = a - start;
+        if (a + bytes < start + size) free_list[a + bytes] = start + size - (a + bytes);
+        live[a] = bytes;
         *sym_off = a;
         return SHMEMG_OK;
     }
@@ -152,26 +159,93 @@ extern "C" int shmemg_calloc(shmemg_world_t *w, size_t count, size_t size, uint6
     SHMEMG_CUDA(w, cudaMemset2DAsync(w->base + *sym_off, w->stride, 0, width, (size_t)w->npes, (cudaStream_t)stream));
     return SHMEMG_OK;
 }
-extern "C" int shmemg_free(shmemg_world_t *w, uint64_t sym_off) {
-    if (!w) return SHMEMG_ERR_ARG;
-    auto it = w->live.find(sym_off);
-    if (it == w->live.end()) return SHMEMG_ERR_ARG;
+static int free_in(std::map<uint64_t, size_t> &free_list, std::map<uint64_t, size_t> &live, uint64_t sym_off) {
+    auto it = live.find(sym_off);
+    if (it == live.end()) return SHMEMG_ERR_ARG;
     uint64_t start = it->first, size = it->second;
-    w->live.erase(it);
-    auto nxt = w->free_list.lower_bound(start);
-    if (nxt != w->free_list.end() && start + size == nxt->first) {   // merge with the following block
+    live.erase(it);
+    auto nxt = free_list.lower_bound(start);
+    if (nxt != free_list.end() && start + size == nxt->first) {   // merge with the following block
         size += nxt->second;
-        nxt = w->free_list.erase(nxt);
+        nxt = free_list.erase(nxt);
     }
-    if (nxt != w->free_list.begin()) {                                // merge with the preceding block
+    if (nxt != free_list.begin()) {                                // merge with the preceding block
         auto prv = std::prev(nxt);
         if (prv->first + prv->second == start) {
             prv->second += size;
             return SHMEMG_OK;
         }
     }
-    w->free_list[start] = size;
+    free_list[start] = size;
     return SHMEMG_OK;
+}
+extern "C" int shmemg_free(shmemg_world_t *w, uint64_t sym_off) {
+    if (!w) return SHMEMG_ERR_ARG;
+    return free_in(w->free_list, w->live, sym_off);
+}
+
+// ---- the CPU space of the two-space model (Fig. 4) -----------------------------------------------------------
+extern "C" int shmemg_cpu_heap_attach(shmemg_world_t *w, void *host_slab, size_t heap_bytes_per_pe, size_t slab_bytes) {
+    if (!w || !host_slab || heap_bytes_per_pe == 0 || w->cpu_base) return SHMEMG_ERR_ARG;
+    if ((uintptr_t)host_slab % SHMEMG_MIN_ALIGN) return SHMEMG_ERR_ALIGN;
+    const size_t stride = round_up(heap_bytes_per_pe, SHMEMG_STRIDE_ALIGN);
+    if (slab_bytes < (size_t)w->npes * stride) return SHMEMG_ERR_NOMEM;
+    cudaPointerAttributes attr;
+    if (cudaPointerGetAttributes(&attr, host_slab) != cudaSuccess || attr.type != cudaMemoryTypeHost) {
+        cudaGetLastError();
+        return SHMEMG_ERR_ARG;            // pageable or device memory: the CPU space must be page-locked host memory (L456)
+    }
+    w->cpu_base = (uint8_t *)host_slab;
+    w->cpu_heap_bytes = heap_bytes_per_pe;
+    w->cpu_stride = stride;
+    w->cpu_free_list.clear(); w->cpu_live.clear();
+    w->cpu_free_list[0] = heap_bytes_per_pe;
+    return SHMEMG_OK;
+}
+extern "C" int shmemg_cpu_malloc(shmemg_world_t *w, size_t bytes, uint64_t *sym_off) {
+    if (!w || !sym_off || !w->cpu_base) return SHMEMG_ERR_ARG;
+    return alloc_in(w->cpu_free_list, w->cpu_live, SHMEMG_MIN_ALIGN, bytes, sym_off);
+}
+extern "C" int shmemg_cpu_free(shmemg_world_t *w, uint64_t sym_off) {
+    if (!w || !w->cpu_base) return SHMEMG_ERR_ARG;
+    return free_in(w->cpu_free_list, w->cpu_live, sym_off);
+}
+extern "C" void *shmemg_cpu_ptr(const shmemg_world_t *w, uint64_t sym_off, int pe) {
+    if (!w || !w->cpu_base || !shmemg_pe_ok(w, pe) || sym_off >= w->cpu_heap_bytes) return nullptr;
+    return w->cpu_base + (size_t)pe * w->cpu_stride + sym_off;
+}
+
+// put / get between the two spaces: GPU <-> GPU runs the copy kernels, anything that touches the CPU space is a DMA transfer
+extern "C" int shmemg_put_on_stream(shmemg_world_t *w, uint64_t dest_off, uint64_t source_off, size_t nbytes, int pe, int target_pe,
+                                    void *stream);
+static int copy_spaces(shmemg_world *w, int dst_space, int dst_pe, uint64_t dst_off, int src_space, int src_pe, uint64_t src_off,
+                       size_t nbytes, void *stream) {
+    if (!w || dst_space < SHMEMG_SPACE_GPU || dst_space > SHMEMG_SPACE_CPU || src_space < SHMEMG_SPACE_GPU || src_space > SHMEMG_SPACE_CPU)
+        return SHMEMG_ERR_ARG;
+    if ((dst_space == SHMEMG_SPACE_CPU || src_space == SHMEMG_SPACE_CPU) && !w->cpu_base) return SHMEMG_ERR_ARG;
+    if (!shmemg_pe_ok(w, dst_pe) || !shmemg_pe_ok(w, src_pe)) return SHMEMG_ERR_PE;
+    const uint64_t dlim = dst_space == SHMEMG_SPACE_GPU ? w->heap_bytes : w->cpu_heap_bytes;
+    const uint64_t slim = src_space == SHMEMG_SPACE_GPU ? w->heap_bytes : w->cpu_heap_bytes;
+    if (dst_off > dlim || nbytes > dlim - dst_off || src_off > slim || nbytes > slim - src_off) return SHMEMG_ERR_RANGE;
+    if (nbytes == 0) return SHMEMG_OK;
+    uint8_t *d = dst_space == SHMEMG_SPACE_GPU ? shmemg_addr(w, dst_pe, dst_off) : w->cpu_base + (size_t)dst_pe * w->cpu_stride + dst_off;
+    const uint8_t *s = src_space == SHMEMG_SPACE_GPU ? shmemg_addr(w, src_pe, src_off) : w->cpu_base + (size_t)src_pe * w->cpu_stride + src_off;
+    SHMEMG_CUDA(w, cudaMemcpyAsync(d, s, nbytes, cudaMemcpyDefault, (cudaStream_t)stream));
+    return SHMEMG_OK;
+}
+extern "C" int shmemg_put_space_on_stream(shmemg_world_t *w, int dest_space, uint64_t dest_off, int source_space, uint64_t source_off,
+                                          size_t nbytes, int pe, int target_pe, void *stream) {
+    if (w && dest_space == SHMEMG_SPACE_GPU && source_space == SHMEMG_SPACE_GPU)
+        return shmemg_put_on_stream(w, dest_off, source_off, nbytes, pe, target_pe, stream);
+    return copy_spaces(w, dest_space, target_pe, dest_off, source_space, pe, source_off, nbytes, stream);
+}
+extern "C" int shmemg_get_on_stream(shmemg_world_t *w, uint64_t dest_off, uint64_t source_off, size_t nbytes, int pe, int target_pe,
+                                    void *stream);
+extern "C" int shmemg_get_space_on_stream(shmemg_world_t *w, int dest_space, uint64_t dest_off, int source_space, uint64_t source_off,
+                                          size_t nbytes, int pe, int target_pe, void *stream) {
+    if (w && dest_space == SHMEMG_SPACE_GPU && source_space == SHMEMG_SPACE_GPU)
+        return shmemg_get_on_stream(w, dest_off, source_off, nbytes, pe, target_pe, stream);
+    return copy_spaces(w, dest_space, pe, dest_off, source_space, target_pe, source_off, nbytes, stream);
 }
 
 extern "C" void *shmemg_ptr(const shmemg_world_t *w, uint64_t sym_off, int pe) {
