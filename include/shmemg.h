@@ -428,7 +428,6 @@ typedef struct shmemg_device_world {
     int32_t reserved;
     unsigned int *bar_count;    /* DEVICE: device-barrier arrival counter (control region)                    */
     unsigned int *bar_gen;      /* DEVICE: device-barrier generation                                          */
-    unsigned int *bar_flags;    /* DEVICE: one monotonic slot per PE of the flag barrier (shmemg_dev_barrier_all_block_pe) */
 } shmemg_device_world_t;
 /* Fill *out (HOST) for world w; valid until shmemg_finalize. */
 SHMEMG_API int shmemg_device_world_get(const shmemg_world_t *w, shmemg_device_world_t *out);

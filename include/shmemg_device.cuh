@@ -367,37 +367,6 @@ __device__ __forceinline__ void shmemg_dev_put_signal_nbi(const shmemg_device_wo
     shmemg_dev_ctx_push(c, r);
 }
 
-/* The same barrier for callers that know which PE they act for (one thread block per PE, all co-resident): FLAG barrier, no
- * read-modify-write -- block p publishes the barrier's number in slot p (release), its first warp polls all slots (relaxed,
- * 128 slots per 16-byte-per-lane probe) and fences once.  Do not mix with shmemg_dev_barrier_all_block in one kernel. */
-__device__ __forceinline__ void shmemg_dev_barrier_all_block_pe(const shmemg_device_world_t &w, int pe) {
-    shmemg_dev_fence_gpu();                 /* every thread: its own earlier updates */
-    __syncthreads();
-    if (shmemg_dev_block_tid() < 32) {
-        const unsigned lane = (unsigned)shmemg_dev_block_tid(), npes = (unsigned)w.npes;
-        unsigned gen;
-        asm volatile("ld.relaxed.gpu.global.u32 %0, [%1];" : "=r"(gen) : "l"(w.bar_flags + pe) : "memory");
-        ++gen;
-        __syncwarp();
-        if (lane == 0) asm volatile("st.relaxed.gpu.global.u32 [%0], %1;" ::"l"(w.bar_flags + pe), "r"(gen) : "memory");
-        for (unsigned q0 = 0; q0 < npes; q0 += 128) {
-            const unsigned q = q0 + 4 * lane;
-            for (;;) {
-                bool ok = true;
-                if (q < npes) {
-                    unsigned f0, f1, f2, f3;
-                    asm volatile("ld.relaxed.gpu.global.v4.u32 {%0,%1,%2,%3}, [%4];" : "=r"(f0), "=r"(f1), "=r"(f2), "=r"(f3) : "l"(w.bar_flags + q) : "memory");
-                    ok = (int)(f0 - gen) >= 0 && (q + 1 >= npes || (int)(f1 - gen) >= 0) && (q + 2 >= npes || (int)(f2 - gen) >= 0) &&
-                         (q + 3 >= npes || (int)(f3 - gen) >= 0);
-                }
-                if (__all_sync(0xffffffffu, ok)) break;
-            }
-        }
-        shmemg_dev_fence_gpu();
-    }
-    __syncthreads();
-}
-
 /* ---- device collectives (PAPER L226 case study 3 "thread-collaborative collective reductions", L363-L371, Table 6 "Device
  * collectives: if provided, uniform participation") ------------------------------------------------------------------------
  * Block scope, ONE thread block per PE: ALL npes blocks (co-resident: cooperative launch) call the routine with the same
@@ -421,7 +390,7 @@ __device__ __forceinline__ void shmemg_dev_sum_share(const shmemg_device_world_t
 }
 __device__ __forceinline__ void shmemg_dev_sum_reduce_block(const shmemg_device_world_t &w, int dtype, uint64_t dest_off,
                                                             uint64_t source_off, size_t nreduce, int pe) {
-    shmemg_dev_barrier_all_block_pe(w, pe);
+    shmemg_dev_barrier_all_block(w);
     const int tid = shmemg_dev_block_tid(), nthr = shmemg_dev_block_size();
     const size_t per = (nreduce + (size_t)w.npes - 1) / (size_t)w.npes;
     const size_t lo = per * (size_t)pe < nreduce ? per * (size_t)pe : nreduce, hi = lo + per < nreduce ? lo + per : nreduce;
@@ -454,34 +423,34 @@ __device__ __forceinline__ void shmemg_dev_sum_reduce_block(const shmemg_device_
     } else {
         shmemg_dev_sum_share<double, double>(w, dest_off, source_off, lo, hi, tid, nthr);
     }
-    shmemg_dev_barrier_all_block_pe(w, pe);
+    shmemg_dev_barrier_all_block(w);
 }
 /* every PE's dest[p*nbytes .. +nbytes) = PE p's source: block p puts its block into all N windows */
 __device__ __forceinline__ void shmemg_dev_fcollect_block(const shmemg_device_world_t &w, uint64_t dest_off, uint64_t source_off,
                                                           size_t nbytes, int pe) {
-    shmemg_dev_barrier_all_block_pe(w, pe);
+    shmemg_dev_barrier_all_block(w);
     const int tid = shmemg_dev_block_tid(), nthr = shmemg_dev_block_size();
     for (int j = 0; j < w.npes; ++j)
         shmemg_dev_copy(shmemg_dev_ptr(w, dest_off + (uint64_t)pe * nbytes, j), shmemg_dev_ptr(w, source_off, pe), nbytes, tid, nthr);
-    shmemg_dev_barrier_all_block_pe(w, pe);
+    shmemg_dev_barrier_all_block(w);
 }
 /* PE j's dest[i*nbytes .. +nbytes) = PE i's source[j*nbytes .. +nbytes): block i puts its N blocks */
 __device__ __forceinline__ void shmemg_dev_alltoall_block(const shmemg_device_world_t &w, uint64_t dest_off, uint64_t source_off,
                                                           size_t nbytes, int pe) {
-    shmemg_dev_barrier_all_block_pe(w, pe);
+    shmemg_dev_barrier_all_block(w);
     const int tid = shmemg_dev_block_tid(), nthr = shmemg_dev_block_size();
     for (int j = 0; j < w.npes; ++j)
         shmemg_dev_copy(shmemg_dev_ptr(w, dest_off + (uint64_t)pe * nbytes, j), shmemg_dev_ptr(w, source_off + (uint64_t)j * nbytes, pe),
                         nbytes, tid, nthr);
-    shmemg_dev_barrier_all_block_pe(w, pe);
+    shmemg_dev_barrier_all_block(w);
 }
 /* every PE's dest = the root's source: every block gets the root's block (the root's own dest included) */
 __device__ __forceinline__ void shmemg_dev_broadcast_block(const shmemg_device_world_t &w, uint64_t dest_off, uint64_t source_off,
                                                            size_t nbytes, int root_pe, int pe) {
-    shmemg_dev_barrier_all_block_pe(w, pe);
+    shmemg_dev_barrier_all_block(w);
     shmemg_dev_copy(shmemg_dev_ptr(w, dest_off, pe), shmemg_dev_ptr(w, source_off, root_pe), nbytes, shmemg_dev_block_tid(),
                     shmemg_dev_block_size());
-    shmemg_dev_barrier_all_block_pe(w, pe);
+    shmemg_dev_barrier_all_block(w);
 }
 
 #endif /* __CUDACC__ */

@@ -56,11 +56,8 @@ __device__ __forceinline__ unsigned long long shfl64(unsigned long long v, int l
     return __shfl_sync(FULL, v, lane);
 }
 
-#ifndef AMO_MIN_CTAS
-#define AMO_MIN_CTAS 1
-#endif
 template <int IDXB, int OP, bool AGG, bool TEST>
-__global__ void __launch_bounds__(256, AMO_MIN_CTAS) k_amo(const AmoArgs a) {
+__global__ void __launch_bounds__(256) k_amo(const AmoArgs a) {     // (256, 6) and (256, 8) spill and are slower: 661 / 757 us vs 590 (C4 CAS)
     typedef typename IdxT<IDXB>::type idx_t;
     const idx_t *__restrict__ idx = reinterpret_cast<const idx_t *>(a.idx);
     const int *__restrict__ tgt = a.tgt_pe;

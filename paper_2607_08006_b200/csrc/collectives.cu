@@ -407,44 +407,33 @@ __global__ void k_reduce_scalar(uint8_t *base, size_t stride, uint64_t dst_off, 
 // ---- barriers ---------------------------------------------------------------------------------------------------------
 __global__ void k_barrier_epoch(CtlRegion *ctl) { atomicAdd(&ctl->barrier_epoch, 1ull); }
 
-// One CTA (one warp) per PE agent, all co-resident (cooperative launch).  FLAG barrier at GPU scope: agent p publishes the
-// barrier's number in its own slot (release), then its warp polls everybody's slots (relaxed loads, 32 slots per probe round)
-// and fences once.  No read-modify-write anywhere: the critical path is one store becoming visible plus one load round trip.
-// Measured per barrier: 128 agents 1.65 us, 8 agents 0.8 us, 2 agents 1.0 us (= one store becoming visible to another SM plus
-// one load round trip; back-off between probes does not help).  The counter + generation barrier it replaces took 1.8 us for
-// 128 agents (atomic round trip, release store, poll round trip), a two-level counter tree 2.4 us.  Slots are monotonic.
-__device__ __forceinline__ void pe_barrier_flags(unsigned *flags, unsigned npes, unsigned p, unsigned &gen) {
-    const unsigned lane = threadIdx.x & 31;
-    ++gen;
-    if (lane == 0) {
-        fence_acquire();                                         // fence.acq_rel.gpu: release of everything the agent did before
-        asm volatile("st.relaxed.gpu.global.u32 [%0], %1;" ::"l"(flags + p), "r"(gen) : "memory");
+// One CTA per PE agent, all co-resident (cooperative launch).  Sense-reversing counter barrier at GPU scope: one acq_rel arrival
+// atomic per agent, the last arriver resets the counter and releases the generation word, the others poll it with relaxed
+// loads (no L1 invalidate per probe) and fence once.  1.8 us per barrier for 128 agents = atomic round trip + release store +
+// poll round trip.  Measured and not kept: a two-level counter tree (2.4 us: two atomic round trips in series) and a
+// flag barrier without read-modify-write (every agent publishes its slot and polls all slots with 16-byte loads: 0.8 us for 8
+// agents, but 1.65 - 3.15 us for 128 depending on where the agents land: 128 pollers on four L2 lines).
+__device__ __forceinline__ void pe_barrier(CtlRegion *ctl, unsigned npes, unsigned &gen) {
+    // thread 0 of the CTA acts for the PE
+    unsigned old;
+    asm volatile("atom.acq_rel.gpu.global.add.u32 %0, [%1], 1;" : "=r"(old) : "l"(&ctl->bar_count) : "memory");
+    if (old == npes - 1) {
+        ctl->bar_count = 0;                                      // ordered before the release below
+        asm volatile("st.release.gpu.global.u32 [%0], %1;" ::"l"(&ctl->bar_gen), "r"(gen + 1) : "memory");
+    } else {
+        while (ld_relaxed_u32(&ctl->bar_gen) == gen) { }
+        fence_acquire();
     }
-    // one 16-byte load per lane covers 128 slots (512 B = 16 sectors per probe round and agent: slots are packed on purpose,
-    // every agent reads all of them and the L2 serves about a sector per clock and slice)
-    for (unsigned q0 = 0; q0 < npes; q0 += 128) {
-        const unsigned q = q0 + 4 * lane;
-        for (;;) {
-            bool ok = true;
-            if (q < npes) {
-                unsigned f0, f1, f2, f3;
-                asm volatile("ld.relaxed.gpu.global.v4.u32 {%0,%1,%2,%3}, [%4];" : "=r"(f0), "=r"(f1), "=r"(f2), "=r"(f3) : "l"(flags + q) : "memory");
-                ok = (int)(f0 - gen) >= 0 && (q + 1 >= npes || (int)(f1 - gen) >= 0) && (q + 2 >= npes || (int)(f2 - gen) >= 0) &&
-                     (q + 3 >= npes || (int)(f3 - gen) >= 0);      // wrap-safe
-            }
-            if (__all_sync(0xffffffffu, ok)) break;
-        }
-    }
-    fence_acquire();
+    gen++;
 }
 
 __global__ void __launch_bounds__(32) k_barrier_repeat(CtlRegion *ctl, uint8_t *base, size_t stride, unsigned npes,
                                                        unsigned count, unsigned long long stamp_off, int do_stamp) {
+    if (threadIdx.x != 0) return;
     const unsigned p = blockIdx.x;
-    unsigned *flags = ctl->bar_flags;
-    unsigned gen = ld_relaxed_u32(flags + p);                     // my own slot: the number of the last barrier I took part in
+    unsigned gen = ld_acquire_u32(&ctl->bar_gen);          // all agents read the same value: nobody has arrived yet
     if (!do_stamp) {
-        for (unsigned r = 0; r < count; ++r) pe_barrier_flags(flags, npes, p, gen);
+        for (unsigned r = 0; r < count; ++r) pe_barrier(ctl, npes, gen);
         return;
     }
     volatile unsigned long long *mine = reinterpret_cast<volatile unsigned long long *>(base + (size_t)p * stride + stamp_off);
@@ -452,14 +441,13 @@ __global__ void __launch_bounds__(32) k_barrier_repeat(CtlRegion *ctl, uint8_t *
         reinterpret_cast<volatile unsigned long long *>(base + (size_t)((p + 1) % npes) * stride + stamp_off);
     unsigned long long bad = 0;
     for (unsigned r = 1; r <= count; ++r) {
-        if (threadIdx.x == 0) right[r & 1] = r;      // "put" r into slot r&1 of the right neighbour
-        __syncwarp();
-        pe_barrier_flags(flags, npes, p, gen);       // barrier_all: the put is complete and visible
-        if (threadIdx.x == 0 && mine[r & 1] != r) bad++;      // my left neighbour's stamp of THIS round must be there
+        right[r & 1] = r;                 // "put" r into slot r&1 of the right neighbour
+        pe_barrier(ctl, npes, gen);       // barrier_all: the put is complete and visible
+        if (mine[r & 1] != r) bad++;      // my left neighbour's stamp of THIS round must be there
         // no second barrier needed: slot r&1 is next written in round r+2, i.e. after barrier r+1, which this
         // agent only reaches after the read above
     }
-    if (threadIdx.x == 0) mine[2] += bad;
+    mine[2] += bad;
 }
 
 // ---------------------------------------------------------------------------------------------------------
@@ -677,7 +665,7 @@ extern "C" int shmemg_barrier_all_repeat_on_stream(shmemg_world_t *w, uint32_t c
     if (count == 0) return SHMEMG_OK;
     int per_sm = 0;
     SHMEMG_CUDA(w, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_barrier_repeat, 32, 0));
-    if ((long long)per_sm * w->sm_count < w->npes || w->npes > SHMEMG_BAR_FLAGS) return SHMEMG_ERR_NOMEM;   // agents could not all be co-resident
+    if ((long long)per_sm * w->sm_count < w->npes) return SHMEMG_ERR_NOMEM;   // agents could not all be co-resident
     CtlRegion *ctl = w->ctl;
     uint8_t *base = w->base;
     size_t stride = w->stride;

@@ -18,7 +18,6 @@ extern "C" int shmemg_device_world_get(const shmemg_world_t *w, shmemg_device_wo
     out->reserved = 0;
     out->bar_count = &w->ctl->bar_count;
     out->bar_gen = &w->ctl->bar_gen;
-    out->bar_flags = w->ctl->bar_flags;
     return SHMEMG_OK;
 }
 
@@ -138,7 +137,7 @@ extern "C" int shmemg_device_collective_on_stream(shmemg_world_t *w, int kind, i
     if (overlap && !(kind == SHMEMG_DEVCOLL_SUM_REDUCE && dest_off == source_off)) return SHMEMG_ERR_OVERLAP;
     int per_sm = 0;
     SHMEMG_CUDA(w, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_device_collective, COLL_THREADS, 0));
-    if ((long long)per_sm * w->sm_count < w->npes || w->npes > SHMEMG_BAR_FLAGS) return SHMEMG_ERR_NOMEM;
+    if ((long long)per_sm * w->sm_count < w->npes) return SHMEMG_ERR_NOMEM;
     shmemg_device_world_t dw;
     shmemg_device_world_get(w, &dw);
     void *args[] = {&dw, &kind, &dtype, &dest_off, &source_off, &n, &root};

@@ -19,7 +19,6 @@
 #define SHMEMG_TMA_TILE 32768u             // bytes per bulk-copy stage
 #define SHMEMG_TMA_STAGES 4                // stages per CTA (128 KiB of shared memory, one CTA per SM)
 #define SHMEMG_SIG_SLOTS 1024              // completion counters for single put_signal launches
-#define SHMEMG_BAR_FLAGS 2048               // PE agents the in-kernel flag barrier supports
 #define SHMEMG_HOT_MAX 512                 // hot words tracked by SHMEMG_AMO_HOT_AGGREGATE
 
 // ---- control region layout (device) -------------------------------------------------------------------
@@ -30,7 +29,6 @@ struct CtlRegion {
     unsigned int pad[12];
     unsigned int sig_counter[SHMEMG_SIG_SLOTS];   // last-arriver counters of single put_signal launches
     unsigned int group_bar[128];           // per-PE arrival counters of multi-block PE agents (monotonic; halo_app.cu)
-    unsigned int bar_flags[SHMEMG_BAR_FLAGS];   // in-kernel flag barrier: slot p = number of the last barrier agent p has entered
     unsigned int amo_done;                 // SHMEMG_AMO_THEN_BARRIER: CTAs of the AMO kernel that have finished
     unsigned int hot_n;                    // SHMEMG_AMO_HOT_AGGREGATE: number of hot words found by the sampling kernel
     unsigned int hot_done;                 // CTAs of the sampling kernel that have staged their keys
