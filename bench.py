@@ -10,7 +10,8 @@ call is bracketed by CUDA events on the launching stream ("segments"); applicati
 (perturb, pack) and the re-initialisation of AMO targets run between segments and are not library time.
 
   metric `rma_alltoall_GBps` : algorithmic bytes of the copy-class segments (put / put_signal / alltoall / fcollect /
-                               sum_reduce; read + write) / their summed device time, summed over ranks
+                               sum_reduce; read + write) / their summed device time, summed over ranks; the 50 halo rounds
+                               are replayed from one CUDA graph (one event pair around 50 back-to-back launches)
   `amo_mops`                 : AMO ops of C1 + C4 / their summed device time
   `barrier`                  : us per barrier, in-kernel (128 co-resident PE agents) and stream-level
   `roofline`                 : the copy-class kernel with the largest share of the timed step, against MEASURED_PEAKS.json
@@ -177,8 +178,14 @@ def segment_table(inp: Inputs):
     if "c3b" in g:
         seg["put_batch_skewed"] = dict(cls="copy", kernel="k_batch_exec", bytes=2 * int(inp.c3b.sizes.sum()), launches=1)
     if "c2" in g:
+        # the 50 pre-planned rounds replayed from ONE CUDA graph (the launch-bound inner loop of the application), one event
+        # pair around the replay: 50 back-to-back launches of k_batch_exec, nothing else in the timed region
         seg["halo_put_signal_wait"] = dict(cls="copy", kernel="k_batch_exec",
                                            bytes=HALO_ROUNDS * 2 * 48 * inp.halo.face_bytes, launches=HALO_ROUNDS)
+        # the same 50 launches enqueued one by one from the host between the application's kernels, an event pair around
+        # EACH launch (round 1's measurement; an event pair around any kernel costs about 6 us whatever the kernel does)
+        seg["halo_put_signal_wait_event_pairs"] = dict(cls="xcopy", kernel="k_batch_exec",
+                                                       bytes=HALO_ROUNDS * 2 * 48 * inp.halo.face_bytes, launches=HALO_ROUNDS)
     # the ONE-CALL form of the two batch workloads (shmemg_enqueue_batch: device-resident descriptors planned on the device
     # inside the timed segment, 2 launches); reported beside the pre-planned form, not part of `value`
     if "c3b" in g:
@@ -222,6 +229,10 @@ def segment_table(inp: Inputs):
             seg["next1_halo_app_host_batches"] = dict(cls="xtime", kernel="k_halo_perturb + k_halo_pack + k_batch_exec", ops=HALO_ROUNDS, launches=3 * HALO_ROUNDS)
             seg["next1_halo_app_persistent"] = dict(cls="xtime", kernel="k_halo_persistent (device-initiated)", ops=HALO_ROUNDS, launches=1)
             seg["next1_halo_app_compute_only"] = dict(cls="xtime", kernel="k_halo_perturb", ops=HALO_ROUNDS, launches=HALO_ROUNDS)
+            # the application loop from a CUDA graph, with and without the library's launches: the difference is what a
+            # round of put_signal + wait adds to the application's critical path
+            seg["next1_halo_app_graph"] = dict(cls="xtime", kernel="graph: k_halo_perturb + k_halo_pack + k_batch_exec", ops=HALO_ROUNDS, launches=3 * HALO_ROUNDS)
+            seg["next1_halo_app_graph_without_exchange"] = dict(cls="xtime", kernel="graph: k_halo_perturb + k_halo_pack", ops=HALO_ROUNDS, launches=2 * HALO_ROUNDS)
             seg["next2_ibput_faces"] = dict(cls="xcopy", kernel="k_ib_tma/k_ib_elem", bytes=3 * 2 * inp.halo.face_bytes, launches=3)
     if "next4" in g:
         seg["next4_fft_transpose_alltoalls"] = dict(cls="xcopy", kernel="k_alltoalls_tma", bytes=2 * inp.fft.A.size, launches=1)
@@ -286,6 +297,7 @@ class CudaBench:
         self.app_launches = 0
         self.plan_us = {}                              # host planning cost of the pre-planned batches (outside every timed region)
         self.barrier_graph = None
+        self.halo_graphs = None                        # CUDA graphs of the 50 halo rounds (captured in the first step)
         self.worlds = []
         self.flags = 0                                 # warp aggregation buys nothing on these streams (profiles/)
         self.fadd_flags = AMO_HOT_AGGREGATE            # RMAT stream: the hot words are combined per CTA chunk (profiles/r01d)
@@ -425,8 +437,24 @@ class CudaBench:
                     w.app_halo_perturb(self.U_off, h.B, h.seed, r)       # application compute, not library time
                     w.app_halo_pack(send_off, self.U_off, h.B)
                     self.app_launches += 2
-                    with rec.seg("halo_put_signal_wait"):
+                    with rec.seg("halo_put_signal_wait_event_pairs"):
                         w.enqueue_batch(self.halo_batches[r - 1])
+            if self.halo_graphs is None:
+                self.halo_graphs = self._capture_halo_graphs()
+            lib_g, app_g, app_only_g = self.halo_graphs
+            self.ld2.obj("sig").zero_()
+            w.app_halo_pack(send_off, self.U_off, h.B)                   # faces as the application leaves them (outside the timed region)
+            self.app_launches += 1
+            with rec.seg("halo_put_signal_wait"):
+                lib_g.replay()
+            w.launches += HALO_ROUNDS
+            if "next2" in g:
+                with rec.seg("next1_halo_app_graph"):
+                    app_g.replay()
+                w.launches += HALO_ROUNDS
+                with rec.seg("next1_halo_app_graph_without_exchange"):
+                    app_only_g.replay()
+                self.app_launches += 4 * HALO_ROUNDS
         if "c3b" in g:
             with rec.seg("put_batch_skewed_onecall"):
                 self.w3b.enqueue_batch_dev(self.ops3b_dev, self.plan_us["put_batch_skewed"]["nops"], self.work3b)
@@ -489,6 +517,28 @@ class CudaBench:
             with rec.seg("barrier_on_stream_graph"):
                 self.barrier_graph.replay()
                 self.w5.launches += BARRIERS
+
+    def _capture_halo_graphs(self):
+        """Three CUDA graphs over the 50 halo rounds: the library's launches alone (back to back), the application loop
+        (perturb, pack, batch) and the application loop without the exchange.  The pre-planned batches are re-enqueueable
+        (monotonic counters), so a captured launch replays any number of times."""
+        torch, h, w = self.torch, self.inp.halo, self.w2
+        send_off, l0, a0 = self.ld2.off["send"][0], w.launches, self.app_launches
+        graphs = []
+        for app, lib in ((False, True), (True, True), (True, False)):
+            gr = torch.cuda.CUDAGraph()
+            with torch.cuda.graph(gr):
+                if app:
+                    self.ld2.obj("sig").zero_()
+                for r in range(1, HALO_ROUNDS + 1):
+                    if app:
+                        w.app_halo_perturb(self.U_off, h.B, h.seed, r)
+                        w.app_halo_pack(send_off, self.U_off, h.B)
+                    if lib:
+                        w.enqueue_batch(self.halo_batches[r - 1])
+            graphs.append(gr)
+        w.launches, self.app_launches = l0, a0                           # capturing launches nothing
+        return graphs
 
     # ---- end-to-end: the same ops with HOST buffers, H2D / D2H inside the timed region --------------------------------
     def setup_e2e(self):
@@ -708,7 +758,26 @@ class CudaBench:
                 o2.obj("send")[:] = snaps[r]
                 o2.exec_ops(ob.ops2[r - 1])
             assert np.array_equal(ghost, o2.obj("ghost")) and np.array_equal(sig, o2.obj("sig")), "halo ghosts / signal words"
-            ok["halo_put_signal_wait"] = True
+            ok["halo_put_signal_wait_event_pairs"] = True
+            # the timed form: the 50 rounds replayed from the CUDA graph of the library's launches (every round sends what
+            # `send` holds; rounds 49 and 50 fill the two ghost parities, the signal words end at 50)
+            if self.halo_graphs is not None:
+                self.ld2.obj("ghost").zero_()
+                self.ld2.obj("sig").zero_()
+                self.halo_graphs[0].replay()
+                o2.obj("ghost")[:] = 0
+                o2.obj("sig")[:] = 0
+                o2.obj("send")[:] = host(self.ld2.obj("send"))
+                for r in (HALO_ROUNDS - 1, HALO_ROUNDS):
+                    o2.exec_ops(ob.ops2[r - 1])
+                assert np.array_equal(host(self.ld2.obj("ghost")), o2.obj("ghost")), "halo ghosts after the graph replay"
+                assert np.array_equal(host(self.ld2.obj("sig")), o2.obj("sig")), "halo signal words after the graph replay"
+                ok["halo_put_signal_wait"] = True
+                o2.obj("ghost")[:] = 0
+                o2.obj("sig")[:] = 0
+                for r in sorted(snaps):
+                    o2.obj("send")[:] = snaps[r]
+                    o2.exec_ops(ob.ops2[r - 1])
             self.ld2.obj("ghost").zero_()                            # the same two rounds through the one-call form
             self.ld2.obj("sig").zero_()
             for r in sorted(snaps):
@@ -899,7 +968,11 @@ def base_line(args, n_gpus):
                              "uses of any buffer; by-nature L2-resident cases (C1's 512 KiB target, halo faces just packed) "
                              "are kept as the application leaves them",
                        "value_definition": "copy-class algorithmic bytes / summed CUDA-event time of the copy-class "
-                                           "segments (library calls only), summed over ranks"}}
+                                           "segments (library calls only), summed over ranks",
+                       "launch": "single collectives and the Zipf batch: one event pair around the one launch; the 50 halo "
+                                 "rounds (a launch-bound inner loop, 48 MiB per 10 us launch): replayed from ONE CUDA graph of "
+                                 "the 50 pre-planned batch launches, one event pair around the replay; the same launches with "
+                                 "an event pair around each are reported as halo_put_signal_wait_event_pairs"}}
 
 
 def run_reference(args):
