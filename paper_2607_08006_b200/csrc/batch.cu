@@ -147,6 +147,17 @@ __global__ void __launch_bounds__(EXEC_THREADS, 1) k_batch_exec(const ExecArgs a
         STG = (unsigned)h1.x; NST = (unsigned)h1.y;
         ep.all_total = at;
     }
+    // Pre-planned batch: every launch is a programmatic dependent of whatever kernel precedes it in the stream.  Its tile
+    // records are immutable, so the loader's first record is requested now; nothing mutable (ticket, counters, signal
+    // words, payload) is touched before griddepcontrol.wait, which returns when the preceding grid has completed and its
+    // writes are visible.  The executor releases ITS dependents at once: a following executor launch sets up its CTAs
+    // (as SMs become free) while this one still runs, and blocks in the same wait.
+    TileRec r0 = {};
+    if (!a.hdr) {
+        if (tid == 0 && blockIdx.x < ntiles) r0 = ld_rec(tiles + blockIdx.x);
+        asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+        asm volatile("griddepcontrol.wait;" ::: "memory");
+    }
     __syncthreads();
 
     if (tid == 0) {
@@ -159,8 +170,7 @@ __global__ void __launch_bounds__(EXEC_THREADS, 1) k_batch_exec(const ExecArgs a
         // through the epochB mbarrier before their first completion accounting.
         TRACE(1);
         const unsigned long long tk0 = a.hdr ? 0ull : ld_relaxed_u64(a.ticket);   // one-call plans start at launch index 0
-        TileRec r0 = {};
-        if (blockIdx.x < ntiles) r0 = ld_rec(tiles + blockIdx.x);
+        if (a.hdr && blockIdx.x < ntiles) r0 = ld_rec(tiles + blockIdx.x);
         unsigned ia = 0, ig = 0;                                     // ia = stage index, pa = its lap parity
         unsigned pa = 0, nissued = 0;
         auto issue = [&](const TileRec &r, unsigned off) {
@@ -437,6 +447,7 @@ static uint32_t pick_seg_tiles(const shmemg_world *w, const shmemg_op_t *ops, si
         if (ops[i].opcode >= SHMEMG_OP_PUT && ops[i].opcode <= SHMEMG_OP_PUT_SIGNAL)
             tiles += (ops[i].nbytes + SHMEMG_TMA_TILE - 1) / SHMEMG_TMA_TILE;
     const uint64_t per_sm = (tiles + w->sm_count - 1) / w->sm_count;
+    if (const char *e = getenv("SHMEMG_SEG_TILES")) return (uint32_t)atoi(e);      // experiments
     if (per_sm >= SEG_TILES_MAX) return SEG_TILES_MAX;
     return per_sm < 1 ? 1u : (uint32_t)per_sm;
 }
@@ -723,7 +734,8 @@ int shmemg_exec_launch(shmemg_world *w, const ExecArgs &a, unsigned grid, size_t
     cudaLaunchAttribute at[1];
     at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
     at[0].val.programmaticStreamSerializationAllowed = 1;
-    cfg.attrs = at; cfg.numAttrs = (after_planner && !getenv("SHMEMG_NO_PDL")) ? 1 : 0;     // SHMEMG_NO_PDL: experiments
+    (void)after_planner;
+    cfg.attrs = at; cfg.numAttrs = getenv("SHMEMG_NO_PDL") ? 0 : 1;     // SHMEMG_NO_PDL: experiments
     SHMEMG_CUDA(w, cudaLaunchKernelEx(&cfg, k_batch_exec, a));
     return SHMEMG_OK;
 }
