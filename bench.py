@@ -207,9 +207,10 @@ def segment_table(inp: Inputs):
         seg["atomic_add_steady_2p24"] = dict(cls="xamo", kernel="k_amo<add>", ops=len(inp.c1_steady.val), launches=1, bytes_per_op=20)
     if "c4" in g:
         E = len(inp.c4.u)
-        # fetch-add: tgt_pe 4 + idx 4 read, 8 fetched written; compare-swap: tgt_pe 4 + idx 4 + val 8 read, 8 fetched written
+        # fetch-add: tgt_pe 4 + idx 4 read, 8 fetched written; plain compare-swap: tgt_pe 4 + idx 4 + val 8 read, 8 fetched written
         seg["atomic_fetch_add"] = dict(cls="amo", kernel="k_hot_sample + k_amo_hot_main<fetch_add>", ops=E, launches=2, bytes_per_op=16)
-        seg["atomic_compare_swap"] = dict(cls="amo", kernel="k_amo<compare_swap, test-before-swap>", ops=E, launches=1, bytes_per_op=24)
+        # test-before-swap, streaming form: tgt_pe 4 + idx 4 read, 8 fetched written; val (8) is read only by the ops that issue the atomic
+        seg["atomic_compare_swap"] = dict(cls="amo", kernel="k_cas_test (test-before-swap, L1-served test loads, lazy val)", ops=E, launches=1, bytes_per_op=16)
         # every op an L2 atomic (no test load): the variant the atom.cas ceiling bounds; reported, not part of `amo_mops`
         seg["atomic_compare_swap_plain"] = dict(cls="xamo", kernel="k_amo<compare_swap>", ops=E, launches=1, bytes_per_op=24)
     if "next2" in g:
@@ -1120,9 +1121,10 @@ def run_cuda(args):
     if "atomic_fetch_add" in segments and "atom_add_rmat_stream_Mops" in ceil:
         segments["atomic_fetch_add"]["vs_bare_atom_add_on_the_same_stream"] = segments["atomic_fetch_add"]["Mops"] / ceil["atom_add_rmat_stream_Mops"]
     if "atomic_compare_swap" in segments:
-        segments["atomic_compare_swap"]["note"] = ("test-before-swap: most of the 2^26 ops are resolved by a coherent load, so the atom.cas "
-                                                   "probe does not bound this variant; its own bound is the operand / result stream "
-                                                   "(bytes_per_op, frac_of_measured_hbm)")
+        segments["atomic_compare_swap"]["note"] = ("test-before-swap: most of the 2^26 ops are resolved by a load (served by L1 for the hot "
+                                                   "slots), so the atom.cas probe does not bound this variant; its HBM traffic is the operand / "
+                                                   "result stream (bytes_per_op, frac_of_measured_hbm) plus one 32-byte sector per slot that is "
+                                                   "claimed; the random 8-byte test loads are L2 hits (32 MiB of slots)")
     if "atomic_compare_swap_plain" in segments and "atom_cas_32MiB_Mops" in ceil:
         segments["atomic_compare_swap_plain"]["frac_of_l2_atomic_ceiling"] = segments["atomic_compare_swap_plain"]["Mops"] / ceil["atom_cas_32MiB_Mops"]
         if "atom_cas_rmat_stream_Mops" in ceil:

@@ -266,9 +266,11 @@ SHMEMG_API int shmemg_quiet(shmemg_world_t *w, int pe, void *stream);
  * There is NO ordering between the ops of one call (reading 7); fetched values are valid when the stream
  * has passed the call.  flags: SHMEMG_AMO_* below.  64-bit integer types only (wraparound add). */
 #define SHMEMG_AMO_WARP_AGGREGATE 1u   /* combine same-address ops of a warp into one L2 atomic */
-/* compare-swap with a scalar cond only: read the word first (coherent L2 load) and issue the L2 atomic only while the
- * word may still equal cond.  Legal because the ops of one call are unordered and each swaps only cond -> val: once a
- * word differs from cond no op of the call can change it, so the loaded value is the failed swap's fetched value.
+/* compare-swap with a scalar cond only: read the word first and issue the L2 atomic only while the word may still equal
+ * cond.  Legal because the ops of one call are unordered and each swaps only cond -> val: once a word differs from cond no
+ * op of the call can change it, so the loaded value is the failed swap's fetched value (the load may be served by the SM's
+ * L1, which is empty when the call starts: a value found there was the word's value at some instant of this call; a stale
+ * cond is decided by the L2 atomic that follows).  The op's val is read only when the atomic is issued.
  * Requires that nothing outside this call updates the target words while it runs (already undefined). */
 #define SHMEMG_AMO_TEST_BEFORE_SWAP 2u
 /* add / fetch-add with a scalar value (val == NULL), meant for skewed streams (same-line serialisation at the L2 atomic

@@ -10,7 +10,7 @@ from litmus_model import enumerate_outcomes, to_spec_program
 from paper_2607_08006_b200 import CMP, ERR, OP, OP_DTYPE, ShmemgError, World
 from paper_2607_08006_b200.loader import Loaded
 from workloads import configs, gen, litmus
-from workloads.spec import Program
+from workloads.spec import SIGNAL_ADD, Program
 
 pytestmark = pytest.mark.gpu
 M64 = (1 << 64) - 1
@@ -161,6 +161,41 @@ def test_batch_can_be_enqueued_repeatedly_and_stream_order_holds():
     assert np.array_equal(ld.obj_numpy("src"), src0)              # transpose of transpose
 
 
+def test_batches_captured_in_a_cuda_graph_replay_with_stream_order():
+    """A pre-planned batch is re-enqueueable (monotonic counters), so its launch can be captured in a CUDA graph and replayed.
+    Every executor launch is a programmatic dependent of the kernel before it (griddepcontrol.wait before anything mutable is
+    touched): inside the graph, batch B must still read everything batch A wrote, replay after replay."""
+    npes, blk = 8, 20000
+    a = configs.c3a_put_program(npes, blk)                       # src -> dst (transpose)
+    a.obj("sig", 8 * npes)
+    b = a.fork()
+    for i in range(npes):
+        for j in range(npes):
+            b.put_signal(i, j, ("src", i * blk), ("dst", j * blk), blk, ("sig", 8 * i), 1, SIGNAL_ADD)   # dst -> src, counted
+    w = World(npes, heap_bytes_for(a), DEV)
+    ld = Loaded(w, a)
+    ba, bb = w.batch(ld.translate(a)), w.batch(ld.translate(b))
+    src0 = ld.obj_numpy("src").copy()
+    s = torch.cuda.Stream()
+    with torch.cuda.stream(s):
+        w.enqueue_batch(ba)                                      # warm-up outside the capture (module load, attributes)
+        w.enqueue_batch(bb)
+        torch.cuda.synchronize()
+        g = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(g, stream=s):
+            for _ in range(5):
+                w.enqueue_batch(ba)
+                w.enqueue_batch(bb)
+        for _ in range(3):
+            g.replay()
+        w.quiet(0)
+    torch.cuda.synchronize()
+    exp_dst = src0.reshape(npes, npes, blk).transpose(1, 0, 2).reshape(npes, npes * blk)
+    assert np.array_equal(ld.obj_numpy("dst"), exp_dst)
+    assert np.array_equal(ld.obj_numpy("src"), src0)              # transpose of transpose, 16 times over
+    assert (ld.obj_numpy("sig", np.uint64) == 16).all()           # every put_signal of each of the 16 launches signalled once
+
+
 def test_edge_cases_empty_and_zero_byte():
     w = World(4, 1 << 16, DEV)
     b = w.batch(np.zeros(0, dtype=OP_DTYPE))
@@ -209,7 +244,7 @@ def test_bad_descriptors_are_rejected_on_the_host():
 
 def test_context_field_is_validated_and_quiet_is_per_context():
     """ctx >= SHMEMG_CTX_MAX is rejected; a QUIET on an unused context orders nothing but is legal."""
-    from workloads.spec import Program
+    from workloads.spec import SIGNAL_ADD, Program
     w = World(2, 1 << 16, DEV)
     a = w.malloc(4096)
     ops = np.zeros(3, dtype=OP_DTYPE)
