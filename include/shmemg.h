@@ -24,6 +24,10 @@
  *     is enqueued on error.  Data races, overlapping unordered writes and unsatisfiable waits are
  *     undefined behaviour; an unsatisfiable wait hangs the stream (prohibited pattern,
  *     PAPER L404).
+ *   - Threads: a world handle is NOT thread-safe.  Its host bookkeeping (allocator, team views, launch state) is
+ *     unsynchronised, and the team collectives run the world kernels on a temporarily narrowed view of the world
+ *     object: calls on ONE world from several host threads must be serialised by the caller.  Different worlds are
+ *     independent.
  *   - Execution path: every `_on_stream` routine is a HOST-ISSUED,
  *     STREAM-TRIGGERED operation "whose execution is ordered relative to a GPU stream"; the library
  *     "may use internal GPU kernels to accelerate" it.  Effects are visible to later work on the same
