@@ -303,6 +303,30 @@ class OracleWorld:
         return bool(r)
 
 
+# ---- NEXT-4 (iii): PE -> GPU placement ("direct GPU-GPU fabrics ... load-store fabrics") -----------
+# The paper names the fabrics and fixes no placement; SURVEY 8(e) gives "PE p -> GPU p mod G".  Written out: with G shards,
+# global PE g lives on shard g mod G, as that shard's local PE g div G (reading 42).  A sharded world computes the
+# SAME thing as one world of all the PEs, so the oracle of every sharded operation is the existing routine on the global
+# world; these functions only say which rows of the global heap a shard holds.
+def shard_of(g: int, nshards: int) -> int:
+    return g % nshards
+
+
+def shard_local_index(g: int, nshards: int) -> int:
+    return g // nshards
+
+
+def shard_global_pe(shard: int, local: int, nshards: int) -> int:
+    return local * nshards + shard
+
+
+def shard_rows(ow: "OracleWorld", shard: int, nshards: int, off: int, nbytes: int, dtype=np.uint8) -> np.ndarray:
+    """What shard `shard` holds of the symmetric range [off, off + nbytes): the rows of its PEs, in local-PE order."""
+    rows = [g for g in range(ow.npes) if shard_of(g, nshards) == shard]
+    rows.sort(key=lambda g: shard_local_index(g, nshards))
+    return ow.view(off, nbytes, dtype)[rows]
+
+
 # ---- halo application compute (config C2) ----------------------------------------------------------
 def halo_delta(seed: int, rnd: int, gidx: int) -> float:
     return float(lib().orc_halo_delta(seed, rnd, gidx))
