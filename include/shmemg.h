@@ -85,6 +85,7 @@ enum {
 #define SHMEMG_CAP_STREAM_COLLECTIVES         (1ull << 12)  /* barrier/alltoall/fcollect/reduce on stream */
 #define SHMEMG_CAP_DEVICE_BARRIER             (1ull << 13)  /* shmemg_dev_barrier_all_block (L363)       */
 #define SHMEMG_CAP_CPU_HEAP_PRESENT           (1ull << 14)  /* the CPU space of the two-space model is attached (L313-L317) */
+#define SHMEMG_CAP_PEER_SHARDS                (1ull << 15)  /* this world is one shard of a multi-GPU world (shmemg_shard_init, L194) */
 
 /* ---- lifecycle ------------------------------------------------------------------------------------ */
 
@@ -515,6 +516,54 @@ SHMEMG_API int shmemg_device_collective_on_stream(shmemg_world_t *w, int kind, i
  * npes thread blocks cannot be co-resident on the device (progress would not be guaranteed). */
 SHMEMG_API int shmemg_device_exec_ops_on_stream(shmemg_world_t *w, const shmemg_op_t *ops_host, size_t nops, void *ops_dev,
                                                 void *stream, size_t *bad_index);
+
+/* ---- PE -> GPU sharding over a load-store fabric ----------------------------------------
+ * "Direct GPU-GPU fabrics such as NVLink ... load-store fabrics provide direct hardware-assisted communication among GPUs ...
+ * They can offer high-performance remote atomic operations, but not necessarily in the same atomicity domain".
+ * One process (one world) per GPU, G = nshards of them.  Placement (reading 42): GLOBAL PE g lives on shard
+ * g mod G as that shard's LOCAL PE g div G; every shard holds `npes` local PEs (shmemg_init) with the same heap size, and the
+ * symmetric allocator is called identically on every shard, so one offset names the same object everywhere.
+ * The shards see each other's slabs through peer mappings: shmemg_shard_export gives a CUDA IPC handle of this world's slab
+ * (64 bytes, HOST) plus the slab's byte offset inside the exported allocation; the caller carries both to the other processes
+ * (any transport: the tests use torch.distributed/gloo) and gives them to shmemg_shard_attach_ipc there.  Shards that live in
+ * ONE process (peer access enabled by the caller) pass the slab pointer itself to shmemg_shard_attach_ptr.
+ * The g-calls take GLOBAL PE numbers; the initiator must be a local PE of this shard.  Transfers are peer loads / stores issued
+ * by this shard's kernels; AMOs and signal updates on a remote shard are SYSTEM-scope atomics (the atomicity domain of a
+ * sharded world is the fabric, not one GPU's L2); ordering between shards comes from shmemg_gbarrier_all_on_stream or from
+ * put-with-signal + wait, exactly as between PEs of one GPU.  shmemg_gbarrier_all_on_stream is one kernel per shard that
+ * arrives on every shard's counter and waits for its own: the G kernels must be able to run at the same time (one GPU each);
+ * it is a barrier of the STREAMS, so it also orders everything enqueued before it on each shard's stream.
+ * shmemg_galltoall_on_stream: every local PE pushes its block for global PE j into j's window (peer stores), the caller puts a
+ * gbarrier before it (sources ready) and after it (blocks delivered).
+ * Errors: SHMEMG_ERR_ARG before shmemg_shard_init or for a shard that is not attached, SHMEMG_ERR_PE for a PE outside
+ * [0, nshards * npes) or an initiator that is not local.  With nshards == 1 every g-call equals its unsharded counterpart. */
+#define SHMEMG_MAX_SHARDS 16
+SHMEMG_API int shmemg_shard_of(int gpe, int nshards);            /* g mod G, or SHMEMG_ERR_ARG */
+SHMEMG_API int shmemg_shard_local_index(int gpe, int nshards);   /* g div G */
+SHMEMG_API int shmemg_shard_global_pe(int shard, int local_pe, int nshards);
+SHMEMG_API int shmemg_shard_init(shmemg_world_t *w, int nshards, int my_shard);
+SHMEMG_API int shmemg_shard_export(shmemg_world_t *w, void *ipc_handle64_out, uint64_t *offset_out);
+SHMEMG_API int shmemg_shard_attach_ipc(shmemg_world_t *w, int shard, const void *ipc_handle64, uint64_t offset);
+SHMEMG_API int shmemg_shard_attach_ptr(shmemg_world_t *w, int shard, void *peer_slab_dev);
+SHMEMG_API int shmemg_shard_global_npes(const shmemg_world_t *w);
+SHMEMG_API int shmemg_gput_on_stream(shmemg_world_t *w, uint64_t dest_off, uint64_t source_off, size_t nbytes, int gpe,
+                                     int target_gpe, void *stream);
+SHMEMG_API int shmemg_gget_on_stream(shmemg_world_t *w, uint64_t dest_off, uint64_t source_off, size_t nbytes, int gpe,
+                                     int target_gpe, void *stream);
+SHMEMG_API int shmemg_gput_signal_on_stream(shmemg_world_t *w, uint64_t dest_off, uint64_t source_off, size_t nbytes,
+                                            uint64_t sig_off, uint64_t signal, int sig_op, int gpe, int target_gpe, void *stream);
+SHMEMG_API int shmemg_gsignal_wait_until_on_stream(shmemg_world_t *w, uint64_t sig_off, int cmp, uint64_t value, int gpe,
+                                                   void *stream);
+/* SoA AMO batches with GLOBAL target PEs (DEVICE arrays as in shmemg_atomic_*_batch_on_stream; the initiators are this shard's
+ * PEs, which needs no argument: an AMO names only its target).  op: SHMEMG_OP_ATOMIC_ADD / _FETCH_ADD / _COMPARE_SWAP;
+ * val == NULL: val_scalar for every op; cond likewise; fetched_out (DEVICE, n entries) for the two fetching ops. */
+SHMEMG_API int shmemg_gatomic_batch_on_stream(shmemg_world_t *w, int op, uint64_t sym_off, const int32_t *target_gpe,
+                                              const void *elem_idx, int idx_bytes, const uint64_t *cond, uint64_t cond_scalar,
+                                              const uint64_t *val, uint64_t val_scalar, uint64_t *fetched_out, size_t n,
+                                              void *stream);
+SHMEMG_API int shmemg_galltoall_on_stream(shmemg_world_t *w, uint64_t dest_off, uint64_t source_off, size_t nbytes_per_pe,
+                                          void *stream);
+SHMEMG_API int shmemg_gbarrier_all_on_stream(shmemg_world_t *w, void *stream);
 
 #ifdef __cplusplus
 }

@@ -6,7 +6,7 @@ import subprocess
 
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
-SOURCES = ["world.cu", "batch.cu", "plan_dev.cu", "amo.cu", "collectives.cu", "surface2.cu", "halo_app.cu", "probe.cu", "device_path.cu"]
+SOURCES = ["world.cu", "batch.cu", "plan_dev.cu", "amo.cu", "collectives.cu", "surface2.cu", "halo_app.cu", "probe.cu", "device_path.cu", "shard.cu"]
 LIB = os.path.join(HERE, "libshmemg.so")
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC,-fvisibility=hidden", "--shared"]

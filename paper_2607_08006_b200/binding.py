@@ -61,6 +61,7 @@ class CAP:
     STREAM_COLLECTIVES = 1 << 12
     DEVICE_BARRIER = 1 << 13
     CPU_HEAP_PRESENT = 1 << 14
+    PEER_SHARDS = 1 << 15
 
 
 F32, I64, I32, F64 = 0, 1, 2, 3
@@ -119,6 +120,21 @@ SYMBOLS = {
     "shmemg_enqueue_batch": (_i, [_vp, _vp, _sz, _vp]),
     "shmemg_enqueue_batch_ws": (_i, [_vp, _vp, _sz, _vp, _sz, _vp]),
     "shmemg_batch_status": (_i, [_vp, _vp, _vp, C.POINTER(_i), C.POINTER(_sz)]),
+    "shmemg_shard_of": (_i, [_i, _i]),
+    "shmemg_shard_local_index": (_i, [_i, _i]),
+    "shmemg_shard_global_pe": (_i, [_i, _i, _i]),
+    "shmemg_shard_init": (_i, [_vp, _i, _i]),
+    "shmemg_shard_export": (_i, [_vp, _vp, C.POINTER(_u64)]),
+    "shmemg_shard_attach_ipc": (_i, [_vp, _i, _vp, _u64]),
+    "shmemg_shard_attach_ptr": (_i, [_vp, _i, _vp]),
+    "shmemg_shard_global_npes": (_i, [_vp]),
+    "shmemg_gput_on_stream": (_i, [_vp, _u64, _u64, _sz, _i, _i, _vp]),
+    "shmemg_gget_on_stream": (_i, [_vp, _u64, _u64, _sz, _i, _i, _vp]),
+    "shmemg_gput_signal_on_stream": (_i, [_vp, _u64, _u64, _sz, _u64, _u64, _i, _i, _i, _vp]),
+    "shmemg_gsignal_wait_until_on_stream": (_i, [_vp, _u64, _i, _u64, _i, _vp]),
+    "shmemg_gatomic_batch_on_stream": (_i, [_vp, _i, _u64, _vp, _vp, _i, _vp, _u64, _vp, _u64, _vp, _sz, _vp]),
+    "shmemg_galltoall_on_stream": (_i, [_vp, _u64, _u64, _sz, _vp]),
+    "shmemg_gbarrier_all_on_stream": (_i, [_vp, _vp]),
     "shmemg_put_on_stream": (_i, [_vp, _u64, _u64, _sz, _i, _i, _vp]),
     "shmemg_get_on_stream": (_i, [_vp, _u64, _u64, _sz, _i, _i, _vp]),
     "shmemg_put_signal_on_stream": (_i, [_vp, _u64, _u64, _sz, _u64, _u64, _i, _i, _i, _vp]),
@@ -630,6 +646,62 @@ class World:
         self._chk(lib().shmemg_get_space_on_stream(self.h, dst_space, dest_off, src_space, source_off, nbytes, pe, target_pe,
                                                    _stream(stream)), "shmemg_get_space_on_stream")
         self.launches += 1 if nbytes and dst_space == 0 and src_space == 0 else 0
+
+    # ---- PE -> GPU sharding (NEXT-4 (iii)): this world is one shard of a multi-GPU world; g-calls take GLOBAL PE numbers ----
+    def shard_init(self, nshards: int, my_shard: int):
+        self._chk(lib().shmemg_shard_init(self.h, nshards, my_shard), "shmemg_shard_init")
+        self.nshards, self.shard = nshards, my_shard
+
+    def shard_export(self):
+        """(64-byte CUDA IPC handle of this world's slab allocation, offset of the slab inside it): carry both to the peers."""
+        buf, off = C.create_string_buffer(64), C.c_uint64(0)
+        self._chk(lib().shmemg_shard_export(self.h, buf, C.byref(off)), "shmemg_shard_export")
+        return bytes(buf.raw), off.value
+
+    def shard_attach_ipc(self, shard: int, handle: bytes, offset: int):
+        assert len(handle) == 64
+        self._chk(lib().shmemg_shard_attach_ipc(self.h, shard, C.create_string_buffer(handle, 64), offset), "shmemg_shard_attach_ipc")
+
+    def shard_attach_world(self, shard: int, other: "World"):
+        """A shard that lives in THIS process (its slab is addressable here: same device, or peer access enabled)."""
+        self._chk(lib().shmemg_shard_attach_ptr(self.h, shard, other.slab.data_ptr()), "shmemg_shard_attach_ptr")
+
+    def shard_global_npes(self) -> int:
+        return lib().shmemg_shard_global_npes(self.h)
+
+    def gput(self, dest_off, source_off, nbytes, gpe, target_gpe, stream=None):
+        self._chk(lib().shmemg_gput_on_stream(self.h, dest_off, source_off, nbytes, gpe, target_gpe, _stream(stream)), "shmemg_gput_on_stream")
+        self.launches += 1 if nbytes else 0
+
+    def gget(self, dest_off, source_off, nbytes, gpe, target_gpe, stream=None):
+        self._chk(lib().shmemg_gget_on_stream(self.h, dest_off, source_off, nbytes, gpe, target_gpe, _stream(stream)), "shmemg_gget_on_stream")
+        self.launches += 1 if nbytes else 0
+
+    def gput_signal(self, dest_off, source_off, nbytes, sig_off, signal, sig_op, gpe, target_gpe, stream=None):
+        self._chk(lib().shmemg_gput_signal_on_stream(self.h, dest_off, source_off, nbytes, sig_off, signal & NO_STAMP, sig_op, gpe,
+                                                     target_gpe, _stream(stream)), "shmemg_gput_signal_on_stream")
+        self.launches += 1
+
+    def gsignal_wait_until(self, sig_off, cmp, value, gpe, stream=None):
+        self._chk(lib().shmemg_gsignal_wait_until_on_stream(self.h, sig_off, cmp, value & NO_STAMP, gpe, _stream(stream)),
+                  "shmemg_gsignal_wait_until_on_stream")
+        self.launches += 1
+
+    def gatomic_batch(self, op, sym_off, target_gpe, elem_idx, val=None, val_scalar=0, cond=None, cond_scalar=0, fetched_out=None,
+                      stream=None):
+        n = target_gpe.numel()
+        self._chk(lib().shmemg_gatomic_batch_on_stream(self.h, op, sym_off, _dptr(target_gpe), _dptr(elem_idx), self._idx_bytes(elem_idx),
+                                                       _dptr(cond), cond_scalar & NO_STAMP, _dptr(val), val_scalar & NO_STAMP,
+                                                       _dptr(fetched_out), n, _stream(stream)), "shmemg_gatomic_batch_on_stream")
+        self.launches += 1 if n else 0
+
+    def galltoall(self, dest_off, source_off, nbytes, stream=None):
+        self._chk(lib().shmemg_galltoall_on_stream(self.h, dest_off, source_off, nbytes, _stream(stream)), "shmemg_galltoall_on_stream")
+        self.launches += 1 if nbytes else 0
+
+    def gbarrier_all(self, stream=None):
+        self._chk(lib().shmemg_gbarrier_all_on_stream(self.h, _stream(stream)), "shmemg_gbarrier_all_on_stream")
+        self.launches += 1
 
     def alltoall(self, dest_off, source_off, nbytes, stream=None):
         self._chk(lib().shmemg_alltoall_on_stream(self.h, dest_off, source_off, nbytes, _stream(stream)),

@@ -30,6 +30,8 @@ struct CtlRegion {
     unsigned int sig_counter[SHMEMG_SIG_SLOTS];   // last-arriver counters of single put_signal launches
     unsigned int group_bar[128];           // per-PE arrival counters of multi-block PE agents (monotonic; halo_app.cu)
     unsigned int amo_done;                 // SHMEMG_AMO_THEN_BARRIER: CTAs of the AMO kernel that have finished
+    unsigned int pad_sh;
+    unsigned long long shard_bar;          // sharded world: arrivals of every shard's gbarrier (monotonic; system-scope atomics)
     unsigned int hot_n;                    // SHMEMG_AMO_HOT_AGGREGATE: number of hot words found by the sampling kernel
     unsigned int hot_done;                 // CTAs of the sampling kernel that have staged their keys
     unsigned int hot_keys[SHMEMG_HOT_MAX]; // their slab word indices
@@ -63,6 +65,11 @@ struct shmemg_world {
     struct Team { int start, stride, size; };
     int teams_world_npes = 0;              // npes of the world while a team view is active (surface2.cu)
     std::vector<Team> teams;               // user teams (shmemg_team_split_strided); handle = SHMEMG_TEAM_USER0 + index
+    // PE -> GPU sharding (shard.cu): this world is shard `shard` of `nshards`; peer_base[s] = slab of shard s as mapped HERE
+    int nshards = 0, shard = 0;
+    uint8_t *peer_base[SHMEMG_MAX_SHARDS] = {};
+    void *peer_ipc[SHMEMG_MAX_SHARDS] = {};   // what cudaIpcOpenMemHandle returned (closed in shmemg_finalize)
+    unsigned long long shard_epoch = 0;    // gbarriers enqueued so far
     void *scratch = nullptr;               // DEVICE: caller-owned scratch (shmemg_set_scratch), used by SHMEMG_AMO_HOT_AGGREGATE
     size_t scratch_bytes = 0;
     std::string last_cuda_error;
@@ -86,6 +93,8 @@ static inline bool shmemg_pe_ok(const shmemg_world *w, int pe) { return pe >= 0 
 static inline uint8_t *shmemg_addr(const shmemg_world *w, int pe, uint64_t off) {
     return w->base + (size_t)pe * w->stride + off;
 }
+
+void shmemg_shard_release(shmemg_world *w);       // shard.cu: closes the peer mappings (shmemg_finalize)
 
 // host-side validation of one op descriptor (batch.cu); shared with the device-initiated interpreter (device_path.cu)
 int shmemg_validate_op(const shmemg_world *w, const shmemg_op_t &o);

@@ -88,6 +88,7 @@ extern "C" int shmemg_init(int npes, size_t heap_bytes_per_pe, void *device_slab
 
 extern "C" int shmemg_finalize(shmemg_world_t *w) {
     if (!w) return SHMEMG_ERR_ARG;
+    shmemg_shard_release(w);
     delete w;
     return SHMEMG_OK;
 }
@@ -107,6 +108,7 @@ extern "C" int shmem_query_capabilities(const shmemg_world_t *w, int team, uint6
     uint64_t c = SHMEMG_CAP_GPU_HEAP_PRESENT | SHMEMG_CAP_DEFAULT_HEAP_IS_GPU | SHMEMG_CAP_PTR_DEVICE_ACCESSIBLE |
                  SHMEMG_CAP_PROGRESS_GPU_ONLY | SHMEMG_CAP_PATH_DIRECT | SHMEMG_CAP_ATOMICS_64;
     if (w->cpu_base) c |= SHMEMG_CAP_CPU_HEAP_PRESENT;      // the CPU half of the two-space model is attached (L313-L317)
+    if (w->nshards > 1) c |= SHMEMG_CAP_PEER_SHARDS;        // one shard of a multi-GPU world over a load-store fabric (L194)
     if (team == SHMEM_TEAM_WORLD)
         c |= SHMEMG_CAP_HOST_INITIATED_GPU_BUFFERS | SHMEMG_CAP_STREAM_TRIGGERED | SHMEMG_CAP_STREAM_COLLECTIVES;
     else
