@@ -158,6 +158,11 @@ class Inputs:
         if "next4" in groups:
             # NEXT-4 (i): slab transpose of a 1024 x 1024 x 256 complex64 array (2 GiB) over 64 PEs
             self.fft = configs.fft_transpose(16, 128, 128, 64) if small else configs.fft_transpose()
+            # NEXT-4 (iii): the C3a alltoall on a world sharded over TWO worlds (both on this one GPU, attached by pointer)
+            self.sh_npes, self.sh_blk = (16, 65536) if small else (64, 65536)
+            self.sh_payload = getattr(self, "c3a", None)
+            if self.sh_payload is None or self.sh_payload.shape[0] != self.sh_npes:
+                self.sh_payload = configs.c3a_payload(self.sh_npes, self.sh_blk)
         if "c5" in groups or "barrier" in groups:
             self.c5_npes, self.c5_bytes = (32, 1 << 20) if small else (128, 4 << 20)
             self.c5_fc_bytes = 32768
@@ -237,6 +242,8 @@ def segment_table(inp: Inputs):
             seg["next2_ibput_faces"] = dict(cls="xcopy", kernel="k_ib_tma/k_ib_elem", bytes=3 * 2 * inp.halo.face_bytes, launches=3)
     if "next4" in g:
         seg["next4_fft_transpose_alltoalls"] = dict(cls="xcopy", kernel="k_alltoalls_tma", bytes=2 * inp.fft.A.size, launches=1)
+        seg["next4_sharded_alltoall_2_shards_on_one_gpu"] = dict(cls="xcopy", kernel="k_shard_alltoall (one launch per shard)",
+                                                                 bytes=2 * inp.sh_npes ** 2 * inp.sh_blk, launches=2)
     if "barrier" in g:
         seg["barrier_in_kernel"] = dict(cls="sync", kernel="k_barrier_repeat", ops=BARRIERS, launches=1)
         seg["barrier_on_stream"] = dict(cls="sync", kernel="k_barrier_epoch", ops=BARRIERS, launches=BARRIERS)
@@ -352,6 +359,19 @@ class CudaBench:
             w.view(self.f_src, t.slab_bytes).copy_(torch.from_numpy(t.A))
             w.view(self.f_dst, t.slab_bytes).zero_()
             self.worlds.append(w)
+            n, b = inp.sh_npes, inp.sh_blk
+            self.wsh = [World(n // 2, 2 * n * b + 4096, device) for _ in range(2)]
+            for sh, ws in enumerate(self.wsh):
+                ws.shard_init(2, sh)
+            self.wsh[0].shard_attach_world(1, self.wsh[1])
+            self.wsh[1].shard_attach_world(0, self.wsh[0])
+            offs = [(ws.malloc(n * b), ws.malloc(n * b)) for ws in self.wsh]
+            assert offs[0] == offs[1]                                  # the same allocations on every shard: one offset names one object
+            self.sh_src, self.sh_dst = offs[0]
+            for sh, ws in enumerate(self.wsh):
+                ws.view(self.sh_src, n * b).copy_(torch.from_numpy(np.ascontiguousarray(inp.sh_payload[sh::2])))
+                ws.view(self.sh_dst, n * b).zero_()
+                self.worlds.append(ws)
         if "c5" in g or "barrier" in g:
             n, nb = inp.c5_npes, inp.c5_bytes
             w = World(n, 3 * nb + inp.c5_fc_bytes + 65536, device)
@@ -504,6 +524,9 @@ class CudaBench:
             block, nblocks, sbs, sps, dbs, dps = inp.fft.params()
             with rec.seg("next4_fft_transpose_alltoalls"):
                 self.wf.alltoalls(self.f_dst, self.f_src, dps, sps, dbs, sbs, block, nblocks)
+            with rec.seg("next4_sharded_alltoall_2_shards_on_one_gpu"):
+                for ws in self.wsh:
+                    ws.galltoall(self.sh_dst, self.sh_src, inp.sh_blk)
         if "barrier" in g:
             with rec.seg("barrier_in_kernel"):
                 self.w5.barrier_all_repeat(BARRIERS)
@@ -739,6 +762,18 @@ class CudaBench:
             ow.alltoalls(od, os_, dps, sps, dbs, sbs, block, nblocks)
             assert np.array_equal(host(self.wf.view(self.f_dst, t.slab_bytes)), ow.view(od, t.slab_bytes)), "fft transpose"
             ok["next4_fft_transpose_alltoalls"] = True
+            n, b = inp.sh_npes, inp.sh_blk
+            for ws in self.wsh:
+                ws.view(self.sh_dst, n * b).zero_()
+            for ws in self.wsh:
+                ws.galltoall(self.sh_dst, self.sh_src, b)
+            ow = ob.orc.OracleWorld(n, 2 * n * b + 512)                  # the GLOBAL world of all the PEs
+            os_, od = ow.malloc(n * b), ow.malloc(n * b)
+            ow.view(os_, n * b)[:] = inp.sh_payload
+            ow.alltoall(od, os_, b)
+            for sh, ws in enumerate(self.wsh):
+                assert np.array_equal(host(ws.view(self.sh_dst, n * b)), ob.orc.shard_rows(ow, sh, 2, od, n * b)), "sharded alltoall"
+            ok["next4_sharded_alltoall_2_shards_on_one_gpu"] = True
         if "c2" in g:
             h, w, fb = inp.halo, self.w2, inp.halo.face_bytes
             send_off = self.ld2.off["send"][0]
