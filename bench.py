@@ -535,7 +535,7 @@ class CudaBench:
                     self.w5.barrier_all()
             if self.barrier_graph is None:                               # the same 10 000 launches captured once (reading 24)
                 self.barrier_graph = torch.cuda.CUDAGraph()
-                with torch.cuda.graph(self.barrier_graph):
+                with torch.cuda.graph(self.barrier_graph, capture_error_mode="thread_local"):   # other threads (an NCCL watchdog under torchrun) may call CUDA
                     for _ in range(BARRIERS):
                         self.w5.barrier_all()
             with rec.seg("barrier_on_stream_graph"):
@@ -551,7 +551,7 @@ class CudaBench:
         graphs = []
         for app, lib in ((False, True), (True, True), (True, False)):
             gr = torch.cuda.CUDAGraph()
-            with torch.cuda.graph(gr):
+            with torch.cuda.graph(gr, capture_error_mode="thread_local"):
                 if app:
                     self.ld2.obj("sig").zero_()
                 for r in range(1, HALO_ROUNDS + 1):
