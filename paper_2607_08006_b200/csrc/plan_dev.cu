@@ -107,45 +107,62 @@ __device__ __forceinline__ void d_endpoints(const PlanArgs &a, const shmemg_op_t
     src = put ? loc : rem;
 }
 
-// The cut of one copy op into pieces: the same rule as cut_copy (batch.cu).  emit(piece index, kind, offset, bytes).
-template <typename F>
-__device__ __forceinline__ unsigned d_cut_copy(unsigned long long dst, unsigned long long src, unsigned long long n, unsigned seg_tiles,
-                                               F emit) {
-    unsigned np = 0;
-    if (n == 0) { emit(np++, (unsigned)T_NODATA, 0ull, 0u); return np; }
+// The cut of one copy op into pieces: the same rule as cut_copy (batch.cu), computed ONCE per op (the piece count feeds the
+// scan, the pieces are emitted behind it).  Divisions run in 32 bits when the op is shorter than 4 GiB (a 64-bit division is
+// about a hundred instructions, and the planner of a small batch is bound by instruction issue).
+struct Cut {
+    unsigned long long head, body, share;   // bulk mode: unaligned head, 16-byte body cut into `share`-byte pieces, tail
+    unsigned tail, np, bulk;                // np = number of pieces; bulk = 0: register-path tiles of GEN_TILE bytes throughout
+};
+__device__ __forceinline__ Cut d_cut(unsigned long long dst, unsigned long long src, unsigned long long n, unsigned seg_tiles) {
+    Cut c = {0, 0, 0, 0, 1, 0};
+    if (n == 0) return c;                                            // one T_NODATA piece
     const bool congruent = ((dst ^ src) & 15) == 0;
     const bool aligned = congruent && (dst & 15) == 0 && (n & 15) == 0;
     if (aligned || (congruent && n >= TMA_MIN_SPLIT)) {
         unsigned long long head = (16 - (dst & 15)) & 15;
         if (head > n) head = n;
-        const unsigned long long body = (n - head) & ~15ull, tail = n - head - body;
-        if (head) emit(np++, (unsigned)T_COPY, 0ull, (unsigned)head);
+        const unsigned long long body = (n - head) & ~15ull;
+        c.head = head; c.body = body; c.tail = (unsigned)(n - head - body); c.bulk = 1;
         const unsigned long long tiles = (body + SHMEMG_TMA_TILE - 1) / SHMEMG_TMA_TILE;
-        const unsigned long long nseg = (tiles + seg_tiles - 1) / seg_tiles;
-        const unsigned long long share = ((body + nseg - 1) / nseg + 1023ull) & ~1023ull;     // equal shares, cut at 1 KiB
-        for (unsigned long long b0 = 0; b0 < body; b0 += share) emit(np++, (unsigned)T_TMA, head + b0, (unsigned)(body - b0 < share ? body - b0 : share));
-        if (tail) emit(np++, (unsigned)T_COPY, head + body, (unsigned)tail);
-        return np;
+        unsigned nbody;
+        if (body == 0) {
+            nbody = 0;
+        } else if ((body >> 32) == 0) {
+            const unsigned t32 = (unsigned)tiles, b32 = (unsigned)body;
+            const unsigned nseg = (t32 + seg_tiles - 1) / seg_tiles;                 // >= 1
+            const unsigned q = b32 / nseg;
+            const unsigned long long ceilq = (unsigned long long)q + (q * nseg != b32 ? 1u : 0u);
+            c.share = (ceilq + 1023ull) & ~1023ull;                                  // equal shares, cut at 1 KiB
+            if (c.share >> 32) nbody = 1u;
+            else { const unsigned s32 = (unsigned)c.share, q2 = b32 / s32; nbody = q2 + (q2 * s32 != b32 ? 1u : 0u); }
+        } else {
+            const unsigned long long nseg = (tiles + seg_tiles - 1) / seg_tiles;
+            c.share = ((body + nseg - 1) / nseg + 1023ull) & ~1023ull;
+            nbody = (unsigned)((body + c.share - 1) / c.share);
+        }
+        c.np = (head ? 1u : 0u) + nbody + (c.tail ? 1u : 0u);
+        return c;
     }
-    for (unsigned long long o = 0; o < n; o += GEN_TILE) emit(np++, (unsigned)T_COPY, o, (unsigned)(n - o < GEN_TILE ? n - o : GEN_TILE));
-    return np;
+    c.np = (unsigned)((n + GEN_TILE - 1) / GEN_TILE);
+    return c;
 }
-
-// number of pieces d_cut_copy emits, in closed form
-__device__ __forceinline__ unsigned d_count_pieces(unsigned long long dst, unsigned long long src, unsigned long long n, unsigned seg_tiles) {
-    if (n == 0) return 1u;
-    const bool congruent = ((dst ^ src) & 15) == 0;
-    const bool aligned = congruent && (dst & 15) == 0 && (n & 15) == 0;
-    if (aligned || (congruent && n >= TMA_MIN_SPLIT)) {
-        unsigned long long head = (16 - (dst & 15)) & 15;
-        if (head > n) head = n;
-        const unsigned long long body = (n - head) & ~15ull, tail = n - head - body;
-        const unsigned long long tiles = (body + SHMEMG_TMA_TILE - 1) / SHMEMG_TMA_TILE;
-        const unsigned long long nseg = (tiles + seg_tiles - 1) / seg_tiles;
-        const unsigned long long share = ((body + nseg - 1) / nseg + 1023ull) & ~1023ull;
-        return (head ? 1u : 0u) + (unsigned)((body + share - 1) / share) + (tail ? 1u : 0u);
+// emit(piece index, kind, offset, bytes) for every piece of the cut: ONE call site in a rolled loop (the record-writing code is
+// the bulk of the planner's instructions, and the planner pays for every instruction line it fetches)
+template <typename F>
+__device__ __forceinline__ void d_emit_cut(const Cut &c, unsigned long long n, F emit) {
+    const unsigned hp = c.head ? 1u : 0u, last = c.np - 1u;
+#pragma unroll 1
+    for (unsigned p = 0; p < c.np; ++p) {
+        unsigned kind, len;
+        unsigned long long off;
+        if (n == 0) { kind = T_NODATA; off = 0; len = 0; }
+        else if (!c.bulk) { kind = T_COPY; off = (unsigned long long)p * GEN_TILE; len = (unsigned)(n - off < GEN_TILE ? n - off : GEN_TILE); }
+        else if (p < hp) { kind = T_COPY; off = 0; len = (unsigned)c.head; }
+        else if (c.tail && p == last) { kind = T_COPY; off = c.head + c.body; len = c.tail; }
+        else { const unsigned long long b0 = (unsigned long long)(p - hp) * c.share; kind = T_TMA; off = c.head + b0; len = (unsigned)(c.body - b0 < c.share ? c.body - b0 : c.share); }
+        emit(p, kind, off, len);
     }
-    return (unsigned)((n + GEN_TILE - 1) / GEN_TILE);
 }
 
 template <typename T> __device__ __forceinline__ void d_st_rec(T *p, const T &r) {       // 64-byte record, four 16-byte stores
@@ -230,9 +247,13 @@ struct PlanShared {
     unsigned all_total;                          // (rank 0) real ops before the last BARRIER_ALL a real op follows
     unsigned dep[PLAN_CHUNK];                    // per-domain thresholds of this CTA's ops of the super-chunk (written by rank 0)
     unsigned char cls[PLAN_CHUNK + 1];           // class of each op of the chunk (1 AMO, 2 wait) | 0x80 = starts a stretch
+    unsigned short send[PLAN_CHUNK];             // send[first thread of a stretch] = its last thread (written by that one)
 };
 
 // One planner CTA per PLAN_CHUNK ops of a super-chunk (C * PLAN_CHUNK ops); C = cluster size (1 for small batches).
+// CL: launched as a thread-block cluster (large batches).  The single-CTA instantiation carries none of the cluster code: the
+// planner of a small batch is bound by instruction fetch (cold code in every launch), so its code path is kept short.
+template <bool CL>
 __global__ void __launch_bounds__(PLAN_THREADS, 1) k_plan_batch(const PlanArgs a) {
     extern __shared__ unsigned dsm[];                 // 6 tables of ndom entries, then (rank 0) C * PLAN_CHUNK compact keys
     __shared__ PlanShared sh;
@@ -241,7 +262,7 @@ __global__ void __launch_bounds__(PLAN_THREADS, 1) k_plan_batch(const PlanArgs a
     unsigned *fL = dsm + 3 * nd, *fLnw = dsm + 4 * nd, *fM = dsm + 5 * nd;   // reduced over the cluster
     unsigned *issued = pL, *thresh = pLnw, *wrun = fL;               // (rank 0, keyed pass) reuse tables that are dead by then
     unsigned *ckey = dsm + 6 * nd;
-    const unsigned tid = threadIdx.x, C = cl_size(), rank = cl_rank();
+    const unsigned tid = threadIdx.x, C = CL ? cl_size() : 1u, rank = CL ? cl_rank() : 0u;
     const unsigned NT = blockDim.x;                   // = ops per CTA and super-chunk: 1024, or fewer for a batch of fewer ops
     const unsigned long long n = a.nops, SC = (unsigned long long)C * NT;
     const bool single = n <= SC;                      // one super-chunk: every op stays in its thread's registers
@@ -257,20 +278,35 @@ __global__ void __launch_bounds__(PLAN_THREADS, 1) k_plan_batch(const PlanArgs a
     {
         unsigned long long bulk = 0;
         unsigned pt = 0;
-        for (unsigned long long c0 = (unsigned long long)rank * NT; c0 < n; c0 += SC) {
+        // same-address shared-memory atomics serialise (4096 ops of 64 PEs: 7 us of this sweep), so every warp combines first:
+        // ops of one domain are grouped with match.any and the group's HIGHEST lane (the largest op index) updates the table
+        unsigned lall_t = 0;
+        const unsigned lane = tid & 31;
+        for (unsigned long long c0 = (unsigned long long)rank * NT; c0 < n; c0 += SC) {      // uniform trip count per CTA
             const unsigned long long i = c0 + tid;
-            if (i >= n) continue;
-            const shmemg_op_t o = d_ld_op(a.ops + i);
+            const bool have = i < n;
+            shmemg_op_t o = {};
+            if (have) o = d_ld_op(a.ops + i);
             if (single) keep = o;
-            const int rc = d_validate(a, o);
-            if (rc) { atomicMin(&sh.p_bad, (i << 8) | (unsigned long long)(-rc)); continue; }
-            if (d_marker(o.opcode)) continue;
-            const unsigned dom = (unsigned)o.initiator_pe + (unsigned)o.ctx * (unsigned)a.npes;
-            atomicMax(&pL[dom], (unsigned)i + 1u);
-            if (o.opcode != SHMEMG_OP_SIGNAL_WAIT_UNTIL) atomicMax(&pLnw[dom], (unsigned)i + 1u);
-            atomicMax(&sh.p_lall, (unsigned)i + 1u);
-            if (d_copy(o.opcode)) { bulk += o.nbytes; pt += (unsigned)((o.nbytes + SHMEMG_TMA_TILE - 1) / SHMEMG_TMA_TILE); }
+            const int rc = have ? d_validate(a, o) : 0;
+            if (rc) atomicMin(&sh.p_bad, (i << 8) | (unsigned long long)(-rc));
+            const bool real = have && !rc && !d_marker(o.opcode);
+            const unsigned dom = real ? (unsigned)o.initiator_pe + (unsigned)o.ctx * (unsigned)a.npes : 0u;
+            unsigned grp = 1u << lane, nw = (real && o.opcode != SHMEMG_OP_SIGNAL_WAIT_UNTIL) ? grp : 0u;
+            if (CL) {                                   // (a small batch on a few warps: plain atomics are cheaper than the match)
+                grp = __match_any_sync(FULLM, real ? dom : 0x80000000u | lane);
+                nw = __ballot_sync(FULLM, real && o.opcode != SHMEMG_OP_SIGNAL_WAIT_UNTIL);
+            }
+            if (real) {
+                if (lane == 31u - (unsigned)__clz((int)grp)) atomicMax(&pL[dom], (unsigned)i + 1u);
+                const unsigned g2 = grp & nw;
+                if (g2 && lane == 31u - (unsigned)__clz((int)g2)) atomicMax(&pLnw[dom], (unsigned)i + 1u);
+                lall_t = (unsigned)i + 1u;
+                if (d_copy(o.opcode)) { bulk += o.nbytes; pt += (unsigned)((o.nbytes + SHMEMG_TMA_TILE - 1) / SHMEMG_TMA_TILE); }
+            }
         }
+        lall_t = __reduce_max_sync(FULLM, lall_t);
+        if (lane == 0 && lall_t) atomicMax(&sh.p_lall, lall_t);
         for (int o = 16; o; o >>= 1) { bulk += __shfl_xor_sync(FULLM, bulk, o); pt += __shfl_xor_sync(FULLM, pt, o); }
         if ((tid & 31) == 0 && bulk) { atomicAdd(&sh.p_bulk, bulk); atomicAdd(&sh.p_ptiles, pt); }
     }
@@ -282,17 +318,25 @@ __global__ void __launch_bounds__(PLAN_THREADS, 1) k_plan_batch(const PlanArgs a
         if (m1) atomicMax(&fL[d], m1);
         if (m2) atomicMax(&fLnw[d], m2);
     }
-    if (tid == 0) {
-        unsigned long long bad = sh.p_bad, bulk = sh.p_bulk;
-        unsigned lall = sh.p_lall, pt = sh.p_ptiles;
-        for (unsigned r = 0; r < C; ++r) if (r != rank) {
-            const unsigned long long b2 = cl_ld64(cl_map(&sh.p_bad, r));
-            bad = b2 < bad ? b2 : bad;
-            bulk += cl_ld64(cl_map(&sh.p_bulk, r));
-            lall = max(lall, cl_ld(cl_map(&sh.p_lall, r)));
-            pt += cl_ld(cl_map(&sh.p_ptiles, r));
+    if (tid < 32) {                                    // lane r reads CTA r's partials (one DSMEM round trip), the warp combines
+        unsigned long long bad = ~0ull, bulk = 0;
+        unsigned lall = 0, pt = 0;
+        if (tid < C) {
+            if (C > 1) {
+                bad = cl_ld64(cl_map(&sh.p_bad, tid)); bulk = cl_ld64(cl_map(&sh.p_bulk, tid));
+                lall = cl_ld(cl_map(&sh.p_lall, tid)); pt = cl_ld(cl_map(&sh.p_ptiles, tid));
+            } else {
+                bad = sh.p_bad; bulk = sh.p_bulk; lall = sh.p_lall; pt = sh.p_ptiles;
+            }
         }
-        sh.f_bad = bad; sh.f_bulk = bulk; sh.f_lall = lall; sh.f_ptiles = pt;
+        for (int o = 16; o; o >>= 1) {
+            const unsigned long long b2 = __shfl_xor_sync(FULLM, bad, o);
+            bad = b2 < bad ? b2 : bad;
+            bulk += __shfl_xor_sync(FULLM, bulk, o);
+            lall = max(lall, __shfl_xor_sync(FULLM, lall, o));
+            pt += __shfl_xor_sync(FULLM, pt, o);
+        }
+        if (tid == 0) { sh.f_bad = bad; sh.f_bulk = bulk; sh.f_lall = lall; sh.f_ptiles = pt; }
     }
     __syncthreads();
     if (sh.f_bad != ~0ull) {                           // a bad descriptor: nothing is executed (shmemg_batch_status reports it)
@@ -322,10 +366,15 @@ __global__ void __launch_bounds__(PLAN_THREADS, 1) k_plan_batch(const PlanArgs a
         const unsigned m = C > 1 ? cl_ld(cl_map(&pM[d], r)) : pM[d];
         if (m) atomicMax(&fM[d], m);
     }
-    if (tid == 0) {
-        unsigned mb = sh.p_mb, k = sh.p_keyed;
-        for (unsigned r = 0; r < C; ++r) if (r != rank) { mb = max(mb, cl_ld(cl_map(&sh.p_mb, r))); k |= cl_ld(cl_map(&sh.p_keyed, r)); }
-        sh.f_mb = mb; sh.f_keyed = k;
+    if (tid < 32) {
+        unsigned mb = 0, k = 0;
+        if (tid < C) {
+            if (C > 1) { mb = cl_ld(cl_map(&sh.p_mb, tid)); k = cl_ld(cl_map(&sh.p_keyed, tid)); }
+            else { mb = sh.p_mb; k = sh.p_keyed; }
+        }
+        mb = __reduce_max_sync(FULLM, mb);
+        k = __reduce_or_sync(FULLM, k);
+        if (tid == 0) { sh.f_mb = mb; sh.f_keyed = k; }
     }
     cl_sync_all(C);                                    // the partial tables are dead from here on
     PTRACE(2);
@@ -356,12 +405,12 @@ __global__ void __launch_bounds__(PLAN_THREADS, 1) k_plan_batch(const PlanArgs a
         if (copy) v.a = (unsigned)((o.nbytes + SHMEMG_TMA_TILE - 1) / SHMEMG_TMA_TILE);
         v.b = real ? 1u : 0u;
         v.c = cl ? 1u : 0u;
+        sh.cls[tid] = (unsigned char)cl;
+        __syncthreads();
         if (cl) {                                       // a run of AMOs / waits never crosses a chunk boundary
-            unsigned pcl = 0;
-            if (tid > 0) { unsigned po, pc; int pi; d_ld_head(a.ops + i - 1, po, pc, pi); pcl = d_class(po); }
-            if (pcl != cl) v.m = (unsigned)i + 1u;
+            const unsigned pcl = tid > 0 ? (sh.cls[tid - 1] & 0x7fu) : 0u;      // the neighbour's class (its flag bit may or may not be set yet)
+            if (pcl != cl) { v.m = (unsigned)i + 1u; sh.cls[tid] = (unsigned char)(cl | 0x80u); }
         }
-        sh.cls[tid] = (unsigned char)(cl | (v.m ? 0x80u : 0u));
         S4 tot;
         S4 inc = block_scan(v, sh.ws, tot);
         if (C > 1 && tid < C) {                         // my total to every CTA of the cluster
@@ -380,15 +429,19 @@ __global__ void __launch_bounds__(PLAN_THREADS, 1) k_plan_batch(const PlanArgs a
         if (s0 == 0) PTRACE(3);
         const unsigned unit = inc.b - v.b, auxi = inc.c - v.c, sstart = inc.m ? inc.m - 1u : 0u;
         if (have && (unsigned)i + 1u == MBp) { if (C > 1) cl_st(cl_map(&sh.all_total, 0), unit); else sh.all_total = unit; }
+        // the last op of a stretch of AMOs / waits tells the stretch's first thread where it ends (read behind the next scan)
+        if (cl && (tid + 1 == NT || sh.cls[tid + 1] != (unsigned char)cl)) sh.send[sstart - ((unsigned)i - tid)] = (unsigned short)tid;
         // ---- B: tile records per op -> first tile index; unit count at the latest BARRIER_ALL -> barrier threshold ----
         unsigned seg = 0, ntile = 0;
         unsigned long long dst = 0, src = 0;
+        Cut cut = {0, 0, 0, 0, 0, 0};
         S4 v2 = {0, 0, 0, 0};
         if (copy) {
             seg = base_seg;
             if (base_seg == SEG_TILES_MAX && total_ptiles - inc.a < tail_tiles) seg = 2u;
             d_endpoints(a, o, dst, src);
-            ntile = d_count_pieces(dst, src, o.nbytes, seg);
+            cut = d_cut(dst, src, o.nbytes, seg);
+            ntile = cut.np;
         } else if (cl) {
             ntile = ((unsigned)i - sstart) % AMO_RUN_MAX == 0 ? 1u : 0u;
         } else if (have && opc == SHMEMG_OP_BARRIER_ALL && (unsigned)i + 1u <= MBp) {
@@ -473,8 +526,8 @@ __global__ void __launch_bounds__(PLAN_THREADS, 1) k_plan_batch(const PlanArgs a
                 }
                 d_st_rec(a.aux + auxi, r);
                 if (ntile && tile0 < a.cap_tiles) {       // first op of a run: its length = the stretch up to AMO_RUN_MAX ops
-                    unsigned len = 1;
-                    while (len < AMO_RUN_MAX && tid + len < NT && sh.cls[tid + len] == (unsigned char)cl) ++len;
+                    const unsigned left = (unsigned)sh.send[sstart - ((unsigned)i - tid)] - tid + 1u;     // ops of the stretch from here on
+                    const unsigned len = left < AMO_RUN_MAX ? left : AMO_RUN_MAX;
                     TileRec t = {};
                     t.kind = cl == 1 ? T_AMO : T_WAIT; t.nbytes = len; t.nt = 1; t.op = unit;
                     t.src = (unsigned long long)(a.aux + auxi);
@@ -487,7 +540,7 @@ __global__ void __launch_bounds__(PLAN_THREADS, 1) k_plan_batch(const PlanArgs a
                     f |= TF_SIGNAL | ((unsigned)o.sig_op << 8);
                     sig = (unsigned long long)(a.base + (size_t)o.target_pe * a.stride + o.sig_off);
                 }
-                d_cut_copy(dst, src, o.nbytes, seg, [&](unsigned p, unsigned kind, unsigned long long off, unsigned len) {
+                d_emit_cut(cut, o.nbytes, [&](unsigned p, unsigned kind, unsigned long long off, unsigned len) {
                     if (tile0 + p >= a.cap_tiles) return;
                     TileRec t;
                     t.dst = dst + off; t.src = src + off; t.sig = sig; t.value = o.value;
@@ -566,8 +619,10 @@ extern "C" int shmemg_enqueue_batch_ws(shmemg_world_t *w, const shmemg_op_t *ops
     const unsigned NT = nops >= PLAN_CHUNK ? PLAN_CHUNK : (unsigned)((nops + 31) / 32 * 32);
     const size_t smem = (size_t)6 * ndom * 4 + (size_t)C * PLAN_CHUNK * 4;
     if (!w->smem_attr_plan) {
-        SHMEMG_CUDA(w, cudaFuncSetAttribute(k_plan_batch, cudaFuncAttributeMaxDynamicSharedMemorySize,
+        SHMEMG_CUDA(w, cudaFuncSetAttribute(k_plan_batch<true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                             (int)((size_t)6 * PLAN_DOM_MAX * 4 + (size_t)PLAN_CLUSTER * PLAN_CHUNK * 4)));
+        SHMEMG_CUDA(w, cudaFuncSetAttribute(k_plan_batch<false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                            (int)((size_t)6 * PLAN_DOM_MAX * 4 + (size_t)PLAN_CHUNK * 4)));
         w->smem_attr_plan = true;
     }
     cudaStream_t st = (cudaStream_t)stream;
@@ -578,7 +633,8 @@ extern "C" int shmemg_enqueue_batch_ws(shmemg_world_t *w, const shmemg_op_t *ops
         at[0].id = cudaLaunchAttributeClusterDimension;
         at[0].val.clusterDim.x = C; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
         cfg.attrs = at; cfg.numAttrs = 1;
-        SHMEMG_CUDA(w, cudaLaunchKernelEx(&cfg, k_plan_batch, p));
+        if (C > 1) SHMEMG_CUDA(w, cudaLaunchKernelEx(&cfg, k_plan_batch<true>, p));
+        else SHMEMG_CUDA(w, cudaLaunchKernelEx(&cfg, k_plan_batch<false>, p));
     }
     ExecArgs a;
     a.tiles = p.tiles; a.ticket = &p.hdr->ticket; a.done = p.done; a.arrive = p.arrive; a.trace = nullptr;
