@@ -433,8 +433,8 @@ typedef struct shmemg_device_world {
     uint64_t heap_bytes;        /* usable bytes per PE                                                        */
     int32_t npes;
     int32_t reserved;
-    unsigned int *bar_count;    /* DEVICE: device-barrier arrival counter (control region)                    */
-    unsigned int *bar_gen;      /* DEVICE: device-barrier generation                                          */
+    unsigned long long *bar_arrivals;  /* DEVICE: device-barrier arrival counter (control region): monotonic, never reset */
+    void *reserved2;
 } shmemg_device_world_t;
 /* Fill *out (HOST) for world w; valid until shmemg_finalize. */
 SHMEMG_API int shmemg_device_world_get(const shmemg_world_t *w, shmemg_device_world_t *out);

@@ -16,8 +16,8 @@ extern "C" int shmemg_device_world_get(const shmemg_world_t *w, shmemg_device_wo
     out->heap_bytes = w->heap_bytes;
     out->npes = w->npes;
     out->reserved = 0;
-    out->bar_count = &w->ctl->bar_count;
-    out->bar_gen = &w->ctl->bar_gen;
+    out->bar_arrivals = &w->ctl->bar_arrivals;
+    out->reserved2 = nullptr;
     return SHMEMG_OK;
 }
 

@@ -24,8 +24,7 @@
 // ---- control region layout (device) -------------------------------------------------------------------
 struct CtlRegion {
     unsigned long long barrier_epoch;      // bumped by barrier_all_on_stream
-    unsigned int bar_count;                // in-kernel barrier: arrivals of the current generation
-    unsigned int bar_gen;                  // in-kernel barrier: generation (sense)
+    unsigned long long bar_arrivals;       // in-kernel barrier: arrivals ever (monotonic, never reset; always a multiple of npes between kernels)
     unsigned int pad[12];
     unsigned int sig_counter[SHMEMG_SIG_SLOTS];   // last-arriver counters of single put_signal launches
     unsigned int group_bar[128];           // per-PE arrival counters of multi-block PE agents (monotonic; halo_app.cu)
