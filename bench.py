@@ -1047,12 +1047,20 @@ def run_cuda(args):
     local = int(os.environ.get("LOCAL_RANK", "0"))
     if not torch.cuda.is_available():
         raise SystemExit("bench.py: no CUDA device; the shmemg hot path has no CPU fallback")
+    # SHMEMG_BENCH_ONE_GPU=1 (development only, marked in the JSON line): every rank uses cuda:0 and the rendezvous runs over
+    # gloo -- the N > 1 code path on a box with one GPU (NCCL refuses two ranks on one device)
+    one_gpu = os.environ.get("SHMEMG_BENCH_ONE_GPU") == "1"
+    if one_gpu:
+        local = 0
     torch.cuda.set_device(local)
     device = torch.device("cuda", local)
     dist = None
     if world > 1:
         import torch.distributed as dist
-        dist.init_process_group("nccl", device_id=device)
+        if one_gpu:
+            dist.init_process_group("gloo")
+        else:
+            dist.init_process_group("nccl", device_id=device)
     groups = args.only.split(",") if args.only else ALL_GROUPS
     inp = Inputs(args.small, groups)
     table = segment_table(inp)
@@ -1189,6 +1197,8 @@ def run_cuda(args):
                     "traffic_source": "profiles/%s (ncu --set full capture; launch-weighted mean over the kernel's segments)" % TRAFFIC_CSV}
 
     line = base_line(args, world)
+    if one_gpu:
+        line["config"]["workload"] += " [SHMEMG_BENCH_ONE_GPU: all ranks share cuda:0, development only]"
     line.update({"value": gbps, "amo_mops": mops, "ms_per_step": whole_ms / K,
                  "timed_ms_per_step": sum(v for k, v in seg_ms.items() if table[k]["cls"] != "xtime") / K, "dtype": "u8 (copies), u64 (AMOs), f64-accumulated f32 / i64 (sum_reduce)",
                  "segments": segments, "ceilings": ceil, "roofline": roofline, "clocks": clocks, "gpu_launches": launches,
