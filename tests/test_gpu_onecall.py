@@ -6,7 +6,7 @@ import numpy as np
 import pytest
 import torch
 
-from gpu_common import DEV, assert_objects_equal, heap_bytes_for, ops_to_dev, run_gpu_onecall, run_oracle
+from gpu_common import DEV, assert_objects_equal, heap_bytes_for, ops_to_dev, run_gpu, run_gpu_onecall, run_oracle
 from invariants import check_compare_swap_claim, check_fetch_add
 from litmus_model import enumerate_outcomes, to_spec_program
 from paper_2607_08006_b200 import CMP, ERR, OP, OP_DTYPE, ShmemgError, World
@@ -253,3 +253,73 @@ def test_descriptors_generated_on_the_gpu():
     for p in range(npes):
         t = (p + 1) % npes
         assert np.array_equal(got[t, :c[p]], pay[p, :c[p]]) and not got[t, c[p]:].any()
+
+
+def test_onecall_batches_captured_in_a_cuda_graph():
+    """shmemg_enqueue_batch is two kernel launches and nothing else (no host pass, no synchronisation, no allocation), so a
+    sequence of one-call batches can be captured in a CUDA graph; every replay plans the descriptors again on the device (the
+    descriptor array is re-read: it is changed between the replays here) and the batches stay stream-ordered inside the graph."""
+    npes, blk = 8, 20000
+    a = configs.c3a_put_program(npes, blk)                       # src -> dst (transpose)
+    b = a.fork()
+    for i in range(npes):
+        for j in range(npes):
+            b.put(i, j, ("src", i * blk), ("dst", j * blk), blk)   # dst -> src (transpose back)
+    while len(b.ops) < len(a.ops):
+        b.barrier_all()                                          # same number of descriptors as `a` (which ends with a barrier)
+    w = World(npes, heap_bytes_for(a), DEV)
+    ld = Loaded(w, a)
+    oa, ob = ld.translate(a), ld.translate(b)
+    assert len(oa) == len(ob)
+    da, db = ops_to_dev(oa), ops_to_dev(ob)
+    work = torch.empty(w.batch_work_bytes(len(oa), int(oa["nbytes"].sum())), dtype=torch.uint8, device=DEV)
+    src0 = ld.obj_numpy("src").copy()
+    s = torch.cuda.Stream()
+    with torch.cuda.stream(s):
+        w.enqueue_batch_dev(da, len(oa), work)                   # warm-up outside the capture (function attributes)
+        w.enqueue_batch_dev(db, len(ob), work)
+        torch.cuda.synchronize()
+        g = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(g, stream=s):
+            for _ in range(3):
+                w.enqueue_batch_dev(da, len(oa), work)
+                w.enqueue_batch_dev(db, len(ob), work)
+            w.enqueue_batch_dev(da, len(oa), work)
+        g.replay()
+        torch.cuda.synchronize()
+        assert w.batch_status(work) == (0, 0)
+        exp_dst = src0.reshape(npes, npes, blk).transpose(1, 0, 2).reshape(npes, npes * blk)
+        assert np.array_equal(ld.obj_numpy("dst"), exp_dst) and np.array_equal(ld.obj_numpy("src"), src0)
+        # the descriptors are device data read at replay time: make the LAST batch of the graph the back-transpose too
+        ld.obj("dst").copy_(torch.from_numpy(exp_dst))
+        ld.obj("src").zero_()
+        da.copy_(db)
+        g.replay()
+        torch.cuda.synchronize()
+    assert np.array_equal(ld.obj_numpy("src"), src0)              # every batch of this replay was dst -> src
+
+
+@pytest.mark.parametrize("form", ["pre-planned", "one-call"])
+def test_signal_produced_by_one_batch_and_awaited_by_the_next(form):
+    """Every executor launch starts as a programmatic dependent of the kernel before it: its CTAs may be resident while the
+    previous batch still runs.  A batch that WAITS for a signal the previous batch sets, and then forwards the payload, must
+    still see signal and payload (nothing mutable is touched before griddepcontrol.wait).  20 rounds back to back."""
+    npes, n = 6, 30000
+    prog = Program(npes)
+    prog.obj("src", n, gen.u64(npes * n // 8, 17).view(np.uint8).reshape(npes, n))
+    prog.obj("mid", n)
+    prog.obj("dst", n)
+    prog.obj("sig", 8)
+    batches = []
+    for r in range(1, 21):
+        b1 = prog.fork()
+        for i in range(npes):
+            b1.put_signal(i, (i + 1) % npes, ("mid", 0), ("src", 0), n - r, ("sig", 0), r)
+        b2 = prog.fork()
+        for i in range(npes):
+            b2.signal_wait_until(i, ("sig", 0), CMP.GE, r)
+            b2.put(i, (i + 2) % npes, ("dst", 0), ("mid", 0), n - r)
+        batches += [b1, b2]
+    w, ld = (run_gpu if form == "pre-planned" else run_gpu_onecall)(prog, batches=batches)
+    ow = run_oracle(prog, batches=batches)
+    assert_objects_equal(prog, ld, ow)
