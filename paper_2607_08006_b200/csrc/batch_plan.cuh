@@ -24,7 +24,7 @@
 #define TRACE_SLOTS 8
 #define TRACE_CTAS 256
 #define TRACE_BYTES (TRACE_CTAS * TRACE_SLOTS * 8)   // per-CTA timestamps (SHMEMG_TRACE=1)
-#define PLAN_CHUNK_OPS 1024u      // a run of AMOs / waits never crosses a multiple of this op index (the device planner's chunk)
+#define PLAN_CHUNK_OPS 512u       // a run of AMOs / waits never crosses a multiple of this op index (the device planner's chunk)
 #define WAIT_RUN_MAX GEN_THREADS  // consecutive waits (of any PEs) polled by one tile, one per generic thread
 
 // tile kinds (bits 0-7 of TileRec.kind); bits 8-15 hold sig_op (put_signal)

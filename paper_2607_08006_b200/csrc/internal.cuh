@@ -60,6 +60,7 @@ struct shmemg_world {
     bool smem_attr_bcast = false, smem_attr_ib = false;
     bool smem_attr_red[4][7] = {};         // k_sum_reduce_tma<dtype, op>
     bool smem_attr_set = false;            // the batch executor and the single-copy bulk kernel
+    int plan_cluster = 0;                  // CTAs of the device planner's cluster (16, or 8 where 16 cannot be scheduled); 0 = not probed yet
     uint8_t *arena = nullptr;              // DEVICE: plan arena (SHMEMG_ARENA_BYTES) behind the control region
     struct Team { int start, stride, size; };
     int teams_world_npes = 0;              // npes of the world while a team view is active (surface2.cu)

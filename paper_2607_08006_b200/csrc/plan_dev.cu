@@ -3,7 +3,7 @@
 // or stream-triggered operation", L396).  No host pass over the descriptors, no synchronisation: the descriptors may have
 // been produced by an earlier kernel of the stream (the graph workload's natural case).
 //
-//   k_plan_batch (1 CTA, or a cluster of 8 CTAs for more than 2048 ops; 1024 threads each)  validates the descriptors, resolves PE -> address translation, cuts the copies into
+//   k_plan_batch (1 CTA, or a cluster of 16 CTAs for more than 1024 ops; up to 512 threads each)  validates the descriptors, resolves PE -> address translation, cuts the copies into
 //       tiles and writes EXACTLY the plan the host planner of batch.cu writes (same tile / AMO / wait records, same
 //       dependency thresholds), so the same executor kernel runs both forms.  What the host does with two sequential passes
 //       is done here with block-wide scans:
@@ -11,7 +11,7 @@
 //           any later op through a BARRIER_ALL) follows from four maxima per domain -- last op, last op that is not a wait,
 //           last marker a later op follows -- found with shared-memory atomicMax, no scan;
 //         * tile-record / AMO-record / unit indices, the segment-length rule of streaming batches and the BARRIER_ALL
-//           thresholds are prefix sums / prefix maxima over the op array (one op per thread, 1024 ops per CTA, block totals
+//           thresholds are prefix sums / prefix maxima over the op array (one op per thread, 512 ops per CTA, block totals
 //           exchanged through distributed shared memory, a carry between super-chunks);
 //         * the per-domain thresholds (counted ops of the domain before its latest FENCE / QUIET / end of a run of waits) are a
 //           keyed prefix count: one warp walks the ops 32 at a time, ranks them inside their domain with match.any and
@@ -22,7 +22,7 @@
 #include "batch_plan.cuh"
 
 #ifndef PLAN_THREADS
-#define PLAN_THREADS 1024
+#define PLAN_THREADS 512          // threads per planner CTA = ops per CTA and super-chunk: 128 registers per thread, no spills
 #endif
 #define PLAN_DOM_MAX 4096            // SHMEMG_CTX_MAX * npes the planner's shared-memory tables hold (npes <= 512)
 #define FULLM 0xffffffffu
@@ -172,7 +172,7 @@ template <typename T> __device__ __forceinline__ void d_st_rec(T *p, const T &r)
     d[0] = s[0]; d[1] = s[1]; d[2] = s[2]; d[3] = s[3];
 }
 
-// ---- block-wide inclusive scan of (a, b, c: sums; m: maximum), 1024 threads ------------------------------------------------
+// ---- block-wide inclusive scan of (a, b, c: sums; m: maximum), up to 1024 threads ------------------------------------------------
 struct S4 { unsigned a, b, c, m; };
 __device__ __forceinline__ S4 s4_comb(const S4 &x, const S4 &y) { return {x.a + y.a, x.b + y.b, x.c + y.c, x.m > y.m ? x.m : y.m}; }
 __device__ __forceinline__ S4 s4_shfl_up(const S4 &v, int o) {
@@ -223,10 +223,14 @@ __device__ __forceinline__ uint32_t cl_map(const void *p, unsigned rank) {   // 
 }
 __device__ __forceinline__ unsigned cl_ld(uint32_t a) { unsigned v; asm volatile("ld.shared::cluster.u32 %0, [%1];" : "=r"(v) : "r"(a) : "memory"); return v; }
 __device__ __forceinline__ unsigned long long cl_ld64(uint32_t a) { unsigned long long v; asm volatile("ld.shared::cluster.u64 %0, [%1];" : "=l"(v) : "r"(a) : "memory"); return v; }
+__device__ __forceinline__ void cl_red_max(uint32_t a, unsigned v) { asm volatile("red.relaxed.cluster.shared::cluster.max.u32 [%0], %1;" ::"r"(a), "r"(v) : "memory"); }
 __device__ __forceinline__ void cl_st(uint32_t a, unsigned v) { asm volatile("st.shared::cluster.u32 [%0], %1;" ::"r"(a), "r"(v) : "memory"); }
 
-#define PLAN_CLUSTER 8
+#ifndef PLAN_CLUSTER
+#define PLAN_CLUSTER 16              // CTAs of the large-batch planner (non-portable cluster size; 8 where 16 cannot be scheduled)
+#endif
 #define PLAN_CHUNK PLAN_THREADS                  // ops per CTA and super-chunk at full size (the kernel's chunk is blockDim.x)
+static_assert(PLAN_CHUNK == PLAN_CHUNK_OPS, "the host planner cuts runs of AMOs / waits where the device planner's chunks end");
 // -DSHMEMG_PLAN_TRACE: phase timestamps (%globaltimer, ns) of the planner in the header's spare words hdr->pad3[k]
 #ifdef SHMEMG_PLAN_TRACE
 #define PTRACE(k) do { if (rank == 0 && tid == 0) { unsigned long long t_; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t_)); a.hdr->pad3[k] = t_; } } while (0)
@@ -253,8 +257,10 @@ struct PlanShared {
 // One planner CTA per PLAN_CHUNK ops of a super-chunk (C * PLAN_CHUNK ops); C = cluster size (1 for small batches).
 // CL: launched as a thread-block cluster (large batches).  The single-CTA instantiation carries none of the cluster code: the
 // planner of a small batch is bound by instruction fetch (cold code in every launch), so its code path is kept short.
-template <bool CL>
-__global__ void __launch_bounds__(PLAN_THREADS, 1) k_plan_batch(const PlanArgs a) {
+// MAXT: upper bound of the CTA size.  A batch of up to 256 ops runs the <false, 256> instantiation, whose register budget is
+// not the 64 of a 1024-thread CTA (no spills).
+template <bool CL, int MAXT>
+__global__ void __launch_bounds__(MAXT, 1) k_plan_batch(const PlanArgs a) {
     extern __shared__ unsigned dsm[];                 // 6 tables of ndom entries, then (rank 0) C * PLAN_CHUNK compact keys
     __shared__ PlanShared sh;
     const unsigned nd = a.ndom;
@@ -263,15 +269,30 @@ __global__ void __launch_bounds__(PLAN_THREADS, 1) k_plan_batch(const PlanArgs a
     unsigned *issued = pL, *thresh = pLnw, *wrun = fL;               // (rank 0, keyed pass) reuse tables that are dead by then
     unsigned *ckey = dsm + 6 * nd;
     const unsigned tid = threadIdx.x, C = CL ? cl_size() : 1u, rank = CL ? cl_rank() : 0u;
-    const unsigned NT = blockDim.x;                   // = ops per CTA and super-chunk: 1024, or fewer for a batch of fewer ops
+    const unsigned NT = blockDim.x;                   // = ops per CTA and super-chunk: PLAN_THREADS, or fewer for a batch of fewer ops
     const unsigned long long n = a.nops, SC = (unsigned long long)C * NT;
     const bool single = n <= SC;                      // one super-chunk: every op stays in its thread's registers
     // the executor may be set up now: it waits (griddepcontrol.wait) until this grid has finished
     asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
     PTRACE(0);
+    // Cluster path, one super-chunk: this CTA's descriptors (up to 64 KiB) come in with ONE bulk copy (cp.async.bulk, counted
+    // on an mbarrier) while the tables are being zeroed.  A thread that loads its own 64-byte record from global memory makes
+    // every warp-level load touch 16 cache lines: 5.2 us for 1024 threads, whether or not the descriptors are in L2.
+    __shared__ uint64_t opbar;
+    const bool staged = CL && single;
+    shmemg_op_t *const ostage = reinterpret_cast<shmemg_op_t *>(dsm + 6 * nd + (size_t)C * PLAN_CHUNK);
+    if (staged && tid == 0) {
+        mbar_init(&opbar, 1);
+        mbar_init_fence();
+        const unsigned long long first = (unsigned long long)rank * NT;
+        const unsigned cnt = first < n ? (unsigned)(n - first < NT ? n - first : NT) : 0u;
+        mbar_arrive_expect_tx(&opbar, cnt * (unsigned)sizeof(shmemg_op_t));
+        if (cnt) bulk_g2s(ostage, a.ops + first, cnt * (unsigned)sizeof(shmemg_op_t), &opbar);
+    }
     for (unsigned d = tid; d < 6 * nd; d += NT) dsm[d] = 0;
     if (tid == 0) { sh.p_bad = ~0ull; sh.p_bulk = 0; sh.p_lall = 0; sh.p_mb = 0; sh.p_keyed = 0; sh.p_ptiles = 0; sh.all_total = 0; }
     __syncthreads();
+    if (staged) mbar_wait(&opbar, 0);
 
     // ======== sweep 1: validate; maxima per domain; totals =====================================================================
     shmemg_op_t keep = {};
@@ -286,7 +307,7 @@ __global__ void __launch_bounds__(PLAN_THREADS, 1) k_plan_batch(const PlanArgs a
             const unsigned long long i = c0 + tid;
             const bool have = i < n;
             shmemg_op_t o = {};
-            if (have) o = d_ld_op(a.ops + i);
+            if (have) o = staged ? ostage[tid] : d_ld_op(a.ops + i);
             if (single) keep = o;
             const int rc = have ? d_validate(a, o) : 0;
             if (rc) atomicMin(&sh.p_bad, (i << 8) | (unsigned long long)(-rc));
@@ -312,11 +333,21 @@ __global__ void __launch_bounds__(PLAN_THREADS, 1) k_plan_batch(const PlanArgs a
     }
     PTRACE(1);
     cl_sync_all(C);
-    for (unsigned k = tid; k < nd * C; k += NT) {                    // last real op / last non-wait real op of every domain:
-        const unsigned d = k % nd, r = k / nd;                       // one (domain, CTA) pair per thread
-        const unsigned m1 = C > 1 ? cl_ld(cl_map(&pL[d], r)) : pL[d], m2 = C > 1 ? cl_ld(cl_map(&pLnw[d], r)) : pLnw[d];
-        if (m1) atomicMax(&fL[d], m1);
-        if (m2) atomicMax(&fLnw[d], m2);
+    // last real op / last non-wait real op of every domain, over the cluster: every CTA PUSHES its non-zero partial maxima into
+    // every CTA's table with fire-and-forget remote atomics (a pull costs one DSMEM round trip per (domain, CTA) pair and most
+    // pairs are empty: 13 us for 512 domains x 16 CTAs); the cluster barrier below makes them visible
+    for (unsigned d = tid; d < nd; d += NT) {                        // one domain per thread; most domains are empty
+        const unsigned m1 = pL[d], m2 = pLnw[d];
+        if (!(m1 | m2)) continue;
+        if (C > 1) {
+            for (unsigned r = 0; r < C; ++r) {
+                if (m1) cl_red_max(cl_map(&fL[d], r), m1);
+                if (m2) cl_red_max(cl_map(&fLnw[d], r), m2);
+            }
+        } else {
+            fL[d] = m1;
+            fLnw[d] = m2;
+        }
     }
     if (tid < 32) {                                    // lane r reads CTA r's partials (one DSMEM round trip), the warp combines
         unsigned long long bad = ~0ull, bulk = 0;
@@ -338,7 +369,7 @@ __global__ void __launch_bounds__(PLAN_THREADS, 1) k_plan_batch(const PlanArgs a
         }
         if (tid == 0) { sh.f_bad = bad; sh.f_bulk = bulk; sh.f_lall = lall; sh.f_ptiles = pt; }
     }
-    __syncthreads();
+    cl_sync_all(C);                                    // the pushed maxima have landed in every CTA's tables
     if (sh.f_bad != ~0ull) {                           // a bad descriptor: nothing is executed (shmemg_batch_status reports it)
         if (rank == 0 && tid == 0) {
             a.hdr->ntiles = 0; a.hdr->nunits = 0; a.hdr->npes = nd; a.hdr->trace_on = 0; a.hdr->ticket = 0; a.hdr->all_total = 0;
@@ -361,10 +392,11 @@ __global__ void __launch_bounds__(PLAN_THREADS, 1) k_plan_batch(const PlanArgs a
         else if (opc == SHMEMG_OP_SIGNAL_WAIT_UNTIL) { if ((unsigned)i + 1u < fLnw[dom]) { atomicMax(&pM[dom], (unsigned)i + 1u); sh.p_keyed = 1; } }
     }
     cl_sync_all(C);
-    for (unsigned k = tid; k < nd * C; k += NT) {
-        const unsigned d = k % nd, r = k / nd;
-        const unsigned m = C > 1 ? cl_ld(cl_map(&pM[d], r)) : pM[d];
-        if (m) atomicMax(&fM[d], m);
+    for (unsigned d = tid; d < nd; d += NT) {
+        const unsigned m = pM[d];
+        if (!m) continue;
+        if (C > 1) { for (unsigned r = 0; r < C; ++r) cl_red_max(cl_map(&fM[d], r), m); }
+        else fM[d] = m;
     }
     if (tid < 32) {
         unsigned mb = 0, k = 0;
@@ -612,16 +644,37 @@ extern "C" int shmemg_enqueue_batch_ws(shmemg_world_t *w, const shmemg_op_t *ops
     p.done = (unsigned *)(wk + l.done_off); p.arrive = (unsigned *)(wk + l.arrive_off);
     p.cap_tiles = (unsigned)cap; p.ndom = ndom;
     p.tiles_off = l.tiles_off; p.aux_off = l.aux_off; p.done_off = l.done_off; p.arrive_off = l.arrive_off;
-    // a small batch is planned by one CTA (no cluster barriers on its critical path), a large one by a cluster of 8
-    const unsigned C = nops <= 2 * PLAN_CHUNK ? 1u : PLAN_CLUSTER;
-    // one thread per op: a batch of fewer than 1024 ops is planned by as many warps as it needs (the planner of a small
+    // a small batch is planned by one CTA (no cluster barriers on its critical path), a large one by a cluster of 16 (or 8)
+    if (!w->plan_cluster) {                                      // once per world: can a cluster of PLAN_CLUSTER planner CTAs be scheduled?
+        w->plan_cluster = 8;
+        if (PLAN_CLUSTER > 8 &&
+            cudaFuncSetAttribute(k_plan_batch<true, PLAN_THREADS>, cudaFuncAttributeNonPortableClusterSizeAllowed, 1) == cudaSuccess) {
+            cudaLaunchConfig_t q = {};
+            q.gridDim = dim3(PLAN_CLUSTER); q.blockDim = dim3(PLAN_THREADS);
+            q.dynamicSmemBytes = (size_t)6 * PLAN_DOM_MAX * 4 + (size_t)PLAN_CLUSTER * PLAN_CHUNK * 4 + (size_t)PLAN_CHUNK * sizeof(shmemg_op_t);
+            cudaLaunchAttribute qa[1];
+            qa[0].id = cudaLaunchAttributeClusterDimension;
+            qa[0].val.clusterDim.x = PLAN_CLUSTER; qa[0].val.clusterDim.y = 1; qa[0].val.clusterDim.z = 1;
+            q.attrs = qa; q.numAttrs = 1;
+            int nclusters = 0;
+            cudaFuncSetAttribute(k_plan_batch<true, PLAN_THREADS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)q.dynamicSmemBytes);
+            if (cudaOccupancyMaxActiveClusters(&nclusters, k_plan_batch<true, PLAN_THREADS>, &q) == cudaSuccess && nclusters >= 1)
+                w->plan_cluster = PLAN_CLUSTER;
+        }
+        cudaGetLastError();
+    }
+    const unsigned C = nops <= 2 * PLAN_CHUNK ? 1u : (unsigned)w->plan_cluster;
+    // one thread per op: a batch of fewer than PLAN_CHUNK ops is planned by as many warps as it needs (the planner of a small
     // batch is bound by instruction issue: 96 ops on 32 warps take 12 us, on 3 warps 5 us)
     const unsigned NT = nops >= PLAN_CHUNK ? PLAN_CHUNK : (unsigned)((nops + 31) / 32 * 32);
-    const size_t smem = (size_t)6 * ndom * 4 + (size_t)C * PLAN_CHUNK * 4;
+    const size_t smem = (size_t)6 * ndom * 4 + (size_t)C * PLAN_CHUNK * 4 + (C > 1 ? (size_t)PLAN_CHUNK * sizeof(shmemg_op_t) : 0);
     if (!w->smem_attr_plan) {
-        SHMEMG_CUDA(w, cudaFuncSetAttribute(k_plan_batch<true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                            (int)((size_t)6 * PLAN_DOM_MAX * 4 + (size_t)PLAN_CLUSTER * PLAN_CHUNK * 4)));
-        SHMEMG_CUDA(w, cudaFuncSetAttribute(k_plan_batch<false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+        SHMEMG_CUDA(w, cudaFuncSetAttribute(k_plan_batch<true, PLAN_THREADS>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                            (int)((size_t)6 * PLAN_DOM_MAX * 4 + (size_t)PLAN_CLUSTER * PLAN_CHUNK * 4 +
+                                                  (size_t)PLAN_CHUNK * sizeof(shmemg_op_t))));
+        SHMEMG_CUDA(w, cudaFuncSetAttribute(k_plan_batch<false, PLAN_THREADS>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                            (int)((size_t)6 * PLAN_DOM_MAX * 4 + (size_t)PLAN_CHUNK * 4)));
+        SHMEMG_CUDA(w, cudaFuncSetAttribute(k_plan_batch<false, 256>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                             (int)((size_t)6 * PLAN_DOM_MAX * 4 + (size_t)PLAN_CHUNK * 4)));
         w->smem_attr_plan = true;
     }
@@ -633,8 +686,9 @@ extern "C" int shmemg_enqueue_batch_ws(shmemg_world_t *w, const shmemg_op_t *ops
         at[0].id = cudaLaunchAttributeClusterDimension;
         at[0].val.clusterDim.x = C; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
         cfg.attrs = at; cfg.numAttrs = 1;
-        if (C > 1) SHMEMG_CUDA(w, cudaLaunchKernelEx(&cfg, k_plan_batch<true>, p));
-        else SHMEMG_CUDA(w, cudaLaunchKernelEx(&cfg, k_plan_batch<false>, p));
+        if (C > 1) SHMEMG_CUDA(w, cudaLaunchKernelEx(&cfg, k_plan_batch<true, PLAN_THREADS>, p));
+        else if (NT <= 256) SHMEMG_CUDA(w, cudaLaunchKernelEx(&cfg, k_plan_batch<false, 256>, p));
+        else SHMEMG_CUDA(w, cudaLaunchKernelEx(&cfg, k_plan_batch<false, PLAN_THREADS>, p));
     }
     ExecArgs a;
     a.tiles = p.tiles; a.ticket = &p.hdr->ticket; a.done = p.done; a.arrive = p.arrive; a.trace = nullptr;
