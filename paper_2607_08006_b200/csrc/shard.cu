@@ -250,11 +250,16 @@ static int check_transfer(const shmemg_world *w, ShardView &v, uint64_t dest_off
     return SHMEMG_OK;
 }
 
+// both endpoints on this shard: the single-GPU path (bulk-copy pipeline, GPU-scope signal) does the transfer
+static bool both_local(const shmemg_world *w, int target_gpe) { return target_gpe % w->nshards == w->shard; }
+
 extern "C" int shmemg_gput_on_stream(shmemg_world_t *w, uint64_t dest_off, uint64_t source_off, size_t nbytes, int gpe,
                                      int target_gpe, void *stream) {
     ShardView v;
     int rc = check_transfer(w, v, dest_off, source_off, nbytes, gpe, target_gpe);
     if (rc) return rc;
+    if (both_local(w, target_gpe))
+        return shmemg_put_on_stream(w, dest_off, source_off, nbytes, gpe / w->nshards, target_gpe / w->nshards, stream);
     return launch_shard_copy(w, host_g_addr(w, target_gpe, dest_off), host_g_addr(w, gpe, source_off), nbytes, nullptr, 0, 0,
                              (cudaStream_t)stream);
 }
@@ -263,6 +268,8 @@ extern "C" int shmemg_gget_on_stream(shmemg_world_t *w, uint64_t dest_off, uint6
     ShardView v;
     int rc = check_transfer(w, v, dest_off, source_off, nbytes, gpe, target_gpe);
     if (rc) return rc;
+    if (both_local(w, target_gpe))
+        return shmemg_get_on_stream(w, dest_off, source_off, nbytes, gpe / w->nshards, target_gpe / w->nshards, stream);
     return launch_shard_copy(w, host_g_addr(w, gpe, dest_off), host_g_addr(w, target_gpe, source_off), nbytes, nullptr, 0, 0,
                              (cudaStream_t)stream);
 }
@@ -274,6 +281,10 @@ extern "C" int shmemg_gput_signal_on_stream(shmemg_world_t *w, uint64_t dest_off
     if (rc) return rc;
     if (!shmemg_in_range(w, sig_off, 8)) return SHMEMG_ERR_RANGE;
     if (sig_off & 7) return SHMEMG_ERR_ALIGN;
+    // a signal word may also be updated from another shard (system scope): only a one-shard world takes the GPU-scope path
+    if (w->nshards == 1)
+        return shmemg_put_signal_on_stream(w, dest_off, source_off, nbytes, sig_off, signal, sig_op, gpe / w->nshards,
+                                           target_gpe / w->nshards, stream);
     return launch_shard_copy(w, host_g_addr(w, target_gpe, dest_off), host_g_addr(w, gpe, source_off), nbytes,
                              (unsigned long long *)host_g_addr(w, target_gpe, sig_off), signal, sig_op, (cudaStream_t)stream);
 }
