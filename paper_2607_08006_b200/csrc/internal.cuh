@@ -57,7 +57,7 @@ struct shmemg_world {
     size_t tile_bytes_override = 0;        // SHMEMG_TILE_BYTES (experiments; forces the register copy path)
     // dynamic shared memory opt-in (cudaFuncSetAttribute) done on THIS world's device, per kernel family
     bool smem_attr_coll = false, smem_attr_probe = false, smem_attr_plan = false, smem_attr_hot = false;
-    bool smem_attr_bcast = false, smem_attr_ib = false;
+    bool smem_attr_bcast = false, smem_attr_ib = false, smem_attr_shard = false;
     bool smem_attr_red[4][7] = {};         // k_sum_reduce_tma<dtype, op>
     bool smem_attr_set = false;            // the batch executor and the single-copy bulk kernel
     int plan_cluster = 0;                  // CTAs of the device planner's cluster (16, or 8 where 16 cannot be scheduled); 0 = not probed yet

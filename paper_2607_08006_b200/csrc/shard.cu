@@ -8,13 +8,14 @@
 // from / stores to / performs atomics on peer memory over NVLink 5 / NVSwitch:
 //   put / get / put_signal   register-path copy (16-byte vector accesses where the alignment allows), last-arriver signal;
 //   AMO batches              red / atom at SYSTEM scope (the atomicity domain is the fabric, not one GPU's L2);
-//   alltoall                 every (local source PE, global destination PE) block is pushed into the destination's window;
+//   alltoall                 every (local source PE, global destination PE) block is pushed into the destination's window
+//                            (bulk copies through shared memory when everything is 16-byte aligned);
 //   barrier                  one kernel per shard: arrive on EVERY shard's counter (red.release.sys), wait for the own one.
 // Nothing here touches the single-GPU kernels; with nshards == 1 the g-calls compute what their unsharded counterparts compute.
 #include <stddef.h>
 #include <string.h>
 
-#include "internal.cuh"
+#include "tma_stream.cuh"
 
 struct ShardView {                      // by value into the kernels
     uint8_t *base[SHMEMG_MAX_SHARDS];
@@ -124,6 +125,27 @@ k_shard_alltoall(const ShardView v, unsigned long long dst_off, unsigned long lo
         uint8_t *dst = g_addr(v, j, dst_off) + (size_t)s * nbytes + off;
         copy_coop<8>(dst, src, n, threadIdx.x, SHMEMG_THREADS);
     }
+}
+
+// bulk-copy form (everything 16-byte aligned): one issuing thread per CTA streams (source PE, destination PE, chunk) items
+// through shared memory; the bulk store's destination is the destination shard's window -- local HBM or peer memory alike
+__global__ void __launch_bounds__(32)
+k_shard_alltoall_tma(const ShardView v, unsigned long long dst_off, unsigned long long src_off, size_t nbytes) {
+    extern __shared__ __align__(1024) uint8_t stage[];
+    __shared__ uint64_t full[SHMEMG_TMA_STAGES];
+    if (threadIdx.x != 0) return;
+    tma_stream_init(full);
+    const int gn = v.nshards * v.npes_local;
+    const size_t chunks = (nbytes + SHMEMG_TMA_TILE - 1) / SHMEMG_TMA_TILE;
+    const size_t items = (size_t)v.npes_local * gn * chunks;
+    tma_stream_copy(stage, full, blockIdx.x, gridDim.x, items, [&](size_t it, const uint8_t *&s, uint8_t *&d, unsigned &n) {
+        const size_t c = it % chunks;
+        const int j = (int)((it / chunks) % gn), l = (int)(it / chunks / gn);
+        const size_t off = c * SHMEMG_TMA_TILE;
+        n = (unsigned)(nbytes - off < SHMEMG_TMA_TILE ? nbytes - off : SHMEMG_TMA_TILE);
+        s = v.base[v.shard] + (unsigned long long)l * v.stride + src_off + (size_t)j * nbytes + off;
+        d = g_addr(v, j, dst_off) + (size_t)(l * v.nshards + v.shard) * nbytes + off;
+    });
 }
 
 // ---- barrier of the shards' streams ------------------------------------------------------------------------------------
@@ -348,6 +370,17 @@ extern "C" int shmemg_galltoall_on_stream(shmemg_world_t *w, uint64_t dest_off, 
     if (!shmemg_in_range(w, dest_off, span) || !shmemg_in_range(w, source_off, span)) return SHMEMG_ERR_RANGE;
     if (nbytes_per_pe == 0) return SHMEMG_OK;
     if (dest_off < source_off + span && source_off < dest_off + span) return SHMEMG_ERR_OVERLAP;
+    if (((dest_off | source_off | nbytes_per_pe | w->stride) & 15) == 0) {
+        if (!w->smem_attr_shard) {
+            SHMEMG_CUDA(w, cudaFuncSetAttribute(k_shard_alltoall_tma, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SHMEMG_TMA_SMEM));
+            w->smem_attr_shard = true;
+        }
+        const uint64_t it = (uint64_t)w->npes * gn * ((nbytes_per_pe + SHMEMG_TMA_TILE - 1) / SHMEMG_TMA_TILE);
+        k_shard_alltoall_tma<<<(unsigned)(it < (uint64_t)w->sm_count ? it : (uint64_t)w->sm_count), 32, SHMEMG_TMA_SMEM,
+                               (cudaStream_t)stream>>>(v, dest_off, source_off, nbytes_per_pe);
+        SHMEMG_CUDA(w, cudaGetLastError());
+        return SHMEMG_OK;
+    }
     const unsigned chunk = 32768;
     const uint64_t items = (uint64_t)w->npes * gn * ((nbytes_per_pe + chunk - 1) / chunk);
     const uint64_t maxgrid = (uint64_t)w->sm_count * w->ctas_per_sm;

@@ -34,6 +34,9 @@ class Case:
         p.obj("par", 8 * self.nwords, np.full((NP, 8 * self.nwords), 255, dtype=np.uint8))   # compare-swap slots, init -1
         p.obj("a2a_src", NP * self.blk, gen.u64(NP * NP * self.blk // 8, 92).view(np.uint8).reshape(NP, NP * self.blk))
         p.obj("a2a_dst", NP * self.blk)
+        self.blk2 = 48 * 1024 + 16                        # aligned blocks: the bulk-copy form, a ragged second chunk
+        p.obj("a2b_src", NP * self.blk2, gen.u64(NP * NP * self.blk2 // 8, 93).view(np.uint8).reshape(NP, NP * self.blk2))
+        p.obj("a2b_dst", NP * self.blk2)
         self.prog = p
         # phase 1: race-free random puts / gets, any size and alignment, op k owns slot k of `dst` on the PE it writes
         ph1 = p.fork()
@@ -75,6 +78,7 @@ class Case:
             ow.atomic_add_batch(ow.objs["words"][0], a["tgt"], a["idx"], a["val"])
             ow.atomic_fetch_add_batch(ow.objs["cnt"][0], a["tgt"], a["idx"], np.ones(len(a["idx"]), dtype=np.uint64))
         ow.alltoall(ow.objs["a2a_dst"][0], ow.objs["a2a_src"][0], self.blk)
+        ow.alltoall(ow.objs["a2b_dst"][0], ow.objs["a2b_src"][0], self.blk2)
         return ow
 
 
@@ -134,6 +138,7 @@ class ShardRunner:
 
     def run_alltoall(self):
         self.w.galltoall(self.off["a2a_dst"], self.off["a2a_src"], self.case.blk)
+        self.w.galltoall(self.off["a2b_dst"], self.off["a2b_src"], self.case.blk2)
 
     def rows(self, name):
         return self.w.view(self.off[name], self.case.prog.obj_bytes[self.case.prog.obj_names.index(name)]).cpu().numpy()
@@ -152,7 +157,7 @@ def check(case: Case, results: list):
     ow = case.oracle()
     G, NP, nw = case.G, case.NP, case.nwords
     for s in range(G):
-        for name in ("src", "dst", "ps", "sig", "words", "cnt", "a2a_src", "a2a_dst"):
+        for name in ("src", "dst", "ps", "sig", "words", "cnt", "a2a_src", "a2a_dst", "a2b_src", "a2b_dst"):
             off, nb = ow.objs[name]
             assert np.array_equal(results[s][name], orc.shard_rows(ow, s, G, off, nb)), (name, "shard", s)
     # global views of cnt / par assembled from the shards through the placement
