@@ -563,6 +563,15 @@ SHMEMG_API int shmemg_gatomic_batch_on_stream(shmemg_world_t *w, int op, uint64_
                                               void *stream);
 SHMEMG_API int shmemg_galltoall_on_stream(shmemg_world_t *w, uint64_t dest_off, uint64_t source_off, size_t nbytes_per_pe,
                                           void *stream);
+/* shmemg_gfcollect_on_stream: every local PE pushes its nbytes block into block g (its global number) of EVERY global PE's
+ * dest.  shmemg_gsum_reduce_on_stream (dtype SHMEMG_F32 or SHMEMG_I64): an all-reduce over all global PEs computed as
+ * reduce-scatter + all-gather over the fabric -- shard s reduces the s-th share of the nreduce elements over all the windows
+ * (peer loads, ascending GLOBAL PE order, fp32 accumulated in fp64 and rounded once: bit-equal to the single-GPU routine and
+ * to the oracle) and stores it into every PE's dest (peer stores).  source and dest must not overlap.  As for the alltoall,
+ * the caller puts a gbarrier before (sources ready) and after (results delivered). */
+SHMEMG_API int shmemg_gfcollect_on_stream(shmemg_world_t *w, uint64_t dest_off, uint64_t source_off, size_t nbytes, void *stream);
+SHMEMG_API int shmemg_gsum_reduce_on_stream(shmemg_world_t *w, int dtype, uint64_t dest_off, uint64_t source_off, size_t nreduce,
+                                            void *stream);
 SHMEMG_API int shmemg_gbarrier_all_on_stream(shmemg_world_t *w, void *stream);
 
 #ifdef __cplusplus

@@ -134,6 +134,8 @@ SYMBOLS = {
     "shmemg_gsignal_wait_until_on_stream": (_i, [_vp, _u64, _i, _u64, _i, _vp]),
     "shmemg_gatomic_batch_on_stream": (_i, [_vp, _i, _u64, _vp, _vp, _i, _vp, _u64, _vp, _u64, _vp, _sz, _vp]),
     "shmemg_galltoall_on_stream": (_i, [_vp, _u64, _u64, _sz, _vp]),
+    "shmemg_gfcollect_on_stream": (_i, [_vp, _u64, _u64, _sz, _vp]),
+    "shmemg_gsum_reduce_on_stream": (_i, [_vp, _i, _u64, _u64, _sz, _vp]),
     "shmemg_gbarrier_all_on_stream": (_i, [_vp, _vp]),
     "shmemg_put_on_stream": (_i, [_vp, _u64, _u64, _sz, _i, _i, _vp]),
     "shmemg_get_on_stream": (_i, [_vp, _u64, _u64, _sz, _i, _i, _vp]),
@@ -698,6 +700,15 @@ class World:
     def galltoall(self, dest_off, source_off, nbytes, stream=None):
         self._chk(lib().shmemg_galltoall_on_stream(self.h, dest_off, source_off, nbytes, _stream(stream)), "shmemg_galltoall_on_stream")
         self.launches += 1 if nbytes else 0
+
+    def gfcollect(self, dest_off, source_off, nbytes, stream=None):
+        self._chk(lib().shmemg_gfcollect_on_stream(self.h, dest_off, source_off, nbytes, _stream(stream)), "shmemg_gfcollect_on_stream")
+        self.launches += 1 if nbytes else 0
+
+    def gsum_reduce(self, dtype, dest_off, source_off, nreduce, stream=None):
+        self._chk(lib().shmemg_gsum_reduce_on_stream(self.h, dtype, dest_off, source_off, nreduce, _stream(stream)),
+                  "shmemg_gsum_reduce_on_stream")
+        self.launches += 1 if nreduce else 0
 
     def gbarrier_all(self, stream=None):
         self._chk(lib().shmemg_gbarrier_all_on_stream(self.h, _stream(stream)), "shmemg_gbarrier_all_on_stream")

@@ -148,6 +148,44 @@ k_shard_alltoall_tma(const ShardView v, unsigned long long dst_off, unsigned lon
     });
 }
 
+// ---- fcollect: local PE l (global s) pushes its block into block s of every global PE's destination --------------------
+__global__ void __launch_bounds__(SHMEMG_THREADS, 4)
+k_shard_fcollect(const ShardView v, unsigned long long dst_off, unsigned long long src_off, size_t nbytes, unsigned chunk) {
+    const int gn = v.nshards * v.npes_local;
+    const size_t chunks = (nbytes + chunk - 1) / chunk;
+    const size_t items = (size_t)v.npes_local * chunks * gn;
+    for (size_t it = blockIdx.x; it < items; it += gridDim.x) {      // consecutive items share the source chunk (L2)
+        const int j = (int)(it % gn);
+        const size_t c = (it / gn) % chunks;
+        const int l = (int)(it / gn / chunks);
+        const int s = l * v.nshards + v.shard;
+        const size_t off = c * chunk;
+        const size_t n = nbytes - off < chunk ? nbytes - off : chunk;
+        copy_coop<8>(g_addr(v, j, dst_off) + (size_t)s * nbytes + off, v.base[v.shard] + (unsigned long long)l * v.stride + src_off + off,
+                     n, threadIdx.x, SHMEMG_THREADS);
+    }
+}
+
+// ---- sum_reduce = reduce-scatter + all-gather over the fabric: this shard owns elements [e0, e1) -------------------------
+// One element per thread and trip: NP peer / local loads in ascending GLOBAL PE order (fp32 accumulated in fp64, one rounding;
+// int64 wraps), then NP stores.  The loads of one element by consecutive threads are coalesced per window.
+template <typename T> struct GAcc;
+template <> struct GAcc<float> { typedef double acc_t; };
+template <> struct GAcc<long long> { typedef unsigned long long acc_t; };
+template <typename T>
+__global__ void __launch_bounds__(256) k_shard_sum_reduce(const ShardView v, unsigned long long dst_off, unsigned long long src_off,
+                                                          size_t e0, size_t e1) {
+    typedef typename GAcc<T>::acc_t acc_t;
+    const int gn = v.nshards * v.npes_local;
+    for (size_t e = e0 + (size_t)blockIdx.x * blockDim.x + threadIdx.x; e < e1; e += (size_t)gridDim.x * blockDim.x) {
+        acc_t acc = 0;                                               // fp: +0.0 + x_0 + x_1 + ... (reading 13)
+        for (int g = 0; g < gn; ++g)
+            acc += (acc_t)*reinterpret_cast<const volatile T *>(g_addr(v, g, src_off) + e * sizeof(T));
+        const T r = (T)acc;
+        for (int g = 0; g < gn; ++g) *reinterpret_cast<T *>(g_addr(v, g, dst_off) + e * sizeof(T)) = r;
+    }
+}
+
 // ---- barrier of the shards' streams ------------------------------------------------------------------------------------
 // Everything this shard's stream did before the kernel is complete (kernel boundary); the system-scope release makes it visible to
 // whoever observes the arrival.  Each shard's counter advances by G per barrier; epoch = barriers enqueued so far on this world.
@@ -386,6 +424,52 @@ extern "C" int shmemg_galltoall_on_stream(shmemg_world_t *w, uint64_t dest_off, 
     const uint64_t maxgrid = (uint64_t)w->sm_count * w->ctas_per_sm;
     k_shard_alltoall<<<(unsigned)(items < maxgrid ? items : maxgrid), SHMEMG_THREADS, 0, (cudaStream_t)stream>>>(
         v, dest_off, source_off, nbytes_per_pe, chunk);
+    SHMEMG_CUDA(w, cudaGetLastError());
+    return SHMEMG_OK;
+}
+
+extern "C" int shmemg_gfcollect_on_stream(shmemg_world_t *w, uint64_t dest_off, uint64_t source_off, size_t nbytes, void *stream) {
+    ShardView v;
+    int rc = shard_view(w, v);
+    if (rc) return rc;
+    const uint64_t gn = (uint64_t)w->nshards * w->npes;
+    if (nbytes && gn > w->heap_bytes / nbytes) return SHMEMG_ERR_RANGE;
+    const uint64_t span = gn * nbytes;
+    if (!shmemg_in_range(w, dest_off, span) || !shmemg_in_range(w, source_off, nbytes)) return SHMEMG_ERR_RANGE;
+    if (nbytes == 0) return SHMEMG_OK;
+    if (dest_off < source_off + nbytes && source_off < dest_off + span) return SHMEMG_ERR_OVERLAP;
+    const unsigned chunk = 32768;
+    const uint64_t items = (uint64_t)w->npes * gn * ((nbytes + chunk - 1) / chunk);
+    const uint64_t maxgrid = (uint64_t)w->sm_count * w->ctas_per_sm;
+    k_shard_fcollect<<<(unsigned)(items < maxgrid ? items : maxgrid), SHMEMG_THREADS, 0, (cudaStream_t)stream>>>(v, dest_off, source_off,
+                                                                                                               nbytes, chunk);
+    SHMEMG_CUDA(w, cudaGetLastError());
+    return SHMEMG_OK;
+}
+
+extern "C" int shmemg_gsum_reduce_on_stream(shmemg_world_t *w, int dtype, uint64_t dest_off, uint64_t source_off, size_t nreduce,
+                                            void *stream) {
+    ShardView v;
+    int rc = shard_view(w, v);
+    if (rc) return rc;
+    if (dtype != SHMEMG_F32 && dtype != SHMEMG_I64) return SHMEMG_ERR_ARG;
+    const size_t es = dtype == SHMEMG_F32 ? 4 : 8;
+    if (nreduce > w->heap_bytes / es) return SHMEMG_ERR_RANGE;
+    const uint64_t span = (uint64_t)nreduce * es;
+    if (!shmemg_in_range(w, dest_off, span) || !shmemg_in_range(w, source_off, span)) return SHMEMG_ERR_RANGE;
+    if ((dest_off | source_off) & (es - 1)) return SHMEMG_ERR_ALIGN;
+    if (nreduce == 0) return SHMEMG_OK;
+    if (dest_off < source_off + span && source_off < dest_off + span) return SHMEMG_ERR_OVERLAP;
+    // this shard's share: elements [e0, e1), cut at multiples of 32 elements
+    const size_t per = ((nreduce + (size_t)w->nshards - 1) / (size_t)w->nshards + 31) / 32 * 32;
+    const size_t e0 = per * (size_t)w->shard < nreduce ? per * (size_t)w->shard : nreduce;
+    const size_t e1 = e0 + per < nreduce ? e0 + per : nreduce;
+    if (e1 == e0) return SHMEMG_OK;
+    const uint64_t maxgrid = (uint64_t)w->sm_count * 8;
+    const uint64_t blocks = (e1 - e0 + 255) / 256;
+    const unsigned grid = (unsigned)(blocks < maxgrid ? blocks : maxgrid);
+    if (dtype == SHMEMG_F32) k_shard_sum_reduce<float><<<grid, 256, 0, (cudaStream_t)stream>>>(v, dest_off, source_off, e0, e1);
+    else k_shard_sum_reduce<long long><<<grid, 256, 0, (cudaStream_t)stream>>>(v, dest_off, source_off, e0, e1);
     SHMEMG_CUDA(w, cudaGetLastError());
     return SHMEMG_OK;
 }

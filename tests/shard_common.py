@@ -37,6 +37,14 @@ class Case:
         self.blk2 = 48 * 1024 + 16                        # aligned blocks: the bulk-copy form, a ragged second chunk
         p.obj("a2b_src", NP * self.blk2, gen.u64(NP * NP * self.blk2 // 8, 93).view(np.uint8).reshape(NP, NP * self.blk2))
         p.obj("a2b_dst", NP * self.blk2)
+        # collectives over all global PEs: fp32 / int64 sum_reduce (ragged share per shard), fcollect of an odd block size
+        self.nred, self.fcb = 3000 + 17, 1001
+        p.obj("rf_src", 4 * self.nred, gen.normal_f32(NP * self.nred, 94).view(np.uint8).reshape(NP, 4 * self.nred))
+        p.obj("rf_dst", 4 * self.nred)
+        p.obj("ri_src", 8 * self.nred, gen.uniform_i64(NP * self.nred, -(1 << 62), 1 << 62, 95).view(np.uint8).reshape(NP, 8 * self.nred))
+        p.obj("ri_dst", 8 * self.nred)
+        p.obj("fc_src", self.fcb + 7, gen.u64(NP * (self.fcb + 7 + 7) // 8 + NP, 96).view(np.uint8)[:NP * (self.fcb + 7)].reshape(NP, self.fcb + 7))
+        p.obj("fc_dst", NP * self.fcb)
         self.prog = p
         # phase 1: race-free random puts / gets, any size and alignment, op k owns slot k of `dst` on the PE it writes
         ph1 = p.fork()
@@ -79,6 +87,9 @@ class Case:
             ow.atomic_fetch_add_batch(ow.objs["cnt"][0], a["tgt"], a["idx"], np.ones(len(a["idx"]), dtype=np.uint64))
         ow.alltoall(ow.objs["a2a_dst"][0], ow.objs["a2a_src"][0], self.blk)
         ow.alltoall(ow.objs["a2b_dst"][0], ow.objs["a2b_src"][0], self.blk2)
+        ow.sum_reduce_f32(ow.objs["rf_dst"][0], ow.objs["rf_src"][0], self.nred)
+        ow.sum_reduce_i64(ow.objs["ri_dst"][0], ow.objs["ri_src"][0], self.nred)
+        ow.fcollect(ow.objs["fc_dst"][0], ow.objs["fc_src"][0] + 3, self.fcb)         # unaligned source
         return ow
 
 
@@ -139,6 +150,9 @@ class ShardRunner:
     def run_alltoall(self):
         self.w.galltoall(self.off["a2a_dst"], self.off["a2a_src"], self.case.blk)
         self.w.galltoall(self.off["a2b_dst"], self.off["a2b_src"], self.case.blk2)
+        self.w.gsum_reduce(0, self.off["rf_dst"], self.off["rf_src"], self.case.nred)     # SHMEMG_F32
+        self.w.gsum_reduce(1, self.off["ri_dst"], self.off["ri_src"], self.case.nred)     # SHMEMG_I64
+        self.w.gfcollect(self.off["fc_dst"], self.off["fc_src"] + 3, self.case.fcb)
 
     def rows(self, name):
         return self.w.view(self.off[name], self.case.prog.obj_bytes[self.case.prog.obj_names.index(name)]).cpu().numpy()
@@ -157,7 +171,8 @@ def check(case: Case, results: list):
     ow = case.oracle()
     G, NP, nw = case.G, case.NP, case.nwords
     for s in range(G):
-        for name in ("src", "dst", "ps", "sig", "words", "cnt", "a2a_src", "a2a_dst", "a2b_src", "a2b_dst"):
+        for name in ("src", "dst", "ps", "sig", "words", "cnt", "a2a_src", "a2a_dst", "a2b_src", "a2b_dst", "rf_dst", "ri_dst",
+                     "fc_dst"):
             off, nb = ow.objs[name]
             assert np.array_equal(results[s][name], orc.shard_rows(ow, s, G, off, nb)), (name, "shard", s)
     # global views of cnt / par assembled from the shards through the placement
