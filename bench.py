@@ -198,6 +198,10 @@ def segment_table(inp: Inputs):
     if "c2" in g:
         seg["halo_put_signal_wait_onecall"] = dict(cls="xcopy", kernel="k_plan_batch + k_batch_exec",
                                                    bytes=HALO_ROUNDS * 2 * 48 * inp.halo.face_bytes, launches=HALO_ROUNDS)
+    if "c2" in g:
+        # the 50 one-call rounds replayed from ONE CUDA graph (device planner + executor per round, back to back)
+        seg["halo_put_signal_wait_onecall_graph"] = dict(cls="xcopy", kernel="k_plan_batch + k_batch_exec",
+                                                         bytes=HALO_ROUNDS * 2 * 48 * inp.halo.face_bytes, launches=HALO_ROUNDS)
     if "c5" in g:
         n, nb = inp.c5_npes, inp.c5_bytes
         seg["sum_reduce_f32"] = dict(cls="copy", kernel="k_sum_reduce_tma<f32>", bytes=2 * n * nb, launches=1)
@@ -462,13 +466,17 @@ class CudaBench:
                         w.enqueue_batch(self.halo_batches[r - 1])
             if self.halo_graphs is None:
                 self.halo_graphs = self._capture_halo_graphs()
-            lib_g, app_g, app_only_g = self.halo_graphs
+            lib_g, app_g, app_only_g, onecall_g = self.halo_graphs
             self.ld2.obj("sig").zero_()
             w.app_halo_pack(send_off, self.U_off, h.B)                   # faces as the application leaves them (outside the timed region)
             self.app_launches += 1
             with rec.seg("halo_put_signal_wait"):
                 lib_g.replay()
             w.launches += HALO_ROUNDS
+            self.ld2.obj("sig").zero_()
+            with rec.seg("halo_put_signal_wait_onecall_graph"):
+                onecall_g.replay()
+            w.launches += 2 * HALO_ROUNDS
             if "next2" in g:
                 with rec.seg("next1_halo_app_graph"):
                     app_g.replay()
@@ -549,7 +557,7 @@ class CudaBench:
         torch, h, w = self.torch, self.inp.halo, self.w2
         send_off, l0, a0 = self.ld2.off["send"][0], w.launches, self.app_launches
         graphs = []
-        for app, lib in ((False, True), (True, True), (True, False)):
+        for app, lib in ((False, True), (True, True), (True, False), (False, "one-call")):
             gr = torch.cuda.CUDAGraph()
             with torch.cuda.graph(gr, capture_error_mode="thread_local"):
                 if app:
@@ -558,7 +566,9 @@ class CudaBench:
                     if app:
                         w.app_halo_perturb(self.U_off, h.B, h.seed, r)
                         w.app_halo_pack(send_off, self.U_off, h.B)
-                    if lib:
+                    if lib == "one-call":
+                        w.enqueue_batch_dev(self.halo_ops_dev[r - 1], 96)
+                    elif lib:
                         w.enqueue_batch(self.halo_batches[r - 1])
             graphs.append(gr)
         w.launches, self.app_launches = l0, a0                           # capturing launches nothing
@@ -809,6 +819,13 @@ class CudaBench:
                 assert np.array_equal(host(self.ld2.obj("ghost")), o2.obj("ghost")), "halo ghosts after the graph replay"
                 assert np.array_equal(host(self.ld2.obj("sig")), o2.obj("sig")), "halo signal words after the graph replay"
                 ok["halo_put_signal_wait"] = True
+                self.ld2.obj("ghost").zero_()
+                self.ld2.obj("sig").zero_()
+                self.halo_graphs[3].replay()
+                assert w.batch_status() == (0, 0)
+                assert np.array_equal(host(self.ld2.obj("ghost")), o2.obj("ghost")), "halo ghosts after the one-call graph replay"
+                assert np.array_equal(host(self.ld2.obj("sig")), o2.obj("sig")), "halo signal words after the one-call graph replay"
+                ok["halo_put_signal_wait_onecall_graph"] = True
                 o2.obj("ghost")[:] = 0
                 o2.obj("sig")[:] = 0
                 for r in sorted(snaps):
