@@ -129,6 +129,8 @@ __global__ void __launch_bounds__(EXEC_THREADS, 1) k_batch_exec(const ExecArgs a
         mbar_init(&epochB, 1);
         mbar_init_fence();
     }
+    // every executor releases ITS dependents at once (a following executor or planner launch sets itself up while this one runs)
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
     if (a.hdr) {
         // One-call batch (shmemg_enqueue_batch): the planning kernel is the previous kernel of the stream and this one is
         // launched as its programmatic dependent, so everything above overlaps the planner; from here on its writes
@@ -155,7 +157,6 @@ __global__ void __launch_bounds__(EXEC_THREADS, 1) k_batch_exec(const ExecArgs a
     TileRec r0 = {};
     if (!a.hdr) {
         if (tid == 0 && blockIdx.x < ntiles) r0 = ld_rec(tiles + blockIdx.x);
-        asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
         asm volatile("griddepcontrol.wait;" ::: "memory");
     }
     __syncthreads();

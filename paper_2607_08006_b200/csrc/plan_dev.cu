@@ -281,6 +281,10 @@ __global__ void __launch_bounds__(MAXT, 1) k_plan_batch(const PlanArgs a) {
     __shared__ uint64_t opbar;
     const bool staged = CL && single;
     shmemg_op_t *const ostage = reinterpret_cast<shmemg_op_t *>(dsm + 6 * nd + (size_t)C * PLAN_CHUNK);
+    // The planner is itself a programmatic dependent of the kernel before it (an executor releases its dependents at entry):
+    // it is resident and has fetched its code while that kernel still runs, and touches nothing -- neither the descriptors,
+    // which that kernel may have written, nor the workspace, which a preceding executor still reads -- before this wait.
+    asm volatile("griddepcontrol.wait;" ::: "memory");
     if (staged && tid == 0) {
         mbar_init(&opbar, 1);
         mbar_init_fence();
@@ -685,7 +689,11 @@ extern "C" int shmemg_enqueue_batch_ws(shmemg_world_t *w, const shmemg_op_t *ops
         cudaLaunchAttribute at[1];
         at[0].id = cudaLaunchAttributeClusterDimension;
         at[0].val.clusterDim.x = C; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
-        cfg.attrs = at; cfg.numAttrs = 1;
+        cudaLaunchAttribute at2[2];
+        at2[0] = at[0];
+        at2[1].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+        at2[1].val.programmaticStreamSerializationAllowed = 1;
+        cfg.attrs = at2; cfg.numAttrs = getenv("SHMEMG_NO_PDL") ? 1 : 2;
         if (C > 1) SHMEMG_CUDA(w, cudaLaunchKernelEx(&cfg, k_plan_batch<true, PLAN_THREADS>, p));
         else if (NT <= 256) SHMEMG_CUDA(w, cudaLaunchKernelEx(&cfg, k_plan_batch<false, 256>, p));
         else SHMEMG_CUDA(w, cudaLaunchKernelEx(&cfg, k_plan_batch<false, PLAN_THREADS>, p));
