@@ -16,7 +16,8 @@ call is bracketed by CUDA events on the launching stream ("segments"); applicati
   `barrier`                  : us per barrier, in-kernel (128 co-resident PE agents) and stream-level
   `roofline`                 : the copy-class kernel with the largest share of the timed step, against MEASURED_PEAKS.json
   `e2e`                      : the same metric with every input copied from pinned HOST memory and every result read
-                               back to the host inside the timed region (shmemg_heap_write/read_on_stream)
+                               back to the host inside the timed region (shmemg_heap_write/read_on_stream); `value`
+                               pipelines upload / library call / read-back over three streams, `serial` does not
   `cpu_baseline`             : the CPU oracle (oracle/, single thread) on a bounded sample of the same workload
 
 `--impl reference` times the oracle alone (this tier's reference arm).  N > 1 runs N independent replicas (the path
@@ -612,75 +613,129 @@ class CudaBench:
             w.heap_read(p, host2d[p], off)
         self.d2h += host2d.numel() * host2d.element_size()
 
-    def e2e_step(self):
-        torch, inp, rec, g = self.torch, self.inp, self.rec, self.inp.groups
+    def _e2e_segments(self):
+        """The end-to-end leg as (segment, class, upload, library call, read-back) tuples: `upload` copies the segment's inputs
+        from pinned host memory, `read-back` its results to pinned host memory; all three enqueue on torch's CURRENT stream."""
+        inp, g, out = self.inp, self.inp.groups, []
+
+        def cp_in(dev_t, host_t):
+            dev_t.copy_(host_t, non_blocking=True)
+            self.h2d += host_t.numel() * host_t.element_size()
+
+        def cp_out(host_t, dev_t):
+            host_t.copy_(dev_t, non_blocking=True)
+            self.d2h += host_t.numel() * host_t.element_size()
         if "c3a" in g:
-            with rec.seg("alltoall"):
-                self._up(self.w3a, self.a_src, self.h_a_src)
-                self.w3a.alltoall(self.a_dst, self.a_src, inp.c3a_blk)
-                self._down(self.w3a, self.h_a_dst, self.a_dst)
-        if "c3b" in g:
-            with rec.seg("put_batch_skewed"):                            # descriptors are host inputs too: one-call form
-                self._up(self.w3b, self.ld3b.off["src"][0], self.h_b_src)
-                self.ops3b_dev.copy_(self.ops3b_host, non_blocking=True)
-                self.h2d += self.ops3b_host.numel()
-                self.w3b.enqueue_batch_dev(self.ops3b_dev, self.plan_us["put_batch_skewed"]["nops"], self.work3b)
-                self._down(self.w3b, self.h_b_dst, self.ld3b.off["dst"][0])
+            out.append(("alltoall", "copy", lambda: self._up(self.w3a, self.a_src, self.h_a_src),
+                        lambda: self.w3a.alltoall(self.a_dst, self.a_src, inp.c3a_blk),
+                        lambda: self._down(self.w3a, self.h_a_dst, self.a_dst)))
+        if "c3b" in g:                                                   # descriptors are host inputs too: one-call form
+            out.append(("put_batch_skewed", "copy",
+                        lambda: (self._up(self.w3b, self.ld3b.off["src"][0], self.h_b_src), cp_in(self.ops3b_dev, self.ops3b_host)),
+                        lambda: self.w3b.enqueue_batch_dev(self.ops3b_dev, self.plan_us["put_batch_skewed"]["nops"], self.work3b),
+                        lambda: self._down(self.w3b, self.h_b_dst, self.ld3b.off["dst"][0])))
         if "c5" in g:
-            n = inp.c5_bytes
-            with rec.seg("sum_reduce_f32"):
-                self._up(self.w5, self.s_f32, self.h_f32)
-                self.w5.sum_reduce(0, self.d5, self.s_f32, n // 4)
-                self._down(self.w5, self.h_res[0:1], self.d5)            # every PE holds the same result: read PE 0's
-            with rec.seg("sum_reduce_i64"):
-                self._up(self.w5, self.s_i64, self.h_i64)
-                self.w5.sum_reduce(1, self.d5, self.s_i64, n // 8)
-                self._down(self.w5, self.h_res[1:2], self.d5)
-            with rec.seg("fcollect"):
-                self._up(self.w5, self.s_fc, self.h_fc)
-                self.w5.fcollect(self.d5, self.s_fc, inp.c5_fc_bytes)
-                self._down(self.w5, self.h_res[2:3], self.d5)
+            n = inp.c5_bytes                                             # every PE holds the same result: PE 0's is read back
+            out.append(("sum_reduce_f32", "copy", lambda: self._up(self.w5, self.s_f32, self.h_f32),
+                        lambda: self.w5.sum_reduce(0, self.d5, self.s_f32, n // 4), lambda: self._down(self.w5, self.h_res[0:1], self.d5)))
+            out.append(("sum_reduce_i64", "copy", lambda: self._up(self.w5, self.s_i64, self.h_i64),
+                        lambda: self.w5.sum_reduce(1, self.d5, self.s_i64, n // 8), lambda: self._down(self.w5, self.h_res[1:2], self.d5)))
+            out.append(("fcollect", "copy", lambda: self._up(self.w5, self.s_fc, self.h_fc),
+                        lambda: self.w5.fcollect(self.d5, self.s_fc, inp.c5_fc_bytes), lambda: self._down(self.w5, self.h_res[2:3], self.d5)))
         if "c2" in g:
             w, fb = self.w2, inp.halo.face_bytes
-            self.ld2.obj("sig").zero_()
             send_off, ghost_off = self.ld2.off["send"][0], self.ld2.off["ghost"][0]
             for r in range(1, HALO_ROUNDS + 1):
-                with rec.seg("halo_put_signal_wait"):
-                    self._up(w, send_off, self.h_send)
-                    self.halo_ops_dev[r - 1].copy_(self.halo_ops_host[r - 1], non_blocking=True)
-                    self.h2d += self.halo_ops_host[r - 1].numel()
-                    w.enqueue_batch_dev(self.halo_ops_dev[r - 1], 96)
-                    self._down(w, self.h_ghost, ghost_off + (r & 1) * 6 * fb)
+                out.append(("halo_put_signal_wait", "copy",
+                            lambda r=r: (self._up(w, send_off, self.h_send), cp_in(self.halo_ops_dev[r - 1], self.halo_ops_host[r - 1])),
+                            lambda r=r: ((self.ld2.obj("sig").zero_() if r == 1 else None), w.enqueue_batch_dev(self.halo_ops_dev[r - 1], 96)),
+                            lambda r=r: self._down(w, self.h_ghost, ghost_off + (r & 1) * 6 * fb)))
         if "c1" in g:
-            self.w1.view(self.A, inp.c1.nelem * 8).zero_()
-            with rec.seg("atomic_add"):
-                for d, h in zip((self.c1_t, self.c1_i, self.c1_v), self.h_c1):
-                    d.copy_(h, non_blocking=True)
-                    self.h2d += h.numel() * h.element_size()
-                self.w1.atomic_add_batch(self.A, self.c1_t, self.c1_i, val=self.c1_v, flags=self.flags | self.c1_flags)
-                self._down(self.w1, self.h_A, self.A)
+            out.append(("atomic_add", "amo",
+                        lambda: [cp_in(d, h) for d, h in zip((self.c1_t, self.c1_i, self.c1_v), self.h_c1)],
+                        lambda: (self.w1.view(self.A, inp.c1.nelem * 8).zero_(),
+                                 self.w1.atomic_add_batch(self.A, self.c1_t, self.c1_i, val=self.c1_v, flags=self.flags | self.c1_flags)),
+                        lambda: self._down(self.w1, self.h_A, self.A)))
         if "c4" in g:
             vpp = inp.c4.verts_per_pe
-            self.w4.view(self.deg, vpp * 8).zero_()
-            self.w4.view(self.par, vpp * 8).fill_(255)
-            with rec.seg("atomic_fetch_add"):
-                for d, h in zip((self.c4_ou, self.c4_lu), self.h_c4[:2]):
-                    d.copy_(h, non_blocking=True)
-                    self.h2d += h.numel() * h.element_size()
-                self.w4.atomic_fetch_add_batch(self.deg, self.c4_ou, self.c4_lu, self.f_deg, val=None, val_scalar=1,
-                                               flags=self.fadd_flags)
-                self.h_fdeg.copy_(self.f_deg, non_blocking=True)
-                self.d2h += self.h_fdeg.numel() * 8
-                self._down(self.w4, self.h_deg, self.deg)
-            with rec.seg("atomic_compare_swap"):
-                for d, h in zip((self.c4_ov, self.c4_lv, self.c4_val), self.h_c4[2:]):
-                    d.copy_(h, non_blocking=True)
-                    self.h2d += h.numel() * h.element_size()
-                self.w4.atomic_compare_swap_batch(self.par, self.c4_ov, self.c4_lv, self.f_par, cond=None, cond_scalar=M64,
-                                                  val=self.c4_val, flags=self.cas_flags)
-                self.h_fpar.copy_(self.f_par, non_blocking=True)
-                self.d2h += self.h_fpar.numel() * 8
-                self._down(self.w4, self.h_par, self.par)
+            out.append(("atomic_fetch_add", "amo",
+                        lambda: [cp_in(d, h) for d, h in zip((self.c4_ou, self.c4_lu), self.h_c4[:2])],
+                        lambda: (self.w4.view(self.deg, vpp * 8).zero_(),
+                                 self.w4.atomic_fetch_add_batch(self.deg, self.c4_ou, self.c4_lu, self.f_deg, val=None, val_scalar=1,
+                                                                flags=self.fadd_flags)),
+                        lambda: (cp_out(self.h_fdeg, self.f_deg), self._down(self.w4, self.h_deg, self.deg))))
+            out.append(("atomic_compare_swap", "amo",
+                        lambda: [cp_in(d, h) for d, h in zip((self.c4_ov, self.c4_lv, self.c4_val), self.h_c4[2:])],
+                        lambda: (self.w4.view(self.par, vpp * 8).fill_(255),
+                                 self.w4.atomic_compare_swap_batch(self.par, self.c4_ov, self.c4_lv, self.f_par, cond=None, cond_scalar=M64,
+                                                                   val=self.c4_val, flags=self.cas_flags)),
+                        lambda: (cp_out(self.h_fpar, self.f_par), self._down(self.w4, self.h_par, self.par))))
+        return out
+
+    def e2e_step(self):
+        """Serial form: every segment's upload, library call and read-back on ONE stream inside its own event pair."""
+        for name, _cls, up, call, down in self._e2e_segments():
+            with self.rec.seg(name):
+                up(); call(); down()
+
+    def e2e_check(self):
+        """After a pipelined step: what was read back to the host equals what the device holds (the read-backs were ordered
+        behind their library calls), for every result buffer of the copy-class segments and the AMO arrays."""
+        torch, g, ok = self.torch, self.inp.groups, True
+        torch.cuda.synchronize()
+        eq = lambda host2d, w, off: bool(torch.equal(host2d, w.view(off, host2d.shape[1])[:host2d.shape[0]].cpu()))   # noqa: E731
+        if "c3a" in g:
+            ok &= eq(self.h_a_dst, self.w3a, self.a_dst)
+        if "c3b" in g:
+            ok &= eq(self.h_b_dst, self.w3b, self.ld3b.off["dst"][0])
+        if "c5" in g:
+            ok &= eq(self.h_res[2:3], self.w5, self.d5)            # the last collective's result (fcollect) is what d5 holds
+        if "c1" in g:
+            ok &= eq(self.h_A, self.w1, self.A)
+        if "c4" in g:
+            ok &= eq(self.h_deg, self.w4, self.deg) and eq(self.h_par, self.w4, self.par)
+            ok &= bool(torch.equal(self.h_fdeg, self.f_deg.cpu())) and bool(torch.equal(self.h_fpar, self.f_par.cpu()))
+        return bool(ok)
+
+    def e2e_step_pipelined(self):
+        """Pipelined form: uploads on one stream, library calls on the main stream, read-backs on a third one, chained with
+        events, so the upload of segment k + 1 overlaps the read-back of segment k (PCIe is full duplex: 55 + 57 GB/s one
+        way at a time, 100 GB/s together on this box).  Hazards: an upload waits for the library call of the previous
+        segment (it may overwrite that call's inputs); a library call waits for its own upload and for the read-back of the
+        previous segment (it may overwrite what is still being read).  One event pair around each class of segments (copy,
+        AMO); returns {class: (start, end)}."""
+        torch = self.torch
+        main = torch.cuda.current_stream()
+        if not hasattr(self, "s_up"):
+            self.s_up, self.s_dn = torch.cuda.Stream(), torch.cuda.Stream()
+        ev = lambda: torch.cuda.Event()                                       # noqa: E731
+        out, segs = {}, self._e2e_segments()
+        for cls in ("copy", "amo"):
+            mine = [x for x in segs if x[1] == cls]
+            if not mine:
+                continue
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record(main)
+            prev_c, prev_d = a, None
+            for _name, _cls, up, call, down in mine:
+                self.s_up.wait_event(prev_c)
+                with torch.cuda.stream(self.s_up):
+                    up()
+                    u = ev(); u.record(self.s_up)
+                main.wait_event(u)
+                if prev_d is not None:
+                    main.wait_event(prev_d)
+                call()
+                c = ev(); c.record(main)
+                self.s_dn.wait_event(c)
+                with torch.cuda.stream(self.s_dn):
+                    down()
+                    d = ev(); d.record(self.s_dn)
+                prev_c, prev_d = c, d
+            main.wait_event(prev_d)
+            b.record(main)
+            out[cls] = (a, b)
+        return out
 
     # ---- verification against the CPU oracle, after the timed loops and outside every timed region ------------------------
     def verify(self, ob):
@@ -998,12 +1053,12 @@ def max_over_ranks(dist, device, seg_ms, whole_ms, e2e_ms):
     (names, seg_ms, whole_ms, e2e_ms) with the reduced values; `dist` None = single process."""
     import torch
     names = sorted(seg_ms)
-    vec = torch.tensor([seg_ms[k] for k in names] + [whole_ms] + ([e2e_ms.get(k, 0.0) for k in names] if e2e_ms else []),
-                       dtype=torch.float64, device=device)
+    enames = sorted(e2e_ms) if e2e_ms else []                    # the end-to-end leg has its own keys (segments and pipelined regions)
+    vec = torch.tensor([seg_ms[k] for k in names] + [whole_ms] + [e2e_ms[k] for k in enames], dtype=torch.float64, device=device)
     if dist is not None:
         dist.all_reduce(vec, op=dist.ReduceOp.MAX)
     vec = vec.cpu().tolist()
-    out_e2e = dict(zip(names, vec[len(names) + 1:])) if e2e_ms else e2e_ms
+    out_e2e = dict(zip(enames, vec[len(names) + 1:])) if e2e_ms else e2e_ms
     return names, dict(zip(names, vec[:len(names)])), vec[len(names)], out_e2e
 
 
@@ -1110,7 +1165,7 @@ def run_cuda(args):
     cb.rec.pairs = []
 
     # ---- end-to-end leg ---------------------------------------------------------------------------------------------------
-    e2e_ms, h2d, d2h = None, 0, 0
+    e2e_ms, h2d, d2h, e2e_check = None, 0, 0, None
     if not args.no_e2e:
         cb.setup_e2e()
         cb.e2e_step()
@@ -1124,6 +1179,15 @@ def run_cuda(args):
         e2e_ms = cb.rec.totals_ms()
         h2d, d2h = cb.h2d // args.steps, cb.d2h // args.steps
         cb.rec.pairs = []
+        # the same transfers and calls, pipelined over three streams (upload / call / read-back)
+        cb.e2e_step_pipelined()
+        barrier()
+        regions = [cb.e2e_step_pipelined() for _ in range(args.steps)]
+        barrier()
+        for cls in ("copy", "amo"):
+            if regions and cls in regions[0]:
+                e2e_ms["__pipelined_" + cls] = sum(r[cls][0].elapsed_time(r[cls][1]) for r in regions)
+        e2e_check = cb.e2e_check()
     ceil = cb.ceilings() if rank == 0 else {}
 
     # ---- max over ranks of every segment time ---------------------------------------------------------------------------
@@ -1223,12 +1287,24 @@ def run_cuda(args):
     if e2e_ms:
         eu = {k: units[k] for k in names if k in e2e_ms and table[k]["cls"] != "sync"}
         es = {k: e2e_ms[k] * 1e-3 for k in eu}
-        eg, em, _, _ = class_rates(table, es, eu)
+        eg_serial, em_serial, _, _ = class_rates(table, es, eu)
+        eg, em = eg_serial, em_serial
+        pc, pa = e2e_ms.get("__pipelined_copy"), e2e_ms.get("__pipelined_amo")
+        if pc:                                                   # the same bytes / ops over the pipelined regions' times
+            eg = sum(v for k, v in eu.items() if table[k]["cls"] == "copy") / (pc * 1e-3) / 1e9
+        if pa:
+            em = sum(v for k, v in eu.items() if table[k]["cls"] == "amo") / (pa * 1e-3) / 1e6
         line["e2e"] = {"value": eg, "unit": UNIT, "amo_mops": em, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
-                       "ms_per_step": sum(es.values()) / K * 1e3,
-                       "note": "inputs from pinned host memory and results back to the host inside every segment; the two "
-                               "batch workloads use the one-call form: their descriptors are copied from pinned host memory "
-                               "and planned on the device inside the timed segment (no plan is reused)"}
+                       "ms_per_step": ((pc or 0.0) + (pa or 0.0)) / K if (pc or pa) else sum(es.values()) / K * 1e3,
+                       "serial": {"value": eg_serial, "amo_mops": em_serial, "ms_per_step": sum(es.values()) / K * 1e3},
+                       "results_read_back_equal_the_device_results": e2e_check,
+                       "note": "every step copies every input from pinned host memory and reads every result back to pinned host "
+                               "memory inside the timed region; `value` pipelines the segments over three streams (upload / library "
+                               "call / read-back, so the upload of one segment overlaps the read-back of the previous one: PCIe is "
+                               "full duplex), one event pair around each class of segments; `serial` runs upload, call and read-back "
+                               "of every segment on one stream inside its own event pair; the two batch workloads use the one-call "
+                               "form: their descriptors are copied from pinned host memory and planned on the device inside the "
+                               "timed region (no plan is reused)"}
     if world == 1 and not args.no_cpu:
         ob = OracleBench(inp)
         res = ob.step()
