@@ -457,7 +457,7 @@ __global__ void __launch_bounds__(MAXT, 1) k_plan_batch(const PlanArgs a) {
         cl_sync_all(C);
         {
             S4 pre = carryA, all = carryA;
-            if (C > 1) { for (unsigned r = 0; r < C; ++r) { if (r < rank) pre = s4_comb(pre, sh.xtA[r]); all = s4_comb(all, sh.xtA[r]); } }
+            if constexpr (CL) { for (unsigned r = 0; r < C; ++r) { if (r < rank) pre = s4_comb(pre, sh.xtA[r]); all = s4_comb(all, sh.xtA[r]); } }
             else all = s4_comb(all, tot);
             inc = s4_comb(pre, inc);
             carryA = all;
@@ -500,7 +500,7 @@ __global__ void __launch_bounds__(MAXT, 1) k_plan_batch(const PlanArgs a) {
         cl_sync_all(C);
         {
             S4 pre = carryB, all = carryB;
-            if (C > 1) { for (unsigned r = 0; r < C; ++r) { if (r < rank) pre = s4_comb(pre, sh.xtB[r]); all = s4_comb(all, sh.xtB[r]); } }
+            if constexpr (CL) { for (unsigned r = 0; r < C; ++r) { if (r < rank) pre = s4_comb(pre, sh.xtB[r]); all = s4_comb(all, sh.xtB[r]); } }
             else all = s4_comb(all, tot);
             inc2 = s4_comb(pre, inc2);
             carryB = all;
