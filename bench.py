@@ -1275,7 +1275,11 @@ def run_cuda(args):
                     "frac": b / s / 1e9 / peak, "peak_source": peak_src, "share_of_copy_time": s / copy_s,
                     "algorithmic_bytes_per_launch": b // nl, "avg_launch_us": s / nl * 1e6,
                     "traffic": (tr // nl) if tr_ok and not inp.small else None,
-                    "traffic_source": "profiles/%s (ncu --set full capture; launch-weighted mean over the kernel's segments)" % TRAFFIC_CSV}
+                    "traffic_source": "profiles/%s (ncu --set full capture; launch-weighted mean over the kernel's segments)" % TRAFFIC_CSV,
+                    "note": "k_batch_exec runs the Zipf put batch (HBM-bound: 392 MB per launch) and the 50 halo rounds, whose "
+                            "faces and ghost layers (72 MiB) stay in the 126 MB L2 between rounds: DRAM traffic is about half the "
+                            "algorithmic bytes, and the halo rounds are bound by launch + completion latency and the SMs' own L2 "
+                            "ports (profiles/r02b_halo_graph.md), which is why `achieved` can approach the HBM copy peak"}
 
     line = base_line(args, world)
     if one_gpu:
