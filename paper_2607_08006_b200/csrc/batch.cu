@@ -724,9 +724,10 @@ int shmemg_exec_smem_attr(shmemg_world *w) {
     return SHMEMG_OK;
 }
 
-// Launch the executor.  after_planner: the previous kernel of the stream is the device planner, which releases its
-// dependents early (griddepcontrol.launch_dependents); with programmatic stream serialization the executor's CTAs are set up
-// while the planner still runs and block in griddepcontrol.wait until it has finished.
+// Launch the executor, always as a programmatic dependent of the kernel before it (programmatic stream serialization): when
+// that kernel releases its dependents early (the device planner and every executor do, at entry), the executor's CTAs are set
+// up while it still runs and block in griddepcontrol.wait until it has finished and its writes are visible; behind an ordinary
+// kernel nothing changes.  after_planner only documents the call site (one-call form).
 int shmemg_exec_launch(shmemg_world *w, const ExecArgs &a, unsigned grid, size_t smem, cudaStream_t st, bool after_planner) {
     int rc = shmemg_exec_smem_attr(w);
     if (rc) return rc;
