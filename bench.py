@@ -897,6 +897,37 @@ class CudaBench:
         return ok
 
     # ---- ceilings measured in the same run ---------------------------------------------------------------------------
+    def back_to_back(self, nrep=4, reps=3):
+        """The single-launch copy-class segments once more, each as a CUDA graph of `nrep` back-to-back launches inside ONE
+        event pair (every launch streams 0.4 - 1 GB, far more than the 126 MB L2, so nothing is reused between launches):
+        microseconds per launch without the 6 us an event pair adds around a single launch.  Reported beside the per-launch
+        event-pair figures, not part of `value`."""
+        torch, inp, g, calls = self.torch, self.inp, self.inp.groups, {}
+        if "c3a" in g:
+            calls["alltoall"] = lambda: self.w3a.alltoall(self.a_dst, self.a_src, inp.c3a_blk)
+        if "c3b" in g:
+            calls["put_batch_skewed"] = lambda: self.w3b.enqueue_batch(self.b3b)
+        if "c5" in g:
+            n = inp.c5_bytes
+            calls["sum_reduce_f32"] = lambda: self.w5.sum_reduce(0, self.d5, self.s_f32, n // 4)
+            calls["sum_reduce_i64"] = lambda: self.w5.sum_reduce(1, self.d5, self.s_i64, n // 8)
+            calls["fcollect"] = lambda: self.w5.fcollect(self.d5, self.s_fc, inp.c5_fc_bytes)
+        out = {}
+        for name, fn in calls.items():
+            fn()
+            torch.cuda.synchronize()
+            gr = torch.cuda.CUDAGraph()
+            with torch.cuda.graph(gr, capture_error_mode="thread_local"):
+                for _ in range(nrep):
+                    fn()
+            ts = []
+            for _ in range(reps + 1):
+                a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                a.record(); gr.replay(); b.record(); b.synchronize()
+                ts.append(a.elapsed_time(b) * 1e3 / nrep)
+            out[name] = statistics.mean(ts[1:])
+        return out
+
     def ceilings(self, reps=5):
         """L2-atomic ceilings (bare red / atom / cas at hashed addresses, include/shmemg_probe.h) on the C1 and C4
         footprints, and the library's own plain-copy rate on the C5 world.  Returns Mops/s and GB/s (best of reps)."""
@@ -1189,6 +1220,7 @@ def run_cuda(args):
                 e2e_ms["__pipelined_" + cls] = sum(r[cls][0].elapsed_time(r[cls][1]) for r in regions)
         e2e_check = cb.e2e_check()
     ceil = cb.ceilings() if rank == 0 else {}
+    b2b = cb.back_to_back() if rank == 0 else {}
 
     # ---- max over ranks of every segment time ---------------------------------------------------------------------------
     names, seg_ms, whole_ms, e2e_ms = max_over_ranks(dist, device, seg_ms, whole_ms, e2e_ms)
@@ -1228,6 +1260,10 @@ def run_cuda(args):
         else:
             d["us_per_barrier"] = seg_ms[k] / K / t["ops"] * 1e3
         d["us_per_launch"] = per_launch_ms * 1e3
+        if k in b2b:                                              # the same launch back to back from a CUDA graph (rank 0)
+            d["back_to_back_us_per_launch"] = b2b[k]
+            d["back_to_back_GBps"] = t["bytes"] / t["launches"] / b2b[k] / 1e3
+            d["back_to_back_frac_of_measured_hbm"] = d["back_to_back_GBps"] / peak
         if k in cb.plan_us:
             d["host_planning"] = dict(cb.plan_us[k], note="shmemg_batch_plan_bytes + shmemg_batch_create per batch (host pass, H2D, "
                                       "stream sync); done once before the timed region, the plan is re-enqueued every step "
