@@ -207,13 +207,13 @@ __global__ void __launch_bounds__(256) k_cas_test(const AmoArgs a) {
 // A skewed op stream (C4: RMAT) is bound by same-line serialisation at the L2 atomic unit: the hottest 128-byte line takes
 // 0.71 % of the 2^26 ops and its ops alone last as long as the whole kernel (2.7 ns each), while the atomic units idle
 // (profiles/r01d).  Removing the 256 hottest words from the stream brings the plain kernel from 1339 to 721 us.  So:
-//   k_hot_sample     HOT_SAMPLES ops of the stream are fetched by 16 CTAs; the last one to finish counts them in a shared-memory
-//                    hash table and publishes the words seen at least HOT_THRESHOLD times (at most SHMEMG_HOT_MAX) in the
-//                    control region (about 40 us);
+//   k_hot_sample     HOT_SAMPLES ops of the stream are fetched by 16 co-resident CTAs; each of them then counts the keys of its
+//                    sixteenth of a hash table in shared memory and publishes the words seen at least HOT_THRESHOLD times
+//                    (at most SHMEMG_HOT_MAX) in the control region (13 us);
 //   k_amo_hot_main   k_amo's loop with a two-load shared-memory lookup per op.  Cold ops go straight to L2.  The hot ops of a
 //                    CTA are combined: ONE L2 atomic per hot word and CTA (count * val); a hot fetch-add receives
 //                    old + rank * val, its rank taken from the word's shared-memory counter.
-// Measured on C4 (2^26 fetch-adds, RMAT): 1340 -> 890 us.  What did NOT work on the way (profiles/r01d): a hash table over ALL
+// Measured on C4 (2^26 fetch-adds, RMAT): 1340 -> 850 us (profiles/r02b_fetch_add.md).  What did NOT work on the way (profiles/r01d): a hash table over ALL
 // ops of a chunk (2000 us: barriers behind probe loops); contiguous chunks with per-thread hot bitmasks (1090-1530 us: 38-55
 // registers cut the number of L2 atomics in flight, which is what this kernel lives on); a separate fix-up kernel re-reading
 // the operands of the hot ops (430 us of 32-byte-sector traffic).
