@@ -105,6 +105,7 @@ SHMEMG_API int shmemg_finalize(shmemg_world_t *w);
 SHMEMG_API int shmemg_n_pes(const shmemg_world_t *w);
 SHMEMG_API size_t shmemg_heap_bytes(const shmemg_world_t *w);    /* usable bytes per PE           */
 SHMEMG_API size_t shmemg_heap_stride(const shmemg_world_t *w);   /* distance between PE windows   */
+/* Text of the last SHMEMG_ERR_CUDA on this world; also the reason when shmemg_atomic_fetch_add_batch_static_on_stream refuses a call. */
 SHMEMG_API const char *shmemg_last_cuda_error(const shmemg_world_t *w);
 
 /* Capability discovery ("shmem_query_capabilities", section 6.5).  `team` is one of the
@@ -308,6 +309,39 @@ SHMEMG_API int shmemg_atomic_compare_swap_batch_on_stream(shmemg_world_t *w, uin
                                                           uint64_t cond_scalar, const uint64_t *val,
                                                           uint64_t val_scalar, uint64_t *fetched_out, size_t n,
                                                           uint32_t flags, void *stream);
+
+/* ---- fetch-add for callers that cannot allocate device memory ------------------------------------------------------------
+ * The fast fetch-add on skewed streams (SHMEMG_AMO_HOT_AGGREGATE above) needs device scratch, and everywhere else in this
+ * library the caller provides it (shmemg_set_scratch).  Some callers have no way to get any: a plug-in or callback that a host
+ * runtime hands a stream, the slab and its input / output pointers but not its allocator; a process that gave all of the
+ * GPU's memory to one pool at start-up, so that a later cudaMalloc fails; a caller inside a latency-critical stream pipeline,
+ * where cudaMalloc / cudaFree would synchronise the whole device.  This entry point is for them.  It computes exactly what
+ *     shmemg_atomic_fetch_add_batch_on_stream(w, sym_off, tgt_pe, elem_idx, idx_bytes, NULL, val_scalar, fetched_out, n,
+ *                                             flags | SHMEMG_AMO_HOT_AGGREGATE, stream)
+ * computes (same kernels, same result contract: per word the fetched values are the prefix sums of some order of the
+ * word's ops, the final words are exact), but the scratch of the hot-set kernels is an array that is part of the library
+ * image: SHMEMG_STATIC_SCRATCH_BYTES of device memory on EVERY GPU on which this library is loaded, held until the process
+ * exits, whether or not this call is ever made.  The call itself calls no cudaMalloc / cudaFree and no allocating library
+ * routine; inputs (tgt_pe, elem_idx) and the output (fetched_out) are still the caller's DEVICE arrays of n entries.
+ *   Limit: n <= SHMEMG_STATIC_MAX_OPS.  A larger n is refused with SHMEMG_ERR_NOMEM before anything is launched, and
+ *     shmemg_last_cuda_error(w) then holds a sentence naming n and the limit (split the batch, or use shmemg_set_scratch).
+ *   flags: SHMEMG_AMO_THEN_BARRIER and SHMEMG_AMO_HOT_AGGREGATE (implied) only; any other bit is SHMEMG_ERR_ARG.
+ *   The world's device must be the CURRENT device of the calling thread (SHMEMG_ERR_ARG otherwise).
+ *   First call per device: it looks the array's device address up (cudaGetSymbolAddress, once per device, remembered for
+ *     the life of the process).  Make that first call during set-up, before any stream capture is begun.
+ *   Sharing: there is ONE array per GPU, shared by every call on every world of that GPU, and it keeps whatever the
+ *     previous call left in it.  Nothing in it has to start at zero (each call writes every scratch word before it reads it,
+ *     so no clearing pass runs), but two calls that can overlap in time on the GPU -- different streams, different worlds,
+ *     different host threads -- corrupt each other's hot-op lists: keep all calls on a device stream-ordered.
+ *   When the hot-set kernels do not apply (n < 2^20, a slab of 2^32 or more 64-bit words, or the 16 sampling CTAs cannot be
+ *     made co-resident) the plain fetch-add kernel runs instead; it needs no scratch at all.  *path_out (HOST, may be NULL)
+ *     says which one ran: 1 = hot-set kernels on the built-in scratch, 0 = plain kernel. */
+#define SHMEMG_STATIC_SCRATCH_BYTES (8u << 20)
+#define SHMEMG_STATIC_MAX_OPS ((size_t)1 << 22)
+SHMEMG_API int shmemg_atomic_fetch_add_batch_static_on_stream(shmemg_world_t *w, uint64_t sym_off, const int32_t *tgt_pe,
+                                                              const void *elem_idx, int idx_bytes, uint64_t val_scalar,
+                                                              uint64_t *fetched_out, size_t n, uint32_t flags,
+                                                              void *stream, int *path_out);
 
 /* Generic AMO batch on `width`-byte words (4 or 8), structure-of-arrays like the calls above (the AMO set of OpenSHMEM 1.6,
  * inherited unchanged): word = heap[tgt_pe[i]][sym_off + width*elem_idx[i]]; old = word; word = f(old, val[i]);

@@ -82,6 +82,7 @@ class DEVCOLL:
 AMO_WARP_AGGREGATE = 1
 AMO_TEST_BEFORE_SWAP = 2
 AMO_HOT_AGGREGATE = 4
+STATIC_MAX_OPS = 1 << 22                 # SHMEMG_STATIC_MAX_OPS
 AMO_THEN_BARRIER = 8
 NO_STAMP = (1 << 64) - 1
 
@@ -148,6 +149,7 @@ SYMBOLS = {
     "shmemg_set_scratch": (_i, [_vp, _vp, _sz]),
     "shmemg_atomic_add_batch_on_stream": (_i, [_vp, _u64, _vp, _vp, _i, _vp, _u64, _sz, _u32, _vp]),
     "shmemg_atomic_fetch_add_batch_on_stream": (_i, [_vp, _u64, _vp, _vp, _i, _vp, _u64, _vp, _sz, _u32, _vp]),
+    "shmemg_atomic_fetch_add_batch_static_on_stream": (_i, [_vp, _u64, _vp, _vp, _i, _u64, _vp, _sz, _u32, _vp, C.POINTER(_i)]),
     "shmemg_atomic_compare_swap_batch_on_stream": (_i, [_vp, _u64, _vp, _vp, _i, _vp, _u64, _vp, _u64, _vp, _sz, _u32, _vp]),
     "shmemg_sum_reduce_on_stream": (_i, [_vp, _i, _u64, _u64, _sz, _vp]),
     "shmemg_reduce_on_stream": (_i, [_vp, _i, _i, _u64, _u64, _sz, _vp]),
@@ -500,6 +502,22 @@ class World:
                   "shmemg_atomic_fetch_add_batch_on_stream")
         # launch accounting: SHMEMG_AMO_HOT_AGGREGATE runs a sampling kernel in front of the main one (n >= 2^20, scalar value)
         self.launches += (2 if self._hot(flags, val, n) else 1) if n or (flags & AMO_THEN_BARRIER) else 0
+
+    def atomic_fetch_add_batch_static(self, sym_off, tgt_pe, elem_idx, fetched_out, val_scalar=1, flags=0, stream=None) -> int:
+        """Fetch-add with one scalar value for a caller that has no device allocator to draw scratch from (a plug-in given only
+        its input / output pointers, a process whose GPU memory is all committed to a pool, a pipeline that cannot afford
+        cudaMalloc's device-wide synchronisation): the scratch is a fixed array inside the library, nothing is allocated.  At most
+        STATIC_MAX_OPS ops per call (ShmemgError NOMEM with the reason beyond that); calls on one GPU must not overlap, they
+        share the array.  Returns 1 when the hot-set kernels ran on the built-in scratch, 0 when the plain kernel ran."""
+        n = tgt_pe.numel()
+        path = C.c_int(0)
+        rc = lib().shmemg_atomic_fetch_add_batch_static_on_stream(self.h, sym_off, _dptr(tgt_pe), _dptr(elem_idx),
+                                                                  self._idx_bytes(elem_idx), val_scalar & NO_STAMP,
+                                                                  _dptr(fetched_out), n, flags, _stream(stream), C.byref(path))
+        if rc:
+            raise ShmemgError(rc, "shmemg_atomic_fetch_add_batch_static_on_stream", lib().shmemg_last_cuda_error(self.h).decode())
+        self.launches += (1 + path.value) if n or (flags & AMO_THEN_BARRIER) else 0
+        return path.value
 
     def atomic_compare_swap_batch(self, sym_off, tgt_pe, elem_idx, fetched_out, cond=None, cond_scalar=0, val=None,
                                   val_scalar=0, flags=0, stream=None):

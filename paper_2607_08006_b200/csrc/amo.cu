@@ -558,3 +558,96 @@ extern "C" int shmemg_set_scratch(shmemg_world_t *w, void *scratch_dev, size_t b
     w->scratch_bytes = scratch_dev ? bytes : 0;
     return SHMEMG_OK;
 }
+
+// ---- fetch-add on the library's built-in scratch (shmemg_atomic_fetch_add_batch_static_on_stream) ---------------------------
+// For callers that cannot obtain device memory themselves (see include/shmemg.h): the staged sample keys and the per-CTA
+// hot-op lists of k_hot_sample / k_amo_hot_main live in this file-scope device array instead of a caller-owned buffer.  The
+// array is part of the module image: every GPU that loads libshmemg.so holds these 8 MiB until the process exits.
+//
+// g_static_scratch is a DEVICE symbol.  Host code must never hand the name itself to a kernel: on the host it stands for a
+// shadow object in host memory, so a kernel given `g_static_scratch` faults (or, on a system where the GPU can read host
+// memory, quietly works on the wrong bytes).  static_scratch_ptr() asks the runtime for the real device address, once per
+// device and with that device current, and the launch below passes THAT pointer.
+#include <mutex>
+
+static __device__ __align__(256) unsigned char g_static_scratch[SHMEMG_STATIC_SCRATCH_BYTES];
+
+#define STATIC_MAX_DEVICES 64
+static std::mutex g_static_mu;
+static unsigned char *g_static_ptr[STATIC_MAX_DEVICES];      // device address of g_static_scratch on device d (0: not asked yet)
+
+static int static_scratch_ptr(shmemg_world *w, unsigned char **out) {
+    int cur = -1;
+    SHMEMG_CUDA(w, cudaGetDevice(&cur));
+    if (cur != w->device || cur < 0 || cur >= STATIC_MAX_DEVICES) {
+        w->last_cuda_error = "shmemg_atomic_fetch_add_batch_static_on_stream: the world lives on device " + std::to_string(w->device) +
+                             " but device " + std::to_string(cur) + " is current (the built-in scratch is looked up per device)";
+        return SHMEMG_ERR_ARG;
+    }
+    std::lock_guard<std::mutex> lock(g_static_mu);
+    if (!g_static_ptr[cur]) {
+        void *p = nullptr;
+        const cudaError_t e = cudaGetSymbolAddress(&p, g_static_scratch);
+        if (e != cudaSuccess || !p) return shmemg_cuda_fail(w, e, "cudaGetSymbolAddress(g_static_scratch)");
+        g_static_ptr[cur] = (unsigned char *)p;
+    }
+    *out = g_static_ptr[cur];
+    return SHMEMG_OK;
+}
+
+extern "C" int shmemg_atomic_fetch_add_batch_static_on_stream(shmemg_world_t *w, uint64_t sym_off, const int32_t *tgt_pe,
+                                                              const void *elem_idx, int idx_bytes, uint64_t val_scalar,
+                                                              uint64_t *fetched_out, size_t n, uint32_t flags, void *stream,
+                                                              int *path_out) {
+    if (path_out) *path_out = 0;
+    int rc = check_common(w, sym_off, tgt_pe, elem_idx, idx_bytes, n);
+    if (rc) return rc;
+    if (n && !fetched_out) return SHMEMG_ERR_ARG;
+    if (flags & ~(SHMEMG_AMO_THEN_BARRIER | SHMEMG_AMO_HOT_AGGREGATE)) return SHMEMG_ERR_ARG;
+    if (n > SHMEMG_STATIC_MAX_OPS) {
+        w->last_cuda_error = "shmemg_atomic_fetch_add_batch_static_on_stream: n = " + std::to_string(n) + " ops is more than SHMEMG_STATIC_MAX_OPS = " +
+                             std::to_string((size_t)SHMEMG_STATIC_MAX_OPS) + " (the built-in scratch is " +
+                             std::to_string((size_t)SHMEMG_STATIC_SCRATCH_BYTES) + " bytes); split the batch or register a buffer with shmemg_set_scratch";
+        return SHMEMG_ERR_NOMEM;
+    }
+    cudaStream_t st = (cudaStream_t)stream;
+    AmoArgs a{w->base, w->stride, sym_off, tgt_pe, elem_idx, nullptr, val_scalar, nullptr, 0, (unsigned long long *)fetched_out, n,
+              (flags & SHMEMG_AMO_THEN_BARRIER) ? w->ctl : nullptr};
+    if (!hot_agg_ok(w, a, SHMEMG_AMO_HOT_AGGREGATE))                        // small call or huge slab: the plain kernel needs no scratch
+        return launch_amo<AMO_FADD>(w, a, idx_bytes, 0, st);
+    unsigned char *scratch = nullptr;
+    rc = static_scratch_ptr(w, &scratch);
+    if (rc) return rc;
+    // the geometry of launch_amo_hot: 8 waves of resident CTAs, every CTA may list up to 1/8 of its ops (+32) as hot
+    int per_sm = 0;
+    if (idx_bytes == 4) cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_amo_hot_main<4, AMO_FADD>, 256, 0);
+    else cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_amo_hot_main<8, AMO_FADD>, 256, 0);
+    if (per_sm < 1) per_sm = 1;
+    const size_t blocks = (size_t)w->sm_count * per_sm * 8;
+    const unsigned cap = (unsigned)((n + blocks - 1) / blocks / 8 + 32);    // n <= 2^22: far below the 21-bit rank field
+    const size_t need = (size_t)HOT_SAMPLES * 4 + blocks * (size_t)cap * 8;
+    if (need > SHMEMG_STATIC_SCRATCH_BYTES) {                               // a GPU with far more SMs than the B200 this was sized for
+        w->last_cuda_error = "shmemg_atomic_fetch_add_batch_static_on_stream: " + std::to_string(n) + " ops need " + std::to_string(need) +
+                             " bytes of scratch on this GPU, the built-in scratch is " + std::to_string((size_t)SHMEMG_STATIC_SCRATCH_BYTES);
+        return SHMEMG_ERR_NOMEM;
+    }
+    // Nothing to clear: k_hot_sample writes all HOT_SAMPLES staged keys before any CTA reads one, and k_amo_hot_main reads only
+    // the list records it wrote itself in this launch (their count lives in shared memory), so what the last call left is never read.
+    unsigned *staged = (unsigned *)scratch;
+    unsigned long long *lists = (unsigned long long *)(scratch + (size_t)HOT_SAMPLES * 4);
+    {
+        AmoArgs aa = a;
+        CtlRegion *ctl = w->ctl;
+        void *args[] = {&aa, &ctl, &staged};
+        const void *fn = idx_bytes == 4 ? (const void *)k_hot_sample<4> : (const void *)k_hot_sample<8>;
+        if (cudaLaunchCooperativeKernel(fn, dim3(HOT_SAMPLES / 1024), dim3(1024), args, 0, st) != cudaSuccess) {
+            cudaGetLastError();                                             // the sampling CTAs cannot be co-resident here
+            return launch_amo<AMO_FADD>(w, a, idx_bytes, 0, st);
+        }
+    }
+    if (idx_bytes == 4) k_amo_hot_main<4, AMO_FADD><<<(unsigned)blocks, 256, 0, st>>>(a, w->ctl, lists, cap);
+    else k_amo_hot_main<8, AMO_FADD><<<(unsigned)blocks, 256, 0, st>>>(a, w->ctl, lists, cap);
+    SHMEMG_CUDA(w, cudaGetLastError());
+    if (path_out) *path_out = 1;
+    return SHMEMG_OK;
+}
