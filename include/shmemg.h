@@ -58,7 +58,7 @@ enum {
     SHMEMG_ERR_NOMEM = -5,    /* symmetric heap exhausted / slab or plan buffer too small     */
     SHMEMG_ERR_CUDA = -6,     /* a CUDA runtime call failed (see shmemg_last_cuda_error)       */
     SHMEMG_ERR_OVERLAP = -7,  /* collective source/dest ranges partially overlap              */
-    SHMEMG_ERR_NODEVICE = -8  /* no sm_100 device / wrong architecture                        */
+    SHMEMG_ERR_NODEVICE = -8  /* no sm_100 device / wrong architecture / peer GPU unreachable  */
 };
 
 /* ---- teams and contexts: constants only in this build ------------------ */
@@ -560,7 +560,11 @@ SHMEMG_API int shmemg_device_exec_ops_on_stream(shmemg_world_t *w, const shmemg_
  * The shards see each other's slabs through peer mappings: shmemg_shard_export gives a CUDA IPC handle of this world's slab
  * (64 bytes, HOST) plus the slab's byte offset inside the exported allocation; the caller carries both to the other processes
  * (any transport: the tests use torch.distributed/gloo) and gives them to shmemg_shard_attach_ipc there.  Shards that live in
- * ONE process (peer access enabled by the caller) pass the slab pointer itself to shmemg_shard_attach_ptr.
+ * ONE process pass the slab pointer itself to shmemg_shard_attach_ptr.  Both attach calls check that the peer slab is device
+ * memory this world's GPU can reach: a slab on another GPU needs peer access (enabled here if it is not yet) over a link with
+ * native atomics, since signals, the shard barrier and AMO batches update peer words with system-scope atomics; otherwise
+ * SHMEMG_ERR_NODEVICE (reason in shmemg_last_cuda_error) and nothing is attached.  Status: this layer has been parity-tested
+ * with all shards on ONE GPU only (in one process and as two processes over CUDA IPC); it has not yet run across NVLink.
  * The g-calls take GLOBAL PE numbers; the initiator must be a local PE of this shard.  Transfers are peer loads / stores issued
  * by this shard's kernels; AMOs and signal updates on a remote shard are SYSTEM-scope atomics (the atomicity domain of a
  * sharded world is the fabric, not one GPU's L2); ordering between shards comes from shmemg_gbarrier_all_on_stream or from

@@ -247,6 +247,39 @@ extern "C" int shmemg_shard_export(shmemg_world_t *w, void *ipc_handle64_out, ui
     return SHMEMG_OK;
 }
 
+// A peer slab must be device memory that THIS world's GPU can load, store and -- because signals, the shard barrier and the AMO
+// batches use red / atom at system scope -- atomically update.  A slab on the world's own GPU passes at once; for one on another
+// GPU peer access is required (and enabled here) and the link must support native atomics (NVLink does; PCIe P2P does not).
+// Without this check the first g-call to an unreachable slab is an illegal-address fault, and atomics over a link without
+// native support silently lose their atomicity.
+static int peer_reachable(shmemg_world *w, const void *p) {
+    cudaPointerAttributes at;
+    SHMEMG_CUDA(w, cudaPointerGetAttributes(&at, p));
+    if (at.type != cudaMemoryTypeDevice) {
+        w->last_cuda_error = "shard attach: the peer slab is not device memory";
+        return SHMEMG_ERR_ARG;
+    }
+    if (at.device == w->device) return SHMEMG_OK;
+    int cur = -1;
+    SHMEMG_CUDA(w, cudaGetDevice(&cur));
+    if (cur != w->device) SHMEMG_CUDA(w, cudaSetDevice(w->device));
+    int rc = SHMEMG_OK, can = 0, native_atomics = 0;
+    cudaError_t e = cudaDeviceCanAccessPeer(&can, w->device, at.device);
+    if (e == cudaSuccess && can) {
+        e = cudaDeviceEnablePeerAccess(at.device, 0);
+        if (e == cudaErrorPeerAccessAlreadyEnabled) { cudaGetLastError(); e = cudaSuccess; }
+    }
+    if (e == cudaSuccess && can) e = cudaDeviceGetP2PAttribute(&native_atomics, cudaDevP2PAttrNativeAtomicSupported, w->device, at.device);
+    if (e != cudaSuccess) rc = shmemg_cuda_fail(w, e, "shard attach: peer access");
+    else if (!can || !native_atomics) {
+        w->last_cuda_error = "shard attach: device " + std::to_string(w->device) + (can ? " has no native atomics on" : " cannot access") +
+                             " the memory of device " + std::to_string(at.device);
+        rc = SHMEMG_ERR_NODEVICE;
+    }
+    if (cur != w->device) cudaSetDevice(cur);
+    return rc;
+}
+
 extern "C" int shmemg_shard_attach_ipc(shmemg_world_t *w, int shard, const void *ipc_handle64, uint64_t offset) {
     if (!w || !w->nshards || !ipc_handle64 || shard < 0 || shard >= w->nshards || shard == w->shard) return SHMEMG_ERR_ARG;
     if (w->peer_base[shard]) return SHMEMG_ERR_ARG;
@@ -254,6 +287,8 @@ extern "C" int shmemg_shard_attach_ipc(shmemg_world_t *w, int shard, const void 
     memcpy(&h, ipc_handle64, 64);
     void *p = nullptr;
     SHMEMG_CUDA(w, cudaIpcOpenMemHandle(&p, h, cudaIpcMemLazyEnablePeerAccess));
+    const int rc = peer_reachable(w, p);
+    if (rc) { cudaIpcCloseMemHandle(p); return rc; }
     w->peer_ipc[shard] = p;
     w->peer_base[shard] = (uint8_t *)p + offset;
     return SHMEMG_OK;
@@ -262,6 +297,8 @@ extern "C" int shmemg_shard_attach_ipc(shmemg_world_t *w, int shard, const void 
 extern "C" int shmemg_shard_attach_ptr(shmemg_world_t *w, int shard, void *peer_slab_dev) {
     if (!w || !w->nshards || !peer_slab_dev || shard < 0 || shard >= w->nshards || shard == w->shard) return SHMEMG_ERR_ARG;
     if (w->peer_base[shard]) return SHMEMG_ERR_ARG;
+    const int rc = peer_reachable(w, peer_slab_dev);
+    if (rc) return rc;
     w->peer_base[shard] = (uint8_t *)peer_slab_dev;
     return SHMEMG_OK;
 }

@@ -97,6 +97,13 @@ def test_shard_argument_checks():
     assert e.value.code == ERR.ARG
     w2 = World(2, 1 << 16, sc.DEV)
     w2.shard_init(2, 1)
+    from paper_2607_08006_b200.binding import lib
+    host = torch.empty(1 << 20, dtype=torch.uint8).pin_memory()
+    assert lib().shmemg_shard_attach_ptr(w.h, 1, host.data_ptr()) == ERR.ARG      # a peer slab must be DEVICE memory this GPU can reach
+    assert b"not device memory" in lib().shmemg_last_cuda_error(w.h)
+    with pytest.raises(ShmemgError) as e:
+        w.gput(0, 256, 16, 0, 1)                      # the refused attach left shard 1 unattached
+    assert e.value.code == ERR.ARG
     w.shard_attach_world(1, w2)
     with pytest.raises(ShmemgError) as e:
         w.gput(0, 256, 16, 1, 0)                      # global PE 1 lives on shard 1: not a local initiator
