@@ -198,6 +198,11 @@ typedef struct shmemg_op {
  *     strong reading of L377, always conformant.  A wait also orders the PE's later ops after it.
  *     "Of this PE" means: of the same (PE, ctx) pair -- contexts are independent ordering domains (L124-L130); a QUIET on
  *     context 1 does not wait for the PE's traffic on context 0.  BARRIER_ALL covers every context of every PE.
+ *     This holds for SIGNAL_WAIT_UNTIL too, and there a batch is WEAKER than the device-initiated paths: a wait with ctx = c
+ *     holds back only the later ops of (PE, c), whereas in shmemg_device_exec_ops(_ctx)_on_stream and for shmemg_dev_* calls
+ *     the wait blocks the PE's whole agent, the way OpenSHMEM's shmem_wait_until blocks the calling PE.  An op list that waits
+ *     on context c and then forwards the received data on another context c' is therefore ordered when device-initiated but
+ *     not in a batch; portable lists repeat the wait (same word, same comparison) on c', or issue the dependent op on c.
  *   - PUT_SIGNAL: the signal update is atomic w.r.t. other signal updates and waits, and becomes visible
  *     only after the whole payload (release/acquire at GPU scope).
  *   - atomicity does not imply ordering.

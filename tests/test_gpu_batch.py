@@ -120,6 +120,15 @@ TINY = {
     "ctx_fadd_cas_wait": ([[("fadd", 1, 0, 2, 1, "@3"), ("cas", 1, 2, M64, 9, 3, "@3"), ("quiet", "@3"), ("add", 1, 4, 1, "@3")],
                            [("wait", 4, "ge", 1, "@1"), ("fadd", 1, 0, 5, 1, "@1"), ("cas", 1, 2, M64, 8, 3, "@1")]],
                           [[0, 0, 0, 0, 0], [0, 0, M64, 0, 0]], [0, 0, 0, 0, 1, 1, 1]),
+    # a wait on context 0 followed by a put of the received word on context 1 (shmemg.h "Batch semantics": in a batch the wait
+    # orders only its own context, so the forward may carry the old word; the device-initiated interpreter blocks the whole PE)
+    "ctx_wait_then_forward_on_other_ctx": ([[("put", 1, 0, 2), ("fence",), ("put", 1, 1, 3)],
+                                            [("wait", 1, "eq", 1, "@0"), ("put", 0, 4, 0, "@1")]],
+                                           [[0, 0, 42, 1, 0], [0] * 5], [0, 0, 0, 1, 1]),
+    # ... and the portable form: a wait on the forwarding context too
+    "ctx_wait_on_both_then_forward": ([[("put", 1, 0, 2), ("fence",), ("put", 1, 1, 3)],
+                                       [("wait", 1, "eq", 1, "@0"), ("wait", 1, "eq", 1, "@1"), ("put", 0, 4, 0, "@1")]],
+                                      [[0, 0, 42, 1, 0], [0] * 5], [0, 0, 0, 1, 1, 1]),
     "add_fence_add": ([[("add", 1, 0, 7), ("fence",), ("add", 1, 1, 1)], [("wait", 1, "ge", 1), ("get", 1, 4, 0)]],
                       [[0] * 5, [0] * 5], [0, 0, 0, 1, 1]),
 }

@@ -262,6 +262,19 @@ def test_tiny_programs_with_explicit_contexts_land_in_enumerated_outcome_set(nam
         assert got in allowed, (name, got)
 
 
+def test_wait_blocks_the_whole_pe_agent_in_the_device_interpreter():
+    """Where the two execution paths differ (shmemg.h "Batch semantics"): in k_device_exec_ops_ctx a SIGNAL_WAIT_UNTIL blocks the
+    PE's agent, as OpenSHMEM's shmem_wait_until blocks the calling PE, so an op of ANOTHER context behind the wait always sees
+    the awaited data; the batch executor orders only the wait's own context (both outcomes are in the model's set, and the
+    batch executor's result is checked against that set in test_tiny_programs_land_in_enumerated_outcome_set)."""
+    prog, init, order = TINY["ctx_wait_then_forward_on_other_ctx"]
+    assert {h[0][4] for h in enumerate_outcomes(prog, init)} == {0, 42}
+    sp = to_spec_program(prog, init, order)
+    for _ in range(5):
+        w, ld = run_gpu_device_ctx(sp)
+        assert int(ld.obj_numpy("w", np.uint64)[0][4]) == 42
+
+
 def test_quiet_on_one_context_leaves_the_other_contexts_operations_pending():
     """PAPER L327 / L331 + reading 31: a context has its own completion counters and lives in device memory across kernels.
     Kernel A (its list is not quieted at the end): PE 0 issues a non-blocking put on context 0, another on context 1, and a

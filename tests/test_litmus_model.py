@@ -189,6 +189,21 @@ def test_contexts_are_independent_ordering_domains():
     assert oracle_heaps(w, init2, [0, 0, 0, 1, 1, 1]) in out
 
 
+def test_wait_orders_only_its_own_context_in_a_batch():
+    """The batch contract of shmemg.h: SIGNAL_WAIT_UNTIL with ctx = c orders the later ops of (PE, c) only.  PE1 waits for the
+    flag on context 0 and forwards the received word to PE0 on context 1: the forward may carry the old word (0) or the new one
+    (42).  With a second wait on the forwarding context only 42 is left.  (The device-initiated interpreter blocks the whole PE
+    at a wait and always produces 42, an element of both sets.)"""
+    init = [[0, 0, 42, 1, 0], [0] * 5]
+    send = [("put", 1, 0, 2), ("fence",), ("put", 1, 1, 3)]
+    weak = enumerate_outcomes([send, [("wait", 1, "eq", 1, "@0"), ("put", 0, 4, 0, "@1")]], init)
+    assert {h[0][4] for h in weak} == {0, 42}
+    both = enumerate_outcomes([send, [("wait", 1, "eq", 1, "@0"), ("wait", 1, "eq", 1, "@1"), ("put", 0, 4, 0, "@1")]], init)
+    assert {h[0][4] for h in both} == {42}
+    same_ctx = enumerate_outcomes([send, [("wait", 1, "eq", 1, "@1"), ("put", 0, 4, 0, "@1")]], init)
+    assert {h[0][4] for h in same_ctx} == {42}
+
+
 def test_barrier_covers_every_context():
     init = [[0, 0, 42, 0, 0], [0, 0, 43, 0, 0]]
     prog = [[("put", 1, 0, 2, "@2"), ("barrier",), ("get", 0, 4, 0, "@1")],
