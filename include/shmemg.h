@@ -225,6 +225,14 @@ SHMEMG_API int shmemg_batch_launches(const shmemg_batch_t *b);
 
 /* Launch the batch executor on `stream` (one persistent-grid kernel; tiles are claimed in batch order). */
 SHMEMG_API int shmemg_batch_enqueue_on_stream(shmemg_world_t *w, shmemg_batch_t *b, void *stream);
+/* Every executor launch (and the device planner of the one-call form) is by default a PROGRAMMATIC DEPENDENT of the kernel
+ * before it on the stream, and every executor releases its own dependents when it starts: the next launch sets its CTAs up on
+ * SMs as they become free and blocks until this one has completed (about 1 us per back-to-back launch).  Results never depend
+ * on it.  Forward progress can: while an executor still polls SIGNAL_WAIT_UNTIL ops that only a kernel on ANOTHER stream (a
+ * device-initiated sender) can satisfy, the parked CTAs of the next launch hold SMs that sender may need to become resident.
+ * A caller that relies on such cross-stream senders turns the feature off for the world (enable = 0: plain stream-ordered
+ * launches).  The environment variable SHMEMG_NO_PDL, read once in shmemg_init, sets the initial state to off. */
+SHMEMG_API int shmemg_set_dependent_launch(shmemg_world_t *w, int enable);
 
 /*
  * ONE-CALL FORM: host-initiated enqueue of a DEVICE-RESIDENT descriptor array ("on

@@ -117,6 +117,7 @@ SYMBOLS = {
     "shmemg_batch_destroy": (_i, [_vp]),
     "shmemg_batch_launches": (_i, [_vp]),
     "shmemg_batch_enqueue_on_stream": (_i, [_vp, _vp, _vp]),
+    "shmemg_set_dependent_launch": (_i, [_vp, _i]),
     "shmemg_batch_work_bytes": (_sz, [_vp, _sz, _u64]),
     "shmemg_enqueue_batch": (_i, [_vp, _vp, _sz, _vp]),
     "shmemg_enqueue_batch_ws": (_i, [_vp, _vp, _sz, _vp, _sz, _vp]),
@@ -467,6 +468,10 @@ class World:
         self._chk(lib().shmemg_device_collective_on_stream(self.h, kind, dtype, dest_off, source_off, n, root, _stream(stream)),
                   "shmemg_device_collective_on_stream")
         self.launches += 1 if n else 0
+
+    def set_dependent_launch(self, enable: bool):
+        """Programmatic dependent launch of the executor / planner kernels (on by default; off = plain stream-ordered launches)."""
+        self._chk(lib().shmemg_set_dependent_launch(self.h, 1 if enable else 0), "shmemg_set_dependent_launch")
 
     # ---- SoA AMO batches -------------------------------------------------------------------------------------------
     def set_scratch_for(self, n: int):

@@ -737,7 +737,7 @@ int shmemg_exec_launch(shmemg_world *w, const ExecArgs &a, unsigned grid, size_t
     at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
     at[0].val.programmaticStreamSerializationAllowed = 1;
     (void)after_planner;
-    cfg.attrs = at; cfg.numAttrs = getenv("SHMEMG_NO_PDL") ? 0 : 1;     // SHMEMG_NO_PDL: experiments
+    cfg.attrs = at; cfg.numAttrs = w->dependent_launch ? 1 : 0;        // shmemg_set_dependent_launch
     SHMEMG_CUDA(w, cudaLaunchKernelEx(&cfg, k_batch_exec, a));
     return SHMEMG_OK;
 }

@@ -54,6 +54,7 @@ struct shmemg_world {
     std::map<uint64_t, size_t> cpu_free_list, cpu_live;
     unsigned sig_seq = 0;
     int ctas_per_sm = 4;                   // copy-class persistent grids: ctas_per_sm * sm_count CTAs
+    bool dependent_launch = true;          // executor / planner launches are programmatic dependents (shmemg_set_dependent_launch)
     size_t tile_bytes_override = 0;        // SHMEMG_TILE_BYTES (experiments; forces the register copy path)
     // dynamic shared memory opt-in (cudaFuncSetAttribute) done on THIS world's device, per kernel family
     bool smem_attr_coll = false, smem_attr_probe = false, smem_attr_plan = false, smem_attr_hot = false;

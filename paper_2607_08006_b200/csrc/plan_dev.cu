@@ -693,7 +693,7 @@ extern "C" int shmemg_enqueue_batch_ws(shmemg_world_t *w, const shmemg_op_t *ops
         at2[0] = at[0];
         at2[1].id = cudaLaunchAttributeProgrammaticStreamSerialization;
         at2[1].val.programmaticStreamSerializationAllowed = 1;
-        cfg.attrs = at2; cfg.numAttrs = getenv("SHMEMG_NO_PDL") ? 1 : 2;
+        cfg.attrs = at2; cfg.numAttrs = w->dependent_launch ? 2 : 1;
         if (C > 1) SHMEMG_CUDA(w, cudaLaunchKernelEx(&cfg, k_plan_batch<true, PLAN_THREADS>, p));
         else if (NT <= 256) SHMEMG_CUDA(w, cudaLaunchKernelEx(&cfg, k_plan_batch<false, 256>, p));
         else SHMEMG_CUDA(w, cudaLaunchKernelEx(&cfg, k_plan_batch<false, PLAN_THREADS>, p));

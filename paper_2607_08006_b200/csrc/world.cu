@@ -71,6 +71,7 @@ extern "C" int shmemg_init(int npes, size_t heap_bytes_per_pe, void *device_slab
         int v = atoi(s);
         if (v >= 1 && v <= 8) w->ctas_per_sm = v;
     }
+    if (getenv("SHMEMG_NO_PDL")) w->dependent_launch = false;       // read once, here; shmemg_set_dependent_launch changes it later
     if (const char *s = getenv("SHMEMG_TILE_BYTES")) {
         long v = atol(s);
         if (v >= 1024) w->tile_bytes_override = (size_t)v;
@@ -273,5 +274,12 @@ extern "C" int shmemg_heap_read_on_stream(shmemg_world_t *w, int pe, void *dst_h
     if (nbytes == 0) return SHMEMG_OK;
     SHMEMG_CUDA(w, cudaMemcpyAsync(dst_host, shmemg_addr(w, pe, src_off), nbytes, cudaMemcpyDeviceToHost,
                                    (cudaStream_t)stream));
+    return SHMEMG_OK;
+}
+
+// Programmatic dependent launch of the batch executor and the device planner (see include/shmemg.h for when to turn it off).
+extern "C" int shmemg_set_dependent_launch(shmemg_world_t *w, int enable) {
+    if (!w) return SHMEMG_ERR_ARG;
+    w->dependent_launch = enable != 0;
     return SHMEMG_OK;
 }

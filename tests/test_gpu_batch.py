@@ -4,7 +4,7 @@ import numpy as np
 import pytest
 import torch
 
-from gpu_common import DEV, assert_objects_equal, heap_bytes_for, run_gpu, run_oracle
+from gpu_common import DEV, assert_objects_equal, heap_bytes_for, ops_to_dev, run_gpu, run_oracle
 from invariants import check_compare_swap_claim, check_fetch_add
 from litmus_model import enumerate_outcomes, to_spec_program
 from paper_2607_08006_b200 import CMP, ERR, OP, OP_DTYPE, ShmemgError, World
@@ -144,6 +144,31 @@ def test_tiny_programs_land_in_enumerated_outcome_set(name):
         w, ld = run_gpu(sp)
         got = tuple(tuple(int(x) for x in row) for row in ld.obj_numpy("w", np.uint64))
         assert got in allowed, (name, got)
+
+
+@pytest.mark.parametrize("onecall", [False, True])
+def test_dependent_launch_can_be_turned_off(onecall):
+    """shmemg_set_dependent_launch(w, 0): plain stream-ordered launches of the executor (and of the device planner in the
+    one-call form).  Same results: a program whose second batch awaits signals raised by the first, back to back on one stream."""
+    prog = litmus.wait_after_wait(npes=4, groups=3, chain=8, nbytes=1 << 16)
+    ow = run_oracle(prog)
+    w = World(prog.npes, heap_bytes_for(prog), DEV)
+    w.set_dependent_launch(False)
+    ld = Loaded(w, prog)
+    ops = ld.translate(prog)
+    half = len(ops) // 2
+    keep = []
+    for part in (ops[:half], ops[half:]):
+        if onecall:
+            od = ops_to_dev(part)
+            w.enqueue_batch_dev(od, len(part), None)
+            keep.append(od)
+        else:
+            keep.append(w.batch(part))
+            w.enqueue_batch(keep[-1])
+    w.quiet(0)
+    assert_objects_equal(prog, ld, ow)
+    w.set_dependent_launch(True)
 
 
 def test_batch_can_be_enqueued_repeatedly_and_stream_order_holds():
