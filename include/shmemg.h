@@ -470,6 +470,14 @@ SHMEMG_API int shmemg_barrier_all_on_stream(shmemg_world_t *w, void *stream);
 SHMEMG_API int shmemg_barrier_all_repeat_on_stream(shmemg_world_t *w, uint32_t count, uint64_t stamp_off,
                                                    void *stream);
 SHMEMG_API uint64_t shmemg_barrier_epoch(shmemg_world_t *w, void *stream);   /* synchronises `stream` */
+/* Recovery.  The in-kernel barriers (shmemg_barrier_all_repeat_on_stream, shmemg_dev_barrier_all_block and the device
+ * collectives built on it) and the sampling kernel of SHMEMG_AMO_HOT_AGGREGATE count arrivals in monotonic counters and find
+ * their round from the count alone, which requires every kernel to finish its rounds.  After one that did not -- an aborted or
+ * timed-out kernel, or a user kernel in which fewer than npes blocks reached a barrier -- every later barrier of the world
+ * would release early, silently.  This call (one tiny kernel on `stream`; nothing of the world may be running concurrently)
+ * rounds those counters up to the next round boundary and clears the last-arriver counters of put_signal / the AMO barrier
+ * fold.  Harmless when nothing was wrong. */
+SHMEMG_API int shmemg_realign_counters_on_stream(shmemg_world_t *w, void *stream);
 
 /* ---- device-initiated path (Tier-1) ---------------------------------------------------
  * include/shmemg_device.cuh holds header-only `__device__` entry points (put/get/put_signal/wait/test/AMOs/fence/quiet

@@ -181,6 +181,7 @@ SYMBOLS = {
     "shmemg_barrier_all_on_stream": (_i, [_vp, _vp]),
     "shmemg_barrier_all_repeat_on_stream": (_i, [_vp, _u32, _u64, _vp]),
     "shmemg_barrier_epoch": (_u64, [_vp, _vp]),
+    "shmemg_realign_counters_on_stream": (_i, [_vp, _vp]),
     "shmemg_device_world_get": (_i, [_vp, _vp]),
     "shmemg_ctx_bytes": (_sz, [_u32]),
     "shmemg_ctx_create": (_i, [_vp, _i, _u32, _vp, _sz, _vp, _vp]),
@@ -750,6 +751,11 @@ class World:
         self._chk(lib().shmemg_barrier_all_repeat_on_stream(self.h, count, stamp_off, _stream(stream)),
                   "shmemg_barrier_all_repeat_on_stream")
         self.launches += 1 if count else 0
+
+    def realign_counters(self, stream=None):
+        """After a kernel that did not finish its barrier rounds: round the monotonic arrival counters up to a round boundary."""
+        self._chk(lib().shmemg_realign_counters_on_stream(self.h, _stream(stream)), "shmemg_realign_counters_on_stream")
+        self.launches += 1
 
     def barrier_epoch(self, stream=None) -> int:
         return lib().shmemg_barrier_epoch(self.h, _stream(stream))

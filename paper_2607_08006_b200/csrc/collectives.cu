@@ -448,6 +448,28 @@ __global__ void __launch_bounds__(32) k_barrier_repeat(CtlRegion *ctl, uint8_t *
     mine[2] += bad;
 }
 
+// Recovery after a kernel that did not finish its rounds (aborted, timed out, or a user kernel in which fewer than npes agents
+// reached a barrier): the monotonic arrival counters find their round from the count alone, so a residue would make every later
+// barrier of the world release early.  Rounds the counters up to the next round boundary and clears the last-arriver counters.
+__global__ void k_realign_counters(CtlRegion *ctl, unsigned npes) {
+    const unsigned t = threadIdx.x;
+    if (t == 0) {
+        const unsigned long long c = ctl->bar_arrivals, r = c % npes;
+        if (r) ctl->bar_arrivals = c + (npes - r);
+        const unsigned h = ctl->hot_done, hr = h % 16u;                  // 16 sampling CTAs per call (2^32 is a multiple of 16)
+        if (hr) ctl->hot_done = h + (16u - hr);
+        ctl->amo_done = 0;
+    }
+    for (unsigned i = t; i < SHMEMG_SIG_SLOTS; i += blockDim.x) ctl->sig_counter[i] = 0;
+}
+
+extern "C" int shmemg_realign_counters_on_stream(shmemg_world_t *w, void *stream) {
+    if (!w) return SHMEMG_ERR_ARG;
+    k_realign_counters<<<1, 256, 0, (cudaStream_t)stream>>>(w->ctl, (unsigned)w->npes);
+    SHMEMG_CUDA(w, cudaGetLastError());
+    return SHMEMG_OK;
+}
+
 // ---------------------------------------------------------------------------------------------------------
 // host entry points
 // ---------------------------------------------------------------------------------------------------------

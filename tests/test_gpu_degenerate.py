@@ -71,3 +71,43 @@ def test_whole_window_transfer_and_single_word_storm():
     w.quiet(0)
     assert w.view(0, 8, torch.int64).cpu().numpy()[0, 0] == 3 * n
     assert np.array_equal(np.sort(f.cpu().numpy()), 3 * np.arange(n, dtype=np.int64))
+
+
+def test_realign_counters_after_short_participation():
+    """A kernel that left its barrier round unfinished (here: three stray arrivals written straight into the control region, as an
+    aborted kernel would leave them) makes the round arithmetic of every later in-kernel barrier wrong.  After
+    shmemg_realign_counters_on_stream the stamped barrier invariant holds again; on an intact world the call changes nothing."""
+    npes = 8
+    w = World(npes, 4096, DEV)
+    st = w.calloc(3, 8)
+    w.barrier_all_repeat(50, st)
+    w.realign_counters()                                     # nothing wrong: no change
+    w.quiet(0)
+    ctl = w.slab[npes * w.stride:].view(torch.int64)         # control region: [0] barrier epoch, [1] in-kernel arrivals
+    assert int(ctl[1]) == 50 * npes
+    ctl[1] += 3                                              # residue of an unfinished round
+    w.realign_counters()
+    w.quiet(0)
+    assert int(ctl[1]) == 51 * npes
+    w.view(st, 24, torch.int64).zero_()
+    w.barrier_all_repeat(1000, st)
+    w.quiet(0)
+    sv = w.view(st, 24, torch.int64).cpu().numpy()
+    assert (sv[:, 2] == 0).all() and int(ctl[1]) == 1051 * npes
+    # the sampling kernel's arrival counter (16 CTAs per call) is realigned the same way
+    n = 1 << 20
+    a = w.calloc(8, 8)
+    z = torch.zeros(n, dtype=torch.int32, device=DEV)
+    f = torch.empty(n, dtype=torch.int64, device=DEV)
+    w.set_scratch_for(n)
+    hot_done = w.slab[npes * w.stride:].view(torch.int32)
+    off = (16 + 48 + 4 * 1024 + 4 * 128 + 4 + 4 + 8 + 4) // 4                # offsetof(CtlRegion, hot_done) / 4
+    w.atomic_fetch_add_batch(a, z, z, f, val_scalar=1, flags=AMO_HOT_AGGREGATE)
+    w.quiet(0)
+    assert int(hot_done[off]) == 16
+    hot_done[off] += 5
+    w.realign_counters()
+    w.atomic_fetch_add_batch(a, z, z, f, val_scalar=1, flags=AMO_HOT_AGGREGATE)
+    w.quiet(0)
+    assert int(hot_done[off]) == 48
+    assert np.array_equal(np.sort(f.cpu().numpy()), np.arange(n, 2 * n))
