@@ -310,6 +310,11 @@ SHMEMG_API int shmemg_quiet(shmemg_world_t *w, int pe, void *stream);
  * stream-ordered.  shmemg_amo_scratch_bytes: what a SHMEMG_AMO_HOT_AGGREGATE call of n ops needs. */
 SHMEMG_API size_t shmemg_amo_scratch_bytes(const shmemg_world_t *w, size_t n);
 SHMEMG_API int shmemg_set_scratch(shmemg_world_t *w, void *scratch_dev, size_t bytes);
+/* Which kernels the world's LAST shmemg_atomic_add_batch_on_stream / shmemg_atomic_fetch_add_batch_on_stream call enqueued:
+ * 1 = the hot-set kernels (SHMEMG_AMO_HOT_AGGREGATE honoured), 0 = the plain kernel (flag absent, or ignored for one of the
+ * reasons listed above, or the sampling CTAs could not be made co-resident).  The result is the same either way; a benchmark
+ * asks so that a number is never attributed to the wrong kernel. */
+SHMEMG_API int shmemg_amo_last_path(const shmemg_world_t *w);
 SHMEMG_API int shmemg_atomic_add_batch_on_stream(shmemg_world_t *w, uint64_t sym_off, const int32_t *tgt_pe,
                                                  const void *elem_idx, int idx_bytes, const uint64_t *val,
                                                  uint64_t val_scalar, size_t n, uint32_t flags, void *stream);

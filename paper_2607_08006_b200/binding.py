@@ -148,6 +148,7 @@ SYMBOLS = {
     "shmemg_quiet": (_i, [_vp, _i, _vp]),
     "shmemg_amo_scratch_bytes": (_sz, [_vp, _sz]),
     "shmemg_set_scratch": (_i, [_vp, _vp, _sz]),
+    "shmemg_amo_last_path": (_i, [_vp]),
     "shmemg_atomic_add_batch_on_stream": (_i, [_vp, _u64, _vp, _vp, _i, _vp, _u64, _sz, _u32, _vp]),
     "shmemg_atomic_fetch_add_batch_on_stream": (_i, [_vp, _u64, _vp, _vp, _i, _vp, _u64, _vp, _sz, _u32, _vp]),
     "shmemg_atomic_fetch_add_batch_static_on_stream": (_i, [_vp, _u64, _vp, _vp, _i, _u64, _vp, _sz, _u32, _vp, C.POINTER(_i)]),
@@ -480,6 +481,10 @@ class World:
         need = lib().shmemg_amo_scratch_bytes(self.h, n)
         self._scratch = torch.empty(need, dtype=torch.uint8, device=self.device)
         self._chk(lib().shmemg_set_scratch(self.h, self._scratch.data_ptr(), need), "shmemg_set_scratch")
+
+    def amo_last_path(self) -> int:
+        """1 if the last add / fetch-add batch call ran the hot-set kernels, 0 if the plain kernel."""
+        return lib().shmemg_amo_last_path(self.h)
 
     def _hot(self, flags, val, n):
         return bool(flags & AMO_HOT_AGGREGATE) and val is None and n >= (1 << 20) and getattr(self, "_scratch", None) is not None \

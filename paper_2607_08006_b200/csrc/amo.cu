@@ -422,7 +422,9 @@ static int launch_amo_hot(shmemg_world *w, const AmoArgs &a, int idx_bytes, cuda
     else cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_amo_hot_main<8, OP>, 256, 0);
     if (per_sm < 1) per_sm = 1;
     size_t waves = 8;                                         // measured on C4: 1 wave 970 us, 8 waves 890 us, 32 waves 980 us
-    if (const char *e = getenv("SHMEMG_HOT_WAVES")) waves = (size_t)atoi(e) > 0 ? (size_t)atoi(e) : waves;   // experiments
+#ifdef SHMEMG_EXPERIMENTS
+    if (const char *e = getenv("SHMEMG_HOT_WAVES")) waves = (size_t)atoi(e) > 0 ? (size_t)atoi(e) : waves;   // shmemg_amo_scratch_bytes assumes 8
+#endif
     const size_t blocks = (size_t)w->sm_count * per_sm * waves;
     const size_t per_cta = (a.n + blocks - 1) / blocks;
     if (per_cta >= ((size_t)1 << 21) * 8 || a.n >= ((size_t)1 << HOT_I_BITS)) return SHMEMG_ERR_NOMEM;   // caller falls back
@@ -461,7 +463,7 @@ static int launch_amo(shmemg_world *w, const AmoArgs &a, int idx_bytes, uint32_t
     if (blocks > cap) blocks = cap;
     const bool agg = flags & SHMEMG_AMO_WARP_AGGREGATE;
     const bool test = OP == AMO_CAS && (flags & SHMEMG_AMO_TEST_BEFORE_SWAP) && a.cond == nullptr;
-    if (test && !agg && (a.stride & 7) == 0 && ((uint64_t)w->npes * a.stride >> 3) < 0xffffffffull && !getenv("SHMEMG_NO_CAS_STREAM")) {
+    if (test && !agg && (a.stride & 7) == 0 && ((uint64_t)w->npes * a.stride >> 3) < 0xffffffffull) {
         // streaming form: every word of the slab has a 32-bit index (slab < 32 GiB)
         if (idx_bytes == 4) k_cas_test<4><<<(unsigned)blocks, threads, 0, st>>>(a);
         else k_cas_test<8><<<(unsigned)blocks, threads, 0, st>>>(a);
@@ -501,8 +503,10 @@ extern "C" int shmemg_atomic_add_batch_on_stream(shmemg_world_t *w, uint64_t sym
     if (rc) return rc;
     AmoArgs a{w->base, w->stride, sym_off, tgt_pe, elem_idx, (const unsigned long long *)val, val_scalar, nullptr, 0, nullptr, n,
               (flags & SHMEMG_AMO_THEN_BARRIER) ? w->ctl : nullptr};
+    w->amo_last_path = 0;
     if (hot_agg_ok(w, a, flags)) {
         rc = launch_amo_hot<AMO_ADD>(w, a, idx_bytes, (cudaStream_t)stream);
+        if (rc == SHMEMG_OK) w->amo_last_path = 1;
         if (rc != SHMEMG_ERR_NOMEM) return rc;                 // no (or too small a) scratch buffer: the plain kernel
     }
     return launch_amo<AMO_ADD>(w, a, idx_bytes, flags, (cudaStream_t)stream);
@@ -517,8 +521,10 @@ extern "C" int shmemg_atomic_fetch_add_batch_on_stream(shmemg_world_t *w, uint64
     if (n && !fetched_out) return SHMEMG_ERR_ARG;
     AmoArgs a{w->base, w->stride, sym_off, tgt_pe, elem_idx, (const unsigned long long *)val, val_scalar, nullptr, 0,
               (unsigned long long *)fetched_out, n, (flags & SHMEMG_AMO_THEN_BARRIER) ? w->ctl : nullptr};
+    w->amo_last_path = 0;
     if (hot_agg_ok(w, a, flags)) {
         rc = launch_amo_hot<AMO_FADD>(w, a, idx_bytes, (cudaStream_t)stream);
+        if (rc == SHMEMG_OK) w->amo_last_path = 1;
         if (rc != SHMEMG_ERR_NOMEM) return rc;
     }
     return launch_amo<AMO_FADD>(w, a, idx_bytes, flags, (cudaStream_t)stream);
@@ -551,6 +557,7 @@ extern "C" size_t shmemg_amo_scratch_bytes(const shmemg_world_t *w, size_t n) {
     if (cap > ((size_t)1 << 21)) cap = (size_t)1 << 21;
     return (size_t)HOT_SAMPLES * 4 + blocks * cap * 8;
 }
+extern "C" int shmemg_amo_last_path(const shmemg_world_t *w) { return w ? w->amo_last_path : SHMEMG_ERR_ARG; }
 extern "C" int shmemg_set_scratch(shmemg_world_t *w, void *scratch_dev, size_t bytes) {
     if (!w || (!scratch_dev && bytes)) return SHMEMG_ERR_ARG;
     if ((uintptr_t)scratch_dev % 256) return SHMEMG_ERR_ALIGN;

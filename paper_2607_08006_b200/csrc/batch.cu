@@ -104,7 +104,12 @@ __device__ __forceinline__ unsigned long long gtime() {
     asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t));
     return t;
 }
+// (builds with -DSHMEMG_EXPERIMENTS only: the shipped kernel carries no stamps)
+#ifdef SHMEMG_EXPERIMENTS
 #define TRACE(slot) do { if (trace) trace[blockIdx.x * TRACE_SLOTS + (slot)] = gtime(); } while (0)
+#else
+#define TRACE(slot) do { } while (0)
+#endif
 
 __global__ void __launch_bounds__(EXEC_THREADS, 1) k_batch_exec(const ExecArgs a) {
     extern __shared__ __align__(1024) uint8_t stage[];
@@ -118,7 +123,9 @@ __global__ void __launch_bounds__(EXEC_THREADS, 1) k_batch_exec(const ExecArgs a
     unsigned ntiles = a.ntiles;
     unsigned STG = a.stage_bytes, NST = a.nstages;
     const int tid = threadIdx.x;
+#ifdef SHMEMG_EXPERIMENTS
     unsigned long long *trace = blockIdx.x < TRACE_CTAS ? a.trace : nullptr;
+#endif
     Epoch ep;
     ep.e = 0; ep.all_total = a.all_total; ep.npes = a.npes;
 
@@ -448,7 +455,12 @@ static uint32_t pick_seg_tiles(const shmemg_world *w, const shmemg_op_t *ops, si
         if (ops[i].opcode >= SHMEMG_OP_PUT && ops[i].opcode <= SHMEMG_OP_PUT_SIGNAL)
             tiles += (ops[i].nbytes + SHMEMG_TMA_TILE - 1) / SHMEMG_TMA_TILE;
     const uint64_t per_sm = (tiles + w->sm_count - 1) / w->sm_count;
-    if (const char *e = getenv("SHMEMG_SEG_TILES")) return (uint32_t)atoi(e);      // experiments
+#ifdef SHMEMG_EXPERIMENTS
+    if (const char *e = getenv("SHMEMG_SEG_TILES")) {             // host planner only: plans then differ from the device planner's
+        const int v = atoi(e);
+        return v < 1 ? 1u : v > (int)SEG_TILES_MAX ? SEG_TILES_MAX : (uint32_t)v;
+    }
+#endif
     if (per_sm >= SEG_TILES_MAX) return SEG_TILES_MAX;
     return per_sm < 1 ? 1u : (uint32_t)per_sm;
 }
@@ -598,7 +610,9 @@ extern "C" int shmemg_batch_create(shmemg_world_t *w, const shmemg_op_t *ops, si
     hdr->all_total = all_total;
     hdr->tiles_off = ps.tiles_off; hdr->aux_off = ps.aux_off; hdr->done_off = ps.done_off; hdr->arrive_off = ps.arrive_off;
     hdr->trace_off = ps.trace_off;
+#ifdef SHMEMG_EXPERIMENTS
     if (const char *e = getenv("SHMEMG_TRACE")) hdr->trace_on = (uint32_t)atoi(e);
+#endif
 
     // forward pass: dependencies.  issued[p] = counted units of PE p so far; thresh[p] = what p's next unit must see.
     // (Only counted units advance done[], and every unit before a marker that a later unit depends on is counted.)
@@ -699,11 +713,13 @@ extern "C" int shmemg_batch_create(shmemg_world_t *w, const shmemg_op_t *ops, si
         const bool small = bulk <= (uint64_t)EXEC_SMALL_PER_SM * (uint64_t)w->sm_count;
         b->stage_bytes = small ? 16384u : 32768u;
         b->nstages = small ? 12u : 7u;
-        if (const char *e = getenv("SHMEMG_EXEC_RING")) {            // experiments: "<stage_bytes>x<nstages>"
+#ifdef SHMEMG_EXPERIMENTS
+        if (const char *e = getenv("SHMEMG_EXEC_RING")) {            // "<stage_bytes>x<nstages>"
             unsigned sb = 0, ns = 0;
             if (sscanf(e, "%ux%u", &sb, &ns) == 2 && sb >= 1024 && sb % 16 == 0 && ns >= 2 && ns <= EXEC_STAGES_MAX &&
                 (uint64_t)sb * ns <= EXEC_SMEM_MAX) { b->stage_bytes = sb; b->nstages = ns; }
         }
+#endif
     }
     *out = b;
     return SHMEMG_OK;

@@ -575,10 +575,12 @@ extern "C" int shmemg_fcollect_on_stream(shmemg_world_t *w, uint64_t dest_off, u
         // HBM once and from L2 by the others.  Measured on C5 (profiles/r01c): 93.0 us against 96.9 us with 8
         // destinations per loaded tile; the write-only ceiling of bulk stores on this box is 88 us.
         int groups = w->npes;
-        if (const char *e = getenv("SHMEMG_FCOLLECT_GROUPS")) {      // experiments
+#ifdef SHMEMG_EXPERIMENTS
+        if (const char *e = getenv("SHMEMG_FCOLLECT_GROUPS")) {
             groups = atoi(e);
             if (groups < 1 || groups > w->npes) groups = w->npes;
         }
+#endif
         const uint64_t nwork = (uint64_t)w->npes * cpb * groups;
         const unsigned grid = (unsigned)(nwork < (uint64_t)w->sm_count ? nwork : (uint64_t)w->sm_count);
         k_fcollect_tma<<<grid, 32, SHMEMG_TMA_SMEM, st>>>(w->base, w->stride, dest_off, source_off, nbytes, w->npes, cpb, groups);

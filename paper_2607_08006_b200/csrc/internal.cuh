@@ -73,6 +73,7 @@ struct shmemg_world {
     unsigned long long shard_epoch = 0;    // gbarriers enqueued so far
     void *scratch = nullptr;               // DEVICE: caller-owned scratch (shmemg_set_scratch), used by SHMEMG_AMO_HOT_AGGREGATE
     size_t scratch_bytes = 0;
+    int amo_last_path = 0;                 // which kernels the last add / fetch-add batch call ran (shmemg_amo_last_path)
     std::string last_cuda_error;
 };
 

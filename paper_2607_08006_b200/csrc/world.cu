@@ -67,15 +67,17 @@ extern "C" int shmemg_init(int npes, size_t heap_bytes_per_pe, void *device_slab
     w->ctl = (CtlRegion *)(w->base + (size_t)npes * w->stride);
     w->arena = (uint8_t *)w->ctl + SHMEMG_CTL_BYTES;
     w->free_list[0] = heap_bytes_per_pe;
+#ifdef SHMEMG_EXPERIMENTS                                               // tuning knobs: not in the shipped build (_build.py sets no such flag)
     if (const char *s = getenv("SHMEMG_CTAS_PER_SM")) {
         int v = atoi(s);
         if (v >= 1 && v <= 8) w->ctas_per_sm = v;
     }
-    if (getenv("SHMEMG_NO_PDL")) w->dependent_launch = false;       // read once, here; shmemg_set_dependent_launch changes it later
     if (const char *s = getenv("SHMEMG_TILE_BYTES")) {
         long v = atol(s);
         if (v >= 1024) w->tile_bytes_override = (size_t)v;
     }
+#endif
+    if (getenv("SHMEMG_NO_PDL")) w->dependent_launch = false;       // read once, here; shmemg_set_dependent_launch changes it later
     static_assert(sizeof(CtlRegion) <= SHMEMG_CTL_BYTES, "control region too small");
     cudaError_t e = cudaMemset(w->ctl, 0, SHMEMG_CTL_BYTES);
     if (e == cudaSuccess) e = cudaDeviceSynchronize();
