@@ -60,6 +60,7 @@ def lib():
         L.orc_broadcast.argtypes = [vp, i, u64, u64, u64, u64, i]
         L.orc_reduce.argtypes = [vp, i, u64, i, i, u64, u64, u64]
         L.orc_amo_batch.argtypes = [vp, i, u64, i, i, u64, vp, vp, vp, vp, u64]
+        L.orc_amo_cswap_batch.argtypes = [vp, i, u64, i, u64, vp, vp, vp, vp, vp, u64]
         L.orc_ibput.argtypes = [vp, i, u64, u64, u64, u64, u64, u64, u64, i, i, i]
         L.orc_signal_test.argtypes = [vp, i, u64, u64, i, u64, i]
         L.orc_signal_test_vec.argtypes = [vp, i, u64, u64, u64, i, u64, i, vp]
@@ -259,6 +260,15 @@ class OracleWorld:
         _chk(lib().orc_amo_batch(self.heap.ctypes.data, self.npes, self.heap_bytes, self.AMO[op], width, sym_off,
                                  tgt_pe.ctypes.data, idx.ctypes.data, None if val is None else val.ctypes.data,
                                  fetched.ctypes.data if fetch else None, len(idx)), "amo_batch")
+        return fetched
+
+    def amo_cswap_batch(self, width: int, sym_off, tgt_pe, idx, cond, val) -> np.ndarray:
+        tgt_pe = np.ascontiguousarray(tgt_pe, dtype=np.int32)
+        idx, cond, val = _u64arr(idx), _u64arr(cond), _u64arr(val)
+        fetched = np.empty(len(idx), dtype=np.uint64)
+        _chk(lib().orc_amo_cswap_batch(self.heap.ctypes.data, self.npes, self.heap_bytes, width, sym_off, tgt_pe.ctypes.data,
+                                       idx.ctypes.data, cond.ctypes.data, val.ctypes.data, fetched.ctypes.data, len(idx)),
+             "amo_cswap_batch")
         return fetched
 
     def ibput(self, dst_off, src_off, dst_stride, src_stride, block, nblocks, pe, target):

@@ -384,6 +384,30 @@ int orc_amo_batch(uint8_t *heap, int npes, uint64_t heap_bytes, int op, int widt
     return ORC_OK;
 }
 
+/* compare-swap batch on `width`-byte words (4 or 8), structure-of-arrays, executed in index order (the compare_swap of the
+ * OpenSHMEM 1.6 AMO set on its 32- and 64-bit types, inherited unchanged: L361, L363):
+ *   word = heap[tgt_pe[i]][sym_off + width*idx[i]];  old = word;  if (old == cond[i]) word = val[i];  fetched[i] = old.
+ * cond and val are taken modulo 2^(8*width); fetched is zero-extended. */
+int orc_amo_cswap_batch(uint8_t *heap, int npes, uint64_t heap_bytes, int width, uint64_t sym_off, const int32_t *tgt_pe,
+                        const uint64_t *idx, const uint64_t *cond, const uint64_t *val, uint64_t *fetched, uint64_t n) {
+    if (width != 4 && width != 8) return ORC_ERR_OPCODE;
+    if (sym_off % (uint64_t)width) return ORC_ERR_ALIGN;
+    const uint64_t mask = width == 8 ? ~0ull : 0xffffffffull;
+    for (uint64_t i = 0; i < n; ++i) {
+        if (tgt_pe[i] < 0 || tgt_pe[i] >= npes || !in_range(sym_off + (uint64_t)width * idx[i], (uint64_t)width, heap_bytes))
+            return ORC_ERR_RANGE;
+        uint8_t *w = heap + (uint64_t)tgt_pe[i] * heap_bytes + sym_off + (uint64_t)width * idx[i];
+        uint64_t old = 0;
+        memcpy(&old, w, (size_t)width);
+        if (old == (cond[i] & mask)) {
+            const uint64_t nw = val[i] & mask;
+            memcpy(w, &nw, (size_t)width);
+        }
+        fetched[i] = old;
+    }
+    return ORC_OK;
+}
+
 /* block-strided put / get (OpenSHMEM 1.6 ibput / ibget; iput / iget are the case block = one element):
  * for b in [0, nblocks): dest[b*dst_stride : +block] = source[b*src_stride : +block], strides in BYTES.
  * put: source on `pe`, dest on `target`; get: source on `target`, dest on `pe`. */

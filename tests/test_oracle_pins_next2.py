@@ -188,6 +188,81 @@ def test_swap_set_fetch_hand_cases():
         w.amo_batch("add", 8, 0, [2], [0], [1])                                   # PE out of range
 
 
+def test_cswap_hand_cases_both_widths():
+    """compare-swap of the inherited AMO set on 32- and 64-bit words, by hand."""
+    w = orc.OracleWorld(2, 128)
+    w.view(0, 32, np.uint64)[:] = [[1, 2, 3, 4], [5, 6, 7, 8]]
+    f = w.amo_cswap_batch(8, 0, [1, 1, 1, 0], [2, 2, 2, 0], [7, 7, 70, 2], [70, 71, 72, 9])
+    assert f.tolist() == [7, 70, 70, 1]                              # 1st swaps, 2nd fails (word is 70), 3rd swaps, 4th fails
+    assert w.view(0, 32, np.uint64).tolist() == [[1, 2, 3, 4], [5, 6, 72, 8]]
+    # 32-bit: the word is one half of a 64-bit cell; cond / val are truncated; the neighbouring half is untouched
+    w.view(0, 32, np.uint32)[0, :4] = [10, 11, 12, 13]
+    f = w.amo_cswap_batch(4, 0, [0, 0, 0], [1, 1, 2], [0x5_0000_000b, 11, 13], [0x9_0000_0063, 100, 5])
+    assert f.tolist() == [11, 99, 12]                                # cond 0x5_0000_000b == 11 mod 2^32; val -> 99
+    assert w.view(0, 32, np.uint32)[0, :4].tolist() == [10, 99, 12, 13]
+    with pytest.raises(orc.OracleError):
+        w.amo_cswap_batch(4, 2, [0], [0], [0], [0])                   # misaligned 32-bit word
+    with pytest.raises(orc.OracleError):
+        w.amo_cswap_batch(2, 0, [0], [0], [0], [0])                   # no 16-bit AMOs
+    with pytest.raises(orc.OracleError):
+        w.amo_cswap_batch(4, 0, [0], [32], [0], [0])                  # beyond the window
+
+
+@pytest.mark.parametrize("width,npdt,empty", [(8, np.uint64, M64), (4, np.uint32, 0xffffffff)])
+def test_cswap_claim_first_op_in_index_order_wins(width, npdt, empty):
+    """Closed form for claim-style batches (every op is CAS(empty -> its own value) on slots holding `empty`): executed in
+    index order, the FIRST op of a slot wins (np.unique(return_index)), it fetches `empty`, every later op of the slot fetches
+    the winner's value.  width 8 must also agree with the SoA compare-swap routine that was written for config 4."""
+    npes, words, n = 3, 40, 3000
+    w = orc.OracleWorld(npes, words * 8 + 256)
+    a = w.malloc(words * width)
+    w.view(a, words * width, npdt)[:] = empty
+    tgt = gen.uniform_i32(n, 0, npes - 1, 231, 0)
+    idx = gen.uniform_i32(n, 0, words - 2, 231, 1)                    # the last word of every PE is never touched
+    val = (gen.u64(n, 232) >> np.uint64(40)) + np.uint64(1)           # < 2^24 + 1: never equal to `empty`, fits 32 bits
+    f = w.amo_cswap_batch(width, a, tgt, idx, np.full(n, empty, dtype=np.uint64), val)
+    flat = tgt.astype(np.int64) * words + idx
+    keys, first = np.unique(flat, return_index=True)
+    exp = np.full(npes * words, empty, dtype=np.uint64)
+    exp[keys] = val[first]
+    assert np.array_equal(w.view(a, words * width, npdt).reshape(-1).astype(np.uint64), exp)
+    expf = exp[flat].copy()
+    expf[first] = empty
+    assert np.array_equal(f, expf)
+    if width == 8:
+        w2 = orc.OracleWorld(npes, words * 8 + 256)
+        a2 = w2.malloc(words * 8)
+        w2.view(a2, words * 8, np.uint64)[:] = M64
+        f2 = w2.atomic_compare_swap_batch(a2, tgt, idx, np.full(n, M64, dtype=np.uint64), val)
+        assert np.array_equal(f, f2) and np.array_equal(w.heap, w2.heap)
+
+
+@pytest.mark.parametrize("width", [4, 8])
+def test_cswap_general_conditions_replayed_with_python_ints(width):
+    """Arbitrary cond / val on few words with small values, so that many swaps succeed and many fail: replayed op by op."""
+    npes, words, n = 2, 6, 4000
+    mask = (1 << (8 * width)) - 1
+    w = orc.OracleWorld(npes, 256)
+    npdt = np.uint32 if width == 4 else np.uint64
+    init = (gen.u64(npes * words, 233) % np.uint64(4)).astype(npdt).reshape(npes, words)
+    w.view(0, words * width, npdt)[:] = init
+    tgt = gen.uniform_i32(n, 0, npes - 1, 234, 0)
+    idx = gen.uniform_i32(n, 0, words - 1, 234, 1)
+    cond = gen.u64(n, 235) % np.uint64(4) + (gen.u64(n, 236) % np.uint64(2) << np.uint64(32))     # bit 32 set in half of them:
+    val = gen.u64(n, 237) % np.uint64(4) + (gen.u64(n, 238) % np.uint64(2) << np.uint64(32))      # ignored on 32-bit words only
+    f = w.amo_cswap_batch(width, 0, tgt, idx, cond, val)
+    cur = [int(x) for x in init.reshape(-1)]
+    swaps = 0
+    for i in range(n):
+        k = int(tgt[i]) * words + int(idx[i])
+        assert int(f[i]) == cur[k]
+        if cur[k] == int(cond[i]) & mask:
+            cur[k] = int(val[i]) & mask
+            swaps += 1
+    assert 200 < swaps < n - 200
+    assert w.view(0, words * width, npdt).reshape(-1).tolist() == cur
+
+
 def test_swap_chain_permutes_values():
     """Per word, {fetched values} + {final} = {init} + {swapped-in values} as multisets."""
     npes, words, n = 3, 16, 2000
