@@ -374,6 +374,15 @@ SHMEMG_API int shmemg_atomic_op_batch_on_stream(shmemg_world_t *w, int amo, int 
                                                 const uint64_t *val, uint64_t val_scalar, uint64_t *fetched_out,
                                                 size_t n, void *stream);
 
+/* compare-swap of the same AMO set on `width`-byte words (4 or 8): old = word; if (old == cond[i]) word = val[i];
+ * fetched_out[i] = old (required; zero-extended).  cond / val (DEVICE, 64-bit entries, low `width` bytes used) may be NULL ->
+ * cond_scalar / val_scalar.  atom.global.cas.b32 / .b64; no ordering between the ops of one call.  (The 64-bit claim-style
+ * batches of config 4 have their own faster call above, shmemg_atomic_compare_swap_batch_on_stream.) */
+SHMEMG_API int shmemg_atomic_cswap_op_batch_on_stream(shmemg_world_t *w, int width, uint64_t sym_off, const int32_t *tgt_pe,
+                                                      const void *elem_idx, int idx_bytes, const uint64_t *cond,
+                                                      uint64_t cond_scalar, const uint64_t *val, uint64_t val_scalar,
+                                                      uint64_t *fetched_out, size_t n, void *stream);
+
 /* ---- block-strided put / get (OpenSHMEM 1.6 ibput / ibget; iput / iget are the case block = one element) ---------------
  * for b in [0, nblocks): dest[b*dst_stride .. +block_bytes) = source[b*src_stride .. +block_bytes); strides in BYTES, any
  * size and alignment.  put: source in `pe`'s window, dest in `target_pe`'s; get: source in `target_pe`'s, dest in `pe`'s.

@@ -157,6 +157,7 @@ SYMBOLS = {
     "shmemg_reduce_on_stream": (_i, [_vp, _i, _i, _u64, _u64, _sz, _vp]),
     "shmemg_broadcast_on_stream": (_i, [_vp, _u64, _u64, _sz, _i, _vp]),
     "shmemg_atomic_op_batch_on_stream": (_i, [_vp, _i, _i, _u64, _vp, _vp, _i, _vp, _u64, _vp, _sz, _vp]),
+    "shmemg_atomic_cswap_op_batch_on_stream": (_i, [_vp, _i, _u64, _vp, _vp, _i, _vp, _u64, _vp, _u64, _vp, _sz, _vp]),
     "shmemg_ibput_on_stream": (_i, [_vp, _u64, _u64, _u64, _u64, _sz, _sz, _i, _i, _vp]),
     "shmemg_ibget_on_stream": (_i, [_vp, _u64, _u64, _u64, _u64, _sz, _sz, _i, _i, _vp]),
     "shmemg_signal_test_on_stream": (_i, [_vp, _u64, _i, _u64, _i, _vp, _vp]),
@@ -564,6 +565,16 @@ class World:
                                                          self._idx_bytes(elem_idx), _dptr(val), val_scalar & ((1 << 64) - 1),
                                                          _dptr(fetched_out), n, _stream(stream)),
                   "shmemg_atomic_op_batch_on_stream")
+        self.launches += 1 if n else 0
+
+    def atomic_cswap_op_batch(self, width, sym_off, tgt_pe, elem_idx, fetched_out, cond=None, cond_scalar=0, val=None, val_scalar=0,
+                              stream=None):
+        n = tgt_pe.numel()
+        assert elem_idx.numel() == n and (cond is None or cond.numel() == n) and (val is None or val.numel() == n)
+        self._chk(lib().shmemg_atomic_cswap_op_batch_on_stream(self.h, width, sym_off, _dptr(tgt_pe), _dptr(elem_idx),
+                                                               self._idx_bytes(elem_idx), _dptr(cond), cond_scalar & NO_STAMP,
+                                                               _dptr(val), val_scalar & NO_STAMP, _dptr(fetched_out), n,
+                                                               _stream(stream)), "shmemg_atomic_cswap_op_batch_on_stream")
         self.launches += 1 if n else 0
 
     def ibput(self, dest_off, source_off, dst_stride, src_stride, block_bytes, nblocks, pe, target_pe, stream=None):

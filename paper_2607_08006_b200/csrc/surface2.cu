@@ -184,6 +184,75 @@ extern "C" int shmemg_atomic_op_batch_on_stream(shmemg_world_t *w, int amo, int 
     return SHMEMG_OK;
 }
 
+// compare-swap on 4- or 8-byte words (the remaining AMO of the inherited set): atom.global.cas.b32 / .b64, four
+// independent ops per thread in flight, fetched values written coalesced.
+struct Cswap2Args {
+    uint8_t *base;
+    size_t stride;
+    uint64_t sym_off;
+    const int *tgt_pe;
+    const void *idx;
+    const unsigned long long *cond, *val;
+    unsigned long long cond_s, val_s;
+    unsigned long long *fetched;
+    size_t n;
+};
+template <typename T, int IDXB>
+__global__ void __launch_bounds__(256) k_cswap2(const Cswap2Args a) {
+    const size_t T4 = (size_t)gridDim.x * blockDim.x;
+    for (size_t i0 = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i0 < a.n; i0 += 4 * T4) {
+        T *word[4];
+        T c[4], v[4];
+#pragma unroll
+        for (int k = 0; k < 4; ++k) {
+            const size_t i = i0 + (size_t)k * T4;
+            word[k] = nullptr;
+            if (i < a.n) {
+                const unsigned long long e = IDXB == 4 ? (unsigned long long)reinterpret_cast<const unsigned *>(a.idx)[i]
+                                                       : reinterpret_cast<const unsigned long long *>(a.idx)[i];
+                word[k] = reinterpret_cast<T *>(a.base + (size_t)a.tgt_pe[i] * a.stride + a.sym_off) + e;
+                c[k] = (T)(a.cond ? a.cond[i] : a.cond_s);
+                v[k] = (T)(a.val ? a.val[i] : a.val_s);
+            }
+        }
+        T old[4];
+#pragma unroll
+        for (int k = 0; k < 4; ++k)
+            if (word[k]) old[k] = atomicCAS(word[k], c[k], v[k]);
+#pragma unroll
+        for (int k = 0; k < 4; ++k)
+            if (word[k]) a.fetched[i0 + (size_t)k * T4] = (unsigned long long)old[k];
+    }
+}
+
+extern "C" int shmemg_atomic_cswap_op_batch_on_stream(shmemg_world_t *w, int width, uint64_t sym_off, const int32_t *tgt_pe,
+                                                      const void *elem_idx, int idx_bytes, const uint64_t *cond,
+                                                      uint64_t cond_scalar, const uint64_t *val, uint64_t val_scalar,
+                                                      uint64_t *fetched_out, size_t n, void *stream) {
+    if (!w || (width != 4 && width != 8)) return SHMEMG_ERR_ARG;
+    if (n && (!tgt_pe || !elem_idx || !fetched_out)) return SHMEMG_ERR_ARG;
+    if (idx_bytes != 4 && idx_bytes != 8) return SHMEMG_ERR_ARG;
+    if (sym_off & (uint64_t)(width - 1)) return SHMEMG_ERR_ALIGN;
+    if (!shmemg_in_range(w, sym_off, (uint64_t)width)) return SHMEMG_ERR_RANGE;
+    if (n == 0) return SHMEMG_OK;
+    // tgt_pe[] and elem_idx[] are DEVICE arrays: per-op bounds are the caller's contract (undefined otherwise)
+    Cswap2Args a{w->base, w->stride, sym_off, tgt_pe, elem_idx, (const unsigned long long *)cond, (const unsigned long long *)val,
+                 cond_scalar, val_scalar, (unsigned long long *)fetched_out, n};
+    size_t blocks = (n + 1023) / 1024;
+    const size_t cap = (size_t)w->sm_count * 8 * 4;
+    if (blocks > cap) blocks = cap;
+    cudaStream_t st = (cudaStream_t)stream;
+    if (width == 8) {
+        if (idx_bytes == 4) k_cswap2<unsigned long long, 4><<<(unsigned)blocks, 256, 0, st>>>(a);
+        else k_cswap2<unsigned long long, 8><<<(unsigned)blocks, 256, 0, st>>>(a);
+    } else {
+        if (idx_bytes == 4) k_cswap2<unsigned, 4><<<(unsigned)blocks, 256, 0, st>>>(a);
+        else k_cswap2<unsigned, 8><<<(unsigned)blocks, 256, 0, st>>>(a);
+    }
+    SHMEMG_CUDA(w, cudaGetLastError());
+    return SHMEMG_OK;
+}
+
 // ---- block-strided put / get --------------------------------------------------------------------------------------------
 // Three paths, picked on the host:
 //   bulk    blocks >= 1 KiB with 16-byte aligned addresses, strides and size: work item = (block, <= 32 KiB chunk), the

@@ -220,6 +220,64 @@ def test_generic_amo_contended_commutative_finals_and_fetch_chains(amo, width):
 
 
 @pytest.mark.parametrize("width", [8, 4])
+@pytest.mark.parametrize("n,idx_dtype", [(1, np.int32), (1025, np.int64), (70001, np.int32)])
+def test_cswap_on_distinct_words_equals_the_oracle(width, n, idx_dtype):
+    """Every word is the target of at most one op, so the result does not depend on the schedule: heap and fetched values
+    bit-exact against the oracle.  About half of the conditions hold; cond / val carry garbage above bit 31 (ignored on 32-bit
+    words, significant on 64-bit ones)."""
+    npes, words = 3, 30000
+    npdt = np.uint64 if width == 8 else np.uint32
+    w, ow = World(npes, words * 8 + 4096, DEV), orc.OracleWorld(npes, words * 8 + 4096)
+    pad, opad = w.malloc(256), ow.malloc(256)
+    a, oa = w.malloc(words * width), ow.malloc(words * width)
+    init = (gen.u64(npes * words, 361) % np.uint64(2)).astype(npdt).reshape(npes, words)
+    w.view(a, words * width).copy_(torch.from_numpy(init.view(np.uint8)))
+    ow.view(oa, words * width, npdt)[:] = init
+    flat = np.argsort(gen.u64(npes * words, 362))[:n].astype(np.int64)          # n distinct words in random order
+    tgt, idx = (flat // words).astype(np.int32), (flat % words).astype(idx_dtype)
+    hi = (gen.u64(n, 363) % np.uint64(2)) << np.uint64(32)
+    cond = gen.u64(n, 364) % np.uint64(2) + hi
+    val = gen.u64(n, 365) % np.uint64(1000) + np.uint64(2) + hi
+    f = torch.zeros(n, dtype=torch.int64, device=DEV)
+    w.atomic_cswap_op_batch(width, a, to_dev(tgt), to_dev(idx), f, cond=to_dev(cond.view(np.int64)), val=to_dev(val.view(np.int64)))
+    w.quiet(0)
+    of = ow.amo_cswap_batch(width, oa, tgt, idx, cond, val)
+    assert np.array_equal(f.cpu().numpy().view(np.uint64), of)
+    assert np.array_equal(w.view(a, words * width).cpu().numpy().view(npdt), ow.view(oa, words * width, npdt))
+    assert 0 < int((of == (cond & np.uint64((1 << (8 * width)) - 1))).sum()) < n or n == 1
+
+
+@pytest.mark.parametrize("width,empty", [(8, (1 << 64) - 1), (4, 0xffffffff)])
+def test_cswap_claims_on_contended_words(width, empty):
+    """Claim-style batch with scalar cond (CAS(empty -> own value)) on few words, both halves of every 64-bit cell contended
+    separately on 32-bit words: exactly one winner per touched word, it fetched `empty`, the word holds its value, every loser
+    fetched that value; the set of claimed words equals the oracle's."""
+    from invariants import check_compare_swap_claim
+    npes, words, n = 2, 500, 300001
+    npdt = np.uint64 if width == 8 else np.uint32
+    w, ow = World(npes, words * 8 + 4096, DEV), orc.OracleWorld(npes, words * 8 + 4096)
+    a, oa = w.malloc(words * width), ow.malloc(words * width)
+    w.view(a, words * width).fill_(255)
+    ow.view(oa, words * width, npdt)[:] = empty
+    flat = (gen.u64(n, 366) % np.uint64(npes * words - 7)).astype(np.int64)     # the last 7 words stay untouched
+    tgt, idx = (flat // words).astype(np.int32), (flat % words).astype(np.int32)
+    val = (np.arange(n, dtype=np.uint64) + np.uint64(1)) & np.uint64(0x7fffffff)
+    f = torch.zeros(n, dtype=torch.int64, device=DEV)
+    w.atomic_cswap_op_batch(width, a, to_dev(tgt), to_dev(idx), f, cond_scalar=empty, val=to_dev(val.view(np.int64)))
+    w.quiet(0)
+    fin = w.view(a, words * width).cpu().numpy().view(npdt).reshape(-1).astype(np.uint64)
+    check_compare_swap_claim(flat, val, f.cpu().numpy().view(np.uint64), fin, empty=empty)
+    ow.amo_cswap_batch(width, oa, tgt, idx, np.full(n, empty, dtype=np.uint64), val)
+    ofin = ow.view(oa, words * width, npdt).reshape(-1).astype(np.uint64)
+    assert np.array_equal(fin == np.uint64(empty), ofin == np.uint64(empty))
+    with pytest.raises(ShmemgError):
+        w.atomic_cswap_op_batch(2, a, to_dev(tgt), to_dev(idx), f)                # no 16-bit words
+    with pytest.raises(ShmemgError):
+        w.atomic_cswap_op_batch(4, a + 2, to_dev(tgt), to_dev(idx), f)            # misaligned
+    w.atomic_cswap_op_batch(4, a, to_dev(tgt[:0]), to_dev(idx[:0]), f[:0])        # no ops: nothing enqueued
+
+
+@pytest.mark.parametrize("width", [8, 4])
 def test_generic_amo_swap_chain_set_and_fetch(width):
     npes, words, n = 3, 64, 50000
     npdt = np.uint64 if width == 8 else np.uint32
