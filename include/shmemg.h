@@ -383,6 +383,16 @@ SHMEMG_API int shmemg_atomic_cswap_op_batch_on_stream(shmemg_world_t *w, int wid
                                                       uint64_t cond_scalar, const uint64_t *val, uint64_t val_scalar,
                                                       uint64_t *fetched_out, size_t n, void *stream);
 
+/* Debug aid for every structure-of-arrays AMO call above.  Their tgt_pe[] / elem_idx[] are DEVICE arrays, so per-op bounds are
+ * the caller's contract and a bad entry is undefined behaviour: a stray atomic.  This call checks them on the
+ * device with the same addressing (word = heap[tgt_pe[i]][sym_off + width*elem_idx[i]], width 4 or 8; pass 8 for the 64-bit
+ * add / fetch-add / compare-swap calls): *first_bad_dev (DEVICE, 8 bytes, caller-owned) receives the smallest i whose PE is
+ * outside [0, npes) or whose word is not wholly inside the PE's heap window, or UINT64_MAX when every op is in bounds.  Valid
+ * when `stream` has passed the call (one 8-byte memset + one kernel; reads 4 + idx_bytes bytes per op). */
+SHMEMG_API int shmemg_amo_check_batch_on_stream(shmemg_world_t *w, int width, uint64_t sym_off, const int32_t *tgt_pe,
+                                                const void *elem_idx, int idx_bytes, size_t n, uint64_t *first_bad_dev,
+                                                void *stream);
+
 /* ---- block-strided put / get (OpenSHMEM 1.6 ibput / ibget; iput / iget are the case block = one element) ---------------
  * for b in [0, nblocks): dest[b*dst_stride .. +block_bytes) = source[b*src_stride .. +block_bytes); strides in BYTES, any
  * size and alignment.  put: source in `pe`'s window, dest in `target_pe`'s; get: source in `target_pe`'s, dest in `pe`'s.

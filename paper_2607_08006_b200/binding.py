@@ -158,6 +158,7 @@ SYMBOLS = {
     "shmemg_broadcast_on_stream": (_i, [_vp, _u64, _u64, _sz, _i, _vp]),
     "shmemg_atomic_op_batch_on_stream": (_i, [_vp, _i, _i, _u64, _vp, _vp, _i, _vp, _u64, _vp, _sz, _vp]),
     "shmemg_atomic_cswap_op_batch_on_stream": (_i, [_vp, _i, _u64, _vp, _vp, _i, _vp, _u64, _vp, _u64, _vp, _sz, _vp]),
+    "shmemg_amo_check_batch_on_stream": (_i, [_vp, _i, _u64, _vp, _vp, _i, _sz, _vp, _vp]),
     "shmemg_ibput_on_stream": (_i, [_vp, _u64, _u64, _u64, _u64, _sz, _sz, _i, _i, _vp]),
     "shmemg_ibget_on_stream": (_i, [_vp, _u64, _u64, _u64, _u64, _sz, _sz, _i, _i, _vp]),
     "shmemg_signal_test_on_stream": (_i, [_vp, _u64, _i, _u64, _i, _vp, _vp]),
@@ -576,6 +577,16 @@ class World:
                                                                _dptr(val), val_scalar & NO_STAMP, _dptr(fetched_out), n,
                                                                _stream(stream)), "shmemg_atomic_cswap_op_batch_on_stream")
         self.launches += 1 if n else 0
+
+    def amo_check_batch(self, width, sym_off, tgt_pe, elem_idx, stream=None):
+        """Device-side bounds check of the index arrays of an SoA AMO call: index of the first out-of-range op, or None."""
+        out = torch.empty(1, dtype=torch.int64, device=self.device)
+        self._chk(lib().shmemg_amo_check_batch_on_stream(self.h, width, sym_off, _dptr(tgt_pe), _dptr(elem_idx),
+                                                         self._idx_bytes(elem_idx), tgt_pe.numel(), out.data_ptr(),
+                                                         _stream(stream)), "shmemg_amo_check_batch_on_stream")
+        self.launches += 1 if tgt_pe.numel() else 0
+        v = int(out.item())
+        return None if v == -1 else v
 
     def ibput(self, dest_off, source_off, dst_stride, src_stride, block_bytes, nblocks, pe, target_pe, stream=None):
         self._chk(lib().shmemg_ibput_on_stream(self.h, dest_off, source_off, dst_stride, src_stride, block_bytes, nblocks,

@@ -253,6 +253,43 @@ extern "C" int shmemg_atomic_cswap_op_batch_on_stream(shmemg_world_t *w, int wid
     return SHMEMG_OK;
 }
 
+// Debug aid for the structure-of-arrays AMO calls: their tgt_pe[] / elem_idx[] live in DEVICE memory, so the host-side argument
+// checks cannot see them and an out-of-range entry is a stray atomic somewhere in (or beyond) the slab.  This kernel reads the
+// two arrays the way the AMO kernels do and records the smallest op index whose target word is not inside its PE's window.
+template <int IDXB>
+__global__ void __launch_bounds__(256) k_amo_check(const int *tgt_pe, const void *idx, size_t n, int npes, unsigned long long first_word,
+                                                   unsigned long long words_in_window, unsigned long long *first_bad) {
+    unsigned long long bad = ~0ull;
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) {
+        const unsigned long long e = IDXB == 4 ? (unsigned long long)reinterpret_cast<const unsigned *>(idx)[i]
+                                               : reinterpret_cast<const unsigned long long *>(idx)[i];
+        const int t = tgt_pe[i];
+        if ((t < 0 || t >= npes || e >= words_in_window - first_word) && i < bad) bad = i;      // first_word < words_in_window (host check)
+    }
+    if (bad != ~0ull) atomicMin(first_bad, bad);
+}
+
+extern "C" int shmemg_amo_check_batch_on_stream(shmemg_world_t *w, int width, uint64_t sym_off, const int32_t *tgt_pe,
+                                                const void *elem_idx, int idx_bytes, size_t n, uint64_t *first_bad_dev,
+                                                void *stream) {
+    if (!w || (width != 4 && width != 8) || !first_bad_dev) return SHMEMG_ERR_ARG;
+    if (n && (!tgt_pe || !elem_idx)) return SHMEMG_ERR_ARG;
+    if (idx_bytes != 4 && idx_bytes != 8) return SHMEMG_ERR_ARG;
+    if (sym_off & (uint64_t)(width - 1)) return SHMEMG_ERR_ALIGN;
+    if (!shmemg_in_range(w, sym_off, (uint64_t)width)) return SHMEMG_ERR_RANGE;
+    cudaStream_t st = (cudaStream_t)stream;
+    SHMEMG_CUDA(w, cudaMemsetAsync(first_bad_dev, 0xff, 8, st));
+    if (n == 0) return SHMEMG_OK;
+    size_t blocks = (n + 255) / 256;
+    const size_t cap = (size_t)w->sm_count * 8;
+    if (blocks > cap) blocks = cap;
+    const unsigned long long first_word = sym_off / (uint64_t)width, words = w->heap_bytes / (uint64_t)width;   // whole words of the window
+    if (idx_bytes == 4) k_amo_check<4><<<(unsigned)blocks, 256, 0, st>>>(tgt_pe, elem_idx, n, w->npes, first_word, words, (unsigned long long *)first_bad_dev);
+    else k_amo_check<8><<<(unsigned)blocks, 256, 0, st>>>(tgt_pe, elem_idx, n, w->npes, first_word, words, (unsigned long long *)first_bad_dev);
+    SHMEMG_CUDA(w, cudaGetLastError());
+    return SHMEMG_OK;
+}
+
 // ---- block-strided put / get --------------------------------------------------------------------------------------------
 // Three paths, picked on the host:
 //   bulk    blocks >= 1 KiB with 16-byte aligned addresses, strides and size: work item = (block, <= 32 KiB chunk), the

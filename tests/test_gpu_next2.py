@@ -277,6 +277,29 @@ def test_cswap_claims_on_contended_words(width, empty):
     w.atomic_cswap_op_batch(4, a, to_dev(tgt[:0]), to_dev(idx[:0]), f[:0])        # no ops: nothing enqueued
 
 
+@pytest.mark.parametrize("idx_dtype", [np.int32, np.int64])
+def test_amo_check_batch_finds_the_first_out_of_range_op(idx_dtype):
+    """The device-side bounds check of the SoA index arrays (the host cannot see them): None when every op is in bounds, else
+    the smallest offending op index; the last whole word of the window is in bounds, the one after it is not."""
+    npes, hb, n = 3, 4096 + 24, 50001                       # 515 whole 64-bit words, 1030 32-bit words per window
+    w = World(npes, hb, DEV)
+    off = 256
+    tgt = gen.uniform_i32(n, 0, npes - 1, 371, 0)
+    for width, last in ((8, (hb - off) // 8 - 1), (4, (hb - off) // 4 - 1)):
+        idx = (gen.u64(n, 372) % np.uint64(last + 1)).astype(idx_dtype)
+        idx[123] = last                                      # the last whole word: fine
+        assert w.amo_check_batch(width, off, to_dev(tgt), to_dev(idx)) is None
+        bad = idx.copy(); bad[40000] = last + 1; bad[777] = last + 1
+        assert w.amo_check_batch(width, off, to_dev(tgt), to_dev(bad)) == 777
+        t2 = tgt.copy(); t2[31] = npes; t2[9000] = -1
+        assert w.amo_check_batch(width, off, to_dev(t2), to_dev(bad)) == 31
+        neg = idx.copy(); neg[n - 1] = -1                    # a negative index is a huge unsigned one
+        assert w.amo_check_batch(width, off, to_dev(tgt), to_dev(neg)) == n - 1
+    assert w.amo_check_batch(8, off, to_dev(tgt[:0]), to_dev(idx[:0])) is None
+    with pytest.raises(ShmemgError):
+        w.amo_check_batch(8, off + 4, to_dev(tgt), to_dev(idx))
+
+
 @pytest.mark.parametrize("width", [8, 4])
 def test_generic_amo_swap_chain_set_and_fetch(width):
     npes, words, n = 3, 64, 50000
