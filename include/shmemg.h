@@ -19,7 +19,8 @@
  *   - Pointers are marked HOST or DEVICE.  The library never allocates or frees device memory: the
  *     caller owns the slab and every DEVICE array it passes, and must keep them valid until the stream
  *     has passed the call.  The library owns only host bookkeeping plus a control region it carves from
- *     the tail of the slab.
+ *     the tail of the slab -- and one fixed 8 MiB device array that is part of its image (the scratch of
+ *     shmemg_atomic_fetch_add_batch_static_on_stream, for callers that cannot provide any).
  *   - Every routine returns SHMEMG_OK (0) or a negative SHMEMG_ERR_* for host-checkable misuse; nothing
  *     is enqueued on error.  Data races, overlapping unordered writes and unsatisfiable waits are
  *     undefined behaviour; an unsatisfiable wait hangs the stream (prohibited pattern,
